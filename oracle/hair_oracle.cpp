@@ -1,0 +1,1003 @@
+// hair_oracle.cpp — CPU ORACLE of the deferred hair pipeline (arxiv/paper_2607_04230).
+//
+// TEST INFRASTRUCTURE ONLY (see hair_oracle.h). Plain, slow, single-threaded, obviously
+// correct. No blocking, no fusion, no reordering beyond what the paper / DESIGN.md §3
+// state. Build: g++ -std=c++17 -O2 -ffp-contract=off -fno-fast-math -shared -fPIC.
+//
+// Stage map (DESIGN.md §3 numbering; PAPER.md = /root/reference/PAPER.md):
+//   O1 LOD            PAPER.md:102-136  §3.2, Eq. 1-5
+//   O2 generation     PAPER.md:50, 62-64 §2 / §3.1.1, Code 1
+//   O3 calcTangent    PAPER.md:353-359  Code 1 lines 1-4
+//   O4 raster+resolve PAPER.md:66-96    §3.1.2 (two layers PAPER.md:68-74, atomic min PAPER.md:85)
+//   O6 shading        PAPER.md:188-196  §3.4 (stand-in model, R23: parity unpinned vs paper)
+//   O7 filter         PAPER.md:154-176  §3.3, Eq. 9-10, Code 2
+#include "hair_oracle.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+const uint64_t EMPTY = ~0ull;
+const double PI = 3.14159265358979323846;
+
+// ---------------------------------------------------------------- hash (R26)
+// PAPER.md:369-371 "PCG rand(b.strandIndex); uv = rand.next2()". Stateless form:
+// the 32-bit PCG output permutation RXS-M-XS applied to an LCG step, keyed
+// (seed, id, stream): hash = pcg(pcg(pcg(seed) + id) + stream).
+inline uint32_t pcg(uint32_t v) {
+  uint32_t s = v * 747796405u + 2891336453u;
+  uint32_t w = ((s >> ((s >> 28) + 4u)) ^ s) * 277803737u;
+  return (w >> 22) ^ w;
+}
+inline uint32_t hash3(uint32_t seed, uint32_t id, uint32_t stream) {
+  return pcg(pcg(pcg(seed) + id) + stream);
+}
+inline uint32_t u24(uint32_t h) { return h >> 8; }                 // 24-bit integer
+inline double u01(uint32_t h) { return double(h >> 8) / 16777216.0; }  // exact in fp32 and fp64
+
+enum : uint32_t { ST_ROOT1 = 1, ST_ROOT2 = 2, ST_CURL = 3, ST_FRIZZ = 16, ST_LOD = 0xB0 };
+
+struct V3 {
+  double x, y, z;
+};
+inline V3 operator+(V3 a, V3 b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+inline V3 operator-(V3 a, V3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+inline V3 operator*(double s, V3 a) { return {s * a.x, s * a.y, s * a.z}; }
+inline double dot(V3 a, V3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+inline V3 cross(V3 a, V3 b) {
+  return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
+}
+inline V3 normalize(V3 a) {
+  double l = std::sqrt(dot(a, a));
+  return l > 0 ? (1.0 / l) * a : V3{0, 0, 0};
+}
+
+// ---------------------------------------------------------------- O3 calcTangent
+// PAPER.md:353-359, verbatim semantics.
+inline V3 calcTangent(int idx, int count, V3 prev, V3 curr, V3 next) {
+  if (idx == 0) return normalize(next - curr);               // Root
+  else if (idx == count - 1) return normalize(curr - prev);  // Tip
+  else return normalize(next - prev);
+}
+
+// ---------------------------------------------------------------- word (R7, R8)
+// [63:40] dq | [39:16] sid | [15:9] j | [8:0] t9. fp32, one rounding per op.
+inline uint32_t quant_depth(float zn) {
+  float s = zn * 16777215.0f;
+  s = s + 0.5f;
+  uint32_t q = (uint32_t)s;
+  return std::min<uint32_t>(q, 0xFFFFFEu);
+}
+inline uint32_t quant_t(float t) {
+  float s = t * 511.0f;
+  s = s + 0.5f;
+  return (uint32_t)s;
+}
+inline uint64_t pack(float zn, uint32_t sid, uint32_t j, float t) {
+  return (uint64_t(quant_depth(zn)) << 40) | (uint64_t(sid & 0xFFFFFFu) << 16) |
+         (uint64_t(j & 0x7Fu) << 9) | uint64_t(quant_t(t) & 0x1FFu);
+}
+inline uint32_t w_dq(uint64_t w) { return uint32_t(w >> 40); }
+inline uint32_t w_sid(uint64_t w) { return uint32_t(w >> 16) & 0xFFFFFFu; }
+inline uint32_t w_j(uint64_t w) { return uint32_t(w >> 9) & 0x7Fu; }
+inline uint32_t w_t9(uint64_t w) { return uint32_t(w) & 0x1FFu; }
+
+// ---------------------------------------------------------------- camera (R-proj)
+struct Cam {
+  float eye[3], r[3], u[3], f[3];
+  float near_z, fpx, A, B, half_w, half_h;
+  uint32_t W, H;
+};
+Cam make_cam(const orc_camera* c) {
+  Cam k;
+  for (int i = 0; i < 3; ++i) {
+    k.eye[i] = c->eye[i];
+    k.r[i] = c->right[i];
+    k.u[i] = c->up[i];
+    k.f[i] = c->forward[i];
+  }
+  k.near_z = c->near_z;
+  k.W = c->width;
+  k.H = c->height;
+  // constants computed once in double, rounded to float
+  double fpx = (0.5 * double(c->height)) / std::tan(0.5 * double(c->vfov_y));
+  double fn = double(c->far_z) - double(c->near_z);
+  k.fpx = float(fpx);
+  k.A = float(double(c->far_z) / fn);
+  k.B = float(double(c->far_z) * double(c->near_z) / fn);
+  k.half_w = 0.5f * float(c->width);
+  k.half_h = 0.5f * float(c->height);
+  return k;
+}
+struct Proj {
+  float sx, sy, zn, zv;
+  bool valid;
+};
+// fp32, fixed operation order: dot(a,b) = (a.x*b.x + a.y*b.y) + a.z*b.z
+inline float dot3f(float ax, float ay, float az, const float* b) {
+  float s = ax * b[0];
+  float t = ay * b[1];
+  s = s + t;
+  t = az * b[2];
+  return s + t;
+}
+inline Proj project(const Cam& k, float px, float py, float pz) {
+  float qx = px - k.eye[0], qy = py - k.eye[1], qz = pz - k.eye[2];
+  float xv = dot3f(qx, qy, qz, k.r);
+  float yv = dot3f(qx, qy, qz, k.u);
+  float zv = dot3f(qx, qy, qz, k.f);
+  Proj o;
+  o.zv = zv;
+  o.valid = zv >= k.near_z;
+  if (!o.valid) {
+    o.sx = o.sy = o.zn = 0.f;
+    return o;
+  }
+  float a = k.fpx * xv;
+  a = a / zv;
+  o.sx = k.half_w + a;
+  float b = k.fpx * yv;
+  b = b / zv;
+  o.sy = k.half_h - b;
+  float c = k.B / zv;
+  o.zn = k.A - c;
+  return o;
+}
+
+// ---------------------------------------------------------------- scene
+struct Groom {
+  uint32_t V, Lv, T, Q;
+  std::vector<float> pos, ao, xform;
+  std::vector<uint32_t> idx, npt, off;  // off = exclusive scan of npt (size T+1)
+  orc_style st;
+  uint32_t N;         // strands per instance
+  uint32_t sid_base;  // first stable strand id
+  uint32_t gid_base;  // first bundle-instance index
+  uint32_t c_full;
+  const float* X(uint32_t layer, uint32_t v) const { return &pos[(size_t(layer) * V + v) * 3]; }
+  double AO(uint32_t layer, uint32_t v) const { return ao.empty() ? 1.0 : double(ao[size_t(layer) * V + v]); }
+};
+
+struct Entry {
+  uint32_t nlod, C, slot_base, vertex_base;
+};
+
+}  // namespace
+
+struct orc_frame {
+  std::vector<Groom> grooms;
+  std::vector<Entry> table;
+  std::vector<float> L;
+  uint32_t n_strands = 0;
+  uint64_t n_vertices = 0;
+  std::vector<double> v64;
+  std::vector<float> v32;
+  uint32_t W = 0, H = 0;
+  std::vector<uint64_t> gbuf;
+  std::vector<double> colour;
+  std::vector<float> tang;
+  std::vector<double> out;
+};
+
+namespace {
+
+// exclusive scans over bundle-instances in index order (O1 step 6)
+void rescan(orc_frame* f) {
+  uint32_t slot = 0;
+  uint64_t vtx = 0;
+  for (auto& e : f->table) {
+    e.slot_base = slot;
+    e.vertex_base = uint32_t(vtx);
+    slot += e.nlod;
+    vtx += uint64_t(e.nlod) * e.C;
+  }
+  f->n_strands = slot;
+  f->n_vertices = vtx;
+}
+
+// Eq. 1 and Eq. 4-5, fp32. R14: C = min(C, C_full),
+// C_raw = max(C_raw, 3).
+void lod_counts(float L, uint32_t N, float delta, uint32_t Lv, uint32_t c_full, uint32_t out[3]) {
+  uint32_t nlod = 0;
+  if (N > 0) {
+    float a = float(N) + delta;
+    a = L * a;
+    a = std::ceil(a);
+    a = std::min(std::max(a, 1.0f), float(N));
+    nlod = uint32_t(a);
+  }
+  float s = std::sqrt(L);
+  s = s * 127.0f;
+  s = std::floor(s);
+  uint32_t craw = uint32_t(s);
+  craw = std::max(craw, std::max(Lv, 3u));
+  uint32_t lg = 31u - uint32_t(__builtin_clz(craw - 1u));  // floor(log2(craw-1)), craw >= 3
+  uint32_t C = std::min((1u << lg) + 1u, 127u);
+  C = std::min(C, c_full);
+  out[0] = nlod;
+  out[1] = craw;
+  out[2] = C;
+}
+
+// ---------------------------------------------------------------- O2 generation (fp64)
+struct Base {
+  V3 p, T;     // position and unit tangent of the base spline
+  double ao;   // R25
+  uint32_t i;  // interval
+  double t;
+};
+
+struct StrandCtx {
+  const Groom* g;
+  uint32_t tri;
+  std::vector<V3> P, m, Pc, mc;  // strand's and centre curve's layer points / Catmull-Rom tangents
+  std::vector<double> AOl;
+};
+
+void layer_points(const Groom& g, uint32_t tri, const double b[3], std::vector<V3>& P,
+                  std::vector<V3>& m, std::vector<double>* AOl) {
+  const uint32_t* v = &g.idx[size_t(tri) * 3];
+  P.resize(g.Lv);
+  m.resize(g.Lv);
+  if (AOl) AOl->resize(g.Lv);
+  for (uint32_t i = 0; i < g.Lv; ++i) {
+    const float *x0 = g.X(i, v[0]), *x1 = g.X(i, v[1]), *x2 = g.X(i, v[2]);
+    // R1: barycentric interpolation inside the prism layer (paper: bilinear in a quad)
+    P[i] = {b[0] * x0[0] + b[1] * x1[0] + b[2] * x2[0], b[0] * x0[1] + b[1] * x1[1] + b[2] * x2[1],
+            b[0] * x0[2] + b[1] * x1[2] + b[2] * x2[2]};
+    if (AOl) (*AOl)[i] = b[0] * g.AO(i, v[0]) + b[1] * g.AO(i, v[1]) + b[2] * g.AO(i, v[2]);
+  }
+  // R4: finite-difference (Catmull-Rom) tangents, one-sided at the ends (Code 1 pass 1)
+  for (uint32_t i = 0; i < g.Lv; ++i) {
+    if (i == 0) m[i] = P[1] - P[0];
+    else if (i == g.Lv - 1) m[i] = P[i] - P[i - 1];
+    else m[i] = 0.5 * (P[i + 1] - P[i - 1]);
+  }
+}
+
+// R5: control point j of C, uniform in w; layer i at w = i/(Lv-1); integer index arithmetic.
+inline void cp_param(uint32_t j, uint32_t C, uint32_t Lv, uint32_t& i, double& t, double& w) {
+  uint32_t num = j * (Lv - 1), den = C - 1;
+  i = std::min(num / den, Lv - 2);
+  t = double(num - i * den) / double(den);
+  w = double(j) / double(den);
+}
+
+// cubic Hermite between layers i and i+1
+inline void hermite(const std::vector<V3>& P, const std::vector<V3>& m, uint32_t i, double t, V3& p,
+                    V3& T) {
+  double t2 = t * t, t3 = t2 * t;
+  double h00 = 2 * t3 - 3 * t2 + 1, h10 = t3 - 2 * t2 + t, h01 = -2 * t3 + 3 * t2, h11 = t3 - t2;
+  p = h00 * P[i] + h10 * m[i] + h01 * P[i + 1] + h11 * m[i + 1];
+  double d00 = 6 * t2 - 6 * t, d10 = 3 * t2 - 4 * t + 1, d01 = -6 * t2 + 6 * t, d11 = 3 * t2 - 2 * t;
+  T = normalize(d00 * P[i] + d10 * m[i] + d01 * P[i + 1] + d11 * m[i + 1]);
+}
+
+// root barycentrics (R6): fold map on 24-bit integers, so that fp32 and fp64 agree exactly
+void root_bary(const Groom& g, uint32_t id_local, double b[3]) {
+  uint32_t a1 = u24(hash3(g.st.seed, id_local, ST_ROOT1));
+  uint32_t a2 = u24(hash3(g.st.seed, id_local, ST_ROOT2));
+  if (a1 + a2 > 16777216u) {
+    a1 = 16777216u - a1;
+    a2 = 16777216u - a2;
+  }
+  b[1] = double(a1) / 16777216.0;
+  b[2] = double(a2) / 16777216.0;
+  b[0] = (1.0 - b[1]) - b[2];
+}
+
+uint32_t tri_of(const Groom& g, uint32_t id_local) {
+  return uint32_t(std::upper_bound(g.off.begin(), g.off.end(), id_local) - g.off.begin()) - 1u;
+}
+
+// frizz lattice value (R24): four hashed uniforms, variance 1, no transcendental
+double frizz_lattice(const Groom& g, uint32_t id_local, uint32_t n, uint32_t ch) {
+  double s = 0;
+  for (uint32_t q = 0; q < 4; ++q) s += u01(hash3(g.st.seed, id_local, ST_FRIZZ + 8u * n + 4u * ch + q));
+  return (s - 2.0) * std::sqrt(3.0);
+}
+
+// one strand, groom-local space, C control points: out[C][4], base_tan[C][3]
+void strand_local(const Groom& g, uint32_t id_local, uint32_t C, double* out, double* base_tan) {
+  const orc_style& st = g.st;
+  uint32_t tri = tri_of(g, id_local);
+  double b[3];
+  root_bary(g, id_local, b);
+  std::vector<V3> P, m, Pc, mc;
+  std::vector<double> AOl;
+  layer_points(g, tri, b, P, m, &AOl);
+  const double third[3] = {1.0 / 3.0, 1.0 / 3.0, 1.0 / 3.0};
+  layer_points(g, tri, third, Pc, mc, nullptr);
+  const uint32_t* v = &g.idx[size_t(tri) * 3];
+  double curl_u = u01(hash3(st.seed, id_local, ST_CURL));
+  for (uint32_t j = 0; j < C; ++j) {
+    uint32_t i;
+    double t, w;
+    cp_param(j, C, g.Lv, i, t, w);
+    V3 p, T, c, Tc;
+    hermite(P, m, i, t, p, T);
+    hermite(Pc, mc, i, t, c, Tc);
+    double ao = (1 - t) * AOl[i] + t * AOl[i + 1];
+    ao = std::min(std::max(ao, 0.0), 1.0);
+    // frame from the cage edge v0->v1, orthogonalised against the UNSTYLED base tangent
+    const float *e0a = g.X(i, v[0]), *e0b = g.X(i, v[1]), *e1a = g.X(i + 1, v[0]), *e1b = g.X(i + 1, v[1]);
+    V3 E0 = {double(e0b[0]) - e0a[0], double(e0b[1]) - e0a[1], double(e0b[2]) - e0a[2]};
+    V3 E1 = {double(e1b[0]) - e1a[0], double(e1b[1]) - e1a[1], double(e1b[2]) - e1a[2]};
+    V3 E = (1 - t) * E0 + t * E1;
+    V3 Nn = E - dot(E, T) * T;
+    if (dot(Nn, Nn) < 1e-20) {  // degenerate: least-aligned coordinate axis
+      double ax = std::fabs(T.x), ay = std::fabs(T.y), az = std::fabs(T.z);
+      V3 a = (ax <= ay && ax <= az) ? V3{1, 0, 0} : (ay <= az ? V3{0, 1, 0} : V3{0, 0, 1});
+      Nn = a - dot(a, T) * T;
+    }
+    V3 N = normalize(Nn);
+    V3 B = cross(T, N);
+    // styling, fixed order clump -> twist -> curl -> frizz (R24)
+    if (st.op_mask & ORC_OP_CLUMP) {
+      double we = 1.0;
+      for (uint32_t e = 0; e < st.clump_exp; ++e) we *= w;
+      p = p + (double(st.clump_strength) * we) * (c - p);
+    }
+    if (st.op_mask & ORC_OP_TWIST) {
+      double th = 2.0 * PI * double(st.twist_turns) * w;
+      double cs = std::cos(th), sn = std::sin(th);
+      V3 d = p - c;  // Rodrigues rotation of d about Tc
+      V3 dr = cs * d + sn * cross(Tc, d) + (dot(Tc, d) * (1.0 - cs)) * Tc;
+      p = c + dr;
+    }
+    if (st.op_mask & ORC_OP_CURL) {
+      double th = 2.0 * PI * (double(st.curl_turns) * w + curl_u);
+      double a = st.curl_ramp_w0 > 0 ? std::min(w / double(st.curl_ramp_w0), 1.0) : 1.0;
+      p = p + (double(st.curl_radius) * a) * (std::cos(th) * N + std::sin(th) * B);
+    }
+    if (st.op_mask & ORC_OP_FRIZZ) {
+      uint32_t cells = std::max(st.frizz_cells, 1u);
+      double x = w * double(cells);
+      uint32_t c0 = std::min(uint32_t(std::floor(x)), cells - 1u);
+      double fr = x - double(c0);
+      double s = fr * fr * (3.0 - 2.0 * fr);
+      double n0 = (1 - s) * frizz_lattice(g, id_local, c0, 0) + s * frizz_lattice(g, id_local, c0 + 1, 0);
+      double n1 = (1 - s) * frizz_lattice(g, id_local, c0, 1) + s * frizz_lattice(g, id_local, c0 + 1, 1);
+      double env = st.frizz_ramp_w0 > 0 ? std::min(w / double(st.frizz_ramp_w0), 1.0) : 1.0;
+      p = p + (double(st.frizz_sigma) * env) * (n0 * N + n1 * B);
+    }
+    out[j * 4 + 0] = p.x;
+    out[j * 4 + 1] = p.y;
+    out[j * 4 + 2] = p.z;
+    out[j * 4 + 3] = ao;
+    if (base_tan) {
+      base_tan[j * 3 + 0] = T.x;
+      base_tan[j * 3 + 1] = T.y;
+      base_tan[j * 3 + 2] = T.z;
+    }
+  }
+}
+
+// ---------------------------------------------------------------- sid -> vertices
+struct Loc {
+  bool ok;
+  uint64_t voff;
+  uint32_t C;
+};
+Loc locate(const orc_frame* f, uint32_t sid) {
+  for (const Groom& g : f->grooms) {
+    uint32_t n = g.N * g.Q;
+    if (sid >= g.sid_base && sid < g.sid_base + n) {
+      uint32_t rel = sid - g.sid_base;
+      uint32_t q = rel / g.N, id_local = rel % g.N;
+      uint32_t tri = tri_of(g, id_local);
+      uint32_t k = id_local - g.off[tri];
+      const Entry& e = f->table[g.gid_base + q * g.T + tri];
+      if (k >= e.nlod) return {false, 0, 0};
+      return {true, uint64_t(e.vertex_base) + uint64_t(k) * e.C, e.C};
+    }
+  }
+  return {false, 0, 0};
+}
+
+inline V3 vtx(const orc_frame* f, uint64_t i) {
+  return {double(f->v32[i * 4]), double(f->v32[i * 4 + 1]), double(f->v32[i * 4 + 2])};
+}
+
+// screen tangent of the segment a word names (R22), fp32 fixed order
+void screen_tangent(const orc_frame* f, const Cam& k, uint64_t word, float T[2]) {
+  T[0] = 1.f;
+  T[1] = 0.f;
+  Loc l = locate(f, w_sid(word));
+  if (!l.ok) return;
+  uint64_t i0 = l.voff + w_j(word);
+  Proj a = project(k, f->v32[i0 * 4], f->v32[i0 * 4 + 1], f->v32[i0 * 4 + 2]);
+  Proj b = project(k, f->v32[i0 * 4 + 4], f->v32[i0 * 4 + 5], f->v32[i0 * 4 + 6]);
+  float dx = b.sx - a.sx, dy = b.sy - a.sy;
+  float dd = dx * dx;
+  float e = dy * dy;
+  dd = dd + e;
+  if (!(dd >= 1e-12f)) return;
+  float len = std::sqrt(dd);
+  T[0] = dx / len;
+  T[1] = dy / len;
+}
+
+}  // namespace
+
+// =====================================================================================
+extern "C" {
+
+uint32_t orc_pcg(uint32_t v) { return pcg(v); }
+uint32_t orc_hash3(uint32_t seed, uint32_t id, uint32_t stream) { return hash3(seed, id, stream); }
+void orc_lod_counts(float L, uint32_t N, float delta, uint32_t n_layers, uint32_t c_full,
+                    uint32_t out[3]) {
+  lod_counts(L, N, delta, n_layers, c_full, out);
+}
+void orc_calc_tangent(int idx, int count, const double prev[3], const double curr[3],
+                      const double next[3], double out[3]) {
+  V3 t = calcTangent(idx, count, {prev[0], prev[1], prev[2]}, {curr[0], curr[1], curr[2]},
+                     {next[0], next[1], next[2]});
+  out[0] = t.x;
+  out[1] = t.y;
+  out[2] = t.z;
+}
+uint64_t orc_pack(float zn, uint32_t sid, uint32_t j, float t) { return pack(zn, sid, j, t); }
+void orc_unpack(uint64_t w, uint32_t out[4]) {
+  out[0] = w_dq(w);
+  out[1] = w_sid(w);
+  out[2] = w_j(w);
+  out[3] = w_t9(w);
+}
+int orc_project(const orc_camera* cam, const float p[3], float out[4]) {
+  Cam k = make_cam(cam);
+  Proj r = project(k, p[0], p[1], p[2]);
+  out[0] = r.sx;
+  out[1] = r.sy;
+  out[2] = r.zn;
+  out[3] = r.zv;
+  return r.valid ? 1 : 0;
+}
+
+// O4 coverage of one segment at one pixel (fp32, fixed order). Returns bit0 = conservative,
+// bit1 = centre (R9-R11; centre requires conservative, so centre ⊂ conservative exactly).
+static inline int cover_px(float ax, float ay, float bx, float by, float rho2, int x, int y, float& t_out) {
+  float dx = bx - ax, dy = by - ay;
+  float dd = dx * dx;
+  {
+    float e = dy * dy;
+    dd = dd + e;
+  }
+  float cx = float(x) + 0.5f, cy = float(y) + 0.5f;
+  float ux = cx - ax, uy = cy - ay;
+  float t = 0.f;
+  if (dd > 0.f) {
+    float n = ux * dx;
+    float e = uy * dy;
+    n = n + e;
+    t = n / dd;
+    t = std::min(std::max(t, 0.0f), 1.0f);
+  }
+  t_out = t;
+  // conservative: closed segment meets closed pixel square (R10)
+  float mnx = std::min(ax, bx), mxx = std::max(ax, bx), mny = std::min(ay, by), mxy = std::max(ay, by);
+  bool box = mnx <= float(x + 1) && mxx >= float(x) && mny <= float(y + 1) && mxy >= float(y);
+  float c1 = dx * uy;
+  float c2 = dy * ux;
+  float cr = std::fabs(c1 - c2);
+  float ext = std::fabs(dx) + std::fabs(dy);
+  ext = 0.5f * ext;
+  bool cons = box && cr <= ext;
+  if (!cons) return 0;
+  // centre: closest point on the segment within rho of the pixel centre (R9)
+  float qx = t * dx;
+  qx = ax + qx;
+  float qy = t * dy;
+  qy = ay + qy;
+  float ex = cx - qx, ey = cy - qy;
+  float d2 = ex * ex;
+  {
+    float e = ey * ey;
+    d2 = d2 + e;
+  }
+  return (d2 <= rho2) ? 3 : 1;
+}
+
+void orc_segment_cover(const float a[2], const float b[2], float rho, uint32_t w, uint32_t h,
+                       uint8_t* cover, float* tq) {
+  float rho2 = rho * rho;
+  for (uint32_t y = 0; y < h; ++y)
+    for (uint32_t x = 0; x < w; ++x) {
+      float t;
+      cover[y * w + x] = uint8_t(cover_px(a[0], a[1], b[0], b[1], rho2, int(x), int(y), t));
+      if (tq) tq[y * w + x] = t;
+    }
+}
+
+orc_frame* orc_frame_create(void) { return new orc_frame(); }
+void orc_frame_destroy(orc_frame* f) { delete f; }
+
+int orc_frame_add_groom(orc_frame* f, const orc_groom* in) {
+  if (!in || in->n_layers < 2 || in->n_tris == 0 || in->style.spi == 0) return -1;
+  Groom g;
+  g.V = in->n_verts;
+  g.Lv = in->n_layers;
+  g.T = in->n_tris;
+  g.Q = std::max(in->n_instances, 1u);
+  g.pos.assign(in->pos, in->pos + size_t(g.Lv) * g.V * 3);
+  if (in->ao) g.ao.assign(in->ao, in->ao + size_t(g.Lv) * g.V);
+  g.idx.assign(in->idx, in->idx + size_t(g.T) * 3);
+  g.npt.assign(in->strands_per_tri, in->strands_per_tri + g.T);
+  if (in->xform) g.xform.assign(in->xform, in->xform + size_t(g.Q) * 12);
+  g.st = in->style;
+  g.off.resize(g.T + 1);
+  uint32_t acc = 0;
+  for (uint32_t t = 0; t < g.T; ++t) {
+    g.off[t] = acc;
+    acc += g.npt[t];
+  }
+  g.off[g.T] = acc;
+  g.N = acc;
+  g.c_full = (g.Lv - 1) * g.st.spi + 1;  // PAPER.md:406 (Code 1 line 29)
+  if (g.c_full > 127) return -2;
+  if (f->grooms.empty()) {
+    g.sid_base = 0;
+    g.gid_base = 0;
+  } else {
+    const Groom& p = f->grooms.back();
+    g.sid_base = p.sid_base + p.N * p.Q;
+    g.gid_base = p.gid_base + p.T * p.Q;
+  }
+  if (uint64_t(g.sid_base) + uint64_t(g.N) * g.Q >= (1ull << 24)) return -3;
+  f->grooms.push_back(std::move(g));
+  return int(f->grooms.size()) - 1;
+}
+
+// ------------------------------------------------------------------ O1
+int orc_frame_lod(orc_frame* f, const orc_camera* cam, const float* lambda, uint32_t n_lambda) {
+  Cam k = make_cam(cam);
+  f->table.clear();
+  f->L.clear();
+  float Wf = float(k.W), Hf = float(k.H);
+  for (size_t gi = 0; gi < f->grooms.size(); ++gi) {
+    const Groom& g = f->grooms[gi];
+    float lam = n_lambda == 0 ? 0.f : lambda[n_lambda == 1 ? 0 : gi];
+    for (uint32_t q = 0; q < g.Q; ++q)
+      for (uint32_t t = 0; t < g.T; ++t) {
+        Entry e{0, 0, 0, 0};
+        uint32_t N = g.npt[t];
+        float Lsel = -1.f;
+        if (!(lam > 0.f)) {  // R14: LOD and culling off
+          e.nlod = N;
+          e.C = g.c_full;
+        } else {
+          // project each layer's vertices, one AABB over all layers (Eq. 3)
+          float mnx = INFINITY, mny = INFINITY, mxx = -INFINITY, mxy = -INFINITY;
+          uint32_t n_valid = 0, n_all = 0;
+          const float* M = g.xform.empty() ? nullptr : &g.xform[size_t(q) * 12];
+          for (uint32_t i = 0; i < g.Lv; ++i)
+            for (int c = 0; c < 3; ++c) {
+              const float* x = g.X(i, g.idx[size_t(t) * 3 + c]);
+              float wx = x[0], wy = x[1], wz = x[2];
+              if (M) {  // ((m0*x + m1*y) + m2*z) + m3, fp32
+                float r[3];
+                for (int a = 0; a < 3; ++a) {
+                  float s = M[a * 4 + 0] * x[0];
+                  float u = M[a * 4 + 1] * x[1];
+                  s = s + u;
+                  u = M[a * 4 + 2] * x[2];
+                  s = s + u;
+                  r[a] = s + M[a * 4 + 3];
+                }
+                wx = r[0];
+                wy = r[1];
+                wz = r[2];
+              }
+              Proj p = project(k, wx, wy, wz);
+              ++n_all;
+              if (p.valid) {
+                ++n_valid;
+                mnx = std::min(mnx, p.sx);
+                mxx = std::max(mxx, p.sx);
+                mny = std::min(mny, p.sy);
+                mxy = std::max(mxy, p.sy);
+              }
+            }
+          bool culled = false;
+          if (n_valid == 0) culled = true;  // R13: all behind the near plane
+          else if (n_valid < n_all) Lsel = 1.f;  // R13: some behind => full detail
+          else {
+            if (mxx < 0.f || mnx > Wf || mxy < 0.f || mny > Hf) culled = true;
+            else {
+              float dx = mxx - mnx, dy = mxy - mny;
+              float dd = dx * dx;
+              float ee = dy * dy;
+              dd = dd + ee;
+              float diag = std::sqrt(dd);
+              float r = diag / Hf;  // Eq. 2, R_y = H
+              r = r * lam;
+              Lsel = std::min(std::max(r, 0.0f), 1.0f);
+            }
+          }
+          if (culled) {
+            e.nlod = 0;
+            e.C = 0;
+          } else {
+            float delta = float(u01(hash3(g.st.seed, q * g.T + t, ST_LOD)));
+            uint32_t o[3];
+            lod_counts(Lsel, N, delta, g.Lv, g.c_full, o);
+            e.nlod = o[0];
+            e.C = o[0] ? o[2] : 0;
+          }
+        }
+        f->table.push_back(e);
+        f->L.push_back(Lsel);
+      }
+  }
+  rescan(f);
+  return 0;
+}
+
+uint32_t orc_frame_n_bundles(const orc_frame* f) {
+  uint32_t n = 0;
+  for (const Groom& g : f->grooms) n += g.T * g.Q;
+  return n;
+}
+uint32_t orc_frame_n_strands_total(const orc_frame* f) {
+  uint32_t n = 0;
+  for (const Groom& g : f->grooms) n += g.N * g.Q;
+  return n;
+}
+uint32_t orc_frame_n_strands(const orc_frame* f) { return f->n_strands; }
+uint64_t orc_frame_n_vertices(const orc_frame* f) { return f->n_vertices; }
+void orc_frame_get_table(const orc_frame* f, uint32_t* t4, float* L) {
+  for (size_t i = 0; i < f->table.size(); ++i) {
+    if (t4) {
+      t4[i * 4 + 0] = f->table[i].nlod;
+      t4[i * 4 + 1] = f->table[i].C;
+      t4[i * 4 + 2] = f->table[i].slot_base;
+      t4[i * 4 + 3] = f->table[i].vertex_base;
+    }
+    if (L) L[i] = f->L[i];
+  }
+}
+int orc_frame_set_table(orc_frame* f, const uint32_t* t4, uint32_t n) {
+  if (n != orc_frame_n_bundles(f)) return -1;
+  f->table.resize(n);
+  f->L.assign(n, -1.f);
+  for (uint32_t i = 0; i < n; ++i) f->table[i] = {t4[i * 4], t4[i * 4 + 1], 0, 0};
+  rescan(f);
+  for (uint32_t i = 0; i < n; ++i)
+    if (f->table[i].nlod && (f->table[i].slot_base != t4[i * 4 + 2] || f->table[i].vertex_base != t4[i * 4 + 3]))
+      return -2;  // the supplied scans disagree with the definition
+  return 0;
+}
+
+// ------------------------------------------------------------------ O2
+int orc_frame_generate(orc_frame* f) {
+  f->v64.assign(size_t(f->n_vertices) * 4, 0.0);
+  std::vector<double> loc;
+  for (const Groom& g : f->grooms)
+    for (uint32_t q = 0; q < g.Q; ++q)
+      for (uint32_t t = 0; t < g.T; ++t) {
+        const Entry& e = f->table[g.gid_base + q * g.T + t];
+        if (e.nlod == 0) continue;
+        loc.resize(size_t(e.C) * 4);
+        const float* M = g.xform.empty() ? nullptr : &g.xform[size_t(q) * 12];
+        for (uint32_t k = 0; k < e.nlod; ++k) {  // R27: surviving strands = local indices k < N_LOD
+          strand_local(g, g.off[t] + k, e.C, loc.data(), nullptr);
+          double* o = &f->v64[(size_t(e.vertex_base) + size_t(k) * e.C) * 4];
+          for (uint32_t j = 0; j < e.C; ++j) {
+            double x = loc[j * 4], y = loc[j * 4 + 1], z = loc[j * 4 + 2];
+            if (M) {  // instance transform applied last (DESIGN.md R-inst)
+              double wx = double(M[0]) * x + double(M[1]) * y + double(M[2]) * z + double(M[3]);
+              double wy = double(M[4]) * x + double(M[5]) * y + double(M[6]) * z + double(M[7]);
+              double wz = double(M[8]) * x + double(M[9]) * y + double(M[10]) * z + double(M[11]);
+              x = wx;
+              y = wy;
+              z = wz;
+            }
+            o[j * 4 + 0] = x;
+            o[j * 4 + 1] = y;
+            o[j * 4 + 2] = z;
+            o[j * 4 + 3] = loc[j * 4 + 3];
+          }
+        }
+      }
+  f->v32.resize(f->v64.size());
+  for (size_t i = 0; i < f->v64.size(); ++i) f->v32[i] = float(f->v64[i]);
+  return 0;
+}
+void orc_frame_get_vertices_f64(const orc_frame* f, double* o) {
+  std::memcpy(o, f->v64.data(), f->v64.size() * sizeof(double));
+}
+void orc_frame_get_vertices_f32(const orc_frame* f, float* o) {
+  std::memcpy(o, f->v32.data(), f->v32.size() * sizeof(float));
+}
+int orc_frame_set_vertices_f32(orc_frame* f, const float* v, uint64_t n) {
+  if (n != f->n_vertices) return -1;
+  f->v32.assign(v, v + size_t(n) * 4);
+  return 0;
+}
+int orc_strand(const orc_frame* f, uint32_t groom, uint32_t id_local, uint32_t C, double* out,
+               double* base_tan) {
+  if (groom >= f->grooms.size() || id_local >= f->grooms[groom].N || C < 2) return -1;
+  strand_local(f->grooms[groom], id_local, C, out, base_tan);
+  return 0;
+}
+int orc_root(const orc_frame* f, uint32_t groom, uint32_t id_local, double b[3], uint32_t* tri) {
+  if (groom >= f->grooms.size() || id_local >= f->grooms[groom].N) return -1;
+  root_bary(f->grooms[groom], id_local, b);
+  if (tri) *tri = tri_of(f->grooms[groom], id_local);
+  return 0;
+}
+
+// ------------------------------------------------------------------ O4 (+ O5: the min IS the resolve)
+int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
+                     const uint32_t* order, uint64_t counts[3]) {
+  Cam k = make_cam(cam);
+  f->W = k.W;
+  f->H = k.H;
+  f->gbuf.assign(size_t(k.W) * k.H * 2, EMPTY);
+  if (f->v32.size() != size_t(f->n_vertices) * 4) return -1;
+  uint64_t n_center = 0, n_cons = 0, n_seg = 0;
+  // strand directory in slot order
+  struct S {
+    uint64_t voff;
+    uint32_t C, sid;
+    float width;
+  };
+  std::vector<S> dir;
+  dir.reserve(f->n_strands);
+  for (const Groom& g : f->grooms)
+    for (uint32_t q = 0; q < g.Q; ++q)
+      for (uint32_t t = 0; t < g.T; ++t) {
+        const Entry& e = f->table[g.gid_base + q * g.T + t];
+        for (uint32_t kk = 0; kk < e.nlod; ++kk)
+          dir.push_back({uint64_t(e.vertex_base) + uint64_t(kk) * e.C, e.C,
+                         g.sid_base + q * g.N + g.off[t] + kk, g.st.width_world});
+      }
+  for (size_t si = 0; si < dir.size(); ++si) {
+    const S& s = dir[order ? order[si] : si];
+    for (uint32_t j = 0; j + 1 < s.C; ++j) {
+      const float* va = &f->v32[(s.voff + j) * 4];
+      const float* vb = va + 4;
+      Proj a = project(k, va[0], va[1], va[2]);
+      Proj b = project(k, vb[0], vb[1], vb[2]);
+      if (!a.valid || !b.valid) continue;  // R12
+      ++n_seg;
+      // centre radius (R9)
+      float rho;
+      if (s.width > 0.f) {
+        float zm = a.zv + b.zv;
+        zm = 0.5f * zm;
+        float wpx = s.width * k.fpx;
+        wpx = wpx / zm;
+        wpx = std::min(std::max(wpx, 0.25f), 1.0f);
+        rho = 0.5f * wpx;
+      } else
+        rho = 0.5f * prm->center_diameter_px;
+      float rho2 = rho * rho;
+      float mnx = std::min(a.sx, b.sx), mxx = std::max(a.sx, b.sx);
+      float mny = std::min(a.sy, b.sy), mxy = std::max(a.sy, b.sy);
+      // candidate pixels: [floor(min)-1, floor(max)+1] clipped to the viewport
+      float fx0 = std::max(std::floor(mnx) - 1.f, 0.f), fx1 = std::min(std::floor(mxx) + 1.f, float(k.W) - 1.f);
+      float fy0 = std::max(std::floor(mny) - 1.f, 0.f), fy1 = std::min(std::floor(mxy) + 1.f, float(k.H) - 1.f);
+      if (!(fx0 <= fx1) || !(fy0 <= fy1)) continue;
+      int x0 = int(fx0), x1 = int(fx1), y0 = int(fy0), y1 = int(fy1);
+      float dz = b.zn - a.zn;
+      for (int y = y0; y <= y1; ++y)
+        for (int x = x0; x <= x1; ++x) {
+          float t;
+          int c = cover_px(a.sx, a.sy, b.sx, b.sy, rho2, x, y, t);
+          if (!c) continue;
+          float zn = t * dz;  // R11: depth at the closest point, linear in screen space
+          zn = a.zn + zn;
+          if (zn < 0.f || zn > 1.f) continue;
+          uint64_t w = pack(zn, s.sid, j, t);
+          uint64_t* px = &f->gbuf[(size_t(y) * k.W + x) * 2];
+          ++n_cons;
+          px[1] = std::min(px[1], w);  // PAPER.md:85 atomic min, depth in the high bits
+          if (c & 2) {
+            ++n_center;
+            px[0] = std::min(px[0], w);
+          }
+        }
+    }
+  }
+  if (counts) {
+    counts[0] = n_center;
+    counts[1] = n_cons;
+    counts[2] = n_seg;
+  }
+  return 0;
+}
+void orc_frame_get_gbuffer(const orc_frame* f, uint64_t* o) {
+  std::memcpy(o, f->gbuf.data(), f->gbuf.size() * sizeof(uint64_t));
+}
+int orc_frame_set_gbuffer(orc_frame* f, const uint64_t* in, uint32_t w, uint32_t h) {
+  f->W = w;
+  f->H = h;
+  f->gbuf.assign(in, in + size_t(w) * h * 2);
+  return 0;
+}
+
+// ------------------------------------------------------------------ O6
+int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) {
+  Cam k = make_cam(cam);
+  if (f->W != k.W || f->H != k.H) return -1;
+  size_t np = size_t(k.W) * k.H;
+  f->colour.assign(np * 3, 0.0);
+  f->tang.assign(np * 4, 0.f);
+  V3 eye = {double(k.eye[0]), double(k.eye[1]), double(k.eye[2])};
+  for (size_t p = 0; p < np; ++p) {
+    uint64_t G = f->gbuf[p * 2], A = f->gbuf[p * 2 + 1];
+    if (A != EMPTY) screen_tangent(f, k, A, &f->tang[p * 4 + 2]);
+    if (G == EMPTY) continue;
+    screen_tangent(f, k, G, &f->tang[p * 4]);
+    Loc l = locate(f, w_sid(G));
+    if (!l.ok) return -2;
+    const Groom* g = nullptr;
+    for (const Groom& gg : f->grooms)
+      if (w_sid(G) >= gg.sid_base && w_sid(G) < gg.sid_base + gg.N * gg.Q) g = &gg;
+    int j = int(w_j(G)), C = int(l.C);
+    double t = double(w_t9(G)) / 511.0;
+    auto V = [&](int i) { return vtx(f, l.voff + uint64_t(std::min(std::max(i, 0), C - 1))); };
+    V3 pos = (1 - t) * V(j) + t * V(j + 1);
+    double ao = (1 - t) * double(f->v32[(l.voff + j) * 4 + 3]) + t * double(f->v32[(l.voff + j + 1) * 4 + 3]);
+    // O3 tangents on the styled polyline, interpolated along the segment
+    V3 Tj = calcTangent(j, C, V(j - 1), V(j), V(j + 1));
+    V3 Tj1 = calcTangent(j + 1, C, V(j), V(j + 1), V(j + 2));
+    V3 T = normalize((1 - t) * Tj + t * Tj1);
+    double w = (double(j) + t) / double(C - 1);
+    double alb[3];
+    for (int c = 0; c < 3; ++c)
+      alb[c] = (1 - w) * double(g->st.albedo_root[c]) + w * double(g->st.albedo_tip[c]);
+    V3 Vd = normalize(eye - pos);
+    double rgb[3];
+    for (int c = 0; c < 3; ++c) rgb[c] = ao * double(prm->ambient_rgb[c]) * alb[c];
+    double beta = double(g->st.roughness), tilt = double(g->st.tilt);
+    for (uint32_t li = 0; li < prm->n_lights; ++li) {
+      V3 lp = {double(prm->light_pos[li][0]), double(prm->light_pos[li][1]), double(prm->light_pos[li][2])};
+      V3 Lv = lp - pos;
+      double d2 = dot(Lv, Lv);
+      V3 om = (1.0 / std::sqrt(d2)) * Lv;
+      double sin_i = std::min(std::max(dot(T, om), -1.0), 1.0);
+      double sin_o = std::min(std::max(dot(T, Vd), -1.0), 1.0);
+      double cos_i = std::sqrt(std::max(0.0, 1.0 - sin_i * sin_i));
+      double th = 0.5 * (std::asin(sin_i) + std::asin(sin_o));
+      double MR = std::exp(-(th + tilt) * (th + tilt) / (2.0 * beta * beta));
+      double MT = std::exp(-(th - 1.5 * tilt) * (th - 1.5 * tilt) / (8.0 * beta * beta));
+      for (int c = 0; c < 3; ++c) {
+        double E = double(prm->light_rgb[li][c]) / d2;
+        rgb[c] += E * cos_i * (double(prm->k_d) * alb[c] + double(prm->k_R) * MR + double(prm->k_TRT) * MT * alb[c]);
+      }
+    }
+    for (int c = 0; c < 3; ++c) f->colour[p * 3 + c] = rgb[c];
+  }
+  return 0;
+}
+void orc_frame_get_colour(const orc_frame* f, double* o) {
+  std::memcpy(o, f->colour.data(), f->colour.size() * sizeof(double));
+}
+void orc_frame_get_tangents(const orc_frame* f, float* o) {
+  std::memcpy(o, f->tang.data(), f->tang.size() * sizeof(float));
+}
+
+// ------------------------------------------------------------------ O7
+namespace {
+struct AccOut {
+  double C[3];
+  double alpha;
+};
+AccOut accumulate(const orc_frame* f, const orc_params* prm, int W, int H, int px, int py, float Tx,
+                  float Ty, uint32_t dq_ref, bool use_colour, const double* CP, uint32_t tauz_q) {
+  int r = prm->filter_radius;
+  double sp = double(r) * double(prm->s_par), sq = double(r) * double(prm->s_perp);
+  double inv_sp2 = sp > 0 ? 1.0 / (sp * sp) : 0.0, inv_sq2 = sq > 0 ? 1.0 / (sq * sq) : 0.0;
+  double inv_sc2 = 1.0 / (double(prm->sigma_c) * double(prm->sigma_c));
+  double S[3] = {0, 0, 0}, Wsum = 0, Hc = 0, Ha = 0;
+  for (int dy = -r; dy <= r; ++dy)
+    for (int dx = -r; dx <= r; ++dx) {
+      int qx = px + dx, qy = py + dy;
+      if (qx < 0 || qy < 0 || qx >= W || qy >= H) continue;  // PAPER.md:489 bounds check
+      size_t q = size_t(qy) * W + qx;
+      uint64_t GQ = f->gbuf[q * 2], AQ = f->gbuf[q * 2 + 1];
+      // R20: class of Q by a depth test on the quantised depths (integers)
+      auto close = [&](uint64_t w) {
+        uint32_t d = w_dq(w);
+        uint32_t diff = d > dq_ref ? d - dq_ref : dq_ref - d;
+        return diff <= tauz_q;  // PAPER.md:169 threshold 1.45e-3
+      };
+      int cls = 0;  // 1 = centre, 2 = cons-only
+      if (GQ != EMPTY && close(GQ)) cls = 1;
+      else if (AQ != EMPTY && close(AQ)) cls = 2;
+      if (!cls) continue;
+      // Eq. 9, fp32 fixed order (decides the strip membership)
+      float fdx = float(dx), fdy = float(dy);
+      float a = fdx * Tx;
+      float b = fdy * Ty;
+      float dpar = a + b;
+      float ex = dpar * Tx;
+      ex = fdx - ex;
+      float ey = dpar * Ty;
+      ey = fdy - ey;
+      float e2 = ex * ex;
+      {
+        float e3 = ey * ey;
+        e2 = e2 + e3;
+      }
+      float dperp = std::sqrt(e2);
+      if (dperp <= prm->w_strip) {  // PAPER.md:176, 498-503; R18: Q's class
+        if (cls == 1) Hc += 1;
+        else Ha += 1;
+      }
+      if (cls == 1) {  // R19: only centre-class neighbours carry colour
+        double w = std::exp(-double(dpar) * double(dpar) * inv_sp2 - double(dperp) * double(dperp) * inv_sq2);
+        if (use_colour) {
+          double d2 = 0;
+          for (int c = 0; c < 3; ++c) {
+            double d = CP[c] - f->colour[q * 3 + c];
+            d2 += d * d;
+          }
+          w *= std::exp(-d2 * inv_sc2);  // Eq. 10
+        }
+        for (int c = 0; c < 3; ++c) S[c] += w * f->colour[q * 3 + c];
+        Wsum += w;
+      }
+    }
+  AccOut o;
+  for (int c = 0; c < 3; ++c) o.C[c] = Wsum > 0 ? S[c] / Wsum : 0.0;
+  o.alpha = (Hc + Ha) > 0 ? Hc / (Hc + Ha) : 0.0;
+  return o;
+}
+}  // namespace
+
+int orc_frame_filter(orc_frame* f, const orc_camera* cam, const orc_params* prm) {
+  int W = int(cam->width), H = int(cam->height);
+  if (f->W != uint32_t(W) || f->H != uint32_t(H)) return -1;
+  size_t np = size_t(W) * H;
+  if (f->colour.size() != np * 3) return -2;
+  f->out.assign(np * 4, 0.0);
+  uint32_t tauz_q = uint32_t(std::floor(double(prm->tau_z) * 16777215.0 + 0.5));
+  uint32_t taufly_q = uint32_t(std::floor(double(prm->tau_fly) * 16777215.0 + 0.5));
+  double bg[3] = {double(prm->background_rgb[0]), double(prm->background_rgb[1]), double(prm->background_rgb[2])};
+  for (int py = 0; py < H; ++py)
+    for (int px = 0; px < W; ++px) {
+      size_t p = size_t(py) * W + px;
+      uint64_t G = f->gbuf[p * 2], A = f->gbuf[p * 2 + 1];
+      bool isCenter = G != EMPTY, isCons = A != EMPTY;
+      double C[3] = {0, 0, 0}, alpha = 0;
+      const double* CP = &f->colour[p * 3];
+      if (!prm->filter_on) {
+        if (isCenter) {
+          for (int c = 0; c < 3; ++c) C[c] = CP[c];
+          alpha = 1;
+        }
+      } else if (isCenter || isCons) {
+        const float* TG = &f->tang[p * 4];
+        const float* TA = &f->tang[p * 4 + 2];
+        if (isCenter) {
+          AccOut a = accumulate(f, prm, W, H, px, py, TG[0], TG[1], w_dq(G), true, CP, tauz_q);
+          for (int c = 0; c < 3; ++c) C[c] = a.C[c];
+          alpha = a.alpha;
+          // fly-away strand in front of the centre hit (R21)
+          if (isCons && w_dq(G) - w_dq(A) >= taufly_q && w_dq(G) >= w_dq(A)) {
+            AccOut b = accumulate(f, prm, W, H, px, py, TA[0], TA[1], w_dq(A), false, CP, tauz_q);
+            for (int c = 0; c < 3; ++c) C[c] = b.alpha * b.C[c] + (1 - b.alpha) * a.C[c];
+            alpha = 1;
+          }
+        } else {  // promoted pixel: w_color = 1
+          AccOut a = accumulate(f, prm, W, H, px, py, TA[0], TA[1], w_dq(A), false, CP, tauz_q);
+          for (int c = 0; c < 3; ++c) C[c] = a.C[c];
+          alpha = a.alpha;
+        }
+      }
+      for (int c = 0; c < 3; ++c) f->out[p * 4 + c] = alpha * C[c] + (1 - alpha) * bg[c];  // R29
+      f->out[p * 4 + 3] = alpha;
+    }
+  return 0;
+}
+void orc_frame_get_out(const orc_frame* f, double* o) {
+  std::memcpy(o, f->out.data(), f->out.size() * sizeof(double));
+}
+
+}  // extern "C"

@@ -1,0 +1,137 @@
+/* hair_oracle.h — C interface of the CPU ORACLE.
+ *
+ * TEST INFRASTRUCTURE ONLY. This is the plain, slow, single-threaded CPU
+ * restatement of what the deferred hair pipeline of arxiv/paper_2607_04230
+ * computes (§3.1-3.4, Eq. 1-5, Eq. 9-10, Code 1, Code 2), written from
+ * the paper and from the readings listed in DESIGN.md §3. Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may call it. It shares no code, header, table or helper with the CUDA library
+ * (include/hair.h, paper_2607_04230_b200/csrc); the struct layouts below are the
+ * oracle's own.
+ *
+ * Precision. Generation (O2), shading (O6) and the filter's weights (O7) are
+ * fp64. Every place where floating point decides an integer — LOD counts (O1),
+ * the two coverage predicates and the packed word (O4), the filter's sample
+ * classification (O7) — is fp32, one rounding per operation, no FMA contraction
+ * (built with -ffp-contract=off), in the operation order DESIGN.md §3 states,
+ * because the CUDA path takes the same decisions in fp32.
+ *
+ * Pins (tests/test_oracle_*.py): see DESIGN.md §4. Unpinned against the paper:
+ * the hash constants and the stand-in shading model (the paper prints neither).
+ */
+#ifndef HAIR_ORACLE_H
+#define HAIR_ORACLE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+  uint32_t spi, seed, op_mask, clump_exp, frizz_cells;
+  float clump_strength, twist_turns;
+  float curl_radius, curl_turns, curl_ramp_w0;
+  float frizz_sigma, frizz_ramp_w0;
+  float width_world;
+  float albedo_root[3], albedo_tip[3], roughness, tilt;
+} orc_style;
+
+typedef struct {
+  uint32_t n_verts, n_layers, n_tris, n_instances; /* n_instances >= 1 */
+  const float* pos;                /* [n_layers][n_verts][3] */
+  const float* ao;                 /* [n_layers][n_verts] or NULL (= 1) */
+  const uint32_t* idx;             /* [n_tris][3] */
+  const uint32_t* strands_per_tri; /* [n_tris] */
+  const float* xform;              /* [n_instances][12] row-major 3x4, or NULL (identity) */
+  orc_style style;
+} orc_groom;
+
+typedef struct {
+  float eye[3], right[3], up[3], forward[3];
+  float vfov_y, near_z, far_z;
+  uint32_t width, height;
+} orc_camera;
+
+typedef struct {
+  float center_diameter_px;
+  int32_t filter_radius;
+  float s_par, s_perp, sigma_c, tau_z, tau_fly, w_strip;
+  float light_pos[4][3], light_rgb[4][3];
+  uint32_t n_lights;
+  float ambient_rgb[3], k_d, k_R, k_TRT, background_rgb[3];
+  uint32_t filter_on;
+} orc_params;
+
+/* op_mask bits */
+#define ORC_OP_CLUMP 1u
+#define ORC_OP_TWIST 2u
+#define ORC_OP_CURL 4u
+#define ORC_OP_FRIZZ 8u
+
+typedef struct orc_frame orc_frame;
+
+/* ---- small pure functions (pins) ---- */
+uint32_t orc_pcg(uint32_t v);
+uint32_t orc_hash3(uint32_t seed, uint32_t id, uint32_t stream);
+/* Eq. 1 + Eq. 4-5 for one bundle given L: out[0]=N_LOD, out[1]=C_raw, out[2]=C */
+void orc_lod_counts(float L, uint32_t N, float delta, uint32_t n_layers, uint32_t c_full,
+                    uint32_t out[3]);
+void orc_calc_tangent(int idx, int count, const double prev[3], const double curr[3],
+                      const double next[3], double out[3]);
+uint64_t orc_pack(float zn, uint32_t sid, uint32_t j, float t);
+void orc_unpack(uint64_t w, uint32_t out[4]); /* dq, sid, j, t9 */
+/* coverage of ONE screen-space segment on a w x h grid: cover[y*w+x] bit0 = conservative,
+ * bit1 = centre; tq[y*w+x] = closest-point parameter t (fp32). */
+void orc_segment_cover(const float a[2], const float b[2], float rho, uint32_t w, uint32_t h,
+                       uint8_t* cover, float* tq);
+/* project one world point: out = sx, sy, zn, zv; returns valid */
+int orc_project(const orc_camera* cam, const float p[3], float out[4]);
+
+/* ---- frame pipeline ---- */
+orc_frame* orc_frame_create(void);
+void orc_frame_destroy(orc_frame*);
+int orc_frame_add_groom(orc_frame*, const orc_groom*); /* copies; returns groom id */
+
+/* O1 + scans. lambda: per groom (n_lambda = 1 broadcasts); <= 0 => LOD off. */
+int orc_frame_lod(orc_frame*, const orc_camera*, const float* lambda, uint32_t n_lambda);
+uint32_t orc_frame_n_bundles(const orc_frame*);      /* bundle-instances over all grooms */
+uint32_t orc_frame_n_strands_total(const orc_frame*);
+uint32_t orc_frame_n_strands(const orc_frame*);      /* after LOD */
+uint64_t orc_frame_n_vertices(const orc_frame*);
+/* table[gid] = {N_LOD, C, slot_base, vertex_base}; L[gid] = LOD selection value (-1 = culled/off) */
+void orc_frame_get_table(const orc_frame*, uint32_t* table4, float* L);
+/* replace the table (e.g. by the CUDA path's, for stage-wise parity). Recomputes nothing else. */
+int orc_frame_set_table(orc_frame*, const uint32_t* table4, uint32_t n);
+
+/* O2: vertices for the current table. fp64 result, and its fp32 rounding. */
+int orc_frame_generate(orc_frame*);
+void orc_frame_get_vertices_f64(const orc_frame*, double* xyz_ao);
+void orc_frame_get_vertices_f32(const orc_frame*, float* xyz_ao);
+int orc_frame_set_vertices_f32(orc_frame*, const float* xyz_ao, uint64_t n);
+/* one unstyled/styled strand in groom-local space, fp64, for closed-form pins:
+ * out[C][4] (x,y,z,ao), tan[C][3] base tangents (may be NULL) */
+int orc_strand(const orc_frame*, uint32_t groom, uint32_t id_local, uint32_t C, double* out,
+               double* base_tan);
+/* root barycentrics (fp64 exact multiples of 2^-24) and bundle of a strand */
+int orc_root(const orc_frame*, uint32_t groom, uint32_t id_local, double b[3], uint32_t* tri);
+
+/* O4: raster the current fp32 vertices with the current table. gbuffer [H][W][2] (0 = centre, 1 = cons).
+ * order: optional permutation of strand slots (NULL = natural) — result must not depend on it.
+ * counts[0] = centre atomics (predicate-true hits), counts[1] = conservative, counts[2] = segments
+ * with both endpoints valid. */
+int orc_frame_raster(orc_frame*, const orc_camera*, const orc_params*, const uint32_t* order,
+                     uint64_t counts[3]);
+void orc_frame_get_gbuffer(const orc_frame*, uint64_t* out);
+int orc_frame_set_gbuffer(orc_frame*, const uint64_t* in, uint32_t w, uint32_t h);
+
+/* O6: colour[H][W][3] fp64 (0 where no centre hit); tangents[H][W][4] fp32 = (T_G.xy, T_A.xy) */
+int orc_frame_shade(orc_frame*, const orc_camera*, const orc_params*);
+void orc_frame_get_colour(const orc_frame*, double* rgb);
+void orc_frame_get_tangents(const orc_frame*, float* t4);
+/* O7: out[H][W][4] fp64 (rgb premultiplied-composited over background, alpha) */
+int orc_frame_filter(orc_frame*, const orc_camera*, const orc_params*);
+void orc_frame_get_out(const orc_frame*, double* rgba);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
