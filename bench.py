@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py — frame throughput of the deferred hair pipeline on the north-star workload.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl reference]
+
+A "step" is one frame = one pass of the whole hot path (LOD -> scan -> generate -> clear + raster
+-> shade -> filter) over BASELINE.json configs[3]: the five-groom scene, 483 000 strands,
+3840x2160, 1 spp, per-groom LOD lambda {4.0, 5.5, 2.0, 2.8, 3.0} (synthetic, seeded).
+`value` = segments rasterised per second (whole job); `ms_per_step` = frame ms.
+N > 1 = N independent replicas of the same frame ("replicas only": north_star excludes sharding).
+
+Prints ONE JSON line. `--impl reference` times the CPU oracle instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "Gsegments/s at 4K, 483k strands (frame ms = ms_per_step)"
+UNIT = "Gsegments/s"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-i", str(index), "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL,
+                                      text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def scene_for(args):
+    from paper_2607_04230_b200 import synth
+    return synth.config(args.config, scale=args.scale, res_scale=args.res_scale)
+
+
+# ------------------------------------------------------------------------------- oracle legs
+def oracle_sample(config: int, scale: float, res_scale: float):
+    """One oracle frame (all of O1-O7) on a bounded sample; returns (seconds, segments, description)."""
+    import oracle
+    from paper_2607_04230_b200 import synth
+    sc = synth.config(config, scale=scale, res_scale=res_scale)
+    f = oracle.Frame(sc["grooms"])
+    t0 = time.perf_counter()
+    f.lod(sc["camera"], sc["lam"])
+    f.generate()
+    cnt = f.raster(sc["camera"], sc["params"])
+    f.shade(sc["camera"], sc["params"])
+    f.filter(sc["camera"], sc["params"])
+    dt = time.perf_counter() - t0
+    n_seg = int(f.n_vertices - f.n_strands)
+    desc = (f"config {config} with strand counts x{scale} ({synth.n_strands(sc)} strands, {f.n_strands} after LOD, "
+            f"{n_seg} segments) at {sc['camera']['width']}x{sc['camera']['height']}, one full frame O1-O7")
+    return dt, n_seg, desc, cnt
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, single-threaded, on a bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    scale, res_scale = 0.02, 0.5
+    for _ in range(args.warmup):
+        oracle_sample(args.config, scale, res_scale)
+    t, seg, desc = 0.0, 0, ""
+    for _ in range(args.steps):
+        dt, n_seg, desc, _ = oracle_sample(args.config, scale, res_scale)
+        t += dt
+        seg += n_seg
+    val = seg / t / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64/f32",
+            "data": "synthetic", "config": {"workload": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------- CUDA arm
+def run_cuda(args):
+    import numpy as np
+    import torch
+    from paper_2607_04230_b200 import binding, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+
+    sc = scene_for(args)
+    cam, lam = sc["camera"], sc["lam"]
+    W, H = cam["width"], cam["height"]
+    h = binding.Hair(local_rank)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    gb, rgb = h.alloc_outputs(W, H)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- algorithmic counts of the frame (untimed, instrumented kernels)
+    h.set_render_params(sc["params"], flags=binding.FLAG_COUNTERS)
+    h.render(cam, lam, gb, rgb)
+    cnt = h.stats()
+
+    # ---- device-resident timing: K frames, one event pair, stage events inside the library
+    h.set_render_params(sc["params"], flags=binding.FLAG_STAGE_TIMING)
+    for _ in range(max(args.warmup, 3)):
+        h.render(cam, lam, gb, rgb)
+    h.stats()  # drain the warm-up stage timings
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        h.render(cam, lam, gb, rgb)
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    st = h.stats()  # stage means over the timed frames
+    if dist is not None:
+        t = torch.tensor([ms_total], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    n_seg = cnt["n_segments"]
+    value = world * n_seg / (ms_step * 1e-3) / 1e9
+
+    # ---- end to end through the C ABI with HOST buffers: cage upload (pinned) + render + D2H of out_rgb
+    h.set_render_params(sc["params"], flags=0)
+    host_rgb = torch.empty((H, W, 4), dtype=torch.float32).pin_memory()
+    pinned = [(torch.from_numpy(np.ascontiguousarray(g["pos"])).pin_memory(),
+               None if g["ao"] is None else torch.from_numpy(np.ascontiguousarray(g["ao"])).pin_memory())
+              for g in sc["grooms"]]
+    h2d = sum(p.numel() * 4 + (0 if a is None else a.numel() * 4) for p, a in pinned)
+    d2h = host_rgb.numel() * 4
+
+    def e2e_step():
+        for gi, (p, a) in enumerate(pinned):
+            h.mesh_update(gi, p, a)
+        h.render_to_host(cam, lam, host_rgb)
+
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    k_e2e = max(3, min(args.steps, 10))
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(k_e2e):
+        e2e_step()
+    e1.record()
+    barrier()
+    ms_e2e = max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0)) / k_e2e
+    if dist is not None:
+        t = torch.tensor([ms_e2e], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    e2e_val = world * n_seg / (ms_e2e * 1e-3) / 1e9
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- rooflines: algorithmic work per launch / measured stage time
+    hbm_peak, hbm_src = peaks()
+    words = torch.empty(W * H * 2, dtype=torch.int64, device=dev)
+    n_ops = 1 << 28
+    atom = {}
+    for mode, name in ((0, "unique"), (1, "random"), (2, "hot1024")):
+        h.atomic_microbench(mode, words, 1 << 24, 1024)  # warm
+        ms = min(h.atomic_microbench(mode, words, n_ops, 1024) for _ in range(3))
+        atom[name] = n_ops / (ms * 1e-3) / 1e9
+    del words
+    n_px = W * H
+    n_at = cnt["n_atomics_center"] + cnt["n_atomics_cons"]
+    stages = {
+        "generate": {"bound": "hbm", "ms": st["ms_generate"], "bytes": 16 * cnt["n_vertices"]},
+        "clear": {"bound": "hbm", "ms": st["ms_clear"], "bytes": 16 * n_px},
+        "raster": {"bound": "l2_atomic", "ms": st["ms_raster"], "atomics": n_at, "bytes": 16 * cnt["n_vertices"] + 8 * n_at},
+        "shade": {"bound": "hbm", "ms": st["ms_shade"], "bytes": 16 * n_px + (16 + 64) * cnt["n_pixels_center"]},
+        "filter": {"bound": "hbm", "ms": st["ms_filter"], "bytes": 32 * n_px + 16 * cnt["n_pixels_center"]},
+    }
+    for k, s in stages.items():
+        if s["ms"] > 0:
+            s["GBps"] = s["bytes"] / (s["ms"] * 1e-3) / 1e9
+            s["frac_hbm"] = s["GBps"] / hbm_peak
+            if "atomics" in s:
+                s["Gatom_per_s"] = s["atomics"] / (s["ms"] * 1e-3) / 1e9
+                s["frac_l2_atomic_random"] = s["Gatom_per_s"] / atom["random"]
+    stages["lod_scan"] = {"bound": "latency", "ms": st["ms_lod"]}
+    dom = max(("generate", "clear", "raster", "shade", "filter"), key=lambda k: stages[k]["ms"])
+    d = stages[dom]
+    if dom == "raster":
+        roofline = {"kernel": "k_raster", "bound": "l2_atomic", "achieved": d["Gatom_per_s"], "peak": atom["random"],
+                    "unit": "Gatom/s", "frac": d["frac_l2_atomic_random"], "traffic": None,
+                    "peak_source": "hair_atomic_microbench mode 1 (random 64-bit RED.MIN over a G-buffer-sized "
+                                   "buffer), measured live in this run",
+                    "algorithmic": f"{n_at} predicate-true hits (centre + conservative) per frame"}
+    else:
+        roofline = {"kernel": "k_" + dom, "bound": "hbm", "achieved": d["GBps"], "peak": hbm_peak, "unit": "GB/s",
+                    "frac": d["frac_hbm"], "traffic": None, "peak_source": hbm_src,
+                    "algorithmic": f"{d['bytes']} bytes per frame"}
+
+    # ---- the oracle timed beside it on this box's host cores (bounded sample of the same workload)
+    cpu_baseline = None
+    if not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        dt, seg, desc, _ = oracle_sample(args.config, args.cpu_scale, 1.0 if args.res_scale == 1.0 else args.res_scale)
+        cpu_baseline = {"value": seg / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
+                        "seconds": dt, "host_cores_available": os.cpu_count()}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": f"BASELINE configs[{args.config - 1}] '{sc['name']}': {synth.n_strands(sc)} strands, "
+                               f"{len(sc['grooms'])} grooms, {W}x{H}, 1 spp, lod_lambda {list(lam)}",
+                   "strands_after_lod": cnt["n_strands_lod"], "vertices": cnt["n_vertices"], "segments": n_seg,
+                   "l2": "no flush: per-frame working set (G-buffer 16 B/px + colour + out_rgb + vertices = "
+                         f"{(48 * n_px + 16 * cnt['n_vertices']) / 1e6:.0f} MB) exceeds the 126 MB L2",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "frame_ms": ms_step, "strands_per_s": world * cnt["n_strands_lod"] / (ms_step * 1e-3),
+        "segments_per_s": world * n_seg / (ms_step * 1e-3),
+        "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": ms_e2e, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "what": "hair_mesh_update (pinned cage) + hair_render_to_host (out_rgb to pinned host)"},
+        "gpu_launches": st["gpu_launches"] * args.steps,
+        "roofline": roofline, "stages": stages, "l2_atomic_peaks_Gatom_per_s": atom,
+        "hbm_peak_GBps": hbm_peak, "hbm_peak_source": hbm_src,
+        "counts": {k: cnt[k] for k in ("n_bundles", "n_bundles_culled", "n_strands_total", "n_strands_lod", "n_vertices",
+                                       "n_segments", "n_segments_drawn", "n_atomics_center", "n_atomics_cons",
+                                       "n_atomics_issued", "n_pixels_center", "n_pixels_cons")},
+        "cpu_baseline": cpu_baseline, "clocks": clocks,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); 4 = the metric's workload")
+    ap.add_argument("--scale", type=float, default=1.0, help="strand-count multiplier (1.0 = as named)")
+    ap.add_argument("--res-scale", type=float, default=1.0, dest="res_scale")
+    ap.add_argument("--cpu-scale", type=float, default=0.1, dest="cpu_scale",
+                    help="strand-count multiplier of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

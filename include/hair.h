@@ -1,0 +1,172 @@
+/* hair.h — C ABI of libhair: the deferred hair pipeline of arxiv/paper_2607_04230 on one B200.
+ *
+ * The calls follow the paper's statement of the problem (Fig. 2, §3):
+ * inputs are a hair mesh (cage of prism layers + root triangles), a styling function
+ * and a camera; outputs are the 64-bit compressed G-buffer and the
+ * filtered, alpha-composited colour. Everything between runs in hand-written
+ * CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *  - Every function returns HAIR_OK (0) or a negative HAIR_E_* code; hair_last_error() gives text.
+ *  - "host" pointers are read during the call and may be freed after it returns (the library
+ *    copies). "DEVICE" pointers are caller-owned CUDA allocations on the context's device.
+ *  - All work is enqueued on the CUDA stream given to hair_create (the caller's, e.g. torch's
+ *    current stream). hair_render never synchronises and reads no device result back.
+ *  - A context is not thread-safe. No global state.
+ *  - Arithmetic contract (operation order of the fp32 decisions, bit layout): DESIGN.md §3.
+ */
+#ifndef HAIR_H
+#define HAIR_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HAIR_OK 0
+#define HAIR_E_INVALID_ARG (-1)
+#define HAIR_E_CUDA (-2)
+#define HAIR_E_OUT_OF_MEMORY (-3)
+#define HAIR_E_TOO_MANY_STRANDS (-4) /* sum of strands x instances >= 2^24 (24-bit strand id) */
+#define HAIR_E_TOO_MANY_CPS (-5)     /* C_full = (n_layers-1)*spi + 1 > 127 (7-bit segment index) */
+#define HAIR_E_TOO_MANY_GROOMS (-6)  /* > HAIR_MAX_GROOMS */
+#define HAIR_MAX_GROOMS 16
+#define HAIR_MAX_LIGHTS 4
+
+/* styling operators, applied in this order (R24) */
+#define HAIR_OP_CLUMP 1u
+#define HAIR_OP_TWIST 2u
+#define HAIR_OP_CURL 4u
+#define HAIR_OP_FRIZZ 8u
+
+/* render flags */
+#define HAIR_FLAG_FILTER 1u       /* run the reconstruction filter; else pass centre colour */
+#define HAIR_FLAG_COUNTERS 2u     /* count predicate-true hits (algorithmic atomics) in hair_stats; slower */
+#define HAIR_FLAG_STAGE_TIMING 4u /* record CUDA events around each stage for hair_stats.ms_* */
+
+typedef struct hair_ctx hair_ctx; /* opaque; owns all device scratch */
+
+/* Creates a context on `cuda_device` that enqueues on `cuda_stream` (a cudaStream_t; NULL = the
+ * legacy default stream). The stream stays owned by the caller and must outlive the context. */
+int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream);
+void hair_destroy(hair_ctx*);
+const char* hair_last_error(const hair_ctx*);
+
+/* Hair mesh: bundles = triangular prisms over root triangles (R1). */
+typedef struct {
+  uint32_t n_verts;  /* cage vertices per layer */
+  uint32_t n_layers; /* Lv: vertex layers, root layer first, tip last; 2 <= Lv <= 32 */
+  const float* pos;  /* host, [n_layers][n_verts][3], groom-local space */
+  const float* ao;   /* host, [n_layers][n_verts] baked ambient occlusion, or NULL (= 1) */
+} hair_cage;
+
+typedef struct {
+  uint32_t n_tris;                 /* bundles */
+  const uint32_t* idx;             /* host, [n_tris][3] indices into n_verts */
+  const uint32_t* strands_per_tri; /* host, [n_tris]: N of Eq. 1 per bundle */
+} hair_roots;
+
+typedef struct {
+  uint32_t spi;  /* control points per layer interval: C_full = (Lv-1)*spi + 1 */
+  uint32_t seed; /* hash seed (R26) */
+  uint32_t op_mask, clump_exp, frizz_cells;
+  float clump_strength, twist_turns;
+  float curl_radius, curl_turns, curl_ramp_w0;
+  float frizz_sigma, frizz_ramp_w0;
+  float width_world; /* > 0: centre radius from projected width (R9); 0: center_diameter_px */
+  float albedo_root[3], albedo_tip[3], roughness, tilt;
+  uint32_t n_instances;        /* >= 1 */
+  const float* instance_xform; /* host, [n_instances][12] row-major 3x4 [R|t], or NULL = identity */
+} hair_style;
+
+/* Appends a groom. Copies everything to the device (synchronously) and sizes the scratch buffers
+ * for the worst case (LOD off). Strand ids are assigned in upload order (DESIGN.md §3 "sid"). */
+int hair_mesh_upload(hair_ctx*, const hair_cage*, const hair_roots*, const hair_style*, int* out_groom_id);
+/* Replaces positions / AO of an uploaded groom (animated cage). Same sizes. The copy
+ * is enqueued on the context's stream from the caller's (ideally pinned) host memory. */
+int hair_mesh_update(hair_ctx*, int groom_id, const hair_cage*);
+/* Removes all grooms (buffers are kept). */
+int hair_mesh_clear(hair_ctx*);
+
+typedef struct {
+  float eye[3], right[3], up[3], forward[3]; /* orthonormal; +forward = increasing depth */
+  float vfov_y, near_z, far_z;               /* radians; depth range of the 24-bit depth */
+} hair_camera;
+
+typedef struct {
+  float center_diameter_px; /* PAPER.md:74 "configurable diameter"; default 0.5 */
+  int32_t filter_radius;    /* r of PAPER.md:160; 0..7, default 5 */
+  float s_par, s_perp;      /* sigma_par = r*s_par, sigma_perp = r*s_perp */
+  float sigma_c;            /* 0.9 */
+  float tau_z, tau_fly;     /* 1.45e-3, 5e-4 in normalised depth */
+  float w_strip;            /* 0.5 px */
+  float light_pos[HAIR_MAX_LIGHTS][3], light_rgb[HAIR_MAX_LIGHTS][3];
+  uint32_t n_lights;
+  float ambient_rgb[3], k_d, k_R, k_TRT, background_rgb[3];
+  uint32_t flags; /* HAIR_FLAG_* */
+} hair_render_params;
+
+void hair_default_render_params(hair_render_params* out);
+int hair_set_render_params(hair_ctx*, const hair_render_params*);
+
+/* One frame: LOD -> scan -> generate -> clear+raster -> shade -> filter, all on the stream.
+ *  lod_lambda  host, per groom (n_lambda == n_grooms) or one value for all (n_lambda == 1);
+ *              <= 0 switches LOD and culling off for that groom (R14)
+ *  out_gbuffer DEVICE, [height][width][2] uint64, 16-byte aligned: [..][0] centre-sample layer,
+ *              [..][1] conservative layer; word = depth24|strand24|segment7|t9,
+ *              empty = all ones. Cleared by the call.
+ *  out_rgb     DEVICE, [height][width][4] float, 16-byte aligned: linear rgb composited over the
+ *              background, alpha in .w (R29). */
+int hair_render(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height, const float* lod_lambda,
+                uint32_t n_lambda, uint64_t* out_gbuffer, float* out_rgb);
+
+/* Same frame, results copied to HOST memory (pinned for full speed) inside the call:
+ * host_rgb [h][w][4] float is required, host_gbuffer [h][w][2] may be NULL. Synchronises the stream. */
+int hair_render_to_host(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height,
+                        const float* lod_lambda, uint32_t n_lambda, uint64_t* host_gbuffer, float* host_rgb);
+
+typedef struct {
+  uint32_t n_grooms, n_bundles, n_bundles_culled;
+  uint32_t n_strands_total, n_strands_lod;
+  uint32_t n_vertices, n_segments;
+  uint32_t n_segments_drawn;               /* both endpoints in front of the near plane (counters flag) */
+  uint64_t n_atomics_center, n_atomics_cons; /* predicate-true hits before any filtering (counters flag) */
+  uint64_t n_atomics_issued;               /* atomics actually sent to L2 (counters flag) */
+  uint32_t n_pixels_center, n_pixels_cons; /* non-empty pixels after the frame (counters flag) */
+  /* stage-timing flag: mean over the frames rendered since the previous hair_stats (last 64 at most) */
+  float ms_lod, ms_generate, ms_clear, ms_raster, ms_shade, ms_filter, ms_total;
+  uint32_t n_timed_frames;
+  float beta_mean; /* N_remaining / N_total of Eq. 8 over all grooms */
+  uint32_t gpu_launches; /* kernels launched by the last hair_render */
+} hair_stats_t;
+/* Synchronises the stream and reads the device counters of the last frame. */
+int hair_stats(hair_ctx*, hair_stats_t* out);
+
+/* Debug / parity access to the intermediates of the last frame (DEVICE pointers, owned by the context):
+ * vertices float4[n_vertices] = (x, y, z, ao); table uint4[n_bundles] = {N_LOD, C, slot_base,
+ * vertex_base}; colour float4[h][w] = shaded rgb of centre-hit pixels (undefined elsewhere). */
+int hair_debug_buffers(hair_ctx*, const float** dev_vertices, const uint32_t** dev_table, const float** dev_colour);
+/* Stage-wise parity: run only H4..H7 of a frame on caller-supplied intermediates.
+ *  stage_mask bit0 = clear+raster (from the context's vertex buffer), bit1 = shade, bit2 = filter.
+ *  If bit0 is clear, out_gbuffer is taken as input. */
+int hair_render_stages(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height, uint32_t stage_mask,
+                       uint64_t* out_gbuffer, float* out_rgb);
+/* Overwrites the context's vertex buffer of the last frame (DEVICE src, n float4) — lets a test feed
+ * the raster with vertices of its choice. n must equal the last frame's n_vertices. */
+int hair_debug_set_vertices(hair_ctx*, const float* dev_src, uint32_t n);
+
+/* L2-atomic roofline denominators: 64-bit atomicMin (RED.MIN.64) micro-kernels over a
+ * DEVICE buffer of n_words uint64.
+ *  mode 0: each thread its own word, coalesced;  mode 1: hashed uniformly random word per op;
+ *  mode 2: all ops into `hot_words` words (contention floor).
+ * Enqueues `n_ops` atomics; returns the elapsed milliseconds (CUDA events; synchronises). */
+int hair_atomic_microbench(hair_ctx*, int mode, uint64_t* dev_words, uint64_t n_words, uint64_t n_ops,
+                           uint32_t hot_words, float* out_ms);
+
+/* sizeof of {hair_cage, hair_roots, hair_style, hair_camera, hair_render_params, hair_stats_t}, so a
+ * foreign-language binding can check its struct layouts without a GPU. */
+void hair_abi_sizes(uint32_t out[6]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -293,11 +293,13 @@ uint32_t tri_of(const Groom& g, uint32_t id_local) {
   return uint32_t(std::upper_bound(g.off.begin(), g.off.end(), id_local) - g.off.begin()) - 1u;
 }
 
-// frizz lattice value (R24): four hashed uniforms, variance 1, no transcendental
+// frizz lattice value (R24): one hash per (node, channel); the sum of its four bytes is a discrete
+// Irwin-Hall(4) variable with mean 510 and variance 4*(256^2-1)/12 = 21845: unit variance, no
+// transcendental.
 double frizz_lattice(const Groom& g, uint32_t id_local, uint32_t n, uint32_t ch) {
-  double s = 0;
-  for (uint32_t q = 0; q < 4; ++q) s += u01(hash3(g.st.seed, id_local, ST_FRIZZ + 8u * n + 4u * ch + q));
-  return (s - 2.0) * std::sqrt(3.0);
+  uint32_t h = hash3(g.st.seed, id_local, ST_FRIZZ + 2u * n + ch);
+  uint32_t s = (h & 255u) + ((h >> 8) & 255u) + ((h >> 16) & 255u) + (h >> 24);
+  return (double(s) - 510.0) / std::sqrt(21845.0);
 }
 
 // one strand, groom-local space, C control points: out[C][4], base_tan[C][3]
@@ -355,9 +357,10 @@ void strand_local(const Groom& g, uint32_t id_local, uint32_t C, double* out, do
     }
     if (st.op_mask & ORC_OP_FRIZZ) {
       uint32_t cells = std::max(st.frizz_cells, 1u);
-      double x = w * double(cells);
-      uint32_t c0 = std::min(uint32_t(std::floor(x)), cells - 1u);
-      double fr = x - double(c0);
+      // x = w*cells = (j*cells)/(C-1), cell index and fraction in integers (exact)
+      uint32_t xn = j * cells, den = C - 1;
+      uint32_t c0 = std::min(xn / den, cells - 1u);
+      double fr = double(xn - c0 * den) / double(den);
       double s = fr * fr * (3.0 - 2.0 * fr);
       double n0 = (1 - s) * frizz_lattice(g, id_local, c0, 0) + s * frizz_lattice(g, id_local, c0 + 1, 0);
       double n1 = (1 - s) * frizz_lattice(g, id_local, c0, 1) + s * frizz_lattice(g, id_local, c0 + 1, 1);

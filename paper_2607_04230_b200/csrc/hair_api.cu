@@ -1,0 +1,565 @@
+// hair_api.cu — host side of libhair: the C ABI of include/hair.h, the frame scheduler and
+// device-buffer ownership. No torch, no exceptions across the boundary.
+//
+// hair_render enqueues a fixed kernel sequence on the caller's stream:
+//   k_lod -> k_scan -> k_generate -> k_clear -> k_raster -> k_shade -> k_filter
+// Grid sizes never depend on device results: the LOD-dependent stages are persistent kernels
+// that read their work counts from device memory (the CUDA form of the paper's indirect
+// dispatch), so no stage waits for the host.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "hair_internal.cuh"
+
+namespace {
+
+struct GroomHost {
+  float *pos = nullptr, *ao = nullptr, *xform = nullptr;
+  uint32_t *idx = nullptr, *npt = nullptr, *off = nullptr;
+  size_t pos_bytes = 0, ao_bytes = 0;
+};
+
+enum { EV_BEGIN = 0, EV_LOD, EV_GEN, EV_CLEAR, EV_RASTER, EV_SHADE, EV_FILTER, EV_N };
+const int EV_RING = 64;  // stage timings of up to 64 frames are averaged by hair_stats without a sync in between
+
+}  // namespace
+
+struct hair_ctx {
+  int device = 0;
+  int n_sm = 148;
+  cudaStream_t stream = nullptr;
+  std::string err;
+  SceneDev scene;  // host mirror
+  SceneDev* d_scene = nullptr;
+  bool scene_dirty = true;
+  std::vector<GroomHost> grooms;
+  hair_render_params prm;
+  // scratch
+  uint4* d_table = nullptr;
+  size_t table_cap = 0;
+  float4* d_vertices = nullptr;
+  size_t vertex_cap = 0;
+  size_t vertex_need = 0;
+  float4* d_colour = nullptr;
+  size_t colour_cap = 0;
+  unsigned long long* d_counters = nullptr;
+  unsigned long long* h_counters = nullptr;  // pinned
+  uint32_t c_max = 0;
+  // owned outputs for hair_render_to_host
+  unsigned long long* d_own_gbuf = nullptr;
+  float* d_own_rgb = nullptr;
+  size_t own_px = 0;
+  cudaEvent_t ev[EV_RING][EV_N] = {};
+  uint32_t ev_frames = 0;  // timed frames since the last hair_stats
+  bool timed = false, counted = false;
+  uint32_t last_w = 0, last_h = 0, launches = 0;
+  CamDev last_cam;
+};
+
+namespace {
+
+int fail(hair_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+#define CK(call)                                                                                  \
+  do {                                                                                            \
+    cudaError_t e_ = (call);                                                                      \
+    if (e_ != cudaSuccess)                                                                        \
+      return fail(c, e_ == cudaErrorMemoryAllocation ? HAIR_E_OUT_OF_MEMORY : HAIR_E_CUDA,        \
+                  std::string(#call) + ": " + cudaGetErrorString(e_));                            \
+  } while (0)
+
+uint32_t pcg_host(uint32_t v) {
+  uint32_t s = v * 747796405u + 2891336453u;
+  uint32_t w = ((s >> ((s >> 28) + 4u)) ^ s) * 277803737u;
+  return (w >> 22) ^ w;
+}
+
+CamDev make_cam(const hair_camera* cam, uint32_t w, uint32_t h) {
+  CamDev k;
+  for (int i = 0; i < 3; ++i) {
+    k.eye[i] = cam->eye[i];
+    k.r[i] = cam->right[i];
+    k.u[i] = cam->up[i];
+    k.f[i] = cam->forward[i];
+  }
+  k.near_z = cam->near_z;
+  k.W = w;
+  k.H = h;
+  // R-proj: constants in double, rounded once to float
+  double fpx = (0.5 * (double)h) / std::tan(0.5 * (double)cam->vfov_y);
+  double fn = (double)cam->far_z - (double)cam->near_z;
+  k.fpx = (float)fpx;
+  k.A = (float)((double)cam->far_z / fn);
+  k.B = (float)((double)cam->far_z * (double)cam->near_z / fn);
+  k.half_w = 0.5f * (float)w;
+  k.half_h = 0.5f * (float)h;
+  return k;
+}
+
+ShadeParams make_shade(const hair_render_params& p) {
+  ShadeParams s;
+  memset(&s, 0, sizeof(s));
+  memcpy(s.light_pos, p.light_pos, sizeof(s.light_pos));
+  memcpy(s.light_rgb, p.light_rgb, sizeof(s.light_rgb));
+  s.n_lights = p.n_lights > HAIR_MAX_LIGHTS ? HAIR_MAX_LIGHTS : p.n_lights;
+  for (int i = 0; i < 3; ++i) {
+    s.ambient[i] = p.ambient_rgb[i];
+    s.background[i] = p.background_rgb[i];
+  }
+  s.k_d = p.k_d;
+  s.k_R = p.k_R;
+  s.k_TRT = p.k_TRT;
+  s.r = p.filter_radius;
+  double sp = (double)p.filter_radius * (double)p.s_par, sq = (double)p.filter_radius * (double)p.s_perp;
+  s.inv_sp2 = sp > 0 ? (float)(1.0 / (sp * sp)) : 0.f;
+  s.inv_sq2 = sq > 0 ? (float)(1.0 / (sq * sq)) : 0.f;
+  s.inv_sc2 = (float)(1.0 / ((double)p.sigma_c * (double)p.sigma_c));
+  s.w_strip = p.w_strip;
+  s.tauz_q = (uint32_t)std::floor((double)p.tau_z * 16777215.0 + 0.5);    // R20: integer thresholds
+  s.taufly_q = (uint32_t)std::floor((double)p.tau_fly * 16777215.0 + 0.5);
+  s.filter_on = (p.flags & HAIR_FLAG_FILTER) ? 1u : 0u;
+  s.rho_default = 0.5f * p.center_diameter_px;
+  return s;
+}
+
+template <class T>
+int upload(hair_ctx* c, T** dst, const T* src, size_t n) {
+  CK(cudaMalloc((void**)dst, n * sizeof(T)));
+  CK(cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice));
+  return HAIR_OK;
+}
+
+void free_groom(GroomHost& g) {
+  cudaFree(g.pos);
+  cudaFree(g.ao);
+  cudaFree(g.xform);
+  cudaFree(g.idx);
+  cudaFree(g.npt);
+  cudaFree(g.off);
+  g = GroomHost();
+}
+
+int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
+  if (c->scene.n_bi > c->table_cap) {
+    cudaFree(c->d_table);
+    c->d_table = nullptr;
+    CK(cudaMalloc((void**)&c->d_table, (size_t)c->scene.n_bi * sizeof(uint4)));
+    c->table_cap = c->scene.n_bi;
+  }
+  if (c->vertex_need > c->vertex_cap) {
+    cudaFree(c->d_vertices);
+    c->d_vertices = nullptr;
+    CK(cudaMalloc((void**)&c->d_vertices, (c->vertex_need + 32) * sizeof(float4)));
+    c->vertex_cap = c->vertex_need;
+  }
+  size_t px = (size_t)w * h;
+  if (px > c->colour_cap) {
+    cudaFree(c->d_colour);
+    c->d_colour = nullptr;
+    CK(cudaMalloc((void**)&c->d_colour, px * sizeof(float4)));
+    c->colour_cap = px;
+  }
+  if (c->scene_dirty) {
+    CK(cudaMemcpyAsync(c->d_scene, &c->scene, sizeof(SceneDev), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));  // host mirror may change after return
+    c->scene_dirty = false;
+  }
+  return HAIR_OK;
+}
+
+int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
+                uint32_t stage_mask, bool front, unsigned long long* gbuf, float* rgb) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  if (!cam || !gbuf || !rgb || w == 0 || h == 0 || w > 16384 || h > 16384)
+    return fail(c, HAIR_E_INVALID_ARG, "hair_render: null argument or bad resolution");
+  if (((uintptr_t)gbuf & 15) || ((uintptr_t)rgb & 15))
+    return fail(c, HAIR_E_INVALID_ARG, "hair_render: outputs must be 16-byte aligned");
+  if (!(cam->far_z > cam->near_z) || !(cam->near_z > 0.f) || !(cam->vfov_y > 0.f))
+    return fail(c, HAIR_E_INVALID_ARG, "hair_render: bad camera");
+  if (front && !(n_lam == 1 || n_lam == c->scene.n_grooms || (n_lam == 0 && lam == nullptr)))
+    return fail(c, HAIR_E_INVALID_ARG, "hair_render: n_lambda must be 0, 1 or the number of grooms");
+  CK(cudaSetDevice(c->device));
+  int rc = ensure_scratch(c, w, h);
+  if (rc) return rc;
+  const CamDev k = make_cam(cam, w, h);
+  const ShadeParams sp = make_shade(c->prm);
+  const bool timed = (c->prm.flags & HAIR_FLAG_STAGE_TIMING) != 0;
+  const bool count = (c->prm.flags & HAIR_FLAG_COUNTERS) != 0;
+  const uint32_t n_bi = c->scene.n_bi;
+  cudaStream_t st = c->stream;
+  uint32_t launches = 0;
+  cudaEvent_t* evs = c->ev[c->ev_frames % EV_RING];
+  auto mark = [&](int e) {
+    if (timed) cudaEventRecord(evs[e], st);
+  };
+  mark(EV_BEGIN);
+  if (front && !n_bi) CK(cudaMemsetAsync(c->d_counters, 0, CNT_N * sizeof(unsigned long long), st));
+  if (front && n_bi) {
+    LambdaArr la;
+    for (uint32_t i = 0; i < HAIR_MAX_GROOMS; ++i) la.v[i] = n_lam == 0 ? 0.f : lam[n_lam == 1 ? 0 : (i < n_lam ? i : 0)];
+    launch_lod_scan(c->d_scene, n_bi, k, la, c->d_table, c->d_counters, st);
+    launches += 2;
+  }
+  mark(EV_LOD);
+  if (front && n_bi) {
+    launch_generate(c->d_scene, n_bi, c->d_table, c->d_vertices, c->d_counters, c->c_max, c->n_sm, st);
+    ++launches;
+  }
+  mark(EV_GEN);
+  if (stage_mask & 1u) {
+    launch_clear(gbuf, (size_t)w * h, st);
+    ++launches;
+  }
+  mark(EV_CLEAR);
+  if ((stage_mask & 1u) && n_bi) {
+    if (!front) CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER, 0, sizeof(unsigned long long), st));
+    launch_raster(c->d_scene, n_bi, c->d_table, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters, count,
+                  c->n_sm, st);
+    ++launches;
+  }
+  mark(EV_RASTER);
+  if (stage_mask & 2u) {
+    launch_shade(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour, st);
+    ++launches;
+  }
+  mark(EV_SHADE);
+  if (stage_mask & 4u) {
+    launch_filter(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour, (float4*)rgb, c->d_counters,
+                  count, st);
+    ++launches;
+  }
+  mark(EV_FILTER);
+  CK(cudaGetLastError());
+  c->timed = timed;
+  if (timed) ++c->ev_frames;
+  c->counted = count;
+  c->last_w = w;
+  c->last_h = h;
+  c->launches = launches;
+  c->last_cam = k;
+  return HAIR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream) {
+  if (!out) return HAIR_E_INVALID_ARG;
+  *out = nullptr;
+  int n = 0;
+  if (cudaGetDeviceCount(&n) != cudaSuccess || cuda_device < 0 || cuda_device >= n) return HAIR_E_CUDA;
+  hair_ctx* c = new hair_ctx();
+  c->device = cuda_device;
+  c->stream = (cudaStream_t)cuda_stream;
+  memset(&c->scene, 0, sizeof(c->scene));
+  hair_default_render_params(&c->prm);
+  bool ok = cudaSetDevice(cuda_device) == cudaSuccess &&
+            cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, cuda_device) == cudaSuccess &&
+            cudaMalloc((void**)&c->d_scene, sizeof(SceneDev)) == cudaSuccess &&
+            cudaMalloc((void**)&c->d_counters, CNT_N * sizeof(unsigned long long)) == cudaSuccess &&
+            cudaMemset(c->d_counters, 0, CNT_N * sizeof(unsigned long long)) == cudaSuccess &&
+            cudaMallocHost((void**)&c->h_counters, CNT_N * sizeof(unsigned long long)) == cudaSuccess;
+  for (int f = 0; ok && f < EV_RING; ++f)
+    for (int i = 0; ok && i < EV_N; ++i) ok = cudaEventCreate(&c->ev[f][i]) == cudaSuccess;
+  if (!ok) {
+    hair_destroy(c);
+    return HAIR_E_CUDA;
+  }
+  *out = c;
+  return HAIR_OK;
+}
+
+void hair_destroy(hair_ctx* c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  if (c->stream || true) cudaStreamSynchronize(c->stream);
+  for (auto& g : c->grooms) free_groom(g);
+  cudaFree(c->d_scene);
+  cudaFree(c->d_table);
+  cudaFree(c->d_vertices);
+  cudaFree(c->d_colour);
+  cudaFree(c->d_counters);
+  cudaFree(c->d_own_gbuf);
+  cudaFree(c->d_own_rgb);
+  if (c->h_counters) cudaFreeHost(c->h_counters);
+  for (int f = 0; f < EV_RING; ++f)
+    for (int i = 0; i < EV_N; ++i)
+      if (c->ev[f][i]) cudaEventDestroy(c->ev[f][i]);
+  delete c;
+}
+
+const char* hair_last_error(const hair_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+void hair_default_render_params(hair_render_params* p) {
+  if (!p) return;
+  memset(p, 0, sizeof(*p));
+  p->center_diameter_px = 0.5f;
+  p->filter_radius = 5;
+  p->s_par = 0.5f;
+  p->s_perp = 0.15f;
+  p->sigma_c = 0.9f;
+  p->tau_z = 1.45e-3f;
+  p->tau_fly = 5e-4f;
+  p->w_strip = 0.5f;
+  p->n_lights = 0;
+  p->ambient_rgb[0] = p->ambient_rgb[1] = p->ambient_rgb[2] = 0.15f;
+  p->k_d = 0.4f;
+  p->k_R = 0.25f;
+  p->k_TRT = 0.5f;
+  p->flags = HAIR_FLAG_FILTER;
+}
+
+int hair_set_render_params(hair_ctx* c, const hair_render_params* p) {
+  if (!c || !p) return HAIR_E_INVALID_ARG;
+  if (p->filter_radius < 0 || p->filter_radius > 7) return fail(c, HAIR_E_INVALID_ARG, "filter_radius must be 0..7");
+  if (p->n_lights > HAIR_MAX_LIGHTS) return fail(c, HAIR_E_INVALID_ARG, "too many lights");
+  if (!(p->center_diameter_px > 0.f) || p->center_diameter_px > 1.f)
+    return fail(c, HAIR_E_INVALID_ARG, "center_diameter_px must be in (0, 1] (centre layer inside conservative)");
+  if (!(p->sigma_c > 0.f)) return fail(c, HAIR_E_INVALID_ARG, "sigma_c must be positive");
+  c->prm = *p;
+  return HAIR_OK;
+}
+
+int hair_mesh_upload(hair_ctx* c, const hair_cage* cage, const hair_roots* roots, const hair_style* st,
+                     int* out_groom_id) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  if (!cage || !roots || !st || !cage->pos || !roots->idx || !roots->strands_per_tri)
+    return fail(c, HAIR_E_INVALID_ARG, "hair_mesh_upload: null argument");
+  if (cage->n_layers < 2 || cage->n_layers > 32 || cage->n_verts == 0 || roots->n_tris == 0 || st->spi == 0)
+    return fail(c, HAIR_E_INVALID_ARG, "hair_mesh_upload: need 2..32 layers, >= 1 triangle, spi >= 1");
+  if (c->scene.n_grooms >= HAIR_MAX_GROOMS) return fail(c, HAIR_E_TOO_MANY_GROOMS, "too many grooms");
+  const uint32_t c_full = (cage->n_layers - 1) * st->spi + 1;
+  if (c_full > 127) return fail(c, HAIR_E_TOO_MANY_CPS, "C_full = (n_layers-1)*spi+1 exceeds 127");
+  const uint32_t T = roots->n_tris, Q = st->n_instances ? st->n_instances : 1;
+  for (size_t i = 0; i < (size_t)T * 3; ++i)
+    if (roots->idx[i] >= cage->n_verts) return fail(c, HAIR_E_INVALID_ARG, "triangle index out of range");
+  std::vector<uint32_t> off(T + 1);
+  uint64_t acc = 0;
+  for (uint32_t t = 0; t < T; ++t) {
+    off[t] = (uint32_t)acc;
+    acc += roots->strands_per_tri[t];
+  }
+  off[T] = (uint32_t)acc;
+  const uint64_t N = acc;
+  const uint32_t gi = c->scene.n_grooms;
+  uint32_t sid_base = 0, gid_base = 0;
+  if (gi > 0) {
+    const GroomDev& p = c->scene.g[gi - 1];
+    sid_base = p.sid_base + p.N * p.Q;
+    gid_base = p.gid_base + p.T * p.Q;
+  }
+  if (N == 0) return fail(c, HAIR_E_INVALID_ARG, "groom has no strands");
+  if ((uint64_t)sid_base + N * Q >= (1ull << 24)) return fail(c, HAIR_E_TOO_MANY_STRANDS, "more than 2^24 strand ids");
+  if ((uint64_t)c->vertex_need + N * Q * c_full >= (1ull << 32)) return fail(c, HAIR_E_TOO_MANY_STRANDS, "vertex index overflow");
+  CK(cudaSetDevice(c->device));
+  GroomHost gh;
+  GroomDev gd;
+  memset(&gd, 0, sizeof(gd));
+  gh.pos_bytes = (size_t)cage->n_layers * cage->n_verts * 3 * sizeof(float);
+  gh.ao_bytes = (size_t)cage->n_layers * cage->n_verts * sizeof(float);
+  int rc = upload(c, &gh.pos, cage->pos, (size_t)cage->n_layers * cage->n_verts * 3);
+  if (!rc && cage->ao) rc = upload(c, &gh.ao, cage->ao, (size_t)cage->n_layers * cage->n_verts);
+  if (!rc) rc = upload(c, &gh.idx, roots->idx, (size_t)T * 3);
+  if (!rc) rc = upload(c, &gh.npt, roots->strands_per_tri, (size_t)T);
+  if (!rc) rc = upload(c, &gh.off, off.data(), (size_t)T + 1);
+  if (!rc && st->instance_xform) rc = upload(c, &gh.xform, st->instance_xform, (size_t)Q * 12);
+  if (rc) {
+    free_groom(gh);
+    return rc;
+  }
+  gd.pos = gh.pos;
+  gd.ao = gh.ao;
+  gd.idx = gh.idx;
+  gd.npt = gh.npt;
+  gd.off = gh.off;
+  gd.xform = gh.xform;
+  gd.V = cage->n_verts;
+  gd.Lv = cage->n_layers;
+  gd.T = T;
+  gd.Q = Q;
+  gd.N = (uint32_t)N;
+  gd.sid_base = sid_base;
+  gd.gid_base = gid_base;
+  gd.c_full = c_full;
+  gd.spi = st->spi;
+  gd.seed_h = pcg_host(st->seed);
+  gd.op_mask = st->op_mask;
+  gd.clump_exp = st->clump_exp;
+  gd.frizz_cells = st->frizz_cells;
+  gd.clump_strength = st->clump_strength;
+  gd.twist_turns = st->twist_turns;
+  gd.curl_radius = st->curl_radius;
+  gd.curl_turns = st->curl_turns;
+  gd.curl_ramp_w0 = st->curl_ramp_w0;
+  gd.frizz_sigma = st->frizz_sigma;
+  gd.frizz_ramp_w0 = st->frizz_ramp_w0;
+  gd.width_world = st->width_world;
+  for (int i = 0; i < 3; ++i) {
+    gd.albedo_root[i] = st->albedo_root[i];
+    gd.albedo_tip[i] = st->albedo_tip[i];
+  }
+  gd.roughness = st->roughness;
+  gd.tilt = st->tilt;
+  c->scene.g[gi] = gd;
+  c->scene.n_grooms = gi + 1;
+  c->scene.n_bi = gid_base + T * Q;
+  c->scene.n_strands_total = sid_base + (uint32_t)N * Q;
+  c->vertex_need += (size_t)N * Q * c_full;
+  if (c_full > c->c_max) c->c_max = c_full;
+  c->grooms.push_back(gh);
+  c->scene_dirty = true;
+  if (out_groom_id) *out_groom_id = (int)gi;
+  return HAIR_OK;
+}
+
+int hair_mesh_update(hair_ctx* c, int groom_id, const hair_cage* cage) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  if (groom_id < 0 || (uint32_t)groom_id >= c->scene.n_grooms || !cage || !cage->pos)
+    return fail(c, HAIR_E_INVALID_ARG, "hair_mesh_update: bad groom or cage");
+  const GroomDev& gd = c->scene.g[groom_id];
+  if (cage->n_layers != gd.Lv || cage->n_verts != gd.V) return fail(c, HAIR_E_INVALID_ARG, "hair_mesh_update: size mismatch");
+  GroomHost& gh = c->grooms[groom_id];
+  CK(cudaMemcpyAsync(gh.pos, cage->pos, gh.pos_bytes, cudaMemcpyHostToDevice, c->stream));
+  if (cage->ao && gh.ao) CK(cudaMemcpyAsync(gh.ao, cage->ao, gh.ao_bytes, cudaMemcpyHostToDevice, c->stream));
+  return HAIR_OK;
+}
+
+int hair_mesh_clear(hair_ctx* c) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  cudaStreamSynchronize(c->stream);
+  for (auto& g : c->grooms) free_groom(g);
+  c->grooms.clear();
+  memset(&c->scene, 0, sizeof(c->scene));
+  c->vertex_need = 0;
+  c->c_max = 0;
+  c->scene_dirty = true;
+  return HAIR_OK;
+}
+
+int hair_render(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
+                uint64_t* out_gbuffer, float* out_rgb) {
+  return render_impl(c, cam, w, h, lam, n_lam, 7u, true, (unsigned long long*)out_gbuffer, out_rgb);
+}
+
+int hair_render_stages(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, uint32_t stage_mask,
+                       uint64_t* out_gbuffer, float* out_rgb) {
+  return render_impl(c, cam, w, h, nullptr, 0, stage_mask & 7u, false, (unsigned long long*)out_gbuffer, out_rgb);
+}
+
+int hair_render_to_host(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam,
+                        uint32_t n_lam, uint64_t* host_gbuffer, float* host_rgb) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  if (!host_rgb) return fail(c, HAIR_E_INVALID_ARG, "hair_render_to_host: host_rgb is required");
+  CK(cudaSetDevice(c->device));
+  size_t px = (size_t)w * h;
+  if (px > c->own_px) {
+    cudaFree(c->d_own_gbuf);
+    cudaFree(c->d_own_rgb);
+    c->d_own_gbuf = nullptr;
+    c->d_own_rgb = nullptr;
+    c->own_px = 0;
+    CK(cudaMalloc((void**)&c->d_own_gbuf, px * 16));
+    CK(cudaMalloc((void**)&c->d_own_rgb, px * 16));
+    c->own_px = px;
+  }
+  int rc = render_impl(c, cam, w, h, lam, n_lam, 7u, true, c->d_own_gbuf, c->d_own_rgb);
+  if (rc) return rc;
+  CK(cudaMemcpyAsync(host_rgb, c->d_own_rgb, px * 16, cudaMemcpyDeviceToHost, c->stream));
+  if (host_gbuffer) CK(cudaMemcpyAsync(host_gbuffer, c->d_own_gbuf, px * 16, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return HAIR_OK;
+}
+
+int hair_stats(hair_ctx* c, hair_stats_t* out) {
+  if (!c || !out) return HAIR_E_INVALID_ARG;
+  memset(out, 0, sizeof(*out));
+  CK(cudaSetDevice(c->device));
+  CK(cudaMemcpyAsync(c->h_counters, c->d_counters, CNT_N * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  const unsigned long long* k = c->h_counters;
+  out->n_grooms = c->scene.n_grooms;
+  out->n_bundles = c->scene.n_bi;
+  out->n_bundles_culled = (uint32_t)k[CNT_CULLED];
+  out->n_strands_total = c->scene.n_strands_total;
+  out->n_strands_lod = (uint32_t)k[CNT_STRANDS];
+  out->n_vertices = (uint32_t)k[CNT_VERTICES];
+  out->n_segments = (uint32_t)k[CNT_SEGMENTS];
+  out->gpu_launches = c->launches;
+  out->beta_mean = c->scene.n_strands_total ? (float)((double)k[CNT_STRANDS] / (double)c->scene.n_strands_total) : 1.f;
+  if (c->counted) {
+    out->n_segments_drawn = (uint32_t)k[CNT_SEG_DRAWN];
+    out->n_atomics_center = k[CNT_AT_CENTER];
+    out->n_atomics_cons = k[CNT_AT_CONS];
+    out->n_atomics_issued = k[CNT_AT_ISSUED];
+    out->n_pixels_center = (uint32_t)k[CNT_PX_CENTER];
+    out->n_pixels_cons = (uint32_t)k[CNT_PX_CONS];
+  }
+  if (c->timed && c->ev_frames) {  // mean over the timed frames since the last call (at most EV_RING)
+    float* dst[6] = {&out->ms_lod, &out->ms_generate, &out->ms_clear, &out->ms_raster, &out->ms_shade, &out->ms_filter};
+    const uint32_t n = c->ev_frames < (uint32_t)EV_RING ? c->ev_frames : (uint32_t)EV_RING;
+    for (uint32_t f = 0; f < n; ++f) {
+      cudaEvent_t* evs = c->ev[(c->ev_frames - 1 - f) % EV_RING];
+      float ms = 0.f;
+      for (int i = 0; i < 6; ++i) {
+        cudaEventElapsedTime(&ms, evs[i], evs[i + 1]);
+        *dst[i] += ms / (float)n;
+      }
+      cudaEventElapsedTime(&ms, evs[EV_BEGIN], evs[EV_FILTER]);
+      out->ms_total += ms / (float)n;
+    }
+    out->n_timed_frames = n;
+    c->ev_frames = 0;
+  }
+  return HAIR_OK;
+}
+
+int hair_debug_buffers(hair_ctx* c, const float** v, const uint32_t** t, const float** col) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  if (v) *v = (const float*)c->d_vertices;
+  if (t) *t = (const uint32_t*)c->d_table;
+  if (col) *col = (const float*)c->d_colour;
+  return HAIR_OK;
+}
+
+int hair_debug_set_vertices(hair_ctx* c, const float* dev_src, uint32_t n) {
+  if (!c || !dev_src) return HAIR_E_INVALID_ARG;
+  if ((size_t)n > c->vertex_cap) return fail(c, HAIR_E_INVALID_ARG, "hair_debug_set_vertices: too many vertices");
+  CK(cudaMemcpyAsync(c->d_vertices, dev_src, (size_t)n * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+  return HAIR_OK;
+}
+
+void hair_abi_sizes(uint32_t out[6]) {
+  out[0] = sizeof(hair_cage);
+  out[1] = sizeof(hair_roots);
+  out[2] = sizeof(hair_style);
+  out[3] = sizeof(hair_camera);
+  out[4] = sizeof(hair_render_params);
+  out[5] = sizeof(hair_stats_t);
+}
+
+int hair_atomic_microbench(hair_ctx* c, int mode, uint64_t* dev_words, uint64_t n_words, uint64_t n_ops,
+                           uint32_t hot_words, float* out_ms) {
+  if (!c || !dev_words || !out_ms || n_words == 0 || mode < 0 || mode > 2) return HAIR_E_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  cudaEvent_t a, b;
+  CK(cudaEventCreate(&a));
+  CK(cudaEventCreate(&b));
+  CK(cudaMemsetAsync(dev_words, 0xFF, n_words * 8, c->stream));
+  CK(cudaEventRecord(a, c->stream));
+  launch_atomic_microbench(mode, (unsigned long long*)dev_words, n_words, n_ops, hot_words, c->n_sm, c->stream);
+  CK(cudaEventRecord(b, c->stream));
+  CK(cudaEventSynchronize(b));
+  CK(cudaEventElapsedTime(out_ms, a, b));
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  CK(cudaGetLastError());
+  return HAIR_OK;
+}
+
+}  // extern "C"

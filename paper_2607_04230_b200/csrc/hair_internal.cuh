@@ -1,0 +1,167 @@
+// hair_internal.cuh — device-side structs and arithmetic shared by libhair's kernels.
+//
+// The fp32 "decision" arithmetic of DESIGN.md §3 (projection R-proj, coverage R10, word R7/R8,
+// LOD Eq. 1-5, screen tangent R22, strip test Eq. 9) is written with __f*_rn intrinsics: one IEEE
+// rounding per operation, never contracted into FMA, whatever the compiler flags. Everything else
+// (generation, shading, filter weights) is ordinary fp32 with FMA contraction.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/hair.h"
+
+#define HAIR_EMPTY 0xFFFFFFFFFFFFFFFFull
+#define HAIR_ROW 44  // floats per control-point row of the per-bundle table (== 12 mod 32: LDS.128 conflict-free)
+
+struct GroomDev {
+  const float* pos;     // [Lv][V][3]
+  const float* ao;      // [Lv][V] or nullptr
+  const uint32_t* idx;  // [T][3]
+  const uint32_t* npt;  // [T]
+  const uint32_t* off;  // [T+1] exclusive scan of npt
+  const float* xform;   // [Q][12] or nullptr
+  uint32_t V, Lv, T, Q, N, sid_base, gid_base, c_full;
+  uint32_t spi, seed_h, op_mask, clump_exp, frizz_cells;
+  float clump_strength, twist_turns, curl_radius, curl_turns, curl_ramp_w0, frizz_sigma, frizz_ramp_w0;
+  float width_world;
+  float albedo_root[3], albedo_tip[3], roughness, tilt;
+};
+
+struct SceneDev {
+  GroomDev g[HAIR_MAX_GROOMS];
+  uint32_t n_grooms, n_bi, n_strands_total, pad;
+};
+
+struct CamDev {
+  float eye[3], r[3], u[3], f[3];
+  float near_z, fpx, A, B, half_w, half_h;
+  uint32_t W, H;
+};
+
+struct LambdaArr {
+  float v[HAIR_MAX_GROOMS];
+};
+
+struct ShadeParams {
+  float light_pos[HAIR_MAX_LIGHTS][3], light_rgb[HAIR_MAX_LIGHTS][3];
+  uint32_t n_lights;
+  float ambient[3], k_d, k_R, k_TRT, background[3];
+  // filter
+  int r;
+  float inv_sp2, inv_sq2, inv_sc2, w_strip;
+  uint32_t tauz_q, taufly_q, filter_on;
+  float rho_default;  // 0.5 * center_diameter_px
+};
+
+// device counters, one block of 64-bit words (index = enum)
+enum {
+  CNT_STRANDS = 0,   // sum N_LOD
+  CNT_VERTICES,      // sum N_LOD * C
+  CNT_SEGMENTS,      // sum N_LOD * (C-1)
+  CNT_CULLED,        // bundle-instances with N_LOD == 0
+  CNT_WORK_GEN,      // dynamic work counters of the persistent kernels
+  CNT_WORK_RASTER,
+  CNT_SEG_DRAWN,
+  CNT_AT_CENTER,
+  CNT_AT_CONS,
+  CNT_AT_ISSUED,
+  CNT_PX_CENTER,
+  CNT_PX_CONS,
+  CNT_N
+};
+
+// ------------------------------------------------------------------ exact fp32 (one rounding per op)
+__device__ __forceinline__ float xmul(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float xadd(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float xsub(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float xdiv(float a, float b) { return __fdiv_rn(a, b); }
+__device__ __forceinline__ float xsqrt(float a) { return __fsqrt_rn(a); }
+__device__ __forceinline__ float xdot3(float ax, float ay, float az, const float* b) {
+  return xadd(xadd(xmul(ax, b[0]), xmul(ay, b[1])), xmul(az, b[2]));
+}
+
+struct Proj {
+  float sx, sy, zn, zv;
+  bool valid;
+};
+// R-proj
+__device__ __forceinline__ Proj project_exact(const CamDev& c, float px, float py, float pz) {
+  float qx = xsub(px, c.eye[0]), qy = xsub(py, c.eye[1]), qz = xsub(pz, c.eye[2]);
+  float xv = xdot3(qx, qy, qz, c.r);
+  float yv = xdot3(qx, qy, qz, c.u);
+  float zv = xdot3(qx, qy, qz, c.f);
+  Proj o;
+  o.zv = zv;
+  o.valid = zv >= c.near_z;
+  float z = o.valid ? zv : 1.0f;
+  o.sx = xadd(c.half_w, xdiv(xmul(c.fpx, xv), z));
+  o.sy = xsub(c.half_h, xdiv(xmul(c.fpx, yv), z));
+  o.zn = xsub(c.A, xdiv(c.B, z));
+  return o;
+}
+
+// R7/R8 word
+__device__ __forceinline__ uint32_t quant_depth(float zn) {
+  uint32_t q = (uint32_t)xadd(xmul(zn, 16777215.0f), 0.5f);
+  return min(q, 0xFFFFFEu);
+}
+__device__ __forceinline__ uint32_t quant_t(float t) { return (uint32_t)xadd(xmul(t, 511.0f), 0.5f); }
+__device__ __forceinline__ unsigned long long pack_word(float zn, uint32_t sid, uint32_t j, float t) {
+  uint32_t hi = (quant_depth(zn) << 8) | (sid >> 16);
+  uint32_t lo = (sid << 16) | (j << 9) | quant_t(t);
+  return ((unsigned long long)hi << 32) | lo;
+}
+__device__ __forceinline__ uint32_t w_dq(unsigned long long w) { return (uint32_t)(w >> 40); }
+__device__ __forceinline__ uint32_t w_sid(unsigned long long w) { return (uint32_t)(w >> 16) & 0xFFFFFFu; }
+__device__ __forceinline__ uint32_t w_j(unsigned long long w) { return (uint32_t)(w >> 9) & 0x7Fu; }
+__device__ __forceinline__ uint32_t w_t9(unsigned long long w) { return (uint32_t)w & 0x1FFu; }
+
+// R26 hash
+__device__ __forceinline__ uint32_t pcg(uint32_t v) {
+  uint32_t s = v * 747796405u + 2891336453u;
+  uint32_t w = ((s >> ((s >> 28) + 4u)) ^ s) * 277803737u;
+  return (w >> 22) ^ w;
+}
+
+// strand id -> first vertex and control-point count of the strand in this frame's vertex buffer
+struct Loc {
+  uint32_t voff, C, groom;
+};
+__device__ __forceinline__ Loc locate_strand(const SceneDev* __restrict__ sc, const uint4* __restrict__ table,
+                                             uint32_t sid) {
+  uint32_t gi = 0;
+  for (uint32_t k = 1; k < sc->n_grooms; ++k)
+    if (sid >= sc->g[k].sid_base) gi = k;
+  const GroomDev& g = sc->g[gi];
+  uint32_t rel = sid - g.sid_base;
+  uint32_t q = rel / g.N, id_local = rel - q * g.N;
+  uint32_t lo = 0, hi = g.T;  // largest t with off[t] <= id_local
+  while (hi - lo > 1) {
+    uint32_t mid = (lo + hi) >> 1;
+    if (__ldg(&g.off[mid]) <= id_local) lo = mid;
+    else hi = mid;
+  }
+  uint4 e = __ldg(&table[g.gid_base + q * g.T + lo]);
+  Loc l;
+  l.C = e.y;
+  l.voff = e.w + (id_local - __ldg(&g.off[lo])) * e.y;
+  l.groom = gi;
+  return l;
+}
+
+// ------------------------------------------------------------------ launchers (one per .cu)
+void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint4* table,
+                     unsigned long long* counters, cudaStream_t st);
+void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices,
+                     unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st);
+void launch_clear(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
+void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const float4* vertices,
+                   CamDev cam, float rho_default, unsigned long long* gbuf, unsigned long long* counters,
+                   bool count, int n_sm, cudaStream_t st);
+void launch_shade(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+                  ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st);
+void launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+                   ShadeParams sp, const unsigned long long* gbuf, const float4* colour, float4* out,
+                   unsigned long long* counters, bool count, cudaStream_t st);
+void launch_atomic_microbench(int mode, unsigned long long* words, unsigned long long n_words,
+                              unsigned long long n_ops, uint32_t hot, int n_sm, cudaStream_t st);

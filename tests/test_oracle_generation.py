@@ -305,7 +305,7 @@ def test_frizz_is_perpendicular_unit_variance_and_zero_at_root(orc):
     assert np.abs(offs[:, 0, :]).max() == 0.0  # zero at the root (ramp)
     lat = offs[:, 2::2, :][:, :, [0, 2]] / sigma  # lattice points beyond the ramp
     assert abs(lat.var() - 1.0) < 0.05 and abs(lat.mean()) < 0.03
-    assert np.abs(lat).max() <= 2 * math.sqrt(3) + 1e-9  # (sum of 4 uniforms - 2) * sqrt(3)
+    assert np.abs(lat).max() <= 510 / math.sqrt(21845) + 1e-9  # (sum of 4 hash bytes - 510) / sqrt(21845)
 
 
 def test_all_ops_off_is_bit_identical_to_base(orc):
