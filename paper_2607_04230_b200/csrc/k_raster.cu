@@ -6,55 +6,33 @@
 // The predicates and the word are evaluated in the fixed-order fp32 of hair_internal.cuh, so the
 // result is bit-identical to the CPU oracle's brute force whatever the enumeration order.
 //
-// Work distribution: persistent warps fetch one bundle-instance at a time (device-side counter) and
-// walk its strand-major vertex run 31 segments per step: lane l loads + projects vertex v0+l once
-// (coalesced 16-byte loads) and receives vertex v0+l+1 from lane l+1 by shuffle.
+// Paper (prior art): each lane walks its own segment with a DDA; "the DDA rasterization stage
+// exhibits workload imbalance when threads draw lines of varying lengths".
+// Here: a warp takes 31 consecutive segments of a bundle's strand-major vertex run (lane l loads +
+// projects vertex v0+l once with a coalesced 16-byte load and gets vertex v0+l+1 from lane l+1 by
+// shuffle), publishes one 64-byte record per segment in shared memory, and then spreads the
+// (segment, major-axis column) pairs evenly over its lanes: a shuffle scan of the column counts,
+// then per 32 tasks one ballot + one REDUX.OR locate every lane's segment. Each task walks the 1-3
+// pixels of its column; long and sub-pixel segments cost the same per pixel.
 #include "hair_internal.cuh"
 
 #define RAS_WARPS 8
-
-struct Seg {
-  float ax, ay, az, bx, by, bz;  // screen endpoints and post-projection depths
-  float rho2;
-  uint32_t sid, j;
-};
-
-// One pixel of one segment: DESIGN.md R10/R11 in fixed-order fp32. Returns 0, 1 (conservative only)
-// or 3 (centre + conservative), and the packed word.
-__device__ __forceinline__ int cover_pixel(const Seg& s, float dx, float dy, float dd, float ext, float dz,
-                                           int x, int y, unsigned long long& word) {
-  const float cx = (float)x + 0.5f, cy = (float)y + 0.5f;
-  const float ux = xsub(cx, s.ax), uy = xsub(cy, s.ay);
-  const float cr = fabsf(xsub(xmul(dx, uy), xmul(dy, ux)));
-  if (!(cr <= ext)) return 0;
-  float t = 0.f;
-  if (dd > 0.f) t = fminf(fmaxf(xdiv(xadd(xmul(ux, dx), xmul(uy, dy)), dd), 0.f), 1.f);
-  const float zn = xadd(s.az, xmul(t, dz));
-  if (zn < 0.f || zn > 1.f) return 0;
-  word = pack_word(zn, s.sid, s.j, t);
-  const float ex = xsub(cx, xadd(s.ax, xmul(t, dx))), ey = xsub(cy, xadd(s.ay, xmul(t, dy)));
-  const float d2 = xadd(xmul(ex, ex), xmul(ey, ey));
-  return d2 <= s.rho2 ? 3 : 1;
-}
+#define REC_STRIDE 20  // floats per segment record (16 used); 20 mod 32 keeps LDS.128 conflict-free
+#define ENUM_EPS 0.015625f  // slack on the minor-axis range of a column: the enumeration must be a superset
 
 // read-before-atomic ("reads the existing depth buffer"): words only ever decrease, so
 // a stale read can only under-filter, never drop a winner.
-template <bool COUNT>
-__device__ __forceinline__ void resolve(unsigned long long* p, unsigned long long word, uint32_t& issued) {
-  if (word < __ldcg(p)) {
-    atomicMin(p, word);
-    if (COUNT) ++issued;
-  }
-}
-
 template <bool COUNT>
 __global__ void __launch_bounds__(RAS_WARPS * 32)
 k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
          const float4* __restrict__ vertices, CamDev cam, float rho_default, unsigned long long* __restrict__ gbuf,
          unsigned long long* __restrict__ counters) {
-  const uint32_t lane = threadIdx.x & 31;
+  __shared__ __align__(16) float s_rec[RAS_WARPS][32][REC_STRIDE];
+  const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  float(*rec)[REC_STRIDE] = s_rec[warp];
   uint32_t c_center = 0, c_cons = 0, c_drawn = 0, c_issued = 0;
-  const float Wm1 = (float)(cam.W - 1), Hm1 = (float)(cam.H - 1);
+  const int W = (int)cam.W, H = (int)cam.H;
+  const uint32_t le_mask = 0xFFFFFFFFu >> (31 - lane);
   for (;;) {
     uint32_t gid = 0;
     if (lane == 0) gid = (uint32_t)atomicAdd(&counters[CNT_WORK_RASTER], 1ull);
@@ -74,6 +52,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
     const uint32_t n_v = nlod * C;
     const float4* vin = vertices + e.w;
     for (uint32_t v0 = 0; v0 + 1 < n_v; v0 += 31) {
+      // ---- load + project 32 vertices, neighbour by shuffle
       const uint32_t v = v0 + lane;
       Proj a;
       a.valid = false;
@@ -90,41 +69,104 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
       b.valid = __shfl_down_sync(0xffffffffu, (int)a.valid, 1) != 0;
       const uint32_t k = v / C, j = v - k * C;
       const bool seg = lane < 31 && v + 1 < n_v && j + 1 < C && a.valid && b.valid;  // R12
-      if (!seg) continue;
-      if (COUNT) ++c_drawn;
-      Seg s;
-      s.ax = a.sx, s.ay = a.sy, s.az = a.zn, s.bx = b.sx, s.by = b.sy, s.bz = b.zn;
-      s.sid = sid0 + k;
-      s.j = j;
-      float rho = rho_default;
-      if (width > 0.f) {  // R9
-        const float zm = xmul(0.5f, xadd(a.zv, b.zv));
-        const float wpx = fminf(fmaxf(xdiv(xmul(width, cam.fpx), zm), 0.25f), 1.0f);
-        rho = xmul(0.5f, wpx);
+      // ---- segment record in (major, minor) coordinates; every formula below is symmetric in x/y
+      uint32_t n_steps = 0;
+      if (seg) {
+        if (COUNT) ++c_drawn;
+        float rho = rho_default;
+        if (width > 0.f) {  // R9
+          const float zm = xmul(0.5f, xadd(a.zv, b.zv));
+          const float wpx = fminf(fmaxf(xdiv(xmul(width, cam.fpx), zm), 0.25f), 1.0f);
+          rho = xmul(0.5f, wpx);
+        }
+        const float dx = xsub(b.sx, a.sx), dy = xsub(b.sy, a.sy);
+        const bool ymajor = fabsf(dy) > fabsf(dx);
+        const float aM = ymajor ? a.sy : a.sx, aN = ymajor ? a.sx : a.sy;
+        const float bM = ymajor ? b.sy : b.sx, bN = ymajor ? b.sx : b.sy;
+        const float dM = ymajor ? dy : dx, dN = ymajor ? dx : dy;
+        const float limM = (float)((ymajor ? H : W) - 1), limN = (float)((ymajor ? W : H) - 1);
+        // candidate pixels = exactly those whose closed square overlaps the segment's AABB (R10)
+        const float fc0 = fmaxf(ceilf(fminf(aM, bM)) - 1.f, 0.f), fc1 = fminf(floorf(fmaxf(aM, bM)), limM);
+        const float fr0 = fmaxf(ceilf(fminf(aN, bN)) - 1.f, 0.f), fr1 = fminf(floorf(fmaxf(aN, bN)), limN);
+        if (fc0 <= fc1 && fr0 <= fr1) {
+          n_steps = (uint32_t)((int)fc1 - (int)fc0 + 1);
+          float4* r4 = reinterpret_cast<float4*>(rec[lane]);
+          const float dd = xadd(xmul(dx, dx), xmul(dy, dy));
+          r4[0] = make_float4(aM, aN, dM, dN);
+          r4[1] = make_float4(dd, xmul(0.5f, xadd(fabsf(dx), fabsf(dy))), a.zn, xsub(b.zn, a.zn));
+          r4[2] = make_float4(xmul(rho, rho), dM != 0.f ? dN / dM : 0.f, __int_as_float((int)fc0),
+                              __uint_as_float(((uint32_t)(int)fr0 << 16) | (uint32_t)(int)fr1));
+          r4[3].x = __uint_as_float((ymajor ? 0x80000000u : 0u) | ((sid0 + k) << 7) | j);
+        }
       }
-      s.rho2 = xmul(rho, rho);
-      const float dx = xsub(s.bx, s.ax), dy = xsub(s.by, s.ay);
-      const float dd = xadd(xmul(dx, dx), xmul(dy, dy));
-      const float ext = xmul(0.5f, xadd(fabsf(dx), fabsf(dy)));
-      const float dz = xsub(s.bz, s.az);
-      // candidate pixels = exactly those whose closed square overlaps the segment's AABB (R10)
-      const float fx0 = fmaxf(ceilf(fminf(s.ax, s.bx)) - 1.f, 0.f), fx1 = fminf(floorf(fmaxf(s.ax, s.bx)), Wm1);
-      const float fy0 = fmaxf(ceilf(fminf(s.ay, s.by)) - 1.f, 0.f), fy1 = fminf(floorf(fmaxf(s.ay, s.by)), Hm1);
-      if (!(fx0 <= fx1) || !(fy0 <= fy1)) continue;
-      const int x0 = (int)fx0, x1 = (int)fx1, y0 = (int)fy0, y1 = (int)fy1;
-      for (int y = y0; y <= y1; ++y)
-        for (int x = x0; x <= x1; ++x) {
-          unsigned long long word;
-          const int c = cover_pixel(s, dx, dy, dd, ext, dz, x, y, word);
-          if (!c) continue;
-          unsigned long long* px = gbuf + ((size_t)y * cam.W + x) * 2;
-          if (COUNT) ++c_cons;
-          resolve<COUNT>(px + 1, word, c_issued);
-          if (c & 2) {
-            if (COUNT) ++c_center;
-            resolve<COUNT>(px, word, c_issued);
+      // ---- spread (segment, column) tasks over the lanes
+      const uint32_t n_eff = max(n_steps, 1u);  // empty segments keep one no-op task: starts stay distinct
+      uint32_t incl = n_eff;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t up = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += up;
+      }
+      const uint32_t X = incl - n_eff;
+      const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
+      rec[lane][13] = __uint_as_float(X);
+      rec[lane][14] = __uint_as_float(n_steps);
+      __syncwarp();
+      for (uint32_t base = 0; base < total; base += 32) {
+        const uint32_t before = __popc(__ballot_sync(0xffffffffu, X < base));
+        const uint32_t startbits = __reduce_or_sync(0xffffffffu, (X >= base && X < base + 32) ? 1u << (X - base) : 0u);
+        const uint32_t s = before + __popc(startbits & le_mask) - 1;  // owner of task base + lane
+        const uint32_t tau = base + lane;
+        if (tau >= total) continue;
+        const float4* r4 = reinterpret_cast<const float4*>(rec[s]);
+        const float4 q3 = r4[3];
+        const uint32_t step = tau - __float_as_uint(q3.y);
+        if (step >= __float_as_uint(q3.z)) continue;  // the no-op task of an empty segment
+        const float4 q0 = r4[0], q1 = r4[1], q2 = r4[2];
+        const float aM = q0.x, aN = q0.y, dM = q0.z, dN = q0.w;
+        const float dd = q1.x, ext = q1.y, az = q1.z, dz = q1.w;
+        const uint32_t key = __float_as_uint(q3.x);
+        const int c = __float_as_int(q2.z) + (int)step;
+        const int r0 = (int)(__float_as_uint(q2.w) >> 16), r1 = (int)(__float_as_uint(q2.w) & 0xFFFFu);
+        // minor-axis extent of the segment inside column [c, c+1] (superset, ENUM_EPS slack)
+        const float fc = (float)c, bMa = aM + dM;
+        const float lo = fmaxf(fc, fminf(aM, bMa)), hi = fminf(fc + 1.f, fmaxf(aM, bMa));
+        const float m0 = aN + (lo - aM) * q2.y, m1 = aN + (hi - aM) * q2.y;
+        const int rlo = max((int)ceilf(fminf(m0, m1) - ENUM_EPS) - 1, r0);
+        const int rhi = min((int)floorf(fmaxf(m0, m1) + ENUM_EPS), r1);
+        const float cM = fc + 0.5f;
+        const float uM = xsub(cM, aM);
+        for (int r = rlo; r <= rhi; ++r) {
+          // DESIGN.md R10/R11 in fixed-order fp32 (x/y-symmetric, so evaluated in major/minor order)
+          const float cN = (float)r + 0.5f;
+          const float uN = xsub(cN, aN);
+          const float cr = fabsf(xsub(xmul(dM, uN), xmul(dN, uM)));
+          if (!(cr <= ext)) continue;
+          float tt = 0.f;
+          if (dd > 0.f) tt = fminf(fmaxf(xdiv(xadd(xmul(uM, dM), xmul(uN, dN)), dd), 0.f), 1.f);
+          const float zn = xadd(az, xmul(tt, dz));
+          if (zn < 0.f || zn > 1.f) continue;
+          const float eM = xsub(cM, xadd(aM, xmul(tt, dM))), eN = xsub(cN, xadd(aN, xmul(tt, dN)));
+          const bool centre = xadd(xmul(eM, eM), xmul(eN, eN)) <= q2.x;
+          const unsigned long long word = pack_word(zn, (key >> 7) & 0xFFFFFFu, key & 0x7Fu, tt);
+          const int x = (key >> 31) ? r : c, y = (key >> 31) ? c : r;
+          unsigned long long* px = gbuf + ((size_t)y * W + x) * 2;
+          const ulonglong2 cur = __ldcg(reinterpret_cast<const ulonglong2*>(px));
+          if (COUNT) {
+            ++c_cons;
+            c_center += centre ? 1u : 0u;
+          }
+          if (word < cur.y) {
+            atomicMin(px + 1, word);
+            if (COUNT) ++c_issued;
+          }
+          if (centre && word < cur.x) {
+            atomicMin(px, word);
+            if (COUNT) ++c_issued;
           }
         }
+      }
+      __syncwarp();
     }
   }
   if (COUNT) {
