@@ -1,6 +1,9 @@
 """Builds csrc/libhair.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_2607_04230_b200.build [--force] [--verbose]
+
+HAIR_CFLAGS (environment) appends flags to the nvcc compile lines, e.g. "-DRAS_MIN_BLOCKS=4" to
+try another tuning constant; such a build is for measurement only.
 """
 from __future__ import annotations
 
@@ -41,7 +44,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         obj = os.path.join(CSRC, s.replace(".cu", ".o"))
         objs.append(obj)
         if force or _stale(obj, [src] + headers):
-            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+            cmd = ([nvcc] + NVCC_FLAGS + os.environ.get("HAIR_CFLAGS", "").split()
+                   + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj])
             jobs.append(cmd)
 
     def run(cmd):

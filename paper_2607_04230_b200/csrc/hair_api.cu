@@ -18,7 +18,7 @@ namespace {
 
 struct GroomHost {
   float *pos = nullptr, *ao = nullptr, *xform = nullptr;
-  uint32_t *idx = nullptr, *npt = nullptr, *off = nullptr;
+  uint32_t *idx = nullptr, *npt = nullptr, *off = nullptr, *tri_of = nullptr;
   size_t pos_bytes = 0, ao_bytes = 0;
 };
 
@@ -39,6 +39,7 @@ struct hair_ctx {
   hair_render_params prm;
   // scratch
   uint4* d_table = nullptr;
+  uint32_t* d_grp = nullptr;  // [n_bi + 1] exclusive scan of the raster's work groups per bundle-instance
   size_t table_cap = 0;
   float4* d_vertices = nullptr;
   size_t vertex_cap = 0;
@@ -115,12 +116,24 @@ ShadeParams make_shade(const hair_render_params& p) {
   s.k_R = p.k_R;
   s.k_TRT = p.k_TRT;
   s.r = p.filter_radius;
+  const double L2E = 1.4426950408889634;
   double sp = (double)p.filter_radius * (double)p.s_par, sq = (double)p.filter_radius * (double)p.s_perp;
-  s.inv_sp2 = sp > 0 ? (float)(1.0 / (sp * sp)) : 0.f;
-  s.inv_sq2 = sq > 0 ? (float)(1.0 / (sq * sq)) : 0.f;
-  s.inv_sc2 = (float)(1.0 / ((double)p.sigma_c * (double)p.sigma_c));
-  s.w_strip = p.w_strip;
-  s.tauz_q = (uint32_t)std::floor((double)p.tau_z * 16777215.0 + 0.5);    // R20: integer thresholds
+  s.kP = sp > 0 ? (float)(-L2E / (sp * sp)) : 0.f;  // Eq. 10, sigma = r * s
+  s.kQ = sq > 0 ? (float)(-L2E / (sq * sq)) : 0.f;
+  s.kC = (float)(L2E / ((double)p.sigma_c * (double)p.sigma_c));
+  const double e_min = ((double)s.kP + (double)s.kQ) * 2.0 * p.filter_radius * p.filter_radius;  // window corner
+  s.bias_nc = (float)std::fmin(std::fmax(-0.5 * e_min, 0.0), 60.0);
+  s.strip_loose = p.w_strip + 0.01f;
+  if (!(p.w_strip >= 0.f)) s.strip_e2_max = -1.f;  // Eq. 9 distance is never negative
+  else if (p.w_strip > 1e6f) s.strip_e2_max = 3.0e38f;
+  else {  // sqrt_rn(e2) <= w_strip  <=>  e2 <= strip_e2_max (sqrt_rn is monotone; host sqrtf is IEEE)
+    float c = (float)((double)p.w_strip * (double)p.w_strip);
+    while (std::sqrt(c) <= p.w_strip) c = std::nextafter(c, INFINITY);
+    while (c > 0.f && std::sqrt(c) > p.w_strip) c = std::nextafter(c, -INFINITY);
+    s.strip_e2_max = c;
+  }
+  // R20: integer thresholds (depth differences never exceed 2^24 - 2, so clamping changes nothing)
+  s.tauz_q = (uint32_t)std::fmin(std::floor((double)p.tau_z * 16777215.0 + 0.5), 16777215.0);
   s.taufly_q = (uint32_t)std::floor((double)p.tau_fly * 16777215.0 + 0.5);
   s.filter_on = (p.flags & HAIR_FLAG_FILTER) ? 1u : 0u;
   s.rho_default = 0.5f * p.center_diameter_px;
@@ -141,14 +154,19 @@ void free_groom(GroomHost& g) {
   cudaFree(g.idx);
   cudaFree(g.npt);
   cudaFree(g.off);
+  cudaFree(g.tri_of);
   g = GroomHost();
 }
 
 int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
   if (c->scene.n_bi > c->table_cap) {
     cudaFree(c->d_table);
+    cudaFree(c->d_grp);
     c->d_table = nullptr;
+    c->d_grp = nullptr;
+    c->table_cap = 0;
     CK(cudaMalloc((void**)&c->d_table, (size_t)c->scene.n_bi * sizeof(uint4)));
+    CK(cudaMalloc((void**)&c->d_grp, ((size_t)c->scene.n_bi + 1) * sizeof(uint32_t)));
     c->table_cap = c->scene.n_bi;
   }
   if (c->vertex_need > c->vertex_cap) {
@@ -202,7 +220,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   if (front && n_bi) {
     LambdaArr la;
     for (uint32_t i = 0; i < HAIR_MAX_GROOMS; ++i) la.v[i] = n_lam == 0 ? 0.f : lam[n_lam == 1 ? 0 : (i < n_lam ? i : 0)];
-    launch_lod_scan(c->d_scene, n_bi, k, la, c->d_table, c->d_counters, st);
+    launch_lod_scan(c->d_scene, n_bi, k, la, c->d_table, c->d_grp, c->d_counters, st);
     launches += 2;
   }
   mark(EV_LOD);
@@ -218,8 +236,8 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   mark(EV_CLEAR);
   if ((stage_mask & 1u) && n_bi) {
     if (!front) CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER, 0, sizeof(unsigned long long), st));
-    launch_raster(c->d_scene, n_bi, c->d_table, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters, count,
-                  c->n_sm, st);
+    launch_raster(c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters,
+                  count, c->n_sm, st);
     ++launches;
   }
   mark(EV_RASTER);
@@ -229,9 +247,8 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_SHADE);
   if (stage_mask & 4u) {
-    launch_filter(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour, (float4*)rgb, c->d_counters,
-                  count, st);
-    ++launches;
+    launches += launch_filter(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour, (float4*)rgb,
+                              c->d_counters, count, st);
   }
   mark(EV_FILTER);
   CK(cudaGetLastError());
@@ -282,6 +299,7 @@ void hair_destroy(hair_ctx* c) {
   for (auto& g : c->grooms) free_groom(g);
   cudaFree(c->d_scene);
   cudaFree(c->d_table);
+  cudaFree(c->d_grp);
   cudaFree(c->d_vertices);
   cudaFree(c->d_colour);
   cudaFree(c->d_counters);
@@ -368,6 +386,12 @@ int hair_mesh_upload(hair_ctx* c, const hair_cage* cage, const hair_roots* roots
   if (!rc) rc = upload(c, &gh.idx, roots->idx, (size_t)T * 3);
   if (!rc) rc = upload(c, &gh.npt, roots->strands_per_tri, (size_t)T);
   if (!rc) rc = upload(c, &gh.off, off.data(), (size_t)T + 1);
+  if (!rc) {
+    std::vector<uint32_t> tri_of((size_t)N);
+    for (uint32_t t = 0; t < T; ++t)
+      for (uint32_t i = off[t]; i < off[t + 1]; ++i) tri_of[i] = t;
+    rc = upload(c, &gh.tri_of, tri_of.data(), (size_t)N);
+  }
   if (!rc && st->instance_xform) rc = upload(c, &gh.xform, st->instance_xform, (size_t)Q * 12);
   if (rc) {
     free_groom(gh);
@@ -378,6 +402,7 @@ int hair_mesh_upload(hair_ctx* c, const hair_cage* cage, const hair_roots* roots
   gd.idx = gh.idx;
   gd.npt = gh.npt;
   gd.off = gh.off;
+  gd.tri_of = gh.tri_of;
   gd.xform = gh.xform;
   gd.V = cage->n_verts;
   gd.Lv = cage->n_layers;

@@ -11,6 +11,8 @@
 #include "../../include/hair.h"
 
 #define HAIR_EMPTY 0xFFFFFFFFFFFFFFFFull
+#define RAS_CHUNK 31  // segments a raster warp draws at once (32 vertices, neighbour by shuffle)
+#define RAS_GROUP 4   // chunks per unit of the raster's device-side work queue
 #define HAIR_ROW 44  // floats per control-point row of the per-bundle table (== 12 mod 32: LDS.128 conflict-free)
 
 struct GroomDev {
@@ -19,6 +21,7 @@ struct GroomDev {
   const uint32_t* idx;  // [T][3]
   const uint32_t* npt;  // [T]
   const uint32_t* off;  // [T+1] exclusive scan of npt
+  const uint32_t* tri_of;  // [N] bundle (root triangle) of each local strand id: the inverse of off
   const float* xform;   // [Q][12] or nullptr
   uint32_t V, Lv, T, Q, N, sid_base, gid_base, c_full;
   uint32_t spi, seed_h, op_mask, clump_exp, frizz_cells;
@@ -46,9 +49,13 @@ struct ShadeParams {
   float light_pos[HAIR_MAX_LIGHTS][3], light_rgb[HAIR_MAX_LIGHTS][3];
   uint32_t n_lights;
   float ambient[3], k_d, k_R, k_TRT, background[3];
-  // filter
+  // filter (k_shade_filter.cu): exponents are in base 2
   int r;
-  float inv_sp2, inv_sq2, inv_sc2, w_strip;
+  float kP, kQ;        // -log2(e) / sigma_par^2, -log2(e) / sigma_perp^2 (Eq. 10)
+  float kC;            // log2(e) / sigma_c^2
+  float bias_nc;       // exponent bias of the accumulations without colour term (keeps e^-90 weights normal)
+  float strip_loose;   // w_strip + 0.01: taps whose fast cross product is below it take the exact strip test
+  float strip_e2_max;  // largest float e2 with sqrt_rn(e2) <= w_strip
   uint32_t tauz_q, taufly_q, filter_on;
   float rho_default;  // 0.5 * center_diameter_px
 };
@@ -135,12 +142,7 @@ __device__ __forceinline__ Loc locate_strand(const SceneDev* __restrict__ sc, co
   const GroomDev& g = sc->g[gi];
   uint32_t rel = sid - g.sid_base;
   uint32_t q = rel / g.N, id_local = rel - q * g.N;
-  uint32_t lo = 0, hi = g.T;  // largest t with off[t] <= id_local
-  while (hi - lo > 1) {
-    uint32_t mid = (lo + hi) >> 1;
-    if (__ldg(&g.off[mid]) <= id_local) lo = mid;
-    else hi = mid;
-  }
+  const uint32_t lo = __ldg(&g.tri_of[id_local]);
   uint4 e = __ldg(&table[g.gid_base + q * g.T + lo]);
   Loc l;
   l.C = e.y;
@@ -151,16 +153,16 @@ __device__ __forceinline__ Loc locate_strand(const SceneDev* __restrict__ sc, co
 
 // ------------------------------------------------------------------ launchers (one per .cu)
 void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint4* table,
-                     unsigned long long* counters, cudaStream_t st);
+                     uint32_t* grp, unsigned long long* counters, cudaStream_t st);
 void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices,
                      unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st);
 void launch_clear(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
-void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const float4* vertices,
-                   CamDev cam, float rho_default, unsigned long long* gbuf, unsigned long long* counters,
-                   bool count, int n_sm, cudaStream_t st);
+void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
+                   const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
+                   unsigned long long* counters, bool count, int n_sm, cudaStream_t st);
 void launch_shade(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
                   ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st);
-void launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+int launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
                    ShadeParams sp, const unsigned long long* gbuf, const float4* colour, float4* out,
                    unsigned long long* counters, bool count, cudaStream_t st);
 void launch_atomic_microbench(int mode, unsigned long long* words, unsigned long long n_words,

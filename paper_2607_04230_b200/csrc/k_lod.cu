@@ -89,62 +89,74 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
   table[gid] = make_uint4(nlod, C, 0u, 0u);
 }
 
-// Exclusive scans of N_LOD and N_LOD*C over bundle-instances in index order (O1 step 6).
-// One CTA of 1024 threads; each warp owns a contiguous range and walks it 32 entries at a time with
-// a shuffle scan and a running carry; the 32 warp totals are scanned by warp 0; a second pass adds
-// the warp offsets. Coalesced 16-byte accesses throughout.
-__global__ void __launch_bounds__(1024) k_scan(uint4* __restrict__ table, uint32_t n_bi,
+// Exclusive scans of N_LOD, N_LOD*C and the raster's work-group count over bundle-instances in
+// index order (O1 step 6). One CTA of 1024 threads; each warp owns a contiguous range and
+// walks it 32 entries at a time with a shuffle scan and a running carry; the 32 warp totals are
+// scanned by warp 0; a second pass adds the warp offsets. Coalesced 16-byte accesses throughout.
+__device__ __forceinline__ uint32_t raster_groups(uint32_t n_v) {  // units of RAS_GROUP*RAS_CHUNK segment starts
+  return n_v >= 2 ? (n_v - 1 + RAS_GROUP * RAS_CHUNK - 1) / (RAS_GROUP * RAS_CHUNK) : 0u;
+}
+
+__global__ void __launch_bounds__(1024) k_scan(uint4* __restrict__ table, uint32_t* __restrict__ grp, uint32_t n_bi,
                                                unsigned long long* __restrict__ counters) {
-  __shared__ uint32_t s_slot[32], s_vert[32], s_cull[32];
+  __shared__ uint32_t s_slot[32], s_vert[32], s_grp[32], s_cull[32];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t per_warp = ((n_bi + 31) / 32 + 31) / 32 * 32;  // multiple of 32
-  const uint32_t begin = warp * per_warp, end = min(begin + per_warp, n_bi);
-  uint32_t carry_s = 0, carry_v = 0, culled = 0;
+  const uint32_t begin = min(warp * per_warp, n_bi), end = min(begin + per_warp, n_bi);
+  uint32_t carry_s = 0, carry_v = 0, carry_g = 0, culled = 0;
   for (uint32_t base = begin; base < end; base += 32) {
     uint32_t i = base + lane;
     uint4 e = i < end ? table[i] : make_uint4(0, 0, 0, 0);
-    uint32_t s = e.x, v = e.x * e.y;
+    uint32_t s = e.x, v = e.x * e.y, g = raster_groups(v);
     culled += (i < end && e.x == 0) ? 1u : 0u;
-    uint32_t is = s, iv = v;
+    uint32_t is = s, iv = v, ig = g;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
-      uint32_t a = __shfl_up_sync(0xffffffffu, is, d), b = __shfl_up_sync(0xffffffffu, iv, d);
+      uint32_t a = __shfl_up_sync(0xffffffffu, is, d), b = __shfl_up_sync(0xffffffffu, iv, d),
+               c = __shfl_up_sync(0xffffffffu, ig, d);
       if (lane >= d) {
         is += a;
         iv += b;
+        ig += c;
       }
     }
     if (i < end) {
       e.z = carry_s + is - s;
       e.w = carry_v + iv - v;
       table[i] = e;
+      grp[i] = carry_g + ig - g;
     }
     carry_s += __shfl_sync(0xffffffffu, is, 31);
     carry_v += __shfl_sync(0xffffffffu, iv, 31);
+    carry_g += __shfl_sync(0xffffffffu, ig, 31);
   }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) culled += __shfl_xor_sync(0xffffffffu, culled, d);
   if (lane == 0) {
     s_slot[warp] = carry_s;
     s_vert[warp] = carry_v;
+    s_grp[warp] = carry_g;
     s_cull[warp] = culled;
   }
   __syncthreads();
   if (warp == 0) {
-    uint32_t s = s_slot[lane], v = s_vert[lane], c = s_cull[lane];
-    uint32_t is = s, iv = v;
+    uint32_t s = s_slot[lane], v = s_vert[lane], g = s_grp[lane], c = s_cull[lane];
+    uint32_t is = s, iv = v, ig = g;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
-      uint32_t a = __shfl_up_sync(0xffffffffu, is, d), b = __shfl_up_sync(0xffffffffu, iv, d);
+      uint32_t a = __shfl_up_sync(0xffffffffu, is, d), b = __shfl_up_sync(0xffffffffu, iv, d),
+               cc = __shfl_up_sync(0xffffffffu, ig, d);
       if (lane >= d) {
         is += a;
         iv += b;
+        ig += cc;
       }
     }
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
     s_slot[lane] = is - s;
     s_vert[lane] = iv - v;
+    s_grp[lane] = ig - g;
     if (lane == 31) {
       counters[CNT_STRANDS] = is;
       counters[CNT_VERTICES] = iv;
@@ -153,21 +165,23 @@ __global__ void __launch_bounds__(1024) k_scan(uint4* __restrict__ table, uint32
       counters[CNT_WORK_GEN] = 0;
       counters[CNT_WORK_RASTER] = 0;
       for (int k = CNT_SEG_DRAWN; k < CNT_N; ++k) counters[k] = 0;
+      grp[n_bi] = ig;  // total work groups: the raster's queue length
     }
   }
   __syncthreads();
-  uint32_t off_s = s_slot[warp], off_v = s_vert[warp];
+  uint32_t off_s = s_slot[warp], off_v = s_vert[warp], off_g = s_grp[warp];
   if (warp > 0)
     for (uint32_t i = begin + lane; i < end; i += 32) {
       uint4 e = table[i];
       e.z += off_s;
       e.w += off_v;
       table[i] = e;
+      grp[i] += off_g;
     }
 }
 
 void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint4* table,
-                     unsigned long long* counters, cudaStream_t st) {
+                     uint32_t* grp, unsigned long long* counters, cudaStream_t st) {
   k_lod<<<(n_bi + 255) / 256, 256, 0, st>>>(d_scene, n_bi, cam, lam, table);
-  k_scan<<<1, 1024, 0, st>>>(table, n_bi, counters);
+  k_scan<<<1, 1024, 0, st>>>(table, grp, n_bi, counters);
 }

@@ -17,30 +17,55 @@
 #include "hair_internal.cuh"
 
 #define RAS_WARPS 8
+#ifndef RAS_MIN_BLOCKS
+#define RAS_MIN_BLOCKS 5  // CTAs per SM the register budget is held to (40 of 64 warps)
+#endif
 #define REC_STRIDE 20  // floats per segment record (16 used); 20 mod 32 keeps LDS.128 conflict-free
 #define ENUM_EPS 0.015625f  // slack on the minor-axis range of a column: the enumeration must be a superset
+#ifndef ROW_BATCH
+#define ROW_BATCH 1
+#endif
+// ROW_BATCH: rows of one column whose G-buffer words are requested before any is used
 
 // read-before-atomic ("reads the existing depth buffer"): words only ever decrease, so
 // a stale read can only under-filter, never drop a winner.
+//
+// Work distribution: the unit a warp fetches from the device-side queue is a GROUP of RAS_GROUP
+// chunks of RAS_CHUNK segments inside one bundle-instance (k_scan wrote the exclusive scan of the
+// group counts, `grp`); the warp finds the bundle of its group with a 32-ary search (one ballot per
+// level). Bundles differ 50x in work (strand count after LOD x pixel length), so bundle-sized units
+// left a long tail.
 template <bool COUNT>
-__global__ void __launch_bounds__(RAS_WARPS * 32)
+__global__ void __launch_bounds__(RAS_WARPS * 32, RAS_MIN_BLOCKS)
 k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
-         const float4* __restrict__ vertices, CamDev cam, float rho_default, unsigned long long* __restrict__ gbuf,
-         unsigned long long* __restrict__ counters) {
+         const uint32_t* __restrict__ grp, const float4* __restrict__ vertices, CamDev cam, float rho_default,
+         unsigned long long* __restrict__ gbuf, unsigned long long* __restrict__ counters) {
   __shared__ __align__(16) float s_rec[RAS_WARPS][32][REC_STRIDE];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float(*rec)[REC_STRIDE] = s_rec[warp];
   uint32_t c_center = 0, c_cons = 0, c_drawn = 0, c_issued = 0;
   const int W = (int)cam.W, H = (int)cam.H;
   const uint32_t le_mask = 0xFFFFFFFFu >> (31 - lane);
+  const uint32_t n_groups = __ldcg(&grp[n_bi]);
   for (;;) {
-    uint32_t gid = 0;
-    if (lane == 0) gid = (uint32_t)atomicAdd(&counters[CNT_WORK_RASTER], 1ull);
-    gid = __shfl_sync(0xffffffffu, gid, 0);
-    if (gid >= n_bi) break;
+    uint32_t wi = 0;
+    if (lane == 0) wi = (uint32_t)atomicAdd(&counters[CNT_WORK_RASTER], 1ull);
+    wi = __shfl_sync(0xffffffffu, wi, 0);
+    if (wi >= n_groups) break;
+    // ---- bundle of this group: largest gid with grp[gid] <= wi (32 pivots per level)
+    uint32_t lo = 0, n = n_bi;
+    while (n > 1) {
+      const uint32_t step = (n + 31) >> 5;
+      const uint32_t idx = lo + lane * step;
+      const bool le = idx < lo + n && __ldg(&grp[idx]) <= wi;  // non-decreasing => a prefix of the lanes
+      const uint32_t cnt = __popc(__ballot_sync(0xffffffffu, le));
+      const uint32_t nlo = lo + (cnt - 1) * step;
+      n = min(step, lo + n - nlo);
+      lo = nlo;
+    }
+    const uint32_t gid = lo;
     const uint4 e = __ldg(&table[gid]);
     const uint32_t nlod = e.x, C = e.y;
-    if (nlod == 0) continue;
     uint32_t gi = 0;
     for (uint32_t k = 1; k < sc->n_grooms; ++k)
       if (gid >= sc->g[k].gid_base) gi = k;
@@ -51,16 +76,19 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
     const float width = g.width_world;
     const uint32_t n_v = nlod * C;
     const float4* vin = vertices + e.w;
-    for (uint32_t v0 = 0; v0 + 1 < n_v; v0 += 31) {
-      // ---- load + project 32 vertices, neighbour by shuffle
+    const uint32_t v_begin = (wi - __ldg(&grp[gid])) * (RAS_GROUP * RAS_CHUNK);
+    const uint32_t v_end = min(v_begin + RAS_GROUP * RAS_CHUNK, n_v - 1);  // first vertex of the next group
+    float4 p_next = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (v_begin + lane < n_v) p_next = __ldg(&vin[v_begin + lane]);
+    for (uint32_t v0 = v_begin; v0 < v_end; v0 += RAS_CHUNK) {
+      // ---- project 32 vertices (loaded one chunk ahead), neighbour by shuffle
       const uint32_t v = v0 + lane;
+      const float4 p = p_next;
+      if (v0 + RAS_CHUNK < v_end && v + RAS_CHUNK < n_v) p_next = __ldg(&vin[v + RAS_CHUNK]);
       Proj a;
       a.valid = false;
       a.sx = a.sy = a.zn = a.zv = 0.f;
-      if (v < n_v) {
-        const float4 p = __ldg(&vin[v]);
-        a = project_exact(cam, p.x, p.y, p.z);
-      }
+      if (v < n_v) a = project_exact(cam, p.x, p.y, p.z);
       Proj b;
       b.sx = __shfl_down_sync(0xffffffffu, a.sx, 1);
       b.sy = __shfl_down_sync(0xffffffffu, a.sy, 1);
@@ -68,7 +96,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
       b.zv = __shfl_down_sync(0xffffffffu, a.zv, 1);
       b.valid = __shfl_down_sync(0xffffffffu, (int)a.valid, 1) != 0;
       const uint32_t k = v / C, j = v - k * C;
-      const bool seg = lane < 31 && v + 1 < n_v && j + 1 < C && a.valid && b.valid;  // R12
+      const bool seg = lane < 31 && v < v_end && j + 1 < C && a.valid && b.valid;  // R12
       // ---- segment record in (major, minor) coordinates; every formula below is symmetric in x/y
       uint32_t n_steps = 0;
       if (seg) {
@@ -126,43 +154,59 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
         const float aM = q0.x, aN = q0.y, dM = q0.z, dN = q0.w;
         const float dd = q1.x, ext = q1.y, az = q1.z, dz = q1.w;
         const uint32_t key = __float_as_uint(q3.x);
+        const bool ymajor = (key >> 31) != 0;
         const int c = __float_as_int(q2.z) + (int)step;
         const int r0 = (int)(__float_as_uint(q2.w) >> 16), r1 = (int)(__float_as_uint(q2.w) & 0xFFFFu);
         // minor-axis extent of the segment inside column [c, c+1] (superset, ENUM_EPS slack)
         const float fc = (float)c, bMa = aM + dM;
-        const float lo = fmaxf(fc, fminf(aM, bMa)), hi = fminf(fc + 1.f, fmaxf(aM, bMa));
-        const float m0 = aN + (lo - aM) * q2.y, m1 = aN + (hi - aM) * q2.y;
+        const float lo_ = fmaxf(fc, fminf(aM, bMa)), hi_ = fminf(fc + 1.f, fmaxf(aM, bMa));
+        const float m0 = aN + (lo_ - aM) * q2.y, m1 = aN + (hi_ - aM) * q2.y;
         const int rlo = max((int)ceilf(fminf(m0, m1) - ENUM_EPS) - 1, r0);
         const int rhi = min((int)floorf(fmaxf(m0, m1) + ENUM_EPS), r1);
         const float cM = fc + 0.5f;
         const float uM = xsub(cM, aM);
-        for (int r = rlo; r <= rhi; ++r) {
-          // DESIGN.md R10/R11 in fixed-order fp32 (x/y-symmetric, so evaluated in major/minor order)
-          const float cN = (float)r + 0.5f;
-          const float uN = xsub(cN, aN);
-          const float cr = fabsf(xsub(xmul(dM, uN), xmul(dN, uM)));
-          if (!(cr <= ext)) continue;
-          float tt = 0.f;
-          if (dd > 0.f) tt = fminf(fmaxf(xdiv(xadd(xmul(uM, dM), xmul(uN, dN)), dd), 0.f), 1.f);
-          const float zn = xadd(az, xmul(tt, dz));
-          if (zn < 0.f || zn > 1.f) continue;
-          const float eM = xsub(cM, xadd(aM, xmul(tt, dM))), eN = xsub(cN, xadd(aN, xmul(tt, dN)));
-          const bool centre = xadd(xmul(eM, eM), xmul(eN, eN)) <= q2.x;
-          const unsigned long long word = pack_word(zn, (key >> 7) & 0xFFFFFFu, key & 0x7Fu, tt);
-          const int x = (key >> 31) ? r : c, y = (key >> 31) ? c : r;
-          unsigned long long* px = gbuf + ((size_t)y * W + x) * 2;
-          const ulonglong2 cur = __ldcg(reinterpret_cast<const ulonglong2*>(px));
-          if (COUNT) {
-            ++c_cons;
-            c_center += centre ? 1u : 0u;
+        // pixel (c, r) in major/minor order -> word pair address; stride of one minor step
+        const size_t pstep = ymajor ? 2 : (size_t)2 * W;
+        unsigned long long* pcol = gbuf + (ymajor ? (size_t)c * W * 2 : (size_t)c * 2);
+        for (int rb = rlo; rb <= rhi; rb += ROW_BATCH) {
+          // pass 1: the cheap half of the conservative predicate (R10), then request the words
+          bool ok[ROW_BATCH];
+          ulonglong2 cur[ROW_BATCH];
+#pragma unroll
+          for (int i = 0; i < ROW_BATCH; ++i) {
+            const int r = rb + i;
+            const float uN = xsub((float)r + 0.5f, aN);
+            const float cr = fabsf(xsub(xmul(dM, uN), xmul(dN, uM)));
+            ok[i] = r <= rhi && cr <= ext;
+            if (ok[i]) cur[i] = __ldcg(reinterpret_cast<const ulonglong2*>(pcol + (size_t)r * pstep));
           }
-          if (word < cur.y) {
-            atomicMin(px + 1, word);
-            if (COUNT) ++c_issued;
-          }
-          if (centre && word < cur.x) {
-            atomicMin(px, word);
-            if (COUNT) ++c_issued;
+          // pass 2: closest point, depth, centre predicate, word (R10/R11, fixed-order fp32; x/y-symmetric)
+#pragma unroll
+          for (int i = 0; i < ROW_BATCH; ++i) {
+            if (!ok[i]) continue;
+            const int r = rb + i;
+            const float cN = (float)r + 0.5f;
+            const float uN = xsub(cN, aN);
+            float tt = 0.f;
+            if (dd > 0.f) tt = fminf(fmaxf(xdiv(xadd(xmul(uM, dM), xmul(uN, dN)), dd), 0.f), 1.f);
+            const float zn = xadd(az, xmul(tt, dz));
+            if (zn < 0.f || zn > 1.f) continue;
+            const float eM = xsub(cM, xadd(aM, xmul(tt, dM))), eN = xsub(cN, xadd(aN, xmul(tt, dN)));
+            const bool centre = xadd(xmul(eM, eM), xmul(eN, eN)) <= q2.x;
+            const unsigned long long word = pack_word(zn, (key >> 7) & 0xFFFFFFu, key & 0x7Fu, tt);
+            unsigned long long* px = pcol + (size_t)r * pstep;
+            if (COUNT) {
+              ++c_cons;
+              c_center += centre ? 1u : 0u;
+            }
+            if (word < cur[i].y) {
+              atomicMin(px + 1, word);
+              if (COUNT) ++c_issued;
+            }
+            if (centre && word < cur[i].x) {
+              atomicMin(px, word);
+              if (COUNT) ++c_issued;
+            }
           }
         }
       }
@@ -199,14 +243,20 @@ void launch_clear(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st) {
   k_clear<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels);
 }
 
-void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const float4* vertices,
-                   CamDev cam, float rho_default, unsigned long long* gbuf, unsigned long long* counters,
-                   bool count, int n_sm, cudaStream_t st) {
-  uint32_t grid = (uint32_t)n_sm * 4;
-  uint32_t need = (n_bi + RAS_WARPS - 1) / RAS_WARPS;
-  if (grid > need) grid = need;
-  if (count) k_raster<true><<<grid, RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, vertices, cam, rho_default, gbuf, counters);
-  else k_raster<false><<<grid, RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, vertices, cam, rho_default, gbuf, counters);
+void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
+                   const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
+                   unsigned long long* counters, bool count, int n_sm, cudaStream_t st) {
+  // persistent grid: every CTA slot of the device, the queue feeds them
+  static int per_sm[2] = {0, 0};
+  if (!per_sm[count]) {
+    int b = 0;
+    if (count) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<true>, RAS_WARPS * 32, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<false>, RAS_WARPS * 32, 0);
+    per_sm[count] = b > 0 ? b : 1;
+  }
+  const uint32_t grid = (uint32_t)(n_sm * per_sm[count]);
+  if (count) k_raster<true><<<grid, RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters);
+  else k_raster<false><<<grid, RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters);
 }
 
 // ------------------------------------------------------------------ L2-atomic roofline micro-kernels

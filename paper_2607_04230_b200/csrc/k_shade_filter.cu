@@ -93,124 +93,233 @@ __device__ __forceinline__ float2 screen_tangent(const SceneDev* __restrict__ sc
   return make_float2(xdiv(dx, len), xdiv(dy, len));
 }
 
+// ---------------------------------------------------------------------------------------- H7
+// Tiled filter. One CTA owns a 32x16 pixel tile: (1) the tile + an r-pixel halo of the G-buffer
+// (as two 24-bit depths, "none" = DQ_NONE) and of the shaded colour go to shared memory once,
+// (2) every hit pixel emits one or two work items (reference tangent, reference depth, colour
+// mode; two for a fly-away pixel), compacted through a shared counter so sparse tiles still fill
+// their warps, (3) the items are spread over the 256 threads, each walking the (2r+1)^2 window in
+// shared memory, (4) the owning thread combines its items and writes out_rgb.
+// Exact parts (decide integers, must match the oracle bit for bit): sample class by integer depth
+// compare (R20) and the strip membership of Eq. 9 / PAPER.md:176 — the latter is only evaluated in
+// fixed-order fp32 for taps whose fast cross product says they are within 0.01 px of the strip
+// edge or inside; sqrt_rn(e2) <= w_strip is tested as e2 <= strip_e2_max (host: the largest float
+// whose correctly rounded root is <= w_strip; sqrt_rn is monotone). Everything else is fast fp32:
+// the exponent of Eq. 10 is the quadratic form a dx^2 + b dx dy + c dy^2 of the window offset
+// (2 FMA per tap), the colour distance is |CP|^2 + |CQ|^2 - 2 CP.CQ with |CQ|^2 kept per tile pixel,
+// all pre-multiplied by log2(e) so that one ex2.approx gives the weight.
+#define FT_W 32
+#define FT_H 16
+#define DQ_NONE 0x40000000u
+
 struct Acc {
   float r, g, b, alpha;
 };
 
-// One pass over the (2r+1)^2 window around (px, py) for the reference sample (T, dq_ref)
-// (Code 2 PAPER.md:483-515 with DESIGN.md R18-R20).
-__device__ __forceinline__ Acc accumulate(const ShadeParams& sp, const unsigned long long* __restrict__ gbuf,
-                                          const float4* __restrict__ colour, int W, int H, int px, int py,
-                                          float2 T, uint32_t dq_ref, bool use_colour, float4 CP) {
-  float S0 = 0.f, S1 = 0.f, S2 = 0.f, Wsum = 0.f, emax = -INFINITY;
-  uint32_t Hc = 0, Ha = 0;
-  const int r = sp.r;
-  for (int dy = -r; dy <= r; ++dy) {
-    const int qy = py + dy;
-    if (qy < 0 || qy >= H) continue;
-    for (int dx = -r; dx <= r; ++dx) {
-      const int qx = px + dx;
-      if (qx < 0 || qx >= W) continue;
-      const size_t q = (size_t)qy * W + qx;
-      const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + q);
-      // R20: class by integer depth compare; an empty word has dq = 0xFFFFFF, never within tau of a hit
-      const uint32_t dG = raw.y >> 8, dA = raw.w >> 8;
-      const bool cG = (raw.x & raw.y) != 0xFFFFFFFFu && (dG > dq_ref ? dG - dq_ref : dq_ref - dG) <= sp.tauz_q;
-      const bool cA = (raw.z & raw.w) != 0xFFFFFFFFu && (dA > dq_ref ? dA - dq_ref : dq_ref - dA) <= sp.tauz_q;
-      if (!cG && !cA) continue;
-      // Eq. 9, fixed-order fp32
-      const float fdx = (float)dx, fdy = (float)dy;
-      const float dpar = xadd(xmul(fdx, T.x), xmul(fdy, T.y));
-      const float ex = xsub(fdx, xmul(dpar, T.x)), ey = xsub(fdy, xmul(dpar, T.y));
-      const float dperp = xsqrt(xadd(xmul(ex, ex), xmul(ey, ey)));
-      if (dperp <= sp.w_strip) {
-        if (cG) ++Hc;
-        else ++Ha;
-      }
-      if (cG) {  // R19
-        float e = -dpar * dpar * sp.inv_sp2 - dperp * dperp * sp.inv_sq2;
-        const float4 CQ = __ldg(&colour[q]);
-        if (use_colour) {
-          const float d0 = CP.x - CQ.x, d1 = CP.y - CQ.y, d2 = CP.z - CQ.z;
-          e -= (d0 * d0 + d1 * d1 + d2 * d2) * sp.inv_sc2;  // Eq. 10
-        }
-        // normalised sum with a running maximum exponent (online softmax): Eq. 10's ratio is unchanged,
-        // but weights of e^-90 (5 px across the strand) no longer underflow to denormals / 0
-        if (e > emax) {
-          const float sc_ = __expf(emax - e);
-          S0 *= sc_, S1 *= sc_, S2 *= sc_, Wsum *= sc_;
-          emax = e;
-        }
-        const float w = __expf(e - emax);
-        S0 += w * CQ.x;
-        S1 += w * CQ.y;
-        S2 += w * CQ.z;
-        Wsum += w;
-      }
-    }
-  }
-  Acc o;
-  const float inv = Wsum > 0.f ? 1.0f / Wsum : 0.f;
-  o.r = S0 * inv;
-  o.g = S1 * inv;
-  o.b = S2 * inv;
-  o.alpha = (Hc + Ha) > 0 ? (float)Hc / (float)(Hc + Ha) : 0.f;
-  return o;
+__device__ __forceinline__ float fast_ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 
-template <bool COUNT>
+// Eq. 9 in the oracle's operation order; true iff sqrt_rn(e2) <= w_strip
+__device__ __forceinline__ bool in_strip_exact(float fdx, float fdy, float Tx, float Ty, float e2_max) {
+  const float dpar = xadd(xmul(fdx, Tx), xmul(fdy, Ty));
+  const float ex = xsub(fdx, xmul(dpar, Tx)), ey = xsub(fdy, xmul(dpar, Ty));
+  return xadd(xmul(ex, ex), xmul(ey, ey)) <= e2_max;
+}
+
+template <int R>
 __global__ void __launch_bounds__(256)
 k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const float4* __restrict__ vertices,
          CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, const float4* __restrict__ colour,
-         float4* __restrict__ out, unsigned long long* __restrict__ counters) {
+         float4* __restrict__ out) {
+  constexpr int SW = FT_W + 2 * R, SH = FT_H + 2 * R, NS = SW * SH;
+  extern __shared__ float4 fsm[];
+  float4* s_col = fsm;                                  // [NS] rgb, -kC |rgb|^2
+  float4* s_item = fsm + NS;                            // [2 * FT_W * FT_H] item, later its result
+  uint2* s_dq = reinterpret_cast<uint2*>(s_item + 2 * FT_W * FT_H);  // [NS] dq centre, dq conservative
+  __shared__ uint32_t s_n;
   const int W = (int)cam.W, H = (int)cam.H;
-  const int px = blockIdx.x * 32 + (threadIdx.x & 31), py = blockIdx.y * 8 + (threadIdx.x >> 5);
-  const bool inside = px < W && py < H;
-  unsigned long long G = HAIR_EMPTY, A = HAIR_EMPTY;
-  size_t p = 0;
-  if (inside) {
-    p = (size_t)py * W + px;
-    const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
-    G = ((unsigned long long)raw.y << 32) | raw.x;
-    A = ((unsigned long long)raw.w << 32) | raw.z;
-  }
-  const bool isCenter = G != HAIR_EMPTY, isCons = A != HAIR_EMPTY;
-  if (COUNT) {
-    const uint32_t nc = __popc(__ballot_sync(0xffffffffu, isCenter)), na = __popc(__ballot_sync(0xffffffffu, isCons));
-    if ((threadIdx.x & 31) == 0) {
-      if (nc) atomicAdd(&counters[CNT_PX_CENTER], (unsigned long long)nc);
-      if (na) atomicAdd(&counters[CNT_PX_CONS], (unsigned long long)na);
+  const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
+  const int x0 = blockIdx.x * FT_W, y0 = blockIdx.y * FT_H;
+  if (tid == 0) s_n = 0;
+  // ---- own two pixels (rows ly and ly + 8 of the tile)
+  unsigned long long G[2], A[2];
+  bool inside[2];
+  int hit = 0;
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const int px = x0 + lx, py = y0 + ly + 8 * k;
+    inside[k] = px < W && py < H;
+    G[k] = A[k] = HAIR_EMPTY;
+    if (inside[k]) {
+      const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + (size_t)py * W + px);
+      G[k] = ((unsigned long long)raw.y << 32) | raw.x;
+      A[k] = ((unsigned long long)raw.w << 32) | raw.z;
     }
+    hit |= A[k] != HAIR_EMPTY;  // centre layer is a subset of the conservative one (R10)
   }
-  if (!inside) return;
-  float r = 0.f, g = 0.f, b = 0.f, alpha = 0.f;
-  if (!sp.filter_on) {
+  const float4 bg = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
+  if (!__syncthreads_or(hit)) {  // empty tile: background only
+#pragma unroll
+    for (int k = 0; k < 2; ++k)
+      if (inside[k]) out[(size_t)(y0 + ly + 8 * k) * W + x0 + lx] = bg;
+    return;
+  }
+  // ---- (1) tile + halo to shared memory
+  for (int i = tid; i < NS; i += 256) {
+    const int sy = i / SW, sx = i - sy * SW;
+    const int gx = x0 + sx - R, gy = y0 + sy - R;
+    uint2 d = make_uint2(DQ_NONE, DQ_NONE);
+    if (gx >= 0 && gx < W && gy >= 0 && gy < H) {  // samples outside the image do not exist
+      const size_t q = (size_t)gy * W + gx;
+      const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + q);
+      if ((raw.z & raw.w) != 0xFFFFFFFFu) d.y = raw.w >> 8;
+      if ((raw.x & raw.y) != 0xFFFFFFFFu) {
+        d.x = raw.y >> 8;
+        const float4 c = __ldg(&colour[q]);
+        s_col[i] = make_float4(c.x, c.y, c.z, -sp.kC * (c.x * c.x + c.y * c.y + c.z * c.z));
+      }
+    }
+    s_dq[i] = d;
+  }
+  // ---- (2) work items
+  int slot_c[2] = {-1, -1}, slot_a[2] = {-1, -1};
+  bool fly[2] = {false, false};
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const bool isCenter = G[k] != HAIR_EMPTY, isCons = A[k] != HAIR_EMPTY;
+    const uint32_t pix = (uint32_t)((ly + 8 * k) * FT_W + lx);
     if (isCenter) {
-      const float4 CP = __ldg(&colour[p]);
-      r = CP.x, g = CP.y, b = CP.z, alpha = 1.f;
+      const float2 T = screen_tangent(sc, table, vertices, cam, G[k]);
+      slot_c[k] = (int)atomicAdd(&s_n, 1u);
+      s_item[slot_c[k]] = make_float4(T.x, T.y, __uint_as_float(w_dq(G[k]) | 0x1000000u), __uint_as_float(pix));
+      fly[k] = isCons && w_dq(G[k]) >= w_dq(A[k]) && w_dq(G[k]) - w_dq(A[k]) >= sp.taufly_q;  // PAPER.md:175, R21
     }
-  } else if (isCenter) {
-    const float4 CP = __ldg(&colour[p]);
-    const float2 TG = screen_tangent(sc, table, vertices, cam, G);
-    Acc a = accumulate(sp, gbuf, colour, W, H, px, py, TG, w_dq(G), true, CP);
-    r = a.r, g = a.g, b = a.b, alpha = a.alpha;
-    // fly-away strand in front of the centre hit (R21)
-    if (isCons && w_dq(G) >= w_dq(A) && w_dq(G) - w_dq(A) >= sp.taufly_q) {
-      const float2 TA = screen_tangent(sc, table, vertices, cam, A);
-      Acc f = accumulate(sp, gbuf, colour, W, H, px, py, TA, w_dq(A), false, CP);
-      r = f.alpha * f.r + (1.f - f.alpha) * a.r;
-      g = f.alpha * f.g + (1.f - f.alpha) * a.g;
-      b = f.alpha * f.b + (1.f - f.alpha) * a.b;
-      alpha = 1.f;
+    if (fly[k] || (isCons && !isCenter)) {  // fly-away strand, or promoted pixel: w_color = 1
+      const float2 T = screen_tangent(sc, table, vertices, cam, A[k]);
+      slot_a[k] = (int)atomicAdd(&s_n, 1u);
+      s_item[slot_a[k]] = make_float4(T.x, T.y, __uint_as_float(w_dq(A[k])), __uint_as_float(pix));
     }
-  } else if (isCons) {  // promoted pixel: w_color = 1
-    const float2 TA = screen_tangent(sc, table, vertices, cam, A);
-    Acc a = accumulate(sp, gbuf, colour, W, H, px, py, TA, w_dq(A), false, make_float4(0.f, 0.f, 0.f, 0.f));
-    r = a.r, g = a.g, b = a.b, alpha = a.alpha;
   }
-  const float ia = 1.f - alpha;  // R29: composite over the background
-  out[p] = make_float4(alpha * r + ia * sp.background[0], alpha * g + ia * sp.background[1],
-                       alpha * b + ia * sp.background[2], alpha);
+  __syncthreads();
+  // ---- (3) one window walk per item (Code 2 PAPER.md:483-515 with DESIGN.md R18-R20)
+  const int n_item = (int)s_n;
+  const uint32_t tau = sp.tauz_q, tau2 = 2u * sp.tauz_q;
+  for (int it = tid; it < n_item; it += 256) {
+    const float4 I = s_item[it];
+    const float Tx = I.x, Ty = I.y;
+    const uint32_t rm = __float_as_uint(I.z), pix = __float_as_uint(I.w);
+    const uint32_t lo = (rm & 0xFFFFFFu) - tau;  // may wrap: the compare below is modulo 2^32
+    const float m = (rm >> 24) ? 1.f : 0.f;  // 1: bilateral colour term on (centre sample)
+    const int ci = ((int)(pix >> 5) + R) * SW + (int)(pix & 31u) + R;
+    // exponent (base 2) of the spatial weight as a quadratic form of (dx, dy)
+    const float qa = sp.kP * Tx * Tx + sp.kQ * Ty * Ty, qb = 2.f * (sp.kP - sp.kQ) * Tx * Ty,
+                qc = sp.kP * Ty * Ty + sp.kQ * Tx * Tx;
+    float c2x = 0.f, c2y = 0.f, c2z = 0.f, e0 = sp.bias_nc;
+    if (rm >> 24) {  // the centre tap has weight 1, so no bias is needed
+      const float4 CP = s_col[ci];
+      c2x = 2.f * sp.kC * CP.x, c2y = 2.f * sp.kC * CP.y, c2z = 2.f * sp.kC * CP.z;
+      e0 = CP.w;
+    }
+    float S0 = 0.f, S1 = 0.f, S2 = 0.f, Wsum = 0.f;
+    uint32_t Hc = 0, Ha = 0;
+#pragma unroll 1
+    for (int dy = -R; dy <= R; ++dy) {
+      const float fdy = (float)dy;
+      const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy, rc = -fdy * Tx;
+      const uint2* dq_row = s_dq + ci + dy * SW;
+      const float4* col_row = s_col + ci + dy * SW;
+#pragma unroll
+      for (int dx = -R; dx <= R; ++dx) {
+        const uint2 d = dq_row[dx];
+        // R20: class by integer depth compare, |d - ref| <= tau as (unsigned)(d - (ref - tau)) <= 2 tau;
+        // DQ_NONE is farther than tau (<= 2^24) from every depth
+        const bool cG = d.x - lo <= tau2, cA = d.y - lo <= tau2;
+        if (!(cG || cA)) continue;
+        const float fdx = (float)dx;
+        const float cross = fmaf(fdx, Ty, rc);  // ~ signed distance of the tap to the tangent line
+        if (fabsf(cross) <= sp.strip_loose && in_strip_exact(fdx, fdy, Tx, Ty, sp.strip_e2_max)) {
+          if (cG) ++Hc;
+          else ++Ha;
+        }
+        if (cG) {  // R19
+          const float4 q = col_row[dx];
+          float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));                     // Eq. 10 spatial part
+          e = fmaf(c2x, q.x, fmaf(c2y, q.y, fmaf(c2z, q.z, fmaf(m, q.w, e))));  // Eq. 10 colour part
+          const float w = fast_ex2(e);
+          S0 = fmaf(w, q.x, S0);
+          S1 = fmaf(w, q.y, S1);
+          S2 = fmaf(w, q.z, S2);
+          Wsum += w;
+        }
+      }
+    }
+    const float inv = Wsum > 0.f ? 1.0f / Wsum : 0.f;
+    const float alpha = (Hc + Ha) > 0 ? (float)Hc / (float)(Hc + Ha) : 0.f;
+    s_item[it] = make_float4(S0 * inv, S1 * inv, S2 * inv, alpha);
+  }
+  __syncthreads();
+  // ---- (4) combine and composite over the background (R29)
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    if (!inside[k]) continue;
+    float r = 0.f, g = 0.f, b = 0.f, alpha = 0.f;
+    if (slot_c[k] >= 0) {
+      const float4 a = s_item[slot_c[k]];
+      r = a.x, g = a.y, b = a.z, alpha = a.w;
+      if (fly[k]) {  // R21
+        const float4 f = s_item[slot_a[k]];
+        r = f.w * f.x + (1.f - f.w) * a.x;
+        g = f.w * f.y + (1.f - f.w) * a.y;
+        b = f.w * f.z + (1.f - f.w) * a.z;
+        alpha = 1.f;
+      }
+    } else if (slot_a[k] >= 0) {
+      const float4 a = s_item[slot_a[k]];
+      r = a.x, g = a.y, b = a.z, alpha = a.w;
+    }
+    const float ia = 1.f - alpha;
+    out[(size_t)(y0 + ly + 8 * k) * W + x0 + lx] =
+        make_float4(alpha * r + ia * bg.x, alpha * g + ia * bg.y, alpha * b + ia * bg.z, alpha);
+  }
+}
+
+// filter off, or r = 0 (window = the pixel itself): out = centre colour over the background
+__global__ void __launch_bounds__(256)
+k_filter_passthrough(CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf,
+                     const float4* __restrict__ colour, float4* __restrict__ out) {
+  const size_t n_px = (size_t)cam.W * cam.H;
+  const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n_px) return;
+  const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
+  float4 o = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
+  if ((raw.x & raw.y) != 0xFFFFFFFFu) {
+    const float4 c = __ldg(&colour[p]);
+    o = make_float4(c.x, c.y, c.z, 1.f);
+  }
+  out[p] = o;
+}
+
+// hair_stats: non-empty pixels per layer (counters flag only)
+__global__ void __launch_bounds__(256)
+k_count_pixels(const unsigned long long* __restrict__ gbuf, size_t n_px, unsigned long long* __restrict__ counters) {
+  uint32_t nc = 0, na = 0;
+  for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n_px; p += (size_t)gridDim.x * blockDim.x) {
+    const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
+    nc += (raw.x & raw.y) != 0xFFFFFFFFu;
+    na += (raw.z & raw.w) != 0xFFFFFFFFu;
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    nc += __shfl_xor_sync(0xffffffffu, nc, d);
+    na += __shfl_xor_sync(0xffffffffu, na, d);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    if (nc) atomicAdd(&counters[CNT_PX_CENTER], (unsigned long long)nc);
+    if (na) atomicAdd(&counters[CNT_PX_CONS], (unsigned long long)na);
+  }
 }
 
 void launch_shade(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
@@ -219,10 +328,39 @@ void launch_shade(const SceneDev* d_scene, const uint4* table, const float4* ver
   k_shade<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, table, vertices, cam, sp, gbuf, colour);
 }
 
-void launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
-                   ShadeParams sp, const unsigned long long* gbuf, const float4* colour, float4* out,
-                   unsigned long long* counters, bool count, cudaStream_t st) {
-  dim3 grid((cam.W + 31) / 32, (cam.H + 7) / 8);
-  if (count) k_filter<true><<<grid, 256, 0, st>>>(d_scene, table, vertices, cam, sp, gbuf, colour, out, counters);
-  else k_filter<false><<<grid, 256, 0, st>>>(d_scene, table, vertices, cam, sp, gbuf, colour, out, counters);
+template <int R>
+static void launch_filter_r(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+                            ShadeParams sp, const unsigned long long* gbuf, const float4* colour, float4* out,
+                            cudaStream_t st) {
+  constexpr int NS = (FT_W + 2 * R) * (FT_H + 2 * R);
+  constexpr size_t smem = (size_t)NS * (sizeof(float4) + sizeof(uint2)) + 2 * FT_W * FT_H * sizeof(float4);
+  cudaFuncSetAttribute(k_filter<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  dim3 grid((cam.W + FT_W - 1) / FT_W, (cam.H + FT_H - 1) / FT_H);
+  k_filter<R><<<grid, 256, smem, st>>>(d_scene, table, vertices, cam, sp, gbuf, colour, out);
+}
+
+int launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+                  ShadeParams sp, const unsigned long long* gbuf, const float4* colour, float4* out,
+                  unsigned long long* counters, bool count, cudaStream_t st) {
+  const size_t n = (size_t)cam.W * cam.H;
+  int launches = 1;
+  if (count) {
+    k_count_pixels<<<148 * 8, 256, 0, st>>>(gbuf, n, counters);
+    ++launches;
+  }
+  if (!sp.filter_on) {
+    k_filter_passthrough<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cam, sp, gbuf, colour, out);
+    return launches;
+  }
+  switch (sp.r) {
+    case 0: launch_filter_r<0>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
+    case 1: launch_filter_r<1>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
+    case 2: launch_filter_r<2>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
+    case 3: launch_filter_r<3>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
+    case 4: launch_filter_r<4>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
+    case 5: launch_filter_r<5>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
+    case 6: launch_filter_r<6>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
+    default: launch_filter_r<7>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
+  }
+  return launches;
 }
