@@ -291,7 +291,7 @@ def run_cuda(args):
         "roofline": roofline, "stages": stages, "l2_atomic_peaks_Gatom_per_s": atom,
         "hbm_peak_GBps": hbm_peak, "hbm_peak_source": hbm_src,
         "counts": {k: cnt[k] for k in ("n_bundles", "n_bundles_culled", "n_strands_total", "n_strands_lod", "n_vertices",
-                                       "n_segments", "n_segments_drawn", "n_atomics_center", "n_atomics_cons",
+                                       "n_segments", "n_segments_drawn", "n_segments_live", "n_atomics_center", "n_atomics_cons",
                                        "n_atomics_issued", "n_pixels_center", "n_pixels_cons")},
         "cpu_baseline": cpu_baseline, "clocks": clocks,
     }

@@ -129,6 +129,7 @@ typedef struct {
   uint32_t n_strands_total, n_strands_lod;
   uint32_t n_vertices, n_segments;
   uint32_t n_segments_drawn;               /* both endpoints in front of the near plane (counters flag) */
+  uint32_t n_segments_live;                /* segments that won at least one pixel test when drawn (counters flag) */
   uint64_t n_atomics_center, n_atomics_cons; /* predicate-true hits before any filtering (counters flag) */
   uint64_t n_atomics_issued;               /* atomics actually sent to L2 (counters flag) */
   uint32_t n_pixels_center, n_pixels_cons; /* non-empty pixels after the frame (counters flag) */

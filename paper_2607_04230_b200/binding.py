@@ -66,6 +66,7 @@ class hair_stats_t(C.Structure):
     _fields_ = [("n_grooms", C.c_uint32), ("n_bundles", C.c_uint32), ("n_bundles_culled", C.c_uint32),
                 ("n_strands_total", C.c_uint32), ("n_strands_lod", C.c_uint32),
                 ("n_vertices", C.c_uint32), ("n_segments", C.c_uint32), ("n_segments_drawn", C.c_uint32),
+                ("n_segments_live", C.c_uint32),
                 ("n_atomics_center", C.c_uint64), ("n_atomics_cons", C.c_uint64), ("n_atomics_issued", C.c_uint64),
                 ("n_pixels_center", C.c_uint32), ("n_pixels_cons", C.c_uint32),
                 ("ms_lod", C.c_float), ("ms_generate", C.c_float), ("ms_clear", C.c_float),

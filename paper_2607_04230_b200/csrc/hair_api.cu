@@ -522,6 +522,7 @@ int hair_stats(hair_ctx* c, hair_stats_t* out) {
     out->n_atomics_center = k[CNT_AT_CENTER];
     out->n_atomics_cons = k[CNT_AT_CONS];
     out->n_atomics_issued = k[CNT_AT_ISSUED];
+    out->n_segments_live = (uint32_t)k[CNT_SEG_LIVE];
     out->n_pixels_center = (uint32_t)k[CNT_PX_CENTER];
     out->n_pixels_cons = (uint32_t)k[CNT_PX_CONS];
   }

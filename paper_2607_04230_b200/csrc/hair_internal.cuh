@@ -72,6 +72,7 @@ enum {
   CNT_AT_CENTER,
   CNT_AT_CONS,
   CNT_AT_ISSUED,
+  CNT_SEG_LIVE,      // segments that sent at least one atomic (the rest lost every pixel to nearer hair)
   CNT_PX_CENTER,
   CNT_PX_CONS,
   CNT_N

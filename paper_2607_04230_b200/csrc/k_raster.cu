@@ -43,7 +43,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
   __shared__ __align__(16) float s_rec[RAS_WARPS][32][REC_STRIDE];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float(*rec)[REC_STRIDE] = s_rec[warp];
-  uint32_t c_center = 0, c_cons = 0, c_drawn = 0, c_issued = 0;
+  uint32_t c_center = 0, c_cons = 0, c_drawn = 0, c_issued = 0, c_live = 0;
   const int W = (int)cam.W, H = (int)cam.H;
   const uint32_t le_mask = 0xFFFFFFFFu >> (31 - lane);
   const uint32_t n_groups = __ldcg(&grp[n_bi]);
@@ -125,6 +125,10 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
           r4[2] = make_float4(xmul(rho, rho), dM != 0.f ? dN / dM : 0.f, __int_as_float((int)fc0),
                               __uint_as_float(((uint32_t)(int)fr0 << 16) | (uint32_t)(int)fr1));
           r4[3].x = __uint_as_float((ymajor ? 0x80000000u : 0u) | ((sid0 + k) << 7) | j);
+          // nearest depth any pixel of this segment can store, minus 2 steps for the rounding of R11's lerp
+          const uint32_t dqm = quant_depth(fminf(fmaxf(fminf(a.zn, b.zn), 0.f), 1.f));
+          r4[3].w = __uint_as_float(dqm > 2u ? dqm - 2u : 0u);
+          if (COUNT) rec[lane][16] = 0.f;
         }
       }
       // ---- spread (segment, column) tasks over the lanes
@@ -153,7 +157,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
         const float4 q0 = r4[0], q1 = r4[1], q2 = r4[2];
         const float aM = q0.x, aN = q0.y, dM = q0.z, dN = q0.w;
         const float dd = q1.x, ext = q1.y, az = q1.z, dz = q1.w;
-        const uint32_t key = __float_as_uint(q3.x);
+        const uint32_t key = __float_as_uint(q3.x), dq_min = __float_as_uint(q3.w);
         const bool ymajor = (key >> 31) != 0;
         const int c = __float_as_int(q2.z) + (int)step;
         const int r0 = (int)(__float_as_uint(q2.w) >> 16), r1 = (int)(__float_as_uint(q2.w) & 0xFFFFu);
@@ -184,6 +188,9 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
 #pragma unroll
           for (int i = 0; i < ROW_BATCH; ++i) {
             if (!ok[i]) continue;
+            // early reject: centre word >= conservative word (R10), so a segment that lies entirely behind
+            // the pixel's centre hit loses both layers whatever its exact depth at this pixel
+            if (!COUNT && dq_min > (uint32_t)(cur[i].x >> 40)) continue;
             const int r = rb + i;
             const float cN = (float)r + 0.5f;
             const float uN = xsub(cN, aN);
@@ -201,16 +208,17 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
             }
             if (word < cur[i].y) {
               atomicMin(px + 1, word);
-              if (COUNT) ++c_issued;
+              if (COUNT) ++c_issued, rec[s][16] = 1.f;
             }
             if (centre && word < cur[i].x) {
               atomicMin(px, word);
-              if (COUNT) ++c_issued;
+              if (COUNT) ++c_issued, rec[s][16] = 1.f;
             }
           }
         }
       }
       __syncwarp();
+      if (COUNT && n_steps && rec[lane][16] != 0.f) ++c_live;
     }
   }
   if (COUNT) {
@@ -220,12 +228,14 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
       c_cons += __shfl_xor_sync(0xffffffffu, c_cons, d);
       c_drawn += __shfl_xor_sync(0xffffffffu, c_drawn, d);
       c_issued += __shfl_xor_sync(0xffffffffu, c_issued, d);
+      c_live += __shfl_xor_sync(0xffffffffu, c_live, d);
     }
     if (lane == 0) {
       atomicAdd(&counters[CNT_AT_CENTER], (unsigned long long)c_center);
       atomicAdd(&counters[CNT_AT_CONS], (unsigned long long)c_cons);
       atomicAdd(&counters[CNT_SEG_DRAWN], (unsigned long long)c_drawn);
       atomicAdd(&counters[CNT_AT_ISSUED], (unsigned long long)c_issued);
+      atomicAdd(&counters[CNT_SEG_LIVE], (unsigned long long)c_live);
     }
   }
 }

@@ -39,6 +39,14 @@ def gpu_frame(binding, sc, lam=None, flags=0, prm_over=None):
     h.set_render_params(prm, flags=flags | binding.FLAG_COUNTERS)
     gb, rgb = h.render(sc["camera"], sc["lam"] if lam is None else lam)
     st = h.stats()
+    # the production kernels (no counters: per-pixel early reject on) must give the very same frame
+    gb_c, rgb_c = gb.clone(), rgb.clone()
+    h.set_render_params(prm, flags=flags)
+    gb, rgb = h.render(sc["camera"], sc["lam"] if lam is None else lam)
+    import torch
+    assert torch.equal(gb, gb_c), "G-buffer differs between the counted and the production raster"
+    assert torch.equal(rgb, rgb_c)
+    assert h.stats()["gpu_launches"] == st["gpu_launches"] - 1
     out = dict(h=h, gb=binding.gbuffer_to_numpy(gb), rgb=rgb.cpu().numpy().astype(np.float64), stats=st,
                table=h.debug_table().cpu().numpy().view(np.uint32), verts=h.debug_vertices().cpu().numpy(), prm=prm,
                gb_t=gb, rgb_t=rgb)
