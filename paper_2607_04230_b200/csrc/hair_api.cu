@@ -123,7 +123,12 @@ ShadeParams make_shade(const hair_render_params& p) {
   s.kC = (float)(L2E / ((double)p.sigma_c * (double)p.sigma_c));
   const double e_min = ((double)s.kP + (double)s.kQ) * 2.0 * p.filter_radius * p.filter_radius;  // window corner
   s.bias_nc = (float)std::fmin(std::fmax(-0.5 * e_min, 0.0), 60.0);
-  s.strip_loose = p.w_strip + 0.01f;
+  {  // loop B of k_filter: candidates m in [ceil(y* - hmax), ceil(y* - hmax) + nc - 1] cover every integer within hmax of y*
+    const double hmax = ((double)p.w_strip + 0.01) * 1.41421357 + 1e-3;
+    s.strip_hmax = (float)hmax;
+    const double nc = std::floor(2.0 * hmax) + 1.0;
+    s.strip_nc = !(p.w_strip >= 0.f) ? 0 : (nc > 2.0 * p.filter_radius + 1.0 ? 2 * p.filter_radius + 1 : (int)nc);
+  }
   if (!(p.w_strip >= 0.f)) s.strip_e2_max = -1.f;  // Eq. 9 distance is never negative
   else if (p.w_strip > 1e6f) s.strip_e2_max = 3.0e38f;
   else {  // sqrt_rn(e2) <= w_strip  <=>  e2 <= strip_e2_max (sqrt_rn is monotone; host sqrtf is IEEE)

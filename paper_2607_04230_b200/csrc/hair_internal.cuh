@@ -54,7 +54,8 @@ struct ShadeParams {
   float kP, kQ;        // -log2(e) / sigma_par^2, -log2(e) / sigma_perp^2 (Eq. 10)
   float kC;            // log2(e) / sigma_c^2
   float bias_nc;       // exponent bias of the accumulations without colour term (keeps e^-90 weights normal)
-  float strip_loose;   // w_strip + 0.01: taps whose fast cross product is below it take the exact strip test
+  float strip_hmax;    // (w_strip + 0.01) sqrt(2) + 1e-3: reach of the strip along the tangent's minor axis
+  int strip_nc;        // integer minor offsets per major step that can lie within strip_hmax of the line
   float strip_e2_max;  // largest float e2 with sqrt_rn(e2) <= w_strip
   uint32_t tauz_q, taufly_q, filter_on;
   float rho_default;  // 0.5 * center_diameter_px

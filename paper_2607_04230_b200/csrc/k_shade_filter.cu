@@ -98,23 +98,22 @@ __device__ __forceinline__ float2 screen_tangent(const SceneDev* __restrict__ sc
 // (as two 24-bit depths, "none" = DQ_NONE) and of the shaded colour go to shared memory once,
 // (2) every hit pixel emits one or two work items (reference tangent, reference depth, colour
 // mode; two for a fly-away pixel), compacted through a shared counter so sparse tiles still fill
-// their warps, (3) the items are spread over the 256 threads, each walking the (2r+1)^2 window in
-// shared memory, (4) the owning thread combines its items and writes out_rgb.
-// Exact parts (decide integers, must match the oracle bit for bit): sample class by integer depth
-// compare (R20) and the strip membership of Eq. 9 / PAPER.md:176 — the latter is only evaluated in
-// fixed-order fp32 for taps whose fast cross product says they are within 0.01 px of the strip
-// edge or inside; sqrt_rn(e2) <= w_strip is tested as e2 <= strip_e2_max (host: the largest float
-// whose correctly rounded root is <= w_strip; sqrt_rn is monotone). Everything else is fast fp32:
-// the exponent of Eq. 10 is the quadratic form a dx^2 + b dx dy + c dy^2 of the window offset
-// (2 FMA per tap), the colour distance is |CP|^2 + |CQ|^2 - 2 CP.CQ with |CQ|^2 kept per tile pixel,
-// all pre-multiplied by log2(e) so that one ex2.approx gives the weight.
+// their warps, (3) the items are spread over the 256 threads; each item runs two branch-free loops
+// over shared memory, (4) the owning thread combines its items and writes out_rgb.
+//  loop A, Eq. 10: all (2r+1)^2 taps, one LDS.32 (centre depth) + one LDS.128
+//    (colour) per tap; the class test (R20, integer depth compare) becomes a select on the weight,
+//    so lanes never diverge. The exponent is the quadratic form a dx^2 + b dx dy + c dy^2 of the
+//    window offset (2 FMA per tap), the colour distance is |CP|^2 + |CQ|^2 - 2 CP.CQ with -kC|CQ|^2
+//    kept per tile pixel, all pre-multiplied by log2(e) so that one ex2.approx gives the weight.
+//  loop B, strip hit counts: only lattice points within w_strip of the tangent line
+//    can be in the strip, so instead of testing 121 taps the loop walks the 2r+1 steps of the
+//    tangent's major axis and tests the `strip_nc` (2 for w_strip = 0.5) integer minor offsets that
+//    can lie within (w_strip + 0.01) sqrt(2) of the line — a superset; membership itself is Eq. 9 in
+//    the oracle's fixed-order fp32 (sqrt_rn(e2) <= w_strip tested as e2 <= strip_e2_max, host-side
+//    the largest float whose correctly rounded root is <= w_strip; sqrt_rn is monotone).
 #define FT_W 32
 #define FT_H 16
 #define DQ_NONE 0x40000000u
-
-struct Acc {
-  float r, g, b, alpha;
-};
 
 __device__ __forceinline__ float fast_ex2(float x) {
   float y;
@@ -136,9 +135,10 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
          float4* __restrict__ out) {
   constexpr int SW = FT_W + 2 * R, SH = FT_H + 2 * R, NS = SW * SH;
   extern __shared__ float4 fsm[];
-  float4* s_col = fsm;                                  // [NS] rgb, -kC |rgb|^2
+  float4* s_col = fsm;                                  // [NS] rgb, -kC |rgb|^2 (zeros where no centre hit)
   float4* s_item = fsm + NS;                            // [2 * FT_W * FT_H] item, later its result
-  uint2* s_dq = reinterpret_cast<uint2*>(s_item + 2 * FT_W * FT_H);  // [NS] dq centre, dq conservative
+  uint32_t* s_dqG = reinterpret_cast<uint32_t*>(s_item + 2 * FT_W * FT_H);  // [NS] dq of the centre word
+  uint32_t* s_dqA = s_dqG + NS;                                             // [NS] dq of the conservative word
   __shared__ uint32_t s_n;
   const int W = (int)cam.W, H = (int)cam.H;
   const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
@@ -171,18 +171,21 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
   for (int i = tid; i < NS; i += 256) {
     const int sy = i / SW, sx = i - sy * SW;
     const int gx = x0 + sx - R, gy = y0 + sy - R;
-    uint2 d = make_uint2(DQ_NONE, DQ_NONE);
+    uint32_t dG = DQ_NONE, dA = DQ_NONE;
+    float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (gx >= 0 && gx < W && gy >= 0 && gy < H) {  // samples outside the image do not exist
       const size_t q = (size_t)gy * W + gx;
       const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + q);
-      if ((raw.z & raw.w) != 0xFFFFFFFFu) d.y = raw.w >> 8;
+      if ((raw.z & raw.w) != 0xFFFFFFFFu) dA = raw.w >> 8;
       if ((raw.x & raw.y) != 0xFFFFFFFFu) {
-        d.x = raw.y >> 8;
+        dG = raw.y >> 8;
         const float4 c = __ldg(&colour[q]);
-        s_col[i] = make_float4(c.x, c.y, c.z, -sp.kC * (c.x * c.x + c.y * c.y + c.z * c.z));
+        c4 = make_float4(c.x, c.y, c.z, -sp.kC * (c.x * c.x + c.y * c.y + c.z * c.z));
       }
     }
-    s_dq[i] = d;
+    s_col[i] = c4;
+    s_dqG[i] = dG;
+    s_dqA[i] = dA;
   }
   // ---- (2) work items
   int slot_c[2] = {-1, -1}, slot_a[2] = {-1, -1};
@@ -204,55 +207,65 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
     }
   }
   __syncthreads();
-  // ---- (3) one window walk per item (Code 2 PAPER.md:483-515 with DESIGN.md R18-R20)
+  // ---- (3) per item (Code 2 PAPER.md:483-515 with DESIGN.md R18-R20)
   const int n_item = (int)s_n;
   const uint32_t tau = sp.tauz_q, tau2 = 2u * sp.tauz_q;
   for (int it = tid; it < n_item; it += 256) {
     const float4 I = s_item[it];
     const float Tx = I.x, Ty = I.y;
     const uint32_t rm = __float_as_uint(I.z), pix = __float_as_uint(I.w);
-    const uint32_t lo = (rm & 0xFFFFFFu) - tau;  // may wrap: the compare below is modulo 2^32
-    const float m = (rm >> 24) ? 1.f : 0.f;  // 1: bilateral colour term on (centre sample)
+    // R20: class by integer depth compare, |d - ref| <= tau as (unsigned)(d - (ref - tau)) <= 2 tau (mod 2^32);
+    // DQ_NONE is farther than tau (<= 2^24) from every depth
+    const uint32_t lo = (rm & 0xFFFFFFu) - tau;
     const int ci = ((int)(pix >> 5) + R) * SW + (int)(pix & 31u) + R;
-    // exponent (base 2) of the spatial weight as a quadratic form of (dx, dy)
+    // ---- loop A: bilateral sum. Exponent (base 2) of the spatial weight as a quadratic form of (dx, dy)
     const float qa = sp.kP * Tx * Tx + sp.kQ * Ty * Ty, qb = 2.f * (sp.kP - sp.kQ) * Tx * Ty,
                 qc = sp.kP * Ty * Ty + sp.kQ * Tx * Tx;
-    float c2x = 0.f, c2y = 0.f, c2z = 0.f, e0 = sp.bias_nc;
-    if (rm >> 24) {  // the centre tap has weight 1, so no bias is needed
+    float c2x = 0.f, c2y = 0.f, c2z = 0.f, e0 = sp.bias_nc, m = 0.f;
+    if (rm >> 24) {  // centre sample: colour term on; its own tap has weight 1, so no bias is needed
       const float4 CP = s_col[ci];
       c2x = 2.f * sp.kC * CP.x, c2y = 2.f * sp.kC * CP.y, c2z = 2.f * sp.kC * CP.z;
       e0 = CP.w;
+      m = 1.f;
     }
     float S0 = 0.f, S1 = 0.f, S2 = 0.f, Wsum = 0.f;
-    uint32_t Hc = 0, Ha = 0;
 #pragma unroll 1
     for (int dy = -R; dy <= R; ++dy) {
       const float fdy = (float)dy;
-      const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy, rc = -fdy * Tx;
-      const uint2* dq_row = s_dq + ci + dy * SW;
+      const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy;
+      const uint32_t* dq_row = s_dqG + ci + dy * SW;
       const float4* col_row = s_col + ci + dy * SW;
 #pragma unroll
       for (int dx = -R; dx <= R; ++dx) {
-        const uint2 d = dq_row[dx];
-        // R20: class by integer depth compare, |d - ref| <= tau as (unsigned)(d - (ref - tau)) <= 2 tau;
-        // DQ_NONE is farther than tau (<= 2^24) from every depth
-        const bool cG = d.x - lo <= tau2, cA = d.y - lo <= tau2;
-        if (!(cG || cA)) continue;
+        const uint32_t d = dq_row[dx];
+        const float4 q = col_row[dx];
         const float fdx = (float)dx;
-        const float cross = fmaf(fdx, Ty, rc);  // ~ signed distance of the tap to the tangent line
-        if (fabsf(cross) <= sp.strip_loose && in_strip_exact(fdx, fdy, Tx, Ty, sp.strip_e2_max)) {
-          if (cG) ++Hc;
-          else ++Ha;
-        }
-        if (cG) {  // R19
-          const float4 q = col_row[dx];
-          float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));                     // Eq. 10 spatial part
-          e = fmaf(c2x, q.x, fmaf(c2y, q.y, fmaf(c2z, q.z, fmaf(m, q.w, e))));  // Eq. 10 colour part
-          const float w = fast_ex2(e);
-          S0 = fmaf(w, q.x, S0);
-          S1 = fmaf(w, q.y, S1);
-          S2 = fmaf(w, q.z, S2);
-          Wsum += w;
+        float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));                     // Eq. 10 spatial part
+        e = fmaf(c2x, q.x, fmaf(c2y, q.y, fmaf(c2z, q.z, fmaf(m, q.w, e))));  // Eq. 10 colour part
+        const float w = (d - lo <= tau2) ? fast_ex2(e) : 0.f;                 // R19: centre-class taps only
+        S0 = fmaf(w, q.x, S0);
+        S1 = fmaf(w, q.y, S1);
+        S2 = fmaf(w, q.z, S2);
+        Wsum += w;
+      }
+    }
+    // ---- loop B: strip hit counts by Q's class (R18)
+    const bool xmaj = fabsf(Tx) >= fabsf(Ty);
+    const float slope = xmaj ? Ty / Tx : Tx / Ty;  // |slope| <= 1; T is a unit vector, so the major part is >= 0.707
+    uint32_t Hc = 0, Ha = 0;
+#pragma unroll 1
+    for (int s = -R; s <= R; ++s) {
+      const float ystar = (float)s * slope;
+      const int m0 = max((int)ceilf(ystar - sp.strip_hmax), -R);
+      for (int c = 0; c < sp.strip_nc; ++c) {
+        const int mm = m0 + c;
+        const int dx = xmaj ? s : mm, dy = xmaj ? mm : s;
+        if (mm <= R) {
+          const int idx = ci + dy * SW + dx;
+          const bool cG = s_dqG[idx] - lo <= tau2, cA = s_dqA[idx] - lo <= tau2;
+          const bool in = in_strip_exact((float)dx, (float)dy, Tx, Ty, sp.strip_e2_max);
+          Hc += (in && cG) ? 1u : 0u;
+          Ha += (in && cA && !cG) ? 1u : 0u;
         }
       }
     }
@@ -333,7 +346,7 @@ static void launch_filter_r(const SceneDev* d_scene, const uint4* table, const f
                             ShadeParams sp, const unsigned long long* gbuf, const float4* colour, float4* out,
                             cudaStream_t st) {
   constexpr int NS = (FT_W + 2 * R) * (FT_H + 2 * R);
-  constexpr size_t smem = (size_t)NS * (sizeof(float4) + sizeof(uint2)) + 2 * FT_W * FT_H * sizeof(float4);
+  constexpr size_t smem = (size_t)NS * (sizeof(float4) + 2 * sizeof(uint32_t)) + 2 * FT_W * FT_H * sizeof(float4);
   cudaFuncSetAttribute(k_filter<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   dim3 grid((cam.W + FT_W - 1) / FT_W, (cam.H + FT_H - 1) / FT_H);
   k_filter<R><<<grid, 256, smem, st>>>(d_scene, table, vertices, cam, sp, gbuf, colour, out);
