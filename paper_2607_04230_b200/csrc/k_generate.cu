@@ -10,13 +10,18 @@
 //            the centre curve, the frame edge and every w-dependent styling scalar into a shared
 //            per-warp table. The base spline is linear in the root barycentrics
 //            (p(b) = sum_k b_k E_k), so no strand ever repeats the Hermite evaluation.
-//   stage 3  lanes = flattened (strand k, control point j) of the bundle: 3 hashes for the root, one
-//            table row, ~20 FMA for position/tangent/AO, styling, instance transform, and one
-//            coalesced 16-byte store per lane (512 B per warp instruction, strand-major).
+//   stage 3  per strand once (lanes = strands, batches of 32): 3 hashes -> root barycentrics and curl
+//            phase, to shared memory. Then lanes = flattened (strand k, control point j): strand
+//            record + table row, ~20 FMA for position/tangent/AO, styling, instance transform, and
+//            one coalesced 16-byte store per lane (512 B per warp instruction, strand-major); (k, j)
+//            advance incrementally, no division per vertex.
 // Arithmetic: fp32 with FMA; parity gate = 1e-5 max-abs against the fp64 oracle.
 #include "hair_internal.cuh"
 
 #define GEN_WARPS 8
+#ifndef GEN_MIN_BLOCKS
+#define GEN_MIN_BLOCKS 3  // CTAs per SM the register budget is held to
+#endif
 
 struct F3 {
   float x, y, z;
@@ -49,12 +54,16 @@ __device__ __forceinline__ F3 shfl3_down(F3 v) {
 //  [12..15] dE0.xyz, w     [16..19] dE1.xyz, curl amplitude     [20..23] dE2.xyz, frizz amplitude
 //  [24..27] c.xyz, clump factor   [28..31] Tc.xyz, frizz smoothstep   [32..35] Ef.xyz, frizz cell (int bits)
 //  [36..39] cos/sin twist angle, cos/sin of the curl turn angle 2*pi*turns*w
-__global__ void __launch_bounds__(GEN_WARPS * 32)
+__global__ void __launch_bounds__(GEN_WARPS * 32, GEN_MIN_BLOCKS)
 k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
            float4* __restrict__ vertices, unsigned long long* __restrict__ counters, uint32_t c_max) {
   extern __shared__ float4 smem4[];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float* tab = reinterpret_cast<float*>(smem4) + (size_t)warp * c_max * HAIR_ROW;
+  // per warp: the bundle table [c_max][HAIR_ROW], then 32 strand records (b1, b2, cos/sin curl phase) + 32 hashes
+  const size_t warp_floats = (size_t)c_max * HAIR_ROW + 32 * 5;
+  float* tab = reinterpret_cast<float*>(smem4) + (size_t)warp * warp_floats;
+  float4* srec = reinterpret_cast<float4*>(tab + (size_t)c_max * HAIR_ROW);
+  uint32_t* sbase = reinterpret_cast<uint32_t*>(srec + 32);
 
   for (;;) {
     // dynamic work fetch: one bundle-instance per warp (the paper's indirect dispatch, device-side)
@@ -173,77 +182,96 @@ k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restri
 #pragma unroll
       for (int a = 0; a < 12; ++a) M[a] = __ldg(&g.xform[q * 12 + a]);
     const uint32_t off_t = __ldg(&g.off[t]);
-    const uint32_t n_v = nlod * C;
-    float4* out = vertices + e.w;
-    for (uint32_t v = lane; v < n_v; v += 32) {
-      const uint32_t k = v / C, j = v - k * C;
-      const uint32_t base = pcg(g.seed_h + off_t + k);
-      uint32_t a1 = pcg(base + 1u) >> 8, a2 = pcg(base + 2u) >> 8;
-      if (a1 + a2 > 16777216u) {  // R6: fold on the integers
-        a1 = 16777216u - a1;
-        a2 = 16777216u - a2;
-      }
-      const float b1 = (float)a1 * (1.0f / 16777216.0f), b2 = (float)a2 * (1.0f / 16777216.0f);
-      const float b0 = (1.0f - b1) - b2;
-      const float4* r4 = reinterpret_cast<const float4*>(tab + (size_t)j * HAIR_ROW);
-      const float4 E0 = r4[0], E1 = r4[1], E2 = r4[2];
-      F3 p = f3(b0 * E0.x + b1 * E1.x + b2 * E2.x, b0 * E0.y + b1 * E1.y + b2 * E2.y, b0 * E0.z + b1 * E1.z + b2 * E2.z);
-      float aov = fminf(fmaxf(b0 * E0.w + b1 * E1.w + b2 * E2.w, 0.f), 1.f);
-      if (ops) {
-        const float4 D0 = r4[3], D1 = r4[4], D2 = r4[5];
-        if (ops & (HAIR_OP_CLUMP | HAIR_OP_TWIST)) {
-          const float4 cc4 = r4[6];
-          const F3 c = f3(cc4.x, cc4.y, cc4.z);
-          if (ops & HAIR_OP_CLUMP) p = p + cc4.w * (c - p);
-          if (ops & HAIR_OP_TWIST) {
-            const float4 tc4 = r4[7], cs4 = r4[9];
-            const F3 Tc = f3(tc4.x, tc4.y, tc4.z);
-            const F3 d = p - c;  // Rodrigues rotation about Tc
-            const F3 dr = cs4.x * d + cs4.y * cross(Tc, d) + (dot(Tc, d) * (1.f - cs4.x)) * Tc;
-            p = c + dr;
-          }
+    const uint32_t q32 = 32u / C, r32 = 32u - q32 * C;  // (k, j) of a lane advance by 32 vertices per iteration
+    for (uint32_t k0 = 0; k0 < nlod; k0 += 32) {
+      // per strand, once (lanes = strands of this batch): root barycentrics (R6) and the curl phase
+      const uint32_t nk = min(32u, nlod - k0);
+      if (lane < nk) {
+        const uint32_t base = pcg(g.seed_h + off_t + k0 + lane);
+        uint32_t a1 = pcg(base + 1u) >> 8, a2 = pcg(base + 2u) >> 8;
+        if (a1 + a2 > 16777216u) {  // R6: fold on the integers
+          a1 = 16777216u - a1;
+          a2 = 16777216u - a2;
         }
-        if (ops & (HAIR_OP_CURL | HAIR_OP_FRIZZ)) {
-          // frame from the UNSTYLED base spline: T = normalised derivative, N from the cage edge
-          const F3 T = normalize(f3(b0 * D0.x + b1 * D1.x + b2 * D2.x, b0 * D0.y + b1 * D1.y + b2 * D2.y,
-                                    b0 * D0.z + b1 * D1.z + b2 * D2.z));
-          const float4 ef4 = r4[8];
-          const F3 Ef = f3(ef4.x, ef4.y, ef4.z);
-          F3 Nn = Ef - dot(Ef, T) * T;
-          if (dot(Nn, Nn) < 1e-20f) {
-            const float ax = fabsf(T.x), ay = fabsf(T.y), az = fabsf(T.z);
-            const F3 a = (ax <= ay && ax <= az) ? f3(1, 0, 0) : (ay <= az ? f3(0, 1, 0) : f3(0, 0, 1));
-            Nn = a - dot(a, T) * T;
-          }
-          const F3 N = normalize(Nn);
-          const F3 B = cross(T, N);
-          if (ops & HAIR_OP_CURL) {
-            const float4 cs4 = r4[9];
-            const float u = (float)(pcg(base + 3u) >> 8) * (1.0f / 16777216.0f);
-            float sphi, cphi;
-            sincospif(2.f * u, &sphi, &cphi);
-            const float ct = cphi * cs4.z - sphi * cs4.w, st = sphi * cs4.z + cphi * cs4.w;  // angle addition
-            p = p + D1.w * (ct * N + st * B);
-          }
-          if (ops & HAIR_OP_FRIZZ) {
-            const uint32_t cell = __float_as_uint(ef4.w);
-            const float s = r4[7].w;
-            float n[2];
-#pragma unroll
-            for (uint32_t ch = 0; ch < 2; ++ch) {
-              const uint32_t h0 = pcg(base + 16u + 2u * cell + ch), h1 = pcg(base + 16u + 2u * (cell + 1u) + ch);
-              const int s0 = (int)(__vsadu4(h0, 0u)) - 510, s1 = (int)(__vsadu4(h1, 0u)) - 510;  // byte sums
-              const float g0 = (float)s0 * 0.0067658652f, g1 = (float)s1 * 0.0067658652f;       // 1/sqrt(21845)
-              n[ch] = (1.f - s) * g0 + s * g1;
+        float sphi = 0.f, cphi = 1.f;
+        if (ops & HAIR_OP_CURL) sincospif(2.f * ((float)(pcg(base + 3u) >> 8) * (1.0f / 16777216.0f)), &sphi, &cphi);
+        srec[lane] = make_float4((float)a1 * (1.0f / 16777216.0f), (float)a2 * (1.0f / 16777216.0f), cphi, sphi);
+        sbase[lane] = base;
+      }
+      __syncwarp();
+      const uint32_t n_vb = nk * C;
+      float4* out = vertices + e.w + (size_t)k0 * C;
+      uint32_t k = lane / C, j = lane - k * C;
+      for (uint32_t v = lane; v < n_vb; v += 32) {
+        const float4 sr = srec[k];
+        const float b1 = sr.x, b2 = sr.y;
+        const float b0 = (1.0f - b1) - b2;
+        const float4* r4 = reinterpret_cast<const float4*>(tab + (size_t)j * HAIR_ROW);
+        const float4 E0 = r4[0], E1 = r4[1], E2 = r4[2];
+        F3 p = f3(b0 * E0.x + b1 * E1.x + b2 * E2.x, b0 * E0.y + b1 * E1.y + b2 * E2.y, b0 * E0.z + b1 * E1.z + b2 * E2.z);
+        float aov = fminf(fmaxf(b0 * E0.w + b1 * E1.w + b2 * E2.w, 0.f), 1.f);
+        if (ops) {
+          if (ops & (HAIR_OP_CLUMP | HAIR_OP_TWIST)) {
+            const float4 cc4 = r4[6];
+            const F3 c = f3(cc4.x, cc4.y, cc4.z);
+            if (ops & HAIR_OP_CLUMP) p = p + cc4.w * (c - p);
+            if (ops & HAIR_OP_TWIST) {
+              const float4 tc4 = r4[7], cs4 = r4[9];
+              const F3 Tc = f3(tc4.x, tc4.y, tc4.z);
+              const F3 d = p - c;  // Rodrigues rotation about Tc
+              const F3 dr = cs4.x * d + cs4.y * cross(Tc, d) + (dot(Tc, d) * (1.f - cs4.x)) * Tc;
+              p = c + dr;
             }
-            p = p + D2.w * (n[0] * N + n[1] * B);
+          }
+          if (ops & (HAIR_OP_CURL | HAIR_OP_FRIZZ)) {
+            // frame from the UNSTYLED base spline: T = normalised derivative, N from the cage edge
+            const float4 D0 = r4[3], D1 = r4[4], D2 = r4[5];
+            const F3 T = normalize(f3(b0 * D0.x + b1 * D1.x + b2 * D2.x, b0 * D0.y + b1 * D1.y + b2 * D2.y,
+                                      b0 * D0.z + b1 * D1.z + b2 * D2.z));
+            const float4 ef4 = r4[8];
+            const F3 Ef = f3(ef4.x, ef4.y, ef4.z);
+            F3 Nn = Ef - dot(Ef, T) * T;
+            float nn = dot(Nn, Nn);
+            if (nn < 1e-20f) {
+              const float ax = fabsf(T.x), ay = fabsf(T.y), az = fabsf(T.z);
+              const F3 a = (ax <= ay && ax <= az) ? f3(1, 0, 0) : (ay <= az ? f3(0, 1, 0) : f3(0, 0, 1));
+              Nn = a - dot(a, T) * T;
+              nn = dot(Nn, Nn);
+            }
+            const F3 N = (nn > 0.f ? rsqrtf(nn) : 0.f) * Nn;
+            const F3 B = cross(T, N);
+            if (ops & HAIR_OP_CURL) {
+              const float4 cs4 = r4[9];
+              const float ct = sr.z * cs4.z - sr.w * cs4.w, st = sr.w * cs4.z + sr.z * cs4.w;  // angle addition
+              p = p + D1.w * (ct * N + st * B);
+            }
+            if (ops & HAIR_OP_FRIZZ) {
+              const uint32_t cell = __float_as_uint(ef4.w), base = sbase[k];
+              const float s = r4[7].w;
+              float n[2];
+#pragma unroll
+              for (uint32_t ch = 0; ch < 2; ++ch) {
+                const uint32_t h0 = pcg(base + 16u + 2u * cell + ch), h1 = pcg(base + 16u + 2u * (cell + 1u) + ch);
+                const int s0 = (int)(__vsadu4(h0, 0u)) - 510, s1 = (int)(__vsadu4(h1, 0u)) - 510;  // byte sums
+                const float g0 = (float)s0 * 0.0067658652f, g1 = (float)s1 * 0.0067658652f;       // 1/sqrt(21845)
+                n[ch] = (1.f - s) * g0 + s * g1;
+              }
+              p = p + D2.w * (n[0] * N + n[1] * B);
+            }
           }
         }
+        if (has_m)  // R-inst: instance transform applied last
+          p = f3(M[0] * p.x + M[1] * p.y + M[2] * p.z + M[3], M[4] * p.x + M[5] * p.y + M[6] * p.z + M[7],
+                 M[8] * p.x + M[9] * p.y + M[10] * p.z + M[11]);
+        out[v] = make_float4(p.x, p.y, p.z, aov);
+        k += q32;
+        j += r32;
+        if (j >= C) {
+          j -= C;
+          ++k;
+        }
       }
-      if (has_m)  // R-inst: instance transform applied last
-        p = f3(M[0] * p.x + M[1] * p.y + M[2] * p.z + M[3], M[4] * p.x + M[5] * p.y + M[6] * p.z + M[7],
-               M[8] * p.x + M[9] * p.y + M[10] * p.z + M[11]);
-      out[v] = make_float4(p.x, p.y, p.z, aov);
+      __syncwarp();
     }
     __syncwarp();
   }
@@ -251,7 +279,7 @@ k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restri
 
 void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices,
                      unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st) {
-  size_t smem = (size_t)GEN_WARPS * c_max * HAIR_ROW * sizeof(float);
+  size_t smem = (size_t)GEN_WARPS * ((size_t)c_max * HAIR_ROW + 32 * 5) * sizeof(float);
   static size_t configured = 0;
   if (smem > configured) {
     cudaFuncSetAttribute(k_generate, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
