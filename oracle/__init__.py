@@ -109,6 +109,8 @@ def lib():
         L.orc_frame_raster.argtypes = [vp, vp, vp, vp, vp]
         L.orc_frame_get_gbuffer.argtypes = [vp, vp]
         L.orc_frame_set_gbuffer.argtypes = [vp, vp, u32, u32]
+        L.orc_frame_set_window.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.orc_frame_set_window.restype = None
         L.orc_frame_shade.argtypes = [vp, vp, vp]
         L.orc_frame_get_colour.argtypes = [vp, vp]
         L.orc_frame_get_tangents.argtypes = [vp, vp]
@@ -290,6 +292,10 @@ class Frame:
         h, w = g.shape[:2]
         self._wh = (w, h)
         self.L.orc_frame_set_gbuffer(self.h, _ptr(g), w, h)
+
+    def set_window(self, x0: int = 0, y0: int = 0, x1: int = 1 << 30, y1: int = 1 << 30) -> None:
+        """Sample a full-size frame: O4 / O6 / O7 only visit pixels of [x0, x1) x [y0, y1) (O6 grown by 7 px)."""
+        self.L.orc_frame_set_window(self.h, int(x0), int(y0), int(x1), int(y1))
 
     # ---- O6 / O7
     def shade(self, cam: dict, prm: dict):

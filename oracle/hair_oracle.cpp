@@ -180,6 +180,11 @@ struct orc_frame {
   std::vector<double> colour;
   std::vector<float> tang;
   std::vector<double> out;
+  // Pixel window [wx0, wx1) x [wy0, wy1) the pixel loops of O4/O6/O7 are restricted to (default: the whole
+  // image). Pixels are independent in all three stages, so every value inside the window is the value of the
+  // full-frame run; this only lets a test sample a full-size frame in seconds. O6 covers the window grown by
+  // the largest filter radius (7), which is what O7 reads.
+  int wx0 = 0, wy0 = 0, wx1 = 1 << 30, wy1 = 1 << 30;
 };
 
 namespace {
@@ -785,7 +790,8 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
       float fx0 = std::max(std::floor(mnx) - 1.f, 0.f), fx1 = std::min(std::floor(mxx) + 1.f, float(k.W) - 1.f);
       float fy0 = std::max(std::floor(mny) - 1.f, 0.f), fy1 = std::min(std::floor(mxy) + 1.f, float(k.H) - 1.f);
       if (!(fx0 <= fx1) || !(fy0 <= fy1)) continue;
-      int x0 = int(fx0), x1 = int(fx1), y0 = int(fy0), y1 = int(fy1);
+      int x0 = std::max(int(fx0), f->wx0), x1 = std::min(int(fx1), f->wx1 - 1);
+      int y0 = std::max(int(fy0), f->wy0), y1 = std::min(int(fy1), f->wy1 - 1);
       float dz = b.zn - a.zn;
       for (int y = y0; y <= y1; ++y)
         for (int x = x0; x <= x1; ++x) {
@@ -816,6 +822,9 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
 void orc_frame_get_gbuffer(const orc_frame* f, uint64_t* o) {
   std::memcpy(o, f->gbuf.data(), f->gbuf.size() * sizeof(uint64_t));
 }
+void orc_frame_set_window(orc_frame* f, int x0, int y0, int x1, int y1) {
+  f->wx0 = x0, f->wy0 = y0, f->wx1 = x1, f->wy1 = y1;
+}
 int orc_frame_set_gbuffer(orc_frame* f, const uint64_t* in, uint32_t w, uint32_t h) {
   f->W = w;
   f->H = h;
@@ -831,7 +840,11 @@ int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) 
   f->colour.assign(np * 3, 0.0);
   f->tang.assign(np * 4, 0.f);
   V3 eye = {double(k.eye[0]), double(k.eye[1]), double(k.eye[2])};
-  for (size_t p = 0; p < np; ++p) {
+  const int sx0 = std::max(f->wx0 - 7, 0), sx1 = std::min(f->wx1 < (1 << 30) ? f->wx1 + 7 : f->wx1, int(k.W));
+  const int sy0 = std::max(f->wy0 - 7, 0), sy1 = std::min(f->wy1 < (1 << 30) ? f->wy1 + 7 : f->wy1, int(k.H));
+  for (int sy = sy0; sy < sy1; ++sy)
+  for (int sx = sx0; sx < sx1; ++sx) {
+    const size_t p = size_t(sy) * k.W + sx;
     uint64_t G = f->gbuf[p * 2], A = f->gbuf[p * 2 + 1];
     if (A != EMPTY) screen_tangent(f, k, A, &f->tang[p * 4 + 2]);
     if (G == EMPTY) continue;
@@ -963,8 +976,8 @@ int orc_frame_filter(orc_frame* f, const orc_camera* cam, const orc_params* prm)
   uint32_t tauz_q = uint32_t(std::floor(double(prm->tau_z) * 16777215.0 + 0.5));
   uint32_t taufly_q = uint32_t(std::floor(double(prm->tau_fly) * 16777215.0 + 0.5));
   double bg[3] = {double(prm->background_rgb[0]), double(prm->background_rgb[1]), double(prm->background_rgb[2])};
-  for (int py = 0; py < H; ++py)
-    for (int px = 0; px < W; ++px) {
+  for (int py = std::max(f->wy0, 0); py < std::min(f->wy1, H); ++py)
+    for (int px = std::max(f->wx0, 0); px < std::min(f->wx1, W); ++px) {
       size_t p = size_t(py) * W + px;
       uint64_t G = f->gbuf[p * 2], A = f->gbuf[p * 2 + 1];
       bool isCenter = G != EMPTY, isCons = A != EMPTY;

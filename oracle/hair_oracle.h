@@ -122,6 +122,10 @@ int orc_frame_raster(orc_frame*, const orc_camera*, const orc_params*, const uin
                      uint64_t counts[3]);
 void orc_frame_get_gbuffer(const orc_frame*, uint64_t* out);
 int orc_frame_set_gbuffer(orc_frame*, const uint64_t* in, uint32_t w, uint32_t h);
+/* Restrict the pixel loops of O4, O6 (grown by 7 px) and O7 to [x0, x1) x [y0, y1). Pixels are independent in
+ * all three, so values inside the window equal those of the full-frame run: a way to SAMPLE a full-size frame
+ * (the raster's hit counts then cover the window only). Default / reset: 0, 0, 1 << 30, 1 << 30. */
+void orc_frame_set_window(orc_frame*, int x0, int y0, int x1, int y1);
 
 /* O6: colour[H][W][3] fp64 (0 where no centre hit); tangents[H][W][4] fp32 = (T_G.xy, T_A.xy) */
 int orc_frame_shade(orc_frame*, const orc_camera*, const orc_params*);

@@ -139,11 +139,10 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
   float4* s_item = fsm + NS;                            // [2 * FT_W * FT_H] item, later its result
   uint32_t* s_dqG = reinterpret_cast<uint32_t*>(s_item + 2 * FT_W * FT_H);  // [NS] dq of the centre word
   uint32_t* s_dqA = s_dqG + NS;                                             // [NS] dq of the conservative word
-  __shared__ uint32_t s_n;
+  __shared__ uint32_t s_n, s_cnt[32];
   const int W = (int)cam.W, H = (int)cam.H;
   const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
   const int x0 = blockIdx.x * FT_W, y0 = blockIdx.y * FT_H;
-  if (tid == 0) s_n = 0;
   // ---- own two pixels (rows ly and ly + 8 of the tile)
   unsigned long long G[2], A[2];
   bool inside[2];
@@ -187,23 +186,51 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
     s_dqG[i] = dG;
     s_dqA[i] = dA;
   }
-  // ---- (2) work items
+  // ---- (2) work items, compacted in pixel order (row by row, centre items of a row first): neighbouring lanes
+  // then walk neighbouring windows and their shared-memory reads fall on distinct banks
   int slot_c[2] = {-1, -1}, slot_a[2] = {-1, -1};
   bool fly[2] = {false, false};
+  float2 Tc[2], Ta[2];
+  uint32_t bal[4];
+  const uint32_t lt_mask = (1u << lx) - 1u;
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
     const bool isCenter = G[k] != HAIR_EMPTY, isCons = A[k] != HAIR_EMPTY;
-    const uint32_t pix = (uint32_t)((ly + 8 * k) * FT_W + lx);
+    Tc[k] = Ta[k] = make_float2(1.f, 0.f);
     if (isCenter) {
-      const float2 T = screen_tangent(sc, table, vertices, cam, G[k]);
-      slot_c[k] = (int)atomicAdd(&s_n, 1u);
-      s_item[slot_c[k]] = make_float4(T.x, T.y, __uint_as_float(w_dq(G[k]) | 0x1000000u), __uint_as_float(pix));
+      Tc[k] = screen_tangent(sc, table, vertices, cam, G[k]);
       fly[k] = isCons && w_dq(G[k]) >= w_dq(A[k]) && w_dq(G[k]) - w_dq(A[k]) >= sp.taufly_q;  // PAPER.md:175, R21
     }
-    if (fly[k] || (isCons && !isCenter)) {  // fly-away strand, or promoted pixel: w_color = 1
-      const float2 T = screen_tangent(sc, table, vertices, cam, A[k]);
-      slot_a[k] = (int)atomicAdd(&s_n, 1u);
-      s_item[slot_a[k]] = make_float4(T.x, T.y, __uint_as_float(w_dq(A[k])), __uint_as_float(pix));
+    const bool isA = fly[k] || (isCons && !isCenter);  // fly-away strand, or promoted pixel: w_color = 1
+    if (isA) Ta[k] = screen_tangent(sc, table, vertices, cam, A[k]);
+    bal[2 * k] = __ballot_sync(0xffffffffu, isCenter);
+    bal[2 * k + 1] = __ballot_sync(0xffffffffu, isA);
+  }
+  if (lx < 4)  // group = (row of the tile) * 2 + type
+    s_cnt[(lx >> 1) * 16 + ly * 2 + (lx & 1)] = __popc(lx == 0 ? bal[0] : lx == 1 ? bal[1] : lx == 2 ? bal[2] : bal[3]);
+  __syncthreads();
+  {
+    const uint32_t mine = s_cnt[lx];
+    uint32_t incl = mine;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t up = __shfl_up_sync(0xffffffffu, incl, d);
+      if (lx >= d) incl += up;
+    }
+    if (tid == 31) s_n = incl;
+    const uint32_t excl = incl - mine;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const uint32_t base_c = __shfl_sync(0xffffffffu, excl, k * 16 + ly * 2), base_a = __shfl_sync(0xffffffffu, excl, k * 16 + ly * 2 + 1);
+      const uint32_t pix = (uint32_t)((ly + 8 * k) * FT_W + lx);
+      if ((bal[2 * k] >> lx) & 1u) {
+        slot_c[k] = (int)(base_c + __popc(bal[2 * k] & lt_mask));
+        s_item[slot_c[k]] = make_float4(Tc[k].x, Tc[k].y, __uint_as_float(w_dq(G[k]) | 0x1000000u), __uint_as_float(pix));
+      }
+      if ((bal[2 * k + 1] >> lx) & 1u) {
+        slot_a[k] = (int)(base_a + __popc(bal[2 * k + 1] & lt_mask));
+        s_item[slot_a[k]] = make_float4(Ta[k].x, Ta[k].y, __uint_as_float(w_dq(A[k])), __uint_as_float(pix));
+      }
     }
   }
   __syncthreads();

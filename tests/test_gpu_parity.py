@@ -152,6 +152,82 @@ def test_end_to_end_pure_oracle_vs_pure_gpu(orc, hair_mod):
     assert psnr(out[..., :3], G["rgb"][..., :3], max(out[..., :3].max(), 1.0)) > 45.0
 
 
+def check_full_size_sampled(orc, sc, G, windows):
+    """A frame at BASELINE.json's full size: table and all vertices against the oracle, then the oracle's
+    pixel stages on WINDOWS of the frame (oracle.Frame.set_window: pixels are independent, so a window of
+    the oracle's output equals the same window of its full-frame run)."""
+    cam, prm = sc["camera"], G["prm"]
+    f = orc.Frame(sc["grooms"])
+    f.lod(cam, sc["lam"])
+    t_or, _ = f.table()
+    assert np.array_equal(t_or, G["table"]), "bundle table differs"
+    assert G["stats"]["n_strands_lod"] == f.n_strands and G["stats"]["n_vertices"] == f.n_vertices
+    f.generate()
+    err_v = float(np.abs(G["verts"].astype(np.float64) - f.vertices_f64()).max())
+    assert err_v <= TOL_VERTEX, f"vertex max-abs {err_v}"
+    assert (G["gb"][..., 1] <= G["gb"][..., 0]).all()  # centre subset of conservative, every pixel of the frame
+    f.set_vertices_f32(G["verts"])
+    n_hit = n_px = 0
+    worst_rgb, worst_psnr = 0.0, 200.0
+    for (x0, y0, x1, y1) in windows:
+        f.set_window(x0, y0, x1, y1)
+        f.raster(cam, prm)
+        g_or = f.gbuffer()[y0:y1, x0:x1]
+        g_gpu = G["gb"][y0:y1, x0:x1]
+        frac = float((g_or == g_gpu).mean())
+        assert frac >= MIN_EXACT, f"window {(x0, y0, x1, y1)}: G-buffer exact fraction {frac}"
+        assert frac == 1.0, f"window {(x0, y0, x1, y1)}: {frac}"  # same vertex buffer: expected bit-exact
+        n_hit += int((g_gpu[..., 1] != EMPTY).sum())
+        n_px += g_gpu.shape[0] * g_gpu.shape[1]
+    f.set_gbuffer(G["gb"])
+    for (x0, y0, x1, y1) in windows:
+        f.set_window(x0, y0, x1, y1)
+        f.shade(cam, prm)
+        out = f.filter(cam, prm)[y0:y1, x0:x1]
+        got = G["rgb"][y0:y1, x0:x1]
+        worst_rgb = max(worst_rgb, float(np.abs(out - got).max()))
+        worst_psnr = min(worst_psnr, psnr(out[..., :3], got[..., :3], max(float(out[..., :3].max()), 1.0)))
+    assert worst_rgb <= TOL_RGB, f"rgb max-abs {worst_rgb}"
+    assert worst_psnr > MIN_PSNR, f"psnr {worst_psnr}"
+    return dict(vertex_err=err_v, n_hit=n_hit, n_px=n_px, rgb_err=worst_rgb, psnr=worst_psnr)
+
+
+def test_bench_frame_full_size_sampled(orc, hair_mod):
+    """BASELINE config 4 exactly as bench.py times it (483 000 strands, 3840x2160, per-groom lambda): every
+    bundle-table entry and all 9.7 M vertices against the oracle; words and RGB on windows through the dense
+    core of the near groom (~70 hits per pixel), its fringe, the clipped left border and the far grooms."""
+    sc = synth.config(4)
+    W, H = sc["camera"]["width"], sc["camera"]["height"]
+    assert (W, H) == (3840, 2160) and synth.n_strands(sc) == 483000
+    G = gpu_frame(hair_mod, sc)
+    cx = lambda ndc: int((1.0 + ndc) * 0.5 * W)
+    windows = [(cx(-0.75) - 96, H // 2 - 96, cx(-0.75) + 96, H // 2 + 96),      # core of groom 0
+               (0, H // 2 - 200, 120, H // 2 + 40),                             # left border, groom 0 clipped
+               (cx(-0.75) + 380, H // 2 - 420, cx(-0.75) + 540, H // 2 - 300),  # fringe of groom 0
+               (cx(0.15) - 80, H // 2 - 80, cx(0.15) + 80, H // 2 + 80),        # groom 1
+               (cx(0.5) - 64, H // 2 - 64, cx(0.5) + 64, H // 2 + 64),          # groom 2
+               (cx(0.72) - 48, H // 2 - 48, cx(0.72) + 48, H // 2 + 48),        # groom 3
+               (cx(0.88) - 40, H // 2 - 40, cx(0.88) + 40, H // 2 + 40)]        # groom 4, sub-pixel segments
+    rep = check_full_size_sampled(orc, sc, G, windows)
+    assert rep["n_hit"] > 0.3 * rep["n_px"], rep  # the windows do sit on hair
+
+
+def test_crowd_full_size_sampled(orc, hair_mod):
+    """BASELINE config 5 as named: 64 instances x 30 000 strands at 10-40 m, 3840x2160, lambda 4."""
+    sc = synth.config(5)
+    W, H = sc["camera"]["width"], sc["camera"]["height"]
+    G = gpu_frame(hair_mod, sc)
+    # windows on the instances with the most conservative hits (found from the frame itself; any window is valid)
+    hit = (G["gb"][..., 1] != EMPTY)
+    cell = 120
+    grid = hit[: H // cell * cell, : W // cell * cell].reshape(H // cell, cell, W // cell, cell).sum((1, 3))
+    order = np.argsort(grid.reshape(-1))[::-1][:6]
+    windows = [(int(i % (W // cell)) * cell, int(i // (W // cell)) * cell,
+                int(i % (W // cell)) * cell + cell, int(i // (W // cell)) * cell + cell) for i in order]
+    rep = check_full_size_sampled(orc, sc, G, windows)
+    assert rep["n_hit"] > 1000, rep
+
+
 def test_deterministic_and_order_free(orc, hair_mod):
     """atomicMin resolve: two runs give identical buffers whatever the warp scheduling."""
     sc = synth.config(4, scale=0.02, res_scale=0.2)

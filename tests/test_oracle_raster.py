@@ -319,3 +319,36 @@ def test_width_world_sets_centre_radius(orc):
     assert hits[0] == hits[1]  # tiny width clamps to 0.25 px == center_diameter 0.25
     assert hits[1] < hits[2] < hits[3]
     assert hits[3] <= f.raster(sc["camera"], sc["params"])["cons"]
+
+
+def test_window_samples_equal_full_frame(orc):
+    """Frame.set_window (used to sample full-size frames in the GPU tests): inside the window the G-buffer
+    and the filtered image are the full-frame values, outside nothing is written."""
+    from paper_2607_04230_b200 import synth
+    sc = synth.config(1, scale=0.5)
+    cam, prm = sc["camera"], sc["params"]
+    f = orc.Frame(sc["grooms"])
+    f.lod(cam, sc["lam"])
+    f.generate()
+    f.set_vertices_f32(f.vertices_f32())
+    f.raster(cam, prm)
+    g_full = f.gbuffer().copy()
+    f.shade(cam, prm)
+    o_full = f.filter(cam, prm).copy()
+    x0, y0, x1, y1 = 70, 60, 170, 141
+    f.set_window(x0, y0, x1, y1)
+    cnt = f.raster(cam, prm)
+    g_win = f.gbuffer()
+    assert np.array_equal(g_win[y0:y1, x0:x1], g_full[y0:y1, x0:x1])
+    mask = np.ones(g_win.shape[:2], bool)
+    mask[y0:y1, x0:x1] = False
+    assert (g_win[mask] == np.uint64(0xFFFFFFFFFFFFFFFF)).all()
+    assert 0 < cnt["cons"] < int((g_full[..., 1] != np.uint64(0xFFFFFFFFFFFFFFFF)).sum()) * 64
+    f.set_gbuffer(g_full)
+    f.shade(cam, prm)
+    o_win = f.filter(cam, prm)
+    assert np.array_equal(o_win[y0:y1, x0:x1], o_full[y0:y1, x0:x1])
+    assert (o_win[mask] == 0).all()
+    f.set_window()  # reset: whole image again
+    f.raster(cam, prm)
+    assert np.array_equal(f.gbuffer(), g_full)
