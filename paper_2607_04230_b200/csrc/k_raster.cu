@@ -16,14 +16,19 @@
 // pixels of its column; long and sub-pixel segments cost the same per pixel.
 #include "hair_internal.cuh"
 
+#ifndef RAS_WARPS
 #define RAS_WARPS 8
+#endif
 #ifndef RAS_MIN_BLOCKS
 #define RAS_MIN_BLOCKS 5  // CTAs per SM the register budget is held to (40 of 64 warps)
 #endif
 #define REC_STRIDE 20  // floats per segment record (16 used); 20 mod 32 keeps LDS.128 conflict-free
 #define ENUM_EPS 0.015625f  // slack on the minor-axis range of a column: the enumeration must be a superset
 #ifndef ROW_BATCH
-#define ROW_BATCH 1
+#define ROW_BATCH 2
+#endif
+#ifndef GB_LOAD
+#define GB_LOAD __ldcg
 #endif
 // ROW_BATCH: rows of one column whose G-buffer words are requested before any is used
 
@@ -182,7 +187,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
             const float uN = xsub((float)r + 0.5f, aN);
             const float cr = fabsf(xsub(xmul(dM, uN), xmul(dN, uM)));
             ok[i] = r <= rhi && cr <= ext;
-            if (ok[i]) cur[i] = __ldcg(reinterpret_cast<const ulonglong2*>(pcol + (size_t)r * pstep));
+            if (ok[i]) cur[i] = GB_LOAD(reinterpret_cast<const ulonglong2*>(pcol + (size_t)r * pstep));
           }
           // pass 2: closest point, depth, centre predicate, word (R10/R11, fixed-order fp32; x/y-symmetric)
 #pragma unroll
