@@ -45,7 +45,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-i", str(index), "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL,
+                                       "-i", str(index), "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL,
                                       text=True)
         except Exception:
             self.p = None
@@ -226,6 +226,7 @@ def run_cuda(args):
 
     # ---- rooflines: algorithmic work per launch / measured stage time
     hbm_peak, hbm_src = peaks()
+    n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
     words = torch.empty(W * H * 2, dtype=torch.int64, device=dev)
     n_ops = 1 << 28
     atom = {}
@@ -253,16 +254,43 @@ def run_cuda(args):
     stages["lod_scan"] = {"bound": "latency", "ms": st["ms_lod"]}
     dom = max(("generate", "clear", "raster", "shade", "filter"), key=lambda k: stages[k]["ms"])
     d = stages[dom]
-    if dom == "raster":
-        roofline = {"kernel": "k_raster", "bound": "l2_atomic", "achieved": d["Gatom_per_s"], "peak": atom["random"],
-                    "unit": "Gatom/s", "frac": d["frac_l2_atomic_random"], "traffic": None,
-                    "peak_source": "hair_atomic_microbench mode 1 (random 64-bit RED.MIN over a G-buffer-sized "
-                                   "buffer), measured live in this run",
-                    "algorithmic": f"{n_at} predicate-true hits (centre + conservative) per frame"}
+    # Issue-slot ("alu") view of the two kernels that ncu shows are bound by instruction issue, not by memory:
+    # warp instructions per algorithmic unit from the committed ncu capture (profiles/r1_v3_ncu_full.md,
+    # smsp__inst_executed.sum / units of that frame) x the units this run counted, over the live CUDA-event time,
+    # against 148 SMs x 4 schedulers x 1 warp instruction per clock.
+    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    issue_peak = n_sm * 4 * sm_mhz * 1e6 / 1e9  # G warp-instructions / s
+    n_items = cnt["n_pixels_cons"]  # one filter item per hit pixel (+ one per fly-away pixel, not counted here)
+    inst_per_unit = {"raster": (806049027 / 219609409, n_at, "predicate-true hit"),
+                     "filter": (523002207 / 3024726, n_items, "hit pixel")}
+    if not (args.config == 4 and args.scale == 1.0 and args.res_scale == 1.0):
+        inst_per_unit = {}  # the per-unit instruction counts were captured on the bench frame only
+    for k, (ipu, units, what) in inst_per_unit.items():
+        stg = stages[k]
+        stg["warp_inst"] = ipu * units
+        stg["Gwarp_inst_per_s"] = ipu * units / (stg["ms"] * 1e-3) / 1e9
+        stg["frac_issue"] = stg["Gwarp_inst_per_s"] / issue_peak
+        stg["inst_per_unit"] = f"{ipu:.2f} warp instructions per {what} (ncu, profiles/r1_v3_ncu_full.md)"
+    dram = {"generate": 103793920, "raster": 240943616, "shade": 200686336, "filter": 308508928}  # ncu dram read+write per launch, same capture
+    if dom in inst_per_unit:
+        roofline = {"kernel": "k_" + dom, "bound": "alu", "achieved": d["Gwarp_inst_per_s"], "peak": issue_peak,
+                    "unit": "Gwarp-inst/s", "frac": d["frac_issue"], "traffic": dram.get(dom),
+                    "peak_source": f"derived: {n_sm} SMs x 4 schedulers x {sm_mhz:.0f} MHz (clock sampled in this run)",
+                    "algorithmic": d["inst_per_unit"] + f" x {inst_per_unit[dom][1]} units counted in this run"}
     else:
         roofline = {"kernel": "k_" + dom, "bound": "hbm", "achieved": d["GBps"], "peak": hbm_peak, "unit": "GB/s",
-                    "frac": d["frac_hbm"], "traffic": None, "peak_source": hbm_src,
+                    "frac": d["frac_hbm"], "traffic": dram.get(dom), "peak_source": hbm_src,
                     "algorithmic": f"{d['bytes']} bytes per frame"}
+    # the three fractions north_star asks for, as it states them
+    north_star = {
+        "raster_vs_l2_atomic": {"achieved_Gatom_per_s": stages["raster"].get("Gatom_per_s"), "peak_Gatom_per_s": atom["random"],
+                                "frac": stages["raster"].get("frac_l2_atomic_random"),
+                                "note": "algorithmic hits / time over the measured random 64-bit RED.MIN rate; > 1 because "
+                                        "read-before-atomic sends only n_atomics_issued of them to L2",
+                                "issued_Gatom_per_s": cnt["n_atomics_issued"] / (stages["raster"]["ms"] * 1e-3) / 1e9},
+        "generate_vs_hbm": {"GBps": stages["generate"].get("GBps"), "frac": stages["generate"].get("frac_hbm")},
+        "shade_vs_hbm": {"GBps": stages["shade"].get("GBps"), "frac": stages["shade"].get("frac_hbm")},
+    }
 
     # ---- the oracle timed beside it on this box's host cores (bounded sample of the same workload)
     cpu_baseline = None
@@ -288,7 +316,7 @@ def run_cuda(args):
         "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": ms_e2e, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "what": "hair_mesh_update (pinned cage) + hair_render_to_host (out_rgb to pinned host)"},
         "gpu_launches": st["gpu_launches"] * args.steps,
-        "roofline": roofline, "stages": stages, "l2_atomic_peaks_Gatom_per_s": atom,
+        "roofline": roofline, "north_star_fractions": north_star, "stages": stages, "l2_atomic_peaks_Gatom_per_s": atom,
         "hbm_peak_GBps": hbm_peak, "hbm_peak_source": hbm_src,
         "counts": {k: cnt[k] for k in ("n_bundles", "n_bundles_culled", "n_strands_total", "n_strands_lod", "n_vertices",
                                        "n_segments", "n_segments_drawn", "n_segments_live", "n_atomics_center", "n_atomics_cons",
@@ -303,8 +331,8 @@ def run_cuda(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); 4 = the metric's workload")
     ap.add_argument("--scale", type=float, default=1.0, help="strand-count multiplier (1.0 = as named)")
