@@ -127,8 +127,11 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
           const float dd = xadd(xmul(dx, dx), xmul(dy, dy));
           r4[0] = make_float4(aM, aN, dM, dN);
           r4[1] = make_float4(dd, xmul(0.5f, xadd(fabsf(dx), fabsf(dy))), a.zn, xsub(b.zn, a.zn));
-          r4[2] = make_float4(xmul(rho, rho), dM != 0.f ? dN / dM : 0.f, __int_as_float((int)fc0),
+          // minor coordinate of the line at major coordinate x: icpt + x * slope (enumeration only)
+          const float slope = dM != 0.f ? dN / dM : 0.f;
+          r4[2] = make_float4(aN - aM * slope, slope, __int_as_float((int)fc0),
                               __uint_as_float(((uint32_t)(int)fr0 << 16) | (uint32_t)(int)fr1));
+          rec[lane][17] = xmul(rho, rho);
           r4[3].x = __uint_as_float((ymajor ? 0x80000000u : 0u) | ((sid0 + k) << 7) | j);
           // nearest depth any pixel of this segment can store, minus 2 steps for the rounding of R11's lerp
           const uint32_t dqm = quant_depth(fminf(fmaxf(fminf(a.zn, b.zn), 0.f), 1.f));
@@ -166,10 +169,10 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
         const bool ymajor = (key >> 31) != 0;
         const int c = __float_as_int(q2.z) + (int)step;
         const int r0 = (int)(__float_as_uint(q2.w) >> 16), r1 = (int)(__float_as_uint(q2.w) & 0xFFFFu);
-        // minor-axis extent of the segment inside column [c, c+1] (superset, ENUM_EPS slack)
-        const float fc = (float)c, bMa = aM + dM;
-        const float lo_ = fmaxf(fc, fminf(aM, bMa)), hi_ = fminf(fc + 1.f, fmaxf(aM, bMa));
-        const float m0 = aN + (lo_ - aM) * q2.y, m1 = aN + (hi_ - aM) * q2.y;
+        // minor-axis extent of the LINE across column [c, c+1], clipped to the rows of the segment's bounding box:
+        // a superset of the rows the segment crosses there (the line is monotone; ENUM_EPS covers the rounding)
+        const float fc = (float)c;
+        const float m0 = fmaf(fc, q2.y, q2.x), m1 = m0 + q2.y;
         const int rlo = max((int)ceilf(fminf(m0, m1) - ENUM_EPS) - 1, r0);
         const int rhi = min((int)floorf(fmaxf(m0, m1) + ENUM_EPS), r1);
         const float cM = fc + 0.5f;
@@ -204,7 +207,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
             const float zn = xadd(az, xmul(tt, dz));
             if (zn < 0.f || zn > 1.f) continue;
             const float eM = xsub(cM, xadd(aM, xmul(tt, dM))), eN = xsub(cN, xadd(aN, xmul(tt, dN)));
-            const bool centre = xadd(xmul(eM, eM), xmul(eN, eN)) <= q2.x;
+            const bool centre = xadd(xmul(eM, eM), xmul(eN, eN)) <= rec[s][17];
             const unsigned long long word = pack_word(zn, (key >> 7) & 0xFFFFFFu, key & 0x7Fu, tt);
             unsigned long long* px = pcol + (size_t)r * pstep;
             if (COUNT) {
