@@ -124,6 +124,19 @@ int hair_render(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height, 
 int hair_render_to_host(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height,
                         const float* lod_lambda, uint32_t n_lambda, uint64_t* host_gbuffer, float* host_rgb);
 
+/* Pipelined form of hair_render_to_host: enqueues the frame on the context's stream and the device->host
+ * copies on the context's own copy stream, then returns without waiting, so the copies of frame i overlap the
+ * kernels of frame i+1. Results live in one of HAIR_HOST_SLOTS device buffer pairs owned by the context; a
+ * slot is reused (stream-ordered, no host wait) once its previous copies are done. *out_slot receives the
+ * slot; host_rgb / host_gbuffer must stay valid and unread until hair_host_wait(ctx, slot) returns.
+ * Use a different host buffer for each frame in flight. */
+#define HAIR_HOST_SLOTS 2
+int hair_render_to_host_async(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height,
+                              const float* lod_lambda, uint32_t n_lambda, uint64_t* host_gbuffer, float* host_rgb,
+                              int* out_slot);
+/* Blocks until the copies of `slot` (0..HAIR_HOST_SLOTS-1), or of every slot (slot < 0), have finished. */
+int hair_host_wait(hair_ctx*, int slot);
+
 typedef struct {
   uint32_t n_grooms, n_bundles, n_bundles_culled;
   uint32_t n_strands_total, n_strands_lod;

@@ -20,7 +20,7 @@ EMPTY = 0xFFFFFFFFFFFFFFFF
 
 EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_render_params",
            "hair_set_render_params", "hair_mesh_upload", "hair_mesh_update", "hair_mesh_clear",
-           "hair_render", "hair_render_to_host", "hair_render_stages", "hair_stats",
+           "hair_render", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
            "hair_debug_buffers", "hair_debug_set_vertices", "hair_atomic_microbench", "hair_abi_sizes"]
 
 
@@ -103,6 +103,8 @@ def load():
     L.hair_mesh_clear.argtypes = [vp]
     L.hair_render.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp]
     L.hair_render_to_host.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp]
+    L.hair_render_to_host_async.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp, C.POINTER(C.c_int)]
+    L.hair_host_wait.argtypes = [vp, C.c_int]
     L.hair_render_stages.argtypes = [vp, C.POINTER(hair_camera), u32, u32, u32, u64p, vp]
     L.hair_stats.argtypes = [vp, C.POINTER(hair_stats_t)]
     L.hair_debug_buffers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
@@ -258,6 +260,21 @@ class Hair:
                                                None if host_gbuffer is None else C.c_void_p(host_gbuffer.data_ptr()),
                                                C.c_void_p(host_rgb.data_ptr())), "hair_render_to_host")
         self._res = (w, h)
+
+    def render_to_host_async(self, cam: dict, lam, host_rgb, host_gbuffer=None) -> int:
+        """Enqueue the frame and its device->host copies; returns the slot to pass to host_wait."""
+        w, h = cam["width"], cam["height"]
+        lam = np.atleast_1d(np.asarray(lam, dtype=np.float32))
+        c = make_camera(cam)
+        slot = C.c_int(-1)
+        self._check(self.L.hair_render_to_host_async(self.h, C.byref(c), w, h, _ptr(lam), len(lam),
+                                                     None if host_gbuffer is None else C.c_void_p(host_gbuffer.data_ptr()),
+                                                     C.c_void_p(host_rgb.data_ptr()), C.byref(slot)), "hair_render_to_host_async")
+        self._res = (w, h)
+        return slot.value
+
+    def host_wait(self, slot: int = -1):
+        self._check(self.L.hair_host_wait(self.h, int(slot)), "hair_host_wait")
 
     def render_stages(self, cam: dict, stage_mask: int, gbuffer, out_rgb):
         w, h = cam["width"], cam["height"]

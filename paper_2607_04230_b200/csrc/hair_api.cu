@@ -49,10 +49,14 @@ struct hair_ctx {
   unsigned long long* d_counters = nullptr;
   unsigned long long* h_counters = nullptr;  // pinned
   uint32_t c_max = 0;
-  // owned outputs for hair_render_to_host
-  unsigned long long* d_own_gbuf = nullptr;
-  float* d_own_rgb = nullptr;
+  // owned outputs for hair_render_to_host(_async): HAIR_HOST_SLOTS frames in flight
+  unsigned long long* d_own_gbuf[HAIR_HOST_SLOTS] = {};
+  float* d_own_rgb[HAIR_HOST_SLOTS] = {};
   size_t own_px = 0;
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_rendered[HAIR_HOST_SLOTS] = {}, ev_copied[HAIR_HOST_SLOTS] = {};
+  bool slot_used[HAIR_HOST_SLOTS] = {};
+  int next_slot = 0;
   cudaEvent_t ev[EV_RING][EV_N] = {};
   uint32_t ev_frames = 0;  // timed frames since the last hair_stats
   bool timed = false, counted = false;
@@ -289,6 +293,10 @@ int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream) {
             cudaMallocHost((void**)&c->h_counters, CNT_N * sizeof(unsigned long long)) == cudaSuccess;
   for (int f = 0; ok && f < EV_RING; ++f)
     for (int i = 0; ok && i < EV_N; ++i) ok = cudaEventCreate(&c->ev[f][i]) == cudaSuccess;
+  ok = ok && cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+  for (int k = 0; ok && k < HAIR_HOST_SLOTS; ++k)
+    ok = cudaEventCreateWithFlags(&c->ev_rendered[k], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&c->ev_copied[k], cudaEventDisableTiming) == cudaSuccess;
   if (!ok) {
     hair_destroy(c);
     return HAIR_E_CUDA;
@@ -308,8 +316,14 @@ void hair_destroy(hair_ctx* c) {
   cudaFree(c->d_vertices);
   cudaFree(c->d_colour);
   cudaFree(c->d_counters);
-  cudaFree(c->d_own_gbuf);
-  cudaFree(c->d_own_rgb);
+  if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+  for (int k = 0; k < HAIR_HOST_SLOTS; ++k) {
+    cudaFree(c->d_own_gbuf[k]);
+    cudaFree(c->d_own_rgb[k]);
+    if (c->ev_rendered[k]) cudaEventDestroy(c->ev_rendered[k]);
+    if (c->ev_copied[k]) cudaEventDestroy(c->ev_copied[k]);
+  }
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->h_counters) cudaFreeHost(c->h_counters);
   for (int f = 0; f < EV_RING; ++f)
     for (int i = 0; i < EV_N; ++i)
@@ -482,26 +496,61 @@ int hair_render_stages(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t
   return render_impl(c, cam, w, h, nullptr, 0, stage_mask & 7u, false, (unsigned long long*)out_gbuffer, out_rgb);
 }
 
-int hair_render_to_host(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam,
-                        uint32_t n_lam, uint64_t* host_gbuffer, float* host_rgb) {
+int hair_render_to_host_async(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam,
+                              uint32_t n_lam, uint64_t* host_gbuffer, float* host_rgb, int* out_slot) {
   if (!c) return HAIR_E_INVALID_ARG;
   if (!host_rgb) return fail(c, HAIR_E_INVALID_ARG, "hair_render_to_host: host_rgb is required");
   CK(cudaSetDevice(c->device));
-  size_t px = (size_t)w * h;
+  const size_t px = (size_t)w * h;
   if (px > c->own_px) {
-    cudaFree(c->d_own_gbuf);
-    cudaFree(c->d_own_rgb);
-    c->d_own_gbuf = nullptr;
-    c->d_own_rgb = nullptr;
+    CK(cudaStreamSynchronize(c->copy_stream));  // copies out of the old buffers
+    CK(cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < HAIR_HOST_SLOTS; ++k) {
+      cudaFree(c->d_own_gbuf[k]);
+      cudaFree(c->d_own_rgb[k]);
+      c->d_own_gbuf[k] = nullptr;
+      c->d_own_rgb[k] = nullptr;
+      c->slot_used[k] = false;
+    }
     c->own_px = 0;
-    CK(cudaMalloc((void**)&c->d_own_gbuf, px * 16));
-    CK(cudaMalloc((void**)&c->d_own_rgb, px * 16));
+    for (int k = 0; k < HAIR_HOST_SLOTS; ++k) {
+      CK(cudaMalloc((void**)&c->d_own_gbuf[k], px * 16));
+      CK(cudaMalloc((void**)&c->d_own_rgb[k], px * 16));
+    }
     c->own_px = px;
   }
-  int rc = render_impl(c, cam, w, h, lam, n_lam, 7u, true, c->d_own_gbuf, c->d_own_rgb);
+  const int k = c->next_slot;
+  // the slot's previous copies must have left before its buffers are overwritten (stream-ordered, no host wait)
+  if (c->slot_used[k]) CK(cudaStreamWaitEvent(c->stream, c->ev_copied[k], 0));
+  int rc = render_impl(c, cam, w, h, lam, n_lam, 7u, true, c->d_own_gbuf[k], c->d_own_rgb[k]);
   if (rc) return rc;
-  CK(cudaMemcpyAsync(host_rgb, c->d_own_rgb, px * 16, cudaMemcpyDeviceToHost, c->stream));
-  if (host_gbuffer) CK(cudaMemcpyAsync(host_gbuffer, c->d_own_gbuf, px * 16, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaEventRecord(c->ev_rendered[k], c->stream));
+  CK(cudaStreamWaitEvent(c->copy_stream, c->ev_rendered[k], 0));
+  CK(cudaMemcpyAsync(host_rgb, c->d_own_rgb[k], px * 16, cudaMemcpyDeviceToHost, c->copy_stream));
+  if (host_gbuffer) CK(cudaMemcpyAsync(host_gbuffer, c->d_own_gbuf[k], px * 16, cudaMemcpyDeviceToHost, c->copy_stream));
+  CK(cudaEventRecord(c->ev_copied[k], c->copy_stream));
+  c->slot_used[k] = true;
+  c->next_slot = (k + 1) % HAIR_HOST_SLOTS;
+  if (out_slot) *out_slot = k;
+  return HAIR_OK;
+}
+
+int hair_host_wait(hair_ctx* c, int slot) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  if (slot >= HAIR_HOST_SLOTS) return fail(c, HAIR_E_INVALID_ARG, "hair_host_wait: no such slot");
+  CK(cudaSetDevice(c->device));
+  for (int k = 0; k < HAIR_HOST_SLOTS; ++k)
+    if ((slot < 0 || slot == k) && c->slot_used[k]) CK(cudaEventSynchronize(c->ev_copied[k]));
+  return HAIR_OK;
+}
+
+int hair_render_to_host(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam,
+                        uint32_t n_lam, uint64_t* host_gbuffer, float* host_rgb) {
+  int slot = -1;
+  int rc = hair_render_to_host_async(c, cam, w, h, lam, n_lam, host_gbuffer, host_rgb, &slot);
+  if (rc) return rc;
+  rc = hair_host_wait(c, slot);
+  if (rc) return rc;
   CK(cudaStreamSynchronize(c->stream));
   return HAIR_OK;
 }

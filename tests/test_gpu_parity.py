@@ -314,6 +314,32 @@ def test_mesh_update_and_render_to_host(orc, hair_mod):
     assert torch.equal(gb2, gb3) and torch.equal(rgb2, rgb3)
 
 
+def test_render_to_host_async_pipeline(hair_mod):
+    """Two frames in flight: each host buffer, after host_wait, holds exactly what hair_render gives."""
+    import torch
+    b = hair_mod
+    sc = synth.config(2, scale=0.02, res_scale=0.3)
+    h = b.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(sc["params"])
+    cams = [dict(sc["camera"]), dict(sc["camera"]), dict(sc["camera"])]
+    cams[1]["eye"] = tuple(np.asarray(cams[1]["eye"]) + np.array([0.02, 0.0, 0.0]))
+    cams[2]["eye"] = tuple(np.asarray(cams[2]["eye"]) + np.array([0.0, 0.03, 0.0]))
+    w, hh = sc["camera"]["width"], sc["camera"]["height"]
+    host = [torch.empty((hh, w, 4), dtype=torch.float32).pin_memory() for _ in range(3)]
+    host_gb = [torch.empty((hh, w, 2), dtype=torch.int64).pin_memory() for _ in range(3)]
+    slots = [h.render_to_host_async(cams[i], sc["lam"], host[i], host_gb[i]) for i in range(3)]  # slot 0 reused
+    assert slots == [0, 1, 0]
+    h.host_wait(-1)
+    for i in range(3):
+        gb, rgb = h.render(cams[i], sc["lam"])
+        assert torch.equal(rgb.cpu(), host[i]) and torch.equal(gb.cpu(), host_gb[i]), i
+    assert not torch.equal(host[0], host[1])
+    with pytest.raises(b.HairError):
+        h.host_wait(7)
+
+
 def test_atomic_microbench_runs(hair_mod):
     import torch
     h = hair_mod.Hair(0)
