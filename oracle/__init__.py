@@ -109,6 +109,7 @@ def lib():
         L.orc_frame_raster.argtypes = [vp, vp, vp, vp, vp]
         L.orc_frame_get_gbuffer.argtypes = [vp, vp]
         L.orc_frame_set_gbuffer.argtypes = [vp, vp, u32, u32]
+        L.orc_frame_set_scene.argtypes = [vp, vp, vp, u32, u32]
         L.orc_frame_set_window.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
         L.orc_frame_set_window.restype = None
         L.orc_frame_shade.argtypes = [vp, vp, vp]
@@ -292,6 +293,15 @@ class Frame:
         h, w = g.shape[:2]
         self._wh = (w, h)
         self.L.orc_frame_set_gbuffer(self.h, _ptr(g), w, h)
+
+    def set_scene(self, zn=None, rgb=None) -> None:
+        """R-scene: zn [h][w] float32 in [0, 1] seeds the depth of both layers; rgb [h][w][3] is composited over."""
+        self._scene = (None if zn is None else np.ascontiguousarray(zn, dtype=np.float32),
+                       None if rgb is None else np.ascontiguousarray(rgb, dtype=np.float32))
+        a = self._scene[0] if self._scene[0] is not None else self._scene[1]
+        h, w = (0, 0) if a is None else a.shape[:2]
+        self.L.orc_frame_set_scene(self.h, None if self._scene[0] is None else _ptr(self._scene[0]),
+                                   None if self._scene[1] is None else _ptr(self._scene[1]), w, h)
 
     def set_window(self, x0: int = 0, y0: int = 0, x1: int = 1 << 30, y1: int = 1 << 30) -> None:
         """Sample a full-size frame: O4 / O6 / O7 only visit pixels of [x0, x1) x [y0, y1) (O6 grown by 7 px)."""

@@ -21,6 +21,10 @@
 namespace {
 
 const uint64_t EMPTY = ~0ull;
+// DESIGN.md R-scene: a word whose 40 payload bits are all ones carries no hair hit; its depth bits are the
+// scene's depth at the pixel (the far end, all ones, without a scene). Real hits never have strand id 2^24 - 1.
+const uint64_t PAYLOAD_NONE = (1ull << 40) - 1;
+inline bool none(uint64_t w) { return (w & PAYLOAD_NONE) == PAYLOAD_NONE; }
 const double PI = 3.14159265358979323846;
 
 // ---------------------------------------------------------------- hash (R26)
@@ -185,6 +189,10 @@ struct orc_frame {
   // full-frame run; this only lets a test sample a full-size frame in seconds. O6 covers the window grown by
   // the largest filter radius (7), which is what O7 reads.
   int wx0 = 0, wy0 = 0, wx1 = 1 << 30, wy1 = 1 << 30;
+  // optional scene behind / in front of the hair (R-scene): depth zn in [0, 1] per pixel and the colour the hair
+  // is composited over ("reads the existing depth buffer ... blended into the main render target")
+  std::vector<float> scene_zn;   // [H][W] or empty
+  std::vector<float> scene_rgb;  // [H][W][3] or empty
 };
 
 namespace {
@@ -745,6 +753,14 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
   f->W = k.W;
   f->H = k.H;
   f->gbuf.assign(size_t(k.W) * k.H * 2, EMPTY);
+  if (!f->scene_zn.empty()) {  // R-scene: both layers start at the scene's quantised depth (R8), payload = none
+    if (f->scene_zn.size() != size_t(k.W) * k.H) return -3;
+    for (size_t p = 0; p < size_t(k.W) * k.H; ++p) {
+      float zn = std::min(std::max(f->scene_zn[p], 0.f), 1.f);
+      uint64_t seed = (uint64_t(quant_depth(zn)) << 40) | PAYLOAD_NONE;
+      f->gbuf[p * 2] = f->gbuf[p * 2 + 1] = seed;
+    }
+  }
   if (f->v32.size() != size_t(f->n_vertices) * 4) return -1;
   uint64_t n_center = 0, n_cons = 0, n_seg = 0;
   // strand directory in slot order
@@ -822,6 +838,13 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
 void orc_frame_get_gbuffer(const orc_frame* f, uint64_t* o) {
   std::memcpy(o, f->gbuf.data(), f->gbuf.size() * sizeof(uint64_t));
 }
+int orc_frame_set_scene(orc_frame* f, const float* zn, const float* rgb, uint32_t w, uint32_t h) {
+  f->scene_zn.clear();
+  f->scene_rgb.clear();
+  if (zn) f->scene_zn.assign(zn, zn + size_t(w) * h);
+  if (rgb) f->scene_rgb.assign(rgb, rgb + size_t(w) * h * 3);
+  return 0;
+}
 void orc_frame_set_window(orc_frame* f, int x0, int y0, int x1, int y1) {
   f->wx0 = x0, f->wy0 = y0, f->wx1 = x1, f->wy1 = y1;
 }
@@ -846,8 +869,8 @@ int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) 
   for (int sx = sx0; sx < sx1; ++sx) {
     const size_t p = size_t(sy) * k.W + sx;
     uint64_t G = f->gbuf[p * 2], A = f->gbuf[p * 2 + 1];
-    if (A != EMPTY) screen_tangent(f, k, A, &f->tang[p * 4 + 2]);
-    if (G == EMPTY) continue;
+    if (!none(A)) screen_tangent(f, k, A, &f->tang[p * 4 + 2]);
+    if (none(G)) continue;
     screen_tangent(f, k, G, &f->tang[p * 4]);
     Loc l = locate(f, w_sid(G));
     if (!l.ok) return -2;
@@ -924,8 +947,8 @@ AccOut accumulate(const orc_frame* f, const orc_params* prm, int W, int H, int p
         return diff <= tauz_q;  // PAPER.md:169 threshold 1.45e-3
       };
       int cls = 0;  // 1 = centre, 2 = cons-only
-      if (GQ != EMPTY && close(GQ)) cls = 1;
-      else if (AQ != EMPTY && close(AQ)) cls = 2;
+      if (!none(GQ) && close(GQ)) cls = 1;
+      else if (!none(AQ) && close(AQ)) cls = 2;
       if (!cls) continue;
       // Eq. 9, fp32 fixed order (decides the strip membership)
       float fdx = float(dx), fdy = float(dy);
@@ -980,7 +1003,9 @@ int orc_frame_filter(orc_frame* f, const orc_camera* cam, const orc_params* prm)
     for (int px = std::max(f->wx0, 0); px < std::min(f->wx1, W); ++px) {
       size_t p = size_t(py) * W + px;
       uint64_t G = f->gbuf[p * 2], A = f->gbuf[p * 2 + 1];
-      bool isCenter = G != EMPTY, isCons = A != EMPTY;
+      bool isCenter = !none(G), isCons = !none(A);
+      if (!f->scene_rgb.empty())
+        for (int c = 0; c < 3; ++c) bg[c] = double(f->scene_rgb[p * 3 + c]);
       double C[3] = {0, 0, 0}, alpha = 0;
       const double* CP = &f->colour[p * 3];
       if (!prm->filter_on) {

@@ -122,6 +122,11 @@ int orc_frame_raster(orc_frame*, const orc_camera*, const orc_params*, const uin
                      uint64_t counts[3]);
 void orc_frame_get_gbuffer(const orc_frame*, uint64_t* out);
 int orc_frame_set_gbuffer(orc_frame*, const uint64_t* in, uint32_t w, uint32_t h);
+/* R-scene: optional scene the hair is drawn into. zn[h][w] in [0, 1] (NULL: none) seeds both layers
+ * of every pixel with depth = quant(zn), payload = all ones ("no hair hit"): a hit behind it loses the atomic
+ * min ("reads the existing depth buffer", 208-210 "keeping depth"). rgb[h][w][3] (NULL: the constant
+ * background) is what O7 composites over ("blended into the main render target"). */
+int orc_frame_set_scene(orc_frame*, const float* zn, const float* rgb, uint32_t w, uint32_t h);
 /* Restrict the pixel loops of O4, O6 (grown by 7 px) and O7 to [x0, x1) x [y0, y1). Pixels are independent in
  * all three, so values inside the window equal those of the full-frame run: a way to SAMPLE a full-size frame
  * (the raster's hit counts then cover the window only). Default / reset: 0, 0, 1 << 30, 1 << 30. */
