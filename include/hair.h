@@ -119,6 +119,19 @@ int hair_set_render_params(hair_ctx*, const hair_render_params*);
 int hair_render(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height, const float* lod_lambda,
                 uint32_t n_lambda, uint64_t* out_gbuffer, float* out_rgb);
 
+/* hair_render into an existing scene (DESIGN.md R-scene; "reads the existing depth buffer ... blended
+ * into the main render target", 208-210 "keeping depth"):
+ *  scene_zn   DEVICE, [height][width] float, normalised depth zn = A - B / z_view in [0, 1] of what is already in
+ *             the frame (clamped), or NULL. Both layers of every pixel start at its 24-bit quantisation with an
+ *             all-ones payload, so a hair hit behind the scene loses the atomic min; a hit at the same quantised
+ *             depth wins. In out_gbuffer a word whose low 40 bits are all ones means "no hair hit" (its depth bits
+ *             are the scene's; without a scene such words are all ones as in hair_render).
+ *  scene_rgb  DEVICE, [height][width][4] float, 16-byte aligned (.w ignored), or NULL: what the hair is composited
+ *             over instead of background_rgb. out_rgb.w is the hair's alpha alone. */
+int hair_render_scene(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height, const float* lod_lambda,
+                      uint32_t n_lambda, const float* scene_zn, const float* scene_rgb, uint64_t* out_gbuffer,
+                      float* out_rgb);
+
 /* Same frame, results copied to HOST memory (pinned for full speed) inside the call:
  * host_rgb [h][w][4] float is required, host_gbuffer [h][w][2] may be NULL. Synchronises the stream. */
 int hair_render_to_host(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height,

@@ -20,7 +20,7 @@ EMPTY = 0xFFFFFFFFFFFFFFFF
 
 EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_render_params",
            "hair_set_render_params", "hair_mesh_upload", "hair_mesh_update", "hair_mesh_clear",
-           "hair_render", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
+           "hair_render", "hair_render_scene", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
            "hair_debug_buffers", "hair_debug_set_vertices", "hair_atomic_microbench", "hair_abi_sizes"]
 
 
@@ -102,6 +102,7 @@ def load():
     L.hair_mesh_update.argtypes = [vp, C.c_int, C.POINTER(hair_cage)]
     L.hair_mesh_clear.argtypes = [vp]
     L.hair_render.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp]
+    L.hair_render_scene.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, vp, vp, u64p, vp]
     L.hair_render_to_host.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp]
     L.hair_render_to_host_async.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp, C.POINTER(C.c_int)]
     L.hair_host_wait.argtypes = [vp, C.c_int]
@@ -249,6 +250,21 @@ class Hair:
         c = make_camera(cam)
         self._check(self.L.hair_render(self.h, C.byref(c), w, h, _ptr(lam), len(lam),
                                        C.c_void_p(out_gbuffer.data_ptr()), C.c_void_p(out_rgb.data_ptr())), "hair_render")
+        self._res = (w, h)
+        return out_gbuffer, out_rgb
+
+    def render_scene(self, cam: dict, lam, scene_zn=None, scene_rgb=None, out_gbuffer=None, out_rgb=None):
+        """hair_render_scene: scene_zn float32 [h][w], scene_rgb float32 [h][w][4] device tensors (or None)."""
+        w, h = cam["width"], cam["height"]
+        if out_gbuffer is None or out_rgb is None:
+            out_gbuffer, out_rgb = self.alloc_outputs(w, h)
+        lam = np.atleast_1d(np.asarray(lam, dtype=np.float32))
+        c = make_camera(cam)
+        self._check(self.L.hair_render_scene(self.h, C.byref(c), w, h, _ptr(lam), len(lam),
+                                             None if scene_zn is None else C.c_void_p(scene_zn.data_ptr()),
+                                             None if scene_rgb is None else C.c_void_p(scene_rgb.data_ptr()),
+                                             C.c_void_p(out_gbuffer.data_ptr()), C.c_void_p(out_rgb.data_ptr())),
+                    "hair_render_scene")
         self._res = (w, h)
         return out_gbuffer, out_rgb
 

@@ -200,12 +200,13 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
 }
 
 int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
-                uint32_t stage_mask, bool front, unsigned long long* gbuf, float* rgb) {
+                uint32_t stage_mask, bool front, unsigned long long* gbuf, float* rgb,
+                const float* scene_zn = nullptr, const float* scene_rgb = nullptr) {
   if (!c) return HAIR_E_INVALID_ARG;
   if (!cam || !gbuf || !rgb || w == 0 || h == 0 || w > 16384 || h > 16384)
     return fail(c, HAIR_E_INVALID_ARG, "hair_render: null argument or bad resolution");
-  if (((uintptr_t)gbuf & 15) || ((uintptr_t)rgb & 15))
-    return fail(c, HAIR_E_INVALID_ARG, "hair_render: outputs must be 16-byte aligned");
+  if (((uintptr_t)gbuf & 15) || ((uintptr_t)rgb & 15) || ((uintptr_t)scene_rgb & 15) || ((uintptr_t)scene_zn & 3))
+    return fail(c, HAIR_E_INVALID_ARG, "hair_render: outputs and scene_rgb must be 16-byte aligned");
   if (!(cam->far_z > cam->near_z) || !(cam->near_z > 0.f) || !(cam->vfov_y > 0.f))
     return fail(c, HAIR_E_INVALID_ARG, "hair_render: bad camera");
   if (front && !(n_lam == 1 || n_lam == c->scene.n_grooms || (n_lam == 0 && lam == nullptr)))
@@ -239,7 +240,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_GEN);
   if (stage_mask & 1u) {
-    launch_clear(gbuf, (size_t)w * h, st);
+    launch_clear(gbuf, (size_t)w * h, scene_zn, st);
     ++launches;
   }
   mark(EV_CLEAR);
@@ -256,8 +257,8 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_SHADE);
   if (stage_mask & 4u) {
-    launches += launch_filter(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour, (float4*)rgb,
-                              c->d_counters, count, st);
+    launches += launch_filter(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour,
+                              (const float4*)scene_rgb, (float4*)rgb, c->d_counters, count, st);
   }
   mark(EV_FILTER);
   CK(cudaGetLastError());
@@ -489,6 +490,11 @@ int hair_mesh_clear(hair_ctx* c) {
 int hair_render(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
                 uint64_t* out_gbuffer, float* out_rgb) {
   return render_impl(c, cam, w, h, lam, n_lam, 7u, true, (unsigned long long*)out_gbuffer, out_rgb);
+}
+
+int hair_render_scene(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
+                      const float* scene_zn, const float* scene_rgb, uint64_t* out_gbuffer, float* out_rgb) {
+  return render_impl(c, cam, w, h, lam, n_lam, 7u, true, (unsigned long long*)out_gbuffer, out_rgb, scene_zn, scene_rgb);
 }
 
 int hair_render_stages(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, uint32_t stage_mask,

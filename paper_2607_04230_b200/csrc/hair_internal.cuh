@@ -11,6 +11,8 @@
 #include "../../include/hair.h"
 
 #define HAIR_EMPTY 0xFFFFFFFFFFFFFFFFull
+// R-scene: a word whose 40 payload bits are all ones carries no hair hit (its depth is the scene's, or the far end)
+#define HAIR_PAYLOAD_NONE 0xFFFFFFFFFFull
 #define RAS_CHUNK 31  // segments a raster warp draws at once (32 vertices, neighbour by shuffle)
 #define RAS_GROUP 4   // chunks per unit of the raster's device-side work queue
 #define HAIR_ROW 44  // floats per control-point row of the per-bundle table (== 12 mod 32: LDS.128 conflict-free)
@@ -120,6 +122,8 @@ __device__ __forceinline__ unsigned long long pack_word(float zn, uint32_t sid, 
   uint32_t lo = (sid << 16) | (j << 9) | quant_t(t);
   return ((unsigned long long)hi << 32) | lo;
 }
+__device__ __forceinline__ bool w_none(unsigned long long w) { return (w & HAIR_PAYLOAD_NONE) == HAIR_PAYLOAD_NONE; }
+__device__ __forceinline__ bool w_none(uint32_t lo, uint32_t hi) { return lo == 0xFFFFFFFFu && (hi & 0xFFu) == 0xFFu; }
 __device__ __forceinline__ uint32_t w_dq(unsigned long long w) { return (uint32_t)(w >> 40); }
 __device__ __forceinline__ uint32_t w_sid(unsigned long long w) { return (uint32_t)(w >> 16) & 0xFFFFFFu; }
 __device__ __forceinline__ uint32_t w_j(unsigned long long w) { return (uint32_t)(w >> 9) & 0x7Fu; }
@@ -158,14 +162,14 @@ void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaA
                      uint32_t* grp, unsigned long long* counters, cudaStream_t st);
 void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices,
                      unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st);
-void launch_clear(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
+void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_zn, cudaStream_t st);
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                    unsigned long long* counters, bool count, int n_sm, cudaStream_t st);
 void launch_shade(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
                   ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st);
 int launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
-                   ShadeParams sp, const unsigned long long* gbuf, const float4* colour, float4* out,
-                   unsigned long long* counters, bool count, cudaStream_t st);
+                   ShadeParams sp, const unsigned long long* gbuf, const float4* colour, const float4* scene_rgb,
+                   float4* out, unsigned long long* counters, bool count, cudaStream_t st);
 void launch_atomic_microbench(int mode, unsigned long long* words, unsigned long long n_words,
                               unsigned long long n_ops, uint32_t hot, int n_sm, cudaStream_t st);

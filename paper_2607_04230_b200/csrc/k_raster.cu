@@ -248,17 +248,25 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
   }
 }
 
-// clear both layers to "empty" (all ones): 16 B per pixel, streaming stores
-__global__ void __launch_bounds__(256) k_clear(uint4* __restrict__ g, size_t n16) {
+// clear both layers to "no hit": all ones, or (R-scene) the scene's quantised depth (R8) with an all-ones payload,
+// which is the paper's pre-existing depth buffer: a hit behind it loses the atomic min
+__global__ void __launch_bounds__(256) k_clear(uint4* __restrict__ g, size_t n16, const float* __restrict__ scene_zn) {
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) g[i] = ones;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) {
+    uint4 v = ones;
+    if (scene_zn) {
+      const uint32_t hi = (quant_depth(fminf(fmaxf(__ldg(&scene_zn[i]), 0.f), 1.f)) << 8) | 0xFFu;
+      v.y = v.w = hi;
+    }
+    g[i] = v;
+  }
 }
 
-void launch_clear(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st) {
+void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_zn, cudaStream_t st) {
   size_t blocks = (n_pixels + 255) / 256;
   if (blocks > 148 * 16) blocks = 148 * 16;
-  k_clear<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels);
+  k_clear<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels, scene_zn);
 }
 
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,

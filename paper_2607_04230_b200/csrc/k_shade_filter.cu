@@ -38,7 +38,7 @@ k_shade(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const 
   if (p >= n_px) return;
   const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
   const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
-  if (G == HAIR_EMPTY) return;  // colour is only ever read where a centre hit exists
+  if (w_none(G)) return;  // colour is only ever read where a centre hit exists
   const Loc l = locate_strand(sc, table, w_sid(G));
   const GroomDev& g = sc->g[l.groom];
   const int j = (int)w_j(G), C = (int)l.C;
@@ -132,7 +132,7 @@ template <int R>
 __global__ void __launch_bounds__(256)
 k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const float4* __restrict__ vertices,
          CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, const float4* __restrict__ colour,
-         float4* __restrict__ out) {
+         const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
   constexpr int SW = FT_W + 2 * R, SH = FT_H + 2 * R, NS = SW * SH;
   extern __shared__ float4 fsm[];
   float4* s_col = fsm;                                  // [NS] rgb, -kC |rgb|^2 (zeros where no centre hit)
@@ -157,13 +157,22 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
       G[k] = ((unsigned long long)raw.y << 32) | raw.x;
       A[k] = ((unsigned long long)raw.w << 32) | raw.z;
     }
-    hit |= A[k] != HAIR_EMPTY;  // centre layer is a subset of the conservative one (R10)
+    hit |= !w_none(A[k]);  // centre layer is a subset of the conservative one (R10)
   }
-  const float4 bg = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
+  // what the hair is composited over (R29): the constant background, or the scene's colour (R-scene)
+  float4 bg[2];
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    bg[k] = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
+    if (scene_rgb && inside[k]) {
+      const float4 b = __ldg(&scene_rgb[(size_t)(y0 + ly + 8 * k) * W + x0 + lx]);
+      bg[k] = make_float4(b.x, b.y, b.z, 0.f);
+    }
+  }
   if (!__syncthreads_or(hit)) {  // empty tile: background only
 #pragma unroll
     for (int k = 0; k < 2; ++k)
-      if (inside[k]) out[(size_t)(y0 + ly + 8 * k) * W + x0 + lx] = bg;
+      if (inside[k]) out[(size_t)(y0 + ly + 8 * k) * W + x0 + lx] = bg[k];
     return;
   }
   // ---- (1) tile + halo to shared memory
@@ -175,8 +184,8 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
     if (gx >= 0 && gx < W && gy >= 0 && gy < H) {  // samples outside the image do not exist
       const size_t q = (size_t)gy * W + gx;
       const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + q);
-      if ((raw.z & raw.w) != 0xFFFFFFFFu) dA = raw.w >> 8;
-      if ((raw.x & raw.y) != 0xFFFFFFFFu) {
+      if (!w_none(raw.z, raw.w)) dA = raw.w >> 8;
+      if (!w_none(raw.x, raw.y)) {
         dG = raw.y >> 8;
         const float4 c = __ldg(&colour[q]);
         c4 = make_float4(c.x, c.y, c.z, -sp.kC * (c.x * c.x + c.y * c.y + c.z * c.z));
@@ -195,7 +204,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
   const uint32_t lt_mask = (1u << lx) - 1u;
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
-    const bool isCenter = G[k] != HAIR_EMPTY, isCons = A[k] != HAIR_EMPTY;
+    const bool isCenter = !w_none(G[k]), isCons = !w_none(A[k]);
     Tc[k] = Ta[k] = make_float2(1.f, 0.f);
     if (isCenter) {
       Tc[k] = screen_tangent(sc, table, vertices, cam, G[k]);
@@ -322,20 +331,24 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
     }
     const float ia = 1.f - alpha;
     out[(size_t)(y0 + ly + 8 * k) * W + x0 + lx] =
-        make_float4(alpha * r + ia * bg.x, alpha * g + ia * bg.y, alpha * b + ia * bg.z, alpha);
+        make_float4(alpha * r + ia * bg[k].x, alpha * g + ia * bg[k].y, alpha * b + ia * bg[k].z, alpha);
   }
 }
 
 // filter off, or r = 0 (window = the pixel itself): out = centre colour over the background
 __global__ void __launch_bounds__(256)
 k_filter_passthrough(CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf,
-                     const float4* __restrict__ colour, float4* __restrict__ out) {
+                     const float4* __restrict__ colour, const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
   const size_t n_px = (size_t)cam.W * cam.H;
   const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n_px) return;
   const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
   float4 o = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
-  if ((raw.x & raw.y) != 0xFFFFFFFFu) {
+  if (scene_rgb) {
+    const float4 b = __ldg(&scene_rgb[p]);
+    o = make_float4(b.x, b.y, b.z, 0.f);
+  }
+  if (!w_none(raw.x, raw.y)) {
     const float4 c = __ldg(&colour[p]);
     o = make_float4(c.x, c.y, c.z, 1.f);
   }
@@ -348,8 +361,8 @@ k_count_pixels(const unsigned long long* __restrict__ gbuf, size_t n_px, unsigne
   uint32_t nc = 0, na = 0;
   for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n_px; p += (size_t)gridDim.x * blockDim.x) {
     const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
-    nc += (raw.x & raw.y) != 0xFFFFFFFFu;
-    na += (raw.z & raw.w) != 0xFFFFFFFFu;
+    nc += !w_none(raw.x, raw.y);
+    na += !w_none(raw.z, raw.w);
   }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) {
@@ -370,18 +383,18 @@ void launch_shade(const SceneDev* d_scene, const uint4* table, const float4* ver
 
 template <int R>
 static void launch_filter_r(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
-                            ShadeParams sp, const unsigned long long* gbuf, const float4* colour, float4* out,
-                            cudaStream_t st) {
+                            ShadeParams sp, const unsigned long long* gbuf, const float4* colour,
+                            const float4* scene_rgb, float4* out, cudaStream_t st) {
   constexpr int NS = (FT_W + 2 * R) * (FT_H + 2 * R);
   constexpr size_t smem = (size_t)NS * (sizeof(float4) + 2 * sizeof(uint32_t)) + 2 * FT_W * FT_H * sizeof(float4);
   cudaFuncSetAttribute(k_filter<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   dim3 grid((cam.W + FT_W - 1) / FT_W, (cam.H + FT_H - 1) / FT_H);
-  k_filter<R><<<grid, 256, smem, st>>>(d_scene, table, vertices, cam, sp, gbuf, colour, out);
+  k_filter<R><<<grid, 256, smem, st>>>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out);
 }
 
 int launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
-                  ShadeParams sp, const unsigned long long* gbuf, const float4* colour, float4* out,
-                  unsigned long long* counters, bool count, cudaStream_t st) {
+                  ShadeParams sp, const unsigned long long* gbuf, const float4* colour, const float4* scene_rgb,
+                  float4* out, unsigned long long* counters, bool count, cudaStream_t st) {
   const size_t n = (size_t)cam.W * cam.H;
   int launches = 1;
   if (count) {
@@ -389,18 +402,18 @@ int launch_filter(const SceneDev* d_scene, const uint4* table, const float4* ver
     ++launches;
   }
   if (!sp.filter_on) {
-    k_filter_passthrough<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cam, sp, gbuf, colour, out);
+    k_filter_passthrough<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cam, sp, gbuf, colour, scene_rgb, out);
     return launches;
   }
   switch (sp.r) {
-    case 0: launch_filter_r<0>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
-    case 1: launch_filter_r<1>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
-    case 2: launch_filter_r<2>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
-    case 3: launch_filter_r<3>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
-    case 4: launch_filter_r<4>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
-    case 5: launch_filter_r<5>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
-    case 6: launch_filter_r<6>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
-    default: launch_filter_r<7>(d_scene, table, vertices, cam, sp, gbuf, colour, out, st); break;
+    case 0: launch_filter_r<0>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 1: launch_filter_r<1>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 2: launch_filter_r<2>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 3: launch_filter_r<3>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 4: launch_filter_r<4>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 5: launch_filter_r<5>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 6: launch_filter_r<6>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    default: launch_filter_r<7>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
   }
   return launches;
 }

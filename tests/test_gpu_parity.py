@@ -314,6 +314,60 @@ def test_mesh_update_and_render_to_host(orc, hair_mod):
     assert torch.equal(gb2, gb3) and torch.equal(rgb2, rgb3)
 
 
+@pytest.mark.parametrize("filter_on", [True, False])
+def test_render_into_scene_stagewise(orc, hair_mod, filter_on):
+    """hair_render_scene (R-scene): a bumpy wall through the groom's depth range and a scene colour, against the
+    oracle stage by stage, plus the min identity on the GPU's own buffers."""
+    import torch
+    b = hair_mod
+    sc = synth.config(2, scale=0.08, res_scale=0.4)
+    cam, lam = sc["camera"], sc["lam"]
+    W, H = cam["width"], cam["height"]
+    prm = dict(sc["params"], filter_on=filter_on)
+    h = b.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(prm)
+    gb0, rgb0 = h.render(cam, lam)
+    g0 = b.gbuffer_to_numpy(gb0)
+    hit = g0[..., 1] != EMPTY
+    zn_hair = ((g0[..., 1] >> np.uint64(40)).astype(np.float64) / 16777215.0)[hit]
+    yy, xx = np.mgrid[0:H, 0:W]
+    zn = (np.median(zn_hair) + 0.5 * (zn_hair.max() - zn_hair.min()) * np.sin(xx / 17.0) * np.cos(yy / 23.0)).astype(np.float32)
+    zn[: H // 8] = 1.5   # clamped to the far end
+    zn[-H // 8:] = -0.5  # clamped to the near end: hides everything there
+    rng = np.random.default_rng(11)
+    srgb = rng.random((H, W, 4)).astype(np.float32)
+    gb, rgb = h.render_scene(cam, lam, torch.from_numpy(zn).cuda(), torch.from_numpy(srgb).cuda())
+    G = b.gbuffer_to_numpy(gb)
+    verts = h.debug_vertices().cpu().numpy()
+    # (i) min identity on the GPU's own results: seeded resolve == min(hair-only resolve, seed)
+    z = np.clip(zn, np.float32(0), np.float32(1))
+    dq = np.minimum((z * np.float32(16777215.0) + np.float32(0.5)).astype(np.float32).astype(np.uint64), np.uint64(0xFFFFFE))
+    seed = (dq << np.uint64(40)) | np.uint64((1 << 40) - 1)
+    assert np.array_equal(G, np.minimum(g0, seed[..., None]))
+    assert (hit & (G[..., 1] == seed)).sum() > 500 and (hit & (G[..., 1] != seed)).sum() > 500
+    # (ii) oracle raster into the same scene on the GPU's vertices
+    f = orc.Frame(sc["grooms"])
+    f.lod(cam, lam)
+    f.generate()
+    f.set_vertices_f32(verts)
+    f.set_scene(zn=zn, rgb=srgb[..., :3])
+    f.raster(cam, prm)
+    assert np.array_equal(f.gbuffer(), G)
+    # (iii) oracle shade + filter on the GPU's G-buffer, composited over the scene colour
+    f.set_gbuffer(G)
+    f.shade(cam, prm)
+    out = f.filter(cam, prm)
+    got = rgb.cpu().numpy().astype(np.float64)
+    assert np.abs(out - got).max() <= TOL_RGB
+    assert psnr(out[..., :3], got[..., :3], max(float(out[..., :3].max()), 1.0)) > MIN_PSNR
+    assert np.array_equal(got[-H // 8:, :, :3], srgb[-H // 8:, :, :3].astype(np.float64)) and (got[-H // 8:, :, 3] == 0).all()
+    # NULL scene == hair_render
+    gb2, rgb2 = h.render_scene(cam, lam, None, None)
+    assert torch.equal(gb2, gb0) and torch.equal(rgb2, rgb0)
+
+
 def test_render_to_host_async_pipeline(hair_mod):
     """Two frames in flight: each host buffer, after host_wait, holds exactly what hair_render gives."""
     import torch
