@@ -110,6 +110,7 @@ def lib():
         L.orc_frame_get_gbuffer.argtypes = [vp, vp]
         L.orc_frame_set_gbuffer.argtypes = [vp, vp, u32, u32]
         L.orc_frame_set_scene.argtypes = [vp, vp, vp, u32, u32]
+        L.orc_frame_set_pass.argtypes = [vp, u32, vp, vp, u32, u32]
         L.orc_frame_set_window.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
         L.orc_frame_set_window.restype = None
         L.orc_frame_shade.argtypes = [vp, vp, vp]
@@ -179,6 +180,7 @@ class Frame:
         self.L = lib()
         self.h = C.c_void_p(self.L.orc_frame_create())
         self._keep = []
+        self._n_grooms = 0
         for g in grooms:
             self.add_groom(g)
 
@@ -204,6 +206,7 @@ class Frame:
         r = self.L.orc_frame_add_groom(self.h, C.byref(G))
         if r < 0:
             raise ValueError(f"orc_frame_add_groom failed: {r}")
+        self._n_grooms += 1
         return r
 
     # ---- O1
@@ -302,6 +305,50 @@ class Frame:
         h, w = (0, 0) if a is None else a.shape[:2]
         self.L.orc_frame_set_scene(self.h, None if self._scene[0] is None else _ptr(self._scene[0]),
                                    None if self._scene[1] is None else _ptr(self._scene[1]), w, h)
+
+    def set_pass(self, groom_mask: int = 0xFFFFFFFF, dq=None, alpha=None) -> None:
+        """R-seq: the state of one sequential pass (see hair_oracle.h); no arguments = reset."""
+        self._pass = (None if dq is None else np.ascontiguousarray(dq, dtype=np.uint32),
+                      None if alpha is None else np.ascontiguousarray(alpha, dtype=np.float32))
+        a = self._pass[0] if self._pass[0] is not None else self._pass[1]
+        h, w = (0, 0) if a is None else a.shape[:2]
+        self.L.orc_frame_set_pass(self.h, groom_mask & 0xFFFFFFFF, None if self._pass[0] is None else _ptr(self._pass[0]),
+                                  None if self._pass[1] is None else _ptr(self._pass[1]), w, h)
+
+    def render_sequential(self, cam: dict, prm: dict, lam, scene_zn=None, scene_rgb=None):
+        """PAPER.md:208-210, DESIGN.md R-seq: the grooms one after the other, each through O1-O7 on its own, its
+        result blended over the target so far, the centre layer's depth kept for the next pass. Returns
+        (out [h][w][4], G-buffer of the last pass, kept depth [h][w] uint32)."""
+        h, w = cam["height"], cam["width"]
+        bgc = np.asarray(prm.get("background_rgb", (0.0, 0.0, 0.0)), dtype=np.float32)
+        target = (np.broadcast_to(bgc, (h, w, 3)).copy() if scene_rgb is None
+                  else np.ascontiguousarray(scene_rgb, dtype=np.float32)[..., :3].copy())
+        alpha = np.zeros((h, w), np.float32)
+        if scene_zn is None:
+            dq = np.full((h, w), 0xFFFFFF, np.uint32)
+        else:  # R8 quantisation of the scene's depth, in fp32
+            z = np.clip(np.asarray(scene_zn, np.float32), np.float32(0), np.float32(1))
+            dq = np.minimum((z * np.float32(16777215.0) + np.float32(0.5)).astype(np.float32).astype(np.uint32),
+                            np.uint32(0xFFFFFE))
+        out = np.concatenate([target.astype(np.float64), np.zeros((h, w, 1))], -1)
+        g = None
+        for gi in range(self._n_grooms):
+            self.set_pass(1 << gi, dq, alpha)
+            self.set_scene(None, target)
+            self.lod(cam, lam)
+            self.generate()
+            self.set_vertices_f32(self.vertices_f32())
+            self.raster(cam, prm)
+            self.shade(cam, prm)
+            out = self.filter(cam, prm)
+            g = self.gbuffer()
+            dq = (g[..., 0] >> np.uint64(40)).astype(np.uint32)  # centre layer: hit depth, else the depth kept so far
+            # the next pass composites over this pass's result (fp32 target, as the render target is)
+            target = out[..., :3].astype(np.float32)
+            alpha = out[..., 3].astype(np.float32)
+        self.set_pass()
+        self.set_scene(None, None)
+        return out, g, dq
 
     def set_window(self, x0: int = 0, y0: int = 0, x1: int = 1 << 30, y1: int = 1 << 30) -> None:
         """Sample a full-size frame: O4 / O6 / O7 only visit pixels of [x0, x1) x [y0, y1) (O6 grown by 7 px)."""

@@ -193,6 +193,11 @@ struct orc_frame {
   // is composited over ("reads the existing depth buffer ... blended into the main render target")
   std::vector<float> scene_zn;   // [H][W] or empty
   std::vector<float> scene_rgb;  // [H][W][3] or empty
+  // sequential per-groom passes (DESIGN.md R-seq): the depth kept from the passes before,
+  // already quantised (takes precedence over scene_zn), the alpha accumulated so far, and the grooms of this pass
+  std::vector<uint32_t> scene_dq;   // [H][W] or empty
+  std::vector<float> scene_alpha;   // [H][W] or empty
+  uint32_t groom_mask = 0xFFFFFFFFu;
 };
 
 namespace {
@@ -644,6 +649,7 @@ int orc_frame_lod(orc_frame* f, const orc_camera* cam, const float* lambda, uint
             e.C = o[0] ? o[2] : 0;
           }
         }
+        if (!((f->groom_mask >> (&g - &f->grooms[0])) & 1u)) e.nlod = e.C = 0;  // R-seq: not in this pass
         f->table.push_back(e);
         f->L.push_back(Lsel);
       }
@@ -761,6 +767,11 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
       f->gbuf[p * 2] = f->gbuf[p * 2 + 1] = seed;
     }
   }
+  if (!f->scene_dq.empty()) {  // R-seq: depth kept from the previous passes, as the 24-bit integers themselves
+    if (f->scene_dq.size() != size_t(k.W) * k.H) return -3;
+    for (size_t p = 0; p < size_t(k.W) * k.H; ++p)
+      f->gbuf[p * 2] = f->gbuf[p * 2 + 1] = (uint64_t(f->scene_dq[p] & 0xFFFFFFu) << 40) | PAYLOAD_NONE;
+  }
   if (f->v32.size() != size_t(f->n_vertices) * 4) return -1;
   uint64_t n_center = 0, n_cons = 0, n_seg = 0;
   // strand directory in slot order
@@ -843,6 +854,14 @@ int orc_frame_set_scene(orc_frame* f, const float* zn, const float* rgb, uint32_
   f->scene_rgb.clear();
   if (zn) f->scene_zn.assign(zn, zn + size_t(w) * h);
   if (rgb) f->scene_rgb.assign(rgb, rgb + size_t(w) * h * 3);
+  return 0;
+}
+int orc_frame_set_pass(orc_frame* f, uint32_t groom_mask, const uint32_t* dq, const float* alpha, uint32_t w, uint32_t h) {
+  f->groom_mask = groom_mask;
+  f->scene_dq.clear();
+  f->scene_alpha.clear();
+  if (dq) f->scene_dq.assign(dq, dq + size_t(w) * h);
+  if (alpha) f->scene_alpha.assign(alpha, alpha + size_t(w) * h);
   return 0;
 }
 void orc_frame_set_window(orc_frame* f, int x0, int y0, int x1, int y1) {
@@ -1033,7 +1052,9 @@ int orc_frame_filter(orc_frame* f, const orc_camera* cam, const orc_params* prm)
         }
       }
       for (int c = 0; c < 3; ++c) f->out[p * 4 + c] = alpha * C[c] + (1 - alpha) * bg[c];  // R29
-      f->out[p * 4 + 3] = alpha;
+      // alpha of everything drawn so far: "over" (R-seq); without earlier passes this is alpha itself
+      double a_bg = f->scene_alpha.empty() ? 0.0 : double(f->scene_alpha[p]);
+      f->out[p * 4 + 3] = alpha + (1 - alpha) * a_bg;
     }
   return 0;
 }

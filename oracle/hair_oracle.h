@@ -127,6 +127,12 @@ int orc_frame_set_gbuffer(orc_frame*, const uint64_t* in, uint32_t w, uint32_t h
  * min ("reads the existing depth buffer", 208-210 "keeping depth"). rgb[h][w][3] (NULL: the constant
  * background) is what O7 composites over ("blended into the main render target"). */
 int orc_frame_set_scene(orc_frame*, const float* zn, const float* rgb, uint32_t w, uint32_t h);
+/* R-seq ("each groom is processed sequentially ... blended into the render target
+ * before the next ... preserving the depth buffer between groom passes"): state of ONE pass. groom_mask: bit g set
+ * = groom g is drawn in this pass (O1 gives the others N_LOD = 0); dq[h][w]: the depth kept so far as 24-bit
+ * integers (NULL: none; takes precedence over the scene's zn); alpha[h][w]: the alpha accumulated so far (NULL: 0),
+ * O7 writes out.w = a + (1 - a) alpha. Reset with (0xFFFFFFFF, NULL, NULL, 0, 0). */
+int orc_frame_set_pass(orc_frame*, uint32_t groom_mask, const uint32_t* dq, const float* alpha, uint32_t w, uint32_t h);
 /* Restrict the pixel loops of O4, O6 (grown by 7 px) and O7 to [x0, x1) x [y0, y1). Pixels are independent in
  * all three, so values inside the window equal those of the full-frame run: a way to SAMPLE a full-size frame
  * (the raster's hit counts then cover the window only). Default / reset: 0, 0, 1 << 30, 1 << 30. */

@@ -115,3 +115,84 @@ def test_half_wall_leaves_the_other_half_alone(orc, base):
     r = sc["params"].get("filter_radius", 5)
     assert np.array_equal(out[:, W // 2 + r:], out0[:, W // 2 + r:])  # beyond the filter's reach of the wall
     assert (out[:, : W // 2, 3] == 0).all()
+
+
+# ------------------------------------------------------------------ sequential per-groom passes (R-seq)
+def _two_grooms(dz, dx=0.0):
+    """config-1 groom twice: the copy shifted by (dx, 0, -dz) (farther from the camera on +z for dz > 0)."""
+    sc = synth.config(1, scale=0.5)
+    g0 = sc["grooms"][0]
+    g1 = dict(g0)
+    g1["pos"] = (g0["pos"] + np.array([dx, 0.0, -dz], np.float32)).astype(np.float32)
+    g1["style"] = dict(g0["style"], seed=g0["style"]["seed"] + 17)
+    sc["grooms"] = [g0, g1]
+    sc["lam"] = [0.0, 0.0]
+    return sc
+
+
+def test_sequential_single_groom_equals_single_resolve(orc, base):
+    sc, g0, out0 = base
+    f = orc.Frame(sc["grooms"])
+    out, g, dq = f.render_sequential(sc["camera"], sc["params"], sc["lam"])
+    assert np.array_equal(g, g0) and np.array_equal(out, out0)
+    assert np.array_equal(dq, (g0[..., 0] >> np.uint64(40)).astype(np.uint32))
+
+
+def test_sequential_disjoint_grooms_equal_single_resolve(orc):
+    """Two grooms far apart on screen do not interact: both orders of processing and the one-resolve frame
+    give the same image."""
+    sc = _two_grooms(dz=0.0, dx=0.6)
+    sc["camera"] = synth.look_from_z((0.3, 0.05, 0.0), 1.0, 400, 160)
+    f = orc.Frame(sc["grooms"])
+    out_seq, _, _ = f.render_sequential(sc["camera"], sc["params"], sc["lam"])
+    f2 = orc.Frame(sc["grooms"])
+    out_one = f2.render(sc["camera"], sc["params"], sc["lam"])
+    hit = out_one[..., 3] > 0
+    cols = np.where(hit.any(0))[0]
+    assert (np.diff(cols) > 2 * 7 + 2).any(), "the two grooms must be separated by more than the filter's reach"
+    assert np.abs(out_seq - out_one).max() < 1e-6  # fp32 target between the passes
+    f3 = orc.Frame(sc["grooms"][::-1])
+    out_rev, _, _ = f3.render_sequential(sc["camera"], sc["params"], sc["lam"])
+    assert np.abs(out_rev - out_one).max() < 1e-6
+
+
+def test_sequential_groom_behind_an_opaque_one_is_rejected(orc):
+    """Second groom = a copy 40 cm behind the first (more than the groom is deep): wherever the first pass left centre hits, every hit of the
+    second pass is farther and loses against the kept depth in both layers, so those pixels keep pass 1's
+    depth, colour and alpha."""
+    sc = _two_grooms(dz=0.4)
+    cam, prm = sc["camera"], sc["params"]
+    f1 = orc.Frame(sc["grooms"][:1])
+    out1 = f1.render(cam, prm, 0.0)
+    g1 = f1.gbuffer()
+    f = orc.Frame(sc["grooms"])
+    out, g, dq = f.render_sequential(cam, prm, sc["lam"])
+    c1 = (g1[..., 0] & PAYLOAD_NONE) != PAYLOAD_NONE
+    # centre layer of pass 2 at pass-1 centre pixels: no hit, depth = pass 1's
+    assert ((g[..., 0][c1] & PAYLOAD_NONE) == PAYLOAD_NONE).all()
+    assert np.array_equal(dq[c1], (g1[..., 0][c1] >> np.uint64(40)).astype(np.uint32))
+    # the second groom does show where the first left holes
+    assert (((g[..., 0] & PAYLOAD_NONE) != PAYLOAD_NONE) & ~c1).sum() > 50
+    # alpha only grows, and is the "over" of the two passes: 1 - (1 - a1)(1 - a2) >= a1
+    assert (out[..., 3] >= out1[..., 3].astype(np.float32) - 1e-7).all() and out[..., 3].max() <= 1 + 1e-7
+    # no word of pass 2 at those pixels (both layers were seeded with the kept depth), so pass 2 composites
+    # nothing there: the pixel keeps pass 1's colour and alpha (through the fp32 target)
+    assert ((g[..., 1][c1] & PAYLOAD_NONE) == PAYLOAD_NONE).all()
+    assert np.array_equal(out[c1][:, :3], out1[c1][:, :3].astype(np.float32).astype(np.float64))
+    assert np.array_equal(out[c1][:, 3], out1[c1][:, 3].astype(np.float32).astype(np.float64))
+
+
+def test_groom_mask_only_changes_the_masked_bundles(orc):
+    sc = _two_grooms(dz=0.05)
+    f = orc.Frame(sc["grooms"])
+    f.lod(sc["camera"], sc["lam"])
+    t_all, _ = f.table()
+    f.set_pass(0b10)
+    f.lod(sc["camera"], sc["lam"])
+    t_1, _ = f.table()
+    n0 = len(t_all) // 2
+    assert (t_1[:n0, :2] == 0).all() and np.array_equal(t_1[n0:, :2], t_all[n0:, :2])
+    assert np.array_equal(t_1[n0:, 2], t_all[n0:, 2] - t_all[n0, 2])  # scans restart: only this pass's strands exist
+    f.set_pass()
+    f.lod(sc["camera"], sc["lam"])
+    assert np.array_equal(f.table()[0], t_all)
