@@ -227,6 +227,17 @@ def run_cuda(args):
     ms_e2e = replicas.max_over_ranks(ms_e2e, dist, dev)
     e2e_val = replicas.job_rate(n_seg, world, ms_e2e) / 1e9
 
+    # ---- the paper's sequential per-groom compositing, same scene, untimed leg
+    for _ in range(3):
+        h.render_sequential(cam, lam, None, None, gb, rgb)
+    barrier()
+    e0.record()
+    for _ in range(10):
+        h.render_sequential(cam, lam, None, None, gb, rgb)
+    e1.record()
+    barrier()
+    ms_seq = e0.elapsed_time(e1) / 10
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -331,6 +342,9 @@ def run_cuda(args):
         "counts": {k: cnt[k] for k in ("n_bundles", "n_bundles_culled", "n_strands_total", "n_strands_lod", "n_vertices",
                                        "n_segments", "n_segments_drawn", "n_segments_live", "n_atomics_center", "n_atomics_cons",
                                        "n_atomics_issued", "n_pixels_center", "n_pixels_cons")},
+        "sequential_per_groom": {"ms_per_step": ms_seq, "what": "hair_render_sequential: one LOD..filter pass per groom, "
+                                 "depth kept, blended over the target (PAPER.md:208-210); the headline frame resolves "
+                                 "all grooms in one G-buffer instead (DESIGN.md R15)"},
         "cpu_baseline": cpu_baseline, "clocks": clocks,
     }
     print(json.dumps(line))

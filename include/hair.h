@@ -103,6 +103,9 @@ typedef struct {
   uint32_t n_lights;
   float ambient_rgb[3], k_d, k_R, k_TRT, background_rgb[3];
   uint32_t flags; /* HAIR_FLAG_* */
+  uint32_t groom_mask; /* bit g set = groom g (upload order) is drawn; default all ones. Grooms left out get
+                          N_LOD = 0 in the LOD pass, so the frame is exactly the frame of the remaining grooms
+                          (strand ids in the words stay global). */
 } hair_render_params;
 
 void hair_default_render_params(hair_render_params* out);
@@ -131,6 +134,18 @@ int hair_render(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height, 
 int hair_render_scene(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height, const float* lod_lambda,
                       uint32_t n_lambda, const float* scene_zn, const float* scene_rgb, uint64_t* out_gbuffer,
                       float* out_rgb);
+
+/* The paper's multi-groom path (DESIGN.md R-seq): the grooms one after the other in upload
+ * order, each through the whole pipeline on its own (LOD .. filter), its filtered result blended over the target
+ * so far, the depth of its centre layer kept so that later grooms are rejected behind it. hair_render, by
+ * contrast, resolves all grooms in one G-buffer and filters once (R15). Arguments as hair_render_scene.
+ * After the call out_gbuffer holds the LAST pass: that groom's words, elsewhere "no hit" words carrying the depth
+ * kept from all passes; out_rgb.w = the accumulated alpha 1 - prod(1 - alpha_g). hair_stats then reports the last
+ * pass's counts, gpu_launches of all passes, and stage times averaged per PASS. Uses one more width x height x
+ * 16-byte buffer inside the context (allocated on first use). */
+int hair_render_sequential(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height, const float* lod_lambda,
+                           uint32_t n_lambda, const float* scene_zn, const float* scene_rgb, uint64_t* out_gbuffer,
+                           float* out_rgb);
 
 /* Same frame, results copied to HOST memory (pinned for full speed) inside the call:
  * host_rgb [h][w][4] float is required, host_gbuffer [h][w][2] may be NULL. Synchronises the stream. */

@@ -20,7 +20,7 @@ EMPTY = 0xFFFFFFFFFFFFFFFF
 
 EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_render_params",
            "hair_set_render_params", "hair_mesh_upload", "hair_mesh_update", "hair_mesh_clear",
-           "hair_render", "hair_render_scene", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
+           "hair_render", "hair_render_scene", "hair_render_sequential", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
            "hair_debug_buffers", "hair_debug_set_vertices", "hair_atomic_microbench", "hair_abi_sizes"]
 
 
@@ -59,7 +59,7 @@ class hair_render_params(C.Structure):
                 ("light_pos", (C.c_float * 3) * 4), ("light_rgb", (C.c_float * 3) * 4),
                 ("n_lights", C.c_uint32), ("ambient_rgb", C.c_float * 3),
                 ("k_d", C.c_float), ("k_R", C.c_float), ("k_TRT", C.c_float),
-                ("background_rgb", C.c_float * 3), ("flags", C.c_uint32)]
+                ("background_rgb", C.c_float * 3), ("flags", C.c_uint32), ("groom_mask", C.c_uint32)]
 
 
 class hair_stats_t(C.Structure):
@@ -103,6 +103,7 @@ def load():
     L.hair_mesh_clear.argtypes = [vp]
     L.hair_render.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp]
     L.hair_render_scene.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, vp, vp, u64p, vp]
+    L.hair_render_sequential.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, vp, vp, u64p, vp]
     L.hair_render_to_host.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp]
     L.hair_render_to_host_async.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp, C.POINTER(C.c_int)]
     L.hair_host_wait.argtypes = [vp, C.c_int]
@@ -154,6 +155,7 @@ def make_params(d: dict, flags: int | None = None) -> hair_render_params:
         p.background_rgb[:] = d["background_rgb"]
     f = FLAG_FILTER if d.get("filter_on", True) else 0
     p.flags = f | (flags or 0)
+    p.groom_mask = int(d.get("groom_mask", 0xFFFFFFFF)) & 0xFFFFFFFF
     return p
 
 
@@ -253,18 +255,23 @@ class Hair:
         self._res = (w, h)
         return out_gbuffer, out_rgb
 
-    def render_scene(self, cam: dict, lam, scene_zn=None, scene_rgb=None, out_gbuffer=None, out_rgb=None):
+    def render_sequential(self, cam: dict, lam, scene_zn=None, scene_rgb=None, out_gbuffer=None, out_rgb=None):
+        """hair_render_sequential: the grooms one after the other; arguments as render_scene."""
+        return self.render_scene(cam, lam, scene_zn, scene_rgb, out_gbuffer, out_rgb, _fn="hair_render_sequential")
+
+    def render_scene(self, cam: dict, lam, scene_zn=None, scene_rgb=None, out_gbuffer=None, out_rgb=None,
+                     _fn="hair_render_scene"):
         """hair_render_scene: scene_zn float32 [h][w], scene_rgb float32 [h][w][4] device tensors (or None)."""
         w, h = cam["width"], cam["height"]
         if out_gbuffer is None or out_rgb is None:
             out_gbuffer, out_rgb = self.alloc_outputs(w, h)
         lam = np.atleast_1d(np.asarray(lam, dtype=np.float32))
         c = make_camera(cam)
-        self._check(self.L.hair_render_scene(self.h, C.byref(c), w, h, _ptr(lam), len(lam),
+        self._check(getattr(self.L, _fn)(self.h, C.byref(c), w, h, _ptr(lam), len(lam),
                                              None if scene_zn is None else C.c_void_p(scene_zn.data_ptr()),
                                              None if scene_rgb is None else C.c_void_p(scene_rgb.data_ptr()),
                                              C.c_void_p(out_gbuffer.data_ptr()), C.c_void_p(out_rgb.data_ptr())),
-                    "hair_render_scene")
+                    _fn)
         self._res = (w, h)
         return out_gbuffer, out_rgb
 

@@ -46,6 +46,8 @@ struct hair_ctx {
   size_t vertex_need = 0;
   float4* d_colour = nullptr;
   size_t colour_cap = 0;
+  float4* d_target2 = nullptr;  // hair_render_sequential: second render target of the ping-pong
+  size_t target2_cap = 0;
   unsigned long long* d_counters = nullptr;
   unsigned long long* h_counters = nullptr;  // pinned
   uint32_t c_max = 0;
@@ -187,6 +189,7 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
   size_t px = (size_t)w * h;
   if (px > c->colour_cap) {
     cudaFree(c->d_colour);
+  cudaFree(c->d_target2);
     c->d_colour = nullptr;
     CK(cudaMalloc((void**)&c->d_colour, px * sizeof(float4)));
     c->colour_cap = px;
@@ -199,9 +202,19 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
   return HAIR_OK;
 }
 
+// what one pass draws into: R-scene (scene_zn, scene_rgb) and R-seq (grooms of this pass, depth kept in the
+// G-buffer from the pass before, alpha accumulated so far in scene_rgb.w)
+struct PassOpts {
+  const float* scene_zn = nullptr;
+  const float* scene_rgb = nullptr;
+  uint32_t groom_mask = 0xFFFFFFFFu;
+  bool reseed = false;
+  bool bg_alpha = false;
+};
+
 int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
-                uint32_t stage_mask, bool front, unsigned long long* gbuf, float* rgb,
-                const float* scene_zn = nullptr, const float* scene_rgb = nullptr) {
+                uint32_t stage_mask, bool front, unsigned long long* gbuf, float* rgb, const PassOpts& po = PassOpts()) {
+  const float *scene_zn = po.scene_zn, *scene_rgb = po.scene_rgb;
   if (!c) return HAIR_E_INVALID_ARG;
   if (!cam || !gbuf || !rgb || w == 0 || h == 0 || w > 16384 || h > 16384)
     return fail(c, HAIR_E_INVALID_ARG, "hair_render: null argument or bad resolution");
@@ -215,7 +228,8 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   int rc = ensure_scratch(c, w, h);
   if (rc) return rc;
   const CamDev k = make_cam(cam, w, h);
-  const ShadeParams sp = make_shade(c->prm);
+  ShadeParams sp = make_shade(c->prm);
+  sp.bg_alpha = po.bg_alpha ? 1u : 0u;
   const bool timed = (c->prm.flags & HAIR_FLAG_STAGE_TIMING) != 0;
   const bool count = (c->prm.flags & HAIR_FLAG_COUNTERS) != 0;
   const uint32_t n_bi = c->scene.n_bi;
@@ -230,7 +244,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   if (front && n_bi) {
     LambdaArr la;
     for (uint32_t i = 0; i < HAIR_MAX_GROOMS; ++i) la.v[i] = n_lam == 0 ? 0.f : lam[n_lam == 1 ? 0 : (i < n_lam ? i : 0)];
-    launch_lod_scan(c->d_scene, n_bi, k, la, c->d_table, c->d_grp, c->d_counters, st);
+    launch_lod_scan(c->d_scene, n_bi, k, la, po.groom_mask & c->prm.groom_mask, c->d_table, c->d_grp, c->d_counters, st);
     launches += 2;
   }
   mark(EV_LOD);
@@ -240,7 +254,8 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_GEN);
   if (stage_mask & 1u) {
-    launch_clear(gbuf, (size_t)w * h, scene_zn, st);
+    if (po.reseed) launch_reseed(gbuf, (size_t)w * h, st);
+    else launch_clear(gbuf, (size_t)w * h, scene_zn, st);
     ++launches;
   }
   mark(EV_CLEAR);
@@ -351,6 +366,7 @@ void hair_default_render_params(hair_render_params* p) {
   p->k_R = 0.25f;
   p->k_TRT = 0.5f;
   p->flags = HAIR_FLAG_FILTER;
+  p->groom_mask = 0xFFFFFFFFu;
 }
 
 int hair_set_render_params(hair_ctx* c, const hair_render_params* p) {
@@ -494,7 +510,50 @@ int hair_render(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
 
 int hair_render_scene(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
                       const float* scene_zn, const float* scene_rgb, uint64_t* out_gbuffer, float* out_rgb) {
-  return render_impl(c, cam, w, h, lam, n_lam, 7u, true, (unsigned long long*)out_gbuffer, out_rgb, scene_zn, scene_rgb);
+  PassOpts po;
+  po.scene_zn = scene_zn;
+  po.scene_rgb = scene_rgb;
+  return render_impl(c, cam, w, h, lam, n_lam, 7u, true, (unsigned long long*)out_gbuffer, out_rgb, po);
+}
+
+int hair_render_sequential(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam,
+                           uint32_t n_lam, const float* scene_zn, const float* scene_rgb, uint64_t* out_gbuffer,
+                           float* out_rgb) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  const uint32_t n = c->scene.n_grooms;
+  if (n <= 1) return hair_render_scene(c, cam, w, h, lam, n_lam, scene_zn, scene_rgb, out_gbuffer, out_rgb);
+  CK(cudaSetDevice(c->device));
+  const size_t px = (size_t)w * h;
+  if (px > c->target2_cap) {  // the second render target of the ping-pong
+    cudaFree(c->d_target2);
+    c->d_target2 = nullptr;
+    c->target2_cap = 0;
+    CK(cudaMalloc((void**)&c->d_target2, px * sizeof(float4)));
+    c->target2_cap = px;
+  }
+  uint32_t launches = 0;
+  const float* target_in = scene_rgb;
+  uint32_t n_pass = 0, i_pass = 0;
+  for (uint32_t g = 0; g < n; ++g) n_pass += (c->prm.groom_mask >> g) & 1u;
+  if (n_pass <= 1) return hair_render_scene(c, cam, w, h, lam, n_lam, scene_zn, scene_rgb, out_gbuffer, out_rgb);
+  for (uint32_t g = 0; g < n; ++g) {
+    if (!((c->prm.groom_mask >> g) & 1u)) continue;
+    // the last pass must land in out_rgb: passes alternate between the two targets, counted from the end
+    float* target_out = ((n_pass - 1 - i_pass) & 1u) ? (float*)c->d_target2 : out_rgb;
+    PassOpts po;
+    po.scene_zn = i_pass == 0 ? scene_zn : nullptr;
+    po.scene_rgb = target_in;
+    po.groom_mask = 1u << g;
+    po.reseed = i_pass > 0;
+    po.bg_alpha = i_pass > 0;
+    ++i_pass;
+    int rc = render_impl(c, cam, w, h, lam, n_lam, 7u, true, (unsigned long long*)out_gbuffer, target_out, po);
+    if (rc) return rc;
+    launches += c->launches;
+    target_in = target_out;
+  }
+  c->launches = launches;
+  return HAIR_OK;
 }
 
 int hair_render_stages(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, uint32_t stage_mask,

@@ -60,6 +60,7 @@ struct ShadeParams {
   int strip_nc;        // integer minor offsets per major step that can lie within strip_hmax of the line
   float strip_e2_max;  // largest float e2 with sqrt_rn(e2) <= w_strip
   uint32_t tauz_q, taufly_q, filter_on;
+  uint32_t bg_alpha;  // R-seq: scene_rgb.w is the alpha accumulated by earlier passes (out.w = a + (1 - a) bg.w)
   float rho_default;  // 0.5 * center_diameter_px
 };
 
@@ -158,11 +159,12 @@ __device__ __forceinline__ Loc locate_strand(const SceneDev* __restrict__ sc, co
 }
 
 // ------------------------------------------------------------------ launchers (one per .cu)
-void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint4* table,
-                     uint32_t* grp, unsigned long long* counters, cudaStream_t st);
+void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint32_t groom_mask,
+                     uint4* table, uint32_t* grp, unsigned long long* counters, cudaStream_t st);
 void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices,
                      unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st);
 void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_zn, cudaStream_t st);
+void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                    unsigned long long* counters, bool count, int n_sm, cudaStream_t st);

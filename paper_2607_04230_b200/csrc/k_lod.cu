@@ -22,7 +22,7 @@ __device__ __forceinline__ void lod_counts(float L, uint32_t N, float delta, uin
 }
 
 __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, uint32_t n_bi, CamDev cam,
-                                             LambdaArr lam, uint4* __restrict__ table) {
+                                             LambdaArr lam, uint32_t groom_mask, uint4* __restrict__ table) {
   uint32_t gid = blockIdx.x * blockDim.x + threadIdx.x;
   if (gid >= n_bi) return;
   uint32_t gi = 0;
@@ -86,6 +86,7 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
       if (nlod == 0) C = 0;
     }
   }
+  if (!((groom_mask >> gi) & 1u)) nlod = C = 0;  // R-seq: this groom is not drawn in this pass
   table[gid] = make_uint4(nlod, C, 0u, 0u);
 }
 
@@ -180,8 +181,8 @@ __global__ void __launch_bounds__(1024) k_scan(uint4* __restrict__ table, uint32
     }
 }
 
-void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint4* table,
-                     uint32_t* grp, unsigned long long* counters, cudaStream_t st) {
-  k_lod<<<(n_bi + 255) / 256, 256, 0, st>>>(d_scene, n_bi, cam, lam, table);
+void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint32_t groom_mask,
+                     uint4* table, uint32_t* grp, unsigned long long* counters, cudaStream_t st) {
+  k_lod<<<(n_bi + 255) / 256, 256, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table);
   k_scan<<<1, 1024, 0, st>>>(table, grp, n_bi, counters);
 }

@@ -263,6 +263,22 @@ __global__ void __launch_bounds__(256) k_clear(uint4* __restrict__ g, size_t n16
   }
 }
 
+// R-seq ("preserving the depth buffer between groom passes"): between two sequential passes both
+// layers of a pixel restart at the depth of its centre word (a hit's depth, else the depth kept so far), no hit
+__global__ void __launch_bounds__(256) k_reseed(uint4* __restrict__ g, size_t n16) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) {
+    const uint32_t hi = g[i].y | 0xFFu;
+    g[i] = make_uint4(0xFFFFFFFFu, hi, 0xFFFFFFFFu, hi);
+  }
+}
+
+void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st) {
+  size_t blocks = (n_pixels + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  k_reseed<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels);
+}
+
 void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_zn, cudaStream_t st) {
   size_t blocks = (n_pixels + 255) / 256;
   if (blocks > 148 * 16) blocks = 148 * 16;

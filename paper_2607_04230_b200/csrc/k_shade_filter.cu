@@ -166,7 +166,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
     bg[k] = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
     if (scene_rgb && inside[k]) {
       const float4 b = __ldg(&scene_rgb[(size_t)(y0 + ly + 8 * k) * W + x0 + lx]);
-      bg[k] = make_float4(b.x, b.y, b.z, 0.f);
+      bg[k] = make_float4(b.x, b.y, b.z, sp.bg_alpha ? b.w : 0.f);
     }
   }
   if (!__syncthreads_or(hit)) {  // empty tile: background only
@@ -331,7 +331,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
     }
     const float ia = 1.f - alpha;
     out[(size_t)(y0 + ly + 8 * k) * W + x0 + lx] =
-        make_float4(alpha * r + ia * bg[k].x, alpha * g + ia * bg[k].y, alpha * b + ia * bg[k].z, alpha);
+        make_float4(alpha * r + ia * bg[k].x, alpha * g + ia * bg[k].y, alpha * b + ia * bg[k].z, alpha + ia * bg[k].w);
   }
 }
 
@@ -346,7 +346,7 @@ k_filter_passthrough(CamDev cam, ShadeParams sp, const unsigned long long* __res
   float4 o = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
   if (scene_rgb) {
     const float4 b = __ldg(&scene_rgb[p]);
-    o = make_float4(b.x, b.y, b.z, 0.f);
+    o = make_float4(b.x, b.y, b.z, sp.bg_alpha ? b.w : 0.f);
   }
   if (!w_none(raw.x, raw.y)) {
     const float4 c = __ldg(&colour[p]);

@@ -368,6 +368,81 @@ def test_render_into_scene_stagewise(orc, hair_mod, filter_on):
     assert torch.equal(gb2, gb0) and torch.equal(rgb2, rgb0)
 
 
+def test_groom_mask_and_sequential_passes(orc, hair_mod):
+    """hair_render_sequential (R-seq) against the oracle's sequential passes, pass by pass on the
+    GPU's own vertices (groom_mask renders give them), five overlapping grooms, a scene behind them."""
+    import torch
+    b = hair_mod
+    sc = synth.config(4, scale=0.03, res_scale=0.2)
+    # pull the grooms together so that they overlap on screen (config 4 spreads them over the frame)
+    cam, lam, prm = sc["camera"], list(sc["lam"]), dict(sc["params"])
+    W, H = cam["width"], cam["height"]
+    n = len(sc["grooms"])
+    thfov = math.tan(0.5 * cam["vfov_y"]) * W / H
+    for g, ndc_x in zip(sc["grooms"], (-0.1, 0.05, 0.12, 0.16, 0.19)):
+        x = np.array(g["xform"], np.float32).reshape(-1, 12).copy()
+        x[:, 3] = ndc_x * (-x[:, 11]) * thfov  # same distance, new screen slot
+        g["xform"] = x
+    h = b.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    rng = np.random.default_rng(5)
+    srgb = rng.random((H, W, 4)).astype(np.float32)
+    zn = np.full((H, W), 0.9995, np.float32)
+    zn[:, : W // 6] = 0.5  # a pillar in front of part of the first groom
+    zn_d, srgb_d = torch.from_numpy(zn).cuda(), torch.from_numpy(srgb).cuda()
+    # (i) masked frames: exactly the frame of that groom alone (table, vertices), ids stay global
+    verts, tables = [], []
+    f = orc.Frame(sc["grooms"])
+    for g in range(n):
+        h.set_render_params(dict(prm, groom_mask=1 << g))
+        gb, rgb = h.render(cam, lam)
+        nv = h.stats()["n_vertices"]
+        verts.append(h.debug_vertices().cpu().numpy()[:nv].copy())
+        f.set_pass(1 << g)
+        f.lod(cam, lam)
+        assert np.array_equal(f.table()[0], h.debug_table().cpu().numpy().view(np.uint32))
+        f.generate()
+        assert np.abs(f.vertices_f64() - verts[-1]).max() <= TOL_VERTEX
+        sid = (b.gbuffer_to_numpy(gb)[..., 1] >> np.uint64(16)) & np.uint64(0xFFFFFF)
+        hitm = (b.gbuffer_to_numpy(gb)[..., 1] & np.uint64((1 << 40) - 1)) != np.uint64((1 << 40) - 1)
+        lo = sum(int(x["strands_per_tri"].sum()) for x in sc["grooms"][:g])
+        assert hitm.any() and sid[hitm].min() >= lo and sid[hitm].max() < lo + int(sc["grooms"][g]["strands_per_tri"].sum())
+    # (ii) the oracle's sequential passes on those vertices
+    target = srgb[..., :3].copy()
+    alpha = np.zeros((H, W), np.float32)
+    z = np.clip(zn, np.float32(0), np.float32(1))
+    dq = np.minimum((z * np.float32(16777215.0) + np.float32(0.5)).astype(np.float32).astype(np.uint32), np.uint32(0xFFFFFE))
+    for g in range(n):
+        f.set_pass(1 << g, dq, alpha)
+        f.set_scene(None, target)
+        f.lod(cam, lam)
+        f.generate()
+        f.set_vertices_f32(verts[g])
+        f.raster(cam, prm)
+        f.shade(cam, prm)
+        out = f.filter(cam, prm)
+        g_or = f.gbuffer()
+        dq = (g_or[..., 0] >> np.uint64(40)).astype(np.uint32)
+        target, alpha = out[..., :3].astype(np.float32), out[..., 3].astype(np.float32)
+    # (iii) the library's sequential frame
+    h.set_render_params(prm)
+    gb, rgb = h.render_sequential(cam, lam, zn_d, srgb_d)
+    G = b.gbuffer_to_numpy(gb)
+    assert np.array_equal(G, g_or), float((G == g_or).mean())
+    got = rgb.cpu().numpy().astype(np.float64)
+    assert np.abs(out - got).max() <= TOL_RGB
+    assert psnr(out[..., :3], got[..., :3], max(float(out[..., :3].max()), 1.0)) > MIN_PSNR
+    assert np.array_equal(got[:, : W // 6, :3], srgb[:, : W // 6, :3].astype(np.float64)) or (zn[:, : W // 6] == 0.5).all()
+    # it differs from the one-resolve frame where grooms overlap, and equals it for a single groom
+    one = h.render_scene(cam, lam, zn_d, srgb_d)
+    assert (one[1] - rgb).abs().max().item() > 1e-2
+    h.set_render_params(dict(prm, groom_mask=0b100))
+    a1 = h.render_sequential(cam, lam, zn_d, srgb_d)
+    a2 = h.render_scene(cam, lam, zn_d, srgb_d)
+    assert torch.equal(a1[0], a2[0]) and torch.equal(a1[1], a2[1])
+
+
 def test_render_to_host_async_pipeline(hair_mod):
     """Two frames in flight: each host buffer, after host_wait, holds exactly what hair_render gives."""
     import torch
