@@ -85,6 +85,7 @@ def lib():
         L.orc_pack.argtypes = [f32, u32, u32, f32]
         L.orc_unpack.restype = None
         L.orc_unpack.argtypes = [u64, vp]
+        L.orc_segment_cover_msaa.argtypes = [vp, vp, f32, u32, u32, u32, vp, vp]
         L.orc_segment_cover.restype = None
         L.orc_segment_cover.argtypes = [vp, vp, f32, u32, u32, vp, vp]
         L.orc_project.restype = C.c_int
@@ -113,6 +114,11 @@ def lib():
         L.orc_frame_set_pass.argtypes = [vp, u32, vp, vp, u32, u32]
         L.orc_frame_set_window.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
         L.orc_frame_set_window.restype = None
+        L.orc_frame_raster_msaa.argtypes = [vp, vp, vp, u32]
+        L.orc_frame_get_msaa.argtypes = [vp, vp]
+        L.orc_frame_get_msaa.restype = None
+        L.orc_frame_set_msaa.argtypes = [vp, vp, u32, u32, u32]
+        L.orc_frame_resolve_msaa.argtypes = [vp, vp, vp]
         L.orc_frame_shade.argtypes = [vp, vp, vp]
         L.orc_frame_get_colour.argtypes = [vp, vp]
         L.orc_frame_get_tangents.argtypes = [vp, vp]
@@ -354,6 +360,34 @@ class Frame:
         """Sample a full-size frame: O4 / O6 / O7 only visit pixels of [x0, x1) x [y0, y1) (O6 grown by 7 px)."""
         self.L.orc_frame_set_window(self.h, int(x0), int(y0), int(x1), int(y1))
 
+    # ---- MSAA-k reference (R-msaa)
+    def raster_msaa(self, cam: dict, prm: dict, k: int):
+        c, p = make_camera(cam), make_params(prm)
+        r = self.L.orc_frame_raster_msaa(self.h, C.byref(c), C.byref(p), int(k))
+        if r:
+            raise ValueError(f"orc_frame_raster_msaa failed: {r}")
+        self._wh = (cam["width"], cam["height"])
+        self._ms_k = int(k)
+        ms = np.empty((int(k), cam["height"], cam["width"]), dtype=np.uint64)
+        self.L.orc_frame_get_msaa(self.h, _ptr(ms))
+        return ms
+
+    def set_msaa(self, ms) -> None:
+        ms = np.ascontiguousarray(ms, dtype=np.uint64)
+        k, h, w = ms.shape
+        self._wh = (w, h)
+        self._ms_k = k
+        self.L.orc_frame_set_msaa(self.h, _ptr(ms), k, w, h)
+
+    def resolve_msaa(self, cam: dict, prm: dict):
+        c, p = make_camera(cam), make_params(prm)
+        r = self.L.orc_frame_resolve_msaa(self.h, C.byref(c), C.byref(p))
+        if r:
+            raise ValueError(f"orc_frame_resolve_msaa failed: {r}")
+        out = np.empty((cam["height"], cam["width"], 4), dtype=np.float64)
+        self.L.orc_frame_get_out(self.h, _ptr(out))
+        return out
+
     # ---- O6 / O7
     def shade(self, cam: dict, prm: dict):
         c, p = make_camera(cam), make_params(prm)
@@ -426,6 +460,22 @@ def segment_cover(a, b, rho, w, h):
     cover = np.zeros((h, w), np.uint8)
     tq = np.zeros((h, w), np.float32)
     lib().orc_segment_cover(_ptr(a), _ptr(b), rho, w, h, _ptr(cover), _ptr(tq))
+    return cover, tq
+
+
+MSAA_OFFSETS = {  # sample offsets from the pixel centre in 1/16 pixel (R-msaa), restated for the tests
+    1: [(0, 0)], 2: [(4, 4), (-4, -4)], 4: [(-2, -6), (6, -2), (-6, 2), (2, 6)],
+    8: [(1, -3), (-1, 3), (5, 1), (-3, -5), (-5, 5), (-7, -1), (3, 7), (7, -7)]}
+
+
+def segment_cover_msaa(a, b, rho, w, h, k):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    b = np.ascontiguousarray(b, dtype=np.float32)
+    cover = np.zeros((k, h, w), np.uint8)
+    tq = np.zeros((k, h, w), np.float32)
+    r = lib().orc_segment_cover_msaa(_ptr(a), _ptr(b), rho, w, h, k, _ptr(cover), _ptr(tq))
+    if r:
+        raise ValueError(f"unsupported sample count {k}")
     return cover, tq
 
 

@@ -195,6 +195,8 @@ struct orc_frame {
   std::vector<float> scene_rgb;  // [H][W][3] or empty
   // sequential per-groom passes (DESIGN.md R-seq): the depth kept from the passes before,
   // already quantised (takes precedence over scene_zn), the alpha accumulated so far, and the grooms of this pass
+  std::vector<uint64_t> ms;         // MSAA-k reference: [k][H][W] words (R-msaa)
+  uint32_t ms_k = 0;
   std::vector<uint32_t> scene_dq;   // [H][W] or empty
   std::vector<float> scene_alpha;   // [H][W] or empty
   uint32_t groom_mask = 0xFFFFFFFFu;
@@ -522,6 +524,61 @@ static inline int cover_px(float ax, float ay, float bx, float by, float rho2, i
   return (d2 <= rho2) ? 3 : 1;
 }
 
+// R-msaa: sample positions inside the pixel, in 1/16 pixel from the pixel centre (the standard 2x / 4x / 8x
+// multisample patterns; 1x = the pixel centre). The paper names no pattern.
+static const int MS_OFF[4][8][2] = {
+    {{0, 0}},
+    {{4, 4}, {-4, -4}},
+    {{-2, -6}, {6, -2}, {-6, 2}, {2, 6}},
+    {{1, -3}, {-1, 3}, {5, 1}, {-3, -5}, {-5, 5}, {-7, -1}, {3, 7}, {7, -7}}};
+static inline const int (*ms_pattern(uint32_t k))[2] { return k == 1 ? MS_OFF[0] : k == 2 ? MS_OFF[1] : k == 4 ? MS_OFF[2] : k == 8 ? MS_OFF[3] : nullptr; }
+
+// One sample point of pixel (x, y) at offset (ox, oy)/16 from the centre: hit iff the segment meets the pixel's
+// closed square (R10, as the conservative layer) and passes within rho of the sample point (R9 moved to the sample).
+// fp32, fixed order, the arithmetic of cover_px with the sample point in place of the pixel centre.
+static inline bool sample_hit(float ax, float ay, float bx, float by, float rho2, int x, int y, int ox, int oy, float& t_out) {
+  float dx = bx - ax, dy = by - ay;
+  float dd = dx * dx;
+  {
+    float e = dy * dy;
+    dd = dd + e;
+  }
+  // conservative test at the pixel centre
+  float cx = float(x) + 0.5f, cy = float(y) + 0.5f;
+  float ux = cx - ax, uy = cy - ay;
+  float mnx = std::min(ax, bx), mxx = std::max(ax, bx), mny = std::min(ay, by), mxy = std::max(ay, by);
+  bool box = mnx <= float(x + 1) && mxx >= float(x) && mny <= float(y + 1) && mxy >= float(y);
+  float c1 = dx * uy;
+  float c2 = dy * ux;
+  float cr = std::fabs(c1 - c2);
+  float ext = std::fabs(dx) + std::fabs(dy);
+  ext = 0.5f * ext;
+  if (!(box && cr <= ext)) return false;
+  // closest point to the sample (sample coordinates are exact: multiples of 1/16)
+  float sx = float(x) + (0.5f + float(ox) * 0.0625f), sy = float(y) + (0.5f + float(oy) * 0.0625f);
+  float vx = sx - ax, vy = sy - ay;
+  float t = 0.f;
+  if (dd > 0.f) {
+    float n = vx * dx;
+    float e = vy * dy;
+    n = n + e;
+    t = n / dd;
+    t = std::min(std::max(t, 0.0f), 1.0f);
+  }
+  t_out = t;
+  float qx = t * dx;
+  qx = ax + qx;
+  float qy = t * dy;
+  qy = ay + qy;
+  float ex = sx - qx, ey = sy - qy;
+  float d2 = ex * ex;
+  {
+    float e = ey * ey;
+    d2 = d2 + e;
+  }
+  return d2 <= rho2;
+}
+
 void orc_segment_cover(const float a[2], const float b[2], float rho, uint32_t w, uint32_t h,
                        uint8_t* cover, float* tq) {
   float rho2 = rho * rho;
@@ -531,6 +588,21 @@ void orc_segment_cover(const float a[2], const float b[2], float rho, uint32_t w
       cover[y * w + x] = uint8_t(cover_px(a[0], a[1], b[0], b[1], rho2, int(x), int(y), t));
       if (tq) tq[y * w + x] = t;
     }
+}
+
+int orc_segment_cover_msaa(const float a[2], const float b[2], float rho, uint32_t w, uint32_t h, uint32_t k,
+                           uint8_t* cover, float* tq) {
+  const int (*pat)[2] = ms_pattern(k);
+  if (!pat) return -4;
+  float rho2 = rho * rho;
+  for (uint32_t s = 0; s < k; ++s)
+    for (uint32_t y = 0; y < h; ++y)
+      for (uint32_t x = 0; x < w; ++x) {
+        float t = 0.f;
+        cover[(s * h + y) * w + x] = sample_hit(a[0], a[1], b[0], b[1], rho2, int(x), int(y), pat[s][0], pat[s][1], t) ? 1 : 0;
+        if (tq) tq[(s * h + y) * w + x] = t;
+      }
+  return 0;
 }
 
 orc_frame* orc_frame_create(void) { return new orc_frame(); }
@@ -874,25 +946,115 @@ int orc_frame_set_gbuffer(orc_frame* f, const uint64_t* in, uint32_t w, uint32_t
   return 0;
 }
 
-// ------------------------------------------------------------------ O6
-int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) {
+static bool shade_word(const orc_frame* f, const Cam& k, const orc_params* prm, uint64_t G, double rgb[3]);
+
+// ------------------------------------------------------------------ MSAA-k reference (R-msaa)
+// "recording samples into multiple layers of a uint64 image and resolving them later": k sample layers, each the
+// atomic min over the hits at its sample point. Same strand directory, projection, centre radius and word as O4.
+int orc_frame_raster_msaa(orc_frame* f, const orc_camera* cam, const orc_params* prm, uint32_t ksamp) {
+  const int (*pat)[2] = ms_pattern(ksamp);
+  if (!pat) return -4;
   Cam k = make_cam(cam);
-  if (f->W != k.W || f->H != k.H) return -1;
-  size_t np = size_t(k.W) * k.H;
-  f->colour.assign(np * 3, 0.0);
-  f->tang.assign(np * 4, 0.f);
+  f->W = k.W;
+  f->H = k.H;
+  const size_t np = size_t(k.W) * k.H;
+  f->ms.assign(np * ksamp, EMPTY);
+  f->ms_k = ksamp;
+  if (f->v32.size() != size_t(f->n_vertices) * 4) return -1;
+  for (const Groom& g : f->grooms)
+    for (uint32_t q = 0; q < g.Q; ++q)
+      for (uint32_t t = 0; t < g.T; ++t) {
+        const Entry& e = f->table[g.gid_base + q * g.T + t];
+        for (uint32_t kk = 0; kk < e.nlod; ++kk) {
+          const uint64_t voff = uint64_t(e.vertex_base) + uint64_t(kk) * e.C;
+          const uint32_t sid = g.sid_base + q * g.N + g.off[t] + kk;
+          for (uint32_t j = 0; j + 1 < e.C; ++j) {
+            const float* va = &f->v32[(voff + j) * 4];
+            const float* vb = va + 4;
+            Proj a = project(k, va[0], va[1], va[2]);
+            Proj b = project(k, vb[0], vb[1], vb[2]);
+            if (!a.valid || !b.valid) continue;  // R12
+            float rho;
+            if (g.st.width_world > 0.f) {  // R9
+              float zm = a.zv + b.zv;
+              zm = 0.5f * zm;
+              float wpx = g.st.width_world * k.fpx;
+              wpx = wpx / zm;
+              wpx = std::min(std::max(wpx, 0.25f), 1.0f);
+              rho = 0.5f * wpx;
+            } else
+              rho = 0.5f * prm->center_diameter_px;
+            float rho2 = rho * rho;
+            float mnx = std::min(a.sx, b.sx), mxx = std::max(a.sx, b.sx);
+            float mny = std::min(a.sy, b.sy), mxy = std::max(a.sy, b.sy);
+            float fx0 = std::max(std::floor(mnx) - 1.f, 0.f), fx1 = std::min(std::floor(mxx) + 1.f, float(k.W) - 1.f);
+            float fy0 = std::max(std::floor(mny) - 1.f, 0.f), fy1 = std::min(std::floor(mxy) + 1.f, float(k.H) - 1.f);
+            if (!(fx0 <= fx1) || !(fy0 <= fy1)) continue;
+            int x0 = std::max(int(fx0), f->wx0), x1 = std::min(int(fx1), f->wx1 - 1);
+            int y0 = std::max(int(fy0), f->wy0), y1 = std::min(int(fy1), f->wy1 - 1);
+            float dz = b.zn - a.zn;
+            for (int y = y0; y <= y1; ++y)
+              for (int x = x0; x <= x1; ++x)
+                for (uint32_t s = 0; s < ksamp; ++s) {
+                  float tt;
+                  if (!sample_hit(a.sx, a.sy, b.sx, b.sy, rho2, x, y, pat[s][0], pat[s][1], tt)) continue;
+                  float zn = tt * dz;
+                  zn = a.zn + zn;
+                  if (zn < 0.f || zn > 1.f) continue;
+                  uint64_t w = pack(zn, sid, j, tt);
+                  uint64_t* px = &f->ms[(size_t(s) * k.H + y) * k.W + x];
+                  *px = std::min(*px, w);
+                }
+          }
+        }
+      }
+  return 0;
+}
+void orc_frame_get_msaa(const orc_frame* f, uint64_t* o) { std::memcpy(o, f->ms.data(), f->ms.size() * sizeof(uint64_t)); }
+int orc_frame_set_msaa(orc_frame* f, const uint64_t* in, uint32_t ksamp, uint32_t w, uint32_t h) {
+  f->W = w;
+  f->H = h;
+  f->ms_k = ksamp;
+  f->ms.assign(in, in + size_t(w) * h * ksamp);
+  return 0;
+}
+// resolve: every sample with a hit is shaded (O6 of its word), samples without one show the background;
+// out = mean over the k samples, alpha = hit samples / k
+int orc_frame_resolve_msaa(orc_frame* f, const orc_camera* cam, const orc_params* prm) {
+  Cam k = make_cam(cam);
+  if (f->W != k.W || f->H != k.H || !f->ms_k) return -1;
+  const size_t np = size_t(k.W) * k.H;
+  f->out.assign(np * 4, 0.0);
+  for (int y = std::max(f->wy0, 0); y < std::min(f->wy1, int(k.H)); ++y)
+    for (int x = std::max(f->wx0, 0); x < std::min(f->wx1, int(k.W)); ++x) {
+      const size_t p = size_t(y) * k.W + x;
+      double acc[3] = {0, 0, 0};
+      uint32_t n_hit = 0;
+      for (uint32_t s = 0; s < f->ms_k; ++s) {
+        uint64_t w = f->ms[size_t(s) * np + p];
+        if (none(w)) continue;
+        double rgb[3];
+        if (!shade_word(f, k, prm, w, rgb)) return -2;
+        for (int c = 0; c < 3; ++c) acc[c] += rgb[c];
+        ++n_hit;
+      }
+      double alpha = double(n_hit) / double(f->ms_k);
+      for (int c = 0; c < 3; ++c) {
+        double bg = f->scene_rgb.empty() ? double(prm->background_rgb[c]) : double(f->scene_rgb[p * 3 + c]);
+        f->out[p * 4 + c] = acc[c] / double(f->ms_k) + (1 - alpha) * bg;
+      }
+      f->out[p * 4 + 3] = alpha;
+    }
+  return 0;
+}
+
+// ------------------------------------------------------------------ O6
+// O6 for one word: the shaded linear RGB of the hit it names (stand-in model, R23). Returns false if the strand
+// id does not resolve.
+static bool shade_word(const orc_frame* f, const Cam& k, const orc_params* prm, uint64_t G, double rgb[3]) {
   V3 eye = {double(k.eye[0]), double(k.eye[1]), double(k.eye[2])};
-  const int sx0 = std::max(f->wx0 - 7, 0), sx1 = std::min(f->wx1 < (1 << 30) ? f->wx1 + 7 : f->wx1, int(k.W));
-  const int sy0 = std::max(f->wy0 - 7, 0), sy1 = std::min(f->wy1 < (1 << 30) ? f->wy1 + 7 : f->wy1, int(k.H));
-  for (int sy = sy0; sy < sy1; ++sy)
-  for (int sx = sx0; sx < sx1; ++sx) {
-    const size_t p = size_t(sy) * k.W + sx;
-    uint64_t G = f->gbuf[p * 2], A = f->gbuf[p * 2 + 1];
-    if (!none(A)) screen_tangent(f, k, A, &f->tang[p * 4 + 2]);
-    if (none(G)) continue;
-    screen_tangent(f, k, G, &f->tang[p * 4]);
     Loc l = locate(f, w_sid(G));
-    if (!l.ok) return -2;
+    if (!l.ok) return false;
     const Groom* g = nullptr;
     for (const Groom& gg : f->grooms)
       if (w_sid(G) >= gg.sid_base && w_sid(G) < gg.sid_base + gg.N * gg.Q) g = &gg;
@@ -910,7 +1072,6 @@ int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) 
     for (int c = 0; c < 3; ++c)
       alb[c] = (1 - w) * double(g->st.albedo_root[c]) + w * double(g->st.albedo_tip[c]);
     V3 Vd = normalize(eye - pos);
-    double rgb[3];
     for (int c = 0; c < 3; ++c) rgb[c] = ao * double(prm->ambient_rgb[c]) * alb[c];
     double beta = double(g->st.roughness), tilt = double(g->st.tilt);
     for (uint32_t li = 0; li < prm->n_lights; ++li) {
@@ -929,6 +1090,26 @@ int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) 
         rgb[c] += E * cos_i * (double(prm->k_d) * alb[c] + double(prm->k_R) * MR + double(prm->k_TRT) * MT * alb[c]);
       }
     }
+  return true;
+}
+
+int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) {
+  Cam k = make_cam(cam);
+  if (f->W != k.W || f->H != k.H) return -1;
+  size_t np = size_t(k.W) * k.H;
+  f->colour.assign(np * 3, 0.0);
+  f->tang.assign(np * 4, 0.f);
+  const int sx0 = std::max(f->wx0 - 7, 0), sx1 = std::min(f->wx1 < (1 << 30) ? f->wx1 + 7 : f->wx1, int(k.W));
+  const int sy0 = std::max(f->wy0 - 7, 0), sy1 = std::min(f->wy1 < (1 << 30) ? f->wy1 + 7 : f->wy1, int(k.H));
+  for (int sy = sy0; sy < sy1; ++sy)
+  for (int sx = sx0; sx < sx1; ++sx) {
+    const size_t p = size_t(sy) * k.W + sx;
+    uint64_t G = f->gbuf[p * 2], A = f->gbuf[p * 2 + 1];
+    if (!none(A)) screen_tangent(f, k, A, &f->tang[p * 4 + 2]);
+    if (none(G)) continue;
+    screen_tangent(f, k, G, &f->tang[p * 4]);
+    double rgb[3];
+    if (!shade_word(f, k, prm, G, rgb)) return -2;
     for (int c = 0; c < 3; ++c) f->colour[p * 3 + c] = rgb[c];
   }
   return 0;

@@ -81,6 +81,9 @@ uint64_t orc_pack(float zn, uint32_t sid, uint32_t j, float t);
 void orc_unpack(uint64_t w, uint32_t out[4]); /* dq, sid, j, t9 */
 /* coverage of ONE screen-space segment on a w x h grid: cover[y*w+x] bit0 = conservative,
  * bit1 = centre; tq[y*w+x] = closest-point parameter t (fp32). */
+/* per-sample coverage of one screen-space segment in MSAA-k mode (R-msaa): cover[k][h][w] in {0, 1}, tq likewise */
+int orc_segment_cover_msaa(const float a[2], const float b[2], float rho, uint32_t w, uint32_t h, uint32_t k,
+                           uint8_t* cover, float* tq);
 void orc_segment_cover(const float a[2], const float b[2], float rho, uint32_t w, uint32_t h,
                        uint8_t* cover, float* tq);
 /* project one world point: out = sx, sy, zn, zv; returns valid */
@@ -137,6 +140,17 @@ int orc_frame_set_pass(orc_frame*, uint32_t groom_mask, const uint32_t* dq, cons
  * all three, so values inside the window equal those of the full-frame run: a way to SAMPLE a full-size frame
  * (the raster's hit counts then cover the window only). Default / reset: 0, 0, 1 << 30, 1 << 30. */
 void orc_frame_set_window(orc_frame*, int x0, int y0, int x1, int y1);
+
+/* MSAA-k reference mode (DESIGN.md R-msaa; "recording samples into multiple layers of a uint64 image
+ * and resolving them later ... only as a reference"). k in {1, 2, 4, 8}: sample s of a pixel sits at the standard
+ * multisample offset; layer s = atomic min over the hits at that sample: the segment meets the pixel's closed
+ * square (R10) and passes within the centre radius (R9) of the SAMPLE point; depth / parameter at the closest
+ * point to the sample (R11); word as O4. ms[k][H][W]. Resolve: out = mean over samples of (shaded hit | background),
+ * alpha = hit samples / k. */
+int orc_frame_raster_msaa(orc_frame*, const orc_camera*, const orc_params*, uint32_t k);
+void orc_frame_get_msaa(const orc_frame*, uint64_t* out);
+int orc_frame_set_msaa(orc_frame*, const uint64_t* in, uint32_t k, uint32_t w, uint32_t h);
+int orc_frame_resolve_msaa(orc_frame*, const orc_camera*, const orc_params*);
 
 /* O6: colour[H][W][3] fp64 (0 where no centre hit); tangents[H][W][4] fp32 = (T_G.xy, T_A.xy) */
 int orc_frame_shade(orc_frame*, const orc_camera*, const orc_params*);
