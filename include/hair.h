@@ -135,6 +135,15 @@ int hair_render_scene(hair_ctx*, const hair_camera*, uint32_t width, uint32_t he
                       uint32_t n_lambda, const float* scene_zn, const float* scene_rgb, uint64_t* out_gbuffer,
                       float* out_rgb);
 
+/* MSAA-k REFERENCE mode (DESIGN.md R-msaa; "recording samples into multiple layers of a uint64 image
+ * and resolving them later ... only as a reference"): k in {1, 2, 4, 8} sample points per pixel (the standard
+ * multisample patterns), one atomic-min layer per sample; a sample is hit when the segment meets the pixel's closed
+ * square and passes within the centre radius of the sample point. No filter: out_rgb = mean over the samples of
+ * (shaded hit | background), .w = hit samples / k.
+ *  out_samples DEVICE, [k][height][width] uint64, 16-byte aligned, cleared by the call (empty = all ones). */
+int hair_render_msaa(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height, const float* lod_lambda,
+                     uint32_t n_lambda, uint32_t k, uint64_t* out_samples, float* out_rgb);
+
 /* The paper's multi-groom path (DESIGN.md R-seq): the grooms one after the other in upload
  * order, each through the whole pipeline on its own (LOD .. filter), its filtered result blended over the target
  * so far, the depth of its centre layer kept so that later grooms are rejected behind it. hair_render, by

@@ -20,7 +20,7 @@ EMPTY = 0xFFFFFFFFFFFFFFFF
 
 EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_render_params",
            "hair_set_render_params", "hair_mesh_upload", "hair_mesh_update", "hair_mesh_clear",
-           "hair_render", "hair_render_scene", "hair_render_sequential", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
+           "hair_render", "hair_render_scene", "hair_render_sequential", "hair_render_msaa", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
            "hair_debug_buffers", "hair_debug_set_vertices", "hair_atomic_microbench", "hair_abi_sizes"]
 
 
@@ -104,6 +104,7 @@ def load():
     L.hair_render.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp]
     L.hair_render_scene.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, vp, vp, u64p, vp]
     L.hair_render_sequential.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, vp, vp, u64p, vp]
+    L.hair_render_msaa.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u32, u64p, vp]
     L.hair_render_to_host.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp]
     L.hair_render_to_host_async.argtypes = [vp, C.POINTER(hair_camera), u32, u32, vp, u32, u64p, vp, C.POINTER(C.c_int)]
     L.hair_host_wait.argtypes = [vp, C.c_int]
@@ -254,6 +255,19 @@ class Hair:
                                        C.c_void_p(out_gbuffer.data_ptr()), C.c_void_p(out_rgb.data_ptr())), "hair_render")
         self._res = (w, h)
         return out_gbuffer, out_rgb
+
+    def render_msaa(self, cam: dict, lam, k: int):
+        """hair_render_msaa: returns (samples int64 [k][h][w] device tensor, out_rgb float32 [h][w][4])."""
+        import torch
+        w, h = cam["width"], cam["height"]
+        samples = torch.empty((int(k), h, w), dtype=torch.int64, device=f"cuda:{self.device}")
+        out_rgb = torch.empty((h, w, 4), dtype=torch.float32, device=f"cuda:{self.device}")
+        lam = np.atleast_1d(np.asarray(lam, dtype=np.float32))
+        c = make_camera(cam)
+        self._check(self.L.hair_render_msaa(self.h, C.byref(c), w, h, _ptr(lam), len(lam), int(k),
+                                            C.c_void_p(samples.data_ptr()), C.c_void_p(out_rgb.data_ptr())), "hair_render_msaa")
+        self._res = (w, h)
+        return samples, out_rgb
 
     def render_sequential(self, cam: dict, lam, scene_zn=None, scene_rgb=None, out_gbuffer=None, out_rgb=None):
         """hair_render_sequential: the grooms one after the other; arguments as render_scene."""

@@ -210,6 +210,7 @@ struct PassOpts {
   uint32_t groom_mask = 0xFFFFFFFFu;
   bool reseed = false;
   bool bg_alpha = false;
+  uint32_t ms_k = 0;  // R-msaa: gbuf is [ms_k][h][w] sample layers, resolve instead of shade + filter
 };
 
 int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
@@ -254,7 +255,8 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_GEN);
   if (stage_mask & 1u) {
-    if (po.reseed) launch_reseed(gbuf, (size_t)w * h, st);
+    if (po.ms_k) CK(cudaMemsetAsync(gbuf, 0xFF, (size_t)w * h * po.ms_k * sizeof(unsigned long long), st));
+    else if (po.reseed) launch_reseed(gbuf, (size_t)w * h, st);
     else launch_clear(gbuf, (size_t)w * h, scene_zn, st);
     ++launches;
   }
@@ -262,16 +264,21 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   if ((stage_mask & 1u) && n_bi) {
     if (!front) CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER, 0, sizeof(unsigned long long), st));
     launch_raster(c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters,
-                  count, c->n_sm, st);
+                  count && !po.ms_k, po.ms_k, c->n_sm, st);
     ++launches;
   }
   mark(EV_RASTER);
-  if (stage_mask & 2u) {
+  if (po.ms_k) {
+    launch_resolve_msaa(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, po.ms_k, (const float4*)scene_rgb,
+                        (float4*)rgb, st);
+    ++launches;
+  }
+  if ((stage_mask & 2u) && !po.ms_k) {
     launch_shade(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour, st);
     ++launches;
   }
   mark(EV_SHADE);
-  if (stage_mask & 4u) {
+  if ((stage_mask & 4u) && !po.ms_k) {
     launches += launch_filter(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour,
                               (const float4*)scene_rgb, (float4*)rgb, c->d_counters, count, st);
   }
@@ -514,6 +521,15 @@ int hair_render_scene(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t 
   po.scene_zn = scene_zn;
   po.scene_rgb = scene_rgb;
   return render_impl(c, cam, w, h, lam, n_lam, 7u, true, (unsigned long long*)out_gbuffer, out_rgb, po);
+}
+
+int hair_render_msaa(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
+                     uint32_t k, uint64_t* out_samples, float* out_rgb) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  if (k != 1 && k != 2 && k != 4 && k != 8) return fail(c, HAIR_E_INVALID_ARG, "hair_render_msaa: k must be 1, 2, 4 or 8");
+  PassOpts po;
+  po.ms_k = k;
+  return render_impl(c, cam, w, h, lam, n_lam, 7u, true, (unsigned long long*)out_samples, out_rgb, po);
 }
 
 int hair_render_sequential(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam,

@@ -167,7 +167,10 @@ void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_
 void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
-                   unsigned long long* counters, bool count, int n_sm, cudaStream_t st);
+                   unsigned long long* counters, bool count, uint32_t ms_k, int n_sm, cudaStream_t st);
+void launch_resolve_msaa(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+                         ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
+                         float4* out, cudaStream_t st);
 void launch_shade(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
                   ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st);
 int launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,

@@ -40,11 +40,21 @@
 // group counts, `grp`); the warp finds the bundle of its group with a 32-ary search (one ballot per
 // level). Bundles differ 50x in work (strand count after LOD x pixel length), so bundle-sized units
 // left a long tail.
-template <bool COUNT>
+// MSAA-k reference mode (MS = true; DESIGN.md R-msaa, "recording samples into multiple layers of a
+// uint64 image"): same tasks, but a pixel that passes the conservative predicate is tested at its ms_k sample
+// points (closest point to the SAMPLE within the centre radius) and `gbuf` is [ms_k][H][W] words, one layer per
+// sample. A reference: plain atomicMin per sample hit, no read-before-atomic.
+__constant__ int c_ms_off[4][8][2] = {  // sample offsets from the pixel centre in 1/16 pixel: 1x, 2x, 4x, 8x
+    {{0, 0}},
+    {{4, 4}, {-4, -4}},
+    {{-2, -6}, {6, -2}, {-6, 2}, {2, 6}},
+    {{1, -3}, {-1, 3}, {5, 1}, {-3, -5}, {-5, 5}, {-7, -1}, {3, 7}, {7, -7}}};
+
+template <bool COUNT, bool MS>
 __global__ void __launch_bounds__(RAS_WARPS * 32, RAS_MIN_BLOCKS)
 k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
          const uint32_t* __restrict__ grp, const float4* __restrict__ vertices, CamDev cam, float rho_default,
-         unsigned long long* __restrict__ gbuf, unsigned long long* __restrict__ counters) {
+         unsigned long long* __restrict__ gbuf, unsigned long long* __restrict__ counters, uint32_t ms_k) {
   __shared__ __align__(16) float s_rec[RAS_WARPS][32][REC_STRIDE];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float(*rec)[REC_STRIDE] = s_rec[warp];
@@ -190,7 +200,30 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
             const float uN = xsub((float)r + 0.5f, aN);
             const float cr = fabsf(xsub(xmul(dM, uN), xmul(dN, uM)));
             ok[i] = r <= rhi && cr <= ext;
-            if (ok[i]) cur[i] = GB_LOAD(reinterpret_cast<const ulonglong2*>(pcol + (size_t)r * pstep));
+            if (!MS && ok[i]) cur[i] = GB_LOAD(reinterpret_cast<const ulonglong2*>(pcol + (size_t)r * pstep));
+          }
+          if (MS) {  // reference mode: every sample point of the pixels that passed the conservative predicate
+            const int pat = ms_k == 8 ? 3 : ms_k == 4 ? 2 : ms_k == 2 ? 1 : 0;
+#pragma unroll
+            for (int i = 0; i < ROW_BATCH; ++i) {
+              if (!ok[i]) continue;
+              const int r = rb + i;
+              const size_t pix = ymajor ? (size_t)c * W + r : (size_t)r * W + c;
+              for (uint32_t smp = 0; smp < ms_k; ++smp) {
+                const int ox = c_ms_off[pat][smp][0], oy = c_ms_off[pat][smp][1];
+                const float sM = fc + (0.5f + (float)(ymajor ? oy : ox) * 0.0625f);
+                const float sN = (float)r + (0.5f + (float)(ymajor ? ox : oy) * 0.0625f);
+                const float vM = xsub(sM, aM), vN = xsub(sN, aN);
+                float tt = 0.f;
+                if (dd > 0.f) tt = fminf(fmaxf(xdiv(xadd(xmul(vM, dM), xmul(vN, dN)), dd), 0.f), 1.f);
+                const float zn = xadd(az, xmul(tt, dz));
+                if (zn < 0.f || zn > 1.f) continue;
+                const float eM = xsub(sM, xadd(aM, xmul(tt, dM))), eN = xsub(sN, xadd(aN, xmul(tt, dN)));
+                if (xadd(xmul(eM, eM), xmul(eN, eN)) <= rec[s][17])
+                  atomicMin(gbuf + (size_t)smp * W * H + pix, pack_word(zn, (key >> 7) & 0xFFFFFFu, key & 0x7Fu, tt));
+              }
+            }
+            continue;
           }
           // pass 2: closest point, depth, centre predicate, word (R10/R11, fixed-order fp32; x/y-symmetric)
 #pragma unroll
@@ -285,20 +318,28 @@ void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_
   k_clear<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels, scene_zn);
 }
 
+template <bool COUNT, bool MS>
+static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
+                            const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
+                            unsigned long long* counters, uint32_t ms_k, int n_sm, cudaStream_t st) {
+  // persistent grid: every CTA slot of the device, the queue feeds them
+  static int per_sm = 0;
+  if (!per_sm) {
+    int b = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<COUNT, MS>, RAS_WARPS * 32, 0);
+    per_sm = b > 0 ? b : 1;
+  }
+  k_raster<COUNT, MS><<<(uint32_t)(n_sm * per_sm), RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, grp, vertices, cam,
+                                                                             rho_default, gbuf, counters, ms_k);
+}
+
+// ms_k = 0: the two-layer G-buffer; ms_k in {1, 2, 4, 8}: gbuf = [ms_k][H][W] sample layers (reference mode)
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
-                   unsigned long long* counters, bool count, int n_sm, cudaStream_t st) {
-  // persistent grid: every CTA slot of the device, the queue feeds them
-  static int per_sm[2] = {0, 0};
-  if (!per_sm[count]) {
-    int b = 0;
-    if (count) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<true>, RAS_WARPS * 32, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<false>, RAS_WARPS * 32, 0);
-    per_sm[count] = b > 0 ? b : 1;
-  }
-  const uint32_t grid = (uint32_t)(n_sm * per_sm[count]);
-  if (count) k_raster<true><<<grid, RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters);
-  else k_raster<false><<<grid, RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters);
+                   unsigned long long* counters, bool count, uint32_t ms_k, int n_sm, cudaStream_t st) {
+  if (ms_k) launch_raster_t<false, true>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, ms_k, n_sm, st);
+  else if (count) launch_raster_t<true, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
+  else launch_raster_t<false, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
 }
 
 // ------------------------------------------------------------------ L2-atomic roofline micro-kernels

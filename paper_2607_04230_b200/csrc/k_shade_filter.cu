@@ -30,15 +30,10 @@ __device__ __forceinline__ F3 calc_tangent(int idx, int count, F3 prev, F3 curr,
   else return normalize(next - prev);
 }
 
-__global__ void __launch_bounds__(256)
-k_shade(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const float4* __restrict__ vertices,
-        CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, float4* __restrict__ colour) {
-  const size_t n_px = (size_t)cam.W * cam.H;
-  const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= n_px) return;
-  const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
-  const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
-  if (w_none(G)) return;  // colour is only ever read where a centre hit exists
+// O6 for one word: linear RGB of the hit it names (stand-in model, R23)
+__device__ __forceinline__ F3 shade_word(const SceneDev* __restrict__ sc, const uint4* __restrict__ table,
+                                         const float4* __restrict__ vertices, const CamDev& cam, const ShadeParams& sp,
+                                         unsigned long long G) {
   const Loc l = locate_strand(sc, table, w_sid(G));
   const GroomDev& g = sc->g[l.groom];
   const int j = (int)w_j(G), C = (int)l.C;
@@ -75,7 +70,50 @@ k_shade(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const 
     rgb.y += sp.light_rgb[li][1] * s * (sp.k_d * alb.y + sp.k_R * MR + sp.k_TRT * MT * alb.y);
     rgb.z += sp.light_rgb[li][2] * s * (sp.k_d * alb.z + sp.k_R * MR + sp.k_TRT * MT * alb.z);
   }
+  return rgb;
+}
+
+__global__ void __launch_bounds__(256)
+k_shade(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const float4* __restrict__ vertices,
+        CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, float4* __restrict__ colour) {
+  const size_t n_px = (size_t)cam.W * cam.H;
+  const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n_px) return;
+  const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
+  const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
+  if (w_none(G)) return;  // colour is only ever read where a centre hit exists
+  const F3 rgb = shade_word(sc, table, vertices, cam, sp, G);
   colour[p] = make_float4(rgb.x, rgb.y, rgb.z, 1.0f);
+}
+
+// MSAA-k reference resolve (DESIGN.md R-msaa): mean over the k samples of (shaded hit | background)
+__global__ void __launch_bounds__(256)
+k_resolve_msaa(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const float4* __restrict__ vertices,
+               CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ samples, uint32_t ms_k,
+               const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
+  const size_t n_px = (size_t)cam.W * cam.H;
+  const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n_px) return;
+  F3 acc = f3(0.f, 0.f, 0.f);
+  uint32_t n_hit = 0;
+  for (uint32_t s = 0; s < ms_k; ++s) {
+    const unsigned long long w = __ldg(&samples[(size_t)s * n_px + p]);
+    if (w_none(w)) continue;
+    acc = acc + shade_word(sc, table, vertices, cam, sp, w);
+    ++n_hit;
+  }
+  F3 bg = f3(sp.background[0], sp.background[1], sp.background[2]);
+  if (scene_rgb) bg = f3(__ldg(&scene_rgb[p]));
+  const float inv_k = 1.0f / (float)ms_k, alpha = (float)n_hit * inv_k;
+  out[p] = make_float4(acc.x * inv_k + (1.f - alpha) * bg.x, acc.y * inv_k + (1.f - alpha) * bg.y,
+                       acc.z * inv_k + (1.f - alpha) * bg.z, alpha);
+}
+
+void launch_resolve_msaa(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+                         ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
+                         float4* out, cudaStream_t st) {
+  const size_t n = (size_t)cam.W * cam.H;
+  k_resolve_msaa<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, table, vertices, cam, sp, samples, ms_k, scene_rgb, out);
 }
 
 // R22: unit screen direction of the segment a word names; fixed-order fp32 (decides strip membership)

@@ -443,6 +443,39 @@ def test_groom_mask_and_sequential_passes(orc, hair_mod):
     assert torch.equal(a1[0], a2[0]) and torch.equal(a1[1], a2[1])
 
 
+@pytest.mark.parametrize("k", [1, 2, 4, 8])
+def test_msaa_reference_mode(orc, hair_mod, k):
+    """hair_render_msaa (R-msaa): sample layers bit-exact against the oracle on the GPU's vertices, resolve
+    against the oracle's resolve of the GPU's layers."""
+    b = hair_mod
+    sc = synth.config(2, scale=0.05, res_scale=0.33)
+    cam, lam, prm = sc["camera"], sc["lam"], dict(sc["params"], background_rgb=(0.1, 0.2, 0.3))
+    h = b.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(prm)
+    samples, rgb = h.render_msaa(cam, lam, k)
+    S = samples.cpu().numpy().view(np.uint64)
+    verts = h.debug_vertices().cpu().numpy()
+    f = orc.Frame(sc["grooms"])
+    f.lod(cam, lam)
+    f.generate()
+    f.set_vertices_f32(verts[: f.n_vertices])
+    ms = f.raster_msaa(cam, prm, k)
+    assert np.array_equal(ms, S), float((ms == S).mean())
+    assert (S != EMPTY).sum() > 500 * k
+    f.set_msaa(S)
+    out = f.resolve_msaa(cam, prm)
+    got = rgb.cpu().numpy().astype(np.float64)
+    assert np.abs(out - got).max() <= TOL_RGB
+    assert psnr(out[..., :3], got[..., :3], max(float(out[..., :3].max()), 1.0)) > MIN_PSNR
+    if k == 1:  # one sample at the pixel centre = the centre layer of the normal frame
+        gb, _ = h.render(cam, lam)
+        assert np.array_equal(b.gbuffer_to_numpy(gb)[..., 0], S[0])
+    with pytest.raises(b.HairError):
+        h.render_msaa(cam, lam, 3)
+
+
 def test_render_to_host_async_pipeline(hair_mod):
     """Two frames in flight: each host buffer, after host_wait, holds exactly what hair_render gives."""
     import torch
