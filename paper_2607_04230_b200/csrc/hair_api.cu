@@ -41,6 +41,8 @@ struct hair_ctx {
   uint4* d_table = nullptr;
   uint32_t* d_grp = nullptr;  // [n_bi + 1] exclusive scan of the raster's work groups per bundle-instance
   size_t table_cap = 0;
+  uint2* d_srec = nullptr;  // per strand id: {vertex offset, C | groom << 8} of this frame (k_generate)
+  size_t srec_cap = 0;
   float4* d_vertices = nullptr;
   size_t vertex_cap = 0;
   size_t vertex_need = 0;
@@ -180,6 +182,13 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
     CK(cudaMalloc((void**)&c->d_grp, ((size_t)c->scene.n_bi + 1) * sizeof(uint32_t)));
     c->table_cap = c->scene.n_bi;
   }
+  if (c->scene.n_strands_total > c->srec_cap) {
+    cudaFree(c->d_srec);
+    c->d_srec = nullptr;
+    c->srec_cap = 0;
+    CK(cudaMalloc((void**)&c->d_srec, (size_t)c->scene.n_strands_total * sizeof(uint2)));
+    c->srec_cap = c->scene.n_strands_total;
+  }
   if (c->vertex_need > c->vertex_cap) {
     cudaFree(c->d_vertices);
     c->d_vertices = nullptr;
@@ -250,7 +259,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_LOD);
   if (front && n_bi) {
-    launch_generate(c->d_scene, n_bi, c->d_table, c->d_vertices, c->d_counters, c->c_max, c->n_sm, st);
+    launch_generate(c->d_scene, n_bi, c->d_table, c->d_vertices, c->d_srec, c->d_counters, c->c_max, c->n_sm, st);
     ++launches;
   }
   mark(EV_GEN);
@@ -269,17 +278,17 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_RASTER);
   if (po.ms_k) {
-    launch_resolve_msaa(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, po.ms_k, (const float4*)scene_rgb,
+    launch_resolve_msaa(c->d_scene, c->d_srec, c->d_vertices, k, sp, gbuf, po.ms_k, (const float4*)scene_rgb,
                         (float4*)rgb, st);
     ++launches;
   }
   if ((stage_mask & 2u) && !po.ms_k) {
-    launch_shade(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour, st);
+    launch_shade(c->d_scene, c->d_srec, c->d_vertices, k, sp, gbuf, c->d_colour, st);
     ++launches;
   }
   mark(EV_SHADE);
   if ((stage_mask & 4u) && !po.ms_k) {
-    launches += launch_filter(c->d_scene, c->d_table, c->d_vertices, k, sp, gbuf, c->d_colour,
+    launches += launch_filter(c->d_scene, c->d_srec, c->d_vertices, k, sp, gbuf, c->d_colour,
                               (const float4*)scene_rgb, (float4*)rgb, c->d_counters, count, st);
   }
   mark(EV_FILTER);
@@ -337,6 +346,7 @@ void hair_destroy(hair_ctx* c) {
   cudaFree(c->d_table);
   cudaFree(c->d_grp);
   cudaFree(c->d_vertices);
+  cudaFree(c->d_srec);
   cudaFree(c->d_colour);
   cudaFree(c->d_counters);
   if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);

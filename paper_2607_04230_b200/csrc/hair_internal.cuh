@@ -137,43 +137,37 @@ __device__ __forceinline__ uint32_t pcg(uint32_t v) {
   return (w >> 22) ^ w;
 }
 
-// strand id -> first vertex and control-point count of the strand in this frame's vertex buffer
+// strand id -> first vertex, control-point count and groom of the strand in this frame's vertex buffer:
+// one 8-byte record per strand id, written by k_generate for the strands it generates ({vertex offset,
+// C | groom << 8}); one gather instead of the tri_of -> table / off chain when shading and filtering
 struct Loc {
   uint32_t voff, C, groom;
 };
-__device__ __forceinline__ Loc locate_strand(const SceneDev* __restrict__ sc, const uint4* __restrict__ table,
-                                             uint32_t sid) {
-  uint32_t gi = 0;
-  for (uint32_t k = 1; k < sc->n_grooms; ++k)
-    if (sid >= sc->g[k].sid_base) gi = k;
-  const GroomDev& g = sc->g[gi];
-  uint32_t rel = sid - g.sid_base;
-  uint32_t q = rel / g.N, id_local = rel - q * g.N;
-  const uint32_t lo = __ldg(&g.tri_of[id_local]);
-  uint4 e = __ldg(&table[g.gid_base + q * g.T + lo]);
+__device__ __forceinline__ Loc locate_strand(const uint2* __restrict__ srec, uint32_t sid) {
+  const uint2 r = __ldg(&srec[sid]);
   Loc l;
-  l.C = e.y;
-  l.voff = e.w + (id_local - __ldg(&g.off[lo])) * e.y;
-  l.groom = gi;
+  l.voff = r.x;
+  l.C = r.y & 0xFFu;
+  l.groom = r.y >> 8;
   return l;
 }
 
 // ------------------------------------------------------------------ launchers (one per .cu)
 void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint32_t groom_mask,
                      uint4* table, uint32_t* grp, unsigned long long* counters, cudaStream_t st);
-void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices,
+void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices, uint2* srec,
                      unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st);
 void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_zn, cudaStream_t st);
 void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                    unsigned long long* counters, bool count, uint32_t ms_k, int n_sm, cudaStream_t st);
-void launch_resolve_msaa(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
                          float4* out, cudaStream_t st);
-void launch_shade(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                   ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st);
-int launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+int launch_filter(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                    ShadeParams sp, const unsigned long long* gbuf, const float4* colour, const float4* scene_rgb,
                    float4* out, unsigned long long* counters, bool count, cudaStream_t st);
 void launch_atomic_microbench(int mode, unsigned long long* words, unsigned long long n_words,

@@ -56,7 +56,8 @@ __device__ __forceinline__ F3 shfl3_down(F3 v) {
 //  [36..39] cos/sin twist angle, cos/sin of the curl turn angle 2*pi*turns*w
 __global__ void __launch_bounds__(GEN_WARPS * 32, GEN_MIN_BLOCKS)
 k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
-           float4* __restrict__ vertices, unsigned long long* __restrict__ counters, uint32_t c_max) {
+           float4* __restrict__ vertices, uint2* __restrict__ strand_rec, unsigned long long* __restrict__ counters,
+           uint32_t c_max) {
   extern __shared__ float4 smem4[];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   // per warp: the bundle table [c_max][HAIR_ROW], then 32 strand records (b1, b2, cos/sin curl phase) + 32 hashes
@@ -197,6 +198,8 @@ k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restri
         if (ops & HAIR_OP_CURL) sincospif(2.f * ((float)(pcg(base + 3u) >> 8) * (1.0f / 16777216.0f)), &sphi, &cphi);
         srec[lane] = make_float4((float)a1 * (1.0f / 16777216.0f), (float)a2 * (1.0f / 16777216.0f), cphi, sphi);
         sbase[lane] = base;
+        // where shading finds this strand (hair_internal.cuh locate_strand)
+        strand_rec[g.sid_base + q * g.N + off_t + k0 + lane] = make_uint2(e.w + (k0 + lane) * C, C | (gi << 8));
       }
       __syncwarp();
       const uint32_t n_vb = nk * C;
@@ -277,7 +280,7 @@ k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restri
   }
 }
 
-void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices,
+void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices, uint2* srec,
                      unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st) {
   size_t smem = (size_t)GEN_WARPS * ((size_t)c_max * HAIR_ROW + 32 * 5) * sizeof(float);
   static size_t configured = 0;
@@ -291,5 +294,5 @@ void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table,
   uint32_t grid = (uint32_t)(n_sm * per_sm);
   uint32_t need = (n_bi + GEN_WARPS - 1) / GEN_WARPS;
   if (grid > need) grid = need;
-  k_generate<<<grid, GEN_WARPS * 32, smem, st>>>(d_scene, n_bi, table, vertices, counters, c_max);
+  k_generate<<<grid, GEN_WARPS * 32, smem, st>>>(d_scene, n_bi, table, vertices, srec, counters, c_max);
 }

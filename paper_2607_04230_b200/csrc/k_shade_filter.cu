@@ -31,10 +31,10 @@ __device__ __forceinline__ F3 calc_tangent(int idx, int count, F3 prev, F3 curr,
 }
 
 // O6 for one word: linear RGB of the hit it names (stand-in model, R23)
-__device__ __forceinline__ F3 shade_word(const SceneDev* __restrict__ sc, const uint4* __restrict__ table,
+__device__ __forceinline__ F3 shade_word(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec,
                                          const float4* __restrict__ vertices, const CamDev& cam, const ShadeParams& sp,
                                          unsigned long long G) {
-  const Loc l = locate_strand(sc, table, w_sid(G));
+  const Loc l = locate_strand(srec, w_sid(G));
   const GroomDev& g = sc->g[l.groom];
   const int j = (int)w_j(G), C = (int)l.C;
   const float t = (float)w_t9(G) * (1.0f / 511.0f);
@@ -74,7 +74,7 @@ __device__ __forceinline__ F3 shade_word(const SceneDev* __restrict__ sc, const 
 }
 
 __global__ void __launch_bounds__(256)
-k_shade(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const float4* __restrict__ vertices,
+k_shade(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
         CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, float4* __restrict__ colour) {
   const size_t n_px = (size_t)cam.W * cam.H;
   const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -82,13 +82,13 @@ k_shade(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const 
   const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
   const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
   if (w_none(G)) return;  // colour is only ever read where a centre hit exists
-  const F3 rgb = shade_word(sc, table, vertices, cam, sp, G);
+  const F3 rgb = shade_word(sc, srec, vertices, cam, sp, G);
   colour[p] = make_float4(rgb.x, rgb.y, rgb.z, 1.0f);
 }
 
 // MSAA-k reference resolve (DESIGN.md R-msaa): mean over the k samples of (shaded hit | background)
 __global__ void __launch_bounds__(256)
-k_resolve_msaa(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const float4* __restrict__ vertices,
+k_resolve_msaa(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
                CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ samples, uint32_t ms_k,
                const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
   const size_t n_px = (size_t)cam.W * cam.H;
@@ -99,7 +99,7 @@ k_resolve_msaa(const SceneDev* __restrict__ sc, const uint4* __restrict__ table,
   for (uint32_t s = 0; s < ms_k; ++s) {
     const unsigned long long w = __ldg(&samples[(size_t)s * n_px + p]);
     if (w_none(w)) continue;
-    acc = acc + shade_word(sc, table, vertices, cam, sp, w);
+    acc = acc + shade_word(sc, srec, vertices, cam, sp, w);
     ++n_hit;
   }
   F3 bg = f3(sp.background[0], sp.background[1], sp.background[2]);
@@ -109,18 +109,18 @@ k_resolve_msaa(const SceneDev* __restrict__ sc, const uint4* __restrict__ table,
                        acc.z * inv_k + (1.f - alpha) * bg.z, alpha);
 }
 
-void launch_resolve_msaa(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
                          float4* out, cudaStream_t st) {
   const size_t n = (size_t)cam.W * cam.H;
-  k_resolve_msaa<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, table, vertices, cam, sp, samples, ms_k, scene_rgb, out);
+  k_resolve_msaa<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, samples, ms_k, scene_rgb, out);
 }
 
 // R22: unit screen direction of the segment a word names; fixed-order fp32 (decides strip membership)
-__device__ __forceinline__ float2 screen_tangent(const SceneDev* __restrict__ sc, const uint4* __restrict__ table,
+__device__ __forceinline__ float2 screen_tangent(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec,
                                                  const float4* __restrict__ vertices, const CamDev& cam,
                                                  unsigned long long word) {
-  const Loc l = locate_strand(sc, table, w_sid(word));
+  const Loc l = locate_strand(srec, w_sid(word));
   const float4* vs = vertices + l.voff + w_j(word);
   const float4 va = __ldg(vs), vb = __ldg(vs + 1);
   const Proj a = project_exact(cam, va.x, va.y, va.z), b = project_exact(cam, vb.x, vb.y, vb.z);
@@ -168,7 +168,7 @@ __device__ __forceinline__ bool in_strip_exact(float fdx, float fdy, float Tx, f
 
 template <int R>
 __global__ void __launch_bounds__(256)
-k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const float4* __restrict__ vertices,
+k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
          CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, const float4* __restrict__ colour,
          const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
   constexpr int SW = FT_W + 2 * R, SH = FT_H + 2 * R, NS = SW * SH;
@@ -245,11 +245,11 @@ k_filter(const SceneDev* __restrict__ sc, const uint4* __restrict__ table, const
     const bool isCenter = !w_none(G[k]), isCons = !w_none(A[k]);
     Tc[k] = Ta[k] = make_float2(1.f, 0.f);
     if (isCenter) {
-      Tc[k] = screen_tangent(sc, table, vertices, cam, G[k]);
+      Tc[k] = screen_tangent(sc, srec, vertices, cam, G[k]);
       fly[k] = isCons && w_dq(G[k]) >= w_dq(A[k]) && w_dq(G[k]) - w_dq(A[k]) >= sp.taufly_q;  // PAPER.md:175, R21
     }
     const bool isA = fly[k] || (isCons && !isCenter);  // fly-away strand, or promoted pixel: w_color = 1
-    if (isA) Ta[k] = screen_tangent(sc, table, vertices, cam, A[k]);
+    if (isA) Ta[k] = screen_tangent(sc, srec, vertices, cam, A[k]);
     bal[2 * k] = __ballot_sync(0xffffffffu, isCenter);
     bal[2 * k + 1] = __ballot_sync(0xffffffffu, isA);
   }
@@ -413,24 +413,24 @@ k_count_pixels(const unsigned long long* __restrict__ gbuf, size_t n_px, unsigne
   }
 }
 
-void launch_shade(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                   ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st) {
   size_t n = (size_t)cam.W * cam.H;
-  k_shade<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, table, vertices, cam, sp, gbuf, colour);
+  k_shade<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour);
 }
 
 template <int R>
-static void launch_filter_r(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+static void launch_filter_r(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                             ShadeParams sp, const unsigned long long* gbuf, const float4* colour,
                             const float4* scene_rgb, float4* out, cudaStream_t st) {
   constexpr int NS = (FT_W + 2 * R) * (FT_H + 2 * R);
   constexpr size_t smem = (size_t)NS * (sizeof(float4) + 2 * sizeof(uint32_t)) + 2 * FT_W * FT_H * sizeof(float4);
   cudaFuncSetAttribute(k_filter<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   dim3 grid((cam.W + FT_W - 1) / FT_W, (cam.H + FT_H - 1) / FT_H);
-  k_filter<R><<<grid, 256, smem, st>>>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out);
+  k_filter<R><<<grid, 256, smem, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out);
 }
 
-int launch_filter(const SceneDev* d_scene, const uint4* table, const float4* vertices, CamDev cam,
+int launch_filter(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                   ShadeParams sp, const unsigned long long* gbuf, const float4* colour, const float4* scene_rgb,
                   float4* out, unsigned long long* counters, bool count, cudaStream_t st) {
   const size_t n = (size_t)cam.W * cam.H;
@@ -444,14 +444,14 @@ int launch_filter(const SceneDev* d_scene, const uint4* table, const float4* ver
     return launches;
   }
   switch (sp.r) {
-    case 0: launch_filter_r<0>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 1: launch_filter_r<1>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 2: launch_filter_r<2>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 3: launch_filter_r<3>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 4: launch_filter_r<4>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 5: launch_filter_r<5>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 6: launch_filter_r<6>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    default: launch_filter_r<7>(d_scene, table, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 0: launch_filter_r<0>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 1: launch_filter_r<1>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 2: launch_filter_r<2>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 3: launch_filter_r<3>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 4: launch_filter_r<4>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 5: launch_filter_r<5>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 6: launch_filter_r<6>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    default: launch_filter_r<7>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
   }
   return launches;
 }
