@@ -58,6 +58,8 @@ struct hair_ctx {
   float* d_own_rgb[HAIR_HOST_SLOTS] = {};
   size_t own_px = 0;
   cudaStream_t copy_stream = nullptr;
+  cudaStream_t aux_stream = nullptr;  // the G-buffer clear runs here, beside LOD / scan / generate
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   cudaEvent_t ev_rendered[HAIR_HOST_SLOTS] = {}, ev_copied[HAIR_HOST_SLOTS] = {};
   bool slot_used[HAIR_HOST_SLOTS] = {};
   int next_slot = 0;
@@ -250,6 +252,23 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
     if (timed) cudaEventRecord(evs[e], st);
   };
   mark(EV_BEGIN);
+  // The clear of the G-buffer does not depend on LOD / scan / generate: it runs beside them on the context's second
+  // stream (forked after everything already enqueued on `st`, joined before the raster). ms_clear then reads ~0.
+  const bool fork_clear = front && n_bi && (stage_mask & 1u);
+  auto clear_on = [&](cudaStream_t cs) -> int {
+    if (po.ms_k) CK(cudaMemsetAsync(gbuf, 0xFF, (size_t)w * h * po.ms_k * sizeof(unsigned long long), cs));
+    else if (po.reseed) launch_reseed(gbuf, (size_t)w * h, cs);
+    else launch_clear(gbuf, (size_t)w * h, scene_zn, cs);
+    return HAIR_OK;
+  };
+  if (fork_clear) {
+    CK(cudaEventRecord(c->ev_fork, st));
+    CK(cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
+    rc = clear_on(c->aux_stream);
+    if (rc) return rc;
+    CK(cudaEventRecord(c->ev_join, c->aux_stream));
+    ++launches;
+  }
   if (front && !n_bi) CK(cudaMemsetAsync(c->d_counters, 0, CNT_N * sizeof(unsigned long long), st));
   if (front && n_bi) {
     LambdaArr la;
@@ -263,10 +282,10 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
     ++launches;
   }
   mark(EV_GEN);
-  if (stage_mask & 1u) {
-    if (po.ms_k) CK(cudaMemsetAsync(gbuf, 0xFF, (size_t)w * h * po.ms_k * sizeof(unsigned long long), st));
-    else if (po.reseed) launch_reseed(gbuf, (size_t)w * h, st);
-    else launch_clear(gbuf, (size_t)w * h, scene_zn, st);
+  if (fork_clear) CK(cudaStreamWaitEvent(st, c->ev_join, 0));
+  else if (stage_mask & 1u) {
+    rc = clear_on(st);
+    if (rc) return rc;
     ++launches;
   }
   mark(EV_CLEAR);
@@ -325,7 +344,10 @@ int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream) {
             cudaMallocHost((void**)&c->h_counters, CNT_N * sizeof(unsigned long long)) == cudaSuccess;
   for (int f = 0; ok && f < EV_RING; ++f)
     for (int i = 0; ok && i < EV_N; ++i) ok = cudaEventCreate(&c->ev[f][i]) == cudaSuccess;
-  ok = ok && cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+  ok = ok && cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess &&
+       cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking) == cudaSuccess &&
+       cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
+       cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) == cudaSuccess;
   for (int k = 0; ok && k < HAIR_HOST_SLOTS; ++k)
     ok = cudaEventCreateWithFlags(&c->ev_rendered[k], cudaEventDisableTiming) == cudaSuccess &&
          cudaEventCreateWithFlags(&c->ev_copied[k], cudaEventDisableTiming) == cudaSuccess;
@@ -357,6 +379,12 @@ void hair_destroy(hair_ctx* c) {
     if (c->ev_copied[k]) cudaEventDestroy(c->ev_copied[k]);
   }
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->aux_stream) {
+    cudaStreamSynchronize(c->aux_stream);
+    cudaStreamDestroy(c->aux_stream);
+  }
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+  if (c->ev_join) cudaEventDestroy(c->ev_join);
   if (c->h_counters) cudaFreeHost(c->h_counters);
   for (int f = 0; f < EV_RING; ++f)
     for (int i = 0; i < EV_N; ++i)
