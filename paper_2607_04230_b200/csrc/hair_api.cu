@@ -39,6 +39,7 @@ struct hair_ctx {
   hair_render_params prm;
   // scratch
   uint4* d_table = nullptr;
+  uint4* d_part = nullptr;    // [ceil(n_bi / 256)] tile sums between k_lod and k_scan
   uint32_t* d_grp = nullptr;  // [n_bi + 1] exclusive scan of the raster's work groups per bundle-instance
   size_t table_cap = 0;
   uint2* d_srec = nullptr;  // per strand id: {vertex offset, C | groom << 8} of this frame (k_generate)
@@ -177,11 +178,14 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
   if (c->scene.n_bi > c->table_cap) {
     cudaFree(c->d_table);
     cudaFree(c->d_grp);
+    cudaFree(c->d_part);
+    c->d_part = nullptr;
     c->d_table = nullptr;
     c->d_grp = nullptr;
     c->table_cap = 0;
     CK(cudaMalloc((void**)&c->d_table, (size_t)c->scene.n_bi * sizeof(uint4)));
     CK(cudaMalloc((void**)&c->d_grp, ((size_t)c->scene.n_bi + 1) * sizeof(uint32_t)));
+    CK(cudaMalloc((void**)&c->d_part, ((size_t)c->scene.n_bi / 256 + 1) * sizeof(uint4)));
     c->table_cap = c->scene.n_bi;
   }
   if (c->scene.n_strands_total > c->srec_cap) {
@@ -273,7 +277,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   if (front && n_bi) {
     LambdaArr la;
     for (uint32_t i = 0; i < HAIR_MAX_GROOMS; ++i) la.v[i] = n_lam == 0 ? 0.f : lam[n_lam == 1 ? 0 : (i < n_lam ? i : 0)];
-    launch_lod_scan(c->d_scene, n_bi, k, la, po.groom_mask & c->prm.groom_mask, c->d_table, c->d_grp, c->d_counters, st);
+    launch_lod_scan(c->d_scene, n_bi, k, la, po.groom_mask & c->prm.groom_mask, c->d_table, c->d_grp, c->d_part, c->d_counters, st);
     launches += 2;
   }
   mark(EV_LOD);
@@ -367,6 +371,7 @@ void hair_destroy(hair_ctx* c) {
   cudaFree(c->d_scene);
   cudaFree(c->d_table);
   cudaFree(c->d_grp);
+  cudaFree(c->d_part);
   cudaFree(c->d_vertices);
   cudaFree(c->d_srec);
   cudaFree(c->d_colour);

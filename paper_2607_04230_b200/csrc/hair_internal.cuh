@@ -154,7 +154,7 @@ __device__ __forceinline__ Loc locate_strand(const uint2* __restrict__ srec, uin
 
 // ------------------------------------------------------------------ launchers (one per .cu)
 void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint32_t groom_mask,
-                     uint4* table, uint32_t* grp, unsigned long long* counters, cudaStream_t st);
+                     uint4* table, uint32_t* grp, uint4* part, unsigned long long* counters, cudaStream_t st);
 void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices, uint2* srec,
                      unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st);
 void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_zn, cudaStream_t st);

@@ -21,10 +21,16 @@ __device__ __forceinline__ void lod_counts(float L, uint32_t N, float delta, uin
   C = min(min((1u << lg) + 1u, 127u), c_full);
 }
 
+__device__ __forceinline__ uint32_t raster_groups(uint32_t n_v) {  // units of RAS_GROUP*RAS_CHUNK segment starts
+  return n_v >= 2 ? (n_v - 1 + RAS_GROUP * RAS_CHUNK - 1) / (RAS_GROUP * RAS_CHUNK) : 0u;
+}
+
 __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, uint32_t n_bi, CamDev cam,
-                                             LambdaArr lam, uint32_t groom_mask, uint4* __restrict__ table) {
+                                             LambdaArr lam, uint32_t groom_mask, uint4* __restrict__ table,
+                                             uint4* __restrict__ part) {
   uint32_t gid = blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= n_bi) return;
+  uint32_t nlod = 0, C = 0;
+  if (gid < n_bi) {
   uint32_t gi = 0;
   for (uint32_t k = 1; k < sc->n_grooms; ++k)
     if (gid >= sc->g[k].gid_base) gi = k;
@@ -33,7 +39,6 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
   uint32_t q = rel / g.T, t = rel - q * g.T;
   uint32_t N = __ldg(&g.npt[t]);
   float lambda = lam.v[gi];
-  uint32_t nlod, C;
   if (!(lambda > 0.f)) {  // R14: LOD and culling off
     nlod = N;
     C = g.c_full;
@@ -88,101 +93,97 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
   }
   if (!((groom_mask >> gi) & 1u)) nlod = C = 0;  // R-seq: this groom is not drawn in this pass
   table[gid] = make_uint4(nlod, C, 0u, 0u);
+  }
+  // sums of this tile of 256 bundle-instances for the scan: strands, vertices, raster work groups, culled
+  uint32_t ts = nlod, tv = nlod * C, tg = raster_groups(nlod * C), tc = (gid < n_bi && nlod == 0) ? 1u : 0u;
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    ts += __shfl_xor_sync(0xffffffffu, ts, d);
+    tv += __shfl_xor_sync(0xffffffffu, tv, d);
+    tg += __shfl_xor_sync(0xffffffffu, tg, d);
+    tc += __shfl_xor_sync(0xffffffffu, tc, d);
+  }
+  __shared__ uint4 s_w[8];
+  if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = make_uint4(ts, tv, tg, tc);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint4 a = s_w[0];
+    for (int wv = 1; wv < 8; ++wv) a.x += s_w[wv].x, a.y += s_w[wv].y, a.z += s_w[wv].z, a.w += s_w[wv].w;
+    part[blockIdx.x] = a;
+  }
 }
 
 // Exclusive scans of N_LOD, N_LOD*C and the raster's work-group count over bundle-instances in
 // index order (O1 step 6). One CTA of 1024 threads; each warp owns a contiguous range and
 // walks it 32 entries at a time with a shuffle scan and a running carry; the 32 warp totals are
 // scanned by warp 0; a second pass adds the warp offsets. Coalesced 16-byte accesses throughout.
-__device__ __forceinline__ uint32_t raster_groups(uint32_t n_v) {  // units of RAS_GROUP*RAS_CHUNK segment starts
-  return n_v >= 2 ? (n_v - 1 + RAS_GROUP * RAS_CHUNK - 1) / (RAS_GROUP * RAS_CHUNK) : 0u;
-}
 
-__global__ void __launch_bounds__(1024) k_scan(uint4* __restrict__ table, uint32_t* __restrict__ grp, uint32_t n_bi,
-                                               unsigned long long* __restrict__ counters) {
-  __shared__ uint32_t s_slot[32], s_vert[32], s_grp[32], s_cull[32];
-  const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint32_t per_warp = ((n_bi + 31) / 32 + 31) / 32 * 32;  // multiple of 32
-  const uint32_t begin = min(warp * per_warp, n_bi), end = min(begin + per_warp, n_bi);
-  uint32_t carry_s = 0, carry_v = 0, carry_g = 0, culled = 0;
-  for (uint32_t base = begin; base < end; base += 32) {
-    uint32_t i = base + lane;
-    uint4 e = i < end ? table[i] : make_uint4(0, 0, 0, 0);
-    uint32_t s = e.x, v = e.x * e.y, g = raster_groups(v);
-    culled += (i < end && e.x == 0) ? 1u : 0u;
-    uint32_t is = s, iv = v, ig = g;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      uint32_t a = __shfl_up_sync(0xffffffffu, is, d), b = __shfl_up_sync(0xffffffffu, iv, d),
-               c = __shfl_up_sync(0xffffffffu, ig, d);
-      if (lane >= d) {
-        is += a;
-        iv += b;
-        ig += c;
-      }
-    }
-    if (i < end) {
-      e.z = carry_s + is - s;
-      e.w = carry_v + iv - v;
-      table[i] = e;
-      grp[i] = carry_g + ig - g;
-    }
-    carry_s += __shfl_sync(0xffffffffu, is, 31);
-    carry_v += __shfl_sync(0xffffffffu, iv, 31);
-    carry_g += __shfl_sync(0xffffffffu, ig, 31);
+__global__ void __launch_bounds__(256) k_scan(uint4* __restrict__ table, uint32_t* __restrict__ grp, uint32_t n_bi,
+                                              const uint4* __restrict__ part, unsigned long long* __restrict__ counters) {
+  __shared__ uint32_t s_a[8][4], s_b[8][3];
+  const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tile = blockIdx.x;
+  // (1) what lies before this tile: sums of the tiles in front of it
+  uint32_t ps = 0, pv = 0, pg = 0, pc = 0;
+  for (uint32_t t = threadIdx.x; t < tile; t += 256) {
+    const uint4 a = __ldg(&part[t]);
+    ps += a.x, pv += a.y, pg += a.z, pc += a.w;
   }
 #pragma unroll
-  for (int d = 16; d > 0; d >>= 1) culled += __shfl_xor_sync(0xffffffffu, culled, d);
-  if (lane == 0) {
-    s_slot[warp] = carry_s;
-    s_vert[warp] = carry_v;
-    s_grp[warp] = carry_g;
-    s_cull[warp] = culled;
+  for (int d = 16; d > 0; d >>= 1) {
+    ps += __shfl_xor_sync(0xffffffffu, ps, d);
+    pv += __shfl_xor_sync(0xffffffffu, pv, d);
+    pg += __shfl_xor_sync(0xffffffffu, pg, d);
+    pc += __shfl_xor_sync(0xffffffffu, pc, d);
   }
+  // (2) exclusive scan inside the tile: shuffle scan per warp, then the 8 warp totals
+  const uint32_t i = tile * 256 + threadIdx.x;
+  uint4 e = i < n_bi ? table[i] : make_uint4(0, 0, 0, 0);
+  const uint32_t s = e.x, v = e.x * e.y, g = raster_groups(v);
+  uint32_t is = s, iv = v, ig = g;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    uint32_t a = __shfl_up_sync(0xffffffffu, is, d), b = __shfl_up_sync(0xffffffffu, iv, d),
+             c = __shfl_up_sync(0xffffffffu, ig, d);
+    if (lane >= d) {
+      is += a;
+      iv += b;
+      ig += c;
+    }
+  }
+  if (lane == 0) s_a[warp][0] = ps, s_a[warp][1] = pv, s_a[warp][2] = pg, s_a[warp][3] = pc;
+  if (lane == 31) s_b[warp][0] = is, s_b[warp][1] = iv, s_b[warp][2] = ig;
   __syncthreads();
-  if (warp == 0) {
-    uint32_t s = s_slot[lane], v = s_vert[lane], g = s_grp[lane], c = s_cull[lane];
-    uint32_t is = s, iv = v, ig = g;
+  uint32_t off_s = 0, off_v = 0, off_g = 0, culled = 0;
 #pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      uint32_t a = __shfl_up_sync(0xffffffffu, is, d), b = __shfl_up_sync(0xffffffffu, iv, d),
-               cc = __shfl_up_sync(0xffffffffu, ig, d);
-      if (lane >= d) {
-        is += a;
-        iv += b;
-        ig += cc;
-      }
-    }
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
-    s_slot[lane] = is - s;
-    s_vert[lane] = iv - v;
-    s_grp[lane] = ig - g;
-    if (lane == 31) {
-      counters[CNT_STRANDS] = is;
-      counters[CNT_VERTICES] = iv;
-      counters[CNT_SEGMENTS] = iv - is;  // sum N_LOD*(C-1)
-      counters[CNT_CULLED] = c;
-      counters[CNT_WORK_GEN] = 0;
-      counters[CNT_WORK_RASTER] = 0;
-      for (int k = CNT_SEG_DRAWN; k < CNT_N; ++k) counters[k] = 0;
-      grp[n_bi] = ig;  // total work groups: the raster's queue length
-    }
+  for (uint32_t wv = 0; wv < 8; ++wv) {
+    off_s += s_a[wv][0], off_v += s_a[wv][1], off_g += s_a[wv][2], culled += s_a[wv][3];  // tiles in front
+    if (wv < warp) off_s += s_b[wv][0], off_v += s_b[wv][1], off_g += s_b[wv][2];          // warps in front
   }
-  __syncthreads();
-  uint32_t off_s = s_slot[warp], off_v = s_vert[warp], off_g = s_grp[warp];
-  if (warp > 0)
-    for (uint32_t i = begin + lane; i < end; i += 32) {
-      uint4 e = table[i];
-      e.z += off_s;
-      e.w += off_v;
-      table[i] = e;
-      grp[i] += off_g;
-    }
+  if (i < n_bi) {
+    e.z = off_s + is - s;
+    e.w = off_v + iv - v;
+    table[i] = e;
+    grp[i] = off_g + ig - g;
+  }
+  // (3) the last tile knows the totals: device-side counts and queue lengths of the frame
+  if (tile == gridDim.x - 1 && threadIdx.x == 255) {
+    const uint4 mine = __ldg(&part[tile]);
+    const uint32_t n_s = off_s + is, n_v = off_v + iv, n_g = off_g + ig;
+    counters[CNT_STRANDS] = n_s;
+    counters[CNT_VERTICES] = n_v;
+    counters[CNT_SEGMENTS] = n_v - n_s;  // sum N_LOD*(C-1)
+    counters[CNT_CULLED] = culled + mine.w;
+    counters[CNT_WORK_GEN] = 0;
+    counters[CNT_WORK_RASTER] = 0;
+    for (int k = CNT_SEG_DRAWN; k < CNT_N; ++k) counters[k] = 0;
+    grp[n_bi] = n_g;  // total work groups: the raster's queue length
+  }
 }
 
 void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint32_t groom_mask,
-                     uint4* table, uint32_t* grp, unsigned long long* counters, cudaStream_t st) {
-  k_lod<<<(n_bi + 255) / 256, 256, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table);
-  k_scan<<<1, 1024, 0, st>>>(table, grp, n_bi, counters);
+                     uint4* table, uint32_t* grp, uint4* part, unsigned long long* counters, cudaStream_t st) {
+  // part: one uint4 per tile of 256 bundle-instances (sums), written by k_lod, read by k_scan
+  const uint32_t n_tiles = (n_bi + 255) / 256;
+  k_lod<<<n_tiles, 256, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table, part);
+  k_scan<<<n_tiles, 256, 0, st>>>(table, grp, n_bi, part, counters);
 }
