@@ -212,6 +212,39 @@ def test_bench_frame_full_size_sampled(orc, hair_mod):
     assert rep["n_hit"] > 0.3 * rep["n_px"], rep  # the windows do sit on hair
 
 
+def _densest_windows(G, cell, n):
+    H, W = G["gb"].shape[:2]
+    hit = (G["gb"][..., 1] != EMPTY)
+    grid = hit[: H // cell * cell, : W // cell * cell].reshape(H // cell, cell, W // cell, cell).sum((1, 3))
+    order = np.argsort(grid.reshape(-1))[::-1]
+    # the densest cell, a median one among the hit cells, and sparse ones (fringe)
+    nz = order[: int((grid > 0).sum())]
+    pick = list(nz[: n // 2]) + list(nz[len(nz) // 2: len(nz) // 2 + n // 4]) + list(nz[-(n - n // 2 - n // 4):])
+    return [(int(i % (W // cell)) * cell, int(i // (W // cell)) * cell,
+             int(i % (W // cell)) * cell + cell, int(i // (W // cell)) * cell + cell) for i in pick]
+
+
+def test_single_groom_full_size_sampled(orc, hair_mod):
+    """BASELINE config 2 as named: 50 000 strands x 32 segments, curl + frizz, width_world, 1920x1080, LOD off."""
+    sc = synth.config(2)
+    assert (sc["camera"]["width"], sc["camera"]["height"]) == (1920, 1080) and synth.n_strands(sc) == 50000
+    G = gpu_frame(hair_mod, sc)
+    assert G["stats"]["n_segments"] == 50000 * 32
+    rep = check_full_size_sampled(orc, sc, G, _densest_windows(G, 120, 8))
+    assert rep["n_hit"] > 5000, rep
+
+
+@pytest.mark.parametrize("lam,dist", [(0.0, 0.5), (4.0, 2.0), (8.0, 8.0)])
+def test_dense_groom_full_size_sampled(orc, hair_mod, lam, dist):
+    """BASELINE config 3 as named (150 000 strands x 48 segments, twist + clump, 3840x2160) at three points of its
+    lambda x distance sweep: LOD off close up, lambda 4 at 2 m, lambda 8 at 8 m."""
+    sc = synth.config(3, distance=dist, lam=lam)
+    assert (sc["camera"]["width"], sc["camera"]["height"]) == (3840, 2160) and synth.n_strands(sc) == 150000
+    G = gpu_frame(hair_mod, sc)
+    rep = check_full_size_sampled(orc, sc, G, _densest_windows(G, 96 if dist < 4 else 48, 8))
+    assert rep["n_hit"] > 500, rep
+
+
 def test_crowd_full_size_sampled(orc, hair_mod):
     """BASELINE config 5 as named: 64 instances x 30 000 strands at 10-40 m, 3840x2160, lambda 4."""
     sc = synth.config(5)
