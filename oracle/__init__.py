@@ -124,6 +124,16 @@ def lib():
         L.orc_frame_get_tangents.argtypes = [vp, vp]
         L.orc_frame_filter.argtypes = [vp, vp, vp]
         L.orc_frame_get_out.argtypes = [vp, vp]
+        L.orc_frame_set_payload_mode.restype = None
+        L.orc_frame_set_payload_mode.argtypes = [vp, C.c_int]
+        L.orc_oct_encode.restype = None
+        L.orc_oct_encode.argtypes = [vp, vp]
+        L.orc_oct_decode.restype = None
+        L.orc_oct_decode.argtypes = [u32, u32, vp]
+        L.orc_payload40.restype = u64
+        L.orc_payload40.argtypes = [vp, C.c_int, C.c_int, f32, u32, u32]
+        L.orc_unpack_payload.restype = None
+        L.orc_unpack_payload.argtypes = [u64, vp]
         _lib = L
     return _lib
 
@@ -179,8 +189,40 @@ def make_params(d: dict) -> Params:
     return p
 
 
+def oct_encode(T):
+    """R-payload: (ox8, oy8) of a unit vector, fp32 fixed order."""
+    T = np.ascontiguousarray(T, dtype=np.float32)
+    out = np.zeros(2, np.uint32)
+    lib().orc_oct_encode(_ptr(T), _ptr(out))
+    return int(out[0]), int(out[1])
+
+
+def oct_decode(ox: int, oy: int):
+    out = np.zeros(3, np.float32)
+    lib().orc_oct_decode(int(ox), int(oy), _ptr(out))
+    return out
+
+
+def payload40(v, j: int, t: float, a1: int, a2: int) -> int:
+    """R-payload: the 40 payload bits of a hit at parameter t on segment j of the strand v [C][4] float32."""
+    v = np.ascontiguousarray(v, dtype=np.float32).reshape(-1, 4)
+    return int(lib().orc_payload40(_ptr(v), int(j), v.shape[0], float(t), int(a1), int(a2)))
+
+
+def unpack_payload(words):
+    """fields of paper-payload words: dict of arrays dq, ox, oy, u6, v6, w6, ao6 (pure bit slicing)."""
+    w = np.asarray(words, dtype=np.uint64)
+    f = lambda sh, m: ((w >> np.uint64(sh)) & np.uint64(m)).astype(np.uint32)
+    return {"dq": f(40, 0xFFFFFF), "ox": f(32, 0xFF), "oy": f(24, 0xFF), "u6": f(18, 63), "v6": f(12, 63),
+            "w6": f(6, 63), "ao6": f(0, 63)}
+
+
 class Frame:
     """One scene + one frame of oracle state (table, vertices, G-buffer, colour, output)."""
+
+    def set_payload_mode(self, on: bool) -> None:
+        """R-payload: O4 writes / O6 reads the paper's self-contained payload (see hair_oracle.h)."""
+        self.L.orc_frame_set_payload_mode(self.h, 1 if on else 0)
 
     def __init__(self, grooms: list[dict]):
         self.L = lib()

@@ -11,6 +11,9 @@
 //   O4 raster+resolve PAPER.md:66-96    §3.1.2 (two layers PAPER.md:68-74, atomic min PAPER.md:85)
 //   O6 shading        PAPER.md:188-196  §3.4 (stand-in model, R23: parity unpinned vs paper)
 //   O7 filter         PAPER.md:154-176  §3.3, Eq. 9-10, Code 2
+//   O4p/O6p paper payload PAPER.md:78-96 §3.1.2 "G-buffer compression" (DESIGN.md R-payload): the word carries
+//                     octahedral tangent 2 x uint8 + u, v, w, AO 4 x uint6 instead of strand id | segment | t;
+//                     shading reconstructs the position from the depth and reads everything else from the word
 #include "hair_oracle.h"
 
 #include <algorithm>
@@ -88,6 +91,97 @@ inline uint32_t w_dq(uint64_t w) { return uint32_t(w >> 40); }
 inline uint32_t w_sid(uint64_t w) { return uint32_t(w >> 16) & 0xFFFFFFu; }
 inline uint32_t w_j(uint64_t w) { return uint32_t(w >> 9) & 0x7Fu; }
 inline uint32_t w_t9(uint64_t w) { return uint32_t(w) & 0x1FFu; }
+
+// ---------------------------------------------------------------- paper payload (R-payload)
+// [63:40] dq | [39:32] ox8 | [31:24] oy8 | [23:18] u6 | [17:12] v6 | [11:6] w6 | [5:0] ao6: "24 bits are used for
+// depth", "octahedral unit vector encoding" of the tangent, "uvw styling coordinates", ambient occlusion, "all
+// float values except for depth are quantized as either uint8 or uint6" — 2 x 8 + 4 x 6 is the only such split
+// that fills the 40 bits. Every code is a decision taken in fp32, one rounding per operation, in this order.
+struct F3 {
+  float x, y, z;
+};
+inline F3 unit3f(float x, float y, float z) {
+  float dd = x * x;
+  float e = y * y;
+  dd = dd + e;
+  e = z * z;
+  dd = dd + e;
+  if (!(dd > 0.f)) return {1.f, 0.f, 0.f};
+  float len = std::sqrt(dd);
+  return {x / len, y / len, z / len};
+}
+// calcTangent on fp32 vertices
+inline F3 tangent_f32(int idx, int count, const float* prev, const float* curr, const float* next) {
+  const float *a, *b;
+  if (idx == 0) a = next, b = curr;                // Root
+  else if (idx == count - 1) a = curr, b = prev;   // Tip
+  else a = next, b = prev;
+  return unit3f(a[0] - b[0], a[1] - b[1], a[2] - b[2]);
+}
+inline uint32_t q8s(float p) {  // [-1, 1] -> uint8
+  float h = p * 0.5f;
+  h = h + 0.5f;
+  h = h * 255.f;
+  h = h + 0.5f;
+  return std::min<uint32_t>(uint32_t(h), 255u);
+}
+inline uint32_t q6(float v) {  // [0, 1] -> uint6
+  float h = v * 63.f;
+  h = h + 0.5f;
+  return std::min<uint32_t>(uint32_t(h), 63u);
+}
+// octahedral encoding of a unit vector: project on |x| + |y| + |z| = 1, fold the lower hemisphere outwards
+inline void oct_encode(F3 T, uint32_t& ox, uint32_t& oy) {
+  float s = std::fabs(T.x) + std::fabs(T.y);
+  s = s + std::fabs(T.z);
+  float px = T.x / s, py = T.y / s;
+  if (T.z < 0.f) {
+    float ax = 1.f - std::fabs(py), ay = 1.f - std::fabs(px);
+    px = px >= 0.f ? ax : -ax;
+    py = py >= 0.f ? ay : -ay;
+  }
+  ox = q8s(px);
+  oy = q8s(py);
+}
+inline F3 oct_decode(uint32_t ox, uint32_t oy) {
+  float px = float(ox) / 255.f;
+  px = px * 2.f;
+  px = px - 1.f;
+  float py = float(oy) / 255.f;
+  py = py * 2.f;
+  py = py - 1.f;
+  float z = 1.f - std::fabs(px);
+  z = z - std::fabs(py);
+  float tx = px, ty = py;
+  if (z < 0.f) {
+    float ax = 1.f - std::fabs(py), ay = 1.f - std::fabs(px);
+    tx = px >= 0.f ? ax : -ax;
+    ty = py >= 0.f ? ay : -ay;
+  }
+  return unit3f(tx, ty, z);
+}
+inline uint32_t uv6(uint32_t a24) { return (a24 * 63u + (1u << 23)) >> 24; }  // round(a * 2^-24 * 63), integers
+// the 40 payload bits of a hit on segment j (of C control points) at parameter t. v = the strand's fp32 vertices
+// (x, y, z, ao) x C; a1, a2 = the strand's folded 24-bit root coordinates (R6).
+inline uint64_t payload40(const float* v, int j, int C, float t, uint32_t a1, uint32_t a2) {
+  auto P = [&](int i) { return v + 4 * std::min(std::max(i, 0), C - 1); };
+  F3 Tj = tangent_f32(j, C, P(j - 1), P(j), P(j + 1));
+  F3 Tj1 = tangent_f32(j + 1, C, P(j), P(j + 1), P(j + 2));
+  float omt = 1.f - t;
+  float x = omt * Tj.x, y = omt * Tj.y, z = omt * Tj.z;
+  float x1 = t * Tj1.x, y1 = t * Tj1.y, z1 = t * Tj1.z;
+  F3 T = unit3f(x + x1, y + y1, z + z1);
+  uint32_t ox, oy;
+  oct_encode(T, ox, oy);
+  float w = float(j) + t;
+  w = w / float(C - 1);
+  float ao = omt * P(j)[3];
+  float ao1 = t * P(j + 1)[3];
+  ao = ao + ao1;
+  ao = std::min(std::max(ao, 0.f), 1.f);
+  return (uint64_t(ox) << 32) | (uint64_t(oy) << 24) | (uint64_t(uv6(a1)) << 18) | (uint64_t(uv6(a2)) << 12) |
+         (uint64_t(q6(w)) << 6) | uint64_t(q6(ao));
+}
 
 // ---------------------------------------------------------------- camera (R-proj)
 struct Cam {
@@ -200,6 +294,7 @@ struct orc_frame {
   std::vector<uint32_t> scene_dq;   // [H][W] or empty
   std::vector<float> scene_alpha;   // [H][W] or empty
   uint32_t groom_mask = 0xFFFFFFFFu;
+  int payload_mode = 0;  // 0: strand id | segment | t (R7); 1: the paper's payload (R-payload)
 };
 
 namespace {
@@ -297,13 +392,17 @@ inline void hermite(const std::vector<V3>& P, const std::vector<V3>& m, uint32_t
 }
 
 // root barycentrics (R6): fold map on 24-bit integers, so that fp32 and fp64 agree exactly
-void root_bary(const Groom& g, uint32_t id_local, double b[3]) {
-  uint32_t a1 = u24(hash3(g.st.seed, id_local, ST_ROOT1));
-  uint32_t a2 = u24(hash3(g.st.seed, id_local, ST_ROOT2));
+void root_a24(const Groom& g, uint32_t id_local, uint32_t& a1, uint32_t& a2) {
+  a1 = u24(hash3(g.st.seed, id_local, ST_ROOT1));
+  a2 = u24(hash3(g.st.seed, id_local, ST_ROOT2));
   if (a1 + a2 > 16777216u) {
     a1 = 16777216u - a1;
     a2 = 16777216u - a2;
   }
+}
+void root_bary(const Groom& g, uint32_t id_local, double b[3]) {
+  uint32_t a1, a2;
+  root_a24(g, id_local, a1, a2);
   b[1] = double(a1) / 16777216.0;
   b[2] = double(a2) / 16777216.0;
   b[0] = (1.0 - b[1]) - b[2];
@@ -469,6 +568,24 @@ void orc_unpack(uint64_t w, uint32_t out[4]) {
   out[1] = w_sid(w);
   out[2] = w_j(w);
   out[3] = w_t9(w);
+}
+void orc_frame_set_payload_mode(orc_frame* f, int mode) { f->payload_mode = mode ? 1 : 0; }
+void orc_oct_encode(const float T[3], uint32_t out[2]) { oct_encode({T[0], T[1], T[2]}, out[0], out[1]); }
+void orc_oct_decode(uint32_t ox, uint32_t oy, float out[3]) {
+  F3 t = oct_decode(ox, oy);
+  out[0] = t.x, out[1] = t.y, out[2] = t.z;
+}
+uint64_t orc_payload40(const float* v, int j, int C, float t, uint32_t a1, uint32_t a2) {
+  return payload40(v, j, C, t, a1, a2);
+}
+void orc_unpack_payload(uint64_t w, uint32_t out[7]) {
+  out[0] = w_dq(w);
+  out[1] = uint32_t(w >> 32) & 0xFFu;
+  out[2] = uint32_t(w >> 24) & 0xFFu;
+  out[3] = uint32_t(w >> 18) & 63u;
+  out[4] = uint32_t(w >> 12) & 63u;
+  out[5] = uint32_t(w >> 6) & 63u;
+  out[6] = uint32_t(w) & 63u;
 }
 int orc_project(const orc_camera* cam, const float p[3], float out[4]) {
   Cam k = make_cam(cam);
@@ -851,6 +968,7 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
     uint64_t voff;
     uint32_t C, sid;
     float width;
+    uint32_t a1, a2;  // R-payload: the strand's root coordinates (u, v)
   };
   std::vector<S> dir;
   dir.reserve(f->n_strands);
@@ -858,9 +976,12 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
     for (uint32_t q = 0; q < g.Q; ++q)
       for (uint32_t t = 0; t < g.T; ++t) {
         const Entry& e = f->table[g.gid_base + q * g.T + t];
-        for (uint32_t kk = 0; kk < e.nlod; ++kk)
+        for (uint32_t kk = 0; kk < e.nlod; ++kk) {
+          uint32_t a1 = 0, a2 = 0;
+          if (f->payload_mode) root_a24(g, g.off[t] + kk, a1, a2);
           dir.push_back({uint64_t(e.vertex_base) + uint64_t(kk) * e.C, e.C,
-                         g.sid_base + q * g.N + g.off[t] + kk, g.st.width_world});
+                         g.sid_base + q * g.N + g.off[t] + kk, g.st.width_world, a1, a2});
+        }
       }
   for (size_t si = 0; si < dir.size(); ++si) {
     const S& s = dir[order ? order[si] : si];
@@ -901,6 +1022,8 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
           zn = a.zn + zn;
           if (zn < 0.f || zn > 1.f) continue;
           uint64_t w = pack(zn, s.sid, j, t);
+          if (f->payload_mode)  // R-payload: same depth bits, the paper's 40 payload bits
+            w = (uint64_t(quant_depth(zn)) << 40) | payload40(&f->v32[s.voff * 4], int(j), int(s.C), t, s.a1, s.a2);
           uint64_t* px = &f->gbuf[(size_t(y) * k.W + x) * 2];
           ++n_cons;
           px[1] = std::min(px[1], w);  // PAPER.md:85 atomic min, depth in the high bits
@@ -1051,46 +1174,110 @@ int orc_frame_resolve_msaa(orc_frame* f, const orc_camera* cam, const orc_params
 // ------------------------------------------------------------------ O6
 // O6 for one word: the shaded linear RGB of the hit it names (stand-in model, R23). Returns false if the strand
 // id does not resolve.
-static bool shade_word(const orc_frame* f, const Cam& k, const orc_params* prm, uint64_t G, double rgb[3]) {
+// the stand-in shading model (R23) at one point: position, unit tangent, strand parameter w, ambient occlusion
+static void shade_model(const Groom* g, const Cam& k, const orc_params* prm, V3 pos, V3 T, double w, double ao,
+                        double rgb[3]) {
   V3 eye = {double(k.eye[0]), double(k.eye[1]), double(k.eye[2])};
-    Loc l = locate(f, w_sid(G));
-    if (!l.ok) return false;
-    const Groom* g = nullptr;
-    for (const Groom& gg : f->grooms)
-      if (w_sid(G) >= gg.sid_base && w_sid(G) < gg.sid_base + gg.N * gg.Q) g = &gg;
-    int j = int(w_j(G)), C = int(l.C);
-    double t = double(w_t9(G)) / 511.0;
-    auto V = [&](int i) { return vtx(f, l.voff + uint64_t(std::min(std::max(i, 0), C - 1))); };
-    V3 pos = (1 - t) * V(j) + t * V(j + 1);
-    double ao = (1 - t) * double(f->v32[(l.voff + j) * 4 + 3]) + t * double(f->v32[(l.voff + j + 1) * 4 + 3]);
-    // O3 tangents on the styled polyline, interpolated along the segment
-    V3 Tj = calcTangent(j, C, V(j - 1), V(j), V(j + 1));
-    V3 Tj1 = calcTangent(j + 1, C, V(j), V(j + 1), V(j + 2));
-    V3 T = normalize((1 - t) * Tj + t * Tj1);
-    double w = (double(j) + t) / double(C - 1);
-    double alb[3];
-    for (int c = 0; c < 3; ++c)
-      alb[c] = (1 - w) * double(g->st.albedo_root[c]) + w * double(g->st.albedo_tip[c]);
-    V3 Vd = normalize(eye - pos);
-    for (int c = 0; c < 3; ++c) rgb[c] = ao * double(prm->ambient_rgb[c]) * alb[c];
-    double beta = double(g->st.roughness), tilt = double(g->st.tilt);
-    for (uint32_t li = 0; li < prm->n_lights; ++li) {
-      V3 lp = {double(prm->light_pos[li][0]), double(prm->light_pos[li][1]), double(prm->light_pos[li][2])};
-      V3 Lv = lp - pos;
-      double d2 = dot(Lv, Lv);
-      V3 om = (1.0 / std::sqrt(d2)) * Lv;
-      double sin_i = std::min(std::max(dot(T, om), -1.0), 1.0);
-      double sin_o = std::min(std::max(dot(T, Vd), -1.0), 1.0);
-      double cos_i = std::sqrt(std::max(0.0, 1.0 - sin_i * sin_i));
-      double th = 0.5 * (std::asin(sin_i) + std::asin(sin_o));
-      double MR = std::exp(-(th + tilt) * (th + tilt) / (2.0 * beta * beta));
-      double MT = std::exp(-(th - 1.5 * tilt) * (th - 1.5 * tilt) / (8.0 * beta * beta));
-      for (int c = 0; c < 3; ++c) {
-        double E = double(prm->light_rgb[li][c]) / d2;
-        rgb[c] += E * cos_i * (double(prm->k_d) * alb[c] + double(prm->k_R) * MR + double(prm->k_TRT) * MT * alb[c]);
-      }
+  double alb[3];
+  for (int c = 0; c < 3; ++c)
+    alb[c] = (1 - w) * double(g->st.albedo_root[c]) + w * double(g->st.albedo_tip[c]);
+  V3 Vd = normalize(eye - pos);
+  for (int c = 0; c < 3; ++c) rgb[c] = ao * double(prm->ambient_rgb[c]) * alb[c];
+  double beta = double(g->st.roughness), tilt = double(g->st.tilt);
+  for (uint32_t li = 0; li < prm->n_lights; ++li) {
+    V3 lp = {double(prm->light_pos[li][0]), double(prm->light_pos[li][1]), double(prm->light_pos[li][2])};
+    V3 Lv = lp - pos;
+    double d2 = dot(Lv, Lv);
+    V3 om = (1.0 / std::sqrt(d2)) * Lv;
+    double sin_i = std::min(std::max(dot(T, om), -1.0), 1.0);
+    double sin_o = std::min(std::max(dot(T, Vd), -1.0), 1.0);
+    double cos_i = std::sqrt(std::max(0.0, 1.0 - sin_i * sin_i));
+    double th = 0.5 * (std::asin(sin_i) + std::asin(sin_o));
+    double MR = std::exp(-(th + tilt) * (th + tilt) / (2.0 * beta * beta));
+    double MT = std::exp(-(th - 1.5 * tilt) * (th - 1.5 * tilt) / (8.0 * beta * beta));
+    for (int c = 0; c < 3; ++c) {
+      double E = double(prm->light_rgb[li][c]) / d2;
+      rgb[c] += E * cos_i * (double(prm->k_d) * alb[c] + double(prm->k_R) * MR + double(prm->k_TRT) * MT * alb[c]);
     }
+  }
+}
+
+static bool shade_word(const orc_frame* f, const Cam& k, const orc_params* prm, uint64_t G, double rgb[3]) {
+  Loc l = locate(f, w_sid(G));
+  if (!l.ok) return false;
+  const Groom* g = nullptr;
+  for (const Groom& gg : f->grooms)
+    if (w_sid(G) >= gg.sid_base && w_sid(G) < gg.sid_base + gg.N * gg.Q) g = &gg;
+  int j = int(w_j(G)), C = int(l.C);
+  double t = double(w_t9(G)) / 511.0;
+  auto V = [&](int i) { return vtx(f, l.voff + uint64_t(std::min(std::max(i, 0), C - 1))); };
+  V3 pos = (1 - t) * V(j) + t * V(j + 1);
+  double ao = (1 - t) * double(f->v32[(l.voff + j) * 4 + 3]) + t * double(f->v32[(l.voff + j + 1) * 4 + 3]);
+  // O3 tangents on the styled polyline, interpolated along the segment
+  V3 Tj = calcTangent(j, C, V(j - 1), V(j), V(j + 1));
+  V3 Tj1 = calcTangent(j + 1, C, V(j), V(j + 1), V(j + 2));
+  V3 T = normalize((1 - t) * Tj + t * Tj1);
+  double w = (double(j) + t) / double(C - 1);
+  shade_model(g, k, prm, pos, T, w, ao, rgb);
   return true;
+}
+
+// R-payload ("reconstruct it from the depth value ... a specific sample location within the pixel"):
+// the view-space point on the ray through the centre of pixel (x, y) at the word's depth
+static V3 position_from_depth(const Cam& k, int x, int y, uint32_t dq) {
+  double zn = double(dq) / 16777215.0;
+  double zv = double(k.B) / (double(k.A) - zn);
+  double cx = ((double(x) + 0.5) - double(k.half_w)) / double(k.fpx);
+  double cy = (double(k.half_h) - (double(y) + 0.5)) / double(k.fpx);
+  V3 p;
+  p.x = double(k.eye[0]) + zv * (cx * double(k.r[0]) + cy * double(k.u[0]) + double(k.f[0]));
+  p.y = double(k.eye[1]) + zv * (cx * double(k.r[1]) + cy * double(k.u[1]) + double(k.f[1]));
+  p.z = double(k.eye[2]) + zv * (cx * double(k.r[2]) + cy * double(k.u[2]) + double(k.f[2]));
+  return p;
+}
+// O6 from the paper's payload alone: no vertex is read
+static void shade_payload(const Groom* g, const Cam& k, const orc_params* prm, int x, int y, uint64_t G,
+                          double rgb[3]) {
+  F3 Tf = oct_decode(uint32_t(G >> 32) & 0xFFu, uint32_t(G >> 24) & 0xFFu);
+  V3 T = {double(Tf.x), double(Tf.y), double(Tf.z)};
+  double w = double(uint32_t(G >> 6) & 63u) / 63.0, ao = double(uint32_t(G) & 63u) / 63.0;
+  shade_model(g, k, prm, position_from_depth(k, x, y, w_dq(G)), T, w, ao, rgb);
+}
+// R22 for the paper's payload: screen direction of the decoded tangent at the pixel centre. With view-space
+// tangent (tx, ty, tz) and the pixel's ray (cx, cy, 1), d(sx, sy)/ds is parallel to (tx - cx tz, cy tz - ty),
+// whatever the depth. fp32 fixed order (decides the strip membership).
+static void screen_tangent_payload(const Cam& k, int x, int y, uint64_t word, float T[2]) {
+  T[0] = 1.f;
+  T[1] = 0.f;
+  F3 t = oct_decode(uint32_t(word >> 32) & 0xFFu, uint32_t(word >> 24) & 0xFFu);
+  float tx = dot3f(t.x, t.y, t.z, k.r), ty = dot3f(t.x, t.y, t.z, k.u), tz = dot3f(t.x, t.y, t.z, k.f);
+  float cx = float(x) + 0.5f;
+  cx = cx - k.half_w;
+  cx = cx / k.fpx;
+  float cy = float(y) + 0.5f;
+  cy = k.half_h - cy;
+  cy = cy / k.fpx;
+  float a = cx * tz;
+  float Sx = tx - a;
+  float b = cy * tz;
+  float Sy = b - ty;
+  float dd = Sx * Sx;
+  float e = Sy * Sy;
+  dd = dd + e;
+  if (!(dd >= 1e-12f)) return;
+  float len = std::sqrt(dd);
+  T[0] = Sx / len;
+  T[1] = Sy / len;
+}
+// the one groom a payload pass draws (the payload names no groom: the paper shades groom by groom)
+static const Groom* payload_groom(const orc_frame* f) {
+  const Groom* g = nullptr;
+  for (size_t i = 0; i < f->grooms.size(); ++i)
+    if ((f->groom_mask >> i) & 1u) {
+      if (g) return nullptr;
+      g = &f->grooms[i];
+    }
+  return g;
 }
 
 int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) {
@@ -1101,14 +1288,24 @@ int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) 
   f->tang.assign(np * 4, 0.f);
   const int sx0 = std::max(f->wx0 - 7, 0), sx1 = std::min(f->wx1 < (1 << 30) ? f->wx1 + 7 : f->wx1, int(k.W));
   const int sy0 = std::max(f->wy0 - 7, 0), sy1 = std::min(f->wy1 < (1 << 30) ? f->wy1 + 7 : f->wy1, int(k.H));
+  const Groom* pg = f->payload_mode ? payload_groom(f) : nullptr;
   for (int sy = sy0; sy < sy1; ++sy)
   for (int sx = sx0; sx < sx1; ++sx) {
     const size_t p = size_t(sy) * k.W + sx;
     uint64_t G = f->gbuf[p * 2], A = f->gbuf[p * 2 + 1];
+    double rgb[3];
+    if (f->payload_mode) {  // R-payload: everything comes from the word and the pixel position
+      if (!pg) return -4;
+      if (!none(A)) screen_tangent_payload(k, sx, sy, A, &f->tang[p * 4 + 2]);
+      if (none(G)) continue;
+      screen_tangent_payload(k, sx, sy, G, &f->tang[p * 4]);
+      shade_payload(pg, k, prm, sx, sy, G, rgb);
+      for (int c = 0; c < 3; ++c) f->colour[p * 3 + c] = rgb[c];
+      continue;
+    }
     if (!none(A)) screen_tangent(f, k, A, &f->tang[p * 4 + 2]);
     if (none(G)) continue;
     screen_tangent(f, k, G, &f->tang[p * 4]);
-    double rgb[3];
     if (!shade_word(f, k, prm, G, rgb)) return -2;
     for (int c = 0; c < 3; ++c) f->colour[p * 3 + c] = rgb[c];
   }

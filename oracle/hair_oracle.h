@@ -152,6 +152,23 @@ void orc_frame_get_msaa(const orc_frame*, uint64_t* out);
 int orc_frame_set_msaa(orc_frame*, const uint64_t* in, uint32_t k, uint32_t w, uint32_t h);
 int orc_frame_resolve_msaa(orc_frame*, const orc_camera*, const orc_params*);
 
+/* R-payload ("G-buffer compression"): mode 1 makes O4 write the paper's self-contained
+ * word [63:40] dq | [39:32] ox8 | [31:24] oy8 | [23:18] u6 | [17:12] v6 | [11:6] w6 | [5:0] ao6 (octahedral tangent
+ * 2 x uint8; root coordinates u, v, strand parameter w and ambient occlusion 4 x uint6) instead of
+ * strand id | segment | t, and O6 shade from the word alone: position from the depth at the pixel centre
+ * (PAPER.md:90), tangent from the octahedral code, shading parameters from w, AO from the word; the screen tangent
+ * O7 uses is the projected direction of the decoded tangent. The word names no groom, so O6 needs exactly one
+ * groom in the pass mask (the paper shades groom by groom): else orc_frame_shade returns -4.
+ * Mode 0 (default) is the strand-id payload. MSAA mode ignores it. */
+void orc_frame_set_payload_mode(orc_frame*, int mode);
+/* pure functions of the payload, fp32 fixed order (pins): octahedral code of a unit vector / unit vector of a code;
+ * the 40 payload bits of a hit at parameter t on segment j of a strand v[C][4] (x, y, z, ao) with folded 24-bit
+ * root coordinates a1, a2 (R6); fields of a word: dq, ox8, oy8, u6, v6, w6, ao6 */
+void orc_oct_encode(const float T[3], uint32_t out[2]);
+void orc_oct_decode(uint32_t ox, uint32_t oy, float out[3]);
+uint64_t orc_payload40(const float* v, int j, int C, float t, uint32_t a1, uint32_t a2);
+void orc_unpack_payload(uint64_t w, uint32_t out[7]);
+
 /* O6: colour[H][W][3] fp64 (0 where no centre hit); tangents[H][W][4] fp32 = (T_G.xy, T_A.xy) */
 int orc_frame_shade(orc_frame*, const orc_camera*, const orc_params*);
 void orc_frame_get_colour(const orc_frame*, double* rgb);

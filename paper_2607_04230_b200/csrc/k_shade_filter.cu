@@ -151,6 +151,9 @@ __device__ __forceinline__ float2 screen_tangent(const SceneDev* __restrict__ sc
 //    the largest float whose correctly rounded root is <= w_strip; sqrt_rn is monotone).
 #define FT_W 32
 #define FT_H 16
+#ifndef FILT_MIN_BLOCKS
+#define FILT_MIN_BLOCKS 4  // CTAs per SM the register budget is held to
+#endif
 #define DQ_NONE 0x40000000u
 
 __device__ __forceinline__ float fast_ex2(float x) {
@@ -167,7 +170,7 @@ __device__ __forceinline__ bool in_strip_exact(float fdx, float fdy, float Tx, f
 }
 
 template <int R>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, FILT_MIN_BLOCKS)
 k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
          CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, const float4* __restrict__ colour,
          const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
