@@ -42,6 +42,16 @@ extern "C" {
 #define HAIR_FLAG_FILTER 1u       /* run the reconstruction filter; else pass centre colour */
 #define HAIR_FLAG_COUNTERS 2u     /* count predicate-true hits (algorithmic atomics) in hair_stats; slower */
 #define HAIR_FLAG_STAGE_TIMING 4u /* record CUDA events around each stage for hair_stats.ms_* */
+/* The paper's self-contained G-buffer word ("G-buffer compression"; DESIGN.md R-payload) instead of
+ * depth24|strand24|segment7|t9:
+ *   [63:40] depth24 | [39:32] ox8 | [31:24] oy8 | [23:18] u6 | [17:12] v6 | [11:6] w6 | [5:0] ao6
+ * octahedral code of the interpolated calcTangent (2 x uint8), root coordinates u, v, strand parameter w and
+ * ambient occlusion (4 x uint6). Shading then reads no vertex: position from the depth at the pixel centre
+ * (PAPER.md:90), tangent from the code, shading parameters from w; the filter's screen tangent is the projected
+ * decoded tangent. The word names no groom, so exactly ONE groom may be drawn per pass (groom_mask selecting one
+ * groom with hair_render / hair_render_scene, or hair_render_sequential, the paper's groom-by-groom path
+ * PAPER.md:208): otherwise HAIR_E_INVALID_ARG. Not available with hair_render_msaa. */
+#define HAIR_FLAG_PAPER_PAYLOAD 8u
 
 typedef struct hair_ctx hair_ctx; /* opaque; owns all device scratch */
 

@@ -204,7 +204,6 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
   size_t px = (size_t)w * h;
   if (px > c->colour_cap) {
     cudaFree(c->d_colour);
-  cudaFree(c->d_target2);
     c->d_colour = nullptr;
     CK(cudaMalloc((void**)&c->d_colour, px * sizeof(float4)));
     c->colour_cap = px;
@@ -246,6 +245,18 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   const CamDev k = make_cam(cam, w, h);
   ShadeParams sp = make_shade(c->prm);
   sp.bg_alpha = po.bg_alpha ? 1u : 0u;
+  // R-payload: the paper's word names no groom, so a pass draws exactly one
+  const bool pp = (c->prm.flags & HAIR_FLAG_PAPER_PAYLOAD) != 0;
+  sp.paper_payload = pp ? 1u : 0u;
+  sp.pp_groom = 0;
+  if (pp) {
+    if (po.ms_k) return fail(c, HAIR_E_INVALID_ARG, "hair_render_msaa: HAIR_FLAG_PAPER_PAYLOAD is not available in the MSAA reference mode");
+    const uint32_t all = c->scene.n_grooms >= 32 ? 0xFFFFFFFFu : ((1u << c->scene.n_grooms) - 1u);
+    const uint32_t active = po.groom_mask & c->prm.groom_mask & all;
+    if (active == 0 || (active & (active - 1u)))
+      return fail(c, HAIR_E_INVALID_ARG, "HAIR_FLAG_PAPER_PAYLOAD: exactly one groom per pass (groom_mask, or hair_render_sequential)");
+    while (!((active >> sp.pp_groom) & 1u)) ++sp.pp_groom;
+  }
   const bool timed = (c->prm.flags & HAIR_FLAG_STAGE_TIMING) != 0;
   const bool count = (c->prm.flags & HAIR_FLAG_COUNTERS) != 0;
   const uint32_t n_bi = c->scene.n_bi;
@@ -296,7 +307,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   if ((stage_mask & 1u) && n_bi) {
     if (!front) CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER, 0, sizeof(unsigned long long), st));
     launch_raster(c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters,
-                  count && !po.ms_k, po.ms_k, c->n_sm, st);
+                  count && !po.ms_k, po.ms_k, pp, c->n_sm, st);
     ++launches;
   }
   mark(EV_RASTER);
@@ -375,6 +386,7 @@ void hair_destroy(hair_ctx* c) {
   cudaFree(c->d_vertices);
   cudaFree(c->d_srec);
   cudaFree(c->d_colour);
+  cudaFree(c->d_target2);
   cudaFree(c->d_counters);
   if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
   for (int k = 0; k < HAIR_HOST_SLOTS; ++k) {

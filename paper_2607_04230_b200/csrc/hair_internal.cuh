@@ -62,6 +62,8 @@ struct ShadeParams {
   uint32_t tauz_q, taufly_q, filter_on;
   uint32_t bg_alpha;  // R-seq: scene_rgb.w is the alpha accumulated by earlier passes (out.w = a + (1 - a) bg.w)
   float rho_default;  // 0.5 * center_diameter_px
+  uint32_t paper_payload;  // R-payload: words carry the paper's payload; pp_groom = the one groom of the pass
+  uint32_t pp_groom;
 };
 
 // device counters, one block of 64-bit words (index = enum)
@@ -130,6 +132,53 @@ __device__ __forceinline__ uint32_t w_sid(unsigned long long w) { return (uint32
 __device__ __forceinline__ uint32_t w_j(unsigned long long w) { return (uint32_t)(w >> 9) & 0x7Fu; }
 __device__ __forceinline__ uint32_t w_t9(unsigned long long w) { return (uint32_t)w & 0x1FFu; }
 
+// ------------------------------------------------------------------ the paper's payload (DESIGN.md R-payload)
+// [63:40] dq | [39:32] ox8 | [31:24] oy8 | [23:18] u6 | [17:12] v6 | [11:6] w6 | [5:0] ao6. Every
+// code is a decision: fp32, one rounding per operation, in the order DESIGN.md states.
+struct X3 {
+  float x, y, z;
+};
+__device__ __forceinline__ X3 unit3x(float x, float y, float z) {
+  const float dd = xadd(xadd(xmul(x, x), xmul(y, y)), xmul(z, z));
+  if (!(dd > 0.f)) return {1.f, 0.f, 0.f};
+  const float len = xsqrt(dd);
+  return {xdiv(x, len), xdiv(y, len), xdiv(z, len)};
+}
+// calcTangent on fp32 vertices
+__device__ __forceinline__ X3 tangent_x(uint32_t idx, uint32_t count, float4 prev, float4 curr, float4 next) {
+  const float4 a = idx + 1 == count ? curr : next;
+  const float4 b = idx == 0 ? curr : prev;
+  return unit3x(xsub(a.x, b.x), xsub(a.y, b.y), xsub(a.z, b.z));
+}
+__device__ __forceinline__ uint32_t q8s(float p) {
+  return min((uint32_t)xadd(xmul(xadd(xmul(p, 0.5f), 0.5f), 255.f), 0.5f), 255u);
+}
+__device__ __forceinline__ uint32_t q6(float v) { return min((uint32_t)xadd(xmul(v, 63.f), 0.5f), 63u); }
+__device__ __forceinline__ uint32_t uv6(uint32_t a24) { return (a24 * 63u + (1u << 23)) >> 24; }
+__device__ __forceinline__ uint32_t oct_encode_x(X3 T) {  // (ox8 << 8) | oy8
+  const float s = xadd(xadd(fabsf(T.x), fabsf(T.y)), fabsf(T.z));
+  float px = xdiv(T.x, s), py = xdiv(T.y, s);
+  if (T.z < 0.f) {
+    const float ax = xsub(1.f, fabsf(py)), ay = xsub(1.f, fabsf(px));
+    px = px >= 0.f ? ax : -ax;
+    py = py >= 0.f ? ay : -ay;
+  }
+  return (q8s(px) << 8) | q8s(py);
+}
+__device__ __forceinline__ X3 oct_decode_x(uint32_t ox, uint32_t oy) {
+  const float px = xsub(xmul(xdiv((float)ox, 255.f), 2.f), 1.f), py = xsub(xmul(xdiv((float)oy, 255.f), 2.f), 1.f);
+  const float z = xsub(xsub(1.f, fabsf(px)), fabsf(py));
+  float tx = px, ty = py;
+  if (z < 0.f) {
+    const float ax = xsub(1.f, fabsf(py)), ay = xsub(1.f, fabsf(px));
+    tx = px >= 0.f ? ax : -ax;
+    ty = py >= 0.f ? ay : -ay;
+  }
+  return unit3x(tx, ty, z);
+}
+__device__ __forceinline__ uint32_t pw_ox(unsigned long long w) { return (uint32_t)(w >> 32) & 0xFFu; }
+__device__ __forceinline__ uint32_t pw_oy(unsigned long long w) { return (uint32_t)(w >> 24) & 0xFFu; }
+
 // R26 hash
 __device__ __forceinline__ uint32_t pcg(uint32_t v) {
   uint32_t s = v * 747796405u + 2891336453u;
@@ -161,7 +210,8 @@ void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_
 void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
-                   unsigned long long* counters, bool count, uint32_t ms_k, int n_sm, cudaStream_t st);
+                   unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int n_sm,
+                   cudaStream_t st);
 void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
                          float4* out, cudaStream_t st);

@@ -22,7 +22,8 @@
 #ifndef RAS_MIN_BLOCKS
 #define RAS_MIN_BLOCKS 5  // CTAs per SM the register budget is held to (40 of 64 warps)
 #endif
-#define REC_STRIDE 20  // floats per segment record (16 used); 20 mod 32 keeps LDS.128 conflict-free
+#define REC_STRIDE 20  // floats per segment record (18 used); 20 mod 32 keeps LDS.128 conflict-free
+#define REC_STRIDE_PP 28  // paper payload: + tangents at both ends (6), AO at both ends (2), (u6, v6) bits, C
 #define ENUM_EPS 0.015625f  // slack on the minor-axis range of a column: the enumeration must be a superset
 #ifndef ROW_BATCH
 #define ROW_BATCH 2
@@ -50,14 +51,19 @@ __constant__ int c_ms_off[4][8][2] = {  // sample offsets from the pixel centre 
     {{-2, -6}, {6, -2}, {-6, 2}, {2, 6}},
     {{1, -3}, {-1, 3}, {5, 1}, {-3, -5}, {-5, 5}, {-7, -1}, {3, 7}, {7, -7}}};
 
-template <bool COUNT, bool MS>
+// Paper payload (PP = true; DESIGN.md R-payload): same tasks and tests; the projecting lane also
+// computes calcTangent of its vertex (neighbours by shuffle, one extra load at each end of the chunk) and the
+// strand's root codes, the record carries both ends' tangent and AO, and a hit whose depth does not lose builds the
+// 40 payload bits (interpolated tangent -> octahedral code, w, AO) in fixed-order fp32 instead of sid | j | t.
+template <bool COUNT, bool MS, bool PP>
 __global__ void __launch_bounds__(RAS_WARPS * 32, RAS_MIN_BLOCKS)
 k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
          const uint32_t* __restrict__ grp, const float4* __restrict__ vertices, CamDev cam, float rho_default,
          unsigned long long* __restrict__ gbuf, unsigned long long* __restrict__ counters, uint32_t ms_k) {
-  __shared__ __align__(16) float s_rec[RAS_WARPS][32][REC_STRIDE];
+  constexpr int RS = PP ? REC_STRIDE_PP : REC_STRIDE;
+  __shared__ __align__(16) float s_rec[RAS_WARPS][32][RS];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  float(*rec)[REC_STRIDE] = s_rec[warp];
+  float(*rec)[RS] = s_rec[warp];
   uint32_t c_center = 0, c_cons = 0, c_drawn = 0, c_issued = 0, c_live = 0;
   const int W = (int)cam.W, H = (int)cam.H;
   const uint32_t le_mask = 0xFFFFFFFFu >> (31 - lane);
@@ -87,7 +93,8 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
     const GroomDev& g = sc->g[gi];
     const uint32_t rel = gid - g.gid_base;
     const uint32_t q = rel / g.T, t = rel - q * g.T;
-    const uint32_t sid0 = g.sid_base + q * g.N + __ldg(&g.off[t]);
+    const uint32_t off_t = __ldg(&g.off[t]);
+    const uint32_t sid0 = g.sid_base + q * g.N + off_t;
     const float width = g.width_world;
     const uint32_t n_v = nlod * C;
     const float4* vin = vertices + e.w;
@@ -112,6 +119,33 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
       b.valid = __shfl_down_sync(0xffffffffu, (int)a.valid, 1) != 0;
       const uint32_t k = v / C, j = v - k * C;
       const bool seg = lane < 31 && v < v_end && j + 1 < C && a.valid && b.valid;  // R12
+      if (PP) {  // R-payload: tangent of this vertex, exchanged with the neighbour; AO; the strand's root codes
+        float4 pp, pn;
+        pp.x = __shfl_up_sync(0xffffffffu, p.x, 1), pp.y = __shfl_up_sync(0xffffffffu, p.y, 1), pp.z = __shfl_up_sync(0xffffffffu, p.z, 1);
+        pn.x = __shfl_down_sync(0xffffffffu, p.x, 1), pn.y = __shfl_down_sync(0xffffffffu, p.y, 1), pn.z = __shfl_down_sync(0xffffffffu, p.z, 1);
+        pp.w = pn.w = 0.f;
+        X3 Tv = {1.f, 0.f, 0.f};
+        if (v < n_v) {
+          if (lane == 0 && j > 0) pp = __ldg(&vin[v - 1]);
+          if (lane == 31 && j + 1 < C) pn = __ldg(&vin[v + 1]);
+          Tv = tangent_x(j, C, pp, p, pn);
+        }
+        const float t1x = __shfl_down_sync(0xffffffffu, Tv.x, 1), t1y = __shfl_down_sync(0xffffffffu, Tv.y, 1),
+                    t1z = __shfl_down_sync(0xffffffffu, Tv.z, 1), ao1 = __shfl_down_sync(0xffffffffu, p.w, 1);
+        if (seg) {
+          const uint32_t base = pcg(g.seed_h + off_t + k);
+          uint32_t a1 = pcg(base + 1u) >> 8, a2 = pcg(base + 2u) >> 8;
+          if (a1 + a2 > 16777216u) {  // R6
+            a1 = 16777216u - a1;
+            a2 = 16777216u - a2;
+          }
+          float* rp = rec[lane];
+          rp[18] = Tv.x, rp[19] = Tv.y, rp[20] = Tv.z, rp[21] = t1x, rp[22] = t1y, rp[23] = t1z;
+          rp[24] = p.w, rp[25] = ao1;
+          rp[26] = __uint_as_float((uv6(a1) << 18) | (uv6(a2) << 12));
+          rp[27] = __uint_as_float(C);
+        }
+      }
       // ---- segment record in (major, minor) coordinates; every formula below is symmetric in x/y
       uint32_t n_steps = 0;
       if (seg) {
@@ -241,7 +275,24 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
             if (zn < 0.f || zn > 1.f) continue;
             const float eM = xsub(cM, xadd(aM, xmul(tt, dM))), eN = xsub(cN, xadd(aN, xmul(tt, dN)));
             const bool centre = xadd(xmul(eM, eM), xmul(eN, eN)) <= rec[s][17];
-            const unsigned long long word = pack_word(zn, (key >> 7) & 0xFFFFFFu, key & 0x7Fu, tt);
+            unsigned long long word;
+            if (PP) {
+              const uint32_t dq = quant_depth(zn);
+              word = HAIR_EMPTY;
+              // the payload only matters where the depth does not lose outright
+              if (COUNT || dq <= (uint32_t)(cur[i].y >> 40) || (centre && dq <= (uint32_t)(cur[i].x >> 40))) {
+                const float* rp = rec[s];
+                const float omt = xsub(1.f, tt);
+                const X3 T = unit3x(xadd(xmul(omt, rp[18]), xmul(tt, rp[21])), xadd(xmul(omt, rp[19]), xmul(tt, rp[22])),
+                                    xadd(xmul(omt, rp[20]), xmul(tt, rp[23])));
+                const uint32_t oct = oct_encode_x(T);
+                const float w = xdiv(xadd((float)(key & 0x7Fu), tt), (float)(__float_as_uint(rp[27]) - 1u));
+                const float ao = fminf(fmaxf(xadd(xmul(omt, rp[24]), xmul(tt, rp[25])), 0.f), 1.f);
+                const uint32_t lo = ((oct & 0xFFu) << 24) | __float_as_uint(rp[26]) | (q6(w) << 6) | q6(ao);
+                word = ((unsigned long long)((dq << 8) | (oct >> 8)) << 32) | lo;
+              }
+            } else
+              word = pack_word(zn, (key >> 7) & 0xFFFFFFu, key & 0x7Fu, tt);
             unsigned long long* px = pcol + (size_t)r * pstep;
             if (COUNT) {
               ++c_cons;
@@ -318,7 +369,7 @@ void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_
   k_clear<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels, scene_zn);
 }
 
-template <bool COUNT, bool MS>
+template <bool COUNT, bool MS, bool PP>
 static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                             const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                             unsigned long long* counters, uint32_t ms_k, int n_sm, cudaStream_t st) {
@@ -326,20 +377,23 @@ static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4*
   static int per_sm = 0;
   if (!per_sm) {
     int b = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<COUNT, MS>, RAS_WARPS * 32, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<COUNT, MS, PP>, RAS_WARPS * 32, 0);
     per_sm = b > 0 ? b : 1;
   }
-  k_raster<COUNT, MS><<<(uint32_t)(n_sm * per_sm), RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, grp, vertices, cam,
-                                                                             rho_default, gbuf, counters, ms_k);
+  k_raster<COUNT, MS, PP><<<(uint32_t)(n_sm * per_sm), RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, grp, vertices,
+                                                                                 cam, rho_default, gbuf, counters, ms_k);
 }
 
 // ms_k = 0: the two-layer G-buffer; ms_k in {1, 2, 4, 8}: gbuf = [ms_k][H][W] sample layers (reference mode)
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
-                   unsigned long long* counters, bool count, uint32_t ms_k, int n_sm, cudaStream_t st) {
-  if (ms_k) launch_raster_t<false, true>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, ms_k, n_sm, st);
-  else if (count) launch_raster_t<true, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
-  else launch_raster_t<false, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
+                   unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int n_sm,
+                   cudaStream_t st) {
+  if (ms_k) launch_raster_t<false, true, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, ms_k, n_sm, st);
+  else if (paper_payload && count) launch_raster_t<true, false, true>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
+  else if (paper_payload) launch_raster_t<false, false, true>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
+  else if (count) launch_raster_t<true, false, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
+  else launch_raster_t<false, false, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
 }
 
 // ------------------------------------------------------------------ L2-atomic roofline micro-kernels

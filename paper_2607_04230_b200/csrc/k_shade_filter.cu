@@ -30,23 +30,9 @@ __device__ __forceinline__ F3 calc_tangent(int idx, int count, F3 prev, F3 curr,
   else return normalize(next - prev);
 }
 
-// O6 for one word: linear RGB of the hit it names (stand-in model, R23)
-__device__ __forceinline__ F3 shade_word(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec,
-                                         const float4* __restrict__ vertices, const CamDev& cam, const ShadeParams& sp,
-                                         unsigned long long G) {
-  const Loc l = locate_strand(srec, w_sid(G));
-  const GroomDev& g = sc->g[l.groom];
-  const int j = (int)w_j(G), C = (int)l.C;
-  const float t = (float)w_t9(G) * (1.0f / 511.0f);
-  const float4* vs = vertices + l.voff;
-  const float4 v1 = __ldg(&vs[j]), v2 = __ldg(&vs[j + 1]);
-  const float4 v0 = __ldg(&vs[max(j - 1, 0)]), v3 = __ldg(&vs[min(j + 2, C - 1)]);
-  const F3 pos = (1.f - t) * f3(v1) + t * f3(v2);
-  const float ao = (1.f - t) * v1.w + t * v2.w;
-  const F3 Tj = calc_tangent(j, C, f3(v0), f3(v1), f3(v2));
-  const F3 Tj1 = calc_tangent(j + 1, C, f3(v1), f3(v2), f3(v3));
-  const F3 T = normalize((1.f - t) * Tj + t * Tj1);
-  const float w = ((float)j + t) / (float)(C - 1);
+// the stand-in shading model (R23) at one point: position, unit tangent, strand parameter w, AO
+__device__ __forceinline__ F3 shade_model(const GroomDev& g, const CamDev& cam, const ShadeParams& sp, F3 pos, F3 T,
+                                          float w, float ao) {
   const F3 alb = (1.f - w) * f3(g.albedo_root[0], g.albedo_root[1], g.albedo_root[2]) +
                  w * f3(g.albedo_tip[0], g.albedo_tip[1], g.albedo_tip[2]);
   const F3 V = normalize(f3(cam.eye[0], cam.eye[1], cam.eye[2]) - pos);
@@ -73,6 +59,41 @@ __device__ __forceinline__ F3 shade_word(const SceneDev* __restrict__ sc, const 
   return rgb;
 }
 
+// O6 for one word: linear RGB of the hit it names
+__device__ __forceinline__ F3 shade_word(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec,
+                                         const float4* __restrict__ vertices, const CamDev& cam, const ShadeParams& sp,
+                                         unsigned long long G) {
+  const Loc l = locate_strand(srec, w_sid(G));
+  const GroomDev& g = sc->g[l.groom];
+  const int j = (int)w_j(G), C = (int)l.C;
+  const float t = (float)w_t9(G) * (1.0f / 511.0f);
+  const float4* vs = vertices + l.voff;
+  const float4 v1 = __ldg(&vs[j]), v2 = __ldg(&vs[j + 1]);
+  const float4 v0 = __ldg(&vs[max(j - 1, 0)]), v3 = __ldg(&vs[min(j + 2, C - 1)]);
+  const F3 pos = (1.f - t) * f3(v1) + t * f3(v2);
+  const float ao = (1.f - t) * v1.w + t * v2.w;
+  const F3 Tj = calc_tangent(j, C, f3(v0), f3(v1), f3(v2));
+  const F3 Tj1 = calc_tangent(j + 1, C, f3(v1), f3(v2), f3(v3));
+  const F3 T = normalize((1.f - t) * Tj + t * Tj1);
+  const float w = ((float)j + t) / (float)(C - 1);
+  return shade_model(g, cam, sp, pos, T, w, ao);
+}
+
+// R-payload: O6 from the paper's payload alone, no vertex read. Position = the point of the
+// ray through the pixel centre at the word's depth ("reconstruct it from the depth value")
+__device__ __forceinline__ F3 shade_payload(const SceneDev* __restrict__ sc, const CamDev& cam, const ShadeParams& sp,
+                                            int x, int y, unsigned long long G) {
+  const X3 t = oct_decode_x(pw_ox(G), pw_oy(G));
+  const float w = (float)((uint32_t)(G >> 6) & 63u) * (1.0f / 63.0f), ao = (float)((uint32_t)G & 63u) * (1.0f / 63.0f);
+  const float zn = (float)w_dq(G) / 16777215.0f;
+  const float zv = cam.B / (cam.A - zn);
+  const float cx = (((float)x + 0.5f) - cam.half_w) / cam.fpx, cy = (cam.half_h - ((float)y + 0.5f)) / cam.fpx;
+  const F3 pos = f3(cam.eye[0] + zv * (cx * cam.r[0] + cy * cam.u[0] + cam.f[0]),
+                    cam.eye[1] + zv * (cx * cam.r[1] + cy * cam.u[1] + cam.f[1]),
+                    cam.eye[2] + zv * (cx * cam.r[2] + cy * cam.u[2] + cam.f[2]));
+  return shade_model(sc->g[sp.pp_groom], cam, sp, pos, f3(t.x, t.y, t.z), w, ao);
+}
+
 __global__ void __launch_bounds__(256)
 k_shade(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
         CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, float4* __restrict__ colour) {
@@ -83,6 +104,19 @@ k_shade(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const f
   const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
   if (w_none(G)) return;  // colour is only ever read where a centre hit exists
   const F3 rgb = shade_word(sc, srec, vertices, cam, sp, G);
+  colour[p] = make_float4(rgb.x, rgb.y, rgb.z, 1.0f);
+}
+
+__global__ void __launch_bounds__(256)
+k_shade_payload(const SceneDev* __restrict__ sc, CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf,
+                float4* __restrict__ colour) {
+  const uint32_t x = blockIdx.x * 64u + (threadIdx.x & 63u), y = blockIdx.y * 4u + (threadIdx.x >> 6);
+  if (x >= cam.W || y >= cam.H) return;
+  const size_t p = (size_t)y * cam.W + x;
+  const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
+  const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
+  if (w_none(G)) return;
+  const F3 rgb = shade_payload(sc, cam, sp, (int)x, (int)y, G);
   colour[p] = make_float4(rgb.x, rgb.y, rgb.z, 1.0f);
 }
 
@@ -129,6 +163,20 @@ __device__ __forceinline__ float2 screen_tangent(const SceneDev* __restrict__ sc
   if (!(dd >= 1e-12f)) return make_float2(1.f, 0.f);
   const float len = xsqrt(dd);
   return make_float2(xdiv(dx, len), xdiv(dy, len));
+}
+
+// R22 for the paper's payload: screen direction of the decoded tangent at the pixel centre. View-space tangent
+// (tx, ty, tz), pixel ray (cx, cy, 1): d(sx, sy)/ds is parallel to (tx - cx tz, cy tz - ty) whatever the depth
+__device__ __forceinline__ float2 screen_tangent_payload(const CamDev& cam, int x, int y, unsigned long long word) {
+  const X3 t = oct_decode_x(pw_ox(word), pw_oy(word));
+  const float tx = xdot3(t.x, t.y, t.z, cam.r), ty = xdot3(t.x, t.y, t.z, cam.u), tz = xdot3(t.x, t.y, t.z, cam.f);
+  const float cx = xdiv(xsub(xadd((float)x, 0.5f), cam.half_w), cam.fpx);
+  const float cy = xdiv(xsub(cam.half_h, xadd((float)y, 0.5f)), cam.fpx);
+  const float Sx = xsub(tx, xmul(cx, tz)), Sy = xsub(xmul(cy, tz), ty);
+  const float dd = xadd(xmul(Sx, Sx), xmul(Sy, Sy));
+  if (!(dd >= 1e-12f)) return make_float2(1.f, 0.f);
+  const float len = xsqrt(dd);
+  return make_float2(xdiv(Sx, len), xdiv(Sy, len));
 }
 
 // ---------------------------------------------------------------------------------------- H7
@@ -248,11 +296,14 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     const bool isCenter = !w_none(G[k]), isCons = !w_none(A[k]);
     Tc[k] = Ta[k] = make_float2(1.f, 0.f);
     if (isCenter) {
-      Tc[k] = screen_tangent(sc, srec, vertices, cam, G[k]);
+      Tc[k] = sp.paper_payload ? screen_tangent_payload(cam, x0 + lx, y0 + ly + 8 * k, G[k])
+                               : screen_tangent(sc, srec, vertices, cam, G[k]);
       fly[k] = isCons && w_dq(G[k]) >= w_dq(A[k]) && w_dq(G[k]) - w_dq(A[k]) >= sp.taufly_q;  // PAPER.md:175, R21
     }
     const bool isA = fly[k] || (isCons && !isCenter);  // fly-away strand, or promoted pixel: w_color = 1
-    if (isA) Ta[k] = screen_tangent(sc, srec, vertices, cam, A[k]);
+    if (isA)
+      Ta[k] = sp.paper_payload ? screen_tangent_payload(cam, x0 + lx, y0 + ly + 8 * k, A[k])
+                               : screen_tangent(sc, srec, vertices, cam, A[k]);
     bal[2 * k] = __ballot_sync(0xffffffffu, isCenter);
     bal[2 * k + 1] = __ballot_sync(0xffffffffu, isA);
   }
@@ -419,6 +470,10 @@ k_count_pixels(const unsigned long long* __restrict__ gbuf, size_t n_px, unsigne
 void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                   ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st) {
   size_t n = (size_t)cam.W * cam.H;
+  if (sp.paper_payload) {
+    k_shade_payload<<<dim3((cam.W + 63) / 64, (cam.H + 3) / 4), 256, 0, st>>>(d_scene, cam, sp, gbuf, colour);
+    return;
+  }
   k_shade<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour);
 }
 

@@ -58,10 +58,13 @@ def psnr(a, b, peak):
     return 200.0 if mse == 0 else 10.0 * math.log10(peak * peak / mse)
 
 
-def check_stagewise(orc, sc, G, lam=None):
-    """Runs every stage-wise gate; returns a small report."""
+def check_stagewise(orc, sc, G, lam=None, payload=False, groom_mask=None):
+    """Runs every stage-wise gate; returns a small report. payload: the paper's word (R-payload) on both sides."""
     cam, prm = sc["camera"], G["prm"]
     f = orc.Frame(sc["grooms"])
+    f.set_payload_mode(payload)
+    if groom_mask is not None:
+        f.set_pass(groom_mask)
     f.lod(cam, sc["lam"] if lam is None else lam)
     t_or, _ = f.table()
     assert np.array_equal(t_or, G["table"]), "bundle table differs"
@@ -401,11 +404,14 @@ def test_render_into_scene_stagewise(orc, hair_mod, filter_on):
     assert torch.equal(gb2, gb0) and torch.equal(rgb2, rgb0)
 
 
-def test_groom_mask_and_sequential_passes(orc, hair_mod):
+@pytest.mark.parametrize("payload", [False, True])
+def test_groom_mask_and_sequential_passes(orc, hair_mod, payload):
     """hair_render_sequential (R-seq) against the oracle's sequential passes, pass by pass on the
-    GPU's own vertices (groom_mask renders give them), five overlapping grooms, a scene behind them."""
+    GPU's own vertices (groom_mask renders give them), five overlapping grooms, a scene behind them.
+    payload = True: with the paper's word (R-payload) — the paper's own pipeline, groom by groom."""
     import torch
     b = hair_mod
+    fl = b.FLAG_PAPER_PAYLOAD if payload else 0
     sc = synth.config(4, scale=0.03, res_scale=0.2)
     # pull the grooms together so that they overlap on screen (config 4 spreads them over the frame)
     cam, lam, prm = sc["camera"], list(sc["lam"]), dict(sc["params"])
@@ -427,8 +433,9 @@ def test_groom_mask_and_sequential_passes(orc, hair_mod):
     # (i) masked frames: exactly the frame of that groom alone (table, vertices), ids stay global
     verts, tables = [], []
     f = orc.Frame(sc["grooms"])
+    f.set_payload_mode(payload)
     for g in range(n):
-        h.set_render_params(dict(prm, groom_mask=1 << g))
+        h.set_render_params(dict(prm, groom_mask=1 << g), flags=fl)
         gb, rgb = h.render(cam, lam)
         nv = h.stats()["n_vertices"]
         verts.append(h.debug_vertices().cpu().numpy()[:nv].copy())
@@ -440,7 +447,9 @@ def test_groom_mask_and_sequential_passes(orc, hair_mod):
         sid = (b.gbuffer_to_numpy(gb)[..., 1] >> np.uint64(16)) & np.uint64(0xFFFFFF)
         hitm = (b.gbuffer_to_numpy(gb)[..., 1] & np.uint64((1 << 40) - 1)) != np.uint64((1 << 40) - 1)
         lo = sum(int(x["strands_per_tri"].sum()) for x in sc["grooms"][:g])
-        assert hitm.any() and sid[hitm].min() >= lo and sid[hitm].max() < lo + int(sc["grooms"][g]["strands_per_tri"].sum())
+        assert hitm.any()
+        if not payload:
+            assert sid[hitm].min() >= lo and sid[hitm].max() < lo + int(sc["grooms"][g]["strands_per_tri"].sum())
     # (ii) the oracle's sequential passes on those vertices
     target = srgb[..., :3].copy()
     alpha = np.zeros((H, W), np.float32)
@@ -459,7 +468,7 @@ def test_groom_mask_and_sequential_passes(orc, hair_mod):
         dq = (g_or[..., 0] >> np.uint64(40)).astype(np.uint32)
         target, alpha = out[..., :3].astype(np.float32), out[..., 3].astype(np.float32)
     # (iii) the library's sequential frame
-    h.set_render_params(prm)
+    h.set_render_params(prm, flags=fl)
     gb, rgb = h.render_sequential(cam, lam, zn_d, srgb_d)
     G = b.gbuffer_to_numpy(gb)
     assert np.array_equal(G, g_or), float((G == g_or).mean())
@@ -468,12 +477,70 @@ def test_groom_mask_and_sequential_passes(orc, hair_mod):
     assert psnr(out[..., :3], got[..., :3], max(float(out[..., :3].max()), 1.0)) > MIN_PSNR
     assert np.array_equal(got[:, : W // 6, :3], srgb[:, : W // 6, :3].astype(np.float64)) or (zn[:, : W // 6] == 0.5).all()
     # it differs from the one-resolve frame where grooms overlap, and equals it for a single groom
-    one = h.render_scene(cam, lam, zn_d, srgb_d)
-    assert (one[1] - rgb).abs().max().item() > 1e-2
-    h.set_render_params(dict(prm, groom_mask=0b100))
+    if not payload:
+        one = h.render_scene(cam, lam, zn_d, srgb_d)
+        assert (one[1] - rgb).abs().max().item() > 1e-2
+    h.set_render_params(dict(prm, groom_mask=0b100), flags=fl)
     a1 = h.render_sequential(cam, lam, zn_d, srgb_d)
     a2 = h.render_scene(cam, lam, zn_d, srgb_d)
     assert torch.equal(a1[0], a2[0]) and torch.equal(a1[1], a2[1])
+
+
+@pytest.mark.parametrize("idx,scale,res_scale,lam,groom", [
+    (1, 1.0, 1.0, None, None),     # tiny config as named
+    (2, 0.1, 0.5, None, None),     # curl + frizz + width_world: tangents turn inside a segment
+    (3, 0.03, 0.25, None, None),   # twist + clump under LOD
+    (5, 0.01, 0.2, None, None),    # 64 instances, far field
+    (4, 0.03, 0.25, None, 3),      # one groom of the five-groom scene by mask (AO on, curl + frizz)
+])
+def test_paper_payload_stagewise(orc, hair_mod, idx, scale, res_scale, lam, groom):
+    """SURVEY 8f NEXT-1 (DESIGN.md R-payload): the paper's self-contained word. Same gates as the
+    strand-id word: table bit-exact, vertices <= 1e-5, WORDS BIT-EXACT on the same vertex buffer (every code is a
+    fixed-order fp32 decision on both sides), RGB <= 2e-3 from the same G-buffer (shading reads no vertex)."""
+    b = hair_mod
+    sc = synth.config(idx, scale=scale, res_scale=res_scale)
+    over = None if groom is None else dict(groom_mask=1 << groom)
+    G = gpu_frame(b, sc, lam=lam, flags=b.FLAG_PAPER_PAYLOAD, prm_over=over)
+    rep = check_stagewise(orc, sc, G, lam=lam, payload=True, groom_mask=None if groom is None else 1 << groom)
+    assert rep["exact_frac"] == 1.0, rep
+    assert rep["n_hit"] > 500
+    # depth bits are those of the strand-id frame (the min is depth-major), payload bits are not
+    G0 = gpu_frame(b, sc, lam=lam, prm_over=over)
+    assert np.array_equal(G0["gb"] >> np.uint64(40), G["gb"] >> np.uint64(40))
+    assert (G0["gb"] != G["gb"]).any()
+
+
+def test_sequential_as_first_render_of_a_context(hair_mod):
+    """Regression: the first frame of a context may be a sequential one (its second target must survive the
+    allocation of the per-resolution scratch)."""
+    import torch
+    b = hair_mod
+    sc = synth.config(4, scale=0.005, res_scale=0.1)
+    h = b.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(sc["params"])
+    a = h.render_sequential(sc["camera"], sc["lam"])
+    torch.cuda.synchronize()
+    a2 = h.render_sequential(sc["camera"], sc["lam"])
+    assert torch.equal(a[0], a2[0]) and torch.equal(a[1], a2[1])
+
+
+def test_paper_payload_needs_one_groom_per_pass(hair_mod):
+    b = hair_mod
+    sc = synth.config(4, scale=0.005, res_scale=0.1)
+    h = b.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(sc["params"], flags=b.FLAG_PAPER_PAYLOAD)
+    with pytest.raises(RuntimeError):
+        h.render(sc["camera"], sc["lam"])          # five grooms in one resolve: the word names no groom
+    with pytest.raises(RuntimeError):
+        h.render_msaa(sc["camera"], sc["lam"], 2)  # reference mode keeps the strand-id word
+    h.set_render_params(dict(sc["params"], groom_mask=0b10), flags=b.FLAG_PAPER_PAYLOAD)
+    h.render(sc["camera"], sc["lam"])
+    h.set_render_params(sc["params"], flags=b.FLAG_PAPER_PAYLOAD)
+    h.render_sequential(sc["camera"], sc["lam"])   # the paper's groom-by-groom path takes all five
 
 
 @pytest.mark.parametrize("k", [1, 2, 4, 8])
