@@ -377,23 +377,52 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
         Wsum += w;
       }
     }
-    // ---- loop B: strip hit counts by Q's class (R18)
+    // ---- loop B: strip hit counts by Q's class (R18), in (major, minor) coordinates of the tangent: Eq. 9 is
+    // symmetric in x / y and IEEE add / mul commute, so the bits are those of the oracle's x / y order
     const bool xmaj = fabsf(Tx) >= fabsf(Ty);
-    const float slope = xmaj ? Ty / Tx : Tx / Ty;  // |slope| <= 1; T is a unit vector, so the major part is >= 0.707
+    const float TM = xmaj ? Tx : Ty, TN = xmaj ? Ty : Tx;
+    const int strM = xmaj ? 1 : SW, strN = xmaj ? SW : 1;
+    const float slope = TN / TM;  // |slope| <= 1; T is a unit vector, so the major part is >= 0.707
     uint32_t Hc = 0, Ha = 0;
-#pragma unroll 1
-    for (int s = -R; s <= R; ++s) {
-      const float ystar = (float)s * slope;
-      const int m0 = max((int)ceilf(ystar - sp.strip_hmax), -R);
-      for (int c = 0; c < sp.strip_nc; ++c) {
-        const int mm = m0 + c;
-        const int dx = xmaj ? s : mm, dy = xmaj ? mm : s;
-        if (mm <= R) {
-          const int idx = ci + dy * SW + dx;
-          const bool cG = s_dqG[idx] - lo <= tau2, cA = s_dqA[idx] - lo <= tau2;
-          const bool in = in_strip_exact((float)dx, (float)dy, Tx, Ty, sp.strip_e2_max);
+    if (sp.strip_nc == 2) {  // w_strip = 0.5: two candidate minor offsets per major step, all unrolled
+#pragma unroll
+      for (int s = -R; s <= R; ++s) {
+        const float fM = (float)s;
+        const int m0 = max((int)ceilf(fM * slope - sp.strip_hmax), -R);  // <= R: |s slope| <= R, strip_hmax > 0
+        const float pM = xmul(fM, TM);
+        const int idx0 = ci + s * strM + m0 * strN;
+        const bool two = m0 < R;  // m0 + 1 is still a window tap (else its read is clamped and its hit masked)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          const float fN = (float)(m0 + c);
+          const float dpar = xadd(pM, xmul(fN, TN));
+          const float eM = xsub(fM, xmul(dpar, TM)), eN = xsub(fN, xmul(dpar, TN));
+          bool in = xadd(xmul(eM, eM), xmul(eN, eN)) <= sp.strip_e2_max;
+          if (c) in = in && two;
+          const int idc = c ? (two ? idx0 + strN : idx0) : idx0;
+          const bool cG = s_dqG[idc] - lo <= tau2, cA = s_dqA[idc] - lo <= tau2;
           Hc += (in && cG) ? 1u : 0u;
           Ha += (in && cA && !cG) ? 1u : 0u;
+        }
+      }
+    } else {
+#pragma unroll 1
+      for (int s = -R; s <= R; ++s) {
+        const float fM = (float)s;
+        const int m0 = max((int)ceilf(fM * slope - sp.strip_hmax), -R);
+        const float pM = xmul(fM, TM);
+        for (int c = 0; c < sp.strip_nc; ++c) {
+          const int mm = m0 + c;
+          if (mm <= R) {
+            const float fN = (float)mm;
+            const float dpar = xadd(pM, xmul(fN, TN));
+            const float eM = xsub(fM, xmul(dpar, TM)), eN = xsub(fN, xmul(dpar, TN));
+            const bool in = xadd(xmul(eM, eM), xmul(eN, eN)) <= sp.strip_e2_max;
+            const int idx = ci + s * strM + mm * strN;
+            const bool cG = s_dqG[idx] - lo <= tau2, cA = s_dqA[idx] - lo <= tau2;
+            Hc += (in && cG) ? 1u : 0u;
+            Ha += (in && cA && !cG) ? 1u : 0u;
+          }
         }
       }
     }
