@@ -52,6 +52,10 @@ extern "C" {
  * groom with hair_render / hair_render_scene, or hair_render_sequential, the paper's groom-by-groom path
  * PAPER.md:208): otherwise HAIR_E_INVALID_ARG. Not available with hair_render_msaa. */
 #define HAIR_FLAG_PAPER_PAYLOAD 8u
+/* Draw the frame in ONE raster pass. Default: large frames are drawn in two depth-ordered passes with a tile
+ * hi-Z between them, which drops occluded segments of the second pass before any pixel work; the G-buffer is the
+ * same bit for bit (the resolve is an order-free min). For A/B measurements. */
+#define HAIR_FLAG_SINGLE_PASS 16u
 
 typedef struct hair_ctx hair_ctx; /* opaque; owns all device scratch */
 
@@ -198,6 +202,8 @@ typedef struct {
   uint32_t n_timed_frames;
   float beta_mean; /* N_remaining / N_total of Eq. 8 over all grooms */
   uint32_t gpu_launches; /* kernels launched by the last hair_render */
+  uint32_t two_pass;              /* 1: the last frame was drawn in two depth-ordered raster passes */
+  uint32_t n_segments_hiz_culled; /* segments of the second pass dropped by the tile hi-Z test before any pixel work */
 } hair_stats_t;
 /* Synchronises the stream and reads the device counters of the last frame. */
 int hair_stats(hair_ctx*, hair_stats_t* out);

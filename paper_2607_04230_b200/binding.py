@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(_HERE, "csrc", "libhair.so")
 
 OP_BITS = {"clump": 1, "twist": 2, "curl": 4, "frizz": 8}
-FLAG_FILTER, FLAG_COUNTERS, FLAG_STAGE_TIMING, FLAG_PAPER_PAYLOAD = 1, 2, 4, 8
+FLAG_FILTER, FLAG_COUNTERS, FLAG_STAGE_TIMING, FLAG_PAPER_PAYLOAD, FLAG_SINGLE_PASS = 1, 2, 4, 8, 16
 EMPTY = 0xFFFFFFFFFFFFFFFF
 
 EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_render_params",
@@ -71,7 +71,8 @@ class hair_stats_t(C.Structure):
                 ("n_pixels_center", C.c_uint32), ("n_pixels_cons", C.c_uint32),
                 ("ms_lod", C.c_float), ("ms_generate", C.c_float), ("ms_clear", C.c_float),
                 ("ms_raster", C.c_float), ("ms_shade", C.c_float), ("ms_filter", C.c_float),
-                ("ms_total", C.c_float), ("n_timed_frames", C.c_uint32), ("beta_mean", C.c_float), ("gpu_launches", C.c_uint32)]
+                ("ms_total", C.c_float), ("n_timed_frames", C.c_uint32), ("beta_mean", C.c_float), ("gpu_launches", C.c_uint32),
+                ("two_pass", C.c_uint32), ("n_segments_hiz_culled", C.c_uint32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -39,8 +39,14 @@ struct hair_ctx {
   hair_render_params prm;
   // scratch
   uint4* d_table = nullptr;
-  uint4* d_part = nullptr;    // [ceil(n_bi / 256)] tile sums between k_lod and k_scan
-  uint32_t* d_grp = nullptr;  // [n_bi + 1] exclusive scan of the raster's work groups per bundle-instance
+  uint4* d_part = nullptr;    // [2 ceil(n_bi / 256)] tile sums between k_lod and k_scan
+  uint32_t* d_grp = nullptr;  // [2][n_bi + 1] exclusive scans of the work groups of the near and the far raster pass
+  uint32_t* d_zrange = nullptr;  // [2][n_inst][2] min / max bundle depth per instance, ping-pong by frame parity
+  uint32_t n_inst = 0, zrange_cap = 0, frame_no = 0;
+  uint32_t* h_want = nullptr;  // host-mapped: 1 if the last scanned frame was big enough for two raster passes
+  uint32_t* d_want = nullptr;  // its device alias (written by k_scan)
+  uint32_t* d_hiz = nullptr;  // [ceil(h / 16)][ceil(w / 16)] farthest centre depth per tile between the passes
+  size_t hiz_cap = 0;
   size_t table_cap = 0;
   uint2* d_srec = nullptr;  // per strand id: {vertex offset, C | groom << 8} of this frame (k_generate)
   size_t srec_cap = 0;
@@ -66,7 +72,7 @@ struct hair_ctx {
   int next_slot = 0;
   cudaEvent_t ev[EV_RING][EV_N] = {};
   uint32_t ev_frames = 0;  // timed frames since the last hair_stats
-  bool timed = false, counted = false;
+  bool timed = false, counted = false, last_two_pass = false;
   uint32_t last_w = 0, last_h = 0, launches = 0;
   CamDev last_cam;
 };
@@ -184,8 +190,8 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
     c->d_grp = nullptr;
     c->table_cap = 0;
     CK(cudaMalloc((void**)&c->d_table, (size_t)c->scene.n_bi * sizeof(uint4)));
-    CK(cudaMalloc((void**)&c->d_grp, ((size_t)c->scene.n_bi + 1) * sizeof(uint32_t)));
-    CK(cudaMalloc((void**)&c->d_part, ((size_t)c->scene.n_bi / 256 + 1) * sizeof(uint4)));
+    CK(cudaMalloc((void**)&c->d_grp, 2 * ((size_t)c->scene.n_bi + 1) * sizeof(uint32_t)));
+    CK(cudaMalloc((void**)&c->d_part, 2 * ((size_t)c->scene.n_bi / 256 + 1) * sizeof(uint4)));
     c->table_cap = c->scene.n_bi;
   }
   if (c->scene.n_strands_total > c->srec_cap) {
@@ -200,6 +206,25 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
     c->d_vertices = nullptr;
     CK(cudaMalloc((void**)&c->d_vertices, (c->vertex_need + 32) * sizeof(float4)));
     c->vertex_cap = c->vertex_need;
+  }
+  if (c->n_inst > c->zrange_cap) {  // empty ranges: min = a huge float, max = 0 (the first frame then draws in one pass)
+    cudaFree(c->d_zrange);
+    c->d_zrange = nullptr;
+    c->zrange_cap = 0;
+    CK(cudaMalloc((void**)&c->d_zrange, (size_t)c->n_inst * 4 * sizeof(uint32_t)));
+    std::vector<uint32_t> init((size_t)c->n_inst * 4);
+    for (size_t i = 0; i < init.size(); ++i) init[i] = (i & 1) ? 0u : 0x7F000000u;
+    CK(cudaMemcpyAsync(c->d_zrange, init.data(), init.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    c->zrange_cap = c->n_inst;
+  }
+  const size_t n_hiz = (size_t)((w + HIZ_TILE - 1) / HIZ_TILE) * ((h + HIZ_TILE - 1) / HIZ_TILE);
+  if (n_hiz > c->hiz_cap) {
+    cudaFree(c->d_hiz);
+    c->d_hiz = nullptr;
+    c->hiz_cap = 0;
+    CK(cudaMalloc((void**)&c->d_hiz, n_hiz * sizeof(uint32_t)));
+    c->hiz_cap = n_hiz;
   }
   size_t px = (size_t)w * h;
   if (px > c->colour_cap) {
@@ -262,6 +287,12 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   const uint32_t n_bi = c->scene.n_bi;
   cudaStream_t st = c->stream;
   uint32_t launches = 0;
+  // two depth-ordered raster passes with a tile hi-Z between them (k_raster.cu); the counted and the reference
+  // rasters visit every hit, so they draw in one pass
+  // and small frames too: k_scan reports through host-mapped memory whether the frame it scanned was big enough,
+  // and the next frame launches the hi-Z and the second pass only then (no empty launches, no host sync)
+  const bool two_pass = front && !count && !po.ms_k && !(c->prm.flags & HAIR_FLAG_SINGLE_PASS) &&
+                        *(volatile uint32_t*)c->h_want != 0u;
   cudaEvent_t* evs = c->ev[c->ev_frames % EV_RING];
   auto mark = [&](int e) {
     if (timed) cudaEventRecord(evs[e], st);
@@ -288,7 +319,8 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   if (front && n_bi) {
     LambdaArr la;
     for (uint32_t i = 0; i < HAIR_MAX_GROOMS; ++i) la.v[i] = n_lam == 0 ? 0.f : lam[n_lam == 1 ? 0 : (i < n_lam ? i : 0)];
-    launch_lod_scan(c->d_scene, n_bi, k, la, po.groom_mask & c->prm.groom_mask, c->d_table, c->d_grp, c->d_part, c->d_counters, st);
+    launch_lod_scan(c->d_scene, n_bi, k, la, po.groom_mask & c->prm.groom_mask, c->d_table, c->d_grp, c->d_part,
+                    c->d_counters, c->d_zrange, c->n_inst, c->frame_no++, two_pass, c->d_want, st);
     launches += 2;
   }
   mark(EV_LOD);
@@ -305,10 +337,19 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_CLEAR);
   if ((stage_mask & 1u) && n_bi) {
-    if (!front) CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER, 0, sizeof(unsigned long long), st));
+    if (!front) {  // the table (and its pass split) is the last frame's: restart both queues
+      CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER, 0, sizeof(unsigned long long), st));
+      CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER1, 0, sizeof(unsigned long long), st));
+    }
     launch_raster(c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters,
-                  count && !po.ms_k, po.ms_k, pp, c->n_sm, st);
+                  count && !po.ms_k, po.ms_k, pp, 0, nullptr, c->n_sm, st);
     ++launches;
+    if (two_pass || (!front && c->last_two_pass)) {
+      launch_hiz(gbuf, w, h, c->d_hiz, c->d_counters, st);
+      launch_raster(c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters,
+                    false, 0, pp, 1, c->d_hiz, c->n_sm, st);
+      launches += 2;
+    }
   }
   mark(EV_RASTER);
   if (po.ms_k) {
@@ -330,6 +371,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   c->timed = timed;
   if (timed) ++c->ev_frames;
   c->counted = count;
+  if (front) c->last_two_pass = two_pass;
   c->last_w = w;
   c->last_h = h;
   c->launches = launches;
@@ -356,7 +398,10 @@ int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream) {
             cudaMalloc((void**)&c->d_scene, sizeof(SceneDev)) == cudaSuccess &&
             cudaMalloc((void**)&c->d_counters, CNT_N * sizeof(unsigned long long)) == cudaSuccess &&
             cudaMemset(c->d_counters, 0, CNT_N * sizeof(unsigned long long)) == cudaSuccess &&
-            cudaMallocHost((void**)&c->h_counters, CNT_N * sizeof(unsigned long long)) == cudaSuccess;
+            cudaMallocHost((void**)&c->h_counters, CNT_N * sizeof(unsigned long long)) == cudaSuccess &&
+            cudaHostAlloc((void**)&c->h_want, sizeof(uint32_t), cudaHostAllocMapped) == cudaSuccess &&
+            cudaHostGetDevicePointer((void**)&c->d_want, c->h_want, 0) == cudaSuccess;
+  if (ok) *c->h_want = 0u;
   for (int f = 0; ok && f < EV_RING; ++f)
     for (int i = 0; ok && i < EV_N; ++i) ok = cudaEventCreate(&c->ev[f][i]) == cudaSuccess;
   ok = ok && cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess &&
@@ -387,6 +432,8 @@ void hair_destroy(hair_ctx* c) {
   cudaFree(c->d_srec);
   cudaFree(c->d_colour);
   cudaFree(c->d_target2);
+  cudaFree(c->d_zrange);
+  cudaFree(c->d_hiz);
   cudaFree(c->d_counters);
   if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
   for (int k = 0; k < HAIR_HOST_SLOTS; ++k) {
@@ -403,6 +450,7 @@ void hair_destroy(hair_ctx* c) {
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
   if (c->h_counters) cudaFreeHost(c->h_counters);
+  if (c->h_want) cudaFreeHost(c->h_want);
   for (int f = 0; f < EV_RING; ++f)
     for (int i = 0; i < EV_N; ++i)
       if (c->ev[f][i]) cudaEventDestroy(c->ev[f][i]);
@@ -509,6 +557,7 @@ int hair_mesh_upload(hair_ctx* c, const hair_cage* cage, const hair_roots* roots
   gd.N = (uint32_t)N;
   gd.sid_base = sid_base;
   gd.gid_base = gid_base;
+  gd.inst_base = c->n_inst;
   gd.c_full = c_full;
   gd.spi = st->spi;
   gd.seed_h = pcg_host(st->seed);
@@ -533,6 +582,7 @@ int hair_mesh_upload(hair_ctx* c, const hair_cage* cage, const hair_roots* roots
   c->scene.n_grooms = gi + 1;
   c->scene.n_bi = gid_base + T * Q;
   c->scene.n_strands_total = sid_base + (uint32_t)N * Q;
+  c->n_inst += Q;
   c->vertex_need += (size_t)N * Q * c_full;
   if (c_full > c->c_max) c->c_max = c_full;
   c->grooms.push_back(gh);
@@ -561,6 +611,7 @@ int hair_mesh_clear(hair_ctx* c) {
   memset(&c->scene, 0, sizeof(c->scene));
   c->vertex_need = 0;
   c->c_max = 0;
+  c->n_inst = 0;
   c->scene_dirty = true;
   return HAIR_OK;
 }
@@ -706,6 +757,8 @@ int hair_stats(hair_ctx* c, hair_stats_t* out) {
   out->n_vertices = (uint32_t)k[CNT_VERTICES];
   out->n_segments = (uint32_t)k[CNT_SEGMENTS];
   out->gpu_launches = c->launches;
+  out->two_pass = (uint32_t)k[CNT_HIZ_ON];
+  out->n_segments_hiz_culled = (uint32_t)k[CNT_SEG_HIZ];
   out->beta_mean = c->scene.n_strands_total ? (float)((double)k[CNT_STRANDS] / (double)c->scene.n_strands_total) : 1.f;
   if (c->counted) {
     out->n_segments_drawn = (uint32_t)k[CNT_SEG_DRAWN];

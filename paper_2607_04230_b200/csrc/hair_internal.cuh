@@ -15,6 +15,16 @@
 #define HAIR_PAYLOAD_NONE 0xFFFFFFFFFFull
 #define RAS_CHUNK 31  // segments a raster warp draws at once (32 vertices, neighbour by shuffle)
 #define RAS_GROUP 4   // chunks per unit of the raster's device-side work queue
+#ifndef HIZ_TILE
+#define HIZ_TILE 16
+#endif
+// HIZ_TILE: hi-Z tile edge in pixels (k_hiz): a segment's bounding box touches at most 3 x 3 of them
+#ifndef HIZ_MIN_VERTS
+#define HIZ_MIN_VERTS 3000000u  // frames with fewer vertices after LOD are drawn in one pass
+#endif
+#ifndef HIZ_CUT
+#define HIZ_CUT 0.6f  // bundles whose nearest cage depth lies in the front HIZ_CUT of their instance's range go first
+#endif
 #define HAIR_ROW 44  // floats per control-point row of the per-bundle table (== 12 mod 32: LDS.128 conflict-free)
 
 struct GroomDev {
@@ -26,6 +36,7 @@ struct GroomDev {
   const uint32_t* tri_of;  // [N] bundle (root triangle) of each local strand id: the inverse of off
   const float* xform;   // [Q][12] or nullptr
   uint32_t V, Lv, T, Q, N, sid_base, gid_base, c_full;
+  uint32_t inst_base;  // index of this groom's first instance among all instances of the scene
   uint32_t spi, seed_h, op_mask, clump_exp, frizz_cells;
   float clump_strength, twist_turns, curl_radius, curl_turns, curl_ramp_w0, frizz_sigma, frizz_ramp_w0;
   float width_world;
@@ -81,6 +92,9 @@ enum {
   CNT_SEG_LIVE,      // segments that sent at least one atomic (the rest lost every pixel to nearer hair)
   CNT_PX_CENTER,
   CNT_PX_CONS,
+  CNT_WORK_RASTER1,  // queue head of the second (far) raster pass
+  CNT_HIZ_ON,        // 1: the frame is drawn in two depth-ordered passes with a tile hi-Z between them
+  CNT_SEG_HIZ,       // segments dropped by the hi-Z test of the second pass
   CNT_N
 };
 
@@ -202,16 +216,21 @@ __device__ __forceinline__ Loc locate_strand(const uint2* __restrict__ srec, uin
 }
 
 // ------------------------------------------------------------------ launchers (one per .cu)
+// zrange: [2][n_inst][2] u32 (float bits of min / max bundle depth per instance), ping-pong by frame parity;
+// grp: two exclusive scans of n_bi + 1 entries (near pass, far pass); two_pass = false draws everything in the first
 void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint32_t groom_mask,
-                     uint4* table, uint32_t* grp, uint4* part, unsigned long long* counters, cudaStream_t st);
+                     uint4* table, uint32_t* grp, uint4* part, unsigned long long* counters, uint32_t* zrange,
+                     uint32_t n_inst, uint32_t parity, bool two_pass, uint32_t* want_two_pass, cudaStream_t st);
+void launch_hiz(const unsigned long long* gbuf, uint32_t W, uint32_t H, uint32_t* hiz,
+                const unsigned long long* counters, cudaStream_t st);
 void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices, uint2* srec,
                      unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st);
 void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_zn, cudaStream_t st);
 void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
-                   unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int n_sm,
-                   cudaStream_t st);
+                   unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int pass,
+                   const uint32_t* hiz, int n_sm, cudaStream_t st);
 void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
                          float4* out, cudaStream_t st);

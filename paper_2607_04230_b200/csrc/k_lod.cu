@@ -25,11 +25,18 @@ __device__ __forceinline__ uint32_t raster_groups(uint32_t n_v) {  // units of R
   return n_v >= 2 ? (n_v - 1 + RAS_GROUP * RAS_CHUNK - 1) / (RAS_GROUP * RAS_CHUNK) : 0u;
 }
 
+// Depth order of the raster (k_raster.cu): every bundle-instance also reports its nearest cage depth; the range of
+// those depths per instance is accumulated for the NEXT frame (zr_cur) and the range of the PREVIOUS frame (zr_prev)
+// decides which of the two raster passes draws the bundle: the front HIZ_CUT of the range first. Order is a
+// heuristic only — the resolve is an order-free min — so a stale or empty range (first frame: one pass) is fine.
 __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, uint32_t n_bi, CamDev cam,
                                              LambdaArr lam, uint32_t groom_mask, uint4* __restrict__ table,
-                                             uint4* __restrict__ part) {
+                                             uint4* __restrict__ part, const uint32_t* __restrict__ zr_prev,
+                                             uint32_t* __restrict__ zr_cur, uint32_t two_pass) {
   uint32_t gid = blockIdx.x * blockDim.x + threadIdx.x;
-  uint32_t nlod = 0, C = 0;
+  uint32_t nlod = 0, C = 0, far_pass = 0;
+  uint32_t inst = 0xFFFFFFFFu;
+  float zmin = 3.0e38f;
   if (gid < n_bi) {
   uint32_t gi = 0;
   for (uint32_t k = 1; k < sc->n_grooms; ++k)
@@ -39,9 +46,22 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
   uint32_t q = rel / g.T, t = rel - q * g.T;
   uint32_t N = __ldg(&g.npt[t]);
   float lambda = lam.v[gi];
+  inst = g.inst_base + q;
   if (!(lambda > 0.f)) {  // R14: LOD and culling off
     nlod = N;
     C = g.c_full;
+    for (uint32_t i = 0; i < g.Lv; i += g.Lv - 1)  // root and tip layer are enough for an ordering key
+      for (int c = 0; c < 3; ++c) {
+        const float* x = g.pos + ((size_t)i * g.V + __ldg(&g.idx[t * 3 + c])) * 3;
+        float wx = __ldg(x), wy = __ldg(x + 1), wz = __ldg(x + 2);
+        if (g.xform) {
+          const float* M = g.xform + q * 12;
+          const float ax = M[0] * wx + M[1] * wy + M[2] * wz + M[3], ay = M[4] * wx + M[5] * wy + M[6] * wz + M[7];
+          wz = M[8] * wx + M[9] * wy + M[10] * wz + M[11];
+          wx = ax, wy = ay;
+        }
+        zmin = fminf(zmin, (wx - cam.eye[0]) * cam.f[0] + (wy - cam.eye[1]) * cam.f[1] + (wz - cam.eye[2]) * cam.f[2]);
+      }
   } else {
     float M[12];
     bool has_m = g.xform != nullptr;
@@ -61,6 +81,7 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
           wz = xadd(xadd(xadd(xmul(M[8], x0), xmul(M[9], x1)), xmul(M[10], x2)), M[11]);
         }
         Proj p = project_exact(cam, wx, wy, wz);
+        zmin = fminf(zmin, p.zv);
         ++n_all;
         if (p.valid) {
           ++n_valid;
@@ -92,24 +113,54 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
     }
   }
   if (!((groom_mask >> gi) & 1u)) nlod = C = 0;  // R-seq: this groom is not drawn in this pass
-  table[gid] = make_uint4(nlod, C, 0u, 0u);
+  if (two_pass) {
+    const float z0 = __uint_as_float(__ldg(&zr_prev[inst * 2])), z1 = __uint_as_float(__ldg(&zr_prev[inst * 2 + 1]));
+    far_pass = (z1 > z0 && zmin > z0 + HIZ_CUT * (z1 - z0)) ? 1u : 0u;
+  }
+  table[gid] = make_uint4(nlod, C, far_pass, 0u);  // .z: the pass, until k_scan replaces it by the slot base
+  }
+  {  // depth range per instance for the next frame: positive floats order like their bits
+    const uint32_t i0 = __shfl_sync(0xffffffffu, inst, 0);
+    const float zc = fmaxf(zmin, 0.f);
+    if (__all_sync(0xffffffffu, inst == i0)) {
+      float lo = zc, hi = zc;
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) {
+        lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, d));
+        hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, d));
+      }
+      if ((threadIdx.x & 31) == 0 && i0 != 0xFFFFFFFFu) {
+        atomicMin(&zr_cur[i0 * 2], __float_as_uint(lo));
+        atomicMax(&zr_cur[i0 * 2 + 1], __float_as_uint(hi));
+      }
+    } else if (inst != 0xFFFFFFFFu) {
+      atomicMin(&zr_cur[inst * 2], __float_as_uint(zc));
+      atomicMax(&zr_cur[inst * 2 + 1], __float_as_uint(zc));
+    }
   }
   // sums of this tile of 256 bundle-instances for the scan: strands, vertices, raster work groups, culled
-  uint32_t ts = nlod, tv = nlod * C, tg = raster_groups(nlod * C), tc = (gid < n_bi && nlod == 0) ? 1u : 0u;
+  // part[2 tile] = {strands, vertices, work groups of the near pass, of the far pass}, part[2 tile + 1].x = culled
+  const uint32_t ng = raster_groups(nlod * C);
+  uint32_t ts = nlod, tv = nlod * C, tg = far_pass ? 0u : ng, tf = far_pass ? ng : 0u,
+           tc = (gid < n_bi && nlod == 0) ? 1u : 0u;
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) {
     ts += __shfl_xor_sync(0xffffffffu, ts, d);
     tv += __shfl_xor_sync(0xffffffffu, tv, d);
     tg += __shfl_xor_sync(0xffffffffu, tg, d);
+    tf += __shfl_xor_sync(0xffffffffu, tf, d);
     tc += __shfl_xor_sync(0xffffffffu, tc, d);
   }
   __shared__ uint4 s_w[8];
-  if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = make_uint4(ts, tv, tg, tc);
+  __shared__ uint32_t s_c[8];
+  if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = make_uint4(ts, tv, tg, tf), s_c[threadIdx.x >> 5] = tc;
   __syncthreads();
   if (threadIdx.x == 0) {
     uint4 a = s_w[0];
-    for (int wv = 1; wv < 8; ++wv) a.x += s_w[wv].x, a.y += s_w[wv].y, a.z += s_w[wv].z, a.w += s_w[wv].w;
-    part[blockIdx.x] = a;
+    uint32_t cc = s_c[0];
+    for (int wv = 1; wv < 8; ++wv) a.x += s_w[wv].x, a.y += s_w[wv].y, a.z += s_w[wv].z, a.w += s_w[wv].w, cc += s_c[wv];
+    part[blockIdx.x * 2] = a;
+    part[blockIdx.x * 2 + 1] = make_uint4(cc, 0u, 0u, 0u);
   }
 }
 
@@ -119,71 +170,100 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
 // scanned by warp 0; a second pass adds the warp offsets. Coalesced 16-byte accesses throughout.
 
 __global__ void __launch_bounds__(256) k_scan(uint4* __restrict__ table, uint32_t* __restrict__ grp, uint32_t n_bi,
-                                              const uint4* __restrict__ part, unsigned long long* __restrict__ counters) {
-  __shared__ uint32_t s_a[8][4], s_b[8][3];
+                                              const uint4* __restrict__ part, unsigned long long* __restrict__ counters,
+                                              uint32_t* __restrict__ zr_reset, uint32_t n_inst, uint32_t two_pass,
+                                              uint32_t* __restrict__ want_two_pass) {
+  __shared__ uint32_t s_a[8][5], s_b[8][4], s_tot[8];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tile = blockIdx.x;
-  // (1) what lies before this tile: sums of the tiles in front of it
-  uint32_t ps = 0, pv = 0, pg = 0, pc = 0;
-  for (uint32_t t = threadIdx.x; t < tile; t += 256) {
-    const uint4 a = __ldg(&part[t]);
-    ps += a.x, pv += a.y, pg += a.z, pc += a.w;
+  uint32_t* grp1 = grp + n_bi + 1;
+  // (1) what lies before this tile: sums of the tiles in front of it; and the frame's total of vertices
+  uint32_t ps = 0, pv = 0, pg = 0, pf = 0, pc = 0, tot = 0;
+  for (uint32_t t = threadIdx.x; t < gridDim.x; t += 256) {
+    const uint4 a = __ldg(&part[2 * t]);
+    tot += a.y;
+    if (t < tile) ps += a.x, pv += a.y, pg += a.z, pf += a.w, pc += __ldg(&part[2 * t + 1]).x;
   }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) {
     ps += __shfl_xor_sync(0xffffffffu, ps, d);
     pv += __shfl_xor_sync(0xffffffffu, pv, d);
     pg += __shfl_xor_sync(0xffffffffu, pg, d);
+    pf += __shfl_xor_sync(0xffffffffu, pf, d);
     pc += __shfl_xor_sync(0xffffffffu, pc, d);
+    tot += __shfl_xor_sync(0xffffffffu, tot, d);
   }
+  if (lane == 0) s_tot[warp] = tot;
+  __syncthreads();
+  tot = 0;
+#pragma unroll
+  for (uint32_t wv = 0; wv < 8; ++wv) tot += s_tot[wv];
+  // small frames are drawn in one pass: the hi-Z between the passes would cost more than it saves
+  // (the host launches the second pass only when the frame before wanted it: want_two_pass is host-mapped memory)
+  const bool want = tot >= HIZ_MIN_VERTS;
+  const bool two = two_pass != 0u && want;
   // (2) exclusive scan inside the tile: shuffle scan per warp, then the 8 warp totals
   const uint32_t i = tile * 256 + threadIdx.x;
   uint4 e = i < n_bi ? table[i] : make_uint4(0, 0, 0, 0);
-  const uint32_t s = e.x, v = e.x * e.y, g = raster_groups(v);
-  uint32_t is = s, iv = v, ig = g;
+  const uint32_t s = e.x, v = e.x * e.y, ng = raster_groups(v);
+  const bool far_pass = two && e.z != 0u;
+  const uint32_t g = far_pass ? 0u : ng, f = far_pass ? ng : 0u;
+  uint32_t is = s, iv = v, ig = g, jf = f;
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
     uint32_t a = __shfl_up_sync(0xffffffffu, is, d), b = __shfl_up_sync(0xffffffffu, iv, d),
-             c = __shfl_up_sync(0xffffffffu, ig, d);
+             c = __shfl_up_sync(0xffffffffu, ig, d), c1 = __shfl_up_sync(0xffffffffu, jf, d);
     if (lane >= d) {
       is += a;
       iv += b;
       ig += c;
+      jf += c1;
     }
   }
-  if (lane == 0) s_a[warp][0] = ps, s_a[warp][1] = pv, s_a[warp][2] = pg, s_a[warp][3] = pc;
-  if (lane == 31) s_b[warp][0] = is, s_b[warp][1] = iv, s_b[warp][2] = ig;
+  if (!two) pg += pf, pf = 0;  // the tiles in front counted their far bundles apart
+  if (lane == 0) s_a[warp][0] = ps, s_a[warp][1] = pv, s_a[warp][2] = pg, s_a[warp][3] = pc, s_a[warp][4] = pf;
+  if (lane == 31) s_b[warp][0] = is, s_b[warp][1] = iv, s_b[warp][2] = ig, s_b[warp][3] = jf;
   __syncthreads();
-  uint32_t off_s = 0, off_v = 0, off_g = 0, culled = 0;
+  uint32_t off_s = 0, off_v = 0, off_g = 0, off_f = 0, culled = 0;
 #pragma unroll
   for (uint32_t wv = 0; wv < 8; ++wv) {
-    off_s += s_a[wv][0], off_v += s_a[wv][1], off_g += s_a[wv][2], culled += s_a[wv][3];  // tiles in front
-    if (wv < warp) off_s += s_b[wv][0], off_v += s_b[wv][1], off_g += s_b[wv][2];          // warps in front
+    off_s += s_a[wv][0], off_v += s_a[wv][1], off_g += s_a[wv][2], culled += s_a[wv][3], off_f += s_a[wv][4];
+    if (wv < warp) off_s += s_b[wv][0], off_v += s_b[wv][1], off_g += s_b[wv][2], off_f += s_b[wv][3];
   }
   if (i < n_bi) {
     e.z = off_s + is - s;
     e.w = off_v + iv - v;
     table[i] = e;
     grp[i] = off_g + ig - g;
+    grp1[i] = off_f + jf - f;
   }
+  // the depth ranges the previous frame left (k_lod has read them) restart for the frame after this one
+  if (tile == 0)
+    for (uint32_t k = threadIdx.x; k < n_inst; k += 256) zr_reset[2 * k] = 0x7F000000u, zr_reset[2 * k + 1] = 0u;
   // (3) the last tile knows the totals: device-side counts and queue lengths of the frame
   if (tile == gridDim.x - 1 && threadIdx.x == 255) {
-    const uint4 mine = __ldg(&part[tile]);
-    const uint32_t n_s = off_s + is, n_v = off_v + iv, n_g = off_g + ig;
+    const uint32_t mine_c = __ldg(&part[2 * tile + 1]).x;
+    const uint32_t n_s = off_s + is, n_v = off_v + iv, n_g = off_g + ig, n_f = off_f + jf;
     counters[CNT_STRANDS] = n_s;
     counters[CNT_VERTICES] = n_v;
     counters[CNT_SEGMENTS] = n_v - n_s;  // sum N_LOD*(C-1)
-    counters[CNT_CULLED] = culled + mine.w;
+    counters[CNT_CULLED] = culled + mine_c;
     counters[CNT_WORK_GEN] = 0;
     counters[CNT_WORK_RASTER] = 0;
     for (int k = CNT_SEG_DRAWN; k < CNT_N; ++k) counters[k] = 0;
-    grp[n_bi] = n_g;  // total work groups: the raster's queue length
+    counters[CNT_HIZ_ON] = (two && n_f > 0) ? 1ull : 0ull;
+    grp[n_bi] = n_g;  // total work groups of each pass: the raster's queue lengths
+    grp1[n_bi] = n_f;
+    *want_two_pass = want ? 1u : 0u;
   }
 }
 
 void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaArr lam, uint32_t groom_mask,
-                     uint4* table, uint32_t* grp, uint4* part, unsigned long long* counters, cudaStream_t st) {
-  // part: one uint4 per tile of 256 bundle-instances (sums), written by k_lod, read by k_scan
+                     uint4* table, uint32_t* grp, uint4* part, unsigned long long* counters, uint32_t* zrange,
+                     uint32_t n_inst, uint32_t parity, bool two_pass, uint32_t* want_two_pass, cudaStream_t st) {
+  // part: two uint4 per tile of 256 bundle-instances (sums), written by k_lod, read by k_scan
   const uint32_t n_tiles = (n_bi + 255) / 256;
-  k_lod<<<n_tiles, 256, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table, part);
-  k_scan<<<n_tiles, 256, 0, st>>>(table, grp, n_bi, part, counters);
+  uint32_t* zr_cur = zrange + (size_t)(parity & 1u) * n_inst * 2;
+  uint32_t* zr_prev = zrange + (size_t)((parity + 1u) & 1u) * n_inst * 2;
+  k_lod<<<n_tiles, 256, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table, part, zr_prev, zr_cur, two_pass ? 1u : 0u);
+  k_scan<<<n_tiles, 256, 0, st>>>(table, grp, n_bi, part, counters, zr_prev, n_inst, two_pass ? 1u : 0u, want_two_pass);
 }

@@ -55,22 +55,29 @@ __constant__ int c_ms_off[4][8][2] = {  // sample offsets from the pixel centre 
 // computes calcTangent of its vertex (neighbours by shuffle, one extra load at each end of the chunk) and the
 // strand's root codes, the record carries both ends' tangent and AO, and a hit whose depth does not lose builds the
 // 40 payload bits (interpolated tangent -> octahedral code, w, AO) in fixed-order fp32 instead of sid | j | t.
-template <bool COUNT, bool MS, bool PP>
+// Two depth-ordered passes (HZ = true is the second): k_lod sends the bundles whose nearest cage depth lies in the
+// front part of their instance's depth range to the first pass; between the passes k_hiz takes the farthest centre
+// depth of every 16 x 16 pixel tile; the second pass drops a segment before any pixel work when its nearest depth
+// lies behind that bound in every tile its bounding box touches — every one of its pixels would have failed the
+// per-pixel early reject below, so the result is the same G-buffer, bit for bit.
+template <bool COUNT, bool MS, bool PP, bool HZ>
 __global__ void __launch_bounds__(RAS_WARPS * 32, RAS_MIN_BLOCKS)
 k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
          const uint32_t* __restrict__ grp, const float4* __restrict__ vertices, CamDev cam, float rho_default,
-         unsigned long long* __restrict__ gbuf, unsigned long long* __restrict__ counters, uint32_t ms_k) {
+         unsigned long long* __restrict__ gbuf, unsigned long long* __restrict__ counters, uint32_t ms_k,
+         uint32_t queue, const uint32_t* __restrict__ hiz) {
   constexpr int RS = PP ? REC_STRIDE_PP : REC_STRIDE;
   __shared__ __align__(16) float s_rec[RAS_WARPS][32][RS];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float(*rec)[RS] = s_rec[warp];
-  uint32_t c_center = 0, c_cons = 0, c_drawn = 0, c_issued = 0, c_live = 0;
+  uint32_t c_center = 0, c_cons = 0, c_drawn = 0, c_issued = 0, c_live = 0, c_hiz = 0;
   const int W = (int)cam.W, H = (int)cam.H;
+  const int hiz_w = (W + HIZ_TILE - 1) / HIZ_TILE;
   const uint32_t le_mask = 0xFFFFFFFFu >> (31 - lane);
   const uint32_t n_groups = __ldcg(&grp[n_bi]);
   for (;;) {
     uint32_t wi = 0;
-    if (lane == 0) wi = (uint32_t)atomicAdd(&counters[CNT_WORK_RASTER], 1ull);
+    if (lane == 0) wi = (uint32_t)atomicAdd(&counters[queue], 1ull);
     wi = __shfl_sync(0xffffffffu, wi, 0);
     if (wi >= n_groups) break;
     // ---- bundle of this group: largest gid with grp[gid] <= wi (32 pivots per level)
@@ -165,7 +172,27 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
         // candidate pixels = exactly those whose closed square overlaps the segment's AABB (R10)
         const float fc0 = fmaxf(ceilf(fminf(aM, bM)) - 1.f, 0.f), fc1 = fminf(floorf(fmaxf(aM, bM)), limM);
         const float fr0 = fmaxf(ceilf(fminf(aN, bN)) - 1.f, 0.f), fr1 = fminf(floorf(fmaxf(aN, bN)), limN);
-        if (fc0 <= fc1 && fr0 <= fr1) {
+        bool draw = fc0 <= fc1 && fr0 <= fr1;
+        // nearest depth any pixel of this segment can store, minus 2 steps for the rounding of R11's lerp
+        const uint32_t dqm = quant_depth(fminf(fmaxf(fminf(a.zn, b.zn), 0.f), 1.f));
+        const uint32_t dq_lim = dqm > 2u ? dqm - 2u : 0u;
+        if (HZ && draw) {  // hi-Z: farthest centre depth over the (at most 3 x 3) tiles of the bounding box
+          const int x0 = (int)(ymajor ? fr0 : fc0) / HIZ_TILE, x1 = (int)(ymajor ? fr1 : fc1) / HIZ_TILE;
+          const int y0 = (int)(ymajor ? fc0 : fr0) / HIZ_TILE, y1 = (int)(ymajor ? fc1 : fr1) / HIZ_TILE;
+          if (x1 - x0 <= 2 && y1 - y0 <= 2) {
+            uint32_t zfar = 0;
+#pragma unroll
+            for (int ty = 0; ty < 3; ++ty)
+#pragma unroll
+              for (int tx = 0; tx < 3; ++tx)
+                zfar = max(zfar, __ldg(&hiz[min(y0 + ty, y1) * hiz_w + min(x0 + tx, x1)]));
+            if (dq_lim > zfar) {
+              draw = false;
+              ++c_hiz;
+            }
+          }
+        }
+        if (draw) {
           n_steps = (uint32_t)((int)fc1 - (int)fc0 + 1);
           float4* r4 = reinterpret_cast<float4*>(rec[lane]);
           const float dd = xadd(xmul(dx, dx), xmul(dy, dy));
@@ -177,9 +204,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
                               __uint_as_float(((uint32_t)(int)fr0 << 16) | (uint32_t)(int)fr1));
           rec[lane][17] = xmul(rho, rho);
           r4[3].x = __uint_as_float((ymajor ? 0x80000000u : 0u) | ((sid0 + k) << 7) | j);
-          // nearest depth any pixel of this segment can store, minus 2 steps for the rounding of R11's lerp
-          const uint32_t dqm = quant_depth(fminf(fmaxf(fminf(a.zn, b.zn), 0.f), 1.f));
-          r4[3].w = __uint_as_float(dqm > 2u ? dqm - 2u : 0u);
+          r4[3].w = __uint_as_float(dq_lim);
           if (COUNT) rec[lane][16] = 0.f;
         }
       }
@@ -313,6 +338,11 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
       if (COUNT && n_steps && rec[lane][16] != 0.f) ++c_live;
     }
   }
+  if (HZ) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c_hiz += __shfl_xor_sync(0xffffffffu, c_hiz, d);
+    if (lane == 0 && c_hiz) atomicAdd(&counters[CNT_SEG_HIZ], (unsigned long long)c_hiz);
+  }
   if (COUNT) {
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) {
@@ -363,37 +393,71 @@ void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st) {
   k_reseed<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels);
 }
 
+// farthest centre depth of every HIZ_TILE x HIZ_TILE pixel tile (a warp per tile; lane = half a row of the tile).
+// A pixel without a centre hit keeps the depth it was cleared / seeded with (all ones = never occludes).
+__global__ void __launch_bounds__(256) k_hiz(const uint4* __restrict__ g, uint32_t W, uint32_t H,
+                                             uint32_t* __restrict__ hiz, const unsigned long long* __restrict__ counters) {
+  if (__ldcg(&counters[CNT_HIZ_ON]) == 0ull) return;  // one-pass frame (decided on the device by k_scan)
+  const uint32_t tw = (W + HIZ_TILE - 1) / HIZ_TILE, th = (H + HIZ_TILE - 1) / HIZ_TILE;
+  const uint32_t tile = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (tile >= tw * th) return;
+  const uint32_t ty = tile / tw, tx = tile - ty * tw;
+  const uint32_t y = ty * HIZ_TILE + (lane >> 1), x0 = tx * HIZ_TILE + (lane & 1u) * 8u;
+  uint32_t zfar = 0;
+  if (y < H) {
+#pragma unroll
+    for (uint32_t i = 0; i < 8; ++i)
+      if (x0 + i < W) zfar = max(zfar, __ldcg(&g[(size_t)y * W + x0 + i]).y >> 8);
+  }
+  zfar = __reduce_max_sync(0xffffffffu, zfar);
+  if (lane == 0) hiz[tile] = zfar;
+}
+
+void launch_hiz(const unsigned long long* gbuf, uint32_t W, uint32_t H, uint32_t* hiz,
+                const unsigned long long* counters, cudaStream_t st) {
+  const uint32_t n_tiles = ((W + HIZ_TILE - 1) / HIZ_TILE) * ((H + HIZ_TILE - 1) / HIZ_TILE);
+  k_hiz<<<(n_tiles + 7) / 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(gbuf), W, H, hiz, counters);
+}
+
 void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_zn, cudaStream_t st) {
   size_t blocks = (n_pixels + 255) / 256;
   if (blocks > 148 * 16) blocks = 148 * 16;
   k_clear<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels, scene_zn);
 }
 
-template <bool COUNT, bool MS, bool PP>
+template <bool COUNT, bool MS, bool PP, bool HZ>
 static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                             const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
-                            unsigned long long* counters, uint32_t ms_k, int n_sm, cudaStream_t st) {
+                            unsigned long long* counters, uint32_t ms_k, uint32_t queue, const uint32_t* hiz, int n_sm,
+                            cudaStream_t st) {
   // persistent grid: every CTA slot of the device, the queue feeds them
   static int per_sm = 0;
   if (!per_sm) {
     int b = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<COUNT, MS, PP>, RAS_WARPS * 32, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<COUNT, MS, PP, HZ>, RAS_WARPS * 32, 0);
     per_sm = b > 0 ? b : 1;
   }
-  k_raster<COUNT, MS, PP><<<(uint32_t)(n_sm * per_sm), RAS_WARPS * 32, 0, st>>>(d_scene, n_bi, table, grp, vertices,
-                                                                                 cam, rho_default, gbuf, counters, ms_k);
+  k_raster<COUNT, MS, PP, HZ><<<(uint32_t)(n_sm * per_sm), RAS_WARPS * 32, 0, st>>>(
+      d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, ms_k, queue, hiz);
 }
 
-// ms_k = 0: the two-layer G-buffer; ms_k in {1, 2, 4, 8}: gbuf = [ms_k][H][W] sample layers (reference mode)
+// ms_k = 0: the two-layer G-buffer; ms_k in {1, 2, 4, 8}: gbuf = [ms_k][H][W] sample layers (reference mode).
+// pass 0 draws the work groups of grp[0 .. n_bi], pass 1 those of the second scan behind it, with the hi-Z test
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
-                   unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int n_sm,
-                   cudaStream_t st) {
-  if (ms_k) launch_raster_t<false, true, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, ms_k, n_sm, st);
-  else if (paper_payload && count) launch_raster_t<true, false, true>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
-  else if (paper_payload) launch_raster_t<false, false, true>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
-  else if (count) launch_raster_t<true, false, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
-  else launch_raster_t<false, false, false>(d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, n_sm, st);
+                   unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int pass,
+                   const uint32_t* hiz, int n_sm, cudaStream_t st) {
+  const uint32_t* gp = grp + (pass ? (size_t)n_bi + 1 : 0);
+  const uint32_t q = pass ? CNT_WORK_RASTER1 : CNT_WORK_RASTER;
+#define RAS_ARGS d_scene, n_bi, table, gp, vertices, cam, rho_default, gbuf, counters
+  if (ms_k) launch_raster_t<false, true, false, false>(RAS_ARGS, ms_k, q, nullptr, n_sm, st);
+  else if (paper_payload && count) launch_raster_t<true, false, true, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);
+  else if (paper_payload && pass) launch_raster_t<false, false, true, true>(RAS_ARGS, 0, q, hiz, n_sm, st);
+  else if (paper_payload) launch_raster_t<false, false, true, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);
+  else if (count) launch_raster_t<true, false, false, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);
+  else if (pass) launch_raster_t<false, false, false, true>(RAS_ARGS, 0, q, hiz, n_sm, st);
+  else launch_raster_t<false, false, false, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);
+#undef RAS_ARGS
 }
 
 // ------------------------------------------------------------------ L2-atomic roofline micro-kernels

@@ -46,7 +46,9 @@ def gpu_frame(binding, sc, lam=None, flags=0, prm_over=None):
     import torch
     assert torch.equal(gb, gb_c), "G-buffer differs between the counted and the production raster"
     assert torch.equal(rgb, rgb_c)
-    assert h.stats()["gpu_launches"] == st["gpu_launches"] - 1
+    # counted frame: + the pixel counter; a production frame drawn in two passes: + the hi-Z and the second raster
+    st_p = h.stats()
+    assert st_p["gpu_launches"] == st["gpu_launches"] - 1 + 2 * st_p["two_pass"]
     out = dict(h=h, gb=binding.gbuffer_to_numpy(gb), rgb=rgb.cpu().numpy().astype(np.float64), stats=st,
                table=h.debug_table().cpu().numpy().view(np.uint32), verts=h.debug_vertices().cpu().numpy(), prm=prm,
                gb_t=gb, rgb_t=rgb)
@@ -508,6 +510,50 @@ def test_paper_payload_stagewise(orc, hair_mod, idx, scale, res_scale, lam, groo
     G0 = gpu_frame(b, sc, lam=lam, prm_over=over)
     assert np.array_equal(G0["gb"] >> np.uint64(40), G["gb"] >> np.uint64(40))
     assert (G0["gb"] != G["gb"]).any()
+
+
+def test_two_depth_ordered_passes_give_the_same_frame(hair_mod):
+    """The production raster draws large frames in two depth-ordered passes with a tile hi-Z between them (the far
+    pass drops occluded segments whole). The resolve is an order-free min and a dropped segment would have lost
+    every pixel, so the frame must equal the one-pass frame bit for bit, whatever the split."""
+    import torch
+    b = hair_mod
+    sc = synth.config(4, scale=0.45, res_scale=0.5)
+    h = b.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(sc["params"], flags=b.FLAG_SINGLE_PASS)
+    g1, r1 = h.render(sc["camera"], sc["lam"])
+    assert h.stats()["two_pass"] == 0
+    h.set_render_params(sc["params"])
+    frames = []
+    for i in range(3):  # depth ranges come from the frame before (the very first frame of a context draws in one pass)
+        g2, r2 = h.render(sc["camera"], sc["lam"])
+        st = h.stats()
+        frames.append((st["two_pass"], st["n_segments_hiz_culled"]))
+        assert torch.equal(g1, g2), (i, st)
+        assert torch.equal(r1, r2)
+    assert frames[1][0] == 1 and frames[2][0] == 1, frames
+    assert frames[2][1] > 0.1 * st["n_segments"], (frames, st["n_segments"])
+    # a moved camera uses the previous frame's ranges: still the same frame as one pass from there
+    cam = dict(sc["camera"])
+    cam["eye"] = [cam["eye"][0] + 0.2, cam["eye"][1] - 0.1, cam["eye"][2] + 0.3]
+    g3, r3 = h.render(cam, sc["lam"])
+    h.set_render_params(sc["params"], flags=b.FLAG_SINGLE_PASS)
+    g4, r4 = h.render(cam, sc["lam"])
+    assert torch.equal(g3, g4) and torch.equal(r3, r4)
+    # scene depth in front of part of the hair, and the paper payload (one groom)
+    H, W = sc["camera"]["height"], sc["camera"]["width"]
+    zn = torch.full((H, W), 0.9, device="cuda")
+    zn[:, W // 3:] = 1.0
+    srgb = torch.rand((H, W, 4), device="cuda")
+    for fl, over in ((0, {}), (b.FLAG_PAPER_PAYLOAD, dict(groom_mask=1))):
+        h.set_render_params(dict(sc["params"], **over), flags=fl | b.FLAG_SINGLE_PASS)
+        a = h.render_scene(sc["camera"], sc["lam"], zn, srgb)
+        h.set_render_params(dict(sc["params"], **over), flags=fl)
+        for i in range(2):
+            c2 = h.render_scene(sc["camera"], sc["lam"], zn, srgb)
+        assert torch.equal(a[0], c2[0]) and torch.equal(a[1], c2[1]), fl
 
 
 def test_sequential_as_first_render_of_a_context(hair_mod):
