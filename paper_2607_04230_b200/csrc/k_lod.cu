@@ -29,48 +29,40 @@ __device__ __forceinline__ uint32_t raster_groups(uint32_t n_v) {  // units of R
 // those depths per instance is accumulated for the NEXT frame (zr_cur) and the range of the PREVIOUS frame (zr_prev)
 // decides which of the two raster passes draws the bundle: the front HIZ_CUT of the range first. Order is a
 // heuristic only — the resolve is an order-free min — so a stale or empty range (first frame: one pass) is fine.
-__global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, uint32_t n_bi, CamDev cam,
-                                             LambdaArr lam, uint32_t groom_mask, uint4* __restrict__ table,
-                                             uint4* __restrict__ part, const uint32_t* __restrict__ zr_prev,
-                                             uint32_t* __restrict__ zr_cur, uint32_t two_pass) {
-  uint32_t gid = blockIdx.x * blockDim.x + threadIdx.x;
-  uint32_t nlod = 0, C = 0, far_pass = 0;
+// Mapping: a CTA of 1024 threads owns a tile of 256 bundle-instances, FOUR lanes per bundle: lane `sub` projects the
+// cage layers sub, sub + 4, ... and the quad combines its bounding boxes with two shuffles (min / max are exact, so
+// the result does not depend on the split); everything after that is computed by all four, written by lane 0.
+__global__ void __launch_bounds__(1024) k_lod(const SceneDev* __restrict__ sc, uint32_t n_bi, CamDev cam,
+                                              LambdaArr lam, uint32_t groom_mask, uint4* __restrict__ table,
+                                              uint4* __restrict__ part, const uint32_t* __restrict__ zr_prev,
+                                              uint32_t* __restrict__ zr_cur, uint32_t two_pass) {
+  const uint32_t sub = threadIdx.x & 3u;
+  const uint32_t gid = blockIdx.x * 256u + (threadIdx.x >> 2);
+  const bool live = gid < n_bi;
+  uint32_t nlod = 0, C = 0, far_pass = 0, gi = 0, rel = 0, N = 0;
   uint32_t inst = 0xFFFFFFFFu;
-  float zmin = 3.0e38f;
-  if (gid < n_bi) {
-  uint32_t gi = 0;
-  for (uint32_t k = 1; k < sc->n_grooms; ++k)
-    if (gid >= sc->g[k].gid_base) gi = k;
-  const GroomDev& g = sc->g[gi];
-  uint32_t rel = gid - g.gid_base;
-  uint32_t q = rel / g.T, t = rel - q * g.T;
-  uint32_t N = __ldg(&g.npt[t]);
-  float lambda = lam.v[gi];
-  inst = g.inst_base + q;
-  if (!(lambda > 0.f)) {  // R14: LOD and culling off
-    nlod = N;
-    C = g.c_full;
-    for (uint32_t i = 0; i < g.Lv; i += g.Lv - 1)  // root and tip layer are enough for an ordering key
-      for (int c = 0; c < 3; ++c) {
-        const float* x = g.pos + ((size_t)i * g.V + __ldg(&g.idx[t * 3 + c])) * 3;
-        float wx = __ldg(x), wy = __ldg(x + 1), wz = __ldg(x + 2);
-        if (g.xform) {
-          const float* M = g.xform + q * 12;
-          const float ax = M[0] * wx + M[1] * wy + M[2] * wz + M[3], ay = M[4] * wx + M[5] * wy + M[6] * wz + M[7];
-          wz = M[8] * wx + M[9] * wy + M[10] * wz + M[11];
-          wx = ax, wy = ay;
-        }
-        zmin = fminf(zmin, (wx - cam.eye[0]) * cam.f[0] + (wy - cam.eye[1]) * cam.f[1] + (wz - cam.eye[2]) * cam.f[2]);
-      }
-  } else {
+  float zmin = 3.0e38f, lambda = 0.f;
+  float mnx = INFINITY, mny = INFINITY, mxx = -INFINITY, mxy = -INFINITY;
+  uint32_t n_valid = 0, n_all = 0;
+  // ---- phase 1 (per lane): this lane's layers of the cage
+  if (live) {
+    for (uint32_t k = 1; k < sc->n_grooms; ++k)
+      if (gid >= sc->g[k].gid_base) gi = k;
+    const GroomDev& g = sc->g[gi];
+    rel = gid - g.gid_base;
+    const uint32_t q = rel / g.T, t = rel - q * g.T;
+    N = __ldg(&g.npt[t]);
+    lambda = lam.v[gi];
+    inst = g.inst_base + q;
+    const bool lod_on = lambda > 0.f;  // R14: else LOD and culling off, only the ordering key is needed
     float M[12];
-    bool has_m = g.xform != nullptr;
+    const bool has_m = g.xform != nullptr;
     if (has_m)
       for (int a = 0; a < 12; ++a) M[a] = __ldg(&g.xform[q * 12 + a]);
-    uint32_t v[3] = {__ldg(&g.idx[t * 3]), __ldg(&g.idx[t * 3 + 1]), __ldg(&g.idx[t * 3 + 2])};
-    float mnx = INFINITY, mny = INFINITY, mxx = -INFINITY, mxy = -INFINITY;
-    uint32_t n_valid = 0, n_all = 0;
-    for (uint32_t i = 0; i < g.Lv; ++i)
+    const uint32_t v[3] = {__ldg(&g.idx[t * 3]), __ldg(&g.idx[t * 3 + 1]), __ldg(&g.idx[t * 3 + 2])};
+    // LOD off: root and tip layer (lanes 0 and 1 of the quad) are enough for an ordering key
+    const uint32_t i_begin = lod_on ? sub : (sub == 0 ? 0u : sub == 1 ? g.Lv - 1 : g.Lv), i_step = lod_on ? 4u : g.Lv;
+    for (uint32_t i = i_begin; i < g.Lv; i += i_step)
       for (int c = 0; c < 3; ++c) {
         const float* x = g.pos + ((size_t)i * g.V + v[c]) * 3;
         float x0 = __ldg(x), x1 = __ldg(x + 1), x2 = __ldg(x + 2);
@@ -91,33 +83,49 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
           mxy = fmaxf(mxy, p.sy);
         }
       }
-    bool culled = false;
-    float L = 1.f;
-    if (n_valid == 0) culled = true;  // R13
-    else if (n_valid == n_all) {
-      float Wf = (float)cam.W, Hf = (float)cam.H;
-      if (mxx < 0.f || mnx > Wf || mxy < 0.f || mny > Hf) culled = true;
-      else {
-        float dx = xsub(mxx, mnx), dy = xsub(mxy, mny);
-        float diag = xsqrt(xadd(xmul(dx, dx), xmul(dy, dy)));
-        L = fminf(fmaxf(xmul(xdiv(diag, Hf), lambda), 0.f), 1.f);  // Eq. 2
+  }
+  // ---- phase 2 (converged): the quad's four partial boxes
+#pragma unroll
+  for (int d = 1; d <= 2; d <<= 1) {
+    mnx = fminf(mnx, __shfl_xor_sync(0xffffffffu, mnx, d));
+    mny = fminf(mny, __shfl_xor_sync(0xffffffffu, mny, d));
+    mxx = fmaxf(mxx, __shfl_xor_sync(0xffffffffu, mxx, d));
+    mxy = fmaxf(mxy, __shfl_xor_sync(0xffffffffu, mxy, d));
+    zmin = fminf(zmin, __shfl_xor_sync(0xffffffffu, zmin, d));
+    n_valid += __shfl_xor_sync(0xffffffffu, n_valid, d);
+    n_all += __shfl_xor_sync(0xffffffffu, n_all, d);
+  }
+  // ---- phase 3 (all four lanes alike, lane 0 writes): Eq. 1-5
+  if (live) {
+    const GroomDev& g = sc->g[gi];
+    if (!(lambda > 0.f)) {  // R14
+      nlod = N;
+      C = g.c_full;
+    } else {
+      bool culled = false;
+      float L = 1.f;
+      if (n_valid == 0) culled = true;  // R13
+      else if (n_valid == n_all) {
+        float Wf = (float)cam.W, Hf = (float)cam.H;
+        if (mxx < 0.f || mnx > Wf || mxy < 0.f || mny > Hf) culled = true;
+        else {
+          float dx = xsub(mxx, mnx), dy = xsub(mxy, mny);
+          float diag = xsqrt(xadd(xmul(dx, dx), xmul(dy, dy)));
+          L = fminf(fmaxf(xmul(xdiv(diag, Hf), lambda), 0.f), 1.f);  // Eq. 2
+        }
+      }
+      if (!culled) {
+        float delta = (float)(pcg(pcg(g.seed_h + rel) + 0xB0u) >> 8) * (1.0f / 16777216.0f);
+        lod_counts(L, N, delta, g.Lv, g.c_full, nlod, C);
+        if (nlod == 0) C = 0;
       }
     }
-    if (culled) {
-      nlod = 0;
-      C = 0;
-    } else {
-      float delta = (float)(pcg(pcg(g.seed_h + rel) + 0xB0u) >> 8) * (1.0f / 16777216.0f);
-      lod_counts(L, N, delta, g.Lv, g.c_full, nlod, C);
-      if (nlod == 0) C = 0;
+    if (!((groom_mask >> gi) & 1u)) nlod = C = 0;  // R-seq: this groom is not drawn in this pass
+    if (two_pass) {
+      const float z0 = __uint_as_float(__ldg(&zr_prev[inst * 2])), z1 = __uint_as_float(__ldg(&zr_prev[inst * 2 + 1]));
+      far_pass = (z1 > z0 && zmin > z0 + HIZ_CUT * (z1 - z0)) ? 1u : 0u;
     }
-  }
-  if (!((groom_mask >> gi) & 1u)) nlod = C = 0;  // R-seq: this groom is not drawn in this pass
-  if (two_pass) {
-    const float z0 = __uint_as_float(__ldg(&zr_prev[inst * 2])), z1 = __uint_as_float(__ldg(&zr_prev[inst * 2 + 1]));
-    far_pass = (z1 > z0 && zmin > z0 + HIZ_CUT * (z1 - z0)) ? 1u : 0u;
-  }
-  table[gid] = make_uint4(nlod, C, far_pass, 0u);  // .z: the pass, until k_scan replaces it by the slot base
+    if (sub == 0) table[gid] = make_uint4(nlod, C, far_pass, 0u);  // .z: the pass, until k_scan replaces it by the slot base
   }
   {  // depth range per instance for the next frame: positive floats order like their bits
     const uint32_t i0 = __shfl_sync(0xffffffffu, inst, 0);
@@ -140,9 +148,10 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
   }
   // sums of this tile of 256 bundle-instances for the scan: strands, vertices, raster work groups, culled
   // part[2 tile] = {strands, vertices, work groups of the near pass, of the far pass}, part[2 tile + 1].x = culled
+  if (sub != 0) nlod = C = 0;  // one lane of the quad counts
   const uint32_t ng = raster_groups(nlod * C);
   uint32_t ts = nlod, tv = nlod * C, tg = far_pass ? 0u : ng, tf = far_pass ? ng : 0u,
-           tc = (gid < n_bi && nlod == 0) ? 1u : 0u;
+           tc = (gid < n_bi && nlod == 0 && sub == 0) ? 1u : 0u;
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) {
     ts += __shfl_xor_sync(0xffffffffu, ts, d);
@@ -151,14 +160,14 @@ __global__ void __launch_bounds__(256) k_lod(const SceneDev* __restrict__ sc, ui
     tf += __shfl_xor_sync(0xffffffffu, tf, d);
     tc += __shfl_xor_sync(0xffffffffu, tc, d);
   }
-  __shared__ uint4 s_w[8];
-  __shared__ uint32_t s_c[8];
+  __shared__ uint4 s_w[32];
+  __shared__ uint32_t s_c[32];
   if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = make_uint4(ts, tv, tg, tf), s_c[threadIdx.x >> 5] = tc;
   __syncthreads();
   if (threadIdx.x == 0) {
     uint4 a = s_w[0];
     uint32_t cc = s_c[0];
-    for (int wv = 1; wv < 8; ++wv) a.x += s_w[wv].x, a.y += s_w[wv].y, a.z += s_w[wv].z, a.w += s_w[wv].w, cc += s_c[wv];
+    for (int wv = 1; wv < 32; ++wv) a.x += s_w[wv].x, a.y += s_w[wv].y, a.z += s_w[wv].z, a.w += s_w[wv].w, cc += s_c[wv];
     part[blockIdx.x * 2] = a;
     part[blockIdx.x * 2 + 1] = make_uint4(cc, 0u, 0u, 0u);
   }
@@ -264,6 +273,6 @@ void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaA
   const uint32_t n_tiles = (n_bi + 255) / 256;
   uint32_t* zr_cur = zrange + (size_t)(parity & 1u) * n_inst * 2;
   uint32_t* zr_prev = zrange + (size_t)((parity + 1u) & 1u) * n_inst * 2;
-  k_lod<<<n_tiles, 256, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table, part, zr_prev, zr_cur, two_pass ? 1u : 0u);
+  k_lod<<<n_tiles, 1024, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table, part, zr_prev, zr_cur, two_pass ? 1u : 0u);
   k_scan<<<n_tiles, 256, 0, st>>>(table, grp, n_bi, part, counters, zr_prev, n_inst, two_pass ? 1u : 0u, want_two_pass);
 }

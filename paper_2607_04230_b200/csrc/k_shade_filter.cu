@@ -228,7 +228,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
   float4* s_item = fsm + NS;                            // [2 * FT_W * FT_H] item, later its result
   uint32_t* s_dqG = reinterpret_cast<uint32_t*>(s_item + 2 * FT_W * FT_H);  // [NS] dq of the centre word
   uint32_t* s_dqA = s_dqG + NS;                                             // [NS] dq of the conservative word
-  __shared__ uint32_t s_n, s_cnt[32];
+  __shared__ uint32_t s_n, s_nc, s_cnt[32];
   const int W = (int)cam.W, H = (int)cam.H;
   const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
   const int x0 = blockIdx.x * FT_W, y0 = blockIdx.y * FT_H;
@@ -284,8 +284,9 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     s_dqG[i] = dG;
     s_dqA[i] = dA;
   }
-  // ---- (2) work items, compacted in pixel order (row by row, centre items of a row first): neighbouring lanes
-  // then walk neighbouring windows and their shared-memory reads fall on distinct banks
+  // ---- (2) work items, compacted by type (all centre items, then all conservative-sample items) and inside a type
+  // in pixel order: neighbouring lanes walk neighbouring windows, their shared-memory reads fall on distinct banks,
+  // and all but one warp hold items of one type, which take the tap loop with / without the colour term
   int slot_c[2] = {-1, -1}, slot_a[2] = {-1, -1};
   bool fly[2] = {false, false};
   float2 Tc[2], Ta[2];
@@ -307,8 +308,8 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     bal[2 * k] = __ballot_sync(0xffffffffu, isCenter);
     bal[2 * k + 1] = __ballot_sync(0xffffffffu, isA);
   }
-  if (lx < 4)  // group = (row of the tile) * 2 + type
-    s_cnt[(lx >> 1) * 16 + ly * 2 + (lx & 1)] = __popc(lx == 0 ? bal[0] : lx == 1 ? bal[1] : lx == 2 ? bal[2] : bal[3]);
+  if (lx < 4)  // group = type * 16 + (row of the tile)
+    s_cnt[(lx & 1) * 16 + (lx >> 1) * 8 + ly] = __popc(lx == 0 ? bal[0] : lx == 1 ? bal[1] : lx == 2 ? bal[2] : bal[3]);
   __syncthreads();
   {
     const uint32_t mine = s_cnt[lx];
@@ -320,9 +321,10 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     }
     if (tid == 31) s_n = incl;
     const uint32_t excl = incl - mine;
+    if (tid == 16) s_nc = excl;  // number of centre items
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
-      const uint32_t base_c = __shfl_sync(0xffffffffu, excl, k * 16 + ly * 2), base_a = __shfl_sync(0xffffffffu, excl, k * 16 + ly * 2 + 1);
+      const uint32_t base_c = __shfl_sync(0xffffffffu, excl, k * 8 + ly), base_a = __shfl_sync(0xffffffffu, excl, 16 + k * 8 + ly);
       const uint32_t pix = (uint32_t)((ly + 8 * k) * FT_W + lx);
       if ((bal[2 * k] >> lx) & 1u) {
         slot_c[k] = (int)(base_c + __popc(bal[2 * k] & lt_mask));
@@ -336,7 +338,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
   }
   __syncthreads();
   // ---- (3) per item (Code 2 PAPER.md:483-515 with DESIGN.md R18-R20)
-  const int n_item = (int)s_n;
+  const int n_item = (int)s_n, n_centre = (int)s_nc;
   const uint32_t tau = sp.tauz_q, tau2 = 2u * sp.tauz_q;
   for (int it = tid; it < n_item; it += 256) {
     const float4 I = s_item[it];
@@ -357,24 +359,49 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
       m = 1.f;
     }
     float S0 = 0.f, S1 = 0.f, S2 = 0.f, Wsum = 0.f;
+    // items are sorted by type: a warp whose 32 items are all conservative-sample items (no colour term, R21 /
+    // PAPER.md:175 w_color = 1) skips the four colour FMAs of every tap
+    const int it0 = it - lx;
+    if (it0 >= n_centre) {
 #pragma unroll 1
-    for (int dy = -R; dy <= R; ++dy) {
-      const float fdy = (float)dy;
-      const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy;
-      const uint32_t* dq_row = s_dqG + ci + dy * SW;
-      const float4* col_row = s_col + ci + dy * SW;
+      for (int dy = -R; dy <= R; ++dy) {
+        const float fdy = (float)dy;
+        const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy;
+        const uint32_t* dq_row = s_dqG + ci + dy * SW;
+        const float4* col_row = s_col + ci + dy * SW;
 #pragma unroll
-      for (int dx = -R; dx <= R; ++dx) {
-        const uint32_t d = dq_row[dx];
-        const float4 q = col_row[dx];
-        const float fdx = (float)dx;
-        float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));                     // Eq. 10 spatial part
-        e = fmaf(c2x, q.x, fmaf(c2y, q.y, fmaf(c2z, q.z, fmaf(m, q.w, e))));  // Eq. 10 colour part
-        const float w = (d - lo <= tau2) ? fast_ex2(e) : 0.f;                 // R19: centre-class taps only
-        S0 = fmaf(w, q.x, S0);
-        S1 = fmaf(w, q.y, S1);
-        S2 = fmaf(w, q.z, S2);
-        Wsum += w;
+        for (int dx = -R; dx <= R; ++dx) {
+          const uint32_t d = dq_row[dx];
+          const float4 q = col_row[dx];
+          const float fdx = (float)dx;
+          const float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));  // Eq. 10 spatial part
+          const float w = (d - lo <= tau2) ? fast_ex2(e) : 0.f;    // R19: centre-class taps only
+          S0 = fmaf(w, q.x, S0);
+          S1 = fmaf(w, q.y, S1);
+          S2 = fmaf(w, q.z, S2);
+          Wsum += w;
+        }
+      }
+    } else {
+#pragma unroll 1
+      for (int dy = -R; dy <= R; ++dy) {
+        const float fdy = (float)dy;
+        const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy;
+        const uint32_t* dq_row = s_dqG + ci + dy * SW;
+        const float4* col_row = s_col + ci + dy * SW;
+#pragma unroll
+        for (int dx = -R; dx <= R; ++dx) {
+          const uint32_t d = dq_row[dx];
+          const float4 q = col_row[dx];
+          const float fdx = (float)dx;
+          float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));                     // Eq. 10 spatial part
+          e = fmaf(c2x, q.x, fmaf(c2y, q.y, fmaf(c2z, q.z, fmaf(m, q.w, e))));  // Eq. 10 colour part
+          const float w = (d - lo <= tau2) ? fast_ex2(e) : 0.f;                 // R19: centre-class taps only
+          S0 = fmaf(w, q.x, S0);
+          S1 = fmaf(w, q.y, S1);
+          S2 = fmaf(w, q.z, S2);
+          Wsum += w;
+        }
       }
     }
     // ---- loop B: strip hit counts by Q's class (R18), in (major, minor) coordinates of the tangent: Eq. 9 is
