@@ -342,6 +342,10 @@ def run_cuda(args):
         "counts": {k: cnt[k] for k in ("n_bundles", "n_bundles_culled", "n_strands_total", "n_strands_lod", "n_vertices",
                                        "n_segments", "n_segments_drawn", "n_segments_live", "n_atomics_center", "n_atomics_cons",
                                        "n_atomics_issued", "n_pixels_center", "n_pixels_cons")},
+        "raster_passes": {"two_pass": st["two_pass"], "n_segments_hiz_culled": st["n_segments_hiz_culled"],
+                          "what": "production frames: bundles in the front 60 % of their groom's depth range first, 16x16-tile "
+                                  "hi-Z (k_hiz), then the rest; a segment behind every tile of its bounding box is dropped "
+                                  "before any pixel work (same G-buffer bit for bit; DESIGN.md 7.3)"},
         "sequential_per_groom": {"ms_per_step": ms_seq, "what": "hair_render_sequential: one LOD..filter pass per groom, "
                                  "depth kept, blended over the target (PAPER.md:208-210); the headline frame resolves "
                                  "all grooms in one G-buffer instead (DESIGN.md R15)"},

@@ -228,7 +228,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
   float4* s_item = fsm + NS;                            // [2 * FT_W * FT_H] item, later its result
   uint32_t* s_dqG = reinterpret_cast<uint32_t*>(s_item + 2 * FT_W * FT_H);  // [NS] dq of the centre word
   uint32_t* s_dqA = s_dqG + NS;                                             // [NS] dq of the conservative word
-  __shared__ uint32_t s_n, s_nc, s_cnt[32];
+  __shared__ uint32_t s_cc[2][8][FT_H], s_tot[16];
   const int W = (int)cam.W, H = (int)cam.H;
   const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
   const int x0 = blockIdx.x * FT_W, y0 = blockIdx.y * FT_H;
@@ -284,9 +284,12 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     s_dqG[i] = dG;
     s_dqA[i] = dA;
   }
-  // ---- (2) work items, compacted by type (all centre items, then all conservative-sample items) and inside a type
-  // in pixel order: neighbouring lanes walk neighbouring windows, their shared-memory reads fall on distinct banks,
-  // and all but one warp hold items of one type, which take the tap loop with / without the colour term
+  // ---- (2) work items, compacted by type (all centre items, then all conservative-sample items: all but one warp
+  // hold items of one type, which take the tap loop with / without the colour term) and, inside a type, DEALT BY BANK
+  // CLASS: the 16-byte bank group a tap read of pixel (x, y) falls on is (x + (SW mod 8) y + const) mod 8, the same
+  // constant for every lane, so slot = rank * 8 + class puts eight different bank groups in every quarter warp
+  // whatever pixels the items sit on (sparse fly-away / promoted items were 2-way conflicted when merely packed in
+  // pixel order). Classes fill unevenly; the few slots left empty are skipped.
   int slot_c[2] = {-1, -1}, slot_a[2] = {-1, -1};
   bool fly[2] = {false, false};
   float2 Tc[2], Ta[2];
@@ -308,42 +311,52 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     bal[2 * k] = __ballot_sync(0xffffffffu, isCenter);
     bal[2 * k + 1] = __ballot_sync(0xffffffffu, isA);
   }
-  if (lx < 4)  // group = type * 16 + (row of the tile)
-    s_cnt[(lx & 1) * 16 + (lx >> 1) * 8 + ly] = __popc(lx == 0 ? bal[0] : lx == 1 ? bal[1] : lx == 2 ? bal[2] : bal[3]);
-  __syncthreads();
+  constexpr int KS = SW & 7;  // bank-group step of one tile row
   {
-    const uint32_t mine = s_cnt[lx];
-    uint32_t incl = mine;
+    // counts per (type, class, row): lane l of warp ly reports k = l >> 4, type = (l >> 3) & 1, class = l & 7
+    const int rk = lx >> 4, rt = (lx >> 3) & 1, rc = lx & 7, rrow = ly + 8 * rk;
+    const uint32_t rb = rk ? (rt ? bal[3] : bal[2]) : (rt ? bal[1] : bal[0]);
+    s_cc[rt][rc][rrow] = __popc(rb & (0x01010101u << ((rc - KS * rrow) & 7)));
+  }
+  __syncthreads();
+  if (tid < 16) {
+    uint32_t t = 0;
 #pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const uint32_t up = __shfl_up_sync(0xffffffffu, incl, d);
-      if (lx >= d) incl += up;
+    for (int r = 0; r < FT_H; ++r) t += s_cc[tid >> 3][tid & 7][r];
+    s_tot[tid] = t;
+  }
+  __syncthreads();
+  uint32_t max_c = 0, max_a = 0;
+#pragma unroll
+  for (int c = 0; c < 8; ++c) max_c = max(max_c, s_tot[c]), max_a = max(max_a, s_tot[8 + c]);
+  const int n_centre = (int)((8u * max_c + 31u) & ~31u);  // centre slots, rounded up to whole warps
+  const int n_item = n_centre + (int)(8u * max_a);
+  for (int i = tid; i < n_item; i += 256) s_item[i].w = __uint_as_float(0xFFFFFFFFu);  // empty slot
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const int row = ly + 8 * k, cls = (lx + KS * row) & 7;
+    const uint32_t same = 0x01010101u << (lx & 7);  // the four lanes of this row in my class
+    const uint32_t pix = (uint32_t)(row * FT_W + lx);
+    uint32_t before_c = 0, before_a = 0;
+    for (int r = 0; r < row; ++r) before_c += s_cc[0][cls][r], before_a += s_cc[1][cls][r];
+    if ((bal[2 * k] >> lx) & 1u) {
+      slot_c[k] = (int)((before_c + __popc(bal[2 * k] & same & lt_mask)) * 8u) + cls;
+      s_item[slot_c[k]] = make_float4(Tc[k].x, Tc[k].y, __uint_as_float(w_dq(G[k]) | 0x1000000u), __uint_as_float(pix));
     }
-    if (tid == 31) s_n = incl;
-    const uint32_t excl = incl - mine;
-    if (tid == 16) s_nc = excl;  // number of centre items
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const uint32_t base_c = __shfl_sync(0xffffffffu, excl, k * 8 + ly), base_a = __shfl_sync(0xffffffffu, excl, 16 + k * 8 + ly);
-      const uint32_t pix = (uint32_t)((ly + 8 * k) * FT_W + lx);
-      if ((bal[2 * k] >> lx) & 1u) {
-        slot_c[k] = (int)(base_c + __popc(bal[2 * k] & lt_mask));
-        s_item[slot_c[k]] = make_float4(Tc[k].x, Tc[k].y, __uint_as_float(w_dq(G[k]) | 0x1000000u), __uint_as_float(pix));
-      }
-      if ((bal[2 * k + 1] >> lx) & 1u) {
-        slot_a[k] = (int)(base_a + __popc(bal[2 * k + 1] & lt_mask));
-        s_item[slot_a[k]] = make_float4(Ta[k].x, Ta[k].y, __uint_as_float(w_dq(A[k])), __uint_as_float(pix));
-      }
+    if ((bal[2 * k + 1] >> lx) & 1u) {
+      slot_a[k] = n_centre + (int)((before_a + __popc(bal[2 * k + 1] & same & lt_mask)) * 8u) + cls;
+      s_item[slot_a[k]] = make_float4(Ta[k].x, Ta[k].y, __uint_as_float(w_dq(A[k])), __uint_as_float(pix));
     }
   }
   __syncthreads();
   // ---- (3) per item (Code 2 PAPER.md:483-515 with DESIGN.md R18-R20)
-  const int n_item = (int)s_n, n_centre = (int)s_nc;
   const uint32_t tau = sp.tauz_q, tau2 = 2u * sp.tauz_q;
   for (int it = tid; it < n_item; it += 256) {
     const float4 I = s_item[it];
     const float Tx = I.x, Ty = I.y;
     const uint32_t rm = __float_as_uint(I.z), pix = __float_as_uint(I.w);
+    if (pix == 0xFFFFFFFFu) continue;  // empty slot of an under-filled bank class
     // R20: class by integer depth compare, |d - ref| <= tau as (unsigned)(d - (ref - tau)) <= 2 tau (mod 2^32);
     // DQ_NONE is farther than tau (<= 2^24) from every depth
     const uint32_t lo = (rm & 0xFFFFFFu) - tau;
