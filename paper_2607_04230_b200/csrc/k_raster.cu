@@ -393,21 +393,25 @@ void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st) {
   k_reseed<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels);
 }
 
-// farthest centre depth of every HIZ_TILE x HIZ_TILE pixel tile (a warp per tile; lane = half a row of the tile).
+// farthest centre depth of every HIZ_TILE x HIZ_TILE pixel tile. A warp per tile: lanes 0-15 read the 16 words of
+// one tile row, lanes 16-31 those of the next (two coalesced 256-byte runs per load), eight loads cover the tile.
 // A pixel without a centre hit keeps the depth it was cleared / seeded with (all ones = never occludes).
 __global__ void __launch_bounds__(256) k_hiz(const uint4* __restrict__ g, uint32_t W, uint32_t H,
                                              uint32_t* __restrict__ hiz, const unsigned long long* __restrict__ counters) {
+  static_assert(HIZ_TILE == 16, "k_hiz maps 16 lanes to a tile row");
   if (__ldcg(&counters[CNT_HIZ_ON]) == 0ull) return;  // one-pass frame (decided on the device by k_scan)
   const uint32_t tw = (W + HIZ_TILE - 1) / HIZ_TILE, th = (H + HIZ_TILE - 1) / HIZ_TILE;
   const uint32_t tile = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (tile >= tw * th) return;
   const uint32_t ty = tile / tw, tx = tile - ty * tw;
-  const uint32_t y = ty * HIZ_TILE + (lane >> 1), x0 = tx * HIZ_TILE + (lane & 1u) * 8u;
+  const uint32_t x = tx * HIZ_TILE + (lane & 15u), y0 = ty * HIZ_TILE + (lane >> 4);
   uint32_t zfar = 0;
-  if (y < H) {
+  if (x < W) {
 #pragma unroll
-    for (uint32_t i = 0; i < 8; ++i)
-      if (x0 + i < W) zfar = max(zfar, __ldcg(&g[(size_t)y * W + x0 + i]).y >> 8);
+    for (uint32_t i = 0; i < 8; ++i) {
+      const uint32_t y = y0 + 2 * i;
+      if (y < H) zfar = max(zfar, __ldcg(reinterpret_cast<const uint32_t*>(g) + ((size_t)y * W + x) * 4 + 1) >> 8);
+    }
   }
   zfar = __reduce_max_sync(0xffffffffu, zfar);
   if (lane == 0) hiz[tile] = zfar;
