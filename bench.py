@@ -274,14 +274,15 @@ def run_cuda(args):
     dom = max(("generate", "clear", "raster", "shade", "filter"), key=lambda k: stages[k]["ms"])
     d = stages[dom]
     # Issue-slot ("alu") view of the two kernels that ncu shows are bound by instruction issue, not by memory:
-    # warp instructions per algorithmic unit from the committed ncu capture (profiles/r1_v4_ncu_full.md,
+    # warp instructions per algorithmic unit from the committed ncu capture (profiles/r1_v5_ncu_full.md,
     # smsp__inst_executed.sum / units of that frame) x the units this run counted, over the live CUDA-event time,
-    # against 148 SMs x 4 schedulers x 1 warp instruction per clock (DESIGN.md 7.2).
+    # against 148 SMs x 4 schedulers x 1 warp instruction per clock (DESIGN.md 7.5).
     sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
     issue_peak = n_sm * 4 * sm_mhz * 1e6 / 1e9  # G warp-instructions / s
     n_items = cnt["n_pixels_cons"]  # one filter item per hit pixel (+ one per fly-away pixel, not counted here)
-    inst_per_unit = {"raster": (779185260 / 219609409, n_at, "predicate-true hit"),
-                     "filter": (514264854 / 3024726, n_items, "hit pixel")}
+    # raster = near pass + k_hiz + far pass of the two-pass frame
+    inst_per_unit = {"raster": ((465459314 + 4244400 + 129536574) / 219609409, n_at, "predicate-true hit"),
+                     "filter": (448452440 / 3024726, n_items, "hit pixel")}
     if not (args.config == 4 and args.scale == 1.0 and args.res_scale == 1.0):
         inst_per_unit = {}  # the per-unit instruction counts were captured on the bench frame only
     for k, (ipu, units, what) in inst_per_unit.items():
@@ -289,8 +290,9 @@ def run_cuda(args):
         stg["warp_inst"] = ipu * units
         stg["Gwarp_inst_per_s"] = ipu * units / (stg["ms"] * 1e-3) / 1e9
         stg["frac_issue"] = stg["Gwarp_inst_per_s"] / issue_peak
-        stg["inst_per_unit"] = f"{ipu:.2f} warp instructions per {what} (ncu, profiles/r1_v4_ncu_full.md)"
-    dram = {"generate": 105192960, "raster": 242107392, "shade": 200795392, "filter": 311533568}  # ncu dram read+write per launch, same capture
+        stg["inst_per_unit"] = f"{ipu:.2f} warp instructions per {what} (ncu, profiles/r1_v5_ncu_full.md)"
+    # ncu dram read + write per frame, same capture (raster: near pass 156.6 MB + k_hiz 136.2 MB + far pass 83.7 MB)
+    dram = {"generate": 103936256, "raster": 376465152, "shade": 200673536, "filter": 311624448}
     if dom in inst_per_unit:
         roofline = {"kernel": "k_" + dom, "bound": "alu", "achieved": d["Gwarp_inst_per_s"], "peak": issue_peak,
                     "unit": "Gwarp-inst/s", "frac": d["frac_issue"], "traffic": dram.get(dom),
