@@ -224,11 +224,14 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
          const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
   constexpr int SW = FT_W + 2 * R, SH = FT_H + 2 * R, NS = SW * SH;
   extern __shared__ float4 fsm[];
-  float4* s_col = fsm;                                  // [NS] rgb, -kC |rgb|^2 (zeros where no centre hit)
+  float4* s_col = fsm;                                  // [NS] rgb (zeros where no centre hit), dq of the centre word
   float4* s_item = fsm + NS;                            // [2 * FT_W * FT_H] item, later its result
   uint32_t* s_dqG = reinterpret_cast<uint32_t*>(s_item + 2 * FT_W * FT_H);  // [NS] dq of the centre word
   uint32_t* s_dqA = s_dqG + NS;                                             // [NS] dq of the conservative word
-  __shared__ uint32_t s_cc[2][8][FT_H], s_tot[16];
+  float* s_k2 = reinterpret_cast<float*>(s_dqA + NS);                       // [NS] -kC |rgb|^2 (Eq. 10 colour term)
+  // (the centre depth sits both in s_col.w, where the tap loop gets it with the colour in one LDS.128 — the loop of
+  // the conservative-sample items then reads nothing else — and in s_dqG, whose 4-byte stride suits the strip loop)
+  __shared__ uint32_t s_cc[2][FT_H + 1][8];  // items per (type, row, class); then their exclusive prefix over rows
   const int W = (int)cam.W, H = (int)cam.H;
   const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
   const int x0 = blockIdx.x * FT_W, y0 = blockIdx.y * FT_H;
@@ -270,6 +273,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     const int gx = x0 + sx - R, gy = y0 + sy - R;
     uint32_t dG = DQ_NONE, dA = DQ_NONE;
     float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    float k2 = 0.f;
     if (gx >= 0 && gx < W && gy >= 0 && gy < H) {  // samples outside the image do not exist
       const size_t q = (size_t)gy * W + gx;
       const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + q);
@@ -277,10 +281,13 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
       if (!w_none(raw.x, raw.y)) {
         dG = raw.y >> 8;
         const float4 c = __ldg(&colour[q]);
-        c4 = make_float4(c.x, c.y, c.z, -sp.kC * (c.x * c.x + c.y * c.y + c.z * c.z));
+        c4 = make_float4(c.x, c.y, c.z, 0.f);
+        k2 = -sp.kC * (c.x * c.x + c.y * c.y + c.z * c.z);
       }
     }
+    c4.w = __uint_as_float(dG);
     s_col[i] = c4;
+    s_k2[i] = k2;
     s_dqG[i] = dG;
     s_dqA[i] = dA;
   }
@@ -316,19 +323,23 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     // counts per (type, class, row): lane l of warp ly reports k = l >> 4, type = (l >> 3) & 1, class = l & 7
     const int rk = lx >> 4, rt = (lx >> 3) & 1, rc = lx & 7, rrow = ly + 8 * rk;
     const uint32_t rb = rk ? (rt ? bal[3] : bal[2]) : (rt ? bal[1] : bal[0]);
-    s_cc[rt][rc][rrow] = __popc(rb & (0x01010101u << ((rc - KS * rrow) & 7)));
+    s_cc[rt][rrow][rc] = __popc(rb & (0x01010101u << ((rc - KS * rrow) & 7)));
   }
   __syncthreads();
-  if (tid < 16) {
+  if (tid < 16) {  // exclusive prefix over the rows, total in row FT_H
     uint32_t t = 0;
 #pragma unroll
-    for (int r = 0; r < FT_H; ++r) t += s_cc[tid >> 3][tid & 7][r];
-    s_tot[tid] = t;
+    for (int r = 0; r < FT_H; ++r) {
+      const uint32_t n = s_cc[tid >> 3][r][tid & 7];
+      s_cc[tid >> 3][r][tid & 7] = t;
+      t += n;
+    }
+    s_cc[tid >> 3][FT_H][tid & 7] = t;
   }
   __syncthreads();
   uint32_t max_c = 0, max_a = 0;
 #pragma unroll
-  for (int c = 0; c < 8; ++c) max_c = max(max_c, s_tot[c]), max_a = max(max_a, s_tot[8 + c]);
+  for (int c = 0; c < 8; ++c) max_c = max(max_c, s_cc[0][FT_H][c]), max_a = max(max_a, s_cc[1][FT_H][c]);
   const int n_centre = (int)((8u * max_c + 31u) & ~31u);  // centre slots, rounded up to whole warps
   const int n_item = n_centre + (int)(8u * max_a);
   for (int i = tid; i < n_item; i += 256) s_item[i].w = __uint_as_float(0xFFFFFFFFu);  // empty slot
@@ -338,8 +349,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     const int row = ly + 8 * k, cls = (lx + KS * row) & 7;
     const uint32_t same = 0x01010101u << (lx & 7);  // the four lanes of this row in my class
     const uint32_t pix = (uint32_t)(row * FT_W + lx);
-    uint32_t before_c = 0, before_a = 0;
-    for (int r = 0; r < row; ++r) before_c += s_cc[0][cls][r], before_a += s_cc[1][cls][r];
+    const uint32_t before_c = s_cc[0][row][cls], before_a = s_cc[1][row][cls];
     if ((bal[2 * k] >> lx) & 1u) {
       slot_c[k] = (int)((before_c + __popc(bal[2 * k] & same & lt_mask)) * 8u) + cls;
       s_item[slot_c[k]] = make_float4(Tc[k].x, Tc[k].y, __uint_as_float(w_dq(G[k]) | 0x1000000u), __uint_as_float(pix));
@@ -368,7 +378,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     if (rm >> 24) {  // centre sample: colour term on; its own tap has weight 1, so no bias is needed
       const float4 CP = s_col[ci];
       c2x = 2.f * sp.kC * CP.x, c2y = 2.f * sp.kC * CP.y, c2z = 2.f * sp.kC * CP.z;
-      e0 = CP.w;
+      e0 = s_k2[ci];
       m = 1.f;
     }
     float S0 = 0.f, S1 = 0.f, S2 = 0.f, Wsum = 0.f;
@@ -380,12 +390,11 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
       for (int dy = -R; dy <= R; ++dy) {
         const float fdy = (float)dy;
         const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy;
-        const uint32_t* dq_row = s_dqG + ci + dy * SW;
         const float4* col_row = s_col + ci + dy * SW;
 #pragma unroll
         for (int dx = -R; dx <= R; ++dx) {
-          const uint32_t d = dq_row[dx];
           const float4 q = col_row[dx];
+          const uint32_t d = __float_as_uint(q.w);
           const float fdx = (float)dx;
           const float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));  // Eq. 10 spatial part
           const float w = (d - lo <= tau2) ? fast_ex2(e) : 0.f;    // R19: centre-class taps only
@@ -400,15 +409,16 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
       for (int dy = -R; dy <= R; ++dy) {
         const float fdy = (float)dy;
         const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy;
-        const uint32_t* dq_row = s_dqG + ci + dy * SW;
+        const float* k2_row = s_k2 + ci + dy * SW;
         const float4* col_row = s_col + ci + dy * SW;
 #pragma unroll
         for (int dx = -R; dx <= R; ++dx) {
-          const uint32_t d = dq_row[dx];
+          const float k2 = k2_row[dx];
           const float4 q = col_row[dx];
+          const uint32_t d = __float_as_uint(q.w);
           const float fdx = (float)dx;
           float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));                     // Eq. 10 spatial part
-          e = fmaf(c2x, q.x, fmaf(c2y, q.y, fmaf(c2z, q.z, fmaf(m, q.w, e))));  // Eq. 10 colour part
+          e = fmaf(c2x, q.x, fmaf(c2y, q.y, fmaf(c2z, q.z, fmaf(m, k2, e))));   // Eq. 10 colour part
           const float w = (d - lo <= tau2) ? fast_ex2(e) : 0.f;                 // R19: centre-class taps only
           S0 = fmaf(w, q.x, S0);
           S1 = fmaf(w, q.y, S1);
@@ -551,7 +561,7 @@ static void launch_filter_r(const SceneDev* d_scene, const uint2* srec, const fl
                             ShadeParams sp, const unsigned long long* gbuf, const float4* colour,
                             const float4* scene_rgb, float4* out, cudaStream_t st) {
   constexpr int NS = (FT_W + 2 * R) * (FT_H + 2 * R);
-  constexpr size_t smem = (size_t)NS * (sizeof(float4) + 2 * sizeof(uint32_t)) + 2 * FT_W * FT_H * sizeof(float4);
+  constexpr size_t smem = (size_t)NS * (sizeof(float4) + 3 * sizeof(uint32_t)) + 2 * FT_W * FT_H * sizeof(float4);
   cudaFuncSetAttribute(k_filter<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   dim3 grid((cam.W + FT_W - 1) / FT_W, (cam.H + FT_H - 1) / FT_H);
   k_filter<R><<<grid, 256, smem, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out);
