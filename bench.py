@@ -282,7 +282,7 @@ def run_cuda(args):
     n_items = cnt["n_pixels_cons"]  # one filter item per hit pixel (+ one per fly-away pixel, not counted here)
     # raster = near pass + k_hiz + far pass of the two-pass frame
     inst_per_unit = {"raster": ((465459314 + 4244400 + 129536574) / 219609409, n_at, "predicate-true hit"),
-                     "filter": (448452440 / 3024726, n_items, "hit pixel")}
+                     "filter": (439092496 / 3024726, n_items, "hit pixel")}
     if not (args.config == 4 and args.scale == 1.0 and args.res_scale == 1.0):
         inst_per_unit = {}  # the per-unit instruction counts were captured on the bench frame only
     for k, (ipu, units, what) in inst_per_unit.items():
@@ -292,7 +292,7 @@ def run_cuda(args):
         stg["frac_issue"] = stg["Gwarp_inst_per_s"] / issue_peak
         stg["inst_per_unit"] = f"{ipu:.2f} warp instructions per {what} (ncu, profiles/r1_v5_ncu_full.md)"
     # ncu dram read + write per frame, same capture (raster: near pass 156.6 MB + k_hiz 136.2 MB + far pass 83.7 MB)
-    dram = {"generate": 103936256, "raster": 376465152, "shade": 200673536, "filter": 311624448}
+    dram = {"generate": 103936256, "raster": 376465152, "shade": 200673536, "filter": 311918080}
     if dom in inst_per_unit:
         roofline = {"kernel": "k_" + dom, "bound": "alu", "achieved": d["Gwarp_inst_per_s"], "peak": issue_peak,
                     "unit": "Gwarp-inst/s", "frac": d["frac_issue"], "traffic": dram.get(dom),
