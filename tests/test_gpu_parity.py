@@ -49,7 +49,7 @@ def gpu_frame(binding, sc, lam=None, flags=0, prm_over=None):
     # counted frame: + the pixel counter; a production frame drawn in two passes: + the hi-Z and the second raster
     st_p = h.stats()
     assert st_p["gpu_launches"] == st["gpu_launches"] - 1 + 2 * st_p["two_pass"]
-    out = dict(h=h, gb=binding.gbuffer_to_numpy(gb), rgb=rgb.cpu().numpy().astype(np.float64), stats=st,
+    out = dict(h=h, stats_prod=st_p, gb=binding.gbuffer_to_numpy(gb), rgb=rgb.cpu().numpy().astype(np.float64), stats=st,
                table=h.debug_table().cpu().numpy().view(np.uint32), verts=h.debug_vertices().cpu().numpy(), prm=prm,
                gb_t=gb, rgb_t=rgb)
     return out
@@ -157,12 +157,13 @@ def test_end_to_end_pure_oracle_vs_pure_gpu(orc, hair_mod):
     assert psnr(out[..., :3], G["rgb"][..., :3], max(out[..., :3].max(), 1.0)) > 45.0
 
 
-def check_full_size_sampled(orc, sc, G, windows):
+def check_full_size_sampled(orc, sc, G, windows, payload=False):
     """A frame at BASELINE.json's full size: table and all vertices against the oracle, then the oracle's
     pixel stages on WINDOWS of the frame (oracle.Frame.set_window: pixels are independent, so a window of
     the oracle's output equals the same window of its full-frame run)."""
     cam, prm = sc["camera"], G["prm"]
     f = orc.Frame(sc["grooms"])
+    f.set_payload_mode(payload)
     f.lod(cam, sc["lam"])
     t_or, _ = f.table()
     assert np.array_equal(t_or, G["table"]), "bundle table differs"
@@ -215,6 +216,8 @@ def test_bench_frame_full_size_sampled(orc, hair_mod):
                (cx(0.88) - 40, H // 2 - 40, cx(0.88) + 40, H // 2 + 40)]        # groom 4, sub-pixel segments
     rep = check_full_size_sampled(orc, sc, G, windows)
     assert rep["n_hit"] > 0.3 * rep["n_px"], rep  # the windows do sit on hair
+    # the production frame compared here was drawn the way bench.py times it: two depth-ordered raster passes
+    assert G["stats_prod"]["two_pass"] == 1 and G["stats_prod"]["n_segments_hiz_culled"] > 2000000, G["stats_prod"]
 
 
 def _densest_windows(G, cell, n):
@@ -236,6 +239,14 @@ def test_single_groom_full_size_sampled(orc, hair_mod):
     G = gpu_frame(hair_mod, sc)
     assert G["stats"]["n_segments"] == 50000 * 32
     rep = check_full_size_sampled(orc, sc, G, _densest_windows(G, 120, 8))
+    assert rep["n_hit"] > 5000, rep
+
+
+def test_single_groom_full_size_sampled_paper_payload(orc, hair_mod):
+    """BASELINE config 2 as named with the paper's word (R-payload): words bit-exact and RGB on windows."""
+    sc = synth.config(2)
+    G = gpu_frame(hair_mod, sc, flags=hair_mod.FLAG_PAPER_PAYLOAD)
+    rep = check_full_size_sampled(orc, sc, G, _densest_windows(G, 120, 6), payload=True)
     assert rep["n_hit"] > 5000, rep
 
 
