@@ -56,6 +56,12 @@ extern "C" {
  * hi-Z between them, which drops occluded segments of the second pass before any pixel work; the G-buffer is the
  * same bit for bit (the resolve is an order-free min). For A/B measurements. */
 #define HAIR_FLAG_SINGLE_PASS 16u
+/* Fused generation + raster (the paper's own arrangement: "strand vertices stay in
+ * registers"): no vertex buffer is written; the raster's warps build the bundle's spline table and generate the
+ * vertices they draw (the very code k_generate runs, so the words equal the materialised frame's bit for bit).
+ * Requires HAIR_FLAG_PAPER_PAYLOAD (the strand-id word is shaded from the vertex buffer): otherwise
+ * HAIR_E_INVALID_ARG. The debug vertex buffer is not valid after such a frame. An A/B against the default pipeline. */
+#define HAIR_FLAG_FUSED 32u
 
 typedef struct hair_ctx hair_ctx; /* opaque; owns all device scratch */
 

@@ -36,7 +36,7 @@ def _stale(target: str, deps: list[str]) -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    headers = [os.path.join(CSRC, "hair_internal.cuh"), os.path.join(INCLUDE, "hair.h")]
+    headers = [os.path.join(CSRC, "hair_internal.cuh"), os.path.join(CSRC, "gen_device.cuh"), os.path.join(INCLUDE, "hair.h")]
     nvcc = _nvcc()
     objs, jobs = [], []
     for s in SOURCES:

@@ -282,6 +282,11 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
       return fail(c, HAIR_E_INVALID_ARG, "HAIR_FLAG_PAPER_PAYLOAD: exactly one groom per pass (groom_mask, or hair_render_sequential)");
     while (!((active >> sp.pp_groom) & 1u)) ++sp.pp_groom;
   }
+  // the raster generates its own vertices (no vertex buffer); only the paper payload shades without one
+  const bool fused = (c->prm.flags & HAIR_FLAG_FUSED) != 0;
+  if (fused && (!pp || (c->prm.flags & HAIR_FLAG_COUNTERS)))
+    return fail(c, HAIR_E_INVALID_ARG, "HAIR_FLAG_FUSED needs HAIR_FLAG_PAPER_PAYLOAD and no HAIR_FLAG_COUNTERS");
+  if (fused && !front) return fail(c, HAIR_E_INVALID_ARG, "hair_render_stages: not with HAIR_FLAG_FUSED");
   const bool timed = (c->prm.flags & HAIR_FLAG_STAGE_TIMING) != 0;
   const bool count = (c->prm.flags & HAIR_FLAG_COUNTERS) != 0;
   const uint32_t n_bi = c->scene.n_bi;
@@ -324,7 +329,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
     launches += 2;
   }
   mark(EV_LOD);
-  if (front && n_bi) {
+  if (front && n_bi && !fused) {
     launch_generate(c->d_scene, n_bi, c->d_table, c->d_vertices, c->d_srec, c->d_counters, c->c_max, c->n_sm, st);
     ++launches;
   }
@@ -342,12 +347,12 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
       CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER1, 0, sizeof(unsigned long long), st));
     }
     launch_raster(c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters,
-                  count && !po.ms_k, po.ms_k, pp, 0, nullptr, c->n_sm, st);
+                  count && !po.ms_k, po.ms_k, pp, 0, nullptr, c->n_sm, st, fused ? c->c_max : 0u);
     ++launches;
     if (two_pass || (!front && c->last_two_pass)) {
       launch_hiz(gbuf, w, h, c->d_hiz, c->d_counters, st);
       launch_raster(c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters,
-                    false, 0, pp, 1, c->d_hiz, c->n_sm, st);
+                    false, 0, pp, 1, c->d_hiz, c->n_sm, st, fused ? c->c_max : 0u);
       launches += 2;
     }
   }

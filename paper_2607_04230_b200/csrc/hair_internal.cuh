@@ -230,7 +230,7 @@ void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                    unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int pass,
-                   const uint32_t* hiz, int n_sm, cudaStream_t st);
+                   const uint32_t* hiz, int n_sm, cudaStream_t st, uint32_t fused_c_max = 0);
 void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
                          float4* out, cudaStream_t st);

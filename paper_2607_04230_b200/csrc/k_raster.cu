@@ -14,7 +14,7 @@
 // (segment, major-axis column) pairs evenly over its lanes: a shuffle scan of the column counts,
 // then per 32 tasks one ballot + one REDUX.OR locate every lane's segment. Each task walks the 1-3
 // pixels of its column; long and sub-pixel segments cost the same per pixel.
-#include "hair_internal.cuh"
+#include "gen_device.cuh"
 
 #ifndef RAS_WARPS
 #define RAS_WARPS 8
@@ -60,12 +60,17 @@ __constant__ int c_ms_off[4][8][2] = {  // sample offsets from the pixel centre 
 // depth of every 16 x 16 pixel tile; the second pass drops a segment before any pixel work when its nearest depth
 // lies behind that bound in every tile its bounding box touches — every one of its pixels would have failed the
 // per-pixel early reject below, so the result is the same G-buffer, bit for bit.
-template <bool COUNT, bool MS, bool PP, bool HZ>
-__global__ void __launch_bounds__(RAS_WARPS * 32, RAS_MIN_BLOCKS)
+// FUSED ("strand vertices stay in registers"): no vertex buffer. The warp builds the
+// per-bundle spline table of its work group in shared memory (gen::build_table, the code k_generate runs) and every
+// lane GENERATES the vertex it would have loaded (gen::vertex: same source, same bits). Needs the paper payload (the
+// strand-id word is shaded from the vertex buffer). An A/B against the materialised pipeline.
+template <bool COUNT, bool MS, bool PP, bool HZ, bool FUSED = false>
+__global__ void __launch_bounds__(RAS_WARPS * 32, FUSED ? 2 : RAS_MIN_BLOCKS)
 k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
          const uint32_t* __restrict__ grp, const float4* __restrict__ vertices, CamDev cam, float rho_default,
          unsigned long long* __restrict__ gbuf, unsigned long long* __restrict__ counters, uint32_t ms_k,
-         uint32_t queue, const uint32_t* __restrict__ hiz) {
+         uint32_t queue, const uint32_t* __restrict__ hiz, uint32_t c_max) {
+  static_assert(!FUSED || (PP && !COUNT && !MS), "the fused raster writes the paper payload only");
   constexpr int RS = PP ? REC_STRIDE_PP : REC_STRIDE;
   __shared__ __align__(16) float s_rec[RAS_WARPS][32][RS];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -108,12 +113,34 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
     const uint32_t v_begin = (wi - __ldg(&grp[gid])) * (RAS_GROUP * RAS_CHUNK);
     const uint32_t v_end = min(v_begin + RAS_GROUP * RAS_CHUNK, n_v - 1);  // first vertex of the next group
     float4 p_next = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (v_begin + lane < n_v) p_next = __ldg(&vin[v_begin + lane]);
+    float* tab = nullptr;
+    float M[12];
+    bool has_m = false;
+    if constexpr (FUSED) {  // the bundle's spline table, once per work group
+      extern __shared__ float4 s_tab[];
+      tab = reinterpret_cast<float*>(s_tab) + (size_t)warp * c_max * HAIR_ROW;
+      gen::build_table(g, t, C, tab, lane);
+      has_m = g.xform != nullptr;
+      if (has_m)
+#pragma unroll
+        for (int a = 0; a < 12; ++a) M[a] = __ldg(&g.xform[q * 12 + a]);
+    } else {
+      if (v_begin + lane < n_v) p_next = __ldg(&vin[v_begin + lane]);
+    }
     for (uint32_t v0 = v_begin; v0 < v_end; v0 += RAS_CHUNK) {
-      // ---- project 32 vertices (loaded one chunk ahead), neighbour by shuffle
+      // ---- project 32 vertices (loaded one chunk ahead, or generated here), neighbour by shuffle
       const uint32_t v = v0 + lane;
-      const float4 p = p_next;
-      if (v0 + RAS_CHUNK < v_end && v + RAS_CHUNK < n_v) p_next = __ldg(&vin[v + RAS_CHUNK]);
+      float4 p = p_next;
+      gen::Strand S = {};
+      if constexpr (FUSED) {
+        if (v < n_v) {
+          const uint32_t ks = v / C;
+          S = gen::strand_setup(g, off_t + ks);
+          p = gen::vertex(tab, v - ks * C, S.b1, S.b2, S.cphi, S.sphi, S.base, g.op_mask, has_m ? M : nullptr);
+        }
+      } else {
+        if (v0 + RAS_CHUNK < v_end && v + RAS_CHUNK < n_v) p_next = __ldg(&vin[v + RAS_CHUNK]);
+      }
       Proj a;
       a.valid = false;
       a.sx = a.sy = a.zn = a.zv = 0.f;
@@ -133,18 +160,33 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
         pp.w = pn.w = 0.f;
         X3 Tv = {1.f, 0.f, 0.f};
         if (v < n_v) {
-          if (lane == 0 && j > 0) pp = __ldg(&vin[v - 1]);
-          if (lane == 31 && j + 1 < C) pn = __ldg(&vin[v + 1]);
+          if constexpr (FUSED) {  // the neighbours beyond the chunk's ends: one more vertex on lanes 0 and 31
+            const bool e0 = lane == 0 && j > 0, e1 = lane == 31 && j + 1 < C;
+            if (e0 || e1) {
+              const float4 px = gen::vertex(tab, e0 ? j - 1 : j + 1, S.b1, S.b2, S.cphi, S.sphi, S.base, g.op_mask,
+                                            has_m ? M : nullptr);
+              if (e0) pp = px;
+              else pn = px;
+            }
+          } else {
+            if (lane == 0 && j > 0) pp = __ldg(&vin[v - 1]);
+            if (lane == 31 && j + 1 < C) pn = __ldg(&vin[v + 1]);
+          }
           Tv = tangent_x(j, C, pp, p, pn);
         }
         const float t1x = __shfl_down_sync(0xffffffffu, Tv.x, 1), t1y = __shfl_down_sync(0xffffffffu, Tv.y, 1),
                     t1z = __shfl_down_sync(0xffffffffu, Tv.z, 1), ao1 = __shfl_down_sync(0xffffffffu, p.w, 1);
         if (seg) {
-          const uint32_t base = pcg(g.seed_h + off_t + k);
-          uint32_t a1 = pcg(base + 1u) >> 8, a2 = pcg(base + 2u) >> 8;
-          if (a1 + a2 > 16777216u) {  // R6
-            a1 = 16777216u - a1;
-            a2 = 16777216u - a2;
+          uint32_t a1, a2;
+          if constexpr (FUSED) {
+            a1 = S.a1, a2 = S.a2;
+          } else {
+            const uint32_t base = pcg(g.seed_h + off_t + k);
+            a1 = pcg(base + 1u) >> 8, a2 = pcg(base + 2u) >> 8;
+            if (a1 + a2 > 16777216u) {  // R6
+              a1 = 16777216u - a1;
+              a2 = 16777216u - a2;
+            }
           }
           float* rp = rec[lane];
           rp[18] = Tv.x, rp[19] = Tv.y, rp[20] = Tv.z, rp[21] = t1x, rp[22] = t1y, rp[23] = t1z;
@@ -429,20 +471,24 @@ void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_
   k_clear<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(gbuf), n_pixels, scene_zn);
 }
 
-template <bool COUNT, bool MS, bool PP, bool HZ>
+template <bool COUNT, bool MS, bool PP, bool HZ, bool FUSED = false>
 static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                             const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                             unsigned long long* counters, uint32_t ms_k, uint32_t queue, const uint32_t* hiz, int n_sm,
-                            cudaStream_t st) {
+                            cudaStream_t st, uint32_t c_max = 0) {
   // persistent grid: every CTA slot of the device, the queue feeds them
+  const size_t smem = FUSED ? (size_t)RAS_WARPS * c_max * HAIR_ROW * sizeof(float) : 0;  // the warps' spline tables
   static int per_sm = 0;
-  if (!per_sm) {
+  static size_t configured = 0;
+  if (!per_sm || smem > configured) {
+    if (smem) cudaFuncSetAttribute(k_raster<COUNT, MS, PP, HZ, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     int b = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<COUNT, MS, PP, HZ>, RAS_WARPS * 32, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<COUNT, MS, PP, HZ, FUSED>, RAS_WARPS * 32, smem);
     per_sm = b > 0 ? b : 1;
+    configured = smem;
   }
-  k_raster<COUNT, MS, PP, HZ><<<(uint32_t)(n_sm * per_sm), RAS_WARPS * 32, 0, st>>>(
-      d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, ms_k, queue, hiz);
+  k_raster<COUNT, MS, PP, HZ, FUSED><<<(uint32_t)(n_sm * per_sm), RAS_WARPS * 32, smem, st>>>(
+      d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, ms_k, queue, hiz, c_max);
 }
 
 // ms_k = 0: the two-layer G-buffer; ms_k in {1, 2, 4, 8}: gbuf = [ms_k][H][W] sample layers (reference mode).
@@ -450,11 +496,13 @@ static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4*
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                    unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int pass,
-                   const uint32_t* hiz, int n_sm, cudaStream_t st) {
+                   const uint32_t* hiz, int n_sm, cudaStream_t st, uint32_t fused_c_max) {
   const uint32_t* gp = grp + (pass ? (size_t)n_bi + 1 : 0);
   const uint32_t q = pass ? CNT_WORK_RASTER1 : CNT_WORK_RASTER;
 #define RAS_ARGS d_scene, n_bi, table, gp, vertices, cam, rho_default, gbuf, counters
-  if (ms_k) launch_raster_t<false, true, false, false>(RAS_ARGS, ms_k, q, nullptr, n_sm, st);
+  if (fused_c_max && pass) launch_raster_t<false, false, true, true, true>(RAS_ARGS, 0, q, hiz, n_sm, st, fused_c_max);
+  else if (fused_c_max) launch_raster_t<false, false, true, false, true>(RAS_ARGS, 0, q, nullptr, n_sm, st, fused_c_max);
+  else if (ms_k) launch_raster_t<false, true, false, false>(RAS_ARGS, ms_k, q, nullptr, n_sm, st);
   else if (paper_payload && count) launch_raster_t<true, false, true, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);
   else if (paper_payload && pass) launch_raster_t<false, false, true, true>(RAS_ARGS, 0, q, hiz, n_sm, st);
   else if (paper_payload) launch_raster_t<false, false, true, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);

@@ -567,6 +567,44 @@ def test_two_depth_ordered_passes_give_the_same_frame(hair_mod):
         assert torch.equal(a[0], c2[0]) and torch.equal(a[1], c2[1]), fl
 
 
+@pytest.mark.parametrize("idx,scale,res_scale,groom", [
+    (1, 1.0, 1.0, None),      # tiny config as named
+    (2, 0.1, 0.5, None),      # curl + frizz
+    (3, 0.03, 0.25, None),    # twist + clump under LOD
+    (5, 0.01, 0.2, None),     # 64 instances (instance transforms)
+    (4, 0.6, 0.5, 0),         # big enough for the two depth-ordered passes (curl, 72 k strands, 3.5 M vertices)
+])
+def test_fused_generate_raster_equals_the_materialised_frame(hair_mod, idx, scale, res_scale, groom):
+    """HAIR_FLAG_FUSED generates the vertices inside the raster's warps instead of
+    reading the vertex buffer. Same device functions as k_generate, so the G-buffer (paper payload) and the image
+    must equal the materialised frame's bit for bit — which test_paper_payload_stagewise ties to the oracle."""
+    import torch
+    b = hair_mod
+    sc = synth.config(idx, scale=scale, res_scale=res_scale)
+    prm = dict(sc["params"]) if groom is None else dict(sc["params"], groom_mask=1 << groom)
+    h = b.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(prm, flags=b.FLAG_PAPER_PAYLOAD)
+    for _ in range(2):
+        g0, r0 = h.render(sc["camera"], sc["lam"])
+    st0 = h.stats()
+    h.set_render_params(prm, flags=b.FLAG_PAPER_PAYLOAD | b.FLAG_FUSED)
+    for _ in range(2):
+        g1, r1 = h.render(sc["camera"], sc["lam"])
+    st1 = h.stats()
+    assert torch.equal(g0, g1), float((g0 == g1).float().mean())
+    assert torch.equal(r0, r1)
+    assert st1["gpu_launches"] == st0["gpu_launches"] - 1  # no k_generate
+    assert st1["two_pass"] == st0["two_pass"] and st1["n_segments_hiz_culled"] == st0["n_segments_hiz_culled"]
+    if idx == 4:
+        assert st1["two_pass"] == 1
+    # the strand-id word needs the vertex buffer to shade
+    h.set_render_params(prm, flags=b.FLAG_FUSED)
+    with pytest.raises(RuntimeError):
+        h.render(sc["camera"], sc["lam"])
+
+
 def test_sequential_as_first_render_of_a_context(hair_mod):
     """Regression: the first frame of a context may be a sequential one (its second target must survive the
     allocation of the per-resolution scratch)."""
