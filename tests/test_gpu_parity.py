@@ -567,6 +567,56 @@ def test_two_depth_ordered_passes_give_the_same_frame(hair_mod):
         assert torch.equal(a[0], c2[0]) and torch.equal(a[1], c2[1]), fl
 
 
+def test_two_pass_soak_over_cameras_and_grooms(hair_mod):
+    """The hi-Z test must never drop a segment that wins a pixel: random views (off-centre, rolled, partly off screen,
+    grooms overlapping on screen), each drawn in two passes with the PREVIOUS view's depth ranges (stale on purpose)
+    and compared with the one-pass frame word by word."""
+    import torch
+    b = hair_mod
+    sc = synth.config(4, scale=0.5, res_scale=0.5)
+    cam0 = sc["camera"]
+    thfov = math.tan(0.5 * cam0["vfov_y"]) * cam0["width"] / cam0["height"]
+    for g, ndc_x in zip(sc["grooms"], (-0.3, 0.0, 0.1, 0.2, 0.25)):  # pull the grooms together: they occlude each other
+        x = np.array(g["xform"], np.float32).reshape(-1, 12).copy()
+        x[:, 3] = ndc_x * (-x[:, 11]) * thfov
+        g["xform"] = x
+    h1, h2 = b.Hair(0), b.Hair(0)
+    for g in sc["grooms"]:
+        h1.mesh_upload(g)
+        h2.mesh_upload(g)
+    h1.set_render_params(sc["params"], flags=b.FLAG_SINGLE_PASS)
+    h2.set_render_params(sc["params"])
+    rng = np.random.default_rng(11)
+    n_two = n_culled = 0
+    for it in range(10):
+        cam = dict(cam0)
+        eye = np.asarray(cam0["eye"], np.float64) + rng.normal(0, 0.25, 3) * (1.0 if it else 0.0)
+        fwd = np.asarray(cam0["forward"], np.float64) + rng.normal(0, 0.08, 3) * (1.0 if it else 0.0)
+        fwd /= np.linalg.norm(fwd)
+        up0 = np.asarray(cam0["up"], np.float64) + rng.normal(0, 0.2, 3) * (1.0 if it else 0.0)
+        right = np.cross(up0, fwd)   # same handedness as synth.look_from_z: right = up x forward
+        right /= np.linalg.norm(right)
+        if np.dot(right, np.asarray(cam0["right"], np.float64)) < 0:
+            right = -right
+        up = np.cross(fwd, right)
+        if np.dot(up, up0) < 0:
+            up = -up
+        cam.update(eye=[float(v) for v in eye], forward=[float(v) for v in fwd], right=[float(v) for v in right],
+                   up=[float(v) for v in up])
+        # LOD off: every strand drawn, big enough for two passes; one small LOD frame in between makes the next frame
+        # fall back to one pass (the host acts on what the frame before reported)
+        lam = sc["lam"] if it == 5 else [0.0]
+        ga, ra = h1.render(cam, lam)
+        for rep in range(2):  # first with the previous view's depth ranges (a camera cut), then with this view's own
+            gb, rb = h2.render(cam, lam)
+            st = h2.stats()
+            n_two += st["two_pass"]
+            n_culled += st["n_segments_hiz_culled"]
+            assert torch.equal(ga, gb), (it, rep, st, float((ga == gb).float().mean()))
+            assert torch.equal(ra, rb), (it, rep)
+    assert n_two >= 10 and n_culled > 5000000, (n_two, n_culled)
+
+
 @pytest.mark.parametrize("idx,scale,res_scale,groom", [
     (1, 1.0, 1.0, None),      # tiny config as named
     (2, 0.1, 0.5, None),      # curl + frizz
