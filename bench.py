@@ -298,6 +298,9 @@ def run_cuda(args):
                     "unit": "Gwarp-inst/s", "frac": d["frac_issue"], "traffic": dram.get(dom),
                     "peak_source": f"derived: {n_sm} SMs x 4 schedulers x {sm_mhz:.0f} MHz (clock sampled in this run)",
                     "algorithmic": d["inst_per_unit"] + f" x {inst_per_unit[dom][1]} units counted in this run"}
+        if dom == "raster":
+            roofline["covers"] = ("the raster stage of the two-pass frame: k_raster (near pass) + k_hiz + k_raster (far pass); "
+                                  "achieved, traffic and the CUDA-event time all span the three launches")
     else:
         roofline = {"kernel": "k_" + dom, "bound": "hbm", "achieved": d["GBps"], "peak": hbm_peak, "unit": "GB/s",
                     "frac": d["frac_hbm"], "traffic": dram.get(dom), "peak_source": hbm_src,
