@@ -65,7 +65,7 @@ __constant__ int c_ms_off[4][8][2] = {  // sample offsets from the pixel centre 
 // lane GENERATES the vertex it would have loaded (gen::vertex: same source, same bits). Needs the paper payload (the
 // strand-id word is shaded from the vertex buffer). An A/B against the materialised pipeline.
 template <bool COUNT, bool MS, bool PP, bool HZ, bool FUSED = false>
-__global__ void __launch_bounds__(RAS_WARPS * 32, FUSED ? 2 : RAS_MIN_BLOCKS)
+__global__ void __launch_bounds__(RAS_WARPS * 32, FUSED ? 2 : (PP ? 4 : RAS_MIN_BLOCKS))  // payload: 64 registers, no spills
 k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
          const uint32_t* __restrict__ grp, const float4* __restrict__ vertices, CamDev cam, float rho_default,
          unsigned long long* __restrict__ gbuf, unsigned long long* __restrict__ counters, uint32_t ms_k,
