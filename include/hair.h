@@ -11,7 +11,10 @@
  *  - "host" pointers are read during the call and may be freed after it returns (the library
  *    copies). "DEVICE" pointers are caller-owned CUDA allocations on the context's device.
  *  - All work is enqueued on the CUDA stream given to hair_create (the caller's, e.g. torch's
- *    current stream). hair_render never synchronises and reads no device result back.
+ *    current stream). hair_render never synchronises and waits for no device result: grid sizes come from
+ *    device-side counters; the one thing the host looks at is a host-mapped word in which the scan of the frame
+ *    BEFORE said whether that frame was big enough for two raster passes (HAIR_FLAG_SINGLE_PASS), read without
+ *    waiting — a stale value changes the launch count of this frame, never its result.
  *  - A context is not thread-safe. No global state.
  *  - Arithmetic contract (operation order of the fp32 decisions, bit layout): DESIGN.md §3.
  */
