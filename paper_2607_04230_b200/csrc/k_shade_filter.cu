@@ -30,6 +30,32 @@ __device__ __forceinline__ F3 calc_tangent(int idx, int count, F3 prev, F3 curr,
   else return normalize(next - prev);
 }
 
+// fast non-decision arithmetic of the shading model (everything here is far inside the 2e-3 RGB tolerance)
+__device__ __forceinline__ float fast_sqrt(float x) {
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float fast_rcp(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// asin on [-1, 1]: pi/2 - sqrt(1 - |x|) P7(|x|), |error| <= 2e-8 (Abramowitz & Stegun 4.4.46)
+__device__ __forceinline__ float fast_asin(float x) {
+  const float a = fabsf(x);
+  float p = -0.0012624911f;
+  p = fmaf(p, a, 0.0066700901f);
+  p = fmaf(p, a, -0.0170881256f);
+  p = fmaf(p, a, 0.0308918810f);
+  p = fmaf(p, a, -0.0501743046f);
+  p = fmaf(p, a, 0.0889789874f);
+  p = fmaf(p, a, -0.2145988016f);
+  p = fmaf(p, a, 1.5707963050f);
+  const float r = fmaf(-fast_sqrt(1.f - a), p, 1.57079632679f);
+  return copysignf(r, x);
+}
+
 // the stand-in shading model (R23) at one point: position, unit tangent, strand parameter w, AO
 __device__ __forceinline__ F3 shade_model(const GroomDev& g, const CamDev& cam, const ShadeParams& sp, F3 pos, F3 T,
                                           float w, float ao) {
@@ -38,17 +64,17 @@ __device__ __forceinline__ F3 shade_model(const GroomDev& g, const CamDev& cam, 
   const F3 V = normalize(f3(cam.eye[0], cam.eye[1], cam.eye[2]) - pos);
   F3 rgb = f3(ao * sp.ambient[0] * alb.x, ao * sp.ambient[1] * alb.y, ao * sp.ambient[2] * alb.z);
   const float beta = g.roughness, tilt = g.tilt;
-  const float inv2b2 = 1.0f / (2.f * beta * beta);
+  const float inv2b2 = fast_rcp(2.f * beta * beta);
   const float sin_o = fminf(fmaxf(dot(T, V), -1.f), 1.f);
-  const float asin_o = asinf(sin_o);
+  const float asin_o = fast_asin(sin_o);
   for (uint32_t li = 0; li < sp.n_lights; ++li) {
     const F3 Lv = f3(sp.light_pos[li][0], sp.light_pos[li][1], sp.light_pos[li][2]) - pos;
     const float d2 = dot(Lv, Lv);
-    const float inv_d2 = 1.0f / d2;
+    const float inv_d2 = fast_rcp(d2);
     const F3 om = rsqrtf(d2) * Lv;
     const float sin_i = fminf(fmaxf(dot(T, om), -1.f), 1.f);
-    const float cos_i = sqrtf(fmaxf(0.f, 1.f - sin_i * sin_i));
-    const float th = 0.5f * (asinf(sin_i) + asin_o);
+    const float cos_i = fast_sqrt(fmaxf(0.f, 1.f - sin_i * sin_i));
+    const float th = 0.5f * (fast_asin(sin_i) + asin_o);
     const float a = th + tilt, b = th - 1.5f * tilt;
     const float MR = __expf(-a * a * inv2b2), MT = __expf(-b * b * 0.25f * inv2b2);
     const float s = cos_i * inv_d2;
