@@ -1,9 +1,10 @@
 // k_lod.cu — H1 LOD / cull and H2 scan (§3.2, Eq. 1-5).
 //
-// Paper: one thread per bundle writes an indirect-dispatch record. Here: one
-// thread per bundle-instance writes {N_LOD, C} into the bundle table, then a single-CTA scan turns
-// them into {slot_base, vertex_base} and the device-side totals the later persistent kernels read —
-// CUDA's replacement for the indirect dispatch: nothing returns to the host.
+// Paper: one thread per bundle writes an indirect-dispatch record. Here: four
+// lanes per bundle-instance write {N_LOD, C} into the bundle table (and which of the two raster passes
+// draws the bundle), then a tiled scan turns them into {slot_base, vertex_base}, the work-group scans
+// of the raster and the device-side totals the later persistent kernels read — CUDA's replacement for
+// the indirect dispatch: grid sizes never wait for a device result.
 #include "hair_internal.cuh"
 
 // Eq. 1, Eq. 4-5; fp32, fixed order (R14).
