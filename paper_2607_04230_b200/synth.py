@@ -250,3 +250,25 @@ def straight_prism(n_layers=5, h=0.05, axis=1, strands=32, spi=4, ops=(), **styl
     st.update(style)
     return dict(pos=X.astype(np.float32), ao=None, idx=np.array([[0, 1, 2]], np.uint32),
                 strands_per_tri=np.array([strands], np.uint32), xform=None, style=st)
+
+
+def flat_prism(a, b, h, n_layers, strands=64, spi=4):
+    """A flat prism in the plane z = 0: root triangle (0,0,0), (a,0,0), (0,b,0), layers stacked by h along +y.
+    Every cage vertex has the same view depth for a camera on +z, so the projected AABB has a closed form."""
+    X = np.zeros((n_layers, 3, 3))
+    for i in range(n_layers):
+        X[i] = np.array([[0.0, 0.0, 0.0], [a, 0.0, 0.0], [0.0, b, 0.0]])
+        X[i, :, 1] += h * i
+    return dict(pos=X.astype(np.float32), ao=None, idx=np.array([[0, 1, 2]], np.uint32),
+                strands_per_tri=np.array([strands], np.uint32), xform=None, style=dict(spi=spi, seed=9, ops=()))
+
+
+def straddle_prism(n_layers=5, dz=0.5, dx=0.06, strands=24, spi=4):
+    """A prism whose layers march TOWARDS a camera on +z (layer i at z = i dz, x = i dx): a camera placed inside its
+    depth range has some cage vertices and some strand vertices behind the near plane (R12, R13)."""
+    base = np.array([[0.0, 0.0, 0.0], [0.05, 0.0, 0.0], [0.0, 0.05, 0.0]])
+    X = np.zeros((n_layers, 3, 3))
+    for i in range(n_layers):
+        X[i] = base + np.array([dx * i, 0.0, dz * i])
+    return dict(pos=X.astype(np.float32), ao=None, idx=np.array([[0, 1, 2]], np.uint32),
+                strands_per_tri=np.array([strands], np.uint32), xform=None, style=dict(spi=spi, seed=13, ops=()))

@@ -326,6 +326,19 @@ def test_edge_cases(orc, hair_mod):
               params=synth.default_params(np.random.default_rng(2), (0, 0.15, 0)), lam=[0.0])
     G = gpu_frame(b, sc)
     check_stagewise(orc, sc, G)
+    # (g) a camera INSIDE the groom's depth range (R12, R13): some cage vertices behind the near plane => L = 1; strands
+    # cross the plane => segments with an endpoint behind it are dropped, the rest drawn; one layer in front only;
+    # everything behind. Stage-wise against the oracle (whose branches tests/test_oracle_*.py pin).
+    for dist, lam_s, n_lod in ((6.0, 0.05, None), (1.3, 0.05, 24), (1.3, 0.0, 24), (0.55, 0.05, 24), (0.05, 0.05, 0)):
+        sc = dict(grooms=[synth.straddle_prism()], camera=synth.look_from_z((0.1, 0.0, 0.0), dist, 96, 64),
+                  params=synth.default_params(np.random.default_rng(3), (0.1, 0, 1.0), center_diameter_px=1.0), lam=[lam_s])
+        G = gpu_frame(b, sc)
+        rep = check_stagewise(orc, sc, G)
+        assert rep["exact_frac"] == 1.0
+        if n_lod is not None:
+            assert G["stats"]["n_strands_lod"] == n_lod
+        if dist == 1.3:
+            assert 0 < G["stats"]["n_segments_drawn"] < G["stats"]["n_segments"] and rep["n_hit"] > 50
     # (f) invalid arguments are refused loudly
     with pytest.raises(b.HairError):
         h.mesh_upload(synth.straight_prism(n_layers=33, strands=1, spi=1))

@@ -146,6 +146,53 @@ def test_offscreen_bundle_is_culled(orc):
     assert f.n_strands > 0
 
 
+@pytest.mark.parametrize("W,H", [(640, 360), (300, 500)])
+@pytest.mark.parametrize("a,b,h,lv", [(0.02, 0.02, 0.05, 7),    # tall bundle: the extent comes from the layers
+                                      (0.3, 0.02, 0.004, 3)])   # wide bundle: the extent comes from the root triangle
+def test_eq2_eq3_closed_form_of_L(orc, W, H, a, b, h, lv):
+    """Eq. 2-3: L = clamp(||AABB_max - AABB_min|| / R_y * lambda) with the AABB over ALL layers'
+    projected vertices, the 2-D diagonal in pixels and R_y = the vertical resolution. A flat prism facing the camera
+    has every cage vertex at the same depth d, so the box is (f_px a / d) x (f_px (b + (Lv-1) h) / d) pixels."""
+    d, lam = 2.0, 0.8
+    g = synth.flat_prism(a, b, h, lv)
+    ext_y = b + (lv - 1) * h
+    cam = synth.look_from_z((0.5 * a, 0.5 * ext_y, 0.0), d, W, H)
+    f = orc.Frame([g])
+    f.lod(cam, lam)
+    t, L = f.table()
+    fpx = 0.5 * H / math.tan(0.5 * synth.VFOV)
+    want = math.hypot(fpx * a / d, fpx * ext_y / d) / H * lam
+    assert 0.05 < want < 0.5
+    assert abs(float(L[0]) - want) < 1e-6
+    # the mistakes this must catch: /W instead of /R_y, one axis instead of the diagonal, the root layer only
+    assert abs(math.hypot(fpx * a / d, fpx * ext_y / d) / W * lam - want) > 1e-3
+    assert abs(max(fpx * a / d, fpx * ext_y / d) / H * lam - want) > 1e-5
+    assert abs(math.hypot(fpx * a / d, fpx * b / d) / H * lam - want) > 1e-4
+    # and Eq. 1 on that L (delta < 1): N_LOD within one strand of L N
+    assert abs(int(t[0, 0]) - want * 64) <= 1.0 + 1e-6
+
+
+def test_near_plane_straddle_full_detail_or_culled(orc):
+    """DESIGN.md R13 (PAPER.md:114-120 is silent on vertices behind the camera): a bundle with SOME cage vertices
+    behind the near plane gets L = 1 whatever lambda says; one with ALL of them behind is culled."""
+    g = synth.straddle_prism(n_layers=5, dz=0.5)  # layers at z = 0, 0.5, 1, 1.5, 2
+    N = int(g["strands_per_tri"][0])
+    f = orc.Frame([g])
+    lam = 0.05
+    f.lod(synth.look_from_z((0.1, 0.0, 0.0), 6.0, 96, 64), lam)  # whole cage in front: small L, few strands
+    t, L = f.table()
+    assert 0.0 < L[0] < 0.2 and 0 < t[0, 0] < N // 4
+    f.lod(synth.look_from_z((0.1, 0.0, 0.0), 1.3, 96, 64), lam)  # eye at z = 1.3: layers 3, 4 are behind it
+    t, L = f.table()
+    assert L[0] == 1.0 and t[0, 0] == N
+    assert t[0, 1] == orc.lod_counts(1.0, N, 0.0, 5, 17)[2] == 17  # Eq. 4-5 at L = 1, capped by C_full (R14)
+    f.lod(synth.look_from_z((0.1, 0.0, 0.0), 0.55, 96, 64), lam)  # eye at z = 0.55: only layer 0 (zv 0.55) is in front
+    assert f.table()[1][0] == 1.0
+    f.lod(synth.look_from_z((0.1, 0.0, 0.0), 0.05, 96, 64), lam)  # zv = 0.05 < near for layer 0, negative for the rest
+    t, L = f.table()
+    assert t[0, 0] == 0 and f.n_strands == 0
+
+
 # ------------------------------------------------------------------------------- O2: base spline
 @pytest.mark.parametrize("axis", [0, 1, 2])
 def test_straight_prism_is_the_interpolated_line(orc, axis):

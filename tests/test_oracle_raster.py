@@ -266,6 +266,36 @@ def test_gbuffer_vs_brute_force_32x32(orc):
     assert (G[..., 1] <= G[..., 0]).all()
 
 
+def test_segment_with_an_endpoint_behind_the_near_plane_is_dropped(orc):
+    """DESIGN.md R12 (the paper is silent): a segment is drawn only if BOTH endpoints have zv >= near; no clipping.
+    A camera inside the groom's depth range: the strands march towards it and cross the near plane."""
+    g = synth.straddle_prism(n_layers=5, dz=0.5, strands=24, spi=4)
+    cam = synth.look_from_z((0.1, 0.0, 0.0), 1.3, 96, 64)  # eye at z = 1.3 looking down -z
+    prm = dict(center_diameter_px=1.0, lights=[])
+    f = orc.Frame([g])
+    f.lod(cam, 0.0)
+    f.generate()
+    v = f.vertices_f32()
+    f.set_vertices_f32(v)
+    cnt = f.raster(cam, prm)
+    C = 17
+    zv = np.float32(cam["eye"][2]) - v[:, 2].reshape(24, C)  # textbook: depth along -z from the eye
+    valid = zv >= np.float32(cam["near_z"])
+    assert np.abs(zv - np.float32(cam["near_z"])).min() > 1e-4  # no vertex sits on the plane itself
+    drawn = valid[:, :-1] & valid[:, 1:]
+    cut = valid[:, :-1] != valid[:, 1:]  # exactly one endpoint behind the plane
+    assert cut.sum() == 24 and 0 < drawn.sum() < 24 * (C - 1)
+    assert cnt["segments"] == int(drawn.sum())
+    G = f.gbuffer()
+    hit = G[..., 1] != EMPTY
+    sid = ((G[..., 1] >> np.uint64(16)) & np.uint64(0xFFFFFF)).astype(np.int64)[hit]
+    j = ((G[..., 1] >> np.uint64(9)) & np.uint64(0x7F)).astype(np.int64)[hit]
+    assert hit.sum() > 50 and drawn[sid, j].all()          # no pixel names a cut or hidden segment
+    last = drawn.shape[1] - 1 - np.argmax(drawn[:, ::-1], axis=1)  # last drawn segment of each strand ...
+    seen = set(zip(sid.tolist(), j.tolist()))
+    assert sum((s, int(last[s])) in seen for s in range(24)) >= 12  # ... is drawn right up to the cut
+
+
 def test_resolve_is_order_independent(orc):
     # north_star invariant: the depth-sorted resolve is order-independent (min is commutative)
     sc, f = _tiny_frame(orc, res=64, strands=200)

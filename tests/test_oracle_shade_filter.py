@@ -246,6 +246,42 @@ def test_flyaway_strand_in_front_gets_alpha_one(orc):
     assert out3[16, 24, 3] == 1.0 and out3[16, 26, 3] < 0.6
 
 
+def test_flyaway_blend_of_two_different_colours(orc):
+    """PAPER.md:175-176 / DESIGN.md R21: C = alpha_f C_f + (1 - alpha_f) C_c, alpha = 1, where C_c is the centre
+    accumulation and (C_f, alpha_f) the accumulation around the conservative sample. Two strands whose hits differ in
+    colour (root albedo at w = 0 against tip albedo at w = 1) and lie farther apart in depth than tau_z, so each
+    accumulation sees one constant colour and alpha_f is a plain count: the blend is fixed by hand."""
+    root, tip = (0.2, 0.4, 0.6), (1.0, 0.8, 0.2)
+    f, cam = hand_frame(orc, [X_LINE, [(x, 0.0, 0.3) for x, _, _ in X_LINE]], n_strands=2, ao=0.5,
+                        albedo_root=root, albedo_tip=tip)
+    back = orc.pack(0.9, 0, 0, 0.0)            # strand 0 at w = 0
+    front = orc.pack(0.9 - 3e-3, 1, 3, 1.0)    # strand 1 at w = 1, 3e-3 nearer: > tau_fly and > tau_z
+    words = {}
+    for x in range(10, 41):
+        words[(x, 16, 0)] = back
+        words[(x, 16, 1)] = back
+    for x in (23, 24, 27):                     # centre hits of the front strand
+        words[(x, 16, 0)] = front
+        words[(x, 16, 1)] = front
+    for x in (21, 22, 25, 26, 28, 29, 30):     # pixels the front strand only touches
+        words[(x, 16, 1)] = front
+    f.set_gbuffer(gbuf_with(words))
+    col = f.shade(cam, params())
+    out = f.filter(cam, params())
+    amb = float(np.float32(0.2))
+    C_c = 0.5 * amb * np.float32(root).astype(float)
+    C_f = 0.5 * amb * np.float32(tip).astype(float)
+    assert np.allclose(col[16, 25], C_c, atol=1e-12) and np.allclose(col[16, 24], C_f, atol=1e-12)
+    # strip around (25, 16) along the row, x = 20 .. 30, classes relative to the FRONT depth: 23, 24, 27 centre;
+    # 21, 22, 25, 26, 28, 29, 30 conservative-only; 20 (back in both layers) rejected by depth => alpha_f = 3 / 10
+    alpha_f = 3.0 / 10.0
+    want = alpha_f * C_f + (1.0 - alpha_f) * C_c
+    assert out[16, 25, 3] == 1.0
+    assert np.allclose(out[16, 25, :3], want, atol=1e-12)
+    assert np.abs((1.0 - alpha_f) * C_f + alpha_f * C_c - want).max() > 1e-2   # swapped alpha would show
+    assert np.abs(want - C_c).max() > 1e-2 and np.abs(want - C_f).max() > 1e-2
+
+
 def test_filter_off_passes_centre_colour(orc):
     f, cam = line_frame(orc, lambda i: "c" if i % 3 == 0 else "a")
     col = f.shade(cam, params())
