@@ -35,6 +35,20 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per frame and stage from the committed `ncu --set full` capture
+    (profiles/r2_ncu_traffic.csv: stage,dram_bytes,kernels), or {} — never typed in here."""
+    p = os.path.join(ROOT, "profiles", "r2_ncu_traffic.csv")
+    out = {}
+    if os.path.exists(p):
+        for line in open(p).read().splitlines()[1:]:
+            f = line.split(",")
+            if len(f) >= 2 and f[1].strip().isdigit():
+                out[f[0].strip()] = int(f[1])
+        out["source"] = "profiles/r2_ncu_traffic.csv (ncu --set full capture of this command; see profiles/r2_ncu_full.md)"
+    return out
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -163,6 +177,12 @@ def run_cuda(args):
     h.set_render_params(sc["params"], flags=binding.FLAG_COUNTERS)
     h.render(cam, lam, gb, rgb)
     cnt = h.stats()
+    # unique vertices the shading gathers touch (neighbouring pixels share them): v_{j-1} .. v_{j+2} of every centre word
+    G0 = gb[..., 0].reshape(-1)
+    G0 = G0[(G0 & 0xFFFFFFFFFF) != 0xFFFFFFFFFF]
+    sid_j = (G0 >> 9) & 0x7FFFFFFF  # sid << 7 | j
+    n_unique_vertices = int(torch.unique(torch.cat([sid_j - 1, sid_j, sid_j + 1, sid_j + 2])).numel())
+    del G0, sid_j
 
     # ---- device-resident timing: K frames, one event pair, stage events inside the library
     h.set_render_params(sc["params"], flags=binding.FLAG_STAGE_TIMING)
@@ -185,6 +205,21 @@ def run_cuda(args):
     n_seg = cnt["n_segments"]
     assert replicas.same_on_all_ranks(n_seg, dist, dev), "replicas rendered different frames"
     value = replicas.job_rate(n_seg, world, ms_step) / 1e9
+
+    # ---- the same frames under camera motion (untimed for `value`): the depth ranges of the two-pass split and the
+    # choice of passes are then one frame stale; a slow orbit + dolly, ~10 px of image motion per frame
+    k_mov = max(8, min(args.steps, 64))
+    for i in range(3):
+        h.render(synth.moving_camera(cam, i), lam, gb, rgb)
+    h.stats()
+    barrier()
+    e0.record()
+    for i in range(k_mov):
+        h.render(synth.moving_camera(cam, 3 + i), lam, gb, rgb)
+    e1.record()
+    barrier()
+    ms_moving = e0.elapsed_time(e1) / k_mov
+    st_mov = h.stats()
 
     # ---- end to end through the C ABI with HOST buffers: cage upload (pinned) + render + D2H of out_rgb
     h.set_render_params(sc["params"], flags=0)
@@ -243,9 +278,8 @@ def run_cuda(args):
             dist.destroy_process_group()
         return
 
-    # ---- rooflines: algorithmic work per launch / measured stage time
+    # ---- rooflines: algorithmic work per frame / measured stage time, every peak measured in this run
     hbm_peak, hbm_src = peaks()
-    n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
     words = torch.empty(W * H * 2, dtype=torch.int64, device=dev)
     n_ops = 1 << 28
     atom = {}
@@ -254,66 +288,74 @@ def run_cuda(args):
         ms = min(h.atomic_microbench(mode, words, n_ops, 1024) for _ in range(3))
         atom[name] = n_ops / (ms * 1e-3) / 1e9
     del words
+    # 16-byte ld.global.cg of word pairs over the frame's own G-buffer, in the raster's access shapes (G pair loads / s)
+    l2 = {}
+    for mode, name in ((0, "row"), (1, "column"), (2, "random")):
+        h.l2_load_microbench(mode, gb, W, 32)  # warm
+        l2[name] = max(n / (ms * 1e-3) / 1e9 for n, ms in (h.l2_load_microbench(mode, gb, W, 512) for _ in range(3)))
     n_px = W * H
-    n_at = cnt["n_atomics_center"] + cnt["n_atomics_cons"]
+    n_cons, n_cen, n_cons_y = cnt["n_atomics_cons"], cnt["n_atomics_center"], cnt["n_atomics_cons_ymajor"]
+    n_at = n_cen + n_cons
     stages = {
-        "generate": {"bound": "hbm", "ms": st["ms_generate"], "bytes": 16 * cnt["n_vertices"]},
-        "clear": {"bound": "hbm", "ms": st["ms_clear"], "bytes": 16 * n_px},
-        "raster": {"bound": "l2_atomic", "ms": st["ms_raster"], "atomics": n_at, "bytes": 16 * cnt["n_vertices"] + 8 * n_at},
-        "shade": {"bound": "hbm", "ms": st["ms_shade"], "bytes": 16 * n_px + (16 + 64) * cnt["n_pixels_center"]},
-        "filter": {"bound": "hbm", "ms": st["ms_filter"], "bytes": 32 * n_px + 16 * cnt["n_pixels_center"]},
+        "generate": {"bound": "hbm", "ms": st["ms_generate"], "bytes": 16 * cnt["n_vertices"],
+                     "note": "the G-buffer clear (16 B/px) runs beside LOD / scan / generate on the library's second stream "
+                             "and is not in these bytes"},
+        "raster": {"bound": "l2_load", "ms": st["ms_raster"], "pair_loads": n_cons, "hits": n_at,
+                   "bytes": 16 * cnt["n_vertices"] + 8 * n_at},
+        "shade": {"bound": "hbm", "ms": st["ms_shade"], "bytes": 16 * n_px + (16 + 64) * cnt["n_pixels_center"],
+                  "bytes_unique_vertices": 16 * n_px + 16 * cnt["n_pixels_center"] + 16 * n_unique_vertices
+                                           + 8 * cnt["n_strands_lod"]},
+        "filter": {"bound": "hbm (nominal; ALU/issue in practice)", "ms": st["ms_filter"],
+                   "bytes": 32 * n_px + 16 * cnt["n_pixels_center"]},
     }
     for k, s in stages.items():
         if s["ms"] > 0:
             s["GBps"] = s["bytes"] / (s["ms"] * 1e-3) / 1e9
             s["frac_hbm"] = s["GBps"] / hbm_peak
-            if "atomics" in s:
-                s["Gatom_per_s"] = s["atomics"] / (s["ms"] * 1e-3) / 1e9
-                s["frac_l2_atomic_random"] = s["Gatom_per_s"] / atom["random"]
+    sh = stages["shade"]
+    sh["GBps_unique_vertices"] = sh["bytes_unique_vertices"] / (sh["ms"] * 1e-3) / 1e9
+    sh["frac_hbm_unique_vertices"] = sh["GBps_unique_vertices"] / hbm_peak
     stages["lod_scan"] = {"bound": "latency", "ms": st["ms_lod"]}
-    dom = max(("generate", "clear", "raster", "shade", "filter"), key=lambda k: stages[k]["ms"])
+    stages["clear"] = {"bound": "hbm", "ms": None, "bytes": 16 * n_px,
+                       "note": "overlapped: runs on the library's second stream beside lod_scan + generate (not bracketed)"}
+    # The raster (dominant): every pixel that passes the conservative predicate needs the existing word pair before
+    # anything is known about its depth (read-before-atomic) = one 16-byte L2 load, the method's own
+    # minimum. Lower bound of the time = x-major loads at the measured row rate + y-major loads at the column rate.
+    ras = stages["raster"]
+    t_min_ms = ((n_cons - n_cons_y) / l2["row"] + n_cons_y / l2["column"]) / 1e9 * 1e3
+    ras["Gpair_loads_per_s"] = n_cons / (ras["ms"] * 1e-3) / 1e9
+    ras["Ghits_per_s"] = n_at / (ras["ms"] * 1e-3) / 1e9
+    ras["frac_l2_load"] = t_min_ms / ras["ms"]
+    ras["frac_l2_atomic_random"] = ras["Ghits_per_s"] / atom["random"]
+    traffic = ncu_traffic()
+    dom = max(("generate", "raster", "shade", "filter"), key=lambda k: stages[k]["ms"])
     d = stages[dom]
-    # Issue-slot ("alu") view of the two kernels that ncu shows are bound by instruction issue, not by memory:
-    # warp instructions per algorithmic unit from the committed ncu capture (profiles/r1_v5_ncu_full.md,
-    # smsp__inst_executed.sum / units of that frame) x the units this run counted, over the live CUDA-event time,
-    # against 148 SMs x 4 schedulers x 1 warp instruction per clock.
-    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
-    issue_peak = n_sm * 4 * sm_mhz * 1e6 / 1e9  # G warp-instructions / s
-    n_items = cnt["n_pixels_cons"]  # one filter item per hit pixel (+ one per fly-away pixel, not counted here)
-    # raster = near pass + k_hiz + far pass of the two-pass frame
-    inst_per_unit = {"raster": ((465459314 + 4244400 + 129536574) / 219609409, n_at, "predicate-true hit"),
-                     "filter": (439092496 / 3024726, n_items, "hit pixel")}
-    if not (args.config == 4 and args.scale == 1.0 and args.res_scale == 1.0):
-        inst_per_unit = {}  # the per-unit instruction counts were captured on the bench frame only
-    for k, (ipu, units, what) in inst_per_unit.items():
-        stg = stages[k]
-        stg["warp_inst"] = ipu * units
-        stg["Gwarp_inst_per_s"] = ipu * units / (stg["ms"] * 1e-3) / 1e9
-        stg["frac_issue"] = stg["Gwarp_inst_per_s"] / issue_peak
-        stg["inst_per_unit"] = f"{ipu:.2f} warp instructions per {what} (ncu, profiles/r1_v5_ncu_full.md)"
-    # ncu dram read + write per frame, same capture (raster: near pass 156.6 MB + k_hiz 136.2 MB + far pass 83.7 MB)
-    dram = {"generate": 103936256, "raster": 376465152, "shade": 200673536, "filter": 311918080}
-    if dom in inst_per_unit:
-        roofline = {"kernel": "k_" + dom, "bound": "alu", "achieved": d["Gwarp_inst_per_s"], "peak": issue_peak,
-                    "unit": "Gwarp-inst/s", "frac": d["frac_issue"], "traffic": dram.get(dom),
-                    "peak_source": f"derived: {n_sm} SMs x 4 schedulers x {sm_mhz:.0f} MHz (clock sampled in this run)",
-                    "algorithmic": d["inst_per_unit"] + f" x {inst_per_unit[dom][1]} units counted in this run"}
-        if dom == "raster":
-            roofline["covers"] = ("the raster stage of the two-pass frame: k_raster (near pass) + k_hiz + k_raster (far pass); "
-                                  "achieved, traffic and the CUDA-event time all span the three launches")
+    if dom == "raster":
+        roofline = {"kernel": "k_raster", "bound": "l2_load", "achieved": ras["Gpair_loads_per_s"],
+                    "peak": n_cons / (t_min_ms * 1e-3) / 1e9, "unit": "Gpair-loads/s", "frac": ras["frac_l2_load"],
+                    "traffic": traffic.get("raster"),
+                    "algorithmic": f"{n_cons} conservative-predicate-true pixels (counts.n_atomics_cons), one 16-byte "
+                                   f"ld.global.cg of the word pair each; {n_cons_y} of them on y-major segments",
+                    "peak_source": "measured in this run (hair_l2_load_microbench over this frame's G-buffer): "
+                                   f"row {l2['row']:.1f}, column {l2['column']:.1f}, random {l2['random']:.1f} G pair loads/s; "
+                                   "peak = loads / (x-major loads / row rate + y-major loads / column rate)",
+                    "covers": "the raster stage: k_raster (near pass) + k_hiz + k_raster (far pass); time = stages.raster.ms",
+                    "atomic_view": {"hits_per_s_G": ras["Ghits_per_s"], "frac_of_random_RED": ras["frac_l2_atomic_random"],
+                                    "issued_Gatom_per_s": cnt["n_atomics_issued"] / (ras["ms"] * 1e-3) / 1e9,
+                                    "note": "predicate-true hits / time over the measured random RED.MIN.64 rate; > 1 because "
+                                            "read-before-atomic sends only n_atomics_issued of the hits to L2 as atomics: "
+                                            "that ceiling does not bind, the load ceiling above does"}}
     else:
         roofline = {"kernel": "k_" + dom, "bound": "hbm", "achieved": d["GBps"], "peak": hbm_peak, "unit": "GB/s",
-                    "frac": d["frac_hbm"], "traffic": dram.get(dom), "peak_source": hbm_src,
+                    "frac": d["frac_hbm"], "traffic": traffic.get(dom), "peak_source": hbm_src,
                     "algorithmic": f"{d['bytes']} bytes per frame"}
+    roofline["traffic_source"] = traffic.get("source")
     # the three fractions north_star asks for, as it states them
     north_star = {
-        "raster_vs_l2_atomic": {"achieved_Gatom_per_s": stages["raster"].get("Gatom_per_s"), "peak_Gatom_per_s": atom["random"],
-                                "frac": stages["raster"].get("frac_l2_atomic_random"),
-                                "note": "algorithmic hits / time over the measured random 64-bit RED.MIN rate; > 1 because "
-                                        "read-before-atomic sends only n_atomics_issued of them to L2",
-                                "issued_Gatom_per_s": cnt["n_atomics_issued"] / (stages["raster"]["ms"] * 1e-3) / 1e9},
+        "raster_vs_l2": {"frac_l2_load": ras["frac_l2_load"], "frac_l2_atomic_random": ras["frac_l2_atomic_random"]},
         "generate_vs_hbm": {"GBps": stages["generate"].get("GBps"), "frac": stages["generate"].get("frac_hbm")},
-        "shade_vs_hbm": {"GBps": stages["shade"].get("GBps"), "frac": stages["shade"].get("frac_hbm")},
+        "shade_vs_hbm": {"GBps": sh.get("GBps"), "frac": sh.get("frac_hbm"),
+                         "frac_unique_vertices": sh["frac_hbm_unique_vertices"]},
     }
 
     # ---- the oracle timed beside it on this box's host cores (bounded sample of the same workload)
@@ -343,14 +385,18 @@ def run_cuda(args):
                         "pinned host, 2 frames in flight), hair_host_wait after the last; wall clock over the steps"},
         "gpu_launches": st["gpu_launches"] * args.steps,
         "roofline": roofline, "north_star_fractions": north_star, "stages": stages, "l2_atomic_peaks_Gatom_per_s": atom,
+        "l2_pair_load_peaks_Gloads_per_s": l2,
         "hbm_peak_GBps": hbm_peak, "hbm_peak_source": hbm_src,
         "counts": {k: cnt[k] for k in ("n_bundles", "n_bundles_culled", "n_strands_total", "n_strands_lod", "n_vertices",
                                        "n_segments", "n_segments_drawn", "n_segments_live", "n_atomics_center", "n_atomics_cons",
-                                       "n_atomics_issued", "n_pixels_center", "n_pixels_cons")},
+                                       "n_atomics_cons_ymajor", "n_atomics_issued", "n_pixels_center", "n_pixels_cons")},
         "raster_passes": {"two_pass": st["two_pass"], "n_segments_hiz_culled": st["n_segments_hiz_culled"],
                           "what": "production frames: bundles in the front 60 % of their groom's depth range first, 16x16-tile "
                                   "hi-Z (k_hiz), then the rest; a segment behind every tile of its bounding box is dropped "
                                   "before any pixel work (same G-buffer bit for bit; DESIGN.md 7.3)"},
+        "moving_camera": {"ms_per_step": ms_moving, "frames": k_mov, "ms_raster": st_mov["ms_raster"],
+                          "ms_filter": st_mov["ms_filter"], "n_segments_hiz_culled_last_frame": st_mov["n_segments_hiz_culled"],
+                          "what": "synth.moving_camera: yaw +-0.04 rad, sideways swing and dolly, a new camera every frame"},
         "sequential_per_groom": {"ms_per_step": ms_seq, "what": "hair_render_sequential: one LOD..filter pass per groom, "
                                  "depth kept, blended over the target (PAPER.md:208-210); the headline frame resolves "
                                  "all grooms in one G-buffer instead (DESIGN.md R15)"},

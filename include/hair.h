@@ -205,6 +205,8 @@ typedef struct {
   uint32_t n_segments_live;                /* segments that won at least one pixel test when drawn (counters flag) */
   uint64_t n_atomics_center, n_atomics_cons; /* predicate-true hits before any filtering (counters flag) */
   uint64_t n_atomics_issued;               /* atomics actually sent to L2 (counters flag) */
+  uint64_t n_atomics_cons_ymajor;          /* conservative hits of y-major segments: neighbouring lanes of a raster warp
+                                              then sit in neighbouring ROWS of the G-buffer (counters flag) */
   uint32_t n_pixels_center, n_pixels_cons; /* non-empty pixels after the frame (counters flag) */
   /* stage-timing flag: mean over the frames rendered since the previous hair_stats (last 64 at most) */
   float ms_lod, ms_generate, ms_clear, ms_raster, ms_shade, ms_filter, ms_total;
@@ -237,6 +239,15 @@ int hair_debug_set_vertices(hair_ctx*, const float* dev_src, uint32_t n);
  * Enqueues `n_ops` atomics; returns the elapsed milliseconds (CUDA events; synchronises). */
 int hair_atomic_microbench(hair_ctx*, int mode, uint64_t* dev_words, uint64_t n_words, uint64_t n_ops,
                            uint32_t hot_words, float* out_ms);
+
+/* L2-load roofline denominator for the raster's read-before-atomic ("reads the existing depth buffer";
+ * SURVEY.md §8d): 16-byte ld.global.cg of word pairs over a DEVICE buffer of n_pairs pairs laid out as image rows
+ * of `pitch` pairs (n_pairs >= 64 * pitch, pitch >= 64). A warp's 32 loads of one step are
+ *  mode 0: 32 consecutive pairs of a row;  mode 1: one column over 32 consecutive rows;  mode 2: 32 random pairs.
+ * Every thread of n_SM * 8 CTAs of 256 threads issues `n_steps` loads (a multiple of 4). Writes the total number of
+ * loads to *out_loads and the elapsed milliseconds (CUDA events; synchronises) to *out_ms. The buffer is only read. */
+int hair_l2_load_microbench(hair_ctx*, int mode, const uint64_t* dev_pairs, uint64_t n_pairs, uint32_t pitch,
+                            uint32_t n_steps, uint64_t* out_loads, float* out_ms);
 
 /* sizeof of {hair_cage, hair_roots, hair_style, hair_camera, hair_render_params, hair_stats_t}, so a
  * foreign-language binding can check its struct layouts without a GPU. */

@@ -21,7 +21,7 @@ EMPTY = 0xFFFFFFFFFFFFFFFF
 EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_render_params",
            "hair_set_render_params", "hair_mesh_upload", "hair_mesh_update", "hair_mesh_clear",
            "hair_render", "hair_render_scene", "hair_render_sequential", "hair_render_msaa", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
-           "hair_debug_buffers", "hair_debug_set_vertices", "hair_atomic_microbench", "hair_abi_sizes"]
+           "hair_debug_buffers", "hair_debug_set_vertices", "hair_atomic_microbench", "hair_l2_load_microbench", "hair_abi_sizes"]
 
 
 class HairError(RuntimeError):
@@ -68,6 +68,7 @@ class hair_stats_t(C.Structure):
                 ("n_vertices", C.c_uint32), ("n_segments", C.c_uint32), ("n_segments_drawn", C.c_uint32),
                 ("n_segments_live", C.c_uint32),
                 ("n_atomics_center", C.c_uint64), ("n_atomics_cons", C.c_uint64), ("n_atomics_issued", C.c_uint64),
+                ("n_atomics_cons_ymajor", C.c_uint64),
                 ("n_pixels_center", C.c_uint32), ("n_pixels_cons", C.c_uint32),
                 ("ms_lod", C.c_float), ("ms_generate", C.c_float), ("ms_clear", C.c_float),
                 ("ms_raster", C.c_float), ("ms_shade", C.c_float), ("ms_filter", C.c_float),
@@ -114,6 +115,7 @@ def load():
     L.hair_debug_buffers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     L.hair_debug_set_vertices.argtypes = [vp, vp, u32]
     L.hair_atomic_microbench.argtypes = [vp, C.c_int, vp, C.c_uint64, C.c_uint64, u32, C.POINTER(C.c_float)]
+    L.hair_l2_load_microbench.argtypes = [vp, C.c_int, vp, C.c_uint64, u32, u32, C.POINTER(C.c_uint64), C.POINTER(C.c_float)]
     L.hair_abi_sizes.argtypes = [C.POINTER(C.c_uint32 * 6)]
     L.hair_abi_sizes.restype = None
     sizes = (C.c_uint32 * 6)()
@@ -370,6 +372,13 @@ class Hair:
         self._check(self.L.hair_atomic_microbench(self.h, mode, C.c_void_p(words.data_ptr()), words.numel(), n_ops,
                                                   hot_words, C.byref(ms)), "hair_atomic_microbench")
         return ms.value
+
+    def l2_load_microbench(self, mode: int, pairs, pitch: int, n_steps: int = 64):
+        """hair_l2_load_microbench over `pairs` (int64 device tensor [n][2]); returns (loads, ms)."""
+        ms, n = C.c_float(0), C.c_uint64(0)
+        self._check(self.L.hair_l2_load_microbench(self.h, mode, C.c_void_p(pairs.data_ptr()), pairs.numel() // 2, pitch,
+                                                   n_steps, C.byref(n), C.byref(ms)), "hair_l2_load_microbench")
+        return n.value, ms.value
 
 
 def gbuffer_to_numpy(gb) -> np.ndarray:

@@ -58,8 +58,10 @@ struct hair_ctx {
   float4* d_target2 = nullptr;  // hair_render_sequential: second render target of the ping-pong
   size_t target2_cap = 0;
   unsigned long long* d_counters = nullptr;
+  unsigned long long* d_sink = nullptr;  // one word the load micro-benchmark may (never does) write
   unsigned long long* h_counters = nullptr;  // pinned
   uint32_t c_max = 0;
+  LaunchState ls;  // what this context has configured on its device (opt-in shared memory, occupancy)
   // owned outputs for hair_render_to_host(_async): HAIR_HOST_SLOTS frames in flight
   unsigned long long* d_own_gbuf[HAIR_HOST_SLOTS] = {};
   float* d_own_rgb[HAIR_HOST_SLOTS] = {};
@@ -264,6 +266,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
     return fail(c, HAIR_E_INVALID_ARG, "hair_render: bad camera");
   if (front && !(n_lam == 1 || n_lam == c->scene.n_grooms || (n_lam == 0 && lam == nullptr)))
     return fail(c, HAIR_E_INVALID_ARG, "hair_render: n_lambda must be 0, 1 or the number of grooms");
+  if (front && n_lam > 0 && lam == nullptr) return fail(c, HAIR_E_INVALID_ARG, "hair_render: lod_lambda is NULL but n_lambda > 0");
   CK(cudaSetDevice(c->device));
   int rc = ensure_scratch(c, w, h);
   if (rc) return rc;
@@ -330,7 +333,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_LOD);
   if (front && n_bi && !fused) {
-    launch_generate(c->d_scene, n_bi, c->d_table, c->d_vertices, c->d_srec, c->d_counters, c->c_max, c->n_sm, st);
+    launch_generate(c->d_scene, n_bi, c->d_table, c->d_vertices, c->d_srec, c->d_counters, c->c_max, c->n_sm, &c->ls, st);
     ++launches;
   }
   mark(EV_GEN);
@@ -347,12 +350,12 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
       CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER1, 0, sizeof(unsigned long long), st));
     }
     launch_raster(c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters,
-                  count && !po.ms_k, po.ms_k, pp, 0, nullptr, c->n_sm, st, fused ? c->c_max : 0u);
+                  count && !po.ms_k, po.ms_k, pp, 0, nullptr, c->n_sm, &c->ls, st, fused ? c->c_max : 0u);
     ++launches;
     if (two_pass || (!front && c->last_two_pass)) {
       launch_hiz(gbuf, w, h, c->d_hiz, c->d_counters, st);
       launch_raster(c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, gbuf, c->d_counters,
-                    false, 0, pp, 1, c->d_hiz, c->n_sm, st, fused ? c->c_max : 0u);
+                    false, 0, pp, 1, c->d_hiz, c->n_sm, &c->ls, st, fused ? c->c_max : 0u);
       launches += 2;
     }
   }
@@ -369,7 +372,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   mark(EV_SHADE);
   if ((stage_mask & 4u) && !po.ms_k) {
     launches += launch_filter(c->d_scene, c->d_srec, c->d_vertices, k, sp, gbuf, c->d_colour,
-                              (const float4*)scene_rgb, (float4*)rgb, c->d_counters, count, st);
+                              (const float4*)scene_rgb, (float4*)rgb, c->d_counters, count, &c->ls, st);
   }
   mark(EV_FILTER);
   CK(cudaGetLastError());
@@ -402,6 +405,7 @@ int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream) {
             cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, cuda_device) == cudaSuccess &&
             cudaMalloc((void**)&c->d_scene, sizeof(SceneDev)) == cudaSuccess &&
             cudaMalloc((void**)&c->d_counters, CNT_N * sizeof(unsigned long long)) == cudaSuccess &&
+            cudaMalloc((void**)&c->d_sink, sizeof(unsigned long long)) == cudaSuccess &&
             cudaMemset(c->d_counters, 0, CNT_N * sizeof(unsigned long long)) == cudaSuccess &&
             cudaMallocHost((void**)&c->h_counters, CNT_N * sizeof(unsigned long long)) == cudaSuccess &&
             cudaHostAlloc((void**)&c->h_want, sizeof(uint32_t), cudaHostAllocMapped) == cudaSuccess &&
@@ -427,7 +431,7 @@ int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream) {
 void hair_destroy(hair_ctx* c) {
   if (!c) return;
   cudaSetDevice(c->device);
-  if (c->stream || true) cudaStreamSynchronize(c->stream);
+  cudaStreamSynchronize(c->stream);
   for (auto& g : c->grooms) free_groom(g);
   cudaFree(c->d_scene);
   cudaFree(c->d_table);
@@ -440,6 +444,7 @@ void hair_destroy(hair_ctx* c) {
   cudaFree(c->d_zrange);
   cudaFree(c->d_hiz);
   cudaFree(c->d_counters);
+  cudaFree(c->d_sink);
   if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
   for (int k = 0; k < HAIR_HOST_SLOTS; ++k) {
     cudaFree(c->d_own_gbuf[k]);
@@ -617,6 +622,10 @@ int hair_mesh_clear(hair_ctx* c) {
   c->vertex_need = 0;
   c->c_max = 0;
   c->n_inst = 0;
+  c->zrange_cap = 0;  // the per-instance depth ranges of the two-pass split restart empty (one pass on the next frame)
+  c->frame_no = 0;
+  if (c->h_want) *c->h_want = 0u;
+  c->last_two_pass = false;
   c->scene_dirty = true;
   return HAIR_OK;
 }
@@ -770,6 +779,7 @@ int hair_stats(hair_ctx* c, hair_stats_t* out) {
     out->n_atomics_center = k[CNT_AT_CENTER];
     out->n_atomics_cons = k[CNT_AT_CONS];
     out->n_atomics_issued = k[CNT_AT_ISSUED];
+    out->n_atomics_cons_ymajor = k[CNT_AT_CONS_Y];
     out->n_segments_live = (uint32_t)k[CNT_SEG_LIVE];
     out->n_pixels_center = (uint32_t)k[CNT_PX_CENTER];
     out->n_pixels_cons = (uint32_t)k[CNT_PX_CONS];
@@ -833,6 +843,29 @@ int hair_atomic_microbench(hair_ctx* c, int mode, uint64_t* dev_words, uint64_t 
   cudaEventDestroy(a);
   cudaEventDestroy(b);
   CK(cudaGetLastError());
+  return HAIR_OK;
+}
+
+int hair_l2_load_microbench(hair_ctx* c, int mode, const uint64_t* dev_pairs, uint64_t n_pairs, uint32_t pitch,
+                            uint32_t n_steps, uint64_t* out_loads, float* out_ms) {
+  if (!c || !dev_pairs || !out_ms || !out_loads || mode < 0 || mode > 2 || pitch < 64 || n_pairs < 64ull * pitch ||
+      n_pairs >= (1ull << 32) || n_steps == 0 || (n_steps & 3u))
+    return HAIR_E_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  cudaEvent_t a, b;
+  CK(cudaEventCreate(&a));
+  CK(cudaEventCreate(&b));
+  CK(cudaEventRecord(a, c->stream));
+  // the sink is never written (the kernel's guard is false for any real buffer): the counters' last word serves
+  launch_l2_load_microbench(mode, (const unsigned long long*)dev_pairs, (uint32_t)n_pairs, pitch, n_steps,
+                            c->d_sink, c->n_sm, c->stream);
+  CK(cudaEventRecord(b, c->stream));
+  CK(cudaEventSynchronize(b));
+  CK(cudaEventElapsedTime(out_ms, a, b));
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  CK(cudaGetLastError());
+  *out_loads = (uint64_t)c->n_sm * 8ull * 256ull * n_steps;
   return HAIR_OK;
 }
 

@@ -95,6 +95,7 @@ enum {
   CNT_WORK_RASTER1,  // queue head of the second (far) raster pass
   CNT_HIZ_ON,        // 1: the frame is drawn in two depth-ordered passes with a tile hi-Z between them
   CNT_SEG_HIZ,       // segments dropped by the hi-Z test of the second pass
+  CNT_AT_CONS_Y,     // conservative hits of y-major segments (lanes of a warp then sit in different rows)
   CNT_N
 };
 
@@ -215,6 +216,16 @@ __device__ __forceinline__ Loc locate_strand(const uint2* __restrict__ srec, uin
   return l;
 }
 
+// per-context launch state: cudaFuncSetAttribute (dynamic shared memory opt-in) and the occupancy it implies are per
+// DEVICE, and a context is bound to one device, so what has been configured lives in hair_ctx — no function statics
+struct LaunchState {
+  int raster_per_sm[32] = {};      // index = COUNT | MS << 1 | PP << 2 | HZ << 3 | FUSED << 4
+  size_t raster_smem[32] = {};
+  int gen_per_sm = 0;
+  size_t gen_smem = 0;
+  bool filter_set[8] = {};
+};
+
 // ------------------------------------------------------------------ launchers (one per .cu)
 // zrange: [2][n_inst][2] u32 (float bits of min / max bundle depth per instance), ping-pong by frame parity;
 // grp: two exclusive scans of n_bi + 1 entries (near pass, far pass); two_pass = false draws everything in the first
@@ -224,13 +235,13 @@ void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaA
 void launch_hiz(const unsigned long long* gbuf, uint32_t W, uint32_t H, uint32_t* hiz,
                 const unsigned long long* counters, cudaStream_t st);
 void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices, uint2* srec,
-                     unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st);
+                     unsigned long long* counters, uint32_t c_max, int n_sm, LaunchState* ls, cudaStream_t st);
 void launch_clear(unsigned long long* gbuf, size_t n_pixels, const float* scene_zn, cudaStream_t st);
 void launch_reseed(unsigned long long* gbuf, size_t n_pixels, cudaStream_t st);
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                    unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int pass,
-                   const uint32_t* hiz, int n_sm, cudaStream_t st, uint32_t fused_c_max = 0);
+                   const uint32_t* hiz, int n_sm, LaunchState* ls, cudaStream_t st, uint32_t fused_c_max = 0);
 void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
                          float4* out, cudaStream_t st);
@@ -238,6 +249,9 @@ void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vert
                   ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st);
 int launch_filter(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                    ShadeParams sp, const unsigned long long* gbuf, const float4* colour, const float4* scene_rgb,
-                   float4* out, unsigned long long* counters, bool count, cudaStream_t st);
+                   float4* out, unsigned long long* counters, bool count, LaunchState* ls, cudaStream_t st);
 void launch_atomic_microbench(int mode, unsigned long long* words, unsigned long long n_words,
                               unsigned long long n_ops, uint32_t hot, int n_sm, cudaStream_t st);
+// n_steps loads per thread of n_sm * 8 CTAs of 256 threads; sink: one device word nothing is ever written to
+void launch_l2_load_microbench(int mode, const unsigned long long* pairs, uint32_t n_pairs, uint32_t pitch,
+                               uint32_t n_steps, unsigned long long* sink, int n_sm, cudaStream_t st);

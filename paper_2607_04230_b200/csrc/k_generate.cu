@@ -95,16 +95,16 @@ k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restri
 }
 
 void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, float4* vertices, uint2* srec,
-                     unsigned long long* counters, uint32_t c_max, int n_sm, cudaStream_t st) {
+                     unsigned long long* counters, uint32_t c_max, int n_sm, LaunchState* ls, cudaStream_t st) {
   size_t smem = (size_t)GEN_WARPS * ((size_t)c_max * HAIR_ROW + 32 * 5) * sizeof(float);
-  static size_t configured = 0;
-  if (smem > configured) {
+  if (!ls->gen_per_sm || smem != ls->gen_smem) {  // once per context and table size (the opt-in is per device)
     cudaFuncSetAttribute(k_generate, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = smem;
+    int b = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_generate, GEN_WARPS * 32, smem);
+    ls->gen_per_sm = b > 0 ? b : 1;
+    ls->gen_smem = smem;
   }
-  int per_sm = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_generate, GEN_WARPS * 32, smem);
-  if (per_sm < 1) per_sm = 1;
+  const int per_sm = ls->gen_per_sm;
   uint32_t grid = (uint32_t)(n_sm * per_sm);
   uint32_t need = (n_bi + GEN_WARPS - 1) / GEN_WARPS;
   if (grid > need) grid = need;

@@ -175,9 +175,10 @@ __global__ void __launch_bounds__(1024) k_lod(const SceneDev* __restrict__ sc, u
 }
 
 // Exclusive scans of N_LOD, N_LOD*C and the raster's work-group count over bundle-instances in
-// index order (O1 step 6). One CTA of 1024 threads; each warp owns a contiguous range and
-// walks it 32 entries at a time with a shuffle scan and a running carry; the 32 warp totals are
-// scanned by warp 0; a second pass adds the warp offsets. Coalesced 16-byte accesses throughout.
+// index order (O1 step 6). One CTA of 256 threads per tile of 256 bundle-instances: (1) every CTA sums
+// the tile totals k_lod left in `part` for the tiles in front of its own (and the frame's vertex total), (2) a
+// shuffle scan per warp plus the 8 warp totals gives the exclusive scan inside the tile, (3) the last tile writes the
+// device-side totals and queue lengths. Coalesced 16-byte accesses throughout.
 
 __global__ void __launch_bounds__(256) k_scan(uint4* __restrict__ table, uint32_t* __restrict__ grp, uint32_t n_bi,
                                               const uint4* __restrict__ part, unsigned long long* __restrict__ counters,

@@ -75,7 +75,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
   __shared__ __align__(16) float s_rec[RAS_WARPS][32][RS];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float(*rec)[RS] = s_rec[warp];
-  uint32_t c_center = 0, c_cons = 0, c_drawn = 0, c_issued = 0, c_live = 0, c_hiz = 0;
+  uint32_t c_center = 0, c_cons = 0, c_cons_y = 0, c_drawn = 0, c_issued = 0, c_live = 0, c_hiz = 0;
   const int W = (int)cam.W, H = (int)cam.H;
   const int hiz_w = (W + HIZ_TILE - 1) / HIZ_TILE;
   const uint32_t le_mask = 0xFFFFFFFFu >> (31 - lane);
@@ -363,6 +363,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
             unsigned long long* px = pcol + (size_t)r * pstep;
             if (COUNT) {
               ++c_cons;
+              c_cons_y += ymajor ? 1u : 0u;
               c_center += centre ? 1u : 0u;
             }
             if (word < cur[i].y) {
@@ -390,6 +391,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
     for (int d = 16; d > 0; d >>= 1) {
       c_center += __shfl_xor_sync(0xffffffffu, c_center, d);
       c_cons += __shfl_xor_sync(0xffffffffu, c_cons, d);
+      c_cons_y += __shfl_xor_sync(0xffffffffu, c_cons_y, d);
       c_drawn += __shfl_xor_sync(0xffffffffu, c_drawn, d);
       c_issued += __shfl_xor_sync(0xffffffffu, c_issued, d);
       c_live += __shfl_xor_sync(0xffffffffu, c_live, d);
@@ -397,6 +399,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
     if (lane == 0) {
       atomicAdd(&counters[CNT_AT_CENTER], (unsigned long long)c_center);
       atomicAdd(&counters[CNT_AT_CONS], (unsigned long long)c_cons);
+      atomicAdd(&counters[CNT_AT_CONS_Y], (unsigned long long)c_cons_y);
       atomicAdd(&counters[CNT_SEG_DRAWN], (unsigned long long)c_drawn);
       atomicAdd(&counters[CNT_AT_ISSUED], (unsigned long long)c_issued);
       atomicAdd(&counters[CNT_SEG_LIVE], (unsigned long long)c_live);
@@ -475,18 +478,18 @@ template <bool COUNT, bool MS, bool PP, bool HZ, bool FUSED = false>
 static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                             const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                             unsigned long long* counters, uint32_t ms_k, uint32_t queue, const uint32_t* hiz, int n_sm,
-                            cudaStream_t st, uint32_t c_max = 0) {
+                            LaunchState* ls, cudaStream_t st, uint32_t c_max = 0) {
   // persistent grid: every CTA slot of the device, the queue feeds them
   const size_t smem = FUSED ? (size_t)RAS_WARPS * c_max * HAIR_ROW * sizeof(float) : 0;  // the warps' spline tables
-  static int per_sm = 0;
-  static size_t configured = 0;
-  if (!per_sm || smem > configured) {
+  constexpr int V = (COUNT ? 1 : 0) | (MS ? 2 : 0) | (PP ? 4 : 0) | (HZ ? 8 : 0) | (FUSED ? 16 : 0);
+  if (!ls->raster_per_sm[V] || smem != ls->raster_smem[V]) {  // once per context (= device) and table size
     if (smem) cudaFuncSetAttribute(k_raster<COUNT, MS, PP, HZ, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     int b = 0;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<COUNT, MS, PP, HZ, FUSED>, RAS_WARPS * 32, smem);
-    per_sm = b > 0 ? b : 1;
-    configured = smem;
+    ls->raster_per_sm[V] = b > 0 ? b : 1;
+    ls->raster_smem[V] = smem;
   }
+  const int per_sm = ls->raster_per_sm[V];
   k_raster<COUNT, MS, PP, HZ, FUSED><<<(uint32_t)(n_sm * per_sm), RAS_WARPS * 32, smem, st>>>(
       d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, ms_k, queue, hiz, c_max);
 }
@@ -496,41 +499,18 @@ static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4*
 void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                    unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int pass,
-                   const uint32_t* hiz, int n_sm, cudaStream_t st, uint32_t fused_c_max) {
+                   const uint32_t* hiz, int n_sm, LaunchState* ls, cudaStream_t st, uint32_t fused_c_max) {
   const uint32_t* gp = grp + (pass ? (size_t)n_bi + 1 : 0);
   const uint32_t q = pass ? CNT_WORK_RASTER1 : CNT_WORK_RASTER;
 #define RAS_ARGS d_scene, n_bi, table, gp, vertices, cam, rho_default, gbuf, counters
-  if (fused_c_max && pass) launch_raster_t<false, false, true, true, true>(RAS_ARGS, 0, q, hiz, n_sm, st, fused_c_max);
-  else if (fused_c_max) launch_raster_t<false, false, true, false, true>(RAS_ARGS, 0, q, nullptr, n_sm, st, fused_c_max);
-  else if (ms_k) launch_raster_t<false, true, false, false>(RAS_ARGS, ms_k, q, nullptr, n_sm, st);
-  else if (paper_payload && count) launch_raster_t<true, false, true, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);
-  else if (paper_payload && pass) launch_raster_t<false, false, true, true>(RAS_ARGS, 0, q, hiz, n_sm, st);
-  else if (paper_payload) launch_raster_t<false, false, true, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);
-  else if (count) launch_raster_t<true, false, false, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);
-  else if (pass) launch_raster_t<false, false, false, true>(RAS_ARGS, 0, q, hiz, n_sm, st);
-  else launch_raster_t<false, false, false, false>(RAS_ARGS, 0, q, nullptr, n_sm, st);
+  if (fused_c_max && pass) launch_raster_t<false, false, true, true, true>(RAS_ARGS, 0, q, hiz, n_sm, ls, st, fused_c_max);
+  else if (fused_c_max) launch_raster_t<false, false, true, false, true>(RAS_ARGS, 0, q, nullptr, n_sm, ls, st, fused_c_max);
+  else if (ms_k) launch_raster_t<false, true, false, false>(RAS_ARGS, ms_k, q, nullptr, n_sm, ls, st);
+  else if (paper_payload && count) launch_raster_t<true, false, true, false>(RAS_ARGS, 0, q, nullptr, n_sm, ls, st);
+  else if (paper_payload && pass) launch_raster_t<false, false, true, true>(RAS_ARGS, 0, q, hiz, n_sm, ls, st);
+  else if (paper_payload) launch_raster_t<false, false, true, false>(RAS_ARGS, 0, q, nullptr, n_sm, ls, st);
+  else if (count) launch_raster_t<true, false, false, false>(RAS_ARGS, 0, q, nullptr, n_sm, ls, st);
+  else if (pass) launch_raster_t<false, false, false, true>(RAS_ARGS, 0, q, hiz, n_sm, ls, st);
+  else launch_raster_t<false, false, false, false>(RAS_ARGS, 0, q, nullptr, n_sm, ls, st);
 #undef RAS_ARGS
-}
-
-// ------------------------------------------------------------------ L2-atomic roofline micro-kernels
-// 64-bit atomicMin with the result unused (RED.E.MIN.64), the raster's own operation.
-__global__ void __launch_bounds__(256) k_atomic_bench(int mode, unsigned long long* __restrict__ words,
-                                                      unsigned long long n_words, unsigned long long n_ops,
-                                                      uint32_t hot) {
-  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_ops; i += stride) {
-    unsigned long long idx;
-    if (mode == 0) idx = i % n_words;                                   // own word, coalesced
-    else {
-      uint32_t h = pcg((uint32_t)i ^ pcg((uint32_t)(i >> 32) + 0x9E3779B9u));
-      unsigned long long r = ((unsigned long long)h << 32) | pcg(h + 1u);
-      idx = mode == 1 ? r % n_words : (unsigned long long)(h % hot) * (n_words / hot);  // random / hot set
-    }
-    atomicMin(&words[idx], (i << 8) | 1ull);
-  }
-}
-
-void launch_atomic_microbench(int mode, unsigned long long* words, unsigned long long n_words,
-                              unsigned long long n_ops, uint32_t hot, int n_sm, cudaStream_t st) {
-  k_atomic_bench<<<n_sm * 8, 256, 0, st>>>(mode, words, n_words, n_ops, hot ? hot : 1u);
 }

@@ -585,17 +585,20 @@ void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vert
 template <int R>
 static void launch_filter_r(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                             ShadeParams sp, const unsigned long long* gbuf, const float4* colour,
-                            const float4* scene_rgb, float4* out, cudaStream_t st) {
+                            const float4* scene_rgb, float4* out, LaunchState* ls, cudaStream_t st) {
   constexpr int NS = (FT_W + 2 * R) * (FT_H + 2 * R);
   constexpr size_t smem = (size_t)NS * (sizeof(float4) + 3 * sizeof(uint32_t)) + 2 * FT_W * FT_H * sizeof(float4);
-  cudaFuncSetAttribute(k_filter<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (!ls->filter_set[R]) {  // once per context (the opt-in is per device)
+    cudaFuncSetAttribute(k_filter<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    ls->filter_set[R] = true;
+  }
   dim3 grid((cam.W + FT_W - 1) / FT_W, (cam.H + FT_H - 1) / FT_H);
   k_filter<R><<<grid, 256, smem, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out);
 }
 
 int launch_filter(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                   ShadeParams sp, const unsigned long long* gbuf, const float4* colour, const float4* scene_rgb,
-                  float4* out, unsigned long long* counters, bool count, cudaStream_t st) {
+                  float4* out, unsigned long long* counters, bool count, LaunchState* ls, cudaStream_t st) {
   const size_t n = (size_t)cam.W * cam.H;
   int launches = 1;
   if (count) {
@@ -607,14 +610,14 @@ int launch_filter(const SceneDev* d_scene, const uint2* srec, const float4* vert
     return launches;
   }
   switch (sp.r) {
-    case 0: launch_filter_r<0>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 1: launch_filter_r<1>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 2: launch_filter_r<2>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 3: launch_filter_r<3>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 4: launch_filter_r<4>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 5: launch_filter_r<5>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    case 6: launch_filter_r<6>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
-    default: launch_filter_r<7>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, st); break;
+    case 0: launch_filter_r<0>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, ls, st); break;
+    case 1: launch_filter_r<1>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, ls, st); break;
+    case 2: launch_filter_r<2>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, ls, st); break;
+    case 3: launch_filter_r<3>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, ls, st); break;
+    case 4: launch_filter_r<4>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, ls, st); break;
+    case 5: launch_filter_r<5>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, ls, st); break;
+    case 6: launch_filter_r<6>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, ls, st); break;
+    default: launch_filter_r<7>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out, ls, st); break;
   }
   return launches;
 }

@@ -111,6 +111,19 @@ def look_from_z(center, distance, width, height):
                 vfov_y=VFOV, near_z=NEAR, far_z=FAR, width=int(width), height=int(height))
 
 
+def moving_camera(cam: dict, i: int, yaw_step=0.004, dolly_step=0.004):
+    """Frame i of a slow orbit of `cam`: yaw about the up axis by i * yaw_step rad while the eye swings sideways and
+    dollies in and out (up to ~10 px of image motion per frame at 4K) — a bench leg whose depth ranges and hi-Z are one frame stale."""
+    a = yaw_step * 10.0 * math.sin(i * 0.1)
+    ca, sa = math.cos(a), math.sin(a)
+    r, u, f = (np.asarray(cam[k], np.float64) for k in ("right", "up", "forward"))
+    r2, f2 = ca * r + sa * f, ca * f - sa * r
+    eye = np.asarray(cam["eye"], np.float64) + dolly_step * 10.0 * (math.sin(i * 0.07) * r + (1.0 - math.cos(i * 0.05)) * f)
+    out = dict(cam)
+    out.update(eye=tuple(float(v) for v in eye), right=tuple(float(v) for v in r2), forward=tuple(float(v) for v in f2))
+    return out
+
+
 def lights_around(rng, center, scale=1.0):
     out = []
     for i in range(3):  # PAPER.md:200 "three point light sources"
