@@ -102,6 +102,10 @@ def lib():
         L.orc_frame_get_table.argtypes = [vp, vp, vp]
         L.orc_frame_set_table.argtypes = [vp, vp, u32]
         L.orc_frame_generate.argtypes = [vp]
+        L.orc_frame_beta.restype = None
+        L.orc_frame_beta.argtypes = [vp, vp, vp, vp]
+        L.orc_depth_fix.restype = C.c_double
+        L.orc_depth_fix.argtypes = [C.c_double, C.c_double]
         L.orc_frame_get_vertices_f64.argtypes = [vp, vp]
         L.orc_frame_get_vertices_f32.argtypes = [vp, vp]
         L.orc_frame_set_vertices_f32.argtypes = [vp, vp, u64]
@@ -291,6 +295,12 @@ class Frame:
         if r != 0:
             raise ValueError(f"orc_frame_set_table: {r}")
 
+    def beta(self):
+        """Eq. 6-8 from the current table: (beta per groom, delta = -ln beta per groom, beta_min over drawn bundles)."""
+        b, d, m = np.zeros(self._n_grooms), np.zeros(self._n_grooms), C.c_double(1.0)
+        self.L.orc_frame_beta(self.h, _ptr(b), _ptr(d), C.byref(m))
+        return b, d, m.value
+
     # ---- O2
     def generate(self) -> None:
         assert self.L.orc_frame_generate(self.h) == 0
@@ -471,6 +481,11 @@ def pcg(v: int) -> int:
 
 def hash3(seed: int, i: int, stream: int) -> int:
     return lib().orc_hash3(seed, i, stream)
+
+
+def depth_fix(d: float, delta: float) -> float:
+    """Eq. 7-8: the depth a thinned groom is tested at, d exp(-delta)."""
+    return float(lib().orc_depth_fix(float(d), float(delta)))
 
 
 def lod_counts(L: float, N: int, delta: float, n_layers: int, c_full: int):

@@ -857,6 +857,30 @@ uint32_t orc_frame_n_strands_total(const orc_frame* f) {
   for (const Groom& g : f->grooms) n += g.N * g.Q;
   return n;
 }
+// Eq. 6-8: beta = N_remaining / N_total, delta = -log(beta)
+void orc_frame_beta(const orc_frame* f, double* beta, double* delta, double* beta_min) {
+  size_t gid = 0;
+  double bmin = 1.0;
+  for (size_t gi = 0; gi < f->grooms.size(); ++gi) {
+    const Groom& g = f->grooms[gi];
+    uint64_t remaining = 0, total = 0;
+    for (uint32_t q = 0; q < g.Q; ++q)
+      for (uint32_t t = 0; t < g.T; ++t, ++gid) {
+        const uint32_t nlod = f->table[gid].nlod, N = g.npt[t];
+        if (nlod == 0) continue;  // not drawn: frustum-culled, masked, or an empty bundle
+        remaining += nlod;
+        total += N;
+        bmin = std::min(bmin, double(nlod) / double(N));
+      }
+    const double b = total ? double(remaining) / double(total) : 1.0;
+    if (beta) beta[gi] = b;
+    if (delta) delta[gi] = -std::log(b);  // Eq. 8
+  }
+  if (beta_min) *beta_min = bmin;
+}
+// Eq. 7: V'(d) = exp(-sigma (beta d)): thinning to the fraction beta = traversing the depth beta d = d exp(-delta)
+double orc_depth_fix(double d, double delta) { return d * std::exp(-delta); }
+
 uint32_t orc_frame_n_strands(const orc_frame* f) { return f->n_strands; }
 uint64_t orc_frame_n_vertices(const orc_frame* f) { return f->n_vertices; }
 void orc_frame_get_table(const orc_frame* f, uint32_t* t4, float* L) {

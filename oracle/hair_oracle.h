@@ -105,6 +105,17 @@ void orc_frame_get_table(const orc_frame*, uint32_t* table4, float* L);
 /* replace the table (e.g. by the CUDA path's, for stage-wise parity). Recomputes nothing else. */
 int orc_frame_set_table(orc_frame*, const uint32_t* table4, uint32_t n);
 
+/* Depth-comparison fix (§3.2.3, Eq. 6-8; DESIGN.md R-beta), from the current table:
+ *  beta[g]  = N_remaining / N_total of groom g = sum N_LOD / sum N over its bundle-instances that are drawn
+ *             (N_LOD > 0; frustum-culled bundles are outside the view, not stochastically thinned); 1 if none
+ *  delta[g] = -ln beta[g]                                                            (Eq. 8)
+ *  *beta_min = min over all drawn bundle-instances of N_LOD / N (the most thinned bundle); 1 if none.
+ * beta, delta: one double per groom. */
+void orc_frame_beta(const orc_frame*, double* beta, double* delta, double* beta_min);
+/* Eq. 7-8: a depth d INTO the groom (optical-depth axis, sigma * d), tested after stochastic thinning to the fraction
+ * beta = exp(-delta): the additive shift -delta in log-depth space, ln d_eff = ln d - delta, i.e. d_eff = d exp(-delta) */
+double orc_depth_fix(double d, double delta);
+
 /* O2: vertices for the current table. fp64 result, and its fp32 rounding. */
 int orc_frame_generate(orc_frame*);
 void orc_frame_get_vertices_f64(const orc_frame*, double* xyz_ao);
