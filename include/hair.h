@@ -211,7 +211,14 @@ typedef struct {
   /* stage-timing flag: mean over the frames rendered since the previous hair_stats (last 64 at most) */
   float ms_lod, ms_generate, ms_clear, ms_raster, ms_shade, ms_filter, ms_total;
   uint32_t n_timed_frames;
-  float beta_mean; /* N_remaining / N_total of Eq. 8 over all grooms */
+  float beta_mean; /* strands after LOD / strands uploaded, over all grooms (frustum-culled bundles count as removed) */
+  /* Depth-comparison fix (Eq. 6-8; DESIGN.md R-beta), for the consumer of a depth / opacity map
+   * that was built from the full groom: beta_groom[g] = N_remaining / N_total of groom g over its DRAWN
+   * bundle-instances (N_LOD > 0), 1 if none; delta_groom[g] = -ln beta (Eq. 8): a depth d into the groom is to be
+   * tested at d exp(-delta) (the additive shift -delta in log depth, Eq. 7); beta_min = the most thinned drawn
+   * bundle-instance's N_LOD / N. Sums are taken on the device by the scan of every frame. */
+  float beta_min;
+  float beta_groom[HAIR_MAX_GROOMS], delta_groom[HAIR_MAX_GROOMS];
   uint32_t gpu_launches; /* kernels launched by the last hair_render */
   uint32_t two_pass;              /* 1: the last frame was drawn in two depth-ordered raster passes */
   uint32_t n_segments_hiz_culled; /* segments of the second pass dropped by the tile hi-Z test before any pixel work */

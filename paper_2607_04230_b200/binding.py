@@ -72,11 +72,13 @@ class hair_stats_t(C.Structure):
                 ("n_pixels_center", C.c_uint32), ("n_pixels_cons", C.c_uint32),
                 ("ms_lod", C.c_float), ("ms_generate", C.c_float), ("ms_clear", C.c_float),
                 ("ms_raster", C.c_float), ("ms_shade", C.c_float), ("ms_filter", C.c_float),
-                ("ms_total", C.c_float), ("n_timed_frames", C.c_uint32), ("beta_mean", C.c_float), ("gpu_launches", C.c_uint32),
+                ("ms_total", C.c_float), ("n_timed_frames", C.c_uint32), ("beta_mean", C.c_float),
+                ("beta_min", C.c_float), ("beta_groom", C.c_float * 16), ("delta_groom", C.c_float * 16),
+                ("gpu_launches", C.c_uint32),
                 ("two_pass", C.c_uint32), ("n_segments_hiz_culled", C.c_uint32)]
 
     def as_dict(self):
-        return {k: getattr(self, k) for k, _ in self._fields_}
+        return {k: (list(getattr(self, k)) if k in ("beta_groom", "delta_groom") else getattr(self, k)) for k, _ in self._fields_}
 
 
 _lib = None

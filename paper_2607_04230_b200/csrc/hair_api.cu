@@ -774,6 +774,18 @@ int hair_stats(hair_ctx* c, hair_stats_t* out) {
   out->two_pass = (uint32_t)k[CNT_HIZ_ON];
   out->n_segments_hiz_culled = (uint32_t)k[CNT_SEG_HIZ];
   out->beta_mean = c->scene.n_strands_total ? (float)((double)k[CNT_STRANDS] / (double)c->scene.n_strands_total) : 1.f;
+  // Eq. 8: per-groom beta from the device-side sums of the frame's scan, delta = -log(beta)
+  out->beta_min = 1.f;
+  for (uint32_t g = 0; g < HAIR_MAX_GROOMS; ++g) {
+    const unsigned long long num = k[CNT_BETA_NUM + g], den = k[CNT_BETA_DEN + g];
+    const double b = (g < c->scene.n_grooms && den) ? (double)num / (double)den : 1.0;
+    out->beta_groom[g] = (float)b;
+    out->delta_groom[g] = (float)-std::log(b);
+  }
+  if (c->scene.n_bi) {
+    const uint32_t bits = (uint32_t)k[CNT_BETA_MIN];
+    memcpy(&out->beta_min, &bits, sizeof(float));
+  }
   if (c->counted) {
     out->n_segments_drawn = (uint32_t)k[CNT_SEG_DRAWN];
     out->n_atomics_center = k[CNT_AT_CENTER];

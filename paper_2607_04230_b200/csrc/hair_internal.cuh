@@ -96,6 +96,12 @@ enum {
   CNT_HIZ_ON,        // 1: the frame is drawn in two depth-ordered passes with a tile hi-Z between them
   CNT_SEG_HIZ,       // segments dropped by the hi-Z test of the second pass
   CNT_AT_CONS_Y,     // conservative hits of y-major segments (lanes of a warp then sit in different rows)
+  CNT_RESET_END,     // k_scan's last tile zeroes [CNT_SEG_DRAWN, CNT_RESET_END) for the kernels behind it
+  // Eq. 8: per groom, strands remaining / strands in total over the DRAWN bundle-instances; zeroed by
+  // k_lod, accumulated by k_scan (every tile), read by hair_stats
+  CNT_BETA_NUM = CNT_RESET_END,
+  CNT_BETA_DEN = CNT_BETA_NUM + HAIR_MAX_GROOMS,
+  CNT_BETA_MIN = CNT_BETA_DEN + HAIR_MAX_GROOMS,  // float bits of the smallest N_LOD / N of a drawn bundle-instance
   CNT_N
 };
 

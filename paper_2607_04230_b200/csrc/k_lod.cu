@@ -36,7 +36,10 @@ __device__ __forceinline__ uint32_t raster_groups(uint32_t n_v) {  // units of R
 __global__ void __launch_bounds__(1024) k_lod(const SceneDev* __restrict__ sc, uint32_t n_bi, CamDev cam,
                                               LambdaArr lam, uint32_t groom_mask, uint4* __restrict__ table,
                                               uint4* __restrict__ part, const uint32_t* __restrict__ zr_prev,
-                                              uint32_t* __restrict__ zr_cur, uint32_t two_pass) {
+                                              uint32_t* __restrict__ zr_cur, uint32_t two_pass,
+                                              unsigned long long* __restrict__ counters) {
+  if (blockIdx.x == 0 && threadIdx.x <= 2 * HAIR_MAX_GROOMS)  // Eq. 8 sums restart (k_scan accumulates them)
+    counters[CNT_BETA_NUM + threadIdx.x] = threadIdx.x == 2 * HAIR_MAX_GROOMS ? 0x3F800000ull : 0ull;
   const uint32_t sub = threadIdx.x & 3u;
   const uint32_t gid = blockIdx.x * 256u + (threadIdx.x >> 2);
   const bool live = gid < n_bi;
@@ -180,12 +183,15 @@ __global__ void __launch_bounds__(1024) k_lod(const SceneDev* __restrict__ sc, u
 // shuffle scan per warp plus the 8 warp totals gives the exclusive scan inside the tile, (3) the last tile writes the
 // device-side totals and queue lengths. Coalesced 16-byte accesses throughout.
 
-__global__ void __launch_bounds__(256) k_scan(uint4* __restrict__ table, uint32_t* __restrict__ grp, uint32_t n_bi,
+__global__ void __launch_bounds__(256) k_scan(const SceneDev* __restrict__ sc, uint4* __restrict__ table,
+                                              uint32_t* __restrict__ grp, uint32_t n_bi,
                                               const uint4* __restrict__ part, unsigned long long* __restrict__ counters,
                                               uint32_t* __restrict__ zr_reset, uint32_t n_inst, uint32_t two_pass,
                                               uint32_t* __restrict__ want_two_pass) {
   __shared__ uint32_t s_a[8][5], s_b[8][4], s_tot[8];
+  __shared__ uint32_t s_beta[2 * HAIR_MAX_GROOMS + 1];  // per groom: strands kept, strands in total; min ratio (float bits)
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tile = blockIdx.x;
+  if (threadIdx.x <= 2 * HAIR_MAX_GROOMS) s_beta[threadIdx.x] = threadIdx.x == 2 * HAIR_MAX_GROOMS ? 0x3F800000u : 0u;
   uint32_t* grp1 = grp + n_bi + 1;
   // (1) what lies before this tile: sums of the tiles in front of it; and the frame's total of vertices
   uint32_t ps = 0, pv = 0, pg = 0, pf = 0, pc = 0, tot = 0;
@@ -216,6 +222,17 @@ __global__ void __launch_bounds__(256) k_scan(uint4* __restrict__ table, uint32_
   const uint32_t i = tile * 256 + threadIdx.x;
   uint4 e = i < n_bi ? table[i] : make_uint4(0, 0, 0, 0);
   const uint32_t s = e.x, v = e.x * e.y, ng = raster_groups(v);
+  // Eq. 8: beta = N_remaining / N_total of each groom over its drawn bundle-instances
+  if (s) {
+    uint32_t gi = 0;
+    for (uint32_t k = 1; k < sc->n_grooms; ++k)
+      if (i >= sc->g[k].gid_base) gi = k;
+    const GroomDev& gr = sc->g[gi];
+    const uint32_t N = __ldg(&gr.npt[(i - gr.gid_base) % gr.T]);
+    atomicAdd(&s_beta[gi], s);
+    atomicAdd(&s_beta[HAIR_MAX_GROOMS + gi], N);
+    atomicMin(&s_beta[2 * HAIR_MAX_GROOMS], __float_as_uint(__fdiv_rn((float)s, (float)N)));  // positive floats order like their bits
+  }
   const bool far_pass = two && e.z != 0u;
   const uint32_t g = far_pass ? 0u : ng, f = far_pass ? ng : 0u;
   uint32_t is = s, iv = v, ig = g, jf = f;
@@ -247,6 +264,11 @@ __global__ void __launch_bounds__(256) k_scan(uint4* __restrict__ table, uint32_
     grp[i] = off_g + ig - g;
     grp1[i] = off_f + jf - f;
   }
+  // (s_beta is complete: the __syncthreads above follows every thread's atomics)
+  if (threadIdx.x < 2 * HAIR_MAX_GROOMS) {
+    if (s_beta[threadIdx.x]) atomicAdd(&counters[CNT_BETA_NUM + threadIdx.x], (unsigned long long)s_beta[threadIdx.x]);
+  } else if (threadIdx.x == 2 * HAIR_MAX_GROOMS)
+    atomicMin(&counters[CNT_BETA_MIN], (unsigned long long)s_beta[2 * HAIR_MAX_GROOMS]);
   // the depth ranges the previous frame left (k_lod has read them) restart for the frame after this one
   if (tile == 0)
     for (uint32_t k = threadIdx.x; k < n_inst; k += 256) zr_reset[2 * k] = 0x7F000000u, zr_reset[2 * k + 1] = 0u;
@@ -260,7 +282,7 @@ __global__ void __launch_bounds__(256) k_scan(uint4* __restrict__ table, uint32_
     counters[CNT_CULLED] = culled + mine_c;
     counters[CNT_WORK_GEN] = 0;
     counters[CNT_WORK_RASTER] = 0;
-    for (int k = CNT_SEG_DRAWN; k < CNT_N; ++k) counters[k] = 0;
+    for (int k = CNT_SEG_DRAWN; k < CNT_RESET_END; ++k) counters[k] = 0;
     counters[CNT_HIZ_ON] = (two && n_f > 0) ? 1ull : 0ull;
     grp[n_bi] = n_g;  // total work groups of each pass: the raster's queue lengths
     grp1[n_bi] = n_f;
@@ -275,6 +297,6 @@ void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaA
   const uint32_t n_tiles = (n_bi + 255) / 256;
   uint32_t* zr_cur = zrange + (size_t)(parity & 1u) * n_inst * 2;
   uint32_t* zr_prev = zrange + (size_t)((parity + 1u) & 1u) * n_inst * 2;
-  k_lod<<<n_tiles, 1024, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table, part, zr_prev, zr_cur, two_pass ? 1u : 0u);
-  k_scan<<<n_tiles, 256, 0, st>>>(table, grp, n_bi, part, counters, zr_prev, n_inst, two_pass ? 1u : 0u, want_two_pass);
+  k_lod<<<n_tiles, 1024, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table, part, zr_prev, zr_cur, two_pass ? 1u : 0u, counters);
+  k_scan<<<n_tiles, 256, 0, st>>>(d_scene, table, grp, n_bi, part, counters, zr_prev, n_inst, two_pass ? 1u : 0u, want_two_pass);
 }

@@ -60,6 +60,17 @@ def psnr(a, b, peak):
     return 200.0 if mse == 0 else 10.0 * math.log10(peak * peak / mse)
 
 
+def check_beta(f, stats):
+    """Eq. 8: the device-side per-groom beta = N_remaining / N_total, delta = -log(beta) and the most
+    thinned bundle against the oracle's, from the same (bit-exact) table."""
+    beta, delta, bmin = f.beta()
+    n = len(beta)
+    assert np.array_equal(np.float32(beta), np.float32(stats["beta_groom"][:n])), (beta, stats["beta_groom"])
+    assert np.allclose(delta, stats["delta_groom"][:n], rtol=0, atol=1e-6), (delta, stats["delta_groom"])
+    assert np.float32(bmin) == np.float32(stats["beta_min"]), (bmin, stats["beta_min"])
+    assert all(b == 1.0 and d == 0.0 for b, d in zip(stats["beta_groom"][n:], stats["delta_groom"][n:]))
+
+
 def check_stagewise(orc, sc, G, lam=None, payload=False, groom_mask=None):
     """Runs every stage-wise gate; returns a small report. payload: the paper's word (R-payload) on both sides."""
     cam, prm = sc["camera"], G["prm"]
@@ -71,6 +82,7 @@ def check_stagewise(orc, sc, G, lam=None, payload=False, groom_mask=None):
     t_or, _ = f.table()
     assert np.array_equal(t_or, G["table"]), "bundle table differs"
     assert G["stats"]["n_strands_lod"] == f.n_strands and G["stats"]["n_vertices"] == f.n_vertices
+    check_beta(f, G["stats"])
     # (i) vertices vs fp64 oracle
     f.generate()
     v64 = f.vertices_f64()
@@ -352,6 +364,7 @@ def check_full_size_sampled(orc, sc, G, windows, payload=False):
     t_or, _ = f.table()
     assert np.array_equal(t_or, G["table"]), "bundle table differs"
     assert G["stats"]["n_strands_lod"] == f.n_strands and G["stats"]["n_vertices"] == f.n_vertices
+    check_beta(f, G["stats"])
     f.generate()
     err_v = float(np.abs(G["verts"].astype(np.float64) - f.vertices_f64()).max())
     assert err_v <= TOL_VERTEX, f"vertex max-abs {err_v}"
