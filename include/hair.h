@@ -66,6 +66,14 @@ extern "C" {
  * HAIR_E_INVALID_ARG. The debug vertex buffer is not valid after such a frame. An A/B against the default pipeline. */
 #define HAIR_FLAG_FUSED 32u
 
+/* Sort-middle raster (PAPER.md:254 names a hybrid raster as future work): segments are binned to
+ * 64 x 64 pixel screen tiles and each tile's two G-buffer layers are resolved in SHARED memory (pixel tests are
+ * LDS.128 instead of L2 loads, a per-tile hi-Z refreshed while drawing drops occluded segments whole), then stored
+ * once. Same predicates, same words: the G-buffer equals the default raster's bit for bit. Replaces the clear and the
+ * two depth-ordered passes. Ignored (default raster) with HAIR_FLAG_COUNTERS / PAPER_PAYLOAD / FUSED and in
+ * hair_render_msaa. Needs 64 bytes of record pool per worst-case vertex (allocated on first use). */
+#define HAIR_FLAG_TILED 64u
+
 typedef struct hair_ctx hair_ctx; /* opaque; owns all device scratch */
 
 /* Creates a context on `cuda_device` that enqueues on `cuda_stream` (a cudaStream_t; NULL = the
@@ -221,7 +229,11 @@ typedef struct {
   float beta_groom[HAIR_MAX_GROOMS], delta_groom[HAIR_MAX_GROOMS];
   uint32_t gpu_launches; /* kernels launched by the last hair_render */
   uint32_t two_pass;              /* 1: the last frame was drawn in two depth-ordered raster passes */
-  uint32_t n_segments_hiz_culled; /* segments of the second pass dropped by the tile hi-Z test before any pixel work */
+  uint32_t n_segments_hiz_culled; /* segments of the second pass dropped by the tile hi-Z test before any pixel work
+                                     (HAIR_FLAG_TILED: (segment, tile) records dropped by the in-tile hi-Z) */
+  uint32_t tiled;                 /* 1: the last frame was drawn by the tile-binned raster (HAIR_FLAG_TILED) */
+  uint32_t n_tile_records;        /* its (segment, tile) records */
+  uint32_t tile_overflow;         /* 1: they exceeded the record pool and some were dropped (the frame is incomplete) */
 } hair_stats_t;
 /* Synchronises the stream and reads the device counters of the last frame. */
 int hair_stats(hair_ctx*, hair_stats_t* out);

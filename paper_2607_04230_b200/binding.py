@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(_HERE, "csrc", "libhair.so")
 
 OP_BITS = {"clump": 1, "twist": 2, "curl": 4, "frizz": 8}
-FLAG_FILTER, FLAG_COUNTERS, FLAG_STAGE_TIMING, FLAG_PAPER_PAYLOAD, FLAG_SINGLE_PASS, FLAG_FUSED = 1, 2, 4, 8, 16, 32
+FLAG_FILTER, FLAG_COUNTERS, FLAG_STAGE_TIMING, FLAG_PAPER_PAYLOAD, FLAG_SINGLE_PASS, FLAG_FUSED, FLAG_TILED = 1, 2, 4, 8, 16, 32, 64
 EMPTY = 0xFFFFFFFFFFFFFFFF
 
 EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_render_params",
@@ -75,7 +75,8 @@ class hair_stats_t(C.Structure):
                 ("ms_total", C.c_float), ("n_timed_frames", C.c_uint32), ("beta_mean", C.c_float),
                 ("beta_min", C.c_float), ("beta_groom", C.c_float * 16), ("delta_groom", C.c_float * 16),
                 ("gpu_launches", C.c_uint32),
-                ("two_pass", C.c_uint32), ("n_segments_hiz_culled", C.c_uint32)]
+                ("two_pass", C.c_uint32), ("n_segments_hiz_culled", C.c_uint32),
+                ("tiled", C.c_uint32), ("n_tile_records", C.c_uint32), ("tile_overflow", C.c_uint32)]
 
     def as_dict(self):
         return {k: (list(getattr(self, k)) if k in ("beta_groom", "delta_groom") else getattr(self, k)) for k, _ in self._fields_}

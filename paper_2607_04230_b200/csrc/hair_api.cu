@@ -47,6 +47,8 @@ struct hair_ctx {
   uint32_t* d_want = nullptr;  // its device alias (written by k_scan)
   uint32_t* d_hiz = nullptr;  // [ceil(h / 16)][ceil(w / 16)] farthest centre depth per tile between the passes
   size_t hiz_cap = 0;
+  TileBufs tb;  // HAIR_FLAG_TILED: per-tile record lists (allocated on first use)
+  size_t tb_tiles = 0;
   size_t table_cap = 0;
   uint2* d_srec = nullptr;  // per strand id: {vertex offset, C | groom << 8} of this frame (k_generate)
   size_t srec_cap = 0;
@@ -74,7 +76,7 @@ struct hair_ctx {
   int next_slot = 0;
   cudaEvent_t ev[EV_RING][EV_N] = {};
   uint32_t ev_frames = 0;  // timed frames since the last hair_stats
-  bool timed = false, counted = false, last_two_pass = false;
+  bool timed = false, counted = false, last_two_pass = false, last_tiled = false;
   uint32_t last_w = 0, last_h = 0, launches = 0;
   CamDev last_cam;
 };
@@ -243,6 +245,33 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
   return HAIR_OK;
 }
 
+// HAIR_FLAG_TILED: tile arrays for this resolution and a record pool of two records per worst-case vertex
+int ensure_tiles(hair_ctx* c, uint32_t w, uint32_t h) {
+  const size_t n_tiles = (size_t)((w + HAIR_TILE - 1) / HAIR_TILE) * ((h + HAIR_TILE - 1) / HAIR_TILE);
+  if (n_tiles > 65536) return fail(c, HAIR_E_INVALID_ARG, "HAIR_FLAG_TILED: more than 65536 tiles");
+  if (n_tiles > c->tb_tiles) {
+    cudaFree(c->tb.count);
+    c->tb.count = nullptr;
+    c->tb_tiles = 0;
+    CK(cudaMalloc((void**)&c->tb.count, 4 * n_tiles * sizeof(uint32_t)));
+    CK(cudaMemsetAsync(c->tb.count, 0, 4 * n_tiles * sizeof(uint32_t), c->stream));
+    c->tb.base = c->tb.count + n_tiles;
+    c->tb.n = c->tb.base + n_tiles;
+    c->tb.order = c->tb.n + n_tiles;
+    c->tb_tiles = n_tiles;
+  }
+  const size_t want = 2 * c->vertex_need + (1u << 16);
+  if (want > c->tb.cap) {
+    if (want >= (1ull << 32)) return fail(c, HAIR_E_INVALID_ARG, "HAIR_FLAG_TILED: record pool too large");
+    cudaFree(c->tb.entries);
+    c->tb.entries = nullptr;
+    c->tb.cap = 0;
+    CK(cudaMalloc((void**)&c->tb.entries, want * 2 * sizeof(float4)));
+    c->tb.cap = (uint32_t)want;
+  }
+  return HAIR_OK;
+}
+
 // what one pass draws into: R-scene (scene_zn, scene_rgb) and R-seq (grooms of this pass, depth kept in the
 // G-buffer from the pass before, alpha accumulated so far in scene_rgb.w)
 struct PassOpts {
@@ -292,6 +321,12 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   if (fused && !front) return fail(c, HAIR_E_INVALID_ARG, "hair_render_stages: not with HAIR_FLAG_FUSED");
   const bool timed = (c->prm.flags & HAIR_FLAG_STAGE_TIMING) != 0;
   const bool count = (c->prm.flags & HAIR_FLAG_COUNTERS) != 0;
+  // the tile-binned raster (k_raster_tiled.cu) draws production frames of the strand-id word only
+  const bool tiled = (c->prm.flags & HAIR_FLAG_TILED) && !count && !po.ms_k && !pp && !fused && (stage_mask & 1u) && c->scene.n_bi;
+  if (tiled) {
+    rc = ensure_tiles(c, w, h);
+    if (rc) return rc;
+  }
   const uint32_t n_bi = c->scene.n_bi;
   cudaStream_t st = c->stream;
   uint32_t launches = 0;
@@ -308,7 +343,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   mark(EV_BEGIN);
   // The clear of the G-buffer does not depend on LOD / scan / generate: it runs beside them on the context's second
   // stream (forked after everything already enqueued on `st`, joined before the raster). ms_clear then reads ~0.
-  const bool fork_clear = front && n_bi && (stage_mask & 1u);
+  const bool fork_clear = front && n_bi && (stage_mask & 1u) && !tiled;  // (the tile raster initialises its tiles)
   auto clear_on = [&](cudaStream_t cs) -> int {
     if (po.ms_k) CK(cudaMemsetAsync(gbuf, 0xFF, (size_t)w * h * po.ms_k * sizeof(unsigned long long), cs));
     else if (po.reseed) launch_reseed(gbuf, (size_t)w * h, cs);
@@ -338,13 +373,32 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_GEN);
   if (fork_clear) CK(cudaStreamWaitEvent(st, c->ev_join, 0));
-  else if (stage_mask & 1u) {
+  else if ((stage_mask & 1u) && !tiled) {
     rc = clear_on(st);
     if (rc) return rc;
     ++launches;
   }
   mark(EV_CLEAR);
-  if ((stage_mask & 1u) && n_bi) {
+  if (tiled) {
+    if (!front) {  // the table (and its pass split) is the last frame's: restart the queues
+      CK(cudaMemsetAsync(c->d_counters + CNT_WORK_BIN, 0, 5 * sizeof(unsigned long long), st));
+      CK(cudaMemsetAsync(c->d_counters + CNT_SEG_HIZ, 0, sizeof(unsigned long long), st));
+    }
+    const bool far_too = two_pass || (!front && c->last_two_pass);  // near bundles first in every tile's list
+    for (int scatter = 0; scatter < 2; ++scatter) {
+      for (int pass = 0; pass < (far_too ? 2 : 1); ++pass) {
+        launch_bin(scatter != 0, c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, c->d_counters, pass,
+                   c->tb, c->n_sm, st);
+        ++launches;
+      }
+      if (!scatter) {
+        launch_tile_scan(k, c->tb, c->d_counters, st);
+        ++launches;
+      }
+    }
+    launch_raster_tiled(k, gbuf, scene_zn, po.reseed, c->d_counters, c->tb, c->n_sm, &c->ls, st);
+    ++launches;
+  } else if ((stage_mask & 1u) && n_bi) {
     if (!front) {  // the table (and its pass split) is the last frame's: restart both queues
       CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER, 0, sizeof(unsigned long long), st));
       CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER1, 0, sizeof(unsigned long long), st));
@@ -379,6 +433,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   c->timed = timed;
   if (timed) ++c->ev_frames;
   c->counted = count;
+  c->last_tiled = tiled;
   if (front) c->last_two_pass = two_pass;
   c->last_w = w;
   c->last_h = h;
@@ -443,6 +498,8 @@ void hair_destroy(hair_ctx* c) {
   cudaFree(c->d_target2);
   cudaFree(c->d_zrange);
   cudaFree(c->d_hiz);
+  cudaFree(c->tb.count);
+  cudaFree(c->tb.entries);
   cudaFree(c->d_counters);
   cudaFree(c->d_sink);
   if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
@@ -771,7 +828,10 @@ int hair_stats(hair_ctx* c, hair_stats_t* out) {
   out->n_vertices = (uint32_t)k[CNT_VERTICES];
   out->n_segments = (uint32_t)k[CNT_SEGMENTS];
   out->gpu_launches = c->launches;
-  out->two_pass = (uint32_t)k[CNT_HIZ_ON];
+  out->two_pass = c->last_tiled ? 0u : (uint32_t)k[CNT_HIZ_ON];
+  out->tiled = c->last_tiled ? 1u : 0u;
+  out->n_tile_records = c->last_tiled ? (uint32_t)k[CNT_TILE_ENTRIES] : 0u;
+  out->tile_overflow = c->last_tiled ? (uint32_t)k[CNT_TILE_OVERFLOW] : 0u;
   out->n_segments_hiz_culled = (uint32_t)k[CNT_SEG_HIZ];
   out->beta_mean = c->scene.n_strands_total ? (float)((double)k[CNT_STRANDS] / (double)c->scene.n_strands_total) : 1.f;
   // Eq. 8: per-groom beta from the device-side sums of the frame's scan, delta = -log(beta)
