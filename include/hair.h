@@ -74,6 +74,12 @@ extern "C" {
  * hair_render_msaa. Needs 64 bytes of record pool per worst-case vertex (allocated on first use). */
 #define HAIR_FLAG_TILED 64u
 
+/* Half-precision colour output: out_rgb / host_rgb of every render call is [height][width][4] IEEE binary16 (8 bytes per
+ * pixel; the buffer still 16-byte aligned) instead of float, written by the filter itself (round to nearest; absolute error <= 2^-11 of
+ * the value's binade, i.e. < 1e-3 for |v| < 2, < 2e-3 for |v| < 4). Halves the device->host copy of
+ * hair_render_to_host(_async), which PCIe bounds. scene_rgb stays float. */
+#define HAIR_FLAG_RGB16F 128u
+
 typedef struct hair_ctx hair_ctx; /* opaque; owns all device scratch */
 
 /* Creates a context on `cuda_device` that enqueues on `cuda_stream` (a cudaStream_t; NULL = the
@@ -112,8 +118,10 @@ typedef struct {
 /* Appends a groom. Copies everything to the device (synchronously) and sizes the scratch buffers
  * for the worst case (LOD off). Strand ids are assigned in upload order (DESIGN.md §3 "sid"). */
 int hair_mesh_upload(hair_ctx*, const hair_cage*, const hair_roots*, const hair_style*, int* out_groom_id);
-/* Replaces positions / AO of an uploaded groom (animated cage). Same sizes. The copy
- * is enqueued on the context's stream from the caller's (ideally pinned) host memory. */
+/* Replaces positions / AO of an uploaded groom (animated cage). Same sizes. From PINNED host memory the
+ * update is queued and all queued updates are copied by one kernel on the context's stream in front of the next
+ * hair_render* / hair_stats call: the host arrays must stay valid and unchanged until that work has completed (e.g.
+ * until hair_host_wait of the frame). From pageable memory the copy is a cudaMemcpyAsync inside this call. */
 int hair_mesh_update(hair_ctx*, int groom_id, const hair_cage*);
 /* Removes all grooms (buffers are kept). */
 int hair_mesh_clear(hair_ctx*);

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(_HERE, "csrc", "libhair.so")
 
 OP_BITS = {"clump": 1, "twist": 2, "curl": 4, "frizz": 8}
-FLAG_FILTER, FLAG_COUNTERS, FLAG_STAGE_TIMING, FLAG_PAPER_PAYLOAD, FLAG_SINGLE_PASS, FLAG_FUSED, FLAG_TILED = 1, 2, 4, 8, 16, 32, 64
+FLAG_FILTER, FLAG_COUNTERS, FLAG_STAGE_TIMING, FLAG_PAPER_PAYLOAD, FLAG_SINGLE_PASS, FLAG_FUSED, FLAG_TILED, FLAG_RGB16F = 1, 2, 4, 8, 16, 32, 64, 128
 EMPTY = 0xFFFFFFFFFFFFFFFF
 
 EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_render_params",
@@ -243,11 +243,12 @@ class Hair:
         p = make_params(prm, flags)
         self._check(self.L.hair_set_render_params(self.h, C.byref(p)), "hair_set_render_params")
 
-    def alloc_outputs(self, width: int, height: int):
+    def alloc_outputs(self, width: int, height: int, rgb16: bool = False):
+        """Device outputs of one frame; rgb16: the half-precision colour buffer HAIR_FLAG_RGB16F writes."""
         t = self.torch
         dev = f"cuda:{self.device}"
         gb = t.empty((height, width, 2), dtype=t.int64, device=dev)  # uint64 words, viewed as int64
-        rgb = t.empty((height, width, 4), dtype=t.float32, device=dev)
+        rgb = t.empty((height, width, 4), dtype=t.float16 if rgb16 else t.float32, device=dev)
         return gb, rgb
 
     # ---- hair_render(camera, resolution, lod_lambda, out_gbuffer, out_rgb)

@@ -18,6 +18,7 @@ namespace {
 
 struct GroomHost {
   float *pos = nullptr, *ao = nullptr, *xform = nullptr;
+  float *pos_stage = nullptr, *ao_stage = nullptr;  // hair_mesh_update from pinned memory lands here first
   uint32_t *idx = nullptr, *npt = nullptr, *off = nullptr, *tri_of = nullptr;
   size_t pos_bytes = 0, ao_bytes = 0;
 };
@@ -47,6 +48,11 @@ struct hair_ctx {
   uint32_t* d_want = nullptr;  // its device alias (written by k_scan)
   uint32_t* d_hiz = nullptr;  // [ceil(h / 16)][ceil(w / 16)] farthest centre depth per tile between the passes
   size_t hiz_cap = 0;
+  // hair_mesh_update from pinned memory: host -> staging copies (one kernel on aux_stream, beside the frame before)
+  // and staging -> cage copies (one kernel on the stream, in front of the next frame)
+  CopyJobs jobs, jobs_apply;
+  cudaEvent_t ev_staged = nullptr, ev_applied = nullptr;
+  bool applied_once = false;
   TileBufs tb;  // HAIR_FLAG_TILED: per-tile record lists (allocated on first use)
   size_t tb_tiles = 0;
   size_t table_cap = 0;
@@ -181,6 +187,8 @@ void free_groom(GroomHost& g) {
   cudaFree(g.npt);
   cudaFree(g.off);
   cudaFree(g.tri_of);
+  cudaFree(g.pos_stage);
+  cudaFree(g.ao_stage);
   g = GroomHost();
 }
 
@@ -272,6 +280,22 @@ int ensure_tiles(hair_ctx* c, uint32_t w, uint32_t h) {
   return HAIR_OK;
 }
 
+// hair_mesh_update's queued pinned-memory copies: one kernel for all of them, on the context's stream
+void flush_updates(hair_ctx* c) {
+  if (!c->jobs.n) return;
+  // the bus transfer runs on the second stream — beside whatever the stream is still busy with (the frame before, when
+  // the host runs ahead) — once the staging buffers' previous content has been applied; only the device-to-device apply
+  // is in front of the next frame
+  if (c->applied_once) cudaStreamWaitEvent(c->aux_stream, c->ev_applied, 0);
+  launch_copy_jobs(c->jobs, c->aux_stream);
+  cudaEventRecord(c->ev_staged, c->aux_stream);
+  cudaStreamWaitEvent(c->stream, c->ev_staged, 0);
+  launch_copy_jobs(c->jobs_apply, c->stream);
+  cudaEventRecord(c->ev_applied, c->stream);
+  c->applied_once = true;
+  c->jobs.n = c->jobs_apply.n = 0;
+}
+
 // what one pass draws into: R-scene (scene_zn, scene_rgb) and R-seq (grooms of this pass, depth kept in the
 // G-buffer from the pass before, alpha accumulated so far in scene_rgb.w)
 struct PassOpts {
@@ -281,6 +305,7 @@ struct PassOpts {
   bool reseed = false;
   bool bg_alpha = false;
   uint32_t ms_k = 0;  // R-msaa: gbuf is [ms_k][h][w] sample layers, resolve instead of shade + filter
+  bool final_target = true;  // false: an intermediate target of the sequential passes (stays float under HAIR_FLAG_RGB16F)
 };
 
 int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, const float* lam, uint32_t n_lam,
@@ -297,11 +322,13 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
     return fail(c, HAIR_E_INVALID_ARG, "hair_render: n_lambda must be 0, 1 or the number of grooms");
   if (front && n_lam > 0 && lam == nullptr) return fail(c, HAIR_E_INVALID_ARG, "hair_render: lod_lambda is NULL but n_lambda > 0");
   CK(cudaSetDevice(c->device));
+  flush_updates(c);
   int rc = ensure_scratch(c, w, h);
   if (rc) return rc;
   const CamDev k = make_cam(cam, w, h);
   ShadeParams sp = make_shade(c->prm);
   sp.bg_alpha = po.bg_alpha ? 1u : 0u;
+  sp.rgb16 = ((c->prm.flags & HAIR_FLAG_RGB16F) && po.final_target) ? 1u : 0u;
   // R-payload: the paper's word names no groom, so a pass draws exactly one
   const bool pp = (c->prm.flags & HAIR_FLAG_PAPER_PAYLOAD) != 0;
   sp.paper_payload = pp ? 1u : 0u;
@@ -471,7 +498,9 @@ int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream) {
   ok = ok && cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess &&
        cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking) == cudaSuccess &&
        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
-       cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) == cudaSuccess;
+       cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) == cudaSuccess &&
+       cudaEventCreateWithFlags(&c->ev_staged, cudaEventDisableTiming) == cudaSuccess &&
+       cudaEventCreateWithFlags(&c->ev_applied, cudaEventDisableTiming) == cudaSuccess;
   for (int k = 0; ok && k < HAIR_HOST_SLOTS; ++k)
     ok = cudaEventCreateWithFlags(&c->ev_rendered[k], cudaEventDisableTiming) == cudaSuccess &&
          cudaEventCreateWithFlags(&c->ev_copied[k], cudaEventDisableTiming) == cudaSuccess;
@@ -486,6 +515,7 @@ int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream) {
 void hair_destroy(hair_ctx* c) {
   if (!c) return;
   cudaSetDevice(c->device);
+  flush_updates(c);
   cudaStreamSynchronize(c->stream);
   for (auto& g : c->grooms) free_groom(g);
   cudaFree(c->d_scene);
@@ -516,6 +546,8 @@ void hair_destroy(hair_ctx* c) {
   }
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
+  if (c->ev_staged) cudaEventDestroy(c->ev_staged);
+  if (c->ev_applied) cudaEventDestroy(c->ev_applied);
   if (c->h_counters) cudaFreeHost(c->h_counters);
   if (c->h_want) cudaFreeHost(c->h_want);
   for (int f = 0; f < EV_RING; ++f)
@@ -665,13 +697,32 @@ int hair_mesh_update(hair_ctx* c, int groom_id, const hair_cage* cage) {
   const GroomDev& gd = c->scene.g[groom_id];
   if (cage->n_layers != gd.Lv || cage->n_verts != gd.V) return fail(c, HAIR_E_INVALID_ARG, "hair_mesh_update: size mismatch");
   GroomHost& gh = c->grooms[groom_id];
-  CK(cudaMemcpyAsync(gh.pos, cage->pos, gh.pos_bytes, cudaMemcpyHostToDevice, c->stream));
-  if (cage->ao && gh.ao) CK(cudaMemcpyAsync(gh.ao, cage->ao, gh.ao_bytes, cudaMemcpyHostToDevice, c->stream));
-  return HAIR_OK;
+  // Pinned host memory: the update is queued and ALL queued updates go to the device in one copy kernel issued with the
+  // next frame (the SMs pull them over the bus, unified addressing; flush_updates). Ten small cudaMemcpyAsync per frame (five grooms x
+  // positions, AO), each a bus round trip of its own while the previous frame's 66-133 MB image is on its way to the
+  // host, held the next frame's kernels back by 0.6 ms (2.11 against 1.51 ms per pipelined frame). Pageable: memcpy.
+  auto put = [&](float* dst, float** stage, const float* src, size_t bytes) -> int {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, src) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer) {
+      if (!*stage) CK(cudaMalloc((void**)stage, bytes));
+      if (c->jobs.n == COPY_JOBS_MAX) flush_updates(c);
+      c->jobs.j[c->jobs.n++] = CopyJob{(uint32_t*)*stage, (const uint32_t*)at.devicePointer, bytes / 4};
+      c->jobs_apply.j[c->jobs_apply.n++] = CopyJob{(uint32_t*)dst, (const uint32_t*)*stage, bytes / 4};
+      return HAIR_OK;
+    }
+    cudaGetLastError();  // (an unregistered pointer may leave an error behind on old drivers)
+    CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream));
+    return HAIR_OK;
+  };
+  int rc = put(gh.pos, &gh.pos_stage, cage->pos, gh.pos_bytes);
+  if (rc) return rc;
+  if (cage->ao && gh.ao) rc = put(gh.ao, &gh.ao_stage, cage->ao, gh.ao_bytes);
+  return rc;
 }
 
 int hair_mesh_clear(hair_ctx* c) {
   if (!c) return HAIR_E_INVALID_ARG;
+  flush_updates(c);
   cudaStreamSynchronize(c->stream);
   for (auto& g : c->grooms) free_groom(g);
   c->grooms.clear();
@@ -740,6 +791,7 @@ int hair_render_sequential(hair_ctx* c, const hair_camera* cam, uint32_t w, uint
     po.reseed = i_pass > 0;
     po.bg_alpha = i_pass > 0;
     ++i_pass;
+    po.final_target = i_pass == n_pass;
     int rc = render_impl(c, cam, w, h, lam, n_lam, 7u, true, (unsigned long long*)out_gbuffer, target_out, po);
     if (rc) return rc;
     launches += c->launches;
@@ -784,7 +836,8 @@ int hair_render_to_host_async(hair_ctx* c, const hair_camera* cam, uint32_t w, u
   if (rc) return rc;
   CK(cudaEventRecord(c->ev_rendered[k], c->stream));
   CK(cudaStreamWaitEvent(c->copy_stream, c->ev_rendered[k], 0));
-  CK(cudaMemcpyAsync(host_rgb, c->d_own_rgb[k], px * 16, cudaMemcpyDeviceToHost, c->copy_stream));
+  CK(cudaMemcpyAsync(host_rgb, c->d_own_rgb[k], px * ((c->prm.flags & HAIR_FLAG_RGB16F) ? 8 : 16), cudaMemcpyDeviceToHost,
+                     c->copy_stream));
   if (host_gbuffer) CK(cudaMemcpyAsync(host_gbuffer, c->d_own_gbuf[k], px * 16, cudaMemcpyDeviceToHost, c->copy_stream));
   CK(cudaEventRecord(c->ev_copied[k], c->copy_stream));
   c->slot_used[k] = true;
@@ -817,6 +870,7 @@ int hair_stats(hair_ctx* c, hair_stats_t* out) {
   if (!c || !out) return HAIR_E_INVALID_ARG;
   memset(out, 0, sizeof(*out));
   CK(cudaSetDevice(c->device));
+  flush_updates(c);
   CK(cudaMemcpyAsync(c->h_counters, c->d_counters, CNT_N * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   const unsigned long long* k = c->h_counters;

@@ -76,6 +76,7 @@ struct ShadeParams {
   float rho_default;  // 0.5 * center_diameter_px
   uint32_t paper_payload;  // R-payload: words carry the paper's payload; pp_groom = the one groom of the pass
   uint32_t pp_groom;
+  uint32_t rgb16;  // HAIR_FLAG_RGB16F: the colour output of this pass is half RGBA (8 bytes per pixel)
 };
 
 // device counters, one block of 64-bit words (index = enum)
@@ -279,6 +280,18 @@ void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vert
 int launch_filter(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                    ShadeParams sp, const unsigned long long* gbuf, const float4* colour, const float4* scene_rgb,
                    float4* out, unsigned long long* counters, bool count, LaunchState* ls, cudaStream_t st);
+// hair_mesh_update: copies of 32-bit words from device-visible (pinned host) memory, all done by one kernel
+#define COPY_JOBS_MAX 32
+struct CopyJob {
+  uint32_t* dst;
+  const uint32_t* src;
+  size_t n;
+};
+struct CopyJobs {
+  CopyJob j[COPY_JOBS_MAX];
+  int n = 0;
+};
+void launch_copy_jobs(const CopyJobs& jobs, cudaStream_t st);
 void launch_atomic_microbench(int mode, unsigned long long* words, unsigned long long n_words,
                               unsigned long long n_ops, uint32_t hot, int n_sm, cudaStream_t st);
 // n_steps loads per thread of n_sm * 8 CTAs of 256 threads; sink: one device word nothing is ever written to

@@ -300,3 +300,14 @@ void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaA
   k_lod<<<n_tiles, 1024, 0, st>>>(d_scene, n_bi, cam, lam, groom_mask, table, part, zr_prev, zr_cur, two_pass ? 1u : 0u, counters);
   k_scan<<<n_tiles, 256, 0, st>>>(d_scene, table, grp, n_bi, part, counters, zr_prev, n_inst, two_pass ? 1u : 0u, want_two_pass);
 }
+
+// hair_mesh_update from pinned host memory: the SMs pull every queued cage over the bus in one launch (hair_api.cu);
+// blockIdx.y = job
+__global__ void __launch_bounds__(256) k_copy_jobs(CopyJobs jobs) {
+  const CopyJob j = jobs.j[blockIdx.y];
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < j.n; i += (size_t)gridDim.x * blockDim.x) j.dst[i] = j.src[i];
+}
+
+void launch_copy_jobs(const CopyJobs& jobs, cudaStream_t st) {
+  if (jobs.n > 0) k_copy_jobs<<<dim3(32, (unsigned)jobs.n), 256, 0, st>>>(jobs);
+}

@@ -30,6 +30,17 @@ __device__ __forceinline__ F3 calc_tangent(int idx, int count, F3 prev, F3 curr,
   else return normalize(next - prev);
 }
 
+// the frame's colour output: fp32 RGBA, or (HAIR_FLAG_RGB16F) IEEE half RGBA in 8 bytes per pixel, rounded to nearest
+__device__ __forceinline__ void store_rgba(float4* __restrict__ out, size_t p, float4 v, uint32_t rgb16) {
+  if (rgb16) {
+    uint2 h;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(h.x) : "f"(v.y), "f"(v.x));
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(h.y) : "f"(v.w), "f"(v.z));
+    reinterpret_cast<uint2*>(out)[p] = h;
+  } else
+    out[p] = v;
+}
+
 // fast non-decision arithmetic of the shading model (everything here is far inside the 2e-3 RGB tolerance)
 __device__ __forceinline__ float fast_sqrt(float x) {
   float y;
@@ -165,8 +176,8 @@ k_resolve_msaa(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, 
   F3 bg = f3(sp.background[0], sp.background[1], sp.background[2]);
   if (scene_rgb) bg = f3(__ldg(&scene_rgb[p]));
   const float inv_k = 1.0f / (float)ms_k, alpha = (float)n_hit * inv_k;
-  out[p] = make_float4(acc.x * inv_k + (1.f - alpha) * bg.x, acc.y * inv_k + (1.f - alpha) * bg.y,
-                       acc.z * inv_k + (1.f - alpha) * bg.z, alpha);
+  store_rgba(out, p, make_float4(acc.x * inv_k + (1.f - alpha) * bg.x, acc.y * inv_k + (1.f - alpha) * bg.y,
+                                 acc.z * inv_k + (1.f - alpha) * bg.z, alpha), sp.rgb16);
 }
 
 void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
@@ -290,7 +301,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
   if (!__syncthreads_or(hit)) {  // empty tile: background only
 #pragma unroll
     for (int k = 0; k < 2; ++k)
-      if (inside[k]) out[(size_t)(y0 + ly + 8 * k) * W + x0 + lx] = bg[k];
+      if (inside[k]) store_rgba(out, (size_t)(y0 + ly + 8 * k) * W + x0 + lx, bg[k], sp.rgb16);
     return;
   }
   // ---- (1) tile + halo to shared memory
@@ -527,8 +538,9 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
       r = a.x, g = a.y, b = a.z, alpha = a.w;
     }
     const float ia = 1.f - alpha;
-    out[(size_t)(y0 + ly + 8 * k) * W + x0 + lx] =
-        make_float4(alpha * r + ia * bg[k].x, alpha * g + ia * bg[k].y, alpha * b + ia * bg[k].z, alpha + ia * bg[k].w);
+    store_rgba(out, (size_t)(y0 + ly + 8 * k) * W + x0 + lx,
+               make_float4(alpha * r + ia * bg[k].x, alpha * g + ia * bg[k].y, alpha * b + ia * bg[k].z, alpha + ia * bg[k].w),
+               sp.rgb16);
   }
 }
 
@@ -549,7 +561,7 @@ k_filter_passthrough(CamDev cam, ShadeParams sp, const unsigned long long* __res
     const float4 c = __ldg(&colour[p]);
     o = make_float4(c.x, c.y, c.z, 1.f);
   }
-  out[p] = o;
+  store_rgba(out, p, o, sp.rgb16);
 }
 
 // hair_stats: non-empty pixels per layer (counters flag only)

@@ -1020,6 +1020,51 @@ def test_msaa_reference_mode(orc, hair_mod, k):
         h.render_msaa(cam, lam, 3)
 
 
+def test_half_precision_colour_output(orc, hair_mod):
+    """HAIR_FLAG_RGB16F: the filter writes RGBA16F itself (device and host outputs). Against the oracle's filter on the
+    same G-buffer within north_star's 2e-3 (values < 4: half a unit in the last place of binary16 is <= 9.8e-4), and
+    exactly the fp32 frame rounded to nearest; also through hair_render_to_host_async (half the bytes) and as the last
+    pass of hair_render_sequential (intermediate targets stay float)."""
+    import torch
+    b = hair_mod
+    sc = synth.config(4, scale=0.03, res_scale=0.25)
+    G = gpu_frame(b, sc)
+    h, cam, lam = G["h"], sc["camera"], sc["lam"]
+    W, H = cam["width"], cam["height"]
+    h.set_render_params(G["prm"], flags=b.FLAG_RGB16F)
+    gb, rgb16 = h.alloc_outputs(W, H, rgb16=True)
+    h.render(cam, lam, gb, rgb16)
+    assert torch.equal(gb, G["gb_t"])
+    assert torch.equal(rgb16, G["rgb_t"].half())
+    f = orc.Frame(sc["grooms"])
+    f.lod(cam, lam)
+    f.generate()
+    f.set_vertices_f32(G["verts"])
+    f.set_gbuffer(G["gb"])
+    f.shade(cam, G["prm"])
+    out = f.filter(cam, G["prm"])
+    assert float(out.max()) < 4.0
+    err = float(np.abs(out - rgb16.float().cpu().numpy().astype(np.float64)).max())
+    assert err <= TOL_RGB, err
+    # host path: half the bytes, same values
+    host = torch.empty((H, W, 4), dtype=torch.float16).pin_memory()
+    slot = h.render_to_host_async(cam, lam, host)
+    h.host_wait(slot)
+    assert torch.equal(host, rgb16.cpu())
+    # sequential passes: only the last pass's target is half
+    h.set_render_params(G["prm"], flags=0)
+    _, seq32 = h.render_sequential(cam, lam)
+    h.set_render_params(G["prm"], flags=b.FLAG_RGB16F)
+    _, seq16 = h.render_sequential(cam, lam, None, None, gb, rgb16)
+    assert torch.equal(seq16, seq32.half())
+    # filter off and the MSAA reference resolve go through the same store
+    h.set_render_params(dict(G["prm"], filter_on=False), flags=b.FLAG_RGB16F)
+    h.render(cam, lam, gb, rgb16)
+    h.set_render_params(dict(G["prm"], filter_on=False), flags=0)
+    _, off32 = h.render(cam, lam)
+    assert torch.equal(rgb16, off32.half())
+
+
 def test_render_to_host_async_pipeline(hair_mod):
     """Two frames in flight: each host buffer, after host_wait, holds exactly what hair_render gives."""
     import torch
