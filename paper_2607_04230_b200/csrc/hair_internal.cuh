@@ -229,6 +229,16 @@ __device__ __forceinline__ Loc locate_strand(const uint2* __restrict__ srec, uin
   return l;
 }
 
+// The dynamic shared-memory opt-in of a kernel is per device and PROCESS-wide: another context with a smaller table must
+// never lower it under a context that needs more (found by test_two_contexts_with_different_table_sizes_in_either_order).
+// Ask the driver what is set and only ever raise it.
+template <class F>
+inline void raise_dyn_smem(F func, size_t bytes) {
+  cudaFuncAttributes a;
+  if (cudaFuncGetAttributes(&a, func) == cudaSuccess && (size_t)a.maxDynamicSharedSizeBytes >= bytes) return;
+  cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
 // per-context launch state: cudaFuncSetAttribute (dynamic shared memory opt-in) and the occupancy it implies are per
 // DEVICE, and a context is bound to one device, so what has been configured lives in hair_ctx — no function statics
 struct LaunchState {

@@ -98,7 +98,7 @@ void launch_generate(const SceneDev* d_scene, uint32_t n_bi, const uint4* table,
                      unsigned long long* counters, uint32_t c_max, int n_sm, LaunchState* ls, cudaStream_t st) {
   size_t smem = (size_t)GEN_WARPS * ((size_t)c_max * HAIR_ROW + 32 * 5) * sizeof(float);
   if (!ls->gen_per_sm || smem != ls->gen_smem) {  // once per context and table size (the opt-in is per device)
-    cudaFuncSetAttribute(k_generate, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    raise_dyn_smem(k_generate, smem);
     int b = 0;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_generate, GEN_WARPS * 32, smem);
     ls->gen_per_sm = b > 0 ? b : 1;

@@ -483,7 +483,7 @@ static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4*
   const size_t smem = FUSED ? (size_t)RAS_WARPS * c_max * HAIR_ROW * sizeof(float) : 0;  // the warps' spline tables
   constexpr int V = (COUNT ? 1 : 0) | (MS ? 2 : 0) | (PP ? 4 : 0) | (HZ ? 8 : 0) | (FUSED ? 16 : 0);
   if (!ls->raster_per_sm[V] || smem != ls->raster_smem[V]) {  // once per context (= device) and table size
-    if (smem) cudaFuncSetAttribute(k_raster<COUNT, MS, PP, HZ, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (smem) raise_dyn_smem(k_raster<COUNT, MS, PP, HZ, FUSED>, smem);
     int b = 0;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<COUNT, MS, PP, HZ, FUSED>, RAS_WARPS * 32, smem);
     ls->raster_per_sm[V] = b > 0 ? b : 1;

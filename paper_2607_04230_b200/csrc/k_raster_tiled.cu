@@ -416,7 +416,7 @@ void launch_raster_tiled(CamDev cam, unsigned long long* gbuf, const float* scen
   const uint32_t tiles_x = (cam.W + HAIR_TILE - 1) / HAIR_TILE, tiles_y = (cam.H + HAIR_TILE - 1) / HAIR_TILE;
   const size_t smem = (size_t)TILE_PX * sizeof(ulonglong2) + (size_t)TR_WARPS * 32 * REC_STRIDE * sizeof(float);
   if (!ls->tiled_per_sm) {  // once per context (the opt-in is per device)
-    cudaFuncSetAttribute(k_raster_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    raise_dyn_smem(k_raster_tiled, smem);
     int b = 0;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster_tiled, TR_WARPS * 32, smem);
     ls->tiled_per_sm = b > 0 ? b : 1;

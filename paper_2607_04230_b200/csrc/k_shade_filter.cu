@@ -472,12 +472,21 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     const float slope = TN / TM;  // |slope| <= 1; T is a unit vector, so the major part is >= 0.707
     uint32_t Hc = 0, Ha = 0;
     if (sp.strip_nc == 2) {  // w_strip = 0.5: two candidate minor offsets per major step, all unrolled
+      // Eq. 9 is point-symmetric — negating (fM, fN) negates every product and sum exactly, the squares are the same
+      // bits — and so is the candidate interval, so one membership evaluation serves the taps (s, m) and (-s, -m).
+      // (When the interval of step s holds one integer k, the second candidates k + 1 and -k - 1 / -k + 1 all lie
+      // outside it: farther than strip_hmax from the line, never in the strip — the same zero either way.)
+      {  // s = 0: the pixel itself is in the strip; its neighbour at minor offset 1 is 1 > strip_hmax away
+        const bool cG = s_dqG[ci] - lo <= tau2, cA = s_dqA[ci] - lo <= tau2;
+        Hc += cG ? 1u : 0u;
+        Ha += (cA && !cG) ? 1u : 0u;
+      }
 #pragma unroll
-      for (int s = -R; s <= R; ++s) {
+      for (int s = 1; s <= R; ++s) {
         const float fM = (float)s;
         const int m0 = max((int)ceilf(fM * slope - sp.strip_hmax), -R);  // <= R: |s slope| <= R, strip_hmax > 0
         const float pM = xmul(fM, TM);
-        const int idx0 = ci + s * strM + m0 * strN;
+        const int off0 = s * strM + m0 * strN;
         const bool two = m0 < R;  // m0 + 1 is still a window tap (else its read is clamped and its hit masked)
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
@@ -486,10 +495,14 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
           const float eM = xsub(fM, xmul(dpar, TM)), eN = xsub(fN, xmul(dpar, TN));
           bool in = xadd(xmul(eM, eM), xmul(eN, eN)) <= sp.strip_e2_max;
           if (c) in = in && two;
-          const int idc = c ? (two ? idx0 + strN : idx0) : idx0;
-          const bool cG = s_dqG[idc] - lo <= tau2, cA = s_dqA[idc] - lo <= tau2;
-          Hc += (in && cG) ? 1u : 0u;
-          Ha += (in && cA && !cG) ? 1u : 0u;
+          const int off = c ? (two ? off0 + strN : off0) : off0;
+#pragma unroll
+          for (int sg = 0; sg < 2; ++sg) {
+            const int idc = sg ? ci - off : ci + off;
+            const bool cG = s_dqG[idc] - lo <= tau2, cA = s_dqA[idc] - lo <= tau2;
+            Hc += (in && cG) ? 1u : 0u;
+            Ha += (in && cA && !cG) ? 1u : 0u;
+          }
         }
       }
     } else {
@@ -601,7 +614,7 @@ static void launch_filter_r(const SceneDev* d_scene, const uint2* srec, const fl
   constexpr int NS = (FT_W + 2 * R) * (FT_H + 2 * R);
   constexpr size_t smem = (size_t)NS * (sizeof(float4) + 3 * sizeof(uint32_t)) + 2 * FT_W * FT_H * sizeof(float4);
   if (!ls->filter_set[R]) {  // once per context (the opt-in is per device)
-    cudaFuncSetAttribute(k_filter<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    raise_dyn_smem(k_filter<R>, smem);
     ls->filter_set[R] = true;
   }
   dim3 grid((cam.W + FT_W - 1) / FT_W, (cam.H + FT_H - 1) / FT_H);

@@ -954,6 +954,41 @@ def test_tiled_raster_bench_frame_scene_and_sequential(orc, hair_mod):
         assert torch.equal(s[0], s2[0]) and torch.equal(s[1], s2[1]), i
 
 
+def test_two_contexts_with_different_table_sizes_in_either_order(hair_mod):
+    """Launch state (opt-in dynamic shared memory, occupancy) lives in the context, not in function statics: two
+    contexts whose per-bundle tables differ in size (C_max 17 against 49: k_generate's and the fused raster's dynamic
+    shared memory) render materialised, fused and filtered frames interleaved in both orders and reproduce their own
+    single-context frames bit for bit."""
+    import torch
+    b = hair_mod
+    scA = synth.config(1)                               # Lv 3, spi 8: C_max 17
+    scB = synth.config(3, scale=0.03, res_scale=0.25)   # Lv 13, spi 4: C_max 49
+    prmA, prmB = dict(scA["params"]), dict(scB["params"])
+
+    def frames(h, sc, prm):
+        out = []
+        for fl in (0, b.FLAG_PAPER_PAYLOAD, b.FLAG_PAPER_PAYLOAD | b.FLAG_FUSED, b.FLAG_TILED):
+            h.set_render_params(prm, flags=fl)
+            g, r = h.render(sc["camera"], sc["lam"])
+            out.append((g.clone(), r.clone()))
+        return out
+
+    def fresh(sc):
+        h = b.Hair(0)
+        for g in sc["grooms"]:
+            h.mesh_upload(g)
+        return h
+    refA, refB = frames(fresh(scA), scA, prmA), frames(fresh(scB), scB, prmB)
+    for order in ("AB", "BA"):
+        hA, hB = fresh(scA), fresh(scB)
+        for rep in range(2):
+            got = {}
+            for which in order:
+                got[which] = frames(hA, scA, prmA) if which == "A" else frames(hB, scB, prmB)
+            for (g0, r0), (g1, r1) in zip(refA + refB, got["A"] + got["B"]):
+                assert torch.equal(g0, g1) and torch.equal(r0, r1), (order, rep)
+
+
 def test_sequential_as_first_render_of_a_context(hair_mod):
     """Regression: the first frame of a context may be a sequential one (its second target must survive the
     allocation of the per-resolution scratch)."""
