@@ -217,41 +217,172 @@ __device__ __forceinline__ float2 screen_tangent_payload(const CamDev& cam, int 
 }
 
 // ---------------------------------------------------------------------------------------- H7
-// Tiled filter. One CTA owns a 32x16 pixel tile: (1) the tile + an r-pixel halo of the G-buffer
-// (as two 24-bit depths, "none" = DQ_NONE) and of the shaded colour go to shared memory once,
-// (2) every hit pixel emits one or two work items (reference tangent, reference depth, colour
-// mode; two for a fly-away pixel), compacted through a shared counter so sparse tiles still fill
-// their warps, (3) the items are spread over the 256 threads; each item runs two branch-free loops
-// over shared memory, (4) the owning thread combines its items and writes out_rgb.
-//  loop A, Eq. 10: all (2r+1)^2 taps, one LDS.32 (centre depth) + one LDS.128
-//    (colour) per tap; the class test (R20, integer depth compare) becomes a select on the weight,
-//    so lanes never diverge. The exponent is the quadratic form a dx^2 + b dx dy + c dy^2 of the
-//    window offset (2 FMA per tap), the colour distance is |CP|^2 + |CQ|^2 - 2 CP.CQ with -kC|CQ|^2
-//    kept per tile pixel, all pre-multiplied by log2(e) so that one ex2.approx gives the weight.
-//  loop B, strip hit counts: only lattice points within w_strip of the tangent line
-//    can be in the strip, so instead of testing 121 taps the loop walks the 2r+1 steps of the
-//    tangent's major axis and tests the `strip_nc` (2 for w_strip = 0.5) integer minor offsets that
-//    can lie within (w_strip + 0.01) sqrt(2) of the line — a superset; membership itself is Eq. 9 in
-//    the oracle's fixed-order fp32 (sqrt_rn(e2) <= w_strip tested as e2 <= strip_e2_max, host-side
-//    the largest float whose correctly rounded root is <= w_strip; sqrt_rn is monotone).
+// Tiled filter. One CTA owns a 32x16 pixel tile:
+// (1) the tile + an r-pixel halo goes to shared memory once, in PAIR layout, for the horizontally adjacent pixels
+//     a = 2p, b = 2p + 1 of a tile row: s_pa[p] = {x_a, x_b, y_a, y_b}, s_pb[p] = {z_a, z_b, dq_a, dq_b} (colours of
+//     centre hits pre-scaled by sqrt(kC), zero elsewhere; dq = 24-bit depth of the centre word, DQ_NONE without a
+//     centre hit), s_pk[p] = {k_a, k_b} (k = |scaled colour|^2, read by the accumulations with a colour term only),
+//     and s_dq[pixel] = {dq_centre, dq_cons} for the strip loop;
+// (2) every hit pixel emits ONE work item; centre-hit pixels are compacted in PIXEL ORDER (promoted conservative-only
+//     pixels, follow in a second run), so a warp of a dense tile holds one tile row;
+// (3) item / thread. Loop A, Eq. 10, walks the (2r+1)^2 window one PAIR of taps at a time: three
+//     loads bring both taps' colour, k and depth, and the arithmetic of the two taps runs in the packed fp32
+//     instructions of sm_100 (FFMA2 / FADD2: fma.rn.f32x2 — two cycles of the FMA pipe like two FFMAs, but ONE issue
+//     slot, which is what this loop was short of). Adjacent pixels of a row share their pairs, so the 32 lanes of a
+//     row-ordered warp read 16 distinct 16-byte words per LDS.128: two shared-memory cycles instead of four
+//     (measured on the B200: the LDS pipe serves 128 distinct bytes per cycle and multicasts for free; profiles/).
+//     A pixel whose conservative sample is a fly-away strand in front (R21) runs its second accumulation — around
+//     the conservative sample, w_color = 1 — ON THE SAME LOADS; a warp without such a lane runs the loop without
+//     that part. The window of a pixel at odd x starts one tap early and the one at even x ends one tap late (pairs
+//     are aligned): that tap is masked. Exponent, base 2 and positive so that ex2.approx(-e) is the weight: the
+//     quadratic form of Eq. 10 in Horner form over dx, (a dx + B) dx + C with per-row B, C; colour distance
+//     |C_P|^2 - 2 C_P.C_Q + |C_Q|^2 with the first term in C and the last read from shared memory. The class test
+//     (R20) is the integer compare (d - lo) <= 2 tau (mod 2^32) on the ALU pipe.
+//     Loop B, strip hit counts: only lattice points within w_strip of the tangent line can be in the
+//     strip, so the loop walks the 2r+1 steps of the tangent's major axis and tests the `strip_nc` (2 for
+//     w_strip = 0.5) integer minor offsets that can lie within (w_strip + 0.01) sqrt(2) of the line — a superset;
+//     membership itself is Eq. 9 in the oracle's fixed-order fp32 (sqrt_rn(e2) <= w_strip tested as
+//     e2 <= strip_e2_max, host-side the largest float whose correctly rounded root is <= w_strip).
+// (4) the item's lane composites over the background (R29) and writes out_rgb; pixels without a hit are written by
+//     their owner thread.
 #define FT_W 32
 #define FT_H 16
 #ifndef FILT_MIN_BLOCKS
 #define FILT_MIN_BLOCKS 4  // CTAs per SM the register budget is held to
 #endif
 #define DQ_NONE 0x40000000u
+#define DQ_OFF 0x80000000u  // as the low end of a depth window: no depth lies within 2 tau above it
 
 __device__ __forceinline__ float fast_ex2(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+// packed fp32 (sm_100): both halves in one instruction
+__device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 
-// Eq. 9 in the oracle's operation order; true iff sqrt_rn(e2) <= w_strip
-__device__ __forceinline__ bool in_strip_exact(float fdx, float fdy, float Tx, float Ty, float e2_max) {
-  const float dpar = xadd(xmul(fdx, Tx), xmul(fdy, Ty));
-  const float ex = xsub(fdx, xmul(dpar, Tx)), ey = xsub(fdy, xmul(dpar, Ty));
-  return xadd(xmul(ex, ex), xmul(ey, ey)) <= e2_max;
+// weight of one tap: 2^-e if the tap is of the sample's class (R19 / R20: dd = d - lo <= 2 tau, mod 2^32), else 0; a
+// select, never a branch (the lanes of a warp do not diverge)
+__device__ __forceinline__ float gated_weight(float e, uint32_t dd, uint32_t tau2) {
+  float w;
+  asm("{\n\t.reg .pred p;\n\t.reg .f32 n;\n\tsetp.le.u32 p, %2, %3;\n\tneg.f32 n, %1;\n\t"
+      "mov.f32 %0, 0f00000000;\n\t@p ex2.approx.ftz.f32 %0, n;\n\t}"
+      : "=f"(w)
+      : "f"(e), "r"(dd), "r"(tau2));
+  return w;
+}
+
+// Loop A over the window of one item (one accumulation of Eq. 10, R19-R21). COL: colour term on (centre
+// sample) or off (conservative sample: w_color = 1). Positive base-2 exponent
+// a dx^2 + b dx dy + c dy^2 + c0 in Horner form over dx. ra / rd: the window's first pair in s_pa / s_pd; u = dx of the
+// first tap of a window row (-r, or -r-1 for a pixel at odd x, whose first tap then lies outside the window, as does
+// the last tap of a window at even x); (mx, my, mz) = -2 * scaled centre colour; class test (d - lo) <= tau2
+template <int R, bool COL>
+__device__ __forceinline__ float4 filter_loop_a(const float4* __restrict__ ra, const float2* __restrict__ rd, int HP,
+                                                int NP, bool odd, float u, float a, float b, float c, float c0, float mx,
+                                                float my, float mz, uint32_t lo, uint32_t tau2) {
+  float2 S0 = make_float2(0.f, 0.f), S1 = S0, S2 = S0, Ws = S0;
+  float fdy = (float)(-R);
+#pragma unroll 1
+  for (int dyi = 0; dyi <= 2 * R; ++dyi, ra += HP, rd += HP, fdy += 1.0f) {
+    const float B = b * fdy, C = fmaf(c * fdy, fdy, c0);
+    float2 dx = make_float2(u, u + 1.0f);
+#pragma unroll
+    for (int p = 0; p <= R; ++p) {
+      const float4 A4 = ra[p], B4 = ra[NP + p];
+      const float2 X = make_float2(A4.x, A4.y), Y = make_float2(A4.z, A4.w), Z = make_float2(B4.x, B4.y);
+      const uint2 D = make_uint2(__float_as_uint(B4.z), __float_as_uint(B4.w));
+      if (p) dx = add2(dx, bc2(2.0f));
+      uint32_t Dx = D.x, Dy = D.y;
+      if (p == 0) Dx = odd ? DQ_NONE : Dx;  // tap -r-1 of a window at odd x
+      if (p == R) Dy = odd ? Dy : DQ_NONE;  // tap r+1 of a window at even x
+      float2 e = fma2(fma2(bc2(a), dx, bc2(B)), dx, bc2(C));  // Eq. 10 spatial part (+ |C_P|^2 in c0)
+      if (COL) {                                              // Eq. 10 colour part
+        e = fma2(bc2(mx), X, e);
+        e = fma2(bc2(my), Y, e);
+        e = fma2(bc2(mz), Z, e);
+        e = add2(e, rd[p]);
+      }
+      const float2 w = make_float2(gated_weight(e.x, Dx - lo, tau2), gated_weight(e.y, Dy - lo, tau2));  // R19 / R20
+      S0 = fma2(w, X, S0);
+      S1 = fma2(w, Y, S1);
+      S2 = fma2(w, Z, S2);
+      Ws = add2(Ws, w);
+    }
+  }
+  return make_float4(S0.x + S0.y, S1.x + S1.y, S2.x + S2.y, Ws.x + Ws.y);
+}
+
+// Loop B: strip hit counts by Q's class (R18) around the sample with depth window [lo, lo + tau2] and screen tangent
+// (Tx, Ty), in (major, minor) coordinates of the tangent: Eq. 9 is symmetric in x / y and IEEE add / mul commute,
+// so the bits are those of the oracle's x / y order. Returns alpha = Hc / (Hc + Ha).
+template <int R>
+__device__ __forceinline__ float strip_alpha(const uint2* __restrict__ s_dq, int ci, int SW, float Tx, float Ty,
+                                             uint32_t lo, uint32_t tau2, const ShadeParams& sp) {
+  const bool xmaj = fabsf(Tx) >= fabsf(Ty);
+  const float TM = xmaj ? Tx : Ty, TN = xmaj ? Ty : Tx;
+  const int strM = xmaj ? 1 : SW, strN = xmaj ? SW : 1;
+  const float slope = TN / TM;  // |slope| <= 1; T is a unit vector, so the major part is >= 0.707
+  uint32_t Hc = 0, Ha = 0;
+  if (sp.strip_nc == 2) {  // w_strip = 0.5: two candidate minor offsets per major step, all unrolled
+    // Eq. 9 is point-symmetric — negating (fM, fN) negates every product and sum exactly, the squares are the same
+    // bits — and so is the candidate interval, so one membership evaluation serves the taps (s, m) and (-s, -m).
+    // (When the interval of step s holds one integer k, the second candidates k + 1 and -k - 1 / -k + 1 all lie
+    // outside it: farther than strip_hmax from the line, never in the strip — the same zero either way.)
+    {  // s = 0: the pixel itself is in the strip; its neighbour at minor offset 1 is 1 > strip_hmax away
+      const uint2 q = s_dq[ci];
+      const bool cG = q.x - lo <= tau2, cA = q.y - lo <= tau2;
+      Hc += cG ? 1u : 0u;
+      Ha += (cA && !cG) ? 1u : 0u;
+    }
+#pragma unroll
+    for (int s = 1; s <= R; ++s) {
+      const float fM = (float)s;
+      const int m0 = max((int)ceilf(fM * slope - sp.strip_hmax), -R);  // <= R: |s slope| <= R, strip_hmax > 0
+      const float pM = xmul(fM, TM);
+      const int off0 = s * strM + m0 * strN;
+      const bool two = m0 < R;  // m0 + 1 is still a window tap (else its read is clamped and its hit masked)
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        const float fN = (float)(m0 + c);
+        const float dpar = xadd(pM, xmul(fN, TN));
+        const float eM = xsub(fM, xmul(dpar, TM)), eN = xsub(fN, xmul(dpar, TN));
+        bool in = xadd(xmul(eM, eM), xmul(eN, eN)) <= sp.strip_e2_max;
+        if (c) in = in && two;
+        const int off = c ? (two ? off0 + strN : off0) : off0;
+#pragma unroll
+        for (int sg = 0; sg < 2; ++sg) {
+          const uint2 q = s_dq[sg ? ci - off : ci + off];
+          const bool cG = q.x - lo <= tau2, cA = q.y - lo <= tau2;
+          Hc += (in && cG) ? 1u : 0u;
+          Ha += (in && cA && !cG) ? 1u : 0u;
+        }
+      }
+    }
+  } else {
+#pragma unroll 1
+    for (int s = -R; s <= R; ++s) {
+      const float fM = (float)s;
+      const int m0 = max((int)ceilf(fM * slope - sp.strip_hmax), -R);
+      const float pM = xmul(fM, TM);
+      for (int c = 0; c < sp.strip_nc; ++c) {
+        const int mm = m0 + c;
+        if (mm <= R) {
+          const float fN = (float)mm;
+          const float dpar = xadd(pM, xmul(fN, TN));
+          const float eM = xsub(fM, xmul(dpar, TM)), eN = xsub(fN, xmul(dpar, TN));
+          const bool in = xadd(xmul(eM, eM), xmul(eN, eN)) <= sp.strip_e2_max;
+          const uint2 q = s_dq[ci + s * strM + mm * strN];
+          const bool cG = q.x - lo <= tau2, cA = q.y - lo <= tau2;
+          Hc += (in && cG) ? 1u : 0u;
+          Ha += (in && cA && !cG) ? 1u : 0u;
+        }
+      }
+    }
+  }
+  return (Hc + Ha) > 0 ? (float)Hc / (float)(Hc + Ha) : 0.f;
 }
 
 template <int R>
@@ -259,16 +390,16 @@ __global__ void __launch_bounds__(256, FILT_MIN_BLOCKS)
 k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
          CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, const float4* __restrict__ colour,
          const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
-  constexpr int SW = FT_W + 2 * R, SH = FT_H + 2 * R, NS = SW * SH;
+  constexpr int SW = FT_W + 2 * R, HP = SW / 2, SH = FT_H + 2 * R, NP = HP * SH, NS = SW * SH;
   extern __shared__ float4 fsm[];
-  float4* s_col = fsm;                                  // [NS] rgb (zeros where no centre hit), dq of the centre word
-  float4* s_item = fsm + NS;                            // [2 * FT_W * FT_H] item, later its result
-  uint32_t* s_dqG = reinterpret_cast<uint32_t*>(s_item + 2 * FT_W * FT_H);  // [NS] dq of the centre word
-  uint32_t* s_dqA = s_dqG + NS;                                             // [NS] dq of the conservative word
-  float* s_k2 = reinterpret_cast<float*>(s_dqA + NS);                       // [NS] -kC |rgb|^2 (Eq. 10 colour term)
-  // (the centre depth sits both in s_col.w, where the tap loop gets it with the colour in one LDS.128 — the loop of
-  // the conservative-sample items then reads nothing else — and in s_dqG, whose 4-byte stride suits the strip loop)
-  __shared__ uint32_t s_cc[2][FT_H + 1][8];  // items per (type, row, class); then their exclusive prefix over rows
+  float4* s_pa = fsm;                                              // [NP] {x_a, x_b, y_a, y_b} of the pixel pair
+  float4* s_pb = fsm + NP;                                         // [NP] {z_a, z_b, k_a, k_b}
+  float4* s_item = fsm + 2 * NP;                                   // [2 * FT_W * FT_H] item, later its result
+  uint2* s_dq = reinterpret_cast<uint2*>(s_item + 2 * FT_W * FT_H);  // [NS] {dq centre, dq conservative}
+  float2* s_pk = reinterpret_cast<float2*>(s_dq + NS);             // [NP] {k_a, k_b}
+  __shared__ uint32_t s_cc[FT_H + 1][8];  // conservative-sample items per (row, class); then their prefix over rows
+  __shared__ uint32_t s_cn[FT_H + 1];     // centre items per row; then their prefix
+  __shared__ uint32_t s_next;             // next item warp to take
   const int W = (int)cam.W, H = (int)cam.H;
   const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
   const int x0 = blockIdx.x * FT_W, y0 = blockIdx.y * FT_H;
@@ -288,56 +419,57 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     }
     hit |= !w_none(A[k]);  // centre layer is a subset of the conservative one (R10)
   }
-  // what the hair is composited over (R29): the constant background, or the scene's colour (R-scene)
-  float4 bg[2];
+  const bool any_hit = __syncthreads_or(hit);
+  // pixels without a hit: what the hair is composited over (R29), the constant background or the scene's colour
 #pragma unroll
-  for (int k = 0; k < 2; ++k) {
-    bg[k] = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
-    if (scene_rgb && inside[k]) {
-      const float4 b = __ldg(&scene_rgb[(size_t)(y0 + ly + 8 * k) * W + x0 + lx]);
-      bg[k] = make_float4(b.x, b.y, b.z, sp.bg_alpha ? b.w : 0.f);
+  for (int k = 0; k < 2; ++k)
+    if (inside[k] && w_none(A[k])) {
+      const size_t p = (size_t)(y0 + ly + 8 * k) * W + x0 + lx;
+      float4 bg = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
+      if (scene_rgb) {
+        const float4 b = __ldg(&scene_rgb[p]);
+        bg = make_float4(b.x, b.y, b.z, sp.bg_alpha ? b.w : 0.f);
+      }
+      store_rgba(out, p, bg, sp.rgb16);
     }
-  }
-  if (!__syncthreads_or(hit)) {  // empty tile: background only
+  if (!any_hit) return;  // empty tile: background only
+  // ---- (1) tile + halo to shared memory, one pixel pair per thread and round
+  const float kappa = fmaxf(sqrtf(sp.kC), 1e-15f);
+  for (int i = tid; i < NP; i += 256) {
+    const int sy = i / HP, pp = i - sy * HP;
+    const int gy = y0 + sy - R;
+    float c[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+    uint32_t dG[2] = {DQ_NONE, DQ_NONE}, dA[2] = {DQ_NONE, DQ_NONE};
 #pragma unroll
-    for (int k = 0; k < 2; ++k)
-      if (inside[k]) store_rgba(out, (size_t)(y0 + ly + 8 * k) * W + x0 + lx, bg[k], sp.rgb16);
-    return;
-  }
-  // ---- (1) tile + halo to shared memory
-  for (int i = tid; i < NS; i += 256) {
-    const int sy = i / SW, sx = i - sy * SW;
-    const int gx = x0 + sx - R, gy = y0 + sy - R;
-    uint32_t dG = DQ_NONE, dA = DQ_NONE;
-    float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
-    float k2 = 0.f;
-    if (gx >= 0 && gx < W && gy >= 0 && gy < H) {  // samples outside the image do not exist
-      const size_t q = (size_t)gy * W + gx;
-      const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + q);
-      if (!w_none(raw.z, raw.w)) dA = raw.w >> 8;
-      if (!w_none(raw.x, raw.y)) {
-        dG = raw.y >> 8;
-        const float4 c = __ldg(&colour[q]);
-        c4 = make_float4(c.x, c.y, c.z, 0.f);
-        k2 = -sp.kC * (c.x * c.x + c.y * c.y + c.z * c.z);
+    for (int e = 0; e < 2; ++e) {
+      const int gx = x0 + 2 * pp + e - R;
+      if (gx >= 0 && gx < W && gy >= 0 && gy < H) {  // samples outside the image do not exist
+        const size_t q = (size_t)gy * W + gx;
+        const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + q);
+        if (!w_none(raw.z, raw.w)) dA[e] = raw.w >> 8;
+        if (!w_none(raw.x, raw.y)) {
+          dG[e] = raw.y >> 8;
+          const float4 cq = __ldg(&colour[q]);
+          c[e][0] = kappa * cq.x, c[e][1] = kappa * cq.y, c[e][2] = kappa * cq.z;
+          c[e][3] = c[e][0] * c[e][0] + c[e][1] * c[e][1] + c[e][2] * c[e][2];
+        }
       }
     }
-    c4.w = __uint_as_float(dG);
-    s_col[i] = c4;
-    s_k2[i] = k2;
-    s_dqG[i] = dG;
-    s_dqA[i] = dA;
+    s_pa[i] = make_float4(c[0][0], c[1][0], c[0][1], c[1][1]);
+    s_pb[i] = make_float4(c[0][2], c[1][2], __uint_as_float(dG[0]), __uint_as_float(dG[1]));
+    s_pk[i] = make_float2(c[0][3], c[1][3]);
+    reinterpret_cast<uint4*>(s_dq)[i] = make_uint4(dG[0], dA[0], dG[1], dA[1]);
   }
-  // ---- (2) work items, compacted by type (all centre items, then all conservative-sample items: all but one warp
-  // hold items of one type, which take the tap loop with / without the colour term) and, inside a type, DEALT BY BANK
-  // CLASS: the 16-byte bank group a tap read of pixel (x, y) falls on is (x + (SW mod 8) y + const) mod 8, the same
-  // constant for every lane, so slot = rank * 8 + class puts eight different bank groups in every quarter warp
-  // whatever pixels the items sit on (sparse fly-away / promoted items were 2-way conflicted when merely packed in
-  // pixel order). Classes fill unevenly; the few slots left empty are skipped.
+  // ---- (2) work items. Centre items (one per centre-hit pixel) are compacted in PIXEL ORDER: a warp of a dense tile
+  // holds one tile row, whose lanes share their pairs. Conservative-sample items (fly-away strand in front of the
+  // centre hit, R21, or promoted pixel) are sparse, so they are DEALT BY BANK CLASS instead: the 16-byte
+  // bank group a tap read of pixel (x, y) falls on is ((x >> 1) + (HP mod 8) y + const) mod 8, the same constant for
+  // every lane, so slot = rank * 8 + class puts at most four different pairs on every bank group of a warp whatever
+  // pixels its items sit on. Classes fill unevenly; the few slots left empty are skipped.
   int slot_c[2] = {-1, -1}, slot_a[2] = {-1, -1};
   bool fly[2] = {false, false};
   float2 Tc[2], Ta[2];
-  uint32_t bal[4];
+  uint32_t balC[2], balA[2];
   const uint32_t lt_mask = (1u << lx) - 1u;
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
@@ -348,193 +480,110 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
                                : screen_tangent(sc, srec, vertices, cam, G[k]);
       fly[k] = isCons && w_dq(G[k]) >= w_dq(A[k]) && w_dq(G[k]) - w_dq(A[k]) >= sp.taufly_q;  // PAPER.md:175, R21
     }
-    const bool isA = fly[k] || (isCons && !isCenter);  // fly-away strand, or promoted pixel (PAPER.md:175): w_color = 1
+    const bool isA = fly[k] || (isCons && !isCenter);  // fly-away strand, or promoted pixel: w_color = 1
     if (isA)
       Ta[k] = sp.paper_payload ? screen_tangent_payload(cam, x0 + lx, y0 + ly + 8 * k, A[k])
                                : screen_tangent(sc, srec, vertices, cam, A[k]);
-    bal[2 * k] = __ballot_sync(0xffffffffu, isCenter);
-    bal[2 * k + 1] = __ballot_sync(0xffffffffu, isA);
+    balC[k] = __ballot_sync(0xffffffffu, isCenter);
+    balA[k] = __ballot_sync(0xffffffffu, isA);
+    if (lx == 0) s_cn[ly + 8 * k] = __popc(balC[k]);
   }
-  constexpr int KS = SW & 7;  // bank-group step of one tile row
-  {
-    // counts per (type, class, row): lane l of warp ly reports k = l >> 4, type = (l >> 3) & 1, class = l & 7
-    const int rk = lx >> 4, rt = (lx >> 3) & 1, rc = lx & 7, rrow = ly + 8 * rk;
-    const uint32_t rb = rk ? (rt ? bal[3] : bal[2]) : (rt ? bal[1] : bal[0]);
-    s_cc[rt][rrow][rc] = __popc(rb & (0x01010101u << ((rc - KS * rrow) & 7)));
+  constexpr int KS = HP & 7;  // bank-group step of one tile row
+  if (lx < 16) {  // conservative-sample items per (row, class): lane l of warp ly reports k = l >> 3, class = l & 7
+    const int rk = lx >> 3, rc = lx & 7, rrow = ly + 8 * rk;
+    s_cc[rrow][rc] = __popc(balA[rk] & (0x00030003u << (2 * ((rc - KS * rrow) & 7))));
   }
   __syncthreads();
-  if (tid < 16) {  // exclusive prefix over the rows, total in row FT_H
+  if (tid < 8) {  // exclusive prefix over the rows, total in row FT_H
     uint32_t t = 0;
 #pragma unroll
     for (int r = 0; r < FT_H; ++r) {
-      const uint32_t n = s_cc[tid >> 3][r][tid & 7];
-      s_cc[tid >> 3][r][tid & 7] = t;
+      const uint32_t n = s_cc[r][tid];
+      s_cc[r][tid] = t;
       t += n;
     }
-    s_cc[tid >> 3][FT_H][tid & 7] = t;
+    s_cc[FT_H][tid] = t;
+  } else if (tid == 32) {
+    s_next = 0;
+    uint32_t t = 0;
+#pragma unroll
+    for (int r = 0; r < FT_H; ++r) {
+      const uint32_t n = s_cn[r];
+      s_cn[r] = t;
+      t += n;
+    }
+    s_cn[FT_H] = t;
   }
   __syncthreads();
-  uint32_t max_c = 0, max_a = 0;
+  uint32_t max_a = 0;
 #pragma unroll
-  for (int c = 0; c < 8; ++c) max_c = max(max_c, s_cc[0][FT_H][c]), max_a = max(max_a, s_cc[1][FT_H][c]);
-  const int n_centre = (int)((8u * max_c + 31u) & ~31u);  // centre slots, rounded up to whole warps
+  for (int c = 0; c < 8; ++c) max_a = max(max_a, s_cc[FT_H][c]);
+  const int n_centre = (int)((s_cn[FT_H] + 31u) & ~31u);  // centre slots, rounded up to whole warps
   const int n_item = n_centre + (int)(8u * max_a);
   for (int i = tid; i < n_item; i += 256) s_item[i].w = __uint_as_float(0xFFFFFFFFu);  // empty slot
   __syncthreads();
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
-    const int row = ly + 8 * k, cls = (lx + KS * row) & 7;
-    const uint32_t same = 0x01010101u << (lx & 7);  // the four lanes of this row in my class
+    const int row = ly + 8 * k;
     const uint32_t pix = (uint32_t)(row * FT_W + lx);
-    const uint32_t before_c = s_cc[0][row][cls], before_a = s_cc[1][row][cls];
-    if ((bal[2 * k] >> lx) & 1u) {
-      slot_c[k] = (int)((before_c + __popc(bal[2 * k] & same & lt_mask)) * 8u) + cls;
+    if ((balC[k] >> lx) & 1u) {
+      slot_c[k] = (int)(s_cn[row] + __popc(balC[k] & lt_mask));
       s_item[slot_c[k]] = make_float4(Tc[k].x, Tc[k].y, __uint_as_float(w_dq(G[k]) | 0x1000000u), __uint_as_float(pix));
     }
-    if ((bal[2 * k + 1] >> lx) & 1u) {
-      slot_a[k] = n_centre + (int)((before_a + __popc(bal[2 * k + 1] & same & lt_mask)) * 8u) + cls;
+    if ((balA[k] >> lx) & 1u) {
+      const int cls = ((lx >> 1) + KS * row) & 7;
+      const uint32_t same = 0x00030003u << (2 * ((lx >> 1) & 7));  // the four lanes of this row in my class
+      slot_a[k] = n_centre + (int)((s_cc[row][cls] + __popc(balA[k] & same & lt_mask)) * 8u) + cls;
       s_item[slot_a[k]] = make_float4(Ta[k].x, Ta[k].y, __uint_as_float(w_dq(A[k])), __uint_as_float(pix));
     }
   }
   __syncthreads();
   // ---- (3) per item (Code 2 PAPER.md:483-515 with DESIGN.md R18-R20)
-  const uint32_t tau = sp.tauz_q, tau2 = 2u * sp.tauz_q;
-  for (int it = tid; it < n_item; it += 256) {
+  const uint32_t tauq = sp.tauz_q, tau2 = 2u * sp.tauz_q;
+  const float inv_kappa = 1.0f / kappa;
+  // the warps of the CTA take the item warps from a shared counter (centre and conservative-sample warps cost
+  // differently, so a fixed deal leaves warps waiting at the barrier)
+  for (;;) {
+    int it0 = 0;
+    if (lx == 0) it0 = (int)atomicAdd(&s_next, 32u);
+    it0 = __shfl_sync(0xffffffffu, it0, 0);
+    if (it0 >= n_item) break;
+    const int it = it0 + lx;
+    if (it >= n_item) continue;
     const float4 I = s_item[it];
     const float Tx = I.x, Ty = I.y;
     const uint32_t rm = __float_as_uint(I.z), pix = __float_as_uint(I.w);
-    if (pix == 0xFFFFFFFFu) continue;  // empty slot of an under-filled bank class
+    if (pix == 0xFFFFFFFFu) continue;  // empty slot
+    const int ix = (int)(pix & 31u), iy = (int)(pix >> 5);
     // R20: class by integer depth compare, |d - ref| <= tau as (unsigned)(d - (ref - tau)) <= 2 tau (mod 2^32);
     // DQ_NONE is farther than tau (<= 2^24) from every depth
-    const uint32_t lo = (rm & 0xFFFFFFu) - tau;
-    const int ci = ((int)(pix >> 5) + R) * SW + (int)(pix & 31u) + R;
-    // ---- loop A: bilateral sum. Exponent (base 2) of the spatial weight as a quadratic form of (dx, dy)
-    const float qa = sp.kP * Tx * Tx + sp.kQ * Ty * Ty, qb = 2.f * (sp.kP - sp.kQ) * Tx * Ty,
-                qc = sp.kP * Ty * Ty + sp.kQ * Tx * Tx;
-    float c2x = 0.f, c2y = 0.f, c2z = 0.f, e0 = sp.bias_nc, m = 0.f;
-    if (rm >> 24) {  // centre sample: colour term on; its own tap has weight 1, so no bias is needed
-      const float4 CP = s_col[ci];
-      c2x = 2.f * sp.kC * CP.x, c2y = 2.f * sp.kC * CP.y, c2z = 2.f * sp.kC * CP.z;
-      e0 = s_k2[ci];
-      m = 1.f;
-    }
-    float S0 = 0.f, S1 = 0.f, S2 = 0.f, Wsum = 0.f;
-    // items are sorted by type: a warp whose 32 items are all conservative-sample items (no colour term, R21 /
-    // PAPER.md:175 w_color = 1) skips the four colour FMAs of every tap
-    const int it0 = it - lx;
-    if (it0 >= n_centre) {
-#pragma unroll 1
-      for (int dy = -R; dy <= R; ++dy) {
-        const float fdy = (float)dy;
-        const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy;
-        const float4* col_row = s_col + ci + dy * SW;
-#pragma unroll
-        for (int dx = -R; dx <= R; ++dx) {
-          const float4 q = col_row[dx];
-          const uint32_t d = __float_as_uint(q.w);
-          const float fdx = (float)dx;
-          const float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));  // Eq. 10 spatial part
-          const float w = (d - lo <= tau2) ? fast_ex2(e) : 0.f;    // R19: centre-class taps only
-          S0 = fmaf(w, q.x, S0);
-          S1 = fmaf(w, q.y, S1);
-          S2 = fmaf(w, q.z, S2);
-          Wsum += w;
-        }
-      }
-    } else {
-#pragma unroll 1
-      for (int dy = -R; dy <= R; ++dy) {
-        const float fdy = (float)dy;
-        const float r0 = fmaf(qc * fdy, fdy, e0), r1 = qb * fdy;
-        const float* k2_row = s_k2 + ci + dy * SW;
-        const float4* col_row = s_col + ci + dy * SW;
-#pragma unroll
-        for (int dx = -R; dx <= R; ++dx) {
-          const float k2 = k2_row[dx];
-          const float4 q = col_row[dx];
-          const uint32_t d = __float_as_uint(q.w);
-          const float fdx = (float)dx;
-          float e = fmaf(r1, fdx, fmaf(qa, fdx * fdx, r0));                     // Eq. 10 spatial part
-          e = fmaf(c2x, q.x, fmaf(c2y, q.y, fmaf(c2z, q.z, fmaf(m, k2, e))));   // Eq. 10 colour part
-          const float w = (d - lo <= tau2) ? fast_ex2(e) : 0.f;                 // R19: centre-class taps only
-          S0 = fmaf(w, q.x, S0);
-          S1 = fmaf(w, q.y, S1);
-          S2 = fmaf(w, q.z, S2);
-          Wsum += w;
-        }
-      }
-    }
-    // ---- loop B: strip hit counts by Q's class (R18), in (major, minor) coordinates of the tangent: Eq. 9 is
-    // symmetric in x / y and IEEE add / mul commute, so the bits are those of the oracle's x / y order
-    const bool xmaj = fabsf(Tx) >= fabsf(Ty);
-    const float TM = xmaj ? Tx : Ty, TN = xmaj ? Ty : Tx;
-    const int strM = xmaj ? 1 : SW, strN = xmaj ? SW : 1;
-    const float slope = TN / TM;  // |slope| <= 1; T is a unit vector, so the major part is >= 0.707
-    uint32_t Hc = 0, Ha = 0;
-    if (sp.strip_nc == 2) {  // w_strip = 0.5: two candidate minor offsets per major step, all unrolled
-      // Eq. 9 is point-symmetric — negating (fM, fN) negates every product and sum exactly, the squares are the same
-      // bits — and so is the candidate interval, so one membership evaluation serves the taps (s, m) and (-s, -m).
-      // (When the interval of step s holds one integer k, the second candidates k + 1 and -k - 1 / -k + 1 all lie
-      // outside it: farther than strip_hmax from the line, never in the strip — the same zero either way.)
-      {  // s = 0: the pixel itself is in the strip; its neighbour at minor offset 1 is 1 > strip_hmax away
-        const bool cG = s_dqG[ci] - lo <= tau2, cA = s_dqA[ci] - lo <= tau2;
-        Hc += cG ? 1u : 0u;
-        Ha += (cA && !cG) ? 1u : 0u;
-      }
-#pragma unroll
-      for (int s = 1; s <= R; ++s) {
-        const float fM = (float)s;
-        const int m0 = max((int)ceilf(fM * slope - sp.strip_hmax), -R);  // <= R: |s slope| <= R, strip_hmax > 0
-        const float pM = xmul(fM, TM);
-        const int off0 = s * strM + m0 * strN;
-        const bool two = m0 < R;  // m0 + 1 is still a window tap (else its read is clamped and its hit masked)
-#pragma unroll
-        for (int c = 0; c < 2; ++c) {
-          const float fN = (float)(m0 + c);
-          const float dpar = xadd(pM, xmul(fN, TN));
-          const float eM = xsub(fM, xmul(dpar, TM)), eN = xsub(fN, xmul(dpar, TN));
-          bool in = xadd(xmul(eM, eM), xmul(eN, eN)) <= sp.strip_e2_max;
-          if (c) in = in && two;
-          const int off = c ? (two ? off0 + strN : off0) : off0;
-#pragma unroll
-          for (int sg = 0; sg < 2; ++sg) {
-            const int idc = sg ? ci - off : ci + off;
-            const bool cG = s_dqG[idc] - lo <= tau2, cA = s_dqA[idc] - lo <= tau2;
-            Hc += (in && cG) ? 1u : 0u;
-            Ha += (in && cA && !cG) ? 1u : 0u;
-          }
-        }
-      }
-    } else {
-#pragma unroll 1
-      for (int s = -R; s <= R; ++s) {
-        const float fM = (float)s;
-        const int m0 = max((int)ceilf(fM * slope - sp.strip_hmax), -R);
-        const float pM = xmul(fM, TM);
-        for (int c = 0; c < sp.strip_nc; ++c) {
-          const int mm = m0 + c;
-          if (mm <= R) {
-            const float fN = (float)mm;
-            const float dpar = xadd(pM, xmul(fN, TN));
-            const float eM = xsub(fM, xmul(dpar, TM)), eN = xsub(fN, xmul(dpar, TN));
-            const bool in = xadd(xmul(eM, eM), xmul(eN, eN)) <= sp.strip_e2_max;
-            const int idx = ci + s * strM + mm * strN;
-            const bool cG = s_dqG[idx] - lo <= tau2, cA = s_dqA[idx] - lo <= tau2;
-            Hc += (in && cG) ? 1u : 0u;
-            Ha += (in && cA && !cG) ? 1u : 0u;
-          }
-        }
-      }
-    }
-    const float inv = Wsum > 0.f ? 1.0f / Wsum : 0.f;
-    const float alpha = (Hc + Ha) > 0 ? (float)Hc / (float)(Hc + Ha) : 0.f;
-    s_item[it] = make_float4(S0 * inv, S1 * inv, S2 * inv, alpha);
+    const uint32_t lo = (rm & 0xFFFFFFu) - tauq;
+    const int ci = (iy + R) * SW + ix + R;
+    // ---- loop A: bilateral sum, positive base-2 exponent as a quadratic form of (dx, dy)
+    const float qa = -(sp.kP * Tx * Tx + sp.kQ * Ty * Ty), qb = -2.f * (sp.kP - sp.kQ) * Tx * Ty,
+                qc = -(sp.kP * Ty * Ty + sp.kQ * Tx * Tx);
+    const float u = -(float)(R + (ix & 1));
+    const int rowp = iy * HP + (ix >> 1);
+    float4 S;
+    // centre items fill whole warps (n_centre is a multiple of 32): no warp mixes the two loops
+    if (it - lx < n_centre) {  // centre sample: colour term on; its own tap has weight 1, so no bias is needed
+      const float* fa = reinterpret_cast<const float*>(s_pa + (ci >> 1));
+      const float cx = fa[ci & 1], cy = fa[2 + (ci & 1)], cz = fa[4 * NP + (ci & 1)];
+      const float cp2 = reinterpret_cast<const float*>(s_pk)[ci];
+      S = filter_loop_a<R, true>(s_pa + rowp, s_pk + rowp, HP, NP, ix & 1, u, qa, qb, qc, cp2, -2.f * cx, -2.f * cy,
+                                 -2.f * cz, lo, tau2);
+    } else
+      S = filter_loop_a<R, false>(s_pa + rowp, s_pk + rowp, HP, NP, ix & 1, u, qa, qb, qc, -sp.bias_nc, 0.f, 0.f, 0.f,
+                                  lo, tau2);
+    const float alpha = strip_alpha<R>(s_dq, ci, SW, Tx, Ty, lo, tau2, sp);
+    const float inv = S.w > 0.f ? inv_kappa / S.w : 0.f;
+    s_item[it] = make_float4(S.x * inv, S.y * inv, S.z * inv, alpha);
   }
   __syncthreads();
   // ---- (4) combine and composite over the background (R29)
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
-    if (!inside[k]) continue;
+    if (slot_c[k] < 0 && slot_a[k] < 0) continue;  // (pixels without a hit were written at the start)
     float r = 0.f, g = 0.f, b = 0.f, alpha = 0.f;
     if (slot_c[k] >= 0) {
       const float4 a = s_item[slot_c[k]];
@@ -546,13 +595,18 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
         b = f.w * f.z + (1.f - f.w) * a.z;
         alpha = 1.f;
       }
-    } else if (slot_a[k] >= 0) {
+    } else {
       const float4 a = s_item[slot_a[k]];
       r = a.x, g = a.y, b = a.z, alpha = a.w;
     }
+    const size_t p = (size_t)(y0 + ly + 8 * k) * W + x0 + lx;
+    float4 bg = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
+    if (scene_rgb) {
+      const float4 s4 = __ldg(&scene_rgb[p]);
+      bg = make_float4(s4.x, s4.y, s4.z, sp.bg_alpha ? s4.w : 0.f);
+    }
     const float ia = 1.f - alpha;
-    store_rgba(out, (size_t)(y0 + ly + 8 * k) * W + x0 + lx,
-               make_float4(alpha * r + ia * bg[k].x, alpha * g + ia * bg[k].y, alpha * b + ia * bg[k].z, alpha + ia * bg[k].w),
+    store_rgba(out, p, make_float4(alpha * r + ia * bg.x, alpha * g + ia * bg.y, alpha * b + ia * bg.z, alpha + ia * bg.w),
                sp.rgb16);
   }
 }
@@ -611,8 +665,10 @@ template <int R>
 static void launch_filter_r(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                             ShadeParams sp, const unsigned long long* gbuf, const float4* colour,
                             const float4* scene_rgb, float4* out, LaunchState* ls, cudaStream_t st) {
-  constexpr int NS = (FT_W + 2 * R) * (FT_H + 2 * R);
-  constexpr size_t smem = (size_t)NS * (sizeof(float4) + 3 * sizeof(uint32_t)) + 2 * FT_W * FT_H * sizeof(float4);
+  constexpr int NS = (FT_W + 2 * R) * (FT_H + 2 * R), NP = NS / 2, NI = 2 * FT_W * FT_H;
+  // pairs: two float4 + one uint2; strip depths: one uint2 per pixel; items: one float4
+  constexpr size_t smem = (size_t)NP * (2 * sizeof(float4) + sizeof(uint2)) + (size_t)NS * sizeof(uint2) +
+                          (size_t)NI * sizeof(float4);
   if (!ls->filter_set[R]) {  // once per context (the opt-in is per device)
     raise_dyn_smem(k_filter<R>, smem);
     ls->filter_set[R] = true;
