@@ -250,6 +250,9 @@ __device__ __forceinline__ float2 screen_tangent_payload(const CamDev& cam, int 
 #ifndef FILT_MIN_BLOCKS
 #define FILT_MIN_BLOCKS 4  // CTAs per SM the register budget is held to
 #endif
+#ifndef FILT_DEAL
+#define FILT_DEAL 1  // conservative-sample items dealt by bank class (0: packed in pixel order)
+#endif
 #define DQ_NONE 0x40000000u
 #define DQ_OFF 0x80000000u  // as the low end of a depth window: no depth lies within 2 tau above it
 
@@ -519,7 +522,14 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
 #pragma unroll
   for (int c = 0; c < 8; ++c) max_a = max(max_a, s_cc[FT_H][c]);
   const int n_centre = (int)((s_cn[FT_H] + 31u) & ~31u);  // centre slots, rounded up to whole warps
+#if FILT_DEAL
   const int n_item = n_centre + (int)(8u * max_a);
+#else
+  uint32_t tot_a = 0;
+#pragma unroll
+  for (int c = 0; c < 8; ++c) tot_a += s_cc[FT_H][c];
+  const int n_item = n_centre + (int)tot_a;
+#endif
   for (int i = tid; i < n_item; i += 256) s_item[i].w = __uint_as_float(0xFFFFFFFFu);  // empty slot
   __syncthreads();
 #pragma unroll
@@ -531,9 +541,16 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
       s_item[slot_c[k]] = make_float4(Tc[k].x, Tc[k].y, __uint_as_float(w_dq(G[k]) | 0x1000000u), __uint_as_float(pix));
     }
     if ((balA[k] >> lx) & 1u) {
+#if FILT_DEAL
       const int cls = ((lx >> 1) + KS * row) & 7;
       const uint32_t same = 0x00030003u << (2 * ((lx >> 1) & 7));  // the four lanes of this row in my class
       slot_a[k] = n_centre + (int)((s_cc[row][cls] + __popc(balA[k] & same & lt_mask)) * 8u) + cls;
+#else
+      uint32_t before = 0;  // pixel order: items of the rows above, then of the lanes to the left
+#pragma unroll
+      for (int c = 0; c < 8; ++c) before += s_cc[row][c];
+      slot_a[k] = n_centre + (int)(before + __popc(balA[k] & lt_mask));
+#endif
       s_item[slot_a[k]] = make_float4(Ta[k].x, Ta[k].y, __uint_as_float(w_dq(A[k])), __uint_as_float(pix));
     }
   }
