@@ -159,6 +159,11 @@ __device__ __forceinline__ Strand strand_setup(const GroomDev& g, uint32_t id_lo
   return s;
 }
 
+// b0 r0 + b1 r1 + b2 r2 on two components at once
+__device__ __forceinline__ float2 blend2(float b0, float b1, float b2, float2 r0, float2 r1, float2 r2) {
+  return __ffma2_rn(make_float2(b2, b2), r2, __ffma2_rn(make_float2(b1, b1), r1, __fmul2_rn(make_float2(b0, b0), r0)));
+}
+
 // stage 3 for one vertex: control point j of a strand, from the bundle table row and the strand's record; M = the
 // instance transform (R-inst, applied last) or nullptr. Returns (x, y, z, ao).
 __device__ __forceinline__ float4 vertex(const float* __restrict__ tab, uint32_t j, float b1, float b2, float cphi,
@@ -167,8 +172,12 @@ __device__ __forceinline__ float4 vertex(const float* __restrict__ tab, uint32_t
   const float b0 = (1.0f - b1) - b2;
   const float4* r4 = reinterpret_cast<const float4*>(tab + (size_t)j * HAIR_ROW);
   const float4 E0 = r4[0], E1 = r4[1], E2 = r4[2];
-  F3 p = f3(b0 * E0.x + b1 * E1.x + b2 * E2.x, b0 * E0.y + b1 * E1.y + b2 * E2.y, b0 * E0.z + b1 * E1.z + b2 * E2.z);
-  float aov = fminf(fmaxf(b0 * E0.w + b1 * E1.w + b2 * E2.w, 0.f), 1.f);
+  // barycentric blend of the three table rows in packed fp32 (sm_100 FFMA2: the (x, y) and (z, ao) halves of a row
+  // are register pairs as loaded; one issue slot for two FMAs)
+  const float2 pxy = blend2(b0, b1, b2, make_float2(E0.x, E0.y), make_float2(E1.x, E1.y), make_float2(E2.x, E2.y));
+  const float2 pza = blend2(b0, b1, b2, make_float2(E0.z, E0.w), make_float2(E1.z, E1.w), make_float2(E2.z, E2.w));
+  F3 p = f3(pxy.x, pxy.y, pza.x);
+  float aov = fminf(fmaxf(pza.y, 0.f), 1.f);
   if (ops) {
     if (ops & (HAIR_OP_CLUMP | HAIR_OP_TWIST)) {
       const float4 cc4 = r4[6];
@@ -185,8 +194,9 @@ __device__ __forceinline__ float4 vertex(const float* __restrict__ tab, uint32_t
     if (ops & (HAIR_OP_CURL | HAIR_OP_FRIZZ)) {
       // frame from the UNSTYLED base spline: T = normalised derivative, N from the cage edge
       const float4 D0 = r4[3], D1 = r4[4], D2 = r4[5];
-      const F3 T = normalize(f3(b0 * D0.x + b1 * D1.x + b2 * D2.x, b0 * D0.y + b1 * D1.y + b2 * D2.y,
-                                b0 * D0.z + b1 * D1.z + b2 * D2.z));
+      const float2 dxy = blend2(b0, b1, b2, make_float2(D0.x, D0.y), make_float2(D1.x, D1.y), make_float2(D2.x, D2.y));
+      const float2 dzw = blend2(b0, b1, b2, make_float2(D0.z, D0.w), make_float2(D1.z, D1.w), make_float2(D2.z, D2.w));
+      const F3 T = normalize(f3(dxy.x, dxy.y, dzw.x));  // (dzw.y blends the rows' styling scalars: unused)
       const float4 ef4 = r4[8];
       const F3 Ef = f3(ef4.x, ef4.y, ef4.z);
       F3 Nn = Ef - dot(Ef, T) * T;

@@ -51,7 +51,6 @@ k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restri
     const GroomDev& g = sc->g[gi];
     const uint32_t rel = gid - g.gid_base;
     const uint32_t q = rel / g.T, t = rel - q * g.T;
-    const uint32_t Lv = g.Lv;
     const uint32_t ops = g.op_mask;
 
     // ---- stages 1 + 2: the per-bundle table
@@ -63,7 +62,14 @@ k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restri
 #pragma unroll
       for (int a = 0; a < 12; ++a) M[a] = __ldg(&g.xform[q * 12 + a]);
     const uint32_t off_t = __ldg(&g.off[t]);
-    const uint32_t q32 = 32u / C, r32 = 32u - q32 * C;  // (k, j) of a lane advance by 32 vertices per iteration
+    // A warp iteration covers SB strands x (32 / SB) consecutive control points: the lanes of one control point read
+    // the same table row (one shared-memory wavefront per LDS.128 for SB = 4 instead of four when every lane has a row
+    // of its own), each strand's run is 32 / SB consecutive vertices (128 contiguous bytes for SB = 4). Control points
+    // are counted through the groups of SB strands of a batch without a break, so only the batch's last iteration has
+    // idle lanes; small bundles take fewer strands at a time.
+    const uint32_t sb_log = nlod >= 6 ? 2u : (nlod >= 2 ? 1u : 0u), SB = 1u << sb_log, TB = 32u >> sb_log;
+    const uint32_t s_lane = lane & (SB - 1u), t_lane = lane >> sb_log;
+    const uint32_t qT = TB / C, rT = TB - qT * C;  // (group, j) of a lane advance by TB control points per iteration
     for (uint32_t k0 = 0; k0 < nlod; k0 += 32) {
       // per strand, once (lanes = strands of this batch): root barycentrics (R6) and the curl phase
       const uint32_t nk = min(32u, nlod - k0);
@@ -75,17 +81,20 @@ k_generate(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restri
         strand_rec[g.sid_base + q * g.N + off_t + k0 + lane] = make_uint2(e.w + (k0 + lane) * C, C | (gi << 8));
       }
       __syncwarp();
-      const uint32_t n_vb = nk * C;
+      const uint32_t n_t = ((nk + SB - 1u) >> sb_log) * C;  // control points over all groups of the batch
       float4* out = vertices + e.w + (size_t)k0 * C;
-      uint32_t k = lane / C, j = lane - k * C;
-      for (uint32_t v = lane; v < n_vb; v += 32) {
-        const float4 sr = srec[k];
-        out[v] = gen::vertex(tab, j, sr.x, sr.y, sr.z, sr.w, sbase[k], ops, has_m ? M : nullptr);
-        k += q32;
-        j += r32;
+      uint32_t gq = t_lane / C, j = t_lane - gq * C;
+      for (uint32_t t0 = 0; t0 < n_t; t0 += TB) {
+        const uint32_t k = (gq << sb_log) + s_lane;
+        if (t0 + t_lane < n_t && k < nk) {
+          const float4 sr = srec[k];
+          out[k * C + j] = gen::vertex(tab, j, sr.x, sr.y, sr.z, sr.w, sbase[k], ops, has_m ? M : nullptr);
+        }
+        gq += qT;
+        j += rT;
         if (j >= C) {
           j -= C;
-          ++k;
+          ++gq;
         }
       }
       __syncwarp();

@@ -34,6 +34,7 @@ void launch_atomic_microbench(int mode, unsigned long long* words, unsigned long
 //  mode 0  "row":    32 consecutive pairs of one image row (512 contiguous bytes: an x-major segment's columns),
 //  mode 1  "column": the same x in 32 consecutive rows (stride pitch * 16 bytes: a y-major segment's columns),
 //  mode 2  "random": 32 unrelated pairs (sub-pixel segments scattered over the frame),
+//  mode 3 / 4  the column / row walk in a G-buffer laid out in blocks of 2 x 4 pixels,
 // at a hashed position that changes every step. pitch = pairs per image row.
 #define L2_MLP 4
 __global__ void __launch_bounds__(256) k_l2_load_bench(int mode, const ulonglong2* __restrict__ pairs, uint32_t n_pairs,
@@ -52,7 +53,14 @@ __global__ void __launch_bounds__(256) k_l2_load_bench(int mode, const ulonglong
       uint32_t idx;
       if (mode == 0) idx = h % (n_pairs - 32u) + lane;
       else if (mode == 1) idx = ((h >> 12) % (rows - 32u) + lane) * pitch + (h & 0xFFFu) % pitch;
-      else idx = pcg(h ^ (lane * 0x85EBCA6Bu)) % n_pairs;
+      else if (mode == 2) idx = pcg(h ^ (lane * 0x85EBCA6Bu)) % n_pairs;
+      else {  // the same walks in a layout of 2 x 4-pixel blocks (one 128-byte line = 2 columns x 4 rows)
+        uint32_t x, y;
+        if (mode == 3) x = (h & 0xFFFu) % pitch, y = (h >> 12) % (rows - 32u) + lane;  // column
+        else x = h % (pitch - 32u) + lane, y = (h >> 12) % rows;                        // row
+        idx = ((y >> 2) * (pitch >> 1) + (x >> 1)) * 8u + (y & 3u) * 2u + (x & 1u);
+        if (idx >= n_pairs) idx = n_pairs - 1u;
+      }
       v[u] = __ldcg(&pairs[idx]);
     }
 #pragma unroll
