@@ -106,6 +106,14 @@ def lib():
         L.orc_frame_beta.argtypes = [vp, vp, vp, vp]
         L.orc_depth_fix.restype = C.c_double
         L.orc_depth_fix.argtypes = [C.c_double, C.c_double]
+        L.orc_frame_dom_count.restype = C.c_int
+        L.orc_frame_dom_count.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.orc_dom_transmittance.restype = C.c_double
+        L.orc_dom_transmittance.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, vp]
+        L.orc_frame_set_dom.restype = C.c_int
+        L.orc_frame_set_dom.argtypes = [vp, C.c_uint32, vp, vp, vp, vp, C.c_double]
+        L.orc_frame_set_dom_beta.restype = None
+        L.orc_frame_set_dom_beta.argtypes = [vp, vp, C.c_uint32]
         L.orc_frame_get_vertices_f64.argtypes = [vp, vp]
         L.orc_frame_get_vertices_f32.argtypes = [vp, vp]
         L.orc_frame_set_vertices_f32.argtypes = [vp, vp, u64]
@@ -440,6 +448,40 @@ class Frame:
         self.L.orc_frame_get_out(self.h, _ptr(out))
         return out
 
+    # ---- deep opacity maps (DESIGN.md R-dom)
+    def dom_build(self, light_cam: dict, prm: dict, D3):
+        """z0 [h][w] uint32 and fragment counts [h][w][4] uint32 of the frame's CURRENT vertices seen from `light_cam`
+        (runs O4 with that camera first). D3: ends of layers 0..2 in depth steps."""
+        self.raster(light_cam, prm)
+        c, p = make_camera(light_cam), make_params(prm)
+        w, h = light_cam["width"], light_cam["height"]
+        z0 = np.zeros((h, w), np.uint32)
+        cnt = np.zeros((h, w, 4), np.uint32)
+        D = np.ascontiguousarray(D3, dtype=np.uint32)
+        r = self.L.orc_frame_dom_count(self.h, C.byref(c), C.byref(p), _ptr(D), _ptr(z0), _ptr(cnt))
+        assert r == 0, r
+        return z0, cnt
+
+    def set_dom(self, light: int, light_cam, z0=None, cnt=None, D4=None, alpha_s: float = 0.0) -> None:
+        """O6 scales light `light` by the transmittance of this map (light_cam None: off)."""
+        if not hasattr(self, "_dom"):
+            self._dom = {}
+        if light_cam is None:
+            self.L.orc_frame_set_dom(self.h, light, None, None, None, None, 0.0)
+            self._dom.pop(light, None)
+            return
+        c = make_camera(light_cam)
+        z0 = np.ascontiguousarray(z0, dtype=np.uint32)
+        cnt = np.ascontiguousarray(cnt, dtype=np.uint32)
+        D = np.ascontiguousarray(D4, dtype=np.uint32)
+        self._dom[light] = (c, z0, cnt, D)  # the C side keeps the pointers
+        r = self.L.orc_frame_set_dom(self.h, light, C.byref(c), _ptr(z0), _ptr(cnt), _ptr(D), float(alpha_s))
+        assert r == 0, r
+
+    def set_dom_beta(self, beta) -> None:
+        b = np.ascontiguousarray(beta, dtype=np.float64)
+        self.L.orc_frame_set_dom_beta(self.h, _ptr(b), b.size)
+
     # ---- O6 / O7
     def shade(self, cam: dict, prm: dict):
         c, p = make_camera(cam), make_params(prm)
@@ -481,6 +523,16 @@ def pcg(v: int) -> int:
 
 def hash3(seed: int, i: int, stream: int) -> int:
     return lib().orc_hash3(seed, i, stream)
+
+
+def dom_transmittance(light_cam: dict, z0, cnt, D4, alpha_s: float, beta: float, p) -> float:
+    """Transmittance towards the light of the deep opacity map (z0, cnt) at world point p (see hair_oracle.h)."""
+    c = make_camera(light_cam)
+    z0 = np.ascontiguousarray(z0, dtype=np.uint32)
+    cnt = np.ascontiguousarray(cnt, dtype=np.uint32)
+    D = np.ascontiguousarray(D4, dtype=np.uint32)
+    pp = np.ascontiguousarray(p, dtype=np.float32)
+    return float(lib().orc_dom_transmittance(C.byref(c), _ptr(z0), _ptr(cnt), _ptr(D), float(alpha_s), float(beta), _ptr(pp)))
 
 
 def depth_fix(d: float, delta: float) -> float:

@@ -295,6 +295,17 @@ struct orc_frame {
   std::vector<float> scene_alpha;   // [H][W] or empty
   uint32_t groom_mask = 0xFFFFFFFFu;
   int payload_mode = 0;  // 0: strand id | segment | t (R7); 1: the paper's payload (R-payload)
+  // deep opacity maps of the point lights (DESIGN.md R-dom), set by orc_frame_set_dom: O6 then scales
+  // light l's contribution by the transmittance towards it. Not owned: the caller keeps the arrays alive.
+  struct Dom {
+    bool on = false;
+    orc_camera cam;
+    const uint32_t* z0 = nullptr;   // [res][res] depth of the conservative layer seen from the light, 0xFFFFFFFF = none
+    const uint32_t* cnt = nullptr;  // [res][res][4] fragments per layer
+    uint32_t D[4];                  // layer ends, in depth steps behind z0
+    double alpha_s = 0.0;
+  } dom[4];
+  double dom_beta[16] = {1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1};  // Eq. 7: per groom, of the frame being shaded
 };
 
 namespace {
@@ -966,35 +977,22 @@ int orc_root(const orc_frame* f, uint32_t groom, uint32_t id_local, double b[3],
 }
 
 // ------------------------------------------------------------------ O4 (+ O5: the min IS the resolve)
-int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
-                     const uint32_t* order, uint64_t counts[3]) {
-  Cam k = make_cam(cam);
-  f->W = k.W;
-  f->H = k.H;
-  f->gbuf.assign(size_t(k.W) * k.H * 2, EMPTY);
-  if (!f->scene_zn.empty()) {  // R-scene: both layers start at the scene's quantised depth (R8), payload = none
-    if (f->scene_zn.size() != size_t(k.W) * k.H) return -3;
-    for (size_t p = 0; p < size_t(k.W) * k.H; ++p) {
-      float zn = std::min(std::max(f->scene_zn[p], 0.f), 1.f);
-      uint64_t seed = (uint64_t(quant_depth(zn)) << 40) | PAYLOAD_NONE;
-      f->gbuf[p * 2] = f->gbuf[p * 2 + 1] = seed;
-    }
-  }
-  if (!f->scene_dq.empty()) {  // R-seq: depth kept from the previous passes, as the 24-bit integers themselves
-    if (f->scene_dq.size() != size_t(k.W) * k.H) return -3;
-    for (size_t p = 0; p < size_t(k.W) * k.H; ++p)
-      f->gbuf[p * 2] = f->gbuf[p * 2 + 1] = (uint64_t(f->scene_dq[p] & 0xFFFFFFu) << 40) | PAYLOAD_NONE;
-  }
-  if (f->v32.size() != size_t(f->n_vertices) * 4) return -1;
-  uint64_t n_center = 0, n_cons = 0, n_seg = 0;
+// Enumerates every (segment, pixel) hit of the frame's vertices under camera k in strand order (`order`: optional
+// permutation of the strands): fn(strand, j, x, y, cover bits (1 = conservative, 2 = centre), zn, t). The coverage
+// arithmetic of R9-R12 lives here, once, for the G-buffer resolve and for the deep-opacity-map fragment count.
+}  // extern "C"
+namespace {
+struct StrandDir {
+  uint64_t voff;
+  uint32_t C, sid;
+  float width;
+  uint32_t a1, a2;  // R-payload: the strand's root coordinates (u, v)
+};
+template <class Fn>
+uint64_t for_each_hit(const orc_frame* f, const Cam& k, const orc_params* prm, const uint32_t* order, Fn&& fn) {
+  uint64_t n_seg = 0;
   // strand directory in slot order
-  struct S {
-    uint64_t voff;
-    uint32_t C, sid;
-    float width;
-    uint32_t a1, a2;  // R-payload: the strand's root coordinates (u, v)
-  };
-  std::vector<S> dir;
+  std::vector<StrandDir> dir;
   dir.reserve(f->n_strands);
   for (const Groom& g : f->grooms)
     for (uint32_t q = 0; q < g.Q; ++q)
@@ -1008,7 +1006,7 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
         }
       }
   for (size_t si = 0; si < dir.size(); ++si) {
-    const S& s = dir[order ? order[si] : si];
+    const StrandDir& s = dir[order ? order[si] : si];
     for (uint32_t j = 0; j + 1 < s.C; ++j) {
       const float* va = &f->v32[(s.voff + j) * 4];
       const float* vb = va + 4;
@@ -1045,19 +1043,48 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
           float zn = t * dz;  // R11: depth at the closest point, linear in screen space
           zn = a.zn + zn;
           if (zn < 0.f || zn > 1.f) continue;
-          uint64_t w = pack(zn, s.sid, j, t);
-          if (f->payload_mode)  // R-payload: same depth bits, the paper's 40 payload bits
-            w = (uint64_t(quant_depth(zn)) << 40) | payload40(&f->v32[s.voff * 4], int(j), int(s.C), t, s.a1, s.a2);
-          uint64_t* px = &f->gbuf[(size_t(y) * k.W + x) * 2];
-          ++n_cons;
-          px[1] = std::min(px[1], w);  // PAPER.md:85 atomic min, depth in the high bits
-          if (c & 2) {
-            ++n_center;
-            px[0] = std::min(px[0], w);
-          }
+          fn(s, j, x, y, c, zn, t);
         }
     }
   }
+  return n_seg;
+}
+}  // namespace
+extern "C" {
+
+int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
+                     const uint32_t* order, uint64_t counts[3]) {
+  Cam k = make_cam(cam);
+  f->W = k.W;
+  f->H = k.H;
+  f->gbuf.assign(size_t(k.W) * k.H * 2, EMPTY);
+  if (!f->scene_zn.empty()) {  // R-scene: both layers start at the scene's quantised depth (R8), payload = none
+    if (f->scene_zn.size() != size_t(k.W) * k.H) return -3;
+    for (size_t p = 0; p < size_t(k.W) * k.H; ++p) {
+      float zn = std::min(std::max(f->scene_zn[p], 0.f), 1.f);
+      uint64_t seed = (uint64_t(quant_depth(zn)) << 40) | PAYLOAD_NONE;
+      f->gbuf[p * 2] = f->gbuf[p * 2 + 1] = seed;
+    }
+  }
+  if (!f->scene_dq.empty()) {  // R-seq: depth kept from the previous passes, as the 24-bit integers themselves
+    if (f->scene_dq.size() != size_t(k.W) * k.H) return -3;
+    for (size_t p = 0; p < size_t(k.W) * k.H; ++p)
+      f->gbuf[p * 2] = f->gbuf[p * 2 + 1] = (uint64_t(f->scene_dq[p] & 0xFFFFFFu) << 40) | PAYLOAD_NONE;
+  }
+  if (f->v32.size() != size_t(f->n_vertices) * 4) return -1;
+  uint64_t n_center = 0, n_cons = 0;
+  const uint64_t n_seg = for_each_hit(f, k, prm, order, [&](const StrandDir& s, uint32_t j, int x, int y, int c, float zn, float t) {
+    uint64_t w = pack(zn, s.sid, j, t);
+    if (f->payload_mode)  // R-payload: same depth bits, the paper's 40 payload bits
+      w = (uint64_t(quant_depth(zn)) << 40) | payload40(&f->v32[s.voff * 4], int(j), int(s.C), t, s.a1, s.a2);
+    uint64_t* px = &f->gbuf[(size_t(y) * k.W + x) * 2];
+    ++n_cons;
+    px[1] = std::min(px[1], w);  // PAPER.md:85 atomic min, depth in the high bits
+    if (c & 2) {
+      ++n_center;
+      px[0] = std::min(px[0], w);
+    }
+  });
   if (counts) {
     counts[0] = n_center;
     counts[1] = n_cons;
@@ -1065,6 +1092,90 @@ int orc_frame_raster(orc_frame* f, const orc_camera* cam, const orc_params* prm,
   }
   return 0;
 }
+
+// ------------------------------------------------------------------ deep opacity maps (DESIGN.md R-dom)
+// The paper names the technique (Yuksel and Keyser 2008) and no more. As restated here, for one light camera:
+//  z0(u, v)     = depth of the nearest hair that touches light pixel (u, v): the conservative layer of the frame's
+//                 G-buffer rendered from the light, as its 24-bit integer (0xFFFFFFFF where nothing is hit);
+//  cnt(u, v, k) = number of (segment, pixel) conservative hits of that pixel whose depth lies in layer k behind z0,
+//                 layer k = [D[k-1], D[k]) depth steps (D[-1] = 0, the last layer is open-ended).
+// orc_frame_raster under the same camera must have run before (it leaves z0 in the frame's G-buffer).
+int orc_frame_dom_count(orc_frame* f, const orc_camera* cam, const orc_params* prm, const uint32_t D[3],
+                        uint32_t* z0, uint32_t* cnt) {
+  Cam k = make_cam(cam);
+  if (f->W != k.W || f->H != k.H || f->gbuf.size() != size_t(k.W) * k.H * 2) return -1;
+  if (f->v32.size() != size_t(f->n_vertices) * 4) return -1;
+  const size_t n_px = size_t(k.W) * k.H;
+  for (size_t p = 0; p < n_px; ++p) z0[p] = none(f->gbuf[p * 2 + 1]) ? 0xFFFFFFFFu : w_dq(f->gbuf[p * 2 + 1]);
+  std::memset(cnt, 0, n_px * 4 * sizeof(uint32_t));
+  for_each_hit(f, k, prm, nullptr, [&](const StrandDir&, uint32_t, int x, int y, int, float zn, float) {
+    const size_t p = size_t(y) * k.W + x;
+    const uint32_t d = quant_depth(zn) - z0[p];  // >= 0: z0 is the minimum over these very hits
+    const int layer = (d >= D[0]) + (d >= D[1]) + (d >= D[2]);
+    ++cnt[p * 4 + layer];
+  });
+  return 0;
+}
+
+// Optical depth seen from ONE texel at `d` depth steps behind its z0: the cumulative fragment count, piecewise linear
+// through (0, 0), (D0, c0), (D1, c0 + c1), (D2, c0 + c1 + c2), (D3, c0 + .. + c3), constant beyond (the open last
+// layer is taken to end at D3).
+static double dom_texel_omega(const uint32_t* cnt4, const uint32_t D[4], double d) {
+  if (!(d > 0.0)) return 0.0;
+  double lo = 0.0, acc = 0.0;
+  for (int kk = 0; kk < 4; ++kk) {
+    const double hi = double(D[kk]);
+    if (d < hi) return acc + double(cnt4[kk]) * (d - lo) / (hi - lo);
+    acc += double(cnt4[kk]);
+    lo = hi;
+  }
+  return acc;
+}
+
+// Transmittance towards the light of the map at world point p (Eq. 6: V = exp(-sigma d), with sigma d = alpha_s times
+// the fragment count in front of the point). The point's depth behind each texel's z0 is scaled by beta before the
+// lookup (Eq. 7: d_eff = beta d, the depth-comparison fix of PAPER.md:138-152). The four texels around the point are
+// blended bilinearly (texel centres at integer + 1/2); a texel without hair, or outside the map, contributes 0.
+double orc_dom_transmittance(const orc_camera* cam, const uint32_t* z0, const uint32_t* cnt, const uint32_t D[4],
+                             double alpha_s, double beta, const float p[3]) {
+  Cam k = make_cam(cam);
+  Proj q = project(k, p[0], p[1], p[2]);
+  if (!q.valid) return 1.0;
+  const float zc = std::min(std::max(q.zn, 0.f), 1.f);
+  const uint32_t dq = quant_depth(zc);
+  const double fx = double(q.sx) - 0.5, fy = double(q.sy) - 0.5;
+  const double x0 = std::floor(fx), y0 = std::floor(fy);
+  const double wx = fx - x0, wy = fy - y0;
+  double omega = 0.0;
+  for (int dy = 0; dy < 2; ++dy)
+    for (int dx = 0; dx < 2; ++dx) {
+      const double xi = x0 + dx, yi = y0 + dy;
+      if (xi < 0 || yi < 0 || xi >= double(k.W) || yi >= double(k.H)) continue;
+      const size_t t = size_t(yi) * k.W + size_t(xi);
+      if (z0[t] == 0xFFFFFFFFu || dq <= z0[t]) continue;
+      const double w = (dx ? wx : 1.0 - wx) * (dy ? wy : 1.0 - wy);
+      omega += w * dom_texel_omega(&cnt[t * 4], D, beta * double(dq - z0[t]));
+    }
+  return std::exp(-alpha_s * omega);
+}
+
+int orc_frame_set_dom(orc_frame* f, uint32_t light, const orc_camera* cam, const uint32_t* z0, const uint32_t* cnt,
+                      const uint32_t D[4], double alpha_s) {
+  if (light >= 4) return -1;
+  orc_frame::Dom& d = f->dom[light];
+  d.on = cam != nullptr;
+  if (!d.on) return 0;
+  d.cam = *cam;
+  d.z0 = z0;
+  d.cnt = cnt;
+  for (int i = 0; i < 4; ++i) d.D[i] = D[i];
+  d.alpha_s = alpha_s;
+  return 0;
+}
+void orc_frame_set_dom_beta(orc_frame* f, const double* beta, uint32_t n) {
+  for (uint32_t g = 0; g < 16; ++g) f->dom_beta[g] = g < n ? beta[g] : 1.0;
+}
+
 void orc_frame_get_gbuffer(const orc_frame* f, uint64_t* o) {
   std::memcpy(o, f->gbuf.data(), f->gbuf.size() * sizeof(uint64_t));
 }
@@ -1199,8 +1310,8 @@ int orc_frame_resolve_msaa(orc_frame* f, const orc_camera* cam, const orc_params
 // O6 for one word: the shaded linear RGB of the hit it names (stand-in model, R23). Returns false if the strand
 // id does not resolve.
 // the stand-in shading model (R23) at one point: position, unit tangent, strand parameter w, ambient occlusion
-static void shade_model(const Groom* g, const Cam& k, const orc_params* prm, V3 pos, V3 T, double w, double ao,
-                        double rgb[3]) {
+static void shade_model(const orc_frame* f, const Groom* g, const Cam& k, const orc_params* prm, V3 pos, V3 T, double w,
+                        double ao, double rgb[3]) {
   V3 eye = {double(k.eye[0]), double(k.eye[1]), double(k.eye[2])};
   double alb[3];
   for (int c = 0; c < 3; ++c)
@@ -1219,8 +1330,16 @@ static void shade_model(const Groom* g, const Cam& k, const orc_params* prm, V3 
     double th = 0.5 * (std::asin(sin_i) + std::asin(sin_o));
     double MR = std::exp(-(th + tilt) * (th + tilt) / (2.0 * beta * beta));
     double MT = std::exp(-(th - 1.5 * tilt) * (th - 1.5 * tilt) / (8.0 * beta * beta));
+    // volumetric shadow (R-dom): transmittance towards light li from its deep opacity map, looked up
+    // with the depth-comparison fix of the groom being shaded (Eq. 7)
+    double Tl = 1.0;
+    if (li < 4 && f->dom[li].on) {
+      const float pf[3] = {float(pos.x), float(pos.y), float(pos.z)};
+      const orc_frame::Dom& dm = f->dom[li];
+      Tl = orc_dom_transmittance(&dm.cam, dm.z0, dm.cnt, dm.D, dm.alpha_s, f->dom_beta[g - f->grooms.data()], pf);
+    }
     for (int c = 0; c < 3; ++c) {
-      double E = double(prm->light_rgb[li][c]) / d2;
+      double E = Tl * double(prm->light_rgb[li][c]) / d2;
       rgb[c] += E * cos_i * (double(prm->k_d) * alb[c] + double(prm->k_R) * MR + double(prm->k_TRT) * MT * alb[c]);
     }
   }
@@ -1242,7 +1361,7 @@ static bool shade_word(const orc_frame* f, const Cam& k, const orc_params* prm, 
   V3 Tj1 = calcTangent(j + 1, C, V(j), V(j + 1), V(j + 2));
   V3 T = normalize((1 - t) * Tj + t * Tj1);
   double w = (double(j) + t) / double(C - 1);
-  shade_model(g, k, prm, pos, T, w, ao, rgb);
+  shade_model(f, g, k, prm, pos, T, w, ao, rgb);
   return true;
 }
 
@@ -1260,12 +1379,12 @@ static V3 position_from_depth(const Cam& k, int x, int y, uint32_t dq) {
   return p;
 }
 // O6 from the paper's payload alone: no vertex is read
-static void shade_payload(const Groom* g, const Cam& k, const orc_params* prm, int x, int y, uint64_t G,
-                          double rgb[3]) {
+static void shade_payload(const orc_frame* f, const Groom* g, const Cam& k, const orc_params* prm, int x, int y,
+                          uint64_t G, double rgb[3]) {
   F3 Tf = oct_decode(uint32_t(G >> 32) & 0xFFu, uint32_t(G >> 24) & 0xFFu);
   V3 T = {double(Tf.x), double(Tf.y), double(Tf.z)};
   double w = double(uint32_t(G >> 6) & 63u) / 63.0, ao = double(uint32_t(G) & 63u) / 63.0;
-  shade_model(g, k, prm, position_from_depth(k, x, y, w_dq(G)), T, w, ao, rgb);
+  shade_model(f, g, k, prm, position_from_depth(k, x, y, w_dq(G)), T, w, ao, rgb);
 }
 // R22 for the paper's payload: screen direction of the decoded tangent at the pixel centre. With view-space
 // tangent (tx, ty, tz) and the pixel's ray (cx, cy, 1), d(sx, sy)/ds is parallel to (tx - cx tz, cy tz - ty),
@@ -1323,7 +1442,7 @@ int orc_frame_shade(orc_frame* f, const orc_camera* cam, const orc_params* prm) 
       if (!none(A)) screen_tangent_payload(k, sx, sy, A, &f->tang[p * 4 + 2]);
       if (none(G)) continue;
       screen_tangent_payload(k, sx, sy, G, &f->tang[p * 4]);
-      shade_payload(pg, k, prm, sx, sy, G, rgb);
+      shade_payload(f, pg, k, prm, sx, sy, G, rgb);
       for (int c = 0; c < 3; ++c) f->colour[p * 3 + c] = rgb[c];
       continue;
     }

@@ -116,6 +116,27 @@ void orc_frame_beta(const orc_frame*, double* beta, double* delta, double* beta_
  * beta = exp(-delta): the additive shift -delta in log-depth space, ln d_eff = ln d - delta, i.e. d_eff = d exp(-delta) */
 double orc_depth_fix(double d, double delta);
 
+/* Deep opacity maps of the point lights ("Volumetric shadows are computed using deep-opacity maps ...,
+ * which we query using the depth-correction described in Section 3.2"; DESIGN.md R-dom). The paper gives no more
+ * than the name, so this follows the published technique as restated in hair_oracle.cpp: per light pixel the depth
+ * z0 of the nearest hair (the conservative layer of a G-buffer rendered from the light, orc_frame_raster with the
+ * light's camera, which must have run before) and, in layers behind it, the number of hair fragments.
+ *  D[3]  ends of layers 0..2 in 24-bit depth steps behind z0 (layer 3 is open-ended)
+ *  z0    out, [h][w]: 24-bit depth, 0xFFFFFFFF = no hair;  cnt  out, [h][w][4] fragments per layer.
+ * Pins: tests/test_oracle_shadow.py. */
+int orc_frame_dom_count(orc_frame*, const orc_camera* light_cam, const orc_params*, const uint32_t D[3], uint32_t* z0,
+                        uint32_t* cnt);
+/* Transmittance exp(-alpha_s * fragments in front) towards the light at world point p: fragment count piecewise
+ * linear in the depth behind z0 through the layer ends D[0..3] (constant beyond D[3]), that depth scaled by beta
+ * first (Eq. 7, d_eff = beta d: the depth-comparison fix), bilinear over the four texels around the point. */
+double orc_dom_transmittance(const orc_camera* light_cam, const uint32_t* z0, const uint32_t* cnt, const uint32_t D[4],
+                             double alpha_s, double beta, const float p[3]);
+/* O6 then scales light `light`'s contribution by that transmittance (cam == NULL switches it off). The arrays stay
+ * the caller's. beta: per groom, of the frame being shaded (orc_frame_beta). */
+int orc_frame_set_dom(orc_frame*, uint32_t light, const orc_camera* light_cam, const uint32_t* z0, const uint32_t* cnt,
+                      const uint32_t D[4], double alpha_s);
+void orc_frame_set_dom_beta(orc_frame*, const double* beta, uint32_t n);
+
 /* O2: vertices for the current table. fp64 result, and its fp32 rounding. */
 int orc_frame_generate(orc_frame*);
 void orc_frame_get_vertices_f64(const orc_frame*, double* xyz_ao);

@@ -136,6 +136,34 @@ def lights_around(rng, center, scale=1.0):
     return out
 
 
+def light_cameras(sc: dict, res: int = 512):
+    """One square perspective camera per point light of sc["params"], looking from the light at the centre of the
+    scene's cages with the whole scene inside its frustum and depth range (the views deep opacity maps are built
+    from). Geometry only."""
+    lo, hi = np.full(3, np.inf), np.full(3, -np.inf)
+    for g in sc["grooms"]:
+        p = g["pos"].reshape(-1, 3).astype(np.float64)
+        xf = g["xform"] if g["xform"] is not None else np.array([[1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]], np.float64)
+        for M in np.asarray(xf, np.float64).reshape(-1, 3, 4):
+            q = p @ M[:, :3].T + M[:, 3]
+            lo, hi = np.minimum(lo, q.min(0)), np.maximum(hi, q.max(0))
+    c, R = 0.5 * (lo + hi), 0.5 * float(np.linalg.norm(hi - lo)) * 1.05
+    cams = []
+    for pos, _ in sc["params"]["lights"]:
+        e = np.asarray(pos, np.float64)
+        d = float(np.linalg.norm(c - e))
+        f = (c - e) / d
+        up0 = np.array([0.0, 1.0, 0.0]) if abs(f[1]) < 0.9 else np.array([1.0, 0.0, 0.0])
+        r = np.cross(up0, -f)
+        r /= np.linalg.norm(r)
+        u = np.cross(-f, r)
+        cams.append(dict(eye=tuple(float(v) for v in e), right=tuple(float(v) for v in r), up=tuple(float(v) for v in u),
+                         forward=tuple(float(v) for v in f), vfov_y=float(2.0 * math.asin(min(R / d, 0.95)) * 1.05),
+                         near_z=float(max(d - R, 0.05 * d) * 0.98), far_z=float((d + R) * 1.02),
+                         width=int(res), height=int(res)))
+    return cams
+
+
 def default_params(rng, center, scale=1.0, **over):
     p = dict(center_diameter_px=0.5, filter_radius=5, s_par=0.5, s_perp=0.15, sigma_c=0.9,
              tau_z=1.45e-3, tau_fly=5e-4, w_strip=0.5, lights=lights_around(rng, center, scale),
