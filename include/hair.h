@@ -80,6 +80,13 @@ extern "C" {
  * hair_render_to_host(_async), which PCIe bounds. scene_rgb stays float. */
 #define HAIR_FLAG_RGB16F 128u
 
+/* Volumetric shadows (§3.4 "Volumetric shadows are computed using deep-opacity maps ..., which we query
+ * using the depth-correction described in Section 3.2"; DESIGN.md R-dom): the shading of every hair_render* call
+ * scales the contribution of light l by the transmittance towards it, looked up in the deep opacity map that
+ * hair_shadow_build made for that light, at the depth-corrected depth d_eff = beta_g d (Eq. 7) of the groom being
+ * shaded. Lights without a map are unshadowed. */
+#define HAIR_FLAG_SHADOWS 256u
+
 typedef struct hair_ctx hair_ctx; /* opaque; owns all device scratch */
 
 /* Creates a context on `cuda_device` that enqueues on `cuda_stream` (a cudaStream_t; NULL = the
@@ -212,6 +219,38 @@ int hair_render_to_host_async(hair_ctx*, const hair_camera*, uint32_t width, uin
                               int* out_slot);
 /* Blocks until the copies of `slot` (0..HAIR_HOST_SLOTS-1), or of every slot (slot < 0), have finished. */
 int hair_host_wait(hair_ctx*, int slot);
+
+/* Deep opacity maps (Yuksel and Keyser 2008, named by PAPER.md:192; the paper gives no more, DESIGN.md R-dom states
+ * the reading). For each light l < n_lights, from the light's camera cam[l] (eye = the light's position; the caller
+ * frames the scene, e.g. a look-at camera) at res x res:
+ *   z0(u, v)     24-bit depth (the G-buffer's quantisation, R8) of the nearest hair touching light pixel (u, v): the
+ *                conservative layer of a G-buffer rendered from the light, 0xFFFFFFFF where no hair is;
+ *   cnt(u, v, k) number of (segment, pixel) conservative hits of that pixel in layer k behind z0; layer k spans
+ *                [D[k-1], D[k]) depth steps with D[-1] = 0, D[k] = round(layer_d1 * 16777215) * (2^(k+1) - 1) for
+ *                k = 0..2; layer 3 is open-ended and is taken to end at D[3] when looked up.
+ * Built from the FULL grooms (LOD off), as PAPER.md:140 has it ("previously computed depth maps ... recomputing
+ * them is computationally expensive"): this is what makes the depth-comparison fix necessary when a frame thins
+ * the groom. Lookup (in the shading of a frame rendered with HAIR_FLAG_SHADOWS): world point p -> light pixel and
+ * depth dq; per texel d = max(dq - z0, 0), d_eff = beta_g * d (Eq. 7; beta_g = hair_stats_t.beta_groom of the frame
+ * being rendered, taken on the device), fragments in front = the cumulative count, piecewise linear through the
+ * layer ends; bilinear over the four texels around p (texel centres at integer + 1/2; empty texels contribute 0);
+ * transmittance = exp(-alpha_s * fragments in front) (Eq. 6).
+ * The call runs the grooms through LOD (off) -> generate -> clear -> raster -> fragment count once per light on the
+ * context's stream, overwriting the context's vertex buffer and table (render a frame afterwards before using the
+ * debug accessors for it), and keeps 20 bytes per texel and light. Grooms uploaded or updated later need a rebuild. */
+typedef struct {
+  hair_camera cam[HAIR_MAX_LIGHTS];
+  uint32_t n_lights; /* maps to build: lights 0 .. n_lights-1 of the render params in force when frames are shaded */
+  uint32_t res;      /* 16 .. 8192 */
+  float layer_d1;    /* thickness of the first layer in normalised depth of the light's camera, > 0 */
+  float alpha_s;     /* opacity one fragment adds, >= 0 */
+} hair_shadow_params;
+int hair_shadow_build(hair_ctx*, const hair_shadow_params*);
+/* Drops the maps (shading is unshadowed again). */
+int hair_shadow_clear(hair_ctx*);
+/* Parity access: DEVICE pointers to light l's z0 [res][res] uint32 and cnt [res][res][4] uint32, and the four
+ * layer ends. */
+int hair_debug_shadow(hair_ctx*, uint32_t light, const uint32_t** dev_z0, const uint32_t** dev_cnt, uint32_t out_D[4]);
 
 typedef struct {
   uint32_t n_grooms, n_bundles, n_bundles_culled;

@@ -16,12 +16,14 @@ SO_PATH = os.path.join(_HERE, "csrc", "libhair.so")
 
 OP_BITS = {"clump": 1, "twist": 2, "curl": 4, "frizz": 8}
 FLAG_FILTER, FLAG_COUNTERS, FLAG_STAGE_TIMING, FLAG_PAPER_PAYLOAD, FLAG_SINGLE_PASS, FLAG_FUSED, FLAG_TILED, FLAG_RGB16F = 1, 2, 4, 8, 16, 32, 64, 128
+FLAG_SHADOWS = 256
 EMPTY = 0xFFFFFFFFFFFFFFFF
 
 EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_render_params",
            "hair_set_render_params", "hair_mesh_upload", "hair_mesh_update", "hair_mesh_clear",
            "hair_render", "hair_render_scene", "hair_render_sequential", "hair_render_msaa", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
-           "hair_debug_buffers", "hair_debug_set_vertices", "hair_atomic_microbench", "hair_l2_load_microbench", "hair_abi_sizes"]
+           "hair_debug_buffers", "hair_debug_set_vertices", "hair_atomic_microbench", "hair_l2_load_microbench", "hair_abi_sizes",
+           "hair_shadow_build", "hair_shadow_clear", "hair_debug_shadow"]
 
 
 class HairError(RuntimeError):
@@ -50,6 +52,11 @@ class hair_style(C.Structure):
 class hair_camera(C.Structure):
     _fields_ = [("eye", C.c_float * 3), ("right", C.c_float * 3), ("up", C.c_float * 3),
                 ("forward", C.c_float * 3), ("vfov_y", C.c_float), ("near_z", C.c_float), ("far_z", C.c_float)]
+
+
+class hair_shadow_params(C.Structure):
+    _fields_ = [("cam", hair_camera * 4), ("n_lights", C.c_uint32), ("res", C.c_uint32), ("layer_d1", C.c_float),
+                ("alpha_s", C.c_float)]
 
 
 class hair_render_params(C.Structure):
@@ -119,6 +126,9 @@ def load():
     L.hair_debug_set_vertices.argtypes = [vp, vp, u32]
     L.hair_atomic_microbench.argtypes = [vp, C.c_int, vp, C.c_uint64, C.c_uint64, u32, C.POINTER(C.c_float)]
     L.hair_l2_load_microbench.argtypes = [vp, C.c_int, vp, C.c_uint64, u32, u32, C.POINTER(C.c_uint64), C.POINTER(C.c_float)]
+    L.hair_shadow_build.argtypes = [vp, C.POINTER(hair_shadow_params)]
+    L.hair_shadow_clear.argtypes = [vp]
+    L.hair_debug_shadow.argtypes = [vp, u32, C.POINTER(vp), C.POINTER(vp), C.POINTER(u32 * 4)]
     L.hair_abi_sizes.argtypes = [C.POINTER(C.c_uint32 * 6)]
     L.hair_abi_sizes.restype = None
     sizes = (C.c_uint32 * 6)()
@@ -370,6 +380,28 @@ class Hair:
     def debug_set_vertices(self, v):
         v = v.contiguous()
         self._check(self.L.hair_debug_set_vertices(self.h, C.c_void_p(v.data_ptr()), v.shape[0]), "hair_debug_set_vertices")
+
+    def shadow_build(self, light_cams: list, layer_d1: float, alpha_s: float) -> None:
+        """hair_shadow_build: one deep opacity map per camera of `light_cams` (dicts with width == height == res)."""
+        p = hair_shadow_params()
+        p.n_lights, p.res = len(light_cams), int(light_cams[0]["width"])
+        p.layer_d1, p.alpha_s = float(layer_d1), float(alpha_s)
+        for i, lc in enumerate(light_cams):
+            assert lc["width"] == lc["height"] == p.res
+            p.cam[i] = make_camera(lc)
+        self._check(self.L.hair_shadow_build(self.h, C.byref(p)), "hair_shadow_build")
+        self._shadow_res = p.res
+
+    def shadow_clear(self) -> None:
+        self._check(self.L.hair_shadow_clear(self.h), "hair_shadow_clear")
+
+    def debug_shadow(self, light: int):
+        """(z0 [res][res], cnt [res][res][4], D[4]) of light `light`'s map: int32 device tensors (bit patterns of uint32)."""
+        z0, cnt, D = C.c_void_p(), C.c_void_p(), (C.c_uint32 * 4)()
+        self._check(self.L.hair_debug_shadow(self.h, light, C.byref(z0), C.byref(cnt), C.byref(D)), "hair_debug_shadow")
+        r = self._shadow_res
+        return (self._wrap(z0.value, (r, r), self.torch.int32).clone(), self._wrap(cnt.value, (r, r, 4), self.torch.int32).clone(),
+                [int(x) for x in D])
 
     def atomic_microbench(self, mode: int, words, n_ops: int, hot_words: int = 1024) -> float:
         ms = C.c_float(0)

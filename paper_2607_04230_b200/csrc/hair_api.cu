@@ -82,6 +82,15 @@ struct hair_ctx {
   int next_slot = 0;
   cudaEvent_t ev[EV_RING][EV_N] = {};
   uint32_t ev_frames = 0;  // timed frames since the last hair_stats
+  // deep opacity maps (hair_shadow_build): per light z0 + layer counts, the light view's G-buffer (scratch), the
+  // device copy of the lights' cameras and map pointers
+  DomSet dom;  // host mirror
+  DomSet* d_dom = nullptr;
+  uint32_t* d_dom_z0[HAIR_MAX_LIGHTS] = {};
+  uint4* d_dom_cnt[HAIR_MAX_LIGHTS] = {};
+  unsigned long long* d_dom_gbuf = nullptr;
+  size_t dom_px = 0;
+  bool dom_on = false;
   bool timed = false, counted = false, last_two_pass = false, last_tiled = false;
   uint32_t last_w = 0, last_h = 0, launches = 0;
   CamDev last_cam;
@@ -329,6 +338,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   ShadeParams sp = make_shade(c->prm);
   sp.bg_alpha = po.bg_alpha ? 1u : 0u;
   sp.rgb16 = ((c->prm.flags & HAIR_FLAG_RGB16F) && po.final_target) ? 1u : 0u;
+  sp.shadows = ((c->prm.flags & HAIR_FLAG_SHADOWS) && c->dom_on) ? 1u : 0u;
   // R-payload: the paper's word names no groom, so a pass draws exactly one
   const bool pp = (c->prm.flags & HAIR_FLAG_PAPER_PAYLOAD) != 0;
   sp.paper_payload = pp ? 1u : 0u;
@@ -443,11 +453,11 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   mark(EV_RASTER);
   if (po.ms_k) {
     launch_resolve_msaa(c->d_scene, c->d_srec, c->d_vertices, k, sp, gbuf, po.ms_k, (const float4*)scene_rgb,
-                        (float4*)rgb, st);
+                        (float4*)rgb, c->d_dom, c->d_counters, st);
     ++launches;
   }
   if ((stage_mask & 2u) && !po.ms_k) {
-    launch_shade(c->d_scene, c->d_srec, c->d_vertices, k, sp, gbuf, c->d_colour, st);
+    launch_shade(c->d_scene, c->d_srec, c->d_vertices, k, sp, gbuf, c->d_colour, c->d_dom, c->d_counters, st);
     ++launches;
   }
   mark(EV_SHADE);
@@ -532,6 +542,12 @@ void hair_destroy(hair_ctx* c) {
   cudaFree(c->tb.entries);
   cudaFree(c->d_counters);
   cudaFree(c->d_sink);
+  cudaFree(c->d_dom);
+  cudaFree(c->d_dom_gbuf);
+  for (int l = 0; l < HAIR_MAX_LIGHTS; ++l) {
+    cudaFree(c->d_dom_z0[l]);
+    cudaFree(c->d_dom_cnt[l]);
+  }
   if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
   for (int k = 0; k < HAIR_HOST_SLOTS; ++k) {
     cudaFree(c->d_own_gbuf[k]);
@@ -735,6 +751,7 @@ int hair_mesh_clear(hair_ctx* c) {
   if (c->h_want) *c->h_want = 0u;
   c->last_two_pass = false;
   c->scene_dirty = true;
+  c->dom_on = false;  // the maps were built from the grooms just removed
   return HAIR_OK;
 }
 
@@ -863,6 +880,90 @@ int hair_render_to_host(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_
   rc = hair_host_wait(c, slot);
   if (rc) return rc;
   CK(cudaStreamSynchronize(c->stream));
+  return HAIR_OK;
+}
+
+// PAPER.md:192 / DESIGN.md R-dom: one light view per light through LOD (off) -> generate -> clear -> raster (the
+// conservative layer is z0), then the same segments once more, every conservative hit counted into its layer
+int hair_shadow_build(hair_ctx* c, const hair_shadow_params* p) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  if (!p || p->n_lights == 0 || p->n_lights > HAIR_MAX_LIGHTS || p->res < 16 || p->res > 8192 || !(p->layer_d1 > 0.f) ||
+      !(p->alpha_s >= 0.f))
+    return fail(c, HAIR_E_INVALID_ARG, "hair_shadow_build: bad parameters");
+  if (!c->scene.n_bi) return fail(c, HAIR_E_INVALID_ARG, "hair_shadow_build: no groom uploaded");
+  CK(cudaSetDevice(c->device));
+  const uint32_t S = p->res;
+  const size_t px = (size_t)S * S;
+  if (px != c->dom_px) {
+    for (int l = 0; l < HAIR_MAX_LIGHTS; ++l) {
+      cudaFree(c->d_dom_z0[l]);
+      cudaFree(c->d_dom_cnt[l]);
+      c->d_dom_z0[l] = nullptr;
+      c->d_dom_cnt[l] = nullptr;
+    }
+    cudaFree(c->d_dom_gbuf);
+    c->d_dom_gbuf = nullptr;
+    c->dom_px = 0;
+    CK(cudaMalloc((void**)&c->d_dom_gbuf, px * 2 * sizeof(unsigned long long)));
+    c->dom_px = px;
+  }
+  if (!c->d_dom) CK(cudaMalloc((void**)&c->d_dom, sizeof(DomSet)));
+  c->dom_on = false;
+  memset(&c->dom, 0, sizeof(c->dom));
+  const double d1 = std::floor((double)p->layer_d1 * 16777215.0 + 0.5);
+  const uint32_t D1 = (uint32_t)std::fmin(std::fmax(d1, 1.0), 1000000.0);
+  const hair_render_params saved = c->prm;
+  c->prm.flags = HAIR_FLAG_SINGLE_PASS;  // plain strand-id words, one raster pass, no timing
+  c->prm.groom_mask = 0xFFFFFFFFu;
+  int rc = HAIR_OK;
+  for (uint32_t l = 0; l < p->n_lights && rc == HAIR_OK; ++l) {
+    if (!c->d_dom_z0[l]) {
+      if (cudaMalloc((void**)&c->d_dom_z0[l], px * sizeof(uint32_t)) != cudaSuccess ||
+          cudaMalloc((void**)&c->d_dom_cnt[l], px * sizeof(uint4)) != cudaSuccess) {
+        rc = fail(c, HAIR_E_OUT_OF_MEMORY, "hair_shadow_build: out of device memory");
+        break;
+      }
+    }
+    const float lam0 = 0.f;  // the maps are built from the full groom
+    rc = render_impl(c, &p->cam[l], S, S, &lam0, 1, 1u, true, c->d_dom_gbuf, (float*)c->d_dom_gbuf);
+    if (rc) break;
+    DomLight& L = c->dom.l[l];
+    L.cam = c->last_cam;
+    L.z0 = c->d_dom_z0[l];
+    L.cnt = c->d_dom_cnt[l];
+    L.D[0] = D1, L.D[1] = 3u * D1, L.D[2] = 7u * D1, L.D[3] = 15u * D1;
+    L.alpha_s = p->alpha_s;
+    L.on = 1u;
+    cudaMemsetAsync(c->d_dom_cnt[l], 0, px * sizeof(uint4), c->stream);
+    cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER, 0, sizeof(unsigned long long), c->stream);
+    launch_raster_dom(c->d_scene, c->scene.n_bi, c->d_table, c->d_grp, c->d_vertices, L.cam, 0.5f * c->prm.center_diameter_px,
+                      c->d_dom_gbuf, c->d_counters, reinterpret_cast<uint32_t*>(c->d_dom_cnt[l]),
+                      make_uint3(L.D[0], L.D[1], L.D[2]), c->n_sm, &c->ls, c->stream);
+    launch_dom_z0(c->d_dom_gbuf, px, c->d_dom_z0[l], c->stream);
+  }
+  c->prm = saved;
+  if (rc) return rc;
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(c->d_dom, &c->dom, sizeof(DomSet), cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));  // the host mirror may change after return
+  c->dom_on = true;
+  return HAIR_OK;
+}
+
+int hair_shadow_clear(hair_ctx* c) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  c->dom_on = false;
+  return HAIR_OK;
+}
+
+int hair_debug_shadow(hair_ctx* c, uint32_t light, const uint32_t** dev_z0, const uint32_t** dev_cnt, uint32_t out_D[4]) {
+  if (!c) return HAIR_E_INVALID_ARG;
+  if (!c->dom_on || light >= HAIR_MAX_LIGHTS || !c->dom.l[light].on)
+    return fail(c, HAIR_E_INVALID_ARG, "hair_debug_shadow: no map for this light");
+  if (dev_z0) *dev_z0 = c->d_dom_z0[light];
+  if (dev_cnt) *dev_cnt = reinterpret_cast<const uint32_t*>(c->d_dom_cnt[light]);
+  if (out_D)
+    for (int i = 0; i < 4; ++i) out_D[i] = c->dom.l[light].D[i];
   return HAIR_OK;
 }
 

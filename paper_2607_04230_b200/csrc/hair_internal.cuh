@@ -77,6 +77,20 @@ struct ShadeParams {
   uint32_t paper_payload;  // R-payload: words carry the paper's payload; pp_groom = the one groom of the pass
   uint32_t pp_groom;
   uint32_t rgb16;  // HAIR_FLAG_RGB16F: the colour output of this pass is half RGBA (8 bytes per pixel)
+  uint32_t shadows;  // HAIR_FLAG_SHADOWS and maps exist: lights are scaled by the deep-opacity transmittance
+};
+
+// deep opacity maps of the point lights (DESIGN.md R-dom), one per light, in device memory
+struct DomLight {
+  CamDev cam;
+  const uint32_t* z0;  // [res][res] depth of the conservative layer seen from the light, 0xFFFFFFFF = no hair
+  const uint4* cnt;    // [res][res] fragments per layer
+  uint32_t D[4];       // layer ends in depth steps behind z0
+  float alpha_s;
+  uint32_t on;
+};
+struct DomSet {
+  DomLight l[HAIR_MAX_LIGHTS];
 };
 
 // device counters, one block of 64-bit words (index = enum)
@@ -242,8 +256,8 @@ inline void raise_dyn_smem(F func, size_t bytes) {
 // per-context launch state: cudaFuncSetAttribute (dynamic shared memory opt-in) and the occupancy it implies are per
 // DEVICE, and a context is bound to one device, so what has been configured lives in hair_ctx — no function statics
 struct LaunchState {
-  int raster_per_sm[32] = {};      // index = COUNT | MS << 1 | PP << 2 | HZ << 3 | FUSED << 4
-  size_t raster_smem[32] = {};
+  int raster_per_sm[64] = {};      // index = COUNT | MS << 1 | PP << 2 | HZ << 3 | FUSED << 4 | DOM << 5
+  size_t raster_smem[64] = {};
   int gen_per_sm = 0;
   size_t gen_smem = 0;
   bool filter_set[8] = {};
@@ -276,6 +290,13 @@ void launch_raster(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, c
                    const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
                    unsigned long long* counters, bool count, uint32_t ms_k, bool paper_payload, int pass,
                    const uint32_t* hiz, int n_sm, LaunchState* ls, cudaStream_t st, uint32_t fused_c_max = 0);
+// deep opacity map, second step: every conservative hit of the frame's segments under `cam` adds one fragment to the
+// layer of its pixel it falls in behind the conservative depth already in gbuf (dom_D: ends of layers 0..2)
+void launch_raster_dom(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
+                       const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
+                       unsigned long long* counters, uint32_t* dom_cnt, uint3 dom_D, int n_sm, LaunchState* ls,
+                       cudaStream_t st);
+void launch_dom_z0(const unsigned long long* gbuf, size_t n_pixels, uint32_t* z0, cudaStream_t st);
 void launch_bin(bool scatter, const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
                 const float4* vertices, CamDev cam, float rho_default, unsigned long long* counters, int pass,
                 TileBufs tb, int n_sm, cudaStream_t st);
@@ -284,9 +305,10 @@ void launch_raster_tiled(CamDev cam, unsigned long long* gbuf, const float* scen
                          unsigned long long* counters, TileBufs tb, int n_sm, LaunchState* ls, cudaStream_t st);
 void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
-                         float4* out, cudaStream_t st);
+                         float4* out, const DomSet* dom, const unsigned long long* counters, cudaStream_t st);
 void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
-                  ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st);
+                  ShadeParams sp, const unsigned long long* gbuf, float4* colour, const DomSet* dom,
+                  const unsigned long long* counters, cudaStream_t st);
 int launch_filter(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                    ShadeParams sp, const unsigned long long* gbuf, const float4* colour, const float4* scene_rgb,
                    float4* out, unsigned long long* counters, bool count, LaunchState* ls, cudaStream_t st);

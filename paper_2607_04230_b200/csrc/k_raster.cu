@@ -64,13 +64,18 @@ __constant__ int c_ms_off[4][8][2] = {  // sample offsets from the pixel centre 
 // per-bundle spline table of its work group in shared memory (gen::build_table, the code k_generate runs) and every
 // lane GENERATES the vertex it would have loaded (gen::vertex: same source, same bits). Needs the paper payload (the
 // strand-id word is shaded from the vertex buffer). An A/B against the materialised pipeline.
-template <bool COUNT, bool MS, bool PP, bool HZ, bool FUSED = false>
+// DOM (deep opacity maps; DESIGN.md R-dom): the frame is a light's view and gbuf already holds its
+// resolved G-buffer; every conservative hit adds one fragment to the layer of its pixel it falls in behind the
+// pixel's conservative depth (integer compare of 24-bit depths, one RED.ADD.32); nothing is written to gbuf.
+template <bool COUNT, bool MS, bool PP, bool HZ, bool FUSED = false, bool DOM = false>
 __global__ void __launch_bounds__(RAS_WARPS * 32, FUSED ? 2 : (PP ? 4 : RAS_MIN_BLOCKS))  // payload: 64 registers, no spills
 k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict__ table,
          const uint32_t* __restrict__ grp, const float4* __restrict__ vertices, CamDev cam, float rho_default,
          unsigned long long* __restrict__ gbuf, unsigned long long* __restrict__ counters, uint32_t ms_k,
-         uint32_t queue, const uint32_t* __restrict__ hiz, uint32_t c_max) {
+         uint32_t queue, const uint32_t* __restrict__ hiz, uint32_t c_max, uint32_t* __restrict__ dom_cnt = nullptr,
+         uint3 dom_D = make_uint3(0u, 0u, 0u)) {
   static_assert(!FUSED || (PP && !COUNT && !MS), "the fused raster writes the paper payload only");
+  static_assert(!DOM || (!COUNT && !MS && !PP && !HZ && !FUSED), "the fragment count is a pass of its own");
   constexpr int RS = PP ? REC_STRIDE_PP : REC_STRIDE;
   __shared__ __align__(16) float s_rec[RAS_WARPS][32][RS];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -332,7 +337,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
             if (!ok[i]) continue;
             // early reject: centre word >= conservative word (R10), so a segment that lies entirely behind
             // the pixel's centre hit loses both layers whatever its exact depth at this pixel
-            if (!COUNT && dq_min > (uint32_t)(cur[i].x >> 40)) continue;
+            if (!COUNT && !DOM && dq_min > (uint32_t)(cur[i].x >> 40)) continue;
             const int r = rb + i;
             const float cN = (float)r + 0.5f;
             const float uN = xsub(cN, aN);
@@ -341,6 +346,13 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
             const float zn = xadd(az, xmul(tt, dz));
             if (zn < 0.f || zn > 1.f) continue;
             const float eM = xsub(cM, xadd(aM, xmul(tt, dM))), eN = xsub(cN, xadd(aN, xmul(tt, dN)));
+            if (DOM) {  // fragment of the deep opacity map: layer by its depth behind the nearest hair of the pixel
+              const uint32_t d = quant_depth(zn) - (uint32_t)(cur[i].y >> 40);
+              const uint32_t layer = (d >= dom_D.x ? 1u : 0u) + (d >= dom_D.y ? 1u : 0u) + (d >= dom_D.z ? 1u : 0u);
+              const size_t pix = ymajor ? (size_t)c * W + (rb + i) : (size_t)(rb + i) * W + c;
+              atomicAdd(dom_cnt + pix * 4 + layer, 1u);
+              continue;
+            }
             const bool centre = xadd(xmul(eM, eM), xmul(eN, eN)) <= rec[s][17];
             unsigned long long word;
             if (PP) {
@@ -492,6 +504,34 @@ static void launch_raster_t(const SceneDev* d_scene, uint32_t n_bi, const uint4*
   const int per_sm = ls->raster_per_sm[V];
   k_raster<COUNT, MS, PP, HZ, FUSED><<<(uint32_t)(n_sm * per_sm), RAS_WARPS * 32, smem, st>>>(
       d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, ms_k, queue, hiz, c_max);
+}
+
+void launch_raster_dom(const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
+                       const float4* vertices, CamDev cam, float rho_default, unsigned long long* gbuf,
+                       unsigned long long* counters, uint32_t* dom_cnt, uint3 dom_D, int n_sm, LaunchState* ls,
+                       cudaStream_t st) {
+  constexpr int V = 32;
+  if (!ls->raster_per_sm[V]) {
+    int b = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_raster<false, false, false, false, false, true>, RAS_WARPS * 32, 0);
+    ls->raster_per_sm[V] = b > 0 ? b : 1;
+  }
+  k_raster<false, false, false, false, false, true><<<(uint32_t)(n_sm * ls->raster_per_sm[V]), RAS_WARPS * 32, 0, st>>>(
+      d_scene, n_bi, table, grp, vertices, cam, rho_default, gbuf, counters, 0, CNT_WORK_RASTER, nullptr, 0, dom_cnt, dom_D);
+}
+
+// z0 of a deep opacity map: the conservative layer's 24-bit depth, 0xFFFFFFFF where the pixel holds no hair
+__global__ void __launch_bounds__(256) k_dom_z0(const uint4* __restrict__ g, size_t n, uint32_t* __restrict__ z0) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const uint4 v = __ldg(&g[i]);
+    z0[i] = w_none(v.z, v.w) ? 0xFFFFFFFFu : v.w >> 8;
+  }
+}
+void launch_dom_z0(const unsigned long long* gbuf, size_t n_pixels, uint32_t* z0, cudaStream_t st) {
+  size_t blocks = (n_pixels + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  k_dom_z0<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<const uint4*>(gbuf), n_pixels, z0);
 }
 
 // ms_k = 0: the two-layer G-buffer; ms_k in {1, 2, 4, 8}: gbuf = [ms_k][H][W] sample layers (reference mode).

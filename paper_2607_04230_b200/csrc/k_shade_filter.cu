@@ -67,9 +67,52 @@ __device__ __forceinline__ float fast_asin(float x) {
   return copysignf(r, x);
 }
 
+// Volumetric shadow (DESIGN.md R-dom): transmittance towards one light from its deep opacity map at
+// world point pos, the depth behind each texel's nearest hair scaled by beta first (Eq. 7, the depth-comparison fix
+// of PAPER.md:138-152). Fragments in front = the cumulative layer count, piecewise linear through the layer ends;
+// bilinear over the four texels around the point. The projection and the depth quantisation are R-proj / R8 (the
+// same integers as the oracle's); the blend is ordinary fp32.
+__device__ __forceinline__ float dom_texel_omega(uint4 c, const uint32_t* D, float d) {
+  const float D0 = (float)D[0], D1 = (float)D[1], D2 = (float)D[2], D3 = (float)D[3];
+  const float c0 = (float)c.x, c1 = (float)c.y, c2 = (float)c.z, c3 = (float)c.w;
+  if (d < D0) return c0 * d / D0;
+  if (d < D1) return c0 + c1 * (d - D0) / (D1 - D0);
+  if (d < D2) return (c0 + c1) + c2 * (d - D1) / (D2 - D1);
+  if (d < D3) return (c0 + c1 + c2) + c3 * (d - D2) / (D3 - D2);
+  return c0 + c1 + c2 + c3;
+}
+__device__ __forceinline__ float dom_transmittance(const DomLight& L, F3 pos, float beta) {
+  const Proj q = project_exact(L.cam, pos.x, pos.y, pos.z);
+  if (!q.valid) return 1.f;
+  const uint32_t dq = quant_depth(fminf(fmaxf(q.zn, 0.f), 1.f));
+  const float fx = q.sx - 0.5f, fy = q.sy - 0.5f;
+  const float x0 = floorf(fx), y0 = floorf(fy);
+  const float wx = fx - x0, wy = fy - y0;
+  const int W = (int)L.cam.W, H = (int)L.cam.H;
+  float omega = 0.f;
+#pragma unroll
+  for (int dy = 0; dy < 2; ++dy)
+#pragma unroll
+    for (int dx = 0; dx < 2; ++dx) {
+      const int xi = (int)x0 + dx, yi = (int)y0 + dy;
+      if (xi < 0 || yi < 0 || xi >= W || yi >= H) continue;
+      const size_t t = (size_t)yi * W + xi;
+      const uint32_t z0 = __ldg(&L.z0[t]);
+      if (z0 == 0xFFFFFFFFu || dq <= z0) continue;
+      const float w = (dx ? wx : 1.f - wx) * (dy ? wy : 1.f - wy);
+      omega += w * dom_texel_omega(__ldg(&L.cnt[t]), L.D, beta * (float)(dq - z0));
+    }
+  return __expf(-L.alpha_s * omega);
+}
+// beta of Eq. 7 for groom g of the frame being shaded, from the sums k_scan took on the device (R-beta)
+__device__ __forceinline__ float groom_beta(const unsigned long long* __restrict__ counters, uint32_t g) {
+  const unsigned long long num = __ldg(&counters[CNT_BETA_NUM + g]), den = __ldg(&counters[CNT_BETA_DEN + g]);
+  return den ? (float)num / (float)den : 1.f;
+}
+
 // the stand-in shading model (R23) at one point: position, unit tangent, strand parameter w, AO
 __device__ __forceinline__ F3 shade_model(const GroomDev& g, const CamDev& cam, const ShadeParams& sp, F3 pos, F3 T,
-                                          float w, float ao) {
+                                          float w, float ao, const DomSet* __restrict__ dom, float beta_lod) {
   const F3 alb = (1.f - w) * f3(g.albedo_root[0], g.albedo_root[1], g.albedo_root[2]) +
                  w * f3(g.albedo_tip[0], g.albedo_tip[1], g.albedo_tip[2]);
   const F3 V = normalize(f3(cam.eye[0], cam.eye[1], cam.eye[2]) - pos);
@@ -88,7 +131,8 @@ __device__ __forceinline__ F3 shade_model(const GroomDev& g, const CamDev& cam, 
     const float th = 0.5f * (fast_asin(sin_i) + asin_o);
     const float a = th + tilt, b = th - 1.5f * tilt;
     const float MR = __expf(-a * a * inv2b2), MT = __expf(-b * b * 0.25f * inv2b2);
-    const float s = cos_i * inv_d2;
+    float s = cos_i * inv_d2;
+    if (dom && dom->l[li].on) s *= dom_transmittance(dom->l[li], pos, beta_lod);
     rgb.x += sp.light_rgb[li][0] * s * (sp.k_d * alb.x + sp.k_R * MR + sp.k_TRT * MT * alb.x);
     rgb.y += sp.light_rgb[li][1] * s * (sp.k_d * alb.y + sp.k_R * MR + sp.k_TRT * MT * alb.y);
     rgb.z += sp.light_rgb[li][2] * s * (sp.k_d * alb.z + sp.k_R * MR + sp.k_TRT * MT * alb.z);
@@ -99,7 +143,8 @@ __device__ __forceinline__ F3 shade_model(const GroomDev& g, const CamDev& cam, 
 // O6 for one word: linear RGB of the hit it names
 __device__ __forceinline__ F3 shade_word(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec,
                                          const float4* __restrict__ vertices, const CamDev& cam, const ShadeParams& sp,
-                                         unsigned long long G) {
+                                         unsigned long long G, const DomSet* __restrict__ dom,
+                                         const unsigned long long* __restrict__ counters) {
   const Loc l = locate_strand(srec, w_sid(G));
   const GroomDev& g = sc->g[l.groom];
   const int j = (int)w_j(G), C = (int)l.C;
@@ -113,13 +158,14 @@ __device__ __forceinline__ F3 shade_word(const SceneDev* __restrict__ sc, const 
   const F3 Tj1 = calc_tangent(j + 1, C, f3(v1), f3(v2), f3(v3));
   const F3 T = normalize((1.f - t) * Tj + t * Tj1);
   const float w = ((float)j + t) / (float)(C - 1);
-  return shade_model(g, cam, sp, pos, T, w, ao);
+  return shade_model(g, cam, sp, pos, T, w, ao, dom, dom ? groom_beta(counters, l.groom) : 1.f);
 }
 
 // R-payload: O6 from the paper's payload alone, no vertex read. Position = the point of the
 // ray through the pixel centre at the word's depth ("reconstruct it from the depth value")
 __device__ __forceinline__ F3 shade_payload(const SceneDev* __restrict__ sc, const CamDev& cam, const ShadeParams& sp,
-                                            int x, int y, unsigned long long G) {
+                                            int x, int y, unsigned long long G, const DomSet* __restrict__ dom,
+                                            const unsigned long long* __restrict__ counters) {
   const X3 t = oct_decode_x(pw_ox(G), pw_oy(G));
   const float w = (float)((uint32_t)(G >> 6) & 63u) * (1.0f / 63.0f), ao = (float)((uint32_t)G & 63u) * (1.0f / 63.0f);
   const float zn = (float)w_dq(G) / 16777215.0f;
@@ -128,32 +174,35 @@ __device__ __forceinline__ F3 shade_payload(const SceneDev* __restrict__ sc, con
   const F3 pos = f3(cam.eye[0] + zv * (cx * cam.r[0] + cy * cam.u[0] + cam.f[0]),
                     cam.eye[1] + zv * (cx * cam.r[1] + cy * cam.u[1] + cam.f[1]),
                     cam.eye[2] + zv * (cx * cam.r[2] + cy * cam.u[2] + cam.f[2]));
-  return shade_model(sc->g[sp.pp_groom], cam, sp, pos, f3(t.x, t.y, t.z), w, ao);
+  return shade_model(sc->g[sp.pp_groom], cam, sp, pos, f3(t.x, t.y, t.z), w, ao, dom,
+                     dom ? groom_beta(counters, sp.pp_groom) : 1.f);
 }
 
 __global__ void __launch_bounds__(256)
 k_shade(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
-        CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, float4* __restrict__ colour) {
+        CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, float4* __restrict__ colour,
+        const DomSet* __restrict__ dom, const unsigned long long* __restrict__ counters) {
   const size_t n_px = (size_t)cam.W * cam.H;
   const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n_px) return;
   const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
   const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
   if (w_none(G)) return;  // colour is only ever read where a centre hit exists
-  const F3 rgb = shade_word(sc, srec, vertices, cam, sp, G);
+  const F3 rgb = shade_word(sc, srec, vertices, cam, sp, G, dom, counters);
   colour[p] = make_float4(rgb.x, rgb.y, rgb.z, 1.0f);
 }
 
 __global__ void __launch_bounds__(256)
 k_shade_payload(const SceneDev* __restrict__ sc, CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf,
-                float4* __restrict__ colour) {
+                float4* __restrict__ colour, const DomSet* __restrict__ dom,
+                const unsigned long long* __restrict__ counters) {
   const uint32_t x = blockIdx.x * 64u + (threadIdx.x & 63u), y = blockIdx.y * 4u + (threadIdx.x >> 6);
   if (x >= cam.W || y >= cam.H) return;
   const size_t p = (size_t)y * cam.W + x;
   const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
   const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
   if (w_none(G)) return;
-  const F3 rgb = shade_payload(sc, cam, sp, (int)x, (int)y, G);
+  const F3 rgb = shade_payload(sc, cam, sp, (int)x, (int)y, G, dom, counters);
   colour[p] = make_float4(rgb.x, rgb.y, rgb.z, 1.0f);
 }
 
@@ -161,7 +210,8 @@ k_shade_payload(const SceneDev* __restrict__ sc, CamDev cam, ShadeParams sp, con
 __global__ void __launch_bounds__(256)
 k_resolve_msaa(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
                CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ samples, uint32_t ms_k,
-               const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
+               const float4* __restrict__ scene_rgb, float4* __restrict__ out, const DomSet* __restrict__ dom,
+               const unsigned long long* __restrict__ counters) {
   const size_t n_px = (size_t)cam.W * cam.H;
   const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n_px) return;
@@ -170,7 +220,7 @@ k_resolve_msaa(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, 
   for (uint32_t s = 0; s < ms_k; ++s) {
     const unsigned long long w = __ldg(&samples[(size_t)s * n_px + p]);
     if (w_none(w)) continue;
-    acc = acc + shade_word(sc, srec, vertices, cam, sp, w);
+    acc = acc + shade_word(sc, srec, vertices, cam, sp, w, dom, counters);
     ++n_hit;
   }
   F3 bg = f3(sp.background[0], sp.background[1], sp.background[2]);
@@ -182,9 +232,10 @@ k_resolve_msaa(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, 
 
 void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
-                         float4* out, cudaStream_t st) {
+                         float4* out, const DomSet* dom, const unsigned long long* counters, cudaStream_t st) {
   const size_t n = (size_t)cam.W * cam.H;
-  k_resolve_msaa<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, samples, ms_k, scene_rgb, out);
+  k_resolve_msaa<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, samples, ms_k, scene_rgb, out,
+                                                               sp.shadows ? dom : nullptr, counters);
 }
 
 // R22: unit screen direction of the segment a word names; fixed-order fp32 (decides strip membership)
@@ -669,13 +720,15 @@ k_count_pixels(const unsigned long long* __restrict__ gbuf, size_t n_px, unsigne
 }
 
 void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
-                  ShadeParams sp, const unsigned long long* gbuf, float4* colour, cudaStream_t st) {
+                  ShadeParams sp, const unsigned long long* gbuf, float4* colour, const DomSet* dom,
+                  const unsigned long long* counters, cudaStream_t st) {
   size_t n = (size_t)cam.W * cam.H;
+  if (!sp.shadows) dom = nullptr;
   if (sp.paper_payload) {
-    k_shade_payload<<<dim3((cam.W + 63) / 64, (cam.H + 3) / 4), 256, 0, st>>>(d_scene, cam, sp, gbuf, colour);
+    k_shade_payload<<<dim3((cam.W + 63) / 64, (cam.H + 3) / 4), 256, 0, st>>>(d_scene, cam, sp, gbuf, colour, dom, counters);
     return;
   }
-  k_shade<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour);
+  k_shade<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour, dom, counters);
 }
 
 template <int R>

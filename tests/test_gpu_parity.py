@@ -1134,3 +1134,88 @@ def test_atomic_microbench_runs(hair_mod):
         ms = h.atomic_microbench(mode, words, 1 << 22, 1024)
         assert ms > 0
     assert (words != -1).any()
+
+
+@pytest.mark.parametrize("idx,scale,res_scale,res,d1,alpha", [
+    (1, 1.0, 1.0, 256, 2e-4, 0.06),    # config 1 as named, LOD off: beta = 1
+    (4, 0.03, 0.25, 384, 1e-4, 0.04),  # five grooms under LOD: per-groom beta < 1 in the lookup (Eq. 7), xforms, 3 lights
+    (2, 0.1, 0.5, 320, 2e-4, 0.03),    # curl + frizz + width_world (the light views take the projected-width radius)
+])
+def test_deep_opacity_maps_and_shadowed_shading(orc, hair_mod, idx, scale, res_scale, res, d1, alpha):
+    """PAPER.md:192 / DESIGN.md R-dom, stage-wise: (i) the maps hair_shadow_build makes — z0 and the four layer counts
+    of every light — against the oracle's on the library's own full-groom vertex buffer, bit for bit; (ii) a frame
+    shaded with HAIR_FLAG_SHADOWS against the oracle's shade + filter on the same G-buffer with the same maps and
+    its own beta per groom, at north_star's RGB tolerance; (iii) shadows only darken, and do darken."""
+    import torch
+    sc = synth.config(idx, scale=scale, res_scale=res_scale)
+    cam, prm = sc["camera"], sc["params"]
+    lcams = synth.light_cameras(sc, res)
+    h = hair_mod.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(prm)
+    h.shadow_build(lcams, d1, alpha)
+    torch.cuda.synchronize()
+    # the context's vertex buffer now holds the full grooms as drawn for the last light: feed the oracle with it
+    full = orc.Frame(sc["grooms"])
+    full.lod(lcams[-1], [0.0])
+    assert h.stats()["n_vertices"] == full.n_vertices and h.stats()["n_strands_lod"] == full.n_strands
+    verts_full = h.debug_vertices().cpu().numpy()
+    full.generate()
+    assert float(np.abs(verts_full.astype(np.float64) - full.vertices_f64()).max()) <= TOL_VERTEX
+    full.set_vertices_f32(verts_full)
+    maps = []
+    for l, lc in enumerate(lcams):
+        z0_g, cnt_g, D = h.debug_shadow(l)
+        z0_g, cnt_g = z0_g.cpu().numpy().view(np.uint32), cnt_g.cpu().numpy().view(np.uint32)
+        assert D == [D[0], 3 * D[0], 7 * D[0], 15 * D[0]] and D[0] == int(math.floor(d1 * 16777215.0 + 0.5))
+        z0_o, cnt_o = full.dom_build(lc, prm, D[:3])
+        assert np.array_equal(z0_g, z0_o), f"light {l}: z0 differs on {(z0_g != z0_o).sum()} texels"
+        assert np.array_equal(cnt_g, cnt_o), f"light {l}: layer counts differ on {(cnt_g != cnt_o).any(-1).sum()} texels"
+        assert (z0_o != 0xFFFFFFFF).sum() > 200 and cnt_o[..., 1:].sum() > 0
+        maps.append((z0_o, cnt_o, D))
+    # (ii) a frame with and without shadows
+    G0 = {}
+    for name, flags in (("plain", 0), ("shadow", hair_mod.FLAG_SHADOWS)):
+        h.set_render_params(prm, flags=flags)
+        gb, rgb = h.render(cam, sc["lam"])
+        torch.cuda.synchronize()
+        G0[name] = (hair_mod.gbuffer_to_numpy(gb), rgb.cpu().numpy().astype(np.float64))
+    assert np.array_equal(G0["plain"][0], G0["shadow"][0])
+    verts = h.debug_vertices().cpu().numpy()
+    table = h.debug_table().cpu().numpy().view(np.uint32)
+    st = h.stats()
+    f = orc.Frame(sc["grooms"])
+    f.lod(cam, sc["lam"])
+    assert np.array_equal(f.table()[0], table)
+    beta, _, _ = f.beta()
+    assert np.array_equal(np.float32(beta), np.float32(st["beta_groom"][:len(beta)]))
+    if idx == 4:
+        assert (beta < 0.9).any()  # the far grooms are thinned: the depth-comparison fix is exercised
+    f.generate()
+    f.set_vertices_f32(verts)
+    f.set_gbuffer(G0["shadow"][0])
+    for l, (lc, (z0_o, cnt_o, D)) in enumerate(zip(lcams, maps)):
+        f.set_dom(l, lc, z0_o, cnt_o, D, alpha)
+    f.set_dom_beta(beta)
+    f.shade(cam, prm)
+    out = f.filter(cam, prm)
+    err = float(np.abs(out - G0["shadow"][1]).max())
+    peak = max(float(out[..., :3].max()), 1.0)
+    assert err <= TOL_RGB, f"shadowed rgb max-abs {err}"
+    assert psnr(out[..., :3], G0["shadow"][1][..., :3], peak) > MIN_PSNR
+    # the same maps looked up WITHOUT the fix (beta = 1) must differ where grooms are thinned: the fix is not a no-op
+    if idx == 4:
+        f.set_dom_beta(np.ones_like(beta))
+        f.shade(cam, prm)
+        naive = f.filter(cam, prm)
+        assert float(np.abs(naive - out).max()) > 5 * TOL_RGB
+        assert (naive[..., :3].sum() < out[..., :3].sum())  # PAPER.md:140: without it the thinned groom is too dark
+    # (iii) shadows only darken
+    hit = (G0["plain"][0][..., 0] & np.uint64(0xFFFFFFFFFF)) != np.uint64(0xFFFFFFFFFF)
+    assert hit.sum() > 500
+    assert G0["shadow"][1][..., :3].sum() < 0.98 * G0["plain"][1][..., :3].sum()
+    # unshadowed again after hair_shadow_clear, and for lights without a map
+    h.shadow_clear()
+    _, rgb = h.render(cam, sc["lam"])
+    assert np.array_equal(rgb.cpu().numpy().astype(np.float64), G0["plain"][1])
