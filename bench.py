@@ -279,6 +279,31 @@ def run_cuda(args):
     barrier()
     ms_seq = e0.elapsed_time(e1) / 10
 
+    # ---- SURVEY 8f NEXT-4 (last part): deep-opacity shadows, same scene, untimed leg: the maps of the
+    # three lights at 1024^2 from the full grooms (483 k strands, LOD off), then frames shaded with HAIR_FLAG_SHADOWS
+    lcams = synth.light_cameras(sc, 1024)
+    h.shadow_build(lcams, 1e-4, 0.03)  # warm (allocations)
+    barrier()
+    e0.record()
+    h.shadow_build(lcams, 1e-4, 0.03)
+    e1.record()
+    barrier()
+    ms_dom_build = e0.elapsed_time(e1)
+    h.set_render_params(sc["params"], flags=binding.FLAG_SHADOWS | binding.FLAG_STAGE_TIMING)
+    for _ in range(3):
+        h.render(cam, lam, gb, rgb)
+    h.stats()
+    barrier()
+    e0.record()
+    for _ in range(20):
+        h.render(cam, lam, gb, rgb)
+    e1.record()
+    barrier()
+    ms_dom_frame = e0.elapsed_time(e1) / 20
+    st_dom = h.stats()
+    h.shadow_clear()
+    h.set_render_params(sc["params"], flags=0)
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -403,6 +428,10 @@ def run_cuda(args):
                           "what": "production frames: bundles in the front 60 % of their groom's depth range first, 16x16-tile "
                                   "hi-Z (k_hiz), then the rest; a segment behind every tile of its bounding box is dropped "
                                   "before any pixel work (same G-buffer bit for bit; DESIGN.md 7.3)"},
+        "shadows": {"build_ms": ms_dom_build, "lights": len(lcams), "res": 1024, "ms_per_step": ms_dom_frame,
+                    "ms_shade": st_dom["ms_shade"],
+                    "what": "hair_shadow_build: deep opacity maps of the point lights from the full grooms (LOD off); then the "
+                            "bench frame with HAIR_FLAG_SHADOWS (PAPER.md:192, Eq. 7 lookup with the frame's beta per groom)"},
         "moving_camera": {"ms_per_step": ms_moving, "frames": k_mov, "ms_raster": st_mov["ms_raster"],
                           "ms_filter": st_mov["ms_filter"], "n_segments_hiz_culled_last_frame": st_mov["n_segments_hiz_culled"],
                           "what": "synth.moving_camera: yaw +-0.04 rad, sideways swing and dolly, a new camera every frame"},

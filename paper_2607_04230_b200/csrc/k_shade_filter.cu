@@ -178,6 +178,7 @@ __device__ __forceinline__ F3 shade_payload(const SceneDev* __restrict__ sc, con
                      dom ? groom_beta(counters, sp.pp_groom) : 1.f);
 }
 
+template <bool SH>  // SH: deep-opacity shadows on (a kernel of its own: the plain one keeps its 31 registers)
 __global__ void __launch_bounds__(256)
 k_shade(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
         CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, float4* __restrict__ colour,
@@ -188,10 +189,11 @@ k_shade(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const f
   const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
   const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
   if (w_none(G)) return;  // colour is only ever read where a centre hit exists
-  const F3 rgb = shade_word(sc, srec, vertices, cam, sp, G, dom, counters);
+  const F3 rgb = shade_word(sc, srec, vertices, cam, sp, G, SH ? dom : nullptr, counters);
   colour[p] = make_float4(rgb.x, rgb.y, rgb.z, 1.0f);
 }
 
+template <bool SH>
 __global__ void __launch_bounds__(256)
 k_shade_payload(const SceneDev* __restrict__ sc, CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf,
                 float4* __restrict__ colour, const DomSet* __restrict__ dom,
@@ -202,11 +204,12 @@ k_shade_payload(const SceneDev* __restrict__ sc, CamDev cam, ShadeParams sp, con
   const uint4 raw = __ldg(reinterpret_cast<const uint4*>(gbuf) + p);
   const unsigned long long G = ((unsigned long long)raw.y << 32) | raw.x;
   if (w_none(G)) return;
-  const F3 rgb = shade_payload(sc, cam, sp, (int)x, (int)y, G, dom, counters);
+  const F3 rgb = shade_payload(sc, cam, sp, (int)x, (int)y, G, SH ? dom : nullptr, counters);
   colour[p] = make_float4(rgb.x, rgb.y, rgb.z, 1.0f);
 }
 
 // MSAA-k reference resolve (DESIGN.md R-msaa): mean over the k samples of (shaded hit | background)
+template <bool SH>
 __global__ void __launch_bounds__(256)
 k_resolve_msaa(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
                CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ samples, uint32_t ms_k,
@@ -220,7 +223,7 @@ k_resolve_msaa(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, 
   for (uint32_t s = 0; s < ms_k; ++s) {
     const unsigned long long w = __ldg(&samples[(size_t)s * n_px + p]);
     if (w_none(w)) continue;
-    acc = acc + shade_word(sc, srec, vertices, cam, sp, w, dom, counters);
+    acc = acc + shade_word(sc, srec, vertices, cam, sp, w, SH ? dom : nullptr, counters);
     ++n_hit;
   }
   F3 bg = f3(sp.background[0], sp.background[1], sp.background[2]);
@@ -234,8 +237,10 @@ void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
                          float4* out, const DomSet* dom, const unsigned long long* counters, cudaStream_t st) {
   const size_t n = (size_t)cam.W * cam.H;
-  k_resolve_msaa<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, samples, ms_k, scene_rgb, out,
-                                                               sp.shadows ? dom : nullptr, counters);
+  if (sp.shadows && dom)
+    k_resolve_msaa<true><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, samples, ms_k, scene_rgb, out, dom, counters);
+  else
+    k_resolve_msaa<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, samples, ms_k, scene_rgb, out, nullptr, counters);
 }
 
 // R22: unit screen direction of the segment a word names; fixed-order fp32 (decides strip membership)
@@ -724,11 +729,15 @@ void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vert
                   const unsigned long long* counters, cudaStream_t st) {
   size_t n = (size_t)cam.W * cam.H;
   if (!sp.shadows) dom = nullptr;
+  const dim3 gp((cam.W + 63) / 64, (cam.H + 3) / 4);
+  const unsigned gs = (unsigned)((n + 255) / 256);
   if (sp.paper_payload) {
-    k_shade_payload<<<dim3((cam.W + 63) / 64, (cam.H + 3) / 4), 256, 0, st>>>(d_scene, cam, sp, gbuf, colour, dom, counters);
+    if (dom) k_shade_payload<true><<<gp, 256, 0, st>>>(d_scene, cam, sp, gbuf, colour, dom, counters);
+    else k_shade_payload<false><<<gp, 256, 0, st>>>(d_scene, cam, sp, gbuf, colour, nullptr, counters);
     return;
   }
-  k_shade<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour, dom, counters);
+  if (dom) k_shade<true><<<gs, 256, 0, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour, dom, counters);
+  else k_shade<false><<<gs, 256, 0, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour, nullptr, counters);
 }
 
 template <int R>
