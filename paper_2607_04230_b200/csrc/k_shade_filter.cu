@@ -302,9 +302,13 @@ __device__ __forceinline__ float2 screen_tangent_payload(const CamDev& cam, int 
 // (4) the item's lane composites over the background (R29) and writes out_rgb; pixels without a hit are written by
 //     their owner thread.
 #define FT_W 32
-#define FT_H 16
+#ifndef FT_H
+#define FT_H 16  // tile rows; FT_W * FT_H / 2 threads per CTA, each owns the pixels (x, y) and (x, y + FT_H / 2)
+#endif
+#define FT_HH (FT_H / 2)
+#define FT_NT (FT_W * FT_HH)
 #ifndef FILT_MIN_BLOCKS
-#define FILT_MIN_BLOCKS 4  // CTAs per SM the register budget is held to
+#define FILT_MIN_BLOCKS (1024 / FT_NT)  // CTAs per SM the register budget is held to (64 registers per thread)
 #endif
 #ifndef FILT_DEAL
 #define FILT_DEAL 1  // conservative-sample items dealt by bank class (0: packed in pixel order)
@@ -445,7 +449,7 @@ __device__ __forceinline__ float strip_alpha(const uint2* __restrict__ s_dq, int
 }
 
 template <int R>
-__global__ void __launch_bounds__(256, FILT_MIN_BLOCKS)
+__global__ void __launch_bounds__(FT_NT, FILT_MIN_BLOCKS)
 k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const float4* __restrict__ vertices,
          CamDev cam, ShadeParams sp, const unsigned long long* __restrict__ gbuf, const float4* __restrict__ colour,
          const float4* __restrict__ scene_rgb, float4* __restrict__ out) {
@@ -462,13 +466,13 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
   const int W = (int)cam.W, H = (int)cam.H;
   const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
   const int x0 = blockIdx.x * FT_W, y0 = blockIdx.y * FT_H;
-  // ---- own two pixels (rows ly and ly + 8 of the tile)
+  // ---- own two pixels (rows ly and ly + FT_H / 2 of the tile)
   unsigned long long G[2], A[2];
   bool inside[2];
   int hit = 0;
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
-    const int px = x0 + lx, py = y0 + ly + 8 * k;
+    const int px = x0 + lx, py = y0 + ly + FT_HH * k;
     inside[k] = px < W && py < H;
     G[k] = A[k] = HAIR_EMPTY;
     if (inside[k]) {
@@ -483,7 +487,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
 #pragma unroll
   for (int k = 0; k < 2; ++k)
     if (inside[k] && w_none(A[k])) {
-      const size_t p = (size_t)(y0 + ly + 8 * k) * W + x0 + lx;
+      const size_t p = (size_t)(y0 + ly + FT_HH * k) * W + x0 + lx;
       float4 bg = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
       if (scene_rgb) {
         const float4 b = __ldg(&scene_rgb[p]);
@@ -494,7 +498,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
   if (!any_hit) return;  // empty tile: background only
   // ---- (1) tile + halo to shared memory, one pixel pair per thread and round
   const float kappa = fmaxf(sqrtf(sp.kC), 1e-15f);
-  for (int i = tid; i < NP; i += 256) {
+  for (int i = tid; i < NP; i += FT_NT) {
     const int sy = i / HP, pp = i - sy * HP;
     const int gy = y0 + sy - R;
     float c[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
@@ -535,21 +539,21 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
     const bool isCenter = !w_none(G[k]), isCons = !w_none(A[k]);
     Tc[k] = Ta[k] = make_float2(1.f, 0.f);
     if (isCenter) {
-      Tc[k] = sp.paper_payload ? screen_tangent_payload(cam, x0 + lx, y0 + ly + 8 * k, G[k])
+      Tc[k] = sp.paper_payload ? screen_tangent_payload(cam, x0 + lx, y0 + ly + FT_HH * k, G[k])
                                : screen_tangent(sc, srec, vertices, cam, G[k]);
       fly[k] = isCons && w_dq(G[k]) >= w_dq(A[k]) && w_dq(G[k]) - w_dq(A[k]) >= sp.taufly_q;  // PAPER.md:175, R21
     }
     const bool isA = fly[k] || (isCons && !isCenter);  // fly-away strand, or promoted pixel: w_color = 1
     if (isA)
-      Ta[k] = sp.paper_payload ? screen_tangent_payload(cam, x0 + lx, y0 + ly + 8 * k, A[k])
+      Ta[k] = sp.paper_payload ? screen_tangent_payload(cam, x0 + lx, y0 + ly + FT_HH * k, A[k])
                                : screen_tangent(sc, srec, vertices, cam, A[k]);
     balC[k] = __ballot_sync(0xffffffffu, isCenter);
     balA[k] = __ballot_sync(0xffffffffu, isA);
-    if (lx == 0) s_cn[ly + 8 * k] = __popc(balC[k]);
+    if (lx == 0) s_cn[ly + FT_HH * k] = __popc(balC[k]);
   }
   constexpr int KS = HP & 7;  // bank-group step of one tile row
   if (lx < 16) {  // conservative-sample items per (row, class): lane l of warp ly reports k = l >> 3, class = l & 7
-    const int rk = lx >> 3, rc = lx & 7, rrow = ly + 8 * rk;
+    const int rk = lx >> 3, rc = lx & 7, rrow = ly + FT_HH * rk;
     s_cc[rrow][rc] = __popc(balA[rk] & (0x00030003u << (2 * ((rc - KS * rrow) & 7))));
   }
   __syncthreads();
@@ -586,11 +590,11 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
   for (int c = 0; c < 8; ++c) tot_a += s_cc[FT_H][c];
   const int n_item = n_centre + (int)tot_a;
 #endif
-  for (int i = tid; i < n_item; i += 256) s_item[i].w = __uint_as_float(0xFFFFFFFFu);  // empty slot
+  for (int i = tid; i < n_item; i += FT_NT) s_item[i].w = __uint_as_float(0xFFFFFFFFu);  // empty slot
   __syncthreads();
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
-    const int row = ly + 8 * k;
+    const int row = ly + FT_HH * k;
     const uint32_t pix = (uint32_t)(row * FT_W + lx);
     if ((balC[k] >> lx) & 1u) {
       slot_c[k] = (int)(s_cn[row] + __popc(balC[k] & lt_mask));
@@ -672,7 +676,7 @@ k_filter(const SceneDev* __restrict__ sc, const uint2* __restrict__ srec, const 
       const float4 a = s_item[slot_a[k]];
       r = a.x, g = a.y, b = a.z, alpha = a.w;
     }
-    const size_t p = (size_t)(y0 + ly + 8 * k) * W + x0 + lx;
+    const size_t p = (size_t)(y0 + ly + FT_HH * k) * W + x0 + lx;
     float4 bg = make_float4(sp.background[0], sp.background[1], sp.background[2], 0.f);
     if (scene_rgb) {
       const float4 s4 = __ldg(&scene_rgb[p]);
@@ -753,7 +757,7 @@ static void launch_filter_r(const SceneDev* d_scene, const uint2* srec, const fl
     ls->filter_set[R] = true;
   }
   dim3 grid((cam.W + FT_W - 1) / FT_W, (cam.H + FT_H - 1) / FT_H);
-  k_filter<R><<<grid, 256, smem, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out);
+  k_filter<R><<<grid, FT_NT, smem, st>>>(d_scene, srec, vertices, cam, sp, gbuf, colour, scene_rgb, out);
 }
 
 int launch_filter(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
