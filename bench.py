@@ -45,7 +45,7 @@ def ncu_traffic():
             f = line.split(",")
             if len(f) >= 2 and f[1].strip().isdigit():
                 out[f[0].strip()] = int(f[1])
-        out["source"] = "profiles/r2_ncu_traffic.csv (ncu --set full capture of this command; see profiles/r2_ncu_full.md)"
+        out["source"] = "profiles/r2_ncu_traffic.csv (ncu --set full capture of the bench command; see profiles/r2_ncu_traffic.md, r2_v2_ncu_full.md)"
     return out
 
 
