@@ -293,9 +293,10 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
         const int rhi = min((int)floorf(fmaxf(m0, m1) + ENUM_EPS), r1);
         const float cM = fc + 0.5f;
         const float uM = xsub(cM, aM);
-        // pixel (c, r) in major/minor order -> word pair address; stride of one minor step
-        const size_t pstep = ymajor ? 2 : (size_t)2 * W;
-        unsigned long long* pcol = gbuf + (ymajor ? (size_t)c * W * 2 : (size_t)c * 2);
+        // pixel (c, r) in major/minor order -> index of its word pair (32-bit: W * H <= 2^28); step of one minor step
+        const uint32_t pstep = ymajor ? 1u : (uint32_t)W;
+        const uint32_t pcol = ymajor ? (uint32_t)c * (uint32_t)W : (uint32_t)c;
+        ulonglong2* const gpair = reinterpret_cast<ulonglong2*>(gbuf);
         for (int rb = rlo; rb <= rhi; rb += ROW_BATCH) {
           // pass 1: the cheap half of the conservative predicate (R10), then request the words
           bool ok[ROW_BATCH];
@@ -306,7 +307,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
             const float uN = xsub((float)r + 0.5f, aN);
             const float cr = fabsf(xsub(xmul(dM, uN), xmul(dN, uM)));
             ok[i] = r <= rhi && cr <= ext;
-            if (!MS && ok[i]) cur[i] = GB_LOAD(reinterpret_cast<const ulonglong2*>(pcol + (size_t)r * pstep));
+            if (!MS && ok[i]) cur[i] = GB_LOAD(gpair + (pcol + (uint32_t)r * pstep));
           }
           if (MS) {  // reference mode: every sample point of the pixels that passed the conservative predicate
             const int pat = ms_k == 8 ? 3 : ms_k == 4 ? 2 : ms_k == 2 ? 1 : 0;
@@ -372,7 +373,7 @@ k_raster(const SceneDev* __restrict__ sc, uint32_t n_bi, const uint4* __restrict
               }
             } else
               word = pack_word(zn, (key >> 7) & 0xFFFFFFu, key & 0x7Fu, tt);
-            unsigned long long* px = pcol + (size_t)r * pstep;
+            unsigned long long* px = reinterpret_cast<unsigned long long*>(gpair + (pcol + (uint32_t)r * pstep));
             if (COUNT) {
               ++c_cons;
               c_cons_y += ymajor ? 1u : 0u;
