@@ -315,9 +315,9 @@ int hair_atomic_microbench(hair_ctx*, int mode, uint64_t* dev_words, uint64_t n_
 int hair_l2_load_microbench(hair_ctx*, int mode, const uint64_t* dev_pairs, uint64_t n_pairs, uint32_t pitch,
                             uint32_t n_steps, uint64_t* out_loads, float* out_ms);
 
-/* sizeof of {hair_cage, hair_roots, hair_style, hair_camera, hair_render_params, hair_stats_t}, so a
- * foreign-language binding can check its struct layouts without a GPU. */
-void hair_abi_sizes(uint32_t out[6]);
+/* sizeof of {hair_cage, hair_roots, hair_style, hair_camera, hair_render_params, hair_stats_t, hair_shadow_params},
+ * so a foreign-language binding can check its struct layouts without a GPU. */
+void hair_abi_sizes(uint32_t out[7]);
 
 #ifdef __cplusplus
 }

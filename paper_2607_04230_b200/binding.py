@@ -129,11 +129,12 @@ def load():
     L.hair_shadow_build.argtypes = [vp, C.POINTER(hair_shadow_params)]
     L.hair_shadow_clear.argtypes = [vp]
     L.hair_debug_shadow.argtypes = [vp, u32, C.POINTER(vp), C.POINTER(vp), C.POINTER(u32 * 4)]
-    L.hair_abi_sizes.argtypes = [C.POINTER(C.c_uint32 * 6)]
+    L.hair_abi_sizes.argtypes = [C.POINTER(C.c_uint32 * 7)]
     L.hair_abi_sizes.restype = None
-    sizes = (C.c_uint32 * 6)()
+    sizes = (C.c_uint32 * 7)()
     L.hair_abi_sizes(C.byref(sizes))
-    mine = [C.sizeof(t) for t in (hair_cage, hair_roots, hair_style, hair_camera, hair_render_params, hair_stats_t)]
+    mine = [C.sizeof(t) for t in (hair_cage, hair_roots, hair_style, hair_camera, hair_render_params, hair_stats_t,
+                                    hair_shadow_params)]
     if list(sizes) != mine:
         raise HairError(f"struct layout mismatch between binding.py {mine} and libhair {list(sizes)}")
     _lib = L

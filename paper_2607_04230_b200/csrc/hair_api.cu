@@ -1045,13 +1045,14 @@ int hair_debug_set_vertices(hair_ctx* c, const float* dev_src, uint32_t n) {
   return HAIR_OK;
 }
 
-void hair_abi_sizes(uint32_t out[6]) {
+void hair_abi_sizes(uint32_t out[7]) {
   out[0] = sizeof(hair_cage);
   out[1] = sizeof(hair_roots);
   out[2] = sizeof(hair_style);
   out[3] = sizeof(hair_camera);
   out[4] = sizeof(hair_render_params);
   out[5] = sizeof(hair_stats_t);
+  out[6] = sizeof(hair_shadow_params);
 }
 
 int hair_atomic_microbench(hair_ctx* c, int mode, uint64_t* dev_words, uint64_t n_words, uint64_t n_ops,

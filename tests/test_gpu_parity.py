@@ -1219,3 +1219,63 @@ def test_deep_opacity_maps_and_shadowed_shading(orc, hair_mod, idx, scale, res_s
     h.shadow_clear()
     _, rgb = h.render(cam, sc["lam"])
     assert np.array_equal(rgb.cpu().numpy().astype(np.float64), G0["plain"][1])
+
+
+def test_shadows_in_the_payload_shading_and_the_msaa_resolve(orc, hair_mod):
+    """HAIR_FLAG_SHADOWS through the other two shading kernels (R-dom): k_shade_payload (position rebuilt from the
+    word's depth) and k_resolve_msaa (every sample shaded), each against the oracle with the same maps."""
+    import torch
+    b = hair_mod
+    sc = synth.config(2, scale=0.05, res_scale=0.33)
+    cam, lam, prm = sc["camera"], sc["lam"], dict(sc["params"], background_rgb=(0.1, 0.2, 0.3))
+    lcams = synth.light_cameras(sc, 256)
+    d1, alpha = 2e-4, 0.05
+    h = b.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(prm)
+    h.shadow_build(lcams, d1, alpha)
+    maps = []
+    for l in range(len(lcams)):
+        z0, cnt, D = h.debug_shadow(l)
+        maps.append((z0.cpu().numpy().view(np.uint32), cnt.cpu().numpy().view(np.uint32), D))
+
+    def oracle_frame(payload):
+        f = orc.Frame(sc["grooms"])
+        f.set_payload_mode(payload)
+        f.lod(cam, lam)
+        f.generate()
+        for l, (lc, (z0, cnt, D)) in enumerate(zip(lcams, maps)):
+            f.set_dom(l, lc, z0, cnt, D, alpha)
+        return f
+
+    # (i) the paper's payload
+    h.set_render_params(prm, flags=b.FLAG_PAPER_PAYLOAD)
+    _, plain = h.render(cam, lam)
+    plain = plain.clone()
+    h.set_render_params(prm, flags=b.FLAG_PAPER_PAYLOAD | b.FLAG_SHADOWS)
+    gb, rgb = h.render(cam, lam)
+    torch.cuda.synchronize()
+    f = oracle_frame(True)
+    f.set_vertices_f32(h.debug_vertices().cpu().numpy())
+    f.set_gbuffer(b.gbuffer_to_numpy(gb))
+    f.shade(cam, prm)
+    out = f.filter(cam, prm)
+    got = rgb.cpu().numpy().astype(np.float64)
+    assert np.abs(out - got).max() <= TOL_RGB
+    assert psnr(out[..., :3], got[..., :3], max(float(out[..., :3].max()), 1.0)) > MIN_PSNR
+    assert got[..., :3].sum() < 0.98 * float(plain[..., :3].sum())
+    # (ii) the MSAA reference resolve
+    for k in (1, 4):
+        h.set_render_params(prm, flags=b.FLAG_SHADOWS)
+        samples, rgb = h.render_msaa(cam, lam, k)
+        torch.cuda.synchronize()
+        f = oracle_frame(False)
+        f.set_vertices_f32(h.debug_vertices().cpu().numpy()[: f.n_vertices])
+        f.set_msaa(samples.cpu().numpy().view(np.uint64))
+        out = f.resolve_msaa(cam, prm)
+        got = rgb.cpu().numpy().astype(np.float64)
+        assert np.abs(out - got).max() <= TOL_RGB, k
+        h.set_render_params(prm)
+        _, rgb0 = h.render_msaa(cam, lam, k)
+        assert got[..., :3].sum() < 0.98 * float(rgb0[..., :3].sum())
