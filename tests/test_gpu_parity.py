@@ -1279,3 +1279,15 @@ def test_shadows_in_the_payload_shading_and_the_msaa_resolve(orc, hair_mod):
         h.set_render_params(prm)
         _, rgb0 = h.render_msaa(cam, lam, k)
         assert got[..., :3].sum() < 0.98 * float(rgb0[..., :3].sum())
+
+
+@pytest.mark.parametrize("r", [1, 2, 3, 4, 6])
+def test_every_filter_radius(orc, hair_mod, r):
+    """k_filter<R> for the radii the other tests do not reach (0, 5, 7 are covered elsewhere): the pair layout's row
+    pitch, bank classes and masked window-end tap differ per R. Curl + frizz groom at a ragged odd width, so windows
+    hold fly-away and promoted pixels and cross the image border."""
+    sc = synth.config(2, scale=0.03, res_scale=0.2)
+    sc["camera"] = dict(sc["camera"], width=sc["camera"]["width"] | 1, height=sc["camera"]["height"] | 1)
+    G = gpu_frame(hair_mod, sc, prm_over=dict(filter_radius=r))
+    rep = check_stagewise(orc, sc, G)
+    assert rep["n_hit"] > 2000
