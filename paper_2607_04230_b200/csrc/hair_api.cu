@@ -28,6 +28,9 @@ const int EV_RING = 64;  // stage timings of up to 64 frames are averaged by hai
 
 }  // namespace
 
+#ifndef HAIR_STAGE_DMA
+#define HAIR_STAGE_DMA 1  // hair_mesh_update staging by the copy engine on the second stream (0: by one SM copy kernel)
+#endif
 struct hair_ctx {
   int device = 0;
   int n_sm = 148;
@@ -294,9 +297,16 @@ void flush_updates(hair_ctx* c) {
   if (!c->jobs.n) return;
   // the bus transfer runs on the second stream — beside whatever the stream is still busy with (the frame before, when
   // the host runs ahead) — once the staging buffers' previous content has been applied; only the device-to-device apply
-  // is in front of the next frame
+  // is in front of the next frame. The transfer itself is left to the host-to-device copy engine: an SM copy kernel
+  // pulling the cages over the bus (HAIR_STAGE_DMA=0) has to find CTA slots beside the frame's persistent kernels and
+  // measured 1.55 ms per pipelined frame against 1.45 ms (the device-to-host copy of the image, which bounds it)
   if (c->applied_once) cudaStreamWaitEvent(c->aux_stream, c->ev_applied, 0);
+#if HAIR_STAGE_DMA
+  for (int i = 0; i < c->jobs.n; ++i)
+    cudaMemcpyAsync(c->jobs.j[i].dst, c->jobs.j[i].src, c->jobs.j[i].n * 4, cudaMemcpyDefault, c->aux_stream);
+#else
   launch_copy_jobs(c->jobs, c->aux_stream);
+#endif
   cudaEventRecord(c->ev_staged, c->aux_stream);
   cudaStreamWaitEvent(c->stream, c->ev_staged, 0);
   launch_copy_jobs(c->jobs_apply, c->stream);
