@@ -45,7 +45,7 @@ def ncu_traffic():
             f = line.split(",")
             if len(f) >= 2 and f[1].strip().isdigit():
                 out[f[0].strip()] = int(f[1])
-        out["source"] = "profiles/r2_ncu_traffic.csv (ncu --set full capture of the bench command; see profiles/r2_ncu_traffic.md, r2_v2_ncu_full.md)"
+        out["source"] = "profiles/r2_ncu_traffic.csv (ncu --set full capture of the bench command; see profiles/r2_ncu_traffic.md, r2_v3_ncu_full.md)"
     return out
 
 
@@ -321,7 +321,7 @@ def run_cuda(args):
     del words
     # 16-byte ld.global.cg of word pairs over the frame's own G-buffer, in the raster's access shapes (G pair loads / s)
     l2 = {}
-    for mode, name in ((0, "row"), (1, "column"), (2, "random")):
+    for mode, name in ((0, "row"), (1, "column"), (2, "random"), (5, "column_pairs")):
         h.l2_load_microbench(mode, gb, W, 32)  # warm
         l2[name] = max(n / (ms * 1e-3) / 1e9 for n, ms in (h.l2_load_microbench(mode, gb, W, 512) for _ in range(3)))
     n_px = W * H
@@ -353,7 +353,8 @@ def run_cuda(args):
     # anything is known about its depth (read-before-atomic) = one 16-byte L2 load, the method's own
     # minimum. Lower bound of the time = x-major loads at the measured row rate + y-major loads at the column rate.
     ras = stages["raster"]
-    t_min_ms = ((n_cons - n_cons_y) / l2["row"] + n_cons_y / l2["column"]) / 1e9 * 1e3
+    l2_y = max(l2["column"], l2["column_pairs"])  # a y-major task requests the two minor-axis neighbours of a row together
+    t_min_ms = ((n_cons - n_cons_y) / l2["row"] + n_cons_y / l2_y) / 1e9 * 1e3
     ras["Gpair_loads_per_s"] = n_cons / (ras["ms"] * 1e-3) / 1e9
     ras["Ghits_per_s"] = n_at / (ras["ms"] * 1e-3) / 1e9
     ras["frac_l2_load"] = t_min_ms / ras["ms"]
@@ -368,8 +369,9 @@ def run_cuda(args):
                     "algorithmic": f"{n_cons} conservative-predicate-true pixels (counts.n_atomics_cons), one 16-byte "
                                    f"ld.global.cg of the word pair each; {n_cons_y} of them on y-major segments",
                     "peak_source": "measured in this run (hair_l2_load_microbench over this frame's G-buffer): "
-                                   f"row {l2['row']:.1f}, column {l2['column']:.1f}, random {l2['random']:.1f} G pair loads/s; "
-                                   "peak = loads / (x-major loads / row rate + y-major loads / column rate)",
+                                   f"row {l2['row']:.1f}, column {l2['column']:.1f}, column with the two minor-axis neighbours "
+                                   f"requested together {l2['column_pairs']:.1f}, random {l2['random']:.1f} G pair loads/s; "
+                                   "peak = loads / (x-major loads / row rate + y-major loads / the better column rate)",
                     "covers": "the raster stage: k_raster (near pass) + k_hiz + k_raster (far pass); time = stages.raster.ms",
                     "atomic_view": {"hits_per_s_G": ras["Ghits_per_s"], "frac_of_random_RED": ras["frac_l2_atomic_random"],
                                     "issued_Gatom_per_s": cnt["n_atomics_issued"] / (ras["ms"] * 1e-3) / 1e9,

@@ -309,7 +309,10 @@ int hair_atomic_microbench(hair_ctx*, int mode, uint64_t* dev_words, uint64_t n_
 /* L2-load roofline denominator for the raster's read-before-atomic ("reads the existing depth buffer";
  * SURVEY.md §8d): 16-byte ld.global.cg of word pairs over a DEVICE buffer of n_pairs pairs laid out as image rows
  * of `pitch` pairs (n_pairs >= 64 * pitch, pitch >= 64). A warp's 32 loads of one step are
- *  mode 0: 32 consecutive pairs of a row;  mode 1: one column over 32 consecutive rows;  mode 2: 32 random pairs.
+ *  mode 0: 32 consecutive pairs of a row;  mode 1: one column over 32 consecutive rows;  mode 2: 32 random pairs;
+ *  mode 3 / 4: the column / row walk in a layout of 2 x 4-pixel blocks (an experiment);
+ *  mode 5: the column walk with the two horizontally adjacent pairs of a row requested together by each lane, the
+ *          shape of a y-major raster task (two loads per sector).
  * Every thread of n_SM * 8 CTAs of 256 threads issues `n_steps` loads (a multiple of 4). Writes the total number of
  * loads to *out_loads and the elapsed milliseconds (CUDA events; synchronises) to *out_ms. The buffer is only read. */
 int hair_l2_load_microbench(hair_ctx*, int mode, const uint64_t* dev_pairs, uint64_t n_pairs, uint32_t pitch,

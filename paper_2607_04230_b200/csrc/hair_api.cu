@@ -1086,7 +1086,7 @@ int hair_atomic_microbench(hair_ctx* c, int mode, uint64_t* dev_words, uint64_t 
 
 int hair_l2_load_microbench(hair_ctx* c, int mode, const uint64_t* dev_pairs, uint64_t n_pairs, uint32_t pitch,
                             uint32_t n_steps, uint64_t* out_loads, float* out_ms) {
-  if (!c || !dev_pairs || !out_ms || !out_loads || mode < 0 || mode > 4 || pitch < 64 || n_pairs < 64ull * pitch ||
+  if (!c || !dev_pairs || !out_ms || !out_loads || mode < 0 || mode > 5 || pitch < 64 || n_pairs < 64ull * pitch ||
       n_pairs >= (1ull << 32) || n_steps == 0 || (n_steps & 3u))
     return HAIR_E_INVALID_ARG;
   CK(cudaSetDevice(c->device));

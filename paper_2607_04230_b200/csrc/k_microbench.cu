@@ -34,7 +34,9 @@ void launch_atomic_microbench(int mode, unsigned long long* words, unsigned long
 //  mode 0  "row":    32 consecutive pairs of one image row (512 contiguous bytes: an x-major segment's columns),
 //  mode 1  "column": the same x in 32 consecutive rows (stride pitch * 16 bytes: a y-major segment's columns),
 //  mode 2  "random": 32 unrelated pairs (sub-pixel segments scattered over the frame),
-//  mode 3 / 4  the column / row walk in a G-buffer laid out in blocks of 2 x 4 pixels (DESIGN.md 7.1c),
+//  mode 3 / 4  the column / row walk in a G-buffer laid out in blocks of 2 x 4 pixels (DESIGN.md 7.1b),
+//  mode 5  "column pairs": the column walk with the two minor-axis neighbours of a row requested together, as a
+//          y-major task of the raster does (both loads of a lane fall into one 32-byte sector),
 // at a hashed position that changes every step. pitch = pairs per image row.
 #define L2_MLP 4
 __global__ void __launch_bounds__(256) k_l2_load_bench(int mode, const ulonglong2* __restrict__ pairs, uint32_t n_pairs,
@@ -49,11 +51,13 @@ __global__ void __launch_bounds__(256) k_l2_load_bench(int mode, const ulonglong
     ulonglong2 v[L2_MLP];
 #pragma unroll
     for (int u = 0; u < L2_MLP; ++u) {
-      h = pcg(h + (uint32_t)u + 1u);
+      if (mode != 5 || !(u & 1)) h = pcg(h + (uint32_t)u + 1u);
       uint32_t idx;
       if (mode == 0) idx = h % (n_pairs - 32u) + lane;
       else if (mode == 1) idx = ((h >> 12) % (rows - 32u) + lane) * pitch + (h & 0xFFFu) % pitch;
       else if (mode == 2) idx = pcg(h ^ (lane * 0x85EBCA6Bu)) % n_pairs;
+      else if (mode == 5)  // column walk, two horizontally adjacent pairs per lane and row (ROW_BATCH = 2 of a y-major task)
+        idx = ((h >> 12) % (rows - 32u) + lane) * pitch + (((h & 0xFFFu) % (pitch - 1u)) & ~1u) + ((uint32_t)u & 1u);
       else {  // the same walks in a layout of 2 x 4-pixel blocks (one 128-byte line = 2 columns x 4 rows)
         uint32_t x, y;
         if (mode == 3) x = (h & 0xFFFu) % pitch, y = (h >> 12) % (rows - 32u) + lane;  // column
