@@ -213,3 +213,32 @@ def test_shading_is_scaled_by_the_transmittance_light_by_light(orc):
     f.set_dom_beta([0.4])
     brighter = f.shade(cam, prm)
     assert np.all(brighter[hit] >= shadowed[hit] - 1e-15) and (brighter[hit] > shadowed[hit] + 1e-6).any()
+
+
+def test_light_cameras_frame_the_whole_scene(orc):
+    """synth.light_cameras (input generator): orthonormal bases, eye at the light, every cage vertex of every groom
+    and instance inside the view frustum and the depth range when the light stands outside the scene (config 1), and
+    nothing in front of a light beyond its far plane otherwise."""
+    for idx in (1, 4, 5):
+        sc = synth.config(idx, scale=0.01, res_scale=0.1)
+        cams = synth.light_cameras(sc, 128)
+        assert len(cams) == len(sc["params"]["lights"])
+        for cam, (pos, _) in zip(cams, sc["params"]["lights"]):
+            r, u, f = (np.asarray(cam[k]) for k in ("right", "up", "forward"))
+            assert np.allclose(cam["eye"], pos)
+            assert np.allclose([r @ r, u @ u, f @ f], 1.0, atol=1e-12) and np.allclose([r @ u, r @ f, u @ f], 0.0, atol=1e-12)
+            assert np.allclose(np.cross(r, u), -f, atol=1e-12)  # the handedness of look_from_z
+            seen = total = 0
+            for g in sc["grooms"]:
+                p = g["pos"].reshape(-1, 3).astype(np.float64)[::7]
+                xf = g["xform"] if g["xform"] is not None else np.array([[1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]], np.float64)
+                for M in np.asarray(xf, np.float64).reshape(-1, 3, 4)[::9]:
+                    for q in (p @ M[:, :3].T + M[:, 3])[::5]:
+                        o, valid = orc.project(cam, q)
+                        if idx == 1:  # the lights stand outside the groom: all of it is in every map
+                            assert valid and 0.0 <= o[0] <= 128.0 and 0.0 <= o[1] <= 128.0 and 0.0 < o[2] < 1.0, (idx, o)
+                        elif valid:  # a light among the grooms cannot see behind itself (one perspective map per
+                            assert o[2] < 1.0, (idx, o)  # light); what it sees is never beyond the far plane
+                            seen += 1
+                        total += 1
+            assert idx == 1 or seen > 0.3 * total
