@@ -1291,3 +1291,70 @@ def test_every_filter_radius(orc, hair_mod, r):
     G = gpu_frame(hair_mod, sc, prm_over=dict(filter_radius=r))
     rep = check_stagewise(orc, sc, G)
     assert rep["n_hit"] > 2000
+
+
+def test_bench_shadows_full_size_sampled(orc, hair_mod):
+    """The bench's `shadows` leg as it is launched: BASELINE config 4 at full size (483 000 strands, LOD off in the
+    light views: 17.6 M segments), three lights, 1024 x 1024 maps, layer_d1 = 1e-4, alpha_s = 0.03. Sampled as the
+    oracle allows: z0 and the layer counts on windows of every light's map (oracle.Frame.set_window: pixels are
+    independent), bit for bit on the library's own vertices; then the shadowed 4K frame on windows of the image."""
+    import torch
+    sc = synth.config(4)
+    cam, prm, lam = sc["camera"], sc["params"], sc["lam"]
+    W, H = cam["width"], cam["height"]
+    res, d1, alpha = 1024, 1e-4, 0.03
+    lcams = synth.light_cameras(sc, res)
+    h = hair_mod.Hair(0)
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(prm)
+    h.shadow_build(lcams, d1, alpha)
+    torch.cuda.synchronize()
+    full = orc.Frame(sc["grooms"])
+    full.lod(lcams[-1], [0.0])
+    st = h.stats()
+    assert st["n_strands_lod"] == 483000 == full.n_strands and st["n_vertices"] == full.n_vertices
+    full.set_vertices_f32(h.debug_vertices().cpu().numpy())  # (vertex parity of LOD-off frames: the config 2 / 3 tests)
+    maps = []
+    n_tex = 0
+    for l, lc in enumerate(lcams):
+        z0_g, cnt_g, D = h.debug_shadow(l)
+        z0_g, cnt_g = z0_g.cpu().numpy().view(np.uint32), cnt_g.cpu().numpy().view(np.uint32)
+        maps.append((z0_g, cnt_g, D))
+        hit = np.argwhere(z0_g != 0xFFFFFFFF)
+        assert len(hit) > 2000, "the light sees no hair"
+        cy, cx = (int(v) for v in hit[len(hit) // 2])          # a texel in the middle of what the light sees
+        dense = np.unravel_index(int(cnt_g.sum(-1).argmax()), z0_g.shape)  # and the deepest stack of fragments
+        for (py, px) in ((cy, cx), (int(dense[0]), int(dense[1]))):
+            x0, y0 = max(px - 24, 0), max(py - 24, 0)
+            x1, y1 = min(x0 + 48, res), min(y0 + 48, res)
+            full.set_window(x0, y0, x1, y1)
+            z0_o, cnt_o = full.dom_build(lc, prm, D[:3])
+            assert np.array_equal(z0_o[y0:y1, x0:x1], z0_g[y0:y1, x0:x1]), (l, x0, y0)
+            assert np.array_equal(cnt_o[y0:y1, x0:x1], cnt_g[y0:y1, x0:x1]), (l, x0, y0)
+            n_tex += int((z0_g[y0:y1, x0:x1] != 0xFFFFFFFF).sum())
+    assert n_tex > 3000
+    del full
+    # the shadowed frame, as the bench renders it
+    h.set_render_params(prm, flags=hair_mod.FLAG_SHADOWS)
+    gb, rgb = h.render(cam, lam)
+    torch.cuda.synchronize()
+    G, got = hair_mod.gbuffer_to_numpy(gb), rgb.cpu().numpy().astype(np.float64)
+    f = orc.Frame(sc["grooms"])
+    f.lod(cam, lam)
+    assert np.array_equal(f.table()[0], h.debug_table().cpu().numpy().view(np.uint32))
+    beta, _, _ = f.beta()
+    f.set_vertices_f32(h.debug_vertices().cpu().numpy())
+    f.set_gbuffer(G)
+    for l, (lc, (z0, cnt, D)) in enumerate(zip(lcams, maps)):
+        f.set_dom(l, lc, z0, cnt, D, alpha)
+    f.set_dom_beta(beta)
+    cxn = lambda ndc: int((1.0 + ndc) * 0.5 * W)
+    for (x0, y0, x1, y1) in ((cxn(-0.75) - 64, H // 2 - 64, cxn(-0.75) + 64, H // 2 + 64),   # core of groom 0
+                             (cxn(0.15) - 64, H // 2 - 64, cxn(0.15) + 64, H // 2 + 64),    # groom 1 (beta < 1)
+                             (cxn(0.72) - 40, H // 2 - 40, cxn(0.72) + 40, H // 2 + 40)):   # groom 3, far
+        f.set_window(x0, y0, x1, y1)
+        f.shade(cam, prm)
+        out = f.filter(cam, prm)[y0:y1, x0:x1]
+        assert float(np.abs(out - got[y0:y1, x0:x1]).max()) <= TOL_RGB, (x0, y0)
+        assert psnr(out[..., :3], got[y0:y1, x0:x1, :3], max(float(out[..., :3].max()), 1.0)) > MIN_PSNR
