@@ -279,28 +279,29 @@ __device__ __forceinline__ float2 screen_tangent_payload(const CamDev& cam, int 
 //     centre hits pre-scaled by sqrt(kC), zero elsewhere; dq = 24-bit depth of the centre word, DQ_NONE without a
 //     centre hit), s_pk[p] = {k_a, k_b} (k = |scaled colour|^2, read by the accumulations with a colour term only),
 //     and s_dq[pixel] = {dq_centre, dq_cons} for the strip loop;
-// (2) every hit pixel emits ONE work item; centre-hit pixels are compacted in PIXEL ORDER (promoted conservative-only
-//     pixels, follow in a second run), so a warp of a dense tile holds one tile row;
-// (3) item / thread. Loop A, Eq. 10, walks the (2r+1)^2 window one PAIR of taps at a time: three
-//     loads bring both taps' colour, k and depth, and the arithmetic of the two taps runs in the packed fp32
-//     instructions of sm_100 (FFMA2 / FADD2: fma.rn.f32x2 — two cycles of the FMA pipe like two FFMAs, but ONE issue
-//     slot, which is what this loop was short of). Adjacent pixels of a row share their pairs, so the 32 lanes of a
-//     row-ordered warp read 16 distinct 16-byte words per LDS.128: two shared-memory cycles instead of four
-//     (measured on the B200: the LDS pipe serves 128 distinct bytes per cycle and multicasts for free; profiles/).
-//     A pixel whose conservative sample is a fly-away strand in front (R21) runs its second accumulation — around
-//     the conservative sample, w_color = 1 — ON THE SAME LOADS; a warp without such a lane runs the loop without
-//     that part. The window of a pixel at odd x starts one tap early and the one at even x ends one tap late (pairs
-//     are aligned): that tap is masked. Exponent, base 2 and positive so that ex2.approx(-e) is the weight: the
-//     quadratic form of Eq. 10 in Horner form over dx, (a dx + B) dx + C with per-row B, C; colour distance
-//     |C_P|^2 - 2 C_P.C_Q + |C_Q|^2 with the first term in C and the last read from shared memory. The class test
-//     (R20) is the integer compare (d - lo) <= 2 tau (mod 2^32) on the ALU pipe.
+// (2) every hit pixel emits work items: a CENTRE item per centre-hit pixel, compacted in PIXEL ORDER (a warp of a
+//     dense tile holds one tile row), and a CONSERVATIVE-SAMPLE item per promoted pixel and per
+//     centre-hit pixel with a fly-away strand in front (R21: a second accumulation around the conservative sample,
+//     w_color = 1); those are sparse and are dealt by bank class instead;
+// (3) item / thread, the warps of the CTA taking item warps from a shared counter. Loop A, Eq. 10,
+//     walks the (2r+1)^2 window one PAIR of taps at a time: three loads (two for a conservative-sample item) bring
+//     both taps' colour, depth and k, and the arithmetic of the two taps runs in the packed fp32 instructions of
+//     sm_100 (FFMA2 / FADD2: fma.rn.f32x2 — two cycles of the FMA pipe like two FFMAs, but ONE issue slot, which is
+//     what this loop was short of). Adjacent pixels of a row share their pairs, so the 32 lanes of a row-ordered
+//     warp read 16 distinct 16-byte words per LDS.128: two shared-memory cycles instead of four (measured on the
+//     B200: the LDS pipe serves 128 distinct bytes per cycle and multicasts for free). The window of a
+//     pixel at odd x starts one tap early and the one at even x ends one tap late (pairs are aligned): that tap is
+//     masked. Exponent, base 2 and positive so that ex2.approx(-e) is the weight: the quadratic form of Eq. 10 in
+//     Horner form over dx, (a dx + B) dx + C with per-row B, C; colour distance |C_P|^2 - 2 C_P.C_Q + |C_Q|^2 with
+//     the first term in C and the last read from shared memory. The class test (R20) is the integer compare
+//     (d - lo) <= 2 tau (mod 2^32) on the ALU pipe.
 //     Loop B, strip hit counts: only lattice points within w_strip of the tangent line can be in the
 //     strip, so the loop walks the 2r+1 steps of the tangent's major axis and tests the `strip_nc` (2 for
 //     w_strip = 0.5) integer minor offsets that can lie within (w_strip + 0.01) sqrt(2) of the line — a superset;
 //     membership itself is Eq. 9 in the oracle's fixed-order fp32 (sqrt_rn(e2) <= w_strip tested as
 //     e2 <= strip_e2_max, host-side the largest float whose correctly rounded root is <= w_strip).
-// (4) the item's lane composites over the background (R29) and writes out_rgb; pixels without a hit are written by
-//     their owner thread.
+// (4) the owning thread combines its pixel's items (R21 blend for a fly-away pixel), composites over the background
+//     (R29) and writes out_rgb; pixels without a hit were written at the start.
 #define FT_W 32
 #ifndef FT_H
 #define FT_H 16  // tile rows; FT_W * FT_H / 2 threads per CTA, each owns the pixels (x, y) and (x, y + FT_H / 2)
@@ -339,7 +340,7 @@ __device__ __forceinline__ float gated_weight(float e, uint32_t dd, uint32_t tau
 
 // Loop A over the window of one item (one accumulation of Eq. 10, R19-R21). COL: colour term on (centre
 // sample) or off (conservative sample: w_color = 1). Positive base-2 exponent
-// a dx^2 + b dx dy + c dy^2 + c0 in Horner form over dx. ra / rd: the window's first pair in s_pa / s_pd; u = dx of the
+// a dx^2 + b dx dy + c dy^2 + c0 in Horner form over dx. ra / rd: the window's first pair in s_pa / s_pk; u = dx of the
 // first tap of a window row (-r, or -r-1 for a pixel at odd x, whose first tap then lies outside the window, as does
 // the last tap of a window at even x); (mx, my, mz) = -2 * scaled centre colour; class test (d - lo) <= tau2
 template <int R, bool COL>
