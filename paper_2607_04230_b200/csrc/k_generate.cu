@@ -11,10 +11,11 @@
 //            per-warp table. The base spline is linear in the root barycentrics
 //            (p(b) = sum_k b_k E_k), so no strand ever repeats the Hermite evaluation.
 //   stage 3  per strand once (lanes = strands, batches of 32): 3 hashes -> root barycentrics and curl
-//            phase, to shared memory. Then lanes = flattened (strand k, control point j): strand
-//            record + table row, ~20 FMA for position/tangent/AO, styling, instance transform, and
-//            one coalesced 16-byte store per lane (512 B per warp instruction, strand-major); (k, j)
-//            advance incrementally, no division per vertex.
+//            phase, to shared memory. Then a warp iteration covers 4 strands x 8 consecutive control points (fewer
+//            strands at a time for small bundles): the four lanes of a control point read the same table row (one
+//            shared-memory wavefront per LDS.128), the three-row barycentric blends are packed fp32 (FFMA2), then
+//            frame, styling, instance transform, and one 16-byte store per lane (each strand's run of the iteration
+//            is 128 contiguous bytes); (strand group, j) advance incrementally, no division per vertex.
 // Arithmetic: fp32 with FMA; parity gate = 1e-5 max-abs against the fp64 oracle.
 #include "gen_device.cuh"
 
