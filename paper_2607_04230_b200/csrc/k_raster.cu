@@ -20,7 +20,7 @@
 #define RAS_WARPS 8
 #endif
 #ifndef RAS_MIN_BLOCKS
-#define RAS_MIN_BLOCKS 5  // CTAs per SM the register budget is held to (40 of 64 warps)
+#define RAS_MIN_BLOCKS 4  // CTAs per SM the register budget is held to (32 of 64 warps; 64 registers, no spills: 715 vs 720 us at 5)
 #endif
 #define REC_STRIDE 20  // floats per segment record (18 used); 20 mod 32 keeps LDS.128 conflict-free
 #define REC_STRIDE_PP 28  // paper payload: + tangents at both ends (6), AO at both ends (2), (u6, v6) bits, C
