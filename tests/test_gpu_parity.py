@@ -1358,3 +1358,47 @@ def test_bench_shadows_full_size_sampled(orc, hair_mod):
         out = f.filter(cam, prm)[y0:y1, x0:x1]
         assert float(np.abs(out - got[y0:y1, x0:x1]).max()) <= TOL_RGB, (x0, y0)
         assert psnr(out[..., :3], got[y0:y1, x0:x1, :3], max(float(out[..., :3].max()), 1.0)) > MIN_PSNR
+
+
+def test_shadow_api_error_behaviour(hair_mod):
+    """include/hair.h: hair_shadow_build needs a groom and sane parameters; hair_debug_shadow needs a map; the flag
+    without maps (or after hair_mesh_clear, which drops them) leaves the shading unshadowed."""
+    import torch
+    b = hair_mod
+    sc = synth.config(1, scale=0.2, res_scale=0.5)
+    cam, prm, lam = sc["camera"], sc["params"], sc["lam"]
+    lcams = synth.light_cameras(sc, 64)
+    h = b.Hair(0)
+    with pytest.raises(b.HairError):
+        h.shadow_build(lcams, 1e-4, 0.05)  # no groom uploaded
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    h.set_render_params(prm)
+    _, plain = h.render(cam, lam)
+    plain = plain.clone()
+    with pytest.raises(b.HairError):
+        h.debug_shadow(0)  # no map yet
+    with pytest.raises(b.HairError):
+        h.shadow_build([dict(c, width=8, height=8) for c in lcams], 1e-4, 0.05)  # res < 16
+    with pytest.raises(b.HairError):
+        h.shadow_build(lcams, 0.0, 0.05)  # layer_d1 must be positive
+    with pytest.raises(b.HairError):
+        h.shadow_build(lcams, 1e-4, -1.0)  # alpha_s must not be negative
+    h.set_render_params(prm, flags=b.FLAG_SHADOWS)  # the flag without maps: unshadowed
+    _, rgb = h.render(cam, lam)
+    assert torch.equal(rgb, plain)
+    h.shadow_build(lcams[:1], 1e-4, 0.05)  # a map for light 0 only: lights 1, 2 stay unshadowed
+    _, one = h.render(cam, lam)
+    one = one.clone()
+    h.shadow_build(lcams, 1e-4, 0.05)
+    _, allm = h.render(cam, lam)
+    assert float(allm[..., :3].sum()) < float(one[..., :3].sum()) < float(plain[..., :3].sum())
+    with pytest.raises(b.HairError):
+        h.debug_shadow(3)  # only three lights have maps
+    h.shadow_build(synth.light_cameras(sc, 96), 2e-4, 0.05)  # another resolution: buffers are re-made
+    assert h.debug_shadow(2)[0].shape == (96, 96)
+    h.mesh_clear()
+    for g in sc["grooms"]:
+        h.mesh_upload(g)
+    _, rgb = h.render(cam, lam)  # the maps went with the grooms they were built from
+    assert torch.equal(rgb, plain)
