@@ -14,7 +14,9 @@
 // R-scene: a word whose 40 payload bits are all ones carries no hair hit (its depth is the scene's, or the far end)
 #define HAIR_PAYLOAD_NONE 0xFFFFFFFFFFull
 #define RAS_CHUNK 31  // segments a raster warp draws at once (32 vertices, neighbour by shuffle)
+#ifndef RAS_GROUP
 #define RAS_GROUP 4   // chunks per unit of the raster's device-side work queue
+#endif
 #ifndef HIZ_TILE
 #define HIZ_TILE 16
 #endif
