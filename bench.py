@@ -125,7 +125,10 @@ def run_reference(args):
         return
     import oracle
     oracle.build()
-    scale, res_scale = 0.02, 0.5
+    # a bounded sample of the metric's workload at its own resolution: 2 % of every groom's strands at 4K (about 3 s per
+    # step on the GPU box's host), fewer strands when many steps are asked for so that the run ends within minutes
+    n_runs = max(args.steps + args.warmup, 1)
+    scale, res_scale = (0.02 if n_runs <= 40 else max(0.02 * 40.0 / n_runs, 0.002)), 1.0
     for _ in range(args.warmup):
         oracle_sample(args.config, scale, res_scale)
     t, seg, desc = 0.0, 0, ""
