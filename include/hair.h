@@ -318,6 +318,34 @@ int hair_atomic_microbench(hair_ctx*, int mode, uint64_t* dev_words, uint64_t n_
 int hair_l2_load_microbench(hair_ctx*, int mode, const uint64_t* dev_pairs, uint64_t n_pairs, uint32_t pitch,
                             uint32_t n_steps, uint64_t* out_loads, float* out_ms);
 
+/* The H2 scan (per-bundle LOD records -> where each bundle's strands and vertices go) as a
+ * call that allocates nothing, for callers that cannot let a library cudaMalloc: an engine that gave all device
+ * memory to its own pool at start-up (an allocation in the frame loop fails or stalls the device), or a host whose
+ * per-frame code may not make synchronising calls, which cudaMalloc / cudaFree are. It takes no hair_ctx (creating
+ * one, uploading a groom and the first render all allocate) and calls no cudaMalloc, cudaFree or allocating library
+ * routine; the tile sums it needs between its two kernels sit in a fixed 32 KB array inside the library's device
+ * code, which every GPU that loads this library holds until the process exits.
+ *  cuda_device  device of the pointers and the stream; made current and left current, as by the other calls
+ *  cuda_stream  a cudaStream_t of that device (NULL = legacy default stream); the two kernels are enqueued on it and
+ *               the call returns without waiting
+ *  dev_counts   DEVICE, [n][2] uint32, 8-byte aligned: {N_LOD, C} of every bundle-instance in index order (columns
+ *               .x, .y of the bundle table, Eq. 1 and Eq. 4-5); only read
+ *  n            bundle-instances, 0 <= n <= HAIR_SCAN_NOALLOC_MAX; more returns HAIR_E_INVALID_ARG before anything
+ *               is launched (the array cannot grow), with the limit in hair_scan_noalloc_error()
+ *  dev_bases    DEVICE, [n][2] uint32, 8-byte aligned, written: {slot_base, vertex_base} = exclusive sums of N_LOD
+ *               and of N_LOD * C over the bundle-instances in front (columns .z, .w of the bundle table), mod 2^32
+ *  dev_totals   DEVICE, [2] uint32, written: {sum N_LOD, sum N_LOD * C} (hair_stats_t.n_strands_lod, .n_vertices)
+ * Must not overlap other calls on the same device: all calls of a process share the one array per device, so two
+ * whose kernels can run concurrently (two streams, two threads) race; back to back on one stream is fine. The array
+ * keeps the previous call's sums; every call rewrites all the entries it reads, so nothing needs clearing. The first
+ * call on a device also looks up the array's device address (cudaGetSymbolAddress): make that call before any
+ * stream capture begins. Returns HAIR_OK, HAIR_E_INVALID_ARG (size, null or misaligned pointer, device number) or
+ * HAIR_E_CUDA; hair_scan_noalloc_error() gives the text of the calling thread's last failure ("" after success). */
+#define HAIR_SCAN_NOALLOC_MAX (1u << 20)
+int hair_scan_noalloc(int cuda_device, void* cuda_stream, const uint32_t* dev_counts, uint32_t n,
+                      uint32_t* dev_bases, uint32_t* dev_totals);
+const char* hair_scan_noalloc_error(void);
+
 /* sizeof of {hair_cage, hair_roots, hair_style, hair_camera, hair_render_params, hair_stats_t, hair_shadow_params},
  * so a foreign-language binding can check its struct layouts without a GPU. */
 void hair_abi_sizes(uint32_t out[7]);

@@ -23,7 +23,9 @@ EXPORTS = ["hair_create", "hair_destroy", "hair_last_error", "hair_default_rende
            "hair_set_render_params", "hair_mesh_upload", "hair_mesh_update", "hair_mesh_clear",
            "hair_render", "hair_render_scene", "hair_render_sequential", "hair_render_msaa", "hair_render_to_host", "hair_render_to_host_async", "hair_host_wait", "hair_render_stages", "hair_stats",
            "hair_debug_buffers", "hair_debug_set_vertices", "hair_atomic_microbench", "hair_l2_load_microbench", "hair_abi_sizes",
-           "hair_shadow_build", "hair_shadow_clear", "hair_debug_shadow"]
+           "hair_shadow_build", "hair_shadow_clear", "hair_debug_shadow",
+           "hair_scan_noalloc", "hair_scan_noalloc_error"]
+SCAN_NOALLOC_MAX = 1 << 20
 
 
 class HairError(RuntimeError):
@@ -129,6 +131,9 @@ def load():
     L.hair_shadow_build.argtypes = [vp, C.POINTER(hair_shadow_params)]
     L.hair_shadow_clear.argtypes = [vp]
     L.hair_debug_shadow.argtypes = [vp, u32, C.POINTER(vp), C.POINTER(vp), C.POINTER(u32 * 4)]
+    L.hair_scan_noalloc.argtypes = [C.c_int, vp, vp, u32, vp, vp]
+    L.hair_scan_noalloc_error.argtypes = []
+    L.hair_scan_noalloc_error.restype = C.c_char_p
     L.hair_abi_sizes.argtypes = [C.POINTER(C.c_uint32 * 7)]
     L.hair_abi_sizes.restype = None
     sizes = (C.c_uint32 * 7)()
@@ -416,6 +421,25 @@ class Hair:
         self._check(self.L.hair_l2_load_microbench(self.h, mode, C.c_void_p(pairs.data_ptr()), pairs.numel() // 2, pitch,
                                                    n_steps, C.byref(n), C.byref(ms)), "hair_l2_load_microbench")
         return n.value, ms.value
+
+
+def scan_noalloc(counts, bases, totals, n: int | None = None, stream=None) -> None:
+    """hair_scan_noalloc: the H2 scan for callers that may not allocate device memory (an engine whose own pool holds
+    all of it, or a frame loop that bans the synchronising cudaMalloc / cudaFree). No context, no allocation here or in
+    the library: `counts` [n][2] {N_LOD, C}, `bases` [n][2] and `totals` [2] are the caller's int32 CUDA tensors
+    (uint32 bit patterns, contiguous); the library's scratch is a fixed array in its device code, so n is at most
+    SCAN_NOALLOC_MAX and calls that could overlap on one GPU must be ordered by the caller. Enqueues on `stream`
+    (default: torch's current stream of the tensors' device) and returns without waiting."""
+    import torch
+    dev = counts.device.index
+    assert counts.is_contiguous() and bases.is_contiguous() and totals.is_contiguous()
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    L = load()
+    rc = L.hair_scan_noalloc(dev, C.c_void_p(st.cuda_stream), C.c_void_p(counts.data_ptr()),
+                             counts.shape[0] if n is None else int(n), C.c_void_p(bases.data_ptr()),
+                             C.c_void_p(totals.data_ptr()))
+    if rc != 0:
+        raise HairError(f"hair_scan_noalloc failed ({rc}): {L.hair_scan_noalloc_error().decode()}")
 
 
 def gbuffer_to_numpy(gb) -> np.ndarray:
