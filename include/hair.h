@@ -66,13 +66,7 @@ extern "C" {
  * HAIR_E_INVALID_ARG. The debug vertex buffer is not valid after such a frame. An A/B against the default pipeline. */
 #define HAIR_FLAG_FUSED 32u
 
-/* Sort-middle raster (PAPER.md:254 names a hybrid raster as future work): segments are binned to
- * 64 x 64 pixel screen tiles and each tile's two G-buffer layers are resolved in SHARED memory (pixel tests are
- * LDS.128 instead of L2 loads, a per-tile hi-Z refreshed while drawing drops occluded segments whole), then stored
- * once. Same predicates, same words: the G-buffer equals the default raster's bit for bit. Replaces the clear and the
- * two depth-ordered passes. Ignored (default raster) with HAIR_FLAG_COUNTERS / PAPER_PAYLOAD / FUSED and in
- * hair_render_msaa. Needs 64 bytes of record pool per worst-case vertex (allocated on first use). */
-#define HAIR_FLAG_TILED 64u
+/* (bit 64u was HAIR_FLAG_TILED, a tile-binned raster A/B that lost 2.7x and was removed in round 3: DESIGN.md 7.1b) */
 
 /* Half-precision colour output: out_rgb / host_rgb of every render call is [height][width][4] IEEE binary16 (8 bytes per
  * pixel; the buffer still 16-byte aligned) instead of float, written by the filter itself (round to nearest; absolute error <= 2^-11 of
@@ -125,10 +119,16 @@ typedef struct {
 /* Appends a groom. Copies everything to the device (synchronously) and sizes the scratch buffers
  * for the worst case (LOD off). Strand ids are assigned in upload order (DESIGN.md §3 "sid"). */
 int hair_mesh_upload(hair_ctx*, const hair_cage*, const hair_roots*, const hair_style*, int* out_groom_id);
-/* Replaces positions / AO of an uploaded groom (animated cage). Same sizes. From PINNED host memory the
- * update is queued and all queued updates are copied by one kernel on the context's stream in front of the next
- * hair_render* / hair_stats call: the host arrays must stay valid and unchanged until that work has completed (e.g.
- * until hair_host_wait of the frame). From pageable memory the copy is a cudaMemcpyAsync inside this call. */
+/* Replaces positions / AO of an uploaded groom (animated cage). Same sizes.
+ * From PINNED host memory the call only queues the update; nothing is read yet. The next hair_render* / hair_stats /
+ * hair_shadow_build call sends every queued array to a staging buffer on the device with the copy engine
+ * (cudaMemcpyAsync on the context's second stream, so the bus transfer can run beside the frame before) and then
+ * copies staging -> cage with one device-to-device kernel on the context's stream in front of its own work. The host
+ * arrays are therefore read AFTER that later call has been issued: they must stay valid and unchanged until its work
+ * has completed (e.g. until hair_host_wait of that frame, or a hair_stats). hair_mesh_clear and hair_destroy drop
+ * updates still queued without reading them.
+ * From pageable memory the copy is a cudaMemcpyAsync on the context's stream inside this call (updates queued before
+ * it are sent first, so the updates of a groom take effect in call order); the array may be freed when it returns. */
 int hair_mesh_update(hair_ctx*, int groom_id, const hair_cage*);
 /* Removes all grooms (buffers are kept). */
 int hair_mesh_clear(hair_ctx*);
@@ -276,11 +276,7 @@ typedef struct {
   float beta_groom[HAIR_MAX_GROOMS], delta_groom[HAIR_MAX_GROOMS];
   uint32_t gpu_launches; /* kernels launched by the last hair_render */
   uint32_t two_pass;              /* 1: the last frame was drawn in two depth-ordered raster passes */
-  uint32_t n_segments_hiz_culled; /* segments of the second pass dropped by the tile hi-Z test before any pixel work
-                                     (HAIR_FLAG_TILED: (segment, tile) records dropped by the in-tile hi-Z) */
-  uint32_t tiled;                 /* 1: the last frame was drawn by the tile-binned raster (HAIR_FLAG_TILED) */
-  uint32_t n_tile_records;        /* its (segment, tile) records */
-  uint32_t tile_overflow;         /* 1: they exceeded the record pool and some were dropped (the frame is incomplete) */
+  uint32_t n_segments_hiz_culled; /* segments of the second pass dropped by the tile hi-Z test before any pixel work */
 } hair_stats_t;
 /* Synchronises the stream and reads the device counters of the last frame. */
 int hair_stats(hair_ctx*, hair_stats_t* out);

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(_HERE, "csrc", "libhair.so")
 
 OP_BITS = {"clump": 1, "twist": 2, "curl": 4, "frizz": 8}
-FLAG_FILTER, FLAG_COUNTERS, FLAG_STAGE_TIMING, FLAG_PAPER_PAYLOAD, FLAG_SINGLE_PASS, FLAG_FUSED, FLAG_TILED, FLAG_RGB16F = 1, 2, 4, 8, 16, 32, 64, 128
+FLAG_FILTER, FLAG_COUNTERS, FLAG_STAGE_TIMING, FLAG_PAPER_PAYLOAD, FLAG_SINGLE_PASS, FLAG_FUSED, FLAG_RGB16F = 1, 2, 4, 8, 16, 32, 128
 FLAG_SHADOWS = 256
 EMPTY = 0xFFFFFFFFFFFFFFFF
 
@@ -84,8 +84,7 @@ class hair_stats_t(C.Structure):
                 ("ms_total", C.c_float), ("n_timed_frames", C.c_uint32), ("beta_mean", C.c_float),
                 ("beta_min", C.c_float), ("beta_groom", C.c_float * 16), ("delta_groom", C.c_float * 16),
                 ("gpu_launches", C.c_uint32),
-                ("two_pass", C.c_uint32), ("n_segments_hiz_culled", C.c_uint32),
-                ("tiled", C.c_uint32), ("n_tile_records", C.c_uint32), ("tile_overflow", C.c_uint32)]
+                ("two_pass", C.c_uint32), ("n_segments_hiz_culled", C.c_uint32)]
 
     def as_dict(self):
         return {k: (list(getattr(self, k)) if k in ("beta_groom", "delta_groom") else getattr(self, k)) for k, _ in self._fields_}
@@ -198,6 +197,7 @@ class Hair:
         self._check(self.L.hair_create(C.byref(self.h), device, C.c_void_p(self.stream.cuda_stream)), "hair_create")
         self.n_grooms = 0
         self._res = None
+        self._pending_updates = []  # [event or None, arrays] of mesh_update calls whose host arrays may still be read
 
     def close(self):
         if getattr(self, "h", None) and self.h.value:
@@ -244,16 +244,36 @@ class Hair:
         return gid.value
 
     def mesh_update(self, groom_id: int, pos_pinned, ao_pinned=None):
-        """pos_pinned / ao_pinned: torch CPU tensors (pinned for an async copy) or numpy arrays."""
+        """pos_pinned / ao_pinned: torch CPU tensors (pinned for an async copy) or numpy arrays.
+
+        Lifetime: from pinned memory the library only queues the update and reads the arrays when the NEXT render /
+        stats / shadow_build is issued, finishing when that frame completes (include/hair.h). The binding therefore
+        keeps a reference to the arrays until an event recorded behind that frame has completed, so a temporary
+        (`torch.from_numpy(a).pin_memory()`) cannot be handed back to torch's pinned-memory cache and reused while the
+        copy is still to come. The CONTENTS are the caller's to leave alone until then."""
         def hp(x):
             return C.c_void_p(x.data_ptr()) if hasattr(x, "data_ptr") else _ptr(x)
         shp = pos_pinned.shape
         cage = hair_cage(shp[1], shp[0], hp(pos_pinned), None if ao_pinned is None else hp(ao_pinned))
         self._check(self.L.hair_mesh_update(self.h, groom_id, C.byref(cage)), "hair_mesh_update")
+        self._pending_updates.append([None, (pos_pinned, ao_pinned)])
+
+    def _updates_issued(self):
+        """Called after a call that flushed the queued updates onto the stream: mark them with an event behind that
+        work, and let go of the arrays of updates whose event has completed."""
+        ev = None
+        for p in self._pending_updates:
+            if p[0] is None:
+                if ev is None:
+                    ev = self.torch.cuda.Event()
+                    ev.record(self.stream)
+                p[0] = ev
+        self._pending_updates = [p for p in self._pending_updates if not p[0].query()]
 
     def mesh_clear(self):
         self._check(self.L.hair_mesh_clear(self.h), "hair_mesh_clear")
         self.n_grooms = 0
+        self._pending_updates = []  # the library dropped what was queued and synchronised its streams
 
     def set_render_params(self, prm: dict, flags: int = 0):
         p = make_params(prm, flags)
@@ -276,6 +296,7 @@ class Hair:
         c = make_camera(cam)
         self._check(self.L.hair_render(self.h, C.byref(c), w, h, _ptr(lam), len(lam),
                                        C.c_void_p(out_gbuffer.data_ptr()), C.c_void_p(out_rgb.data_ptr())), "hair_render")
+        self._updates_issued()
         self._res = (w, h)
         return out_gbuffer, out_rgb
 
@@ -289,6 +310,7 @@ class Hair:
         c = make_camera(cam)
         self._check(self.L.hair_render_msaa(self.h, C.byref(c), w, h, _ptr(lam), len(lam), int(k),
                                             C.c_void_p(samples.data_ptr()), C.c_void_p(out_rgb.data_ptr())), "hair_render_msaa")
+        self._updates_issued()
         self._res = (w, h)
         return samples, out_rgb
 
@@ -309,6 +331,7 @@ class Hair:
                                              None if scene_rgb is None else C.c_void_p(scene_rgb.data_ptr()),
                                              C.c_void_p(out_gbuffer.data_ptr()), C.c_void_p(out_rgb.data_ptr())),
                     _fn)
+        self._updates_issued()
         self._res = (w, h)
         return out_gbuffer, out_rgb
 
@@ -319,6 +342,7 @@ class Hair:
         self._check(self.L.hair_render_to_host(self.h, C.byref(c), w, h, _ptr(lam), len(lam),
                                                None if host_gbuffer is None else C.c_void_p(host_gbuffer.data_ptr()),
                                                C.c_void_p(host_rgb.data_ptr())), "hair_render_to_host")
+        self._updates_issued()
         self._res = (w, h)
 
     def render_to_host_async(self, cam: dict, lam, host_rgb, host_gbuffer=None) -> int:
@@ -330,6 +354,7 @@ class Hair:
         self._check(self.L.hair_render_to_host_async(self.h, C.byref(c), w, h, _ptr(lam), len(lam),
                                                      None if host_gbuffer is None else C.c_void_p(host_gbuffer.data_ptr()),
                                                      C.c_void_p(host_rgb.data_ptr()), C.byref(slot)), "hair_render_to_host_async")
+        self._updates_issued()
         self._res = (w, h)
         return slot.value
 
@@ -346,6 +371,7 @@ class Hair:
     def stats(self) -> dict:
         s = hair_stats_t()
         self._check(self.L.hair_stats(self.h, C.byref(s)), "hair_stats")
+        self._updates_issued()
         return s.as_dict()
 
     # ---- debug / parity
@@ -396,6 +422,7 @@ class Hair:
             assert lc["width"] == lc["height"] == p.res
             p.cam[i] = make_camera(lc)
         self._check(self.L.hair_shadow_build(self.h, C.byref(p)), "hair_shadow_build")
+        self._updates_issued()
         self._shadow_res = p.res
 
     def shadow_clear(self) -> None:

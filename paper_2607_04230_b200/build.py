@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(CSRC, "libhair.so")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
-SOURCES = ["hair_api.cu", "k_lod.cu", "k_generate.cu", "k_raster.cu", "k_raster_tiled.cu", "k_shade_filter.cu", "k_microbench.cu", "k_scan_noalloc.cu"]
+SOURCES = ["hair_api.cu", "k_lod.cu", "k_generate.cu", "k_raster.cu", "k_shade_filter.cu", "k_microbench.cu", "k_scan_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

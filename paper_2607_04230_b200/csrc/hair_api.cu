@@ -56,8 +56,6 @@ struct hair_ctx {
   CopyJobs jobs, jobs_apply;
   cudaEvent_t ev_staged = nullptr, ev_applied = nullptr;
   bool applied_once = false;
-  TileBufs tb;  // HAIR_FLAG_TILED: per-tile record lists (allocated on first use)
-  size_t tb_tiles = 0;
   size_t table_cap = 0;
   uint2* d_srec = nullptr;  // per strand id: {vertex offset, C | groom << 8} of this frame (k_generate)
   size_t srec_cap = 0;
@@ -94,7 +92,7 @@ struct hair_ctx {
   unsigned long long* d_dom_gbuf = nullptr;
   size_t dom_px = 0;
   bool dom_on = false;
-  bool timed = false, counted = false, last_two_pass = false, last_tiled = false;
+  bool timed = false, counted = false, last_two_pass = false;
   uint32_t last_w = 0, last_h = 0, launches = 0;
   CamDev last_cam;
 };
@@ -265,33 +263,6 @@ int ensure_scratch(hair_ctx* c, uint32_t w, uint32_t h) {
   return HAIR_OK;
 }
 
-// HAIR_FLAG_TILED: tile arrays for this resolution and a record pool of two records per worst-case vertex
-int ensure_tiles(hair_ctx* c, uint32_t w, uint32_t h) {
-  const size_t n_tiles = (size_t)((w + HAIR_TILE - 1) / HAIR_TILE) * ((h + HAIR_TILE - 1) / HAIR_TILE);
-  if (n_tiles > 65536) return fail(c, HAIR_E_INVALID_ARG, "HAIR_FLAG_TILED: more than 65536 tiles");
-  if (n_tiles > c->tb_tiles) {
-    cudaFree(c->tb.count);
-    c->tb.count = nullptr;
-    c->tb_tiles = 0;
-    CK(cudaMalloc((void**)&c->tb.count, 4 * n_tiles * sizeof(uint32_t)));
-    CK(cudaMemsetAsync(c->tb.count, 0, 4 * n_tiles * sizeof(uint32_t), c->stream));
-    c->tb.base = c->tb.count + n_tiles;
-    c->tb.n = c->tb.base + n_tiles;
-    c->tb.order = c->tb.n + n_tiles;
-    c->tb_tiles = n_tiles;
-  }
-  const size_t want = 2 * c->vertex_need + (1u << 16);
-  if (want > c->tb.cap) {
-    if (want >= (1ull << 32)) return fail(c, HAIR_E_INVALID_ARG, "HAIR_FLAG_TILED: record pool too large");
-    cudaFree(c->tb.entries);
-    c->tb.entries = nullptr;
-    c->tb.cap = 0;
-    CK(cudaMalloc((void**)&c->tb.entries, want * 2 * sizeof(float4)));
-    c->tb.cap = (uint32_t)want;
-  }
-  return HAIR_OK;
-}
-
 // hair_mesh_update's queued pinned-memory copies: one kernel for all of them, on the context's stream
 void flush_updates(hair_ctx* c) {
   if (!c->jobs.n) return;
@@ -368,12 +339,6 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   if (fused && !front) return fail(c, HAIR_E_INVALID_ARG, "hair_render_stages: not with HAIR_FLAG_FUSED");
   const bool timed = (c->prm.flags & HAIR_FLAG_STAGE_TIMING) != 0;
   const bool count = (c->prm.flags & HAIR_FLAG_COUNTERS) != 0;
-  // the tile-binned raster (k_raster_tiled.cu) draws production frames of the strand-id word only
-  const bool tiled = (c->prm.flags & HAIR_FLAG_TILED) && !count && !po.ms_k && !pp && !fused && (stage_mask & 1u) && c->scene.n_bi;
-  if (tiled) {
-    rc = ensure_tiles(c, w, h);
-    if (rc) return rc;
-  }
   const uint32_t n_bi = c->scene.n_bi;
   cudaStream_t st = c->stream;
   uint32_t launches = 0;
@@ -390,7 +355,7 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   mark(EV_BEGIN);
   // The clear of the G-buffer does not depend on LOD / scan / generate: it runs beside them on the context's second
   // stream (forked after everything already enqueued on `st`, joined before the raster). ms_clear then reads ~0.
-  const bool fork_clear = front && n_bi && (stage_mask & 1u) && !tiled;  // (the tile raster initialises its tiles)
+  const bool fork_clear = front && n_bi && (stage_mask & 1u);
   auto clear_on = [&](cudaStream_t cs) -> int {
     if (po.ms_k) CK(cudaMemsetAsync(gbuf, 0xFF, (size_t)w * h * po.ms_k * sizeof(unsigned long long), cs));
     else if (po.reseed) launch_reseed(gbuf, (size_t)w * h, cs);
@@ -420,32 +385,13 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   }
   mark(EV_GEN);
   if (fork_clear) CK(cudaStreamWaitEvent(st, c->ev_join, 0));
-  else if ((stage_mask & 1u) && !tiled) {
+  else if (stage_mask & 1u) {
     rc = clear_on(st);
     if (rc) return rc;
     ++launches;
   }
   mark(EV_CLEAR);
-  if (tiled) {
-    if (!front) {  // the table (and its pass split) is the last frame's: restart the queues
-      CK(cudaMemsetAsync(c->d_counters + CNT_WORK_BIN, 0, 5 * sizeof(unsigned long long), st));
-      CK(cudaMemsetAsync(c->d_counters + CNT_SEG_HIZ, 0, sizeof(unsigned long long), st));
-    }
-    const bool far_too = two_pass || (!front && c->last_two_pass);  // near bundles first in every tile's list
-    for (int scatter = 0; scatter < 2; ++scatter) {
-      for (int pass = 0; pass < (far_too ? 2 : 1); ++pass) {
-        launch_bin(scatter != 0, c->d_scene, n_bi, c->d_table, c->d_grp, c->d_vertices, k, sp.rho_default, c->d_counters, pass,
-                   c->tb, c->n_sm, st);
-        ++launches;
-      }
-      if (!scatter) {
-        launch_tile_scan(k, c->tb, c->d_counters, st);
-        ++launches;
-      }
-    }
-    launch_raster_tiled(k, gbuf, scene_zn, po.reseed, c->d_counters, c->tb, c->n_sm, &c->ls, st);
-    ++launches;
-  } else if ((stage_mask & 1u) && n_bi) {
+  if ((stage_mask & 1u) && n_bi) {
     if (!front) {  // the table (and its pass split) is the last frame's: restart both queues
       CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER, 0, sizeof(unsigned long long), st));
       CK(cudaMemsetAsync(c->d_counters + CNT_WORK_RASTER1, 0, sizeof(unsigned long long), st));
@@ -480,7 +426,6 @@ int render_impl(hair_ctx* c, const hair_camera* cam, uint32_t w, uint32_t h, con
   c->timed = timed;
   if (timed) ++c->ev_frames;
   c->counted = count;
-  c->last_tiled = tiled;
   if (front) c->last_two_pass = two_pass;
   c->last_w = w;
   c->last_h = h;
@@ -535,8 +480,9 @@ int hair_create(hair_ctx** out, int cuda_device, void* cuda_stream) {
 void hair_destroy(hair_ctx* c) {
   if (!c) return;
   cudaSetDevice(c->device);
-  flush_updates(c);
+  c->jobs.n = c->jobs_apply.n = 0;  // queued cage updates are dropped, not read: their host arrays may be gone already
   cudaStreamSynchronize(c->stream);
+  cudaStreamSynchronize(c->aux_stream);
   for (auto& g : c->grooms) free_groom(g);
   cudaFree(c->d_scene);
   cudaFree(c->d_table);
@@ -548,8 +494,6 @@ void hair_destroy(hair_ctx* c) {
   cudaFree(c->d_target2);
   cudaFree(c->d_zrange);
   cudaFree(c->d_hiz);
-  cudaFree(c->tb.count);
-  cudaFree(c->tb.entries);
   cudaFree(c->d_counters);
   cudaFree(c->d_sink);
   cudaFree(c->d_dom);
@@ -723,10 +667,14 @@ int hair_mesh_update(hair_ctx* c, int groom_id, const hair_cage* cage) {
   const GroomDev& gd = c->scene.g[groom_id];
   if (cage->n_layers != gd.Lv || cage->n_verts != gd.V) return fail(c, HAIR_E_INVALID_ARG, "hair_mesh_update: size mismatch");
   GroomHost& gh = c->grooms[groom_id];
-  // Pinned host memory: the update is queued and ALL queued updates go to the device in one copy kernel issued with the
-  // next frame (the SMs pull them over the bus, unified addressing; flush_updates). Ten small cudaMemcpyAsync per frame (five grooms x
-  // positions, AO), each a bus round trip of its own while the previous frame's 66-133 MB image is on its way to the
-  // host, held the next frame's kernels back by 0.6 ms (2.11 against 1.51 ms per pipelined frame). Pageable: memcpy.
+  // Pinned host memory: the update is only QUEUED here. flush_updates, called by the next hair_render* / hair_stats /
+  // hair_shadow_build, sends every queued array to a per-groom staging buffer with the copy engine on the second
+  // stream (HAIR_STAGE_DMA=1; beside whatever the main stream is still running) and then applies staging -> cage with
+  // one device-to-device kernel on the main stream in front of the frame. So the host arrays are read AFTER that later
+  // call is issued and must stay valid until its frame has completed. Ten small cudaMemcpyAsync per frame on the main
+  // stream (five grooms x positions, AO), each a bus round trip of its own while the previous frame's 66-133 MB image is
+  // on its way to the host, held the next frame's kernels back by 0.6 ms (2.11 against 1.51 ms per pipelined frame).
+  // Pageable memory: the queue is flushed (call order of updates is kept) and the copy is a cudaMemcpyAsync here.
   auto put = [&](float* dst, float** stage, const float* src, size_t bytes) -> int {
     cudaPointerAttributes at;
     if (cudaPointerGetAttributes(&at, src) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer) {
@@ -737,6 +685,7 @@ int hair_mesh_update(hair_ctx* c, int groom_id, const hair_cage* cage) {
       return HAIR_OK;
     }
     cudaGetLastError();  // (an unregistered pointer may leave an error behind on old drivers)
+    flush_updates(c);  // updates queued earlier go first: the newest data of a groom is the one that stays
     CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream));
     return HAIR_OK;
   };
@@ -748,8 +697,9 @@ int hair_mesh_update(hair_ctx* c, int groom_id, const hair_cage* cage) {
 
 int hair_mesh_clear(hair_ctx* c) {
   if (!c) return HAIR_E_INVALID_ARG;
-  flush_updates(c);
+  c->jobs.n = c->jobs_apply.n = 0;  // queued updates of the grooms being removed are dropped, their host arrays not read
   cudaStreamSynchronize(c->stream);
+  cudaStreamSynchronize(c->aux_stream);  // (staging copies of an earlier flush write into buffers free_groom releases)
   for (auto& g : c->grooms) free_groom(g);
   c->grooms.clear();
   memset(&c->scene, 0, sizeof(c->scene));
@@ -993,10 +943,7 @@ int hair_stats(hair_ctx* c, hair_stats_t* out) {
   out->n_vertices = (uint32_t)k[CNT_VERTICES];
   out->n_segments = (uint32_t)k[CNT_SEGMENTS];
   out->gpu_launches = c->launches;
-  out->two_pass = c->last_tiled ? 0u : (uint32_t)k[CNT_HIZ_ON];
-  out->tiled = c->last_tiled ? 1u : 0u;
-  out->n_tile_records = c->last_tiled ? (uint32_t)k[CNT_TILE_ENTRIES] : 0u;
-  out->tile_overflow = c->last_tiled ? (uint32_t)k[CNT_TILE_OVERFLOW] : 0u;
+  out->two_pass = (uint32_t)k[CNT_HIZ_ON];
   out->n_segments_hiz_culled = (uint32_t)k[CNT_SEG_HIZ];
   out->beta_mean = c->scene.n_strands_total ? (float)((double)k[CNT_STRANDS] / (double)c->scene.n_strands_total) : 1.f;
   // Eq. 8: per-groom beta from the device-side sums of the frame's scan, delta = -log(beta)

@@ -27,7 +27,6 @@
 #ifndef HIZ_CUT
 #define HIZ_CUT 0.6f  // bundles whose nearest cage depth lies in the front HIZ_CUT of their instance's range go first
 #endif
-#define HAIR_TILE 64  // HAIR_FLAG_TILED: edge of a screen tile whose two G-buffer layers live in shared memory (64 KB)
 #define HAIR_ROW 44  // floats per control-point row of the per-bundle table (== 12 mod 32: LDS.128 conflict-free)
 
 struct GroomDev {
@@ -114,11 +113,6 @@ enum {
   CNT_HIZ_ON,        // 1: the frame is drawn in two depth-ordered passes with a tile hi-Z between them
   CNT_SEG_HIZ,       // segments dropped by the hi-Z test of the second pass
   CNT_AT_CONS_Y,     // conservative hits of y-major segments (lanes of a warp then sit in different rows)
-  CNT_WORK_BIN,      // HAIR_FLAG_TILED: queue heads of the four binning launches (count near / far, scatter near / far)
-  CNT_WORK_BIN_LAST = CNT_WORK_BIN + 3,
-  CNT_WORK_TILE,     // queue head of the tile raster
-  CNT_TILE_ENTRIES,  // (segment, tile) records of the frame
-  CNT_TILE_OVERFLOW, // 1: they did not fit the record pool (records beyond it were dropped)
   CNT_RESET_END,     // k_scan's last tile zeroes [CNT_SEG_DRAWN, CNT_RESET_END) for the kernels behind it
   // Eq. 8: per groom, strands remaining / strands in total over the DRAWN bundle-instances; zeroed by
   // k_lod, accumulated by k_scan (every tile), read by hair_stats
@@ -263,17 +257,6 @@ struct LaunchState {
   int gen_per_sm = 0;
   size_t gen_smem = 0;
   bool filter_set[8] = {};
-  int tiled_per_sm = 0;
-};
-
-// HAIR_FLAG_TILED (k_raster_tiled.cu): per-tile record lists of the frame
-struct TileBufs {
-  uint32_t* count = nullptr;  // [n_tiles] counter of the count pass, then cursor of the scatter pass (restarts at 0)
-  uint32_t* base = nullptr;   // [n_tiles] first record of the tile in `entries`
-  uint32_t* n = nullptr;      // [n_tiles] records of the tile
-  uint32_t* order = nullptr;  // [n_tiles] tiles, heaviest first
-  float4* entries = nullptr;  // [cap][2] {a.sx, a.sy, b.sx, b.sy} {a.zn, b.zn, sid << 7 | j, rho^2}
-  uint32_t cap = 0;
 };
 
 // ------------------------------------------------------------------ launchers (one per .cu)
@@ -299,12 +282,6 @@ void launch_raster_dom(const SceneDev* d_scene, uint32_t n_bi, const uint4* tabl
                        unsigned long long* counters, uint32_t* dom_cnt, uint3 dom_D, int n_sm, LaunchState* ls,
                        cudaStream_t st);
 void launch_dom_z0(const unsigned long long* gbuf, size_t n_pixels, uint32_t* z0, cudaStream_t st);
-void launch_bin(bool scatter, const SceneDev* d_scene, uint32_t n_bi, const uint4* table, const uint32_t* grp,
-                const float4* vertices, CamDev cam, float rho_default, unsigned long long* counters, int pass,
-                TileBufs tb, int n_sm, cudaStream_t st);
-void launch_tile_scan(CamDev cam, TileBufs tb, unsigned long long* counters, cudaStream_t st);
-void launch_raster_tiled(CamDev cam, unsigned long long* gbuf, const float* scene_zn, bool reseed,
-                         unsigned long long* counters, TileBufs tb, int n_sm, LaunchState* ls, cudaStream_t st);
 void launch_resolve_msaa(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                          ShadeParams sp, const unsigned long long* samples, uint32_t ms_k, const float4* scene_rgb,
                          float4* out, const DomSet* dom, const unsigned long long* counters, cudaStream_t st);

@@ -48,10 +48,7 @@ def gpu_frame(binding, sc, lam=None, flags=0, prm_over=None):
     assert torch.equal(rgb, rgb_c)
     # counted frame: + the pixel counter; a production frame drawn in two passes: + the hi-Z and the second raster
     st_p = h.stats()
-    if st_p["tiled"]:  # HAIR_FLAG_TILED: no clear, binning (count, scan, scatter; twice with a far list) + the tile raster
-        assert st_p["tile_overflow"] == 0 and st_p["n_tile_records"] >= st["n_segments_live"], st_p
-    else:
-        assert st_p["gpu_launches"] == st["gpu_launches"] - 1 + 2 * st_p["two_pass"]
+    assert st_p["gpu_launches"] == st["gpu_launches"] - 1 + 2 * st_p["two_pass"]
     out = dict(h=h, stats_prod=st_p, gb=binding.gbuffer_to_numpy(gb), rgb=rgb.cpu().numpy().astype(np.float64), stats=st,
                table=h.debug_table().cpu().numpy().view(np.uint32), verts=h.debug_vertices().cpu().numpy(), prm=prm,
                gb_t=gb, rgb_t=rgb)
@@ -576,6 +573,62 @@ def test_mesh_update_and_render_to_host(orc, hair_mod):
     assert torch.equal(gb2, gb3) and torch.equal(rgb2, rgb3)
 
 
+def test_mesh_update_lifetime_and_order(hair_mod):
+    """hair_mesh_update from pinned memory is read at the NEXT render (include/hair.h): the binding must keep temporaries
+    alive until then (torch's pinned-memory cache would hand a released block to the next pin_memory()), updates of one
+    groom take effect in call order whatever memory they come from, and clear / destroy drop queued updates unread."""
+    import gc
+    import torch
+    b = hair_mod
+    sc = synth.config(1, scale=0.25, res_scale=0.5)
+    g = sc["grooms"][0]
+    shift = lambda dx: (g["pos"] + np.array([dx, 0, 0], np.float32)).astype(np.float32)
+
+    def fresh(pos):
+        h2 = b.Hair(0)
+        h2.mesh_upload(dict(g, pos=pos))
+        h2.set_render_params(sc["params"])
+        out = h2.render(sc["camera"], 0.0)
+        torch.cuda.synchronize()
+        h2.close()
+        return out
+
+    h = b.Hair(0)
+    h.mesh_upload(g)
+    h.set_render_params(sc["params"])
+    # (1) temporaries, then another pinned tensor of the same size allocated and overwritten before the render
+    h.mesh_update(0, torch.from_numpy(shift(0.01)).pin_memory(), torch.from_numpy(g["ao"]).pin_memory())
+    gc.collect()
+    junk = torch.from_numpy(shift(0.5)).pin_memory()
+    junk.fill_(123.0)
+    junk_ao = torch.from_numpy(g["ao"].copy()).pin_memory()
+    junk_ao.fill_(0.0)
+    gb1, rgb1 = h.render(sc["camera"], 0.0)
+    torch.cuda.synchronize()
+    ref_gb, ref_rgb = fresh(shift(0.01))
+    assert torch.equal(gb1, ref_gb) and torch.equal(rgb1, ref_rgb)
+    h.stats()
+    assert h._pending_updates == []  # let go once the frame has completed
+    # (2) pinned (queued) first, pageable second: the later call wins
+    h.mesh_update(0, torch.from_numpy(shift(0.03)).pin_memory())
+    h.mesh_update(0, shift(0.02))
+    gb2, rgb2 = h.render(sc["camera"], 0.0)
+    torch.cuda.synchronize()
+    ref_gb, ref_rgb = fresh(shift(0.02))
+    assert torch.equal(gb2, ref_gb) and torch.equal(rgb2, ref_rgb)
+    # (3) a queued update is dropped by mesh_clear / destroy, not read
+    h.mesh_update(0, torch.from_numpy(shift(0.04)).pin_memory())
+    h.mesh_clear()
+    h.mesh_upload(g)
+    gb3, rgb3 = h.render(sc["camera"], 0.0)
+    torch.cuda.synchronize()
+    ref_gb, ref_rgb = fresh(g["pos"])
+    assert torch.equal(gb3, ref_gb) and torch.equal(rgb3, ref_rgb)
+    h.mesh_update(0, torch.from_numpy(shift(0.05)).pin_memory())
+    h.close()
+    torch.cuda.synchronize()
+
+
 @pytest.mark.parametrize("filter_on", [True, False])
 def test_render_into_scene_stagewise(orc, hair_mod, filter_on):
     """hair_render_scene (R-scene): a bumpy wall through the groom's depth range and a scene colour, against the
@@ -904,56 +957,6 @@ def test_fused_generate_raster_equals_the_materialised_frame(orc, hair_mod, idx,
         h.render(sc["camera"], sc["lam"])
 
 
-@pytest.mark.parametrize("idx,scale,res_scale,lam", [
-    (1, 1.0, 1.0, None),     # config 1 as named (16 tiles)
-    (2, 0.1, 0.5, None),     # curl + frizz + width_world, ragged tiles (960x540)
-    (3, 0.03, 0.25, None),
-    (4, 0.03, 0.25, None),   # five grooms
-    (5, 0.01, 0.2, None),    # sub-pixel segments
-])
-def test_tiled_raster_stagewise(orc, hair_mod, idx, scale, res_scale, lam):
-    """HAIR_FLAG_TILED (k_raster_tiled.cu): segments binned to 64 x 64 tiles, the tile's two layers resolved in shared
-    memory. Same gates as the default raster: gpu_frame asserts the tiled production frame equals the counted frame of
-    the default raster bit for bit, check_stagewise that the words are the oracle's on the same vertex buffer."""
-    sc = synth.config(idx, scale=scale, res_scale=res_scale)
-    G = gpu_frame(hair_mod, sc, lam=lam, flags=hair_mod.FLAG_TILED)
-    assert G["stats_prod"]["tiled"] == 1 and G["stats_prod"]["tile_overflow"] == 0
-    rep = check_stagewise(orc, sc, G, lam=lam)
-    assert rep["exact_frac"] == 1.0, rep
-
-
-def test_tiled_raster_bench_frame_scene_and_sequential(orc, hair_mod):
-    """The tile raster on the bench frame as named (config 4, 3840x2160: two lists per tile, hi-Z culling at work)
-    against the oracle on windows; then into a scene depth (tile init from scene_zn) and as sequential per-groom passes
-    (tile init from the depth kept, R-seq) against the default raster, frame by frame under a moving camera."""
-    import torch
-    b = hair_mod
-    sc = synth.config(4)
-    W, H = sc["camera"]["width"], sc["camera"]["height"]
-    G = gpu_frame(b, sc, flags=b.FLAG_TILED)
-    sp = G["stats_prod"]
-    assert sp["tiled"] == 1 and sp["tile_overflow"] == 0 and sp["n_segments_hiz_culled"] > 1000000, sp
-    cx = lambda ndc: int((1.0 + ndc) * 0.5 * W)
-    windows = [(cx(-0.75) - 96, H // 2 - 96, cx(-0.75) + 96, H // 2 + 96), (0, H // 2 - 200, 120, H // 2 + 40),
-               (cx(0.15) - 80, H // 2 - 80, cx(0.15) + 80, H // 2 + 80), (cx(0.88) - 40, H // 2 - 40, cx(0.88) + 40, H // 2 + 40)]
-    check_full_size_sampled(orc, sc, G, windows)
-    h = G["h"]
-    zn = torch.full((H, W), 1.0, device="cuda")
-    zn[:, : W // 4] = 0.85
-    srgb = torch.rand((H, W, 4), device="cuda")
-    for i in range(3):
-        cam = synth.moving_camera(sc["camera"], 7 * i)
-        h.set_render_params(G["prm"], flags=0)
-        a = [t.clone() for t in h.render_scene(cam, sc["lam"], zn, srgb)]
-        s = [t.clone() for t in h.render_sequential(cam, sc["lam"], zn, srgb)]
-        h.set_render_params(G["prm"], flags=b.FLAG_TILED)
-        a2 = h.render_scene(cam, sc["lam"], zn, srgb)
-        assert h.stats()["tiled"] == 1
-        assert torch.equal(a[0], a2[0]) and torch.equal(a[1], a2[1]), i
-        s2 = h.render_sequential(cam, sc["lam"], zn, srgb)
-        assert torch.equal(s[0], s2[0]) and torch.equal(s[1], s2[1]), i
-
-
 def test_two_contexts_with_different_table_sizes_in_either_order(hair_mod):
     """Launch state (opt-in dynamic shared memory, occupancy) lives in the context, not in function statics: two
     contexts whose per-bundle tables differ in size (C_max 17 against 49: k_generate's and the fused raster's dynamic
@@ -967,7 +970,7 @@ def test_two_contexts_with_different_table_sizes_in_either_order(hair_mod):
 
     def frames(h, sc, prm):
         out = []
-        for fl in (0, b.FLAG_PAPER_PAYLOAD, b.FLAG_PAPER_PAYLOAD | b.FLAG_FUSED, b.FLAG_TILED):
+        for fl in (0, b.FLAG_PAPER_PAYLOAD, b.FLAG_PAPER_PAYLOAD | b.FLAG_FUSED):
             h.set_render_params(prm, flags=fl)
             g, r = h.render(sc["camera"], sc["lam"])
             out.append((g.clone(), r.clone()))
