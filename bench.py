@@ -35,18 +35,30 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic():
-    """dram__bytes_read.sum + dram__bytes_write.sum per frame and stage from the committed `ncu --set full` capture
-    (profiles/r2_ncu_traffic.csv: stage,dram_bytes,kernels), or {} — never typed in here."""
-    p = os.path.join(ROOT, "profiles", "r2_ncu_traffic.csv")
-    out = {}
-    if os.path.exists(p):
-        for line in open(p).read().splitlines()[1:]:
-            f = line.split(",")
-            if len(f) >= 2 and f[1].strip().isdigit():
-                out[f[0].strip()] = int(f[1])
-        out["source"] = "profiles/r2_ncu_traffic.csv (ncu --set full capture of the bench command; see profiles/r2_ncu_traffic.md, r2_v3_ncu_full.md)"
-    return out
+def ncu_counters():
+    """Per-stage counters of one production frame from the committed `ncu --set full` capture (dram bytes, warp
+    instructions, lts throughput, issue-active; profiles/r3_ncu_stage_counters.csv written by
+    `python -m paper_2607_04230_b200.ncu_summary`) — never typed in here. The file carries the sha256 of csrc/ at capture
+    time; `fresh` says whether the sources bench.py runs on still have it (a kernel edit makes the capture stale)."""
+    from paper_2607_04230_b200 import ncu_summary
+    p = os.path.join(ROOT, "profiles", "r3_ncu_stage_counters.csv")
+    if not os.path.exists(p):
+        return {}, {"source": None, "fresh": None}
+    stages, sha = ncu_summary.read_stage_csv(p)
+    now = ncu_summary.source_hash()
+    return stages, {"source": "profiles/r3_ncu_stage_counters.csv (see r3_ncu_stage_counters.md)", "captured_src_sha256": sha,
+                    "current_src_sha256": now, "fresh": sha == now,
+                    "label": "fresh" if sha == now else "stale: csrc/ changed since the capture"}
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 class ClockSampler:
@@ -105,13 +117,22 @@ def oracle_sample(config: int, scale: float, res_scale: float):
     from paper_2607_04230_b200 import synth
     sc = synth.config(config, scale=scale, res_scale=res_scale)
     f = oracle.Frame(sc["grooms"])
+    stage_s = {}
+
+    def timed(name, fn, *a):
+        t = time.perf_counter()
+        r = fn(*a)
+        stage_s[name] = time.perf_counter() - t
+        return r
+
     t0 = time.perf_counter()
-    f.lod(sc["camera"], sc["lam"])
-    f.generate()
-    cnt = f.raster(sc["camera"], sc["params"])
-    f.shade(sc["camera"], sc["params"])
-    f.filter(sc["camera"], sc["params"])
+    timed("O1_lod_scan", f.lod, sc["camera"], sc["lam"])
+    timed("O2_generate", f.generate)
+    cnt = timed("O4_raster_resolve", f.raster, sc["camera"], sc["params"])
+    timed("O6_shade", f.shade, sc["camera"], sc["params"])
+    timed("O7_filter", f.filter, sc["camera"], sc["params"])
     dt = time.perf_counter() - t0
+    oracle_sample.last_stage_seconds = stage_s
     n_seg = int(f.n_vertices - f.n_strands)
     desc = (f"config {config} with strand counts x{scale} ({synth.n_strands(sc)} strands, {f.n_strands} after LOD, "
             f"{n_seg} segments) at {sc['camera']['width']}x{sc['camera']['height']}, one full frame O1-O7")
@@ -141,7 +162,9 @@ def run_reference(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64/f32",
             "data": "synthetic", "config": {"workload": desc},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
+                             "stage_seconds_last_step": getattr(oracle_sample, "last_stage_seconds", None),
+                             "cpu_model": cpu_model(), "host_cores_available": os.cpu_count()},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -232,16 +255,17 @@ def run_cuda(args):
               for g in sc["grooms"]]
     h2d = sum(p.numel() * 4 + (0 if a is None else a.numel() * 4) for p, a in pinned)
 
-    def e2e_leg(dtype, flags, k_steps):
+    def e2e_leg(dtype, flags, k_steps, with_gbuffer=False):
         h.set_render_params(sc["params"], flags=flags)
         hosts = [torch.empty((H, W, 4), dtype=dtype).pin_memory() for _ in range(2)]
+        hosts_gb = [torch.empty((H, W, 2), dtype=torch.int64).pin_memory() for _ in range(2)] if with_gbuffer else [None, None]
 
         def step(i):
-            # every step: this step's cages host -> device, the frame, this step's out_rgb device -> host. The copies
+            # every step: this step's cages host -> device, the frame, this step's results device -> host. The copies
             # of step i run on the library's copy stream while step i+1 renders (hair_render_to_host_async).
             for gi, (p, a) in enumerate(pinned):
                 h.mesh_update(gi, p, a)
-            h.render_to_host_async(cam, lam, hosts[i % 2])
+            h.render_to_host_async(cam, lam, hosts[i % 2], hosts_gb[i % 2])
 
         for i in range(4):
             step(i)
@@ -260,13 +284,16 @@ def run_cuda(args):
         for _ in range(5):
             for gi, (p, a) in enumerate(pinned):
                 h.mesh_update(gi, p, a)
-            h.render_to_host(cam, lam, hosts[0])
+            h.render_to_host(cam, lam, hosts[0], hosts_gb[0])
         ms_sync = 1e3 * (time.perf_counter() - t0) / 5
-        return ms, ms_sync, hosts[0].numel() * hosts[0].element_size()
+        return ms, ms_sync, hosts[0].numel() * hosts[0].element_size() + (hosts_gb[0].numel() * 8 if with_gbuffer else 0)
 
+    # Headline e2e: out_rgb as float32, the format hair_render declares (133 MB per 4K frame, PCIe-bound) — the number
+    # comparable from round to round. Beside it: the RGBA16F output option (66 MB) and float32 + the G-buffer (265 MB).
     k_e2e = max(4, min(args.steps, 40))
-    ms_e2e32, ms_e2e32_sync, d2h32 = e2e_leg(torch.float32, 0, k_e2e)
-    ms_e2e, ms_e2e_sync, d2h = e2e_leg(torch.float16, binding.FLAG_RGB16F, k_e2e)
+    ms_e2e, ms_e2e_sync, d2h = e2e_leg(torch.float32, 0, k_e2e)
+    ms_e2e16, ms_e2e16_sync, d2h16 = e2e_leg(torch.float16, binding.FLAG_RGB16F, k_e2e)
+    ms_e2e_gb, ms_e2e_gb_sync, d2h_gb = e2e_leg(torch.float32, 0, max(4, k_e2e // 2), with_gbuffer=True)
     ms_e2e = replicas.max_over_ranks(ms_e2e, dist, dev)
     e2e_val = replicas.job_rate(n_seg, world, ms_e2e) / 1e9
     h.set_render_params(sc["params"], flags=0)
@@ -362,36 +389,68 @@ def run_cuda(args):
     ras["Ghits_per_s"] = n_at / (ras["ms"] * 1e-3) / 1e9
     ras["frac_l2_load"] = t_min_ms / ras["ms"]
     ras["frac_l2_atomic_random"] = ras["Ghits_per_s"] / atom["random"]
-    traffic = ncu_traffic()
+    ncu, ncu_meta = ncu_counters()
     dom = max(("generate", "raster", "shade", "filter"), key=lambda k: stages[k]["ms"])
     d = stages[dom]
+    sm_mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0
+    n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    issue_peak = n_sm * 4 * sm_mhz * 1e6 / 1e9  # G warp instructions / s: one per scheduler (4 per SM) per clock
+    for k in ("generate", "raster", "shade", "filter"):
+        if k in ncu and stages[k]["ms"] > 0:
+            stages[k]["warp_inst_ncu"] = ncu[k].get("warp_inst")
+            stages[k]["frac_issue"] = ncu[k]["warp_inst"] / (stages[k]["ms"] * 1e-3) / 1e9 / issue_peak
+            stages[k]["dram_bytes_ncu"] = ncu[k].get("dram_bytes")
+            stages[k]["ncu_lts_throughput_pct"] = ncu[k].get("lts_throughput_pct")
+            stages[k]["ncu_issue_active_pct"] = ncu[k].get("issue_active_pct")
     if dom == "raster":
-        roofline = {"kernel": "k_raster", "bound": "l2_load", "achieved": ras["Gpair_loads_per_s"],
-                    "peak": n_cons / (t_min_ms * 1e-3) / 1e9, "unit": "Gpair-loads/s", "frac": ras["frac_l2_load"],
-                    "traffic": traffic.get("raster"),
-                    "algorithmic": f"{n_cons} conservative-predicate-true pixels (counts.n_atomics_cons), one 16-byte "
-                                   f"ld.global.cg of the word pair each; {n_cons_y} of them on y-major segments",
-                    "peak_source": "measured in this run (hair_l2_load_microbench over this frame's G-buffer): "
-                                   f"row {l2['row']:.1f}, column {l2['column']:.1f}, column with the two minor-axis neighbours "
-                                   f"requested together {l2['column_pairs']:.1f}, random {l2['random']:.1f} G pair loads/s; "
-                                   "peak = loads / (x-major loads / row rate + y-major loads / the better column rate)",
+        t_min_plain_ms = ((n_cons - n_cons_y) / l2["row"] + n_cons_y / l2["column"]) / 1e9 * 1e3
+        views = {
+            "survey_8d_l2_atomic": {
+                "frac": ras["frac_l2_atomic_random"], "binds": False, "hits_per_s_G": ras["Ghits_per_s"],
+                "peak_random_RED_G_per_s": atom["random"], "frac_of_coalesced_RED": ras["Ghits_per_s"] / atom["unique"],
+                "note": "SURVEY 8(d) as written: predicate-true hits (n_atomics_cons + n_atomics_center) / time over the "
+                        "measured random RED.MIN.64 rate. Far above 1: read-before-atomic sends only n_atomics_issued of "
+                        "the hits to L2 as atomics, so this ceiling does not bind this design"},
+            "issued_atomics": {"frac": cnt["n_atomics_issued"] / (ras["ms"] * 1e-3) / 1e9 / atom["random"],
+                               "issued_Gatom_per_s": cnt["n_atomics_issued"] / (ras["ms"] * 1e-3) / 1e9, "binds": False},
+            "l2_pair_load_model": {
+                "frac_column_pairs": ras["frac_l2_load"], "frac_plain_column": t_min_plain_ms / ras["ms"], "binds": False,
+                "note": "builder-defined: one 16-byte ld.global.cg per conservative-predicate-true pixel, x-major at the "
+                        "measured row rate, y-major at the column rate; the two y-major denominators (plain column walk / "
+                        "the two minor-axis neighbours requested together) bracket it. ncu's lts__throughput of the two "
+                        "passes (below) says L2 is near half of its ceiling: not the binding resource either",
+                "rates_G_pair_loads_per_s": l2},
+            "ncu_capture": {"lts_throughput_pct": ncu.get("raster", {}).get("lts_throughput_pct"),
+                            "issue_active_pct": ncu.get("raster", {}).get("issue_active_pct"),
+                            "order": "near pass / k_hiz / far pass"},
+        }
+        wi = ncu.get("raster", {}).get("warp_inst")
+        roofline = {"kernel": "k_raster", "bound": "alu",
+                    "bound_detail": "warp-instruction issue slots, latency-limited: the pixel loop's integer / fp32 / LSU "
+                                    "instructions, not bytes and not atomics (DESIGN.md 7.5)",
+                    "achieved": None if wi is None else wi / (ras["ms"] * 1e-3) / 1e9, "peak": issue_peak,
+                    "unit": "Gwarp-inst/s", "frac": ras.get("frac_issue"),
+                    "peak_source": f"{n_sm} SMs x 4 schedulers x 1 warp instruction per clock x {sm_mhz:.0f} MHz (the SM clock "
+                                   "sampled during the timed region; unit counts from B300_MICROARCH.md / B200_PROFILING.md)",
+                    "algorithmic": f"{wi} warp instructions per frame (smsp__inst_executed.sum of near pass + k_hiz + far pass, "
+                                   f"from the committed ncu capture: {ncu_meta.get('label')}) / stages.raster.ms measured in this "
+                                   f"run; the frame draws {n_cons} conservative + {n_cen} centre predicate-true hits",
+                    "traffic": ncu.get("raster", {}).get("dram_bytes"),
                     "covers": "the raster stage: k_raster (near pass) + k_hiz + k_raster (far pass); time = stages.raster.ms",
-                    "atomic_view": {"hits_per_s_G": ras["Ghits_per_s"], "frac_of_random_RED": ras["frac_l2_atomic_random"],
-                                    "issued_Gatom_per_s": cnt["n_atomics_issued"] / (ras["ms"] * 1e-3) / 1e9,
-                                    "note": "predicate-true hits / time over the measured random RED.MIN.64 rate; > 1 because "
-                                            "read-before-atomic sends only n_atomics_issued of the hits to L2 as atomics: "
-                                            "that ceiling does not bind, the load ceiling above does"}}
+                    "views": views}
     else:
         roofline = {"kernel": "k_" + dom, "bound": "hbm", "achieved": d["GBps"], "peak": hbm_peak, "unit": "GB/s",
-                    "frac": d["frac_hbm"], "traffic": traffic.get(dom), "peak_source": hbm_src,
+                    "frac": d["frac_hbm"], "traffic": ncu.get(dom, {}).get("dram_bytes"), "peak_source": hbm_src,
                     "algorithmic": f"{d['bytes']} bytes per frame"}
-    roofline["traffic_source"] = traffic.get("source")
+    roofline["traffic_source"] = ncu_meta
     # the three fractions north_star asks for, as it states them
     north_star = {
         "raster_vs_l2": {"frac_l2_load": ras["frac_l2_load"], "frac_l2_atomic_random": ras["frac_l2_atomic_random"]},
         "generate_vs_hbm": {"GBps": stages["generate"].get("GBps"), "frac": stages["generate"].get("frac_hbm")},
         "shade_vs_hbm": {"GBps": sh.get("GBps"), "frac": sh.get("frac_hbm"),
-                         "frac_unique_vertices": sh["frac_hbm_unique_vertices"]},
+                         "frac_unique_vertices": sh["frac_hbm_unique_vertices"],
+                         "note": "frac is on SURVEY 8(d)'s UPPER-BOUND bytes (64 B of gathers per centre hit); on the bytes "
+                                 "actually touched (unique vertices) it is frac_unique_vertices: quote both"},
     }
 
     # ---- the oracle timed beside it on this box's host cores (bounded sample of the same workload)
@@ -401,7 +460,8 @@ def run_cuda(args):
         oracle.build()
         dt, seg, desc, _ = oracle_sample(args.config, args.cpu_scale, 1.0 if args.res_scale == 1.0 else args.res_scale)
         cpu_baseline = {"value": seg / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
-                        "seconds": dt, "host_cores_available": os.cpu_count()}
+                        "seconds": dt, "stage_seconds": oracle_sample.last_stage_seconds, "cpu_model": cpu_model(),
+                        "host_cores_available": os.cpu_count()}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -417,11 +477,18 @@ def run_cuda(args):
         "segments_per_s": world * n_seg / (ms_step * 1e-3),
         "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": ms_e2e, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step_unpipelined": ms_e2e_sync,
-                "what": "per step: hair_mesh_update of every cage (pinned host) + hair_render_to_host_async with "
-                        "HAIR_FLAG_RGB16F (out_rgb as RGBA16F to pinned host, 2 frames in flight), hair_host_wait after the "
-                        "last; wall clock over the steps; out_gbuffer stays on the device",
-                "fp32_host_output": {"ms_per_step": ms_e2e32, "ms_per_step_unpipelined": ms_e2e32_sync,
-                                     "d2h_bytes_per_step": d2h32}},
+                "out_rgb_format": "float32 [h][w][4]", "out_gbuffer_copied": False,
+                "what": "per step: hair_mesh_update of every cage (pinned host) + hair_render_to_host_async (out_rgb as "
+                        "float32 to pinned host, 2 frames in flight), hair_host_wait after the last; wall clock over the "
+                        "steps. out_gbuffer, hair_render's other result, STAYS ON THE DEVICE in this figure (host_gbuffer = "
+                        "NULL); with it copied too see float32_and_gbuffer_host_output. PCIe-bound: the device frame is "
+                        "ms_per_step of the top level",
+                "rgb16f_host_output": {"ms_per_step": ms_e2e16, "ms_per_step_unpipelined": ms_e2e16_sync,
+                                       "d2h_bytes_per_step": d2h16, "Gsegments_per_s": n_seg * world / (ms_e2e16 * 1e-3) / 1e9,
+                                       "what": "HAIR_FLAG_RGB16F: the filter writes RGBA16F (|error| < 2e-3 for |v| < 4); "
+                                               "rounds 1-2 reported this leg as e2e.value"},
+                "float32_and_gbuffer_host_output": {"ms_per_step": ms_e2e_gb, "ms_per_step_unpipelined": ms_e2e_gb_sync,
+                                                    "d2h_bytes_per_step": d2h_gb}},
         "gpu_launches": st["gpu_launches"] * args.steps,
         "roofline": roofline, "north_star_fractions": north_star, "stages": stages, "l2_atomic_peaks_Gatom_per_s": atom,
         "l2_pair_load_peaks_Gloads_per_s": l2,
