@@ -130,7 +130,8 @@ int hair_mesh_upload(hair_ctx*, const hair_cage*, const hair_roots*, const hair_
  * From pageable memory the copy is a cudaMemcpyAsync on the context's stream inside this call (updates queued before
  * it are sent first, so the updates of a groom take effect in call order); the array may be freed when it returns. */
 int hair_mesh_update(hair_ctx*, int groom_id, const hair_cage*);
-/* Removes all grooms (buffers are kept). */
+/* Removes all grooms (buffers are kept), so that another hair mesh can be uploaded into the same context;
+ * the counterpart of hair_mesh_upload in north_star's boundary. */
 int hair_mesh_clear(hair_ctx*);
 
 typedef struct {
@@ -217,7 +218,8 @@ int hair_render_to_host(hair_ctx*, const hair_camera*, uint32_t width, uint32_t 
 int hair_render_to_host_async(hair_ctx*, const hair_camera*, uint32_t width, uint32_t height,
                               const float* lod_lambda, uint32_t n_lambda, uint64_t* host_gbuffer, float* host_rgb,
                               int* out_slot);
-/* Blocks until the copies of `slot` (0..HAIR_HOST_SLOTS-1), or of every slot (slot < 0), have finished. */
+/* Blocks until the copies of `slot` (0..HAIR_HOST_SLOTS-1), or of every slot (slot < 0), have finished. (Host-side
+ * completion of hair_render_to_host_async; not an operation of the paper — the e2e measurement of SURVEY.md §8d needs it.) */
 int hair_host_wait(hair_ctx*, int slot);
 
 /* Deep opacity maps (Yuksel and Keyser 2008, named by PAPER.md:192; the paper gives no more, DESIGN.md R-dom states
@@ -278,10 +280,15 @@ typedef struct {
   uint32_t two_pass;              /* 1: the last frame was drawn in two depth-ordered raster passes */
   uint32_t n_segments_hiz_culled; /* segments of the second pass dropped by the tile hi-Z test before any pixel work */
 } hair_stats_t;
-/* Synchronises the stream and reads the device counters of the last frame. */
+/* hair_stats() of north_star's boundary: synchronises the stream and reads the device counters of the
+ * last frame — the LOD pass's strand / vertex totals, the per-groom beta and delta of the
+ * depth-comparison fix (Eq. 8), the raster's hit counts and the stage times.
+ * hair_stats_t holds every field SURVEY §8(b) lists, in another order and with more. ms_clear reads ~0: the clear runs
+ * on the context's second stream beside LOD / scan / generate and is not bracketed by events. */
 int hair_stats(hair_ctx*, hair_stats_t* out);
 
-/* Debug / parity access to the intermediates of the last frame (DEVICE pointers, owned by the context):
+/* Debug / parity access to the intermediates of the last frame (DEVICE pointers, owned by the context). Replaces
+ * SURVEY.md §8(b)'s hair_debug_vertices(ctx, &verts, &table): same two buffers plus the shaded colour buffer:
  * vertices float4[n_vertices] = (x, y, z, ao); table uint4[n_bundles] = {N_LOD, C, slot_base,
  * vertex_base}; colour float4[h][w] = shaded rgb of centre-hit pixels (undefined elsewhere). */
 int hair_debug_buffers(hair_ctx*, const float** dev_vertices, const uint32_t** dev_table, const float** dev_colour);
@@ -294,7 +301,9 @@ int hair_render_stages(hair_ctx*, const hair_camera*, uint32_t width, uint32_t h
  * the raster with vertices of its choice. n must equal the last frame's n_vertices. */
 int hair_debug_set_vertices(hair_ctx*, const float* dev_src, uint32_t n);
 
-/* L2-atomic roofline denominators: 64-bit atomicMin (RED.MIN.64) micro-kernels over a
+/* MEASUREMENT TOOLING, not part of the render path (bench.py measures its roofline denominators with the two calls
+ * below in the same run as the frame).
+ * L2-atomic roofline denominators: 64-bit atomicMin (RED.MIN.64) micro-kernels over a
  * DEVICE buffer of n_words uint64.
  *  mode 0: each thread its own word, coalesced;  mode 1: hashed uniformly random word per op;
  *  mode 2: all ops into `hot_words` words (contention floor).
