@@ -247,6 +247,46 @@ def run_cuda(args):
     ms_moving = e0.elapsed_time(e1) / k_mov
     st_mov = h.stats()
 
+    # ---- two frames in flight: a second context on a second stream renders every other frame, so
+    # frame i's shade + filter (FMA / XU-bound, L2 idle) can share the SMs with frame i+1's LOD / generate / raster
+    # (L2-latency-bound, FMA pipe idle). Each context owns its scratch, so nothing is shared but the SMs; the frames are
+    # the serial frame bit for bit (checked). Throughput only: a single frame's latency is ms_per_step or worse.
+    h.set_render_params(sc["params"], flags=0)
+    s1 = torch.cuda.current_stream()
+    s2 = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(s2):
+        h_b = binding.Hair(local_rank, stream=s2)
+        for g in sc["grooms"]:
+            h_b.mesh_upload(g)
+        gb_b, rgb_b = h_b.alloc_outputs(W, H)
+        h_b.set_render_params(sc["params"], flags=0)
+    for _ in range(3):
+        h.render(cam, lam, gb, rgb)
+        h_b.render(cam, lam, gb_b, rgb_b)
+    barrier()
+    k_pipe = max(8, min(args.steps, 100)) // 2 * 2
+    e_b = torch.cuda.Event()
+    e0.record(s1)
+    s2.wait_event(e0)
+    for i in range(k_pipe // 2):
+        h.render(cam, lam, gb, rgb)
+        h_b.render(cam, lam, gb_b, rgb_b)
+    e_b.record(s2)
+    s1.wait_event(e_b)
+    e1.record(s1)
+    barrier()
+    ms_pipelined = e0.elapsed_time(e1) / k_pipe
+    pipelined_same = bool(torch.equal(gb, gb_b) and torch.equal(rgb, rgb_b))
+    # the serial frame with the same flags (no stage events), for the comparison
+    e0.record(s1)
+    for _ in range(k_pipe):
+        h.render(cam, lam, gb, rgb)
+    e1.record(s1)
+    barrier()
+    ms_serial_noevents = e0.elapsed_time(e1) / k_pipe
+    h_b.close()
+    del gb_b, rgb_b
+
     # ---- end to end through the C ABI with HOST buffers: cage upload (pinned) + render + D2H of out_rgb, per step.
     # Headline: RGBA16F host output (HAIR_FLAG_RGB16F, written by the filter itself: 66 MB per 4K frame); the fp32 host
     # output (133 MB, PCIe-bound) is timed beside it.
@@ -507,6 +547,11 @@ def run_cuda(args):
         "moving_camera": {"ms_per_step": ms_moving, "frames": k_mov, "ms_raster": st_mov["ms_raster"],
                           "ms_filter": st_mov["ms_filter"], "n_segments_hiz_culled_last_frame": st_mov["n_segments_hiz_culled"],
                           "what": "synth.moving_camera: yaw +-0.04 rad, sideways swing and dolly, a new camera every frame"},
+        "pipelined": {"ms_per_frame": ms_pipelined, "frames": k_pipe, "ms_per_frame_serial_same_flags": ms_serial_noevents,
+                      "bit_identical_to_serial": pipelined_same,
+                      "what": "two contexts on two streams render alternate frames (two frames in flight, each context "
+                              "with its own scratch): throughput over back-to-back frames; single-frame latency is not "
+                              "better than ms_per_step"},
         "sequential_per_groom": {"ms_per_step": ms_seq, "what": "hair_render_sequential: one LOD..filter pass per groom, "
                                  "depth kept, blended over the target (PAPER.md:208-210); the headline frame resolves "
                                  "all grooms in one G-buffer instead (DESIGN.md R15)"},
