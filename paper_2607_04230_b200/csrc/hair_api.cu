@@ -51,8 +51,9 @@ struct hair_ctx {
   uint32_t* d_want = nullptr;  // its device alias (written by k_scan)
   uint32_t* d_hiz = nullptr;  // [ceil(h / 16)][ceil(w / 16)] farthest centre depth per tile between the passes
   size_t hiz_cap = 0;
-  // hair_mesh_update from pinned memory: host -> staging copies (one kernel on aux_stream, beside the frame before)
-  // and staging -> cage copies (one kernel on the stream, in front of the next frame)
+  // hair_mesh_update from pinned memory: host -> staging copies (cudaMemcpyAsync on aux_stream, i.e. the copy engine,
+  // beside the frame before; one SM copy kernel instead with HAIR_STAGE_DMA=0) and staging -> cage copies (one kernel
+  // on the stream, in front of the next frame)
   CopyJobs jobs, jobs_apply;
   cudaEvent_t ev_staged = nullptr, ev_applied = nullptr;
   bool applied_once = false;

@@ -291,7 +291,8 @@ void launch_shade(const SceneDev* d_scene, const uint2* srec, const float4* vert
 int launch_filter(const SceneDev* d_scene, const uint2* srec, const float4* vertices, CamDev cam,
                    ShadeParams sp, const unsigned long long* gbuf, const float4* colour, const float4* scene_rgb,
                    float4* out, unsigned long long* counters, bool count, LaunchState* ls, cudaStream_t st);
-// hair_mesh_update: copies of 32-bit words from device-visible (pinned host) memory, all done by one kernel
+// hair_mesh_update: a list of copies of 32-bit words done by ONE kernel launch — the staging -> cage apply in front of
+// a frame (device to device), and with HAIR_STAGE_DMA=0 also the pinned host -> staging pull over the bus
 #define COPY_JOBS_MAX 32
 struct CopyJob {
   uint32_t* dst;

@@ -301,8 +301,8 @@ void launch_lod_scan(const SceneDev* d_scene, uint32_t n_bi, CamDev cam, LambdaA
   k_scan<<<n_tiles, 256, 0, st>>>(d_scene, table, grp, n_bi, part, counters, zr_prev, n_inst, two_pass ? 1u : 0u, want_two_pass);
 }
 
-// hair_mesh_update from pinned host memory: the SMs pull every queued cage over the bus in one launch (hair_api.cu);
-// blockIdx.y = job
+// hair_mesh_update: every queued copy job in one launch (hair_api.cu flush_updates) — by default the device-to-device
+// apply of the staged cages; with HAIR_STAGE_DMA=0 also the pull of the pinned host arrays over the bus. blockIdx.y = job
 __global__ void __launch_bounds__(256) k_copy_jobs(CopyJobs jobs) {
   const CopyJob j = jobs.j[blockIdx.y];
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < j.n; i += (size_t)gridDim.x * blockDim.x) j.dst[i] = j.src[i];

@@ -30,11 +30,17 @@ UNIT_SCALE = {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "ns": 1, "us"
 
 
 def source_hash() -> str:
+    """sha256[:16] of csrc/*.cu, *.cuh with comments and white space removed (a comment edit does not make a capture
+    stale; any token change does)."""
+    import re
     h = hashlib.sha256()
     for f in sorted(os.listdir(CSRC)):
         if f.endswith((".cu", ".cuh")):
+            txt = open(os.path.join(CSRC, f), encoding="utf-8").read()
+            txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+            txt = re.sub(r"//[^\n]*", "", txt)
             h.update(f.encode())
-            h.update(open(os.path.join(CSRC, f), "rb").read())
+            h.update("".join(txt.split()).encode())
     return h.hexdigest()[:16]
 
 
