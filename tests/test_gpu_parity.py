@@ -992,6 +992,47 @@ def test_two_contexts_with_different_table_sizes_in_either_order(hair_mod):
                 assert torch.equal(g0, g1) and torch.equal(r0, r1), (order, rep)
 
 
+def test_two_contexts_on_two_streams_concurrently(hair_mod):
+    """Two frames in flight (bench.py's `pipelined` leg): two contexts bound to two different streams render the same
+    scene at the same time, many frames back to back with no synchronisation in between. A context owns all of its
+    scratch and the library has no global state on the render path, so every frame of either context must equal the
+    serial frame bit for bit."""
+    import torch
+    b = hair_mod
+    sc = synth.config(4, scale=0.2, res_scale=0.5)
+    cam, lam = sc["camera"], sc["lam"]
+    W, H = cam["width"], cam["height"]
+    h0 = b.Hair(0)
+    for g in sc["grooms"]:
+        h0.mesh_upload(g)
+    h0.set_render_params(sc["params"])
+    ref_gb, ref_rgb = h0.render(cam, lam)
+    ref_gb, ref_rgb = ref_gb.clone(), ref_rgb.clone()   # a second render may switch to two passes: same frame
+    ref2 = h0.render(cam, lam)
+    torch.cuda.synchronize()
+    assert torch.equal(ref2[0], ref_gb) and torch.equal(ref2[1], ref_rgb)
+    ctxs = []
+    for _ in range(2):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            h = b.Hair(0, stream=st)
+            for g in sc["grooms"]:
+                h.mesh_upload(g)
+            h.set_render_params(sc["params"])
+            outs = [h.alloc_outputs(W, H) for _ in range(3)]
+        ctxs.append((h, st, outs))
+    torch.cuda.synchronize()
+    for i in range(9):            # interleaved launches, nothing waits: the two streams run side by side
+        for h, st, outs in ctxs:
+            h.render(cam, lam, *outs[i % 3])
+    torch.cuda.synchronize()
+    for h, st, outs in ctxs:
+        for gb, rgb in outs:
+            assert torch.equal(gb, ref_gb) and torch.equal(rgb, ref_rgb)
+        h.close()
+    h0.close()
+
+
 def test_sequential_as_first_render_of_a_context(hair_mod):
     """Regression: the first frame of a context may be a sequential one (its second target must survive the
     allocation of the per-resolution scratch)."""
